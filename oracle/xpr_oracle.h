@@ -1,0 +1,113 @@
+/*
+ * xpr_oracle.h -- C interface of the CPU ORACLE for the tile-based splatting hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call anything under oracle/.
+ * It shares no code with the CUDA path (paper_2606_11529_b200/csrc, include/xpr.h): the structs
+ * below are the oracle's own, every field a double, and all pointers are HOST pointers.
+ *
+ * What it computes: the plain definition of tile-based 3DGS rendering and its exact reverse-mode
+ * derivative, written from /root/reference/PAPER.md (XPR, arxiv 2606.11529) and the readings
+ * C1..C26 / rules R1..R3 in DESIGN.md.  Each function cites the passage it follows
+ * ("PAPER L<line>").  Scalar type: *_f32 = parity mode (every operation individually rounded in
+ * fp32, in the order DESIGN.md section 3 fixes; compiled with -ffp-contract=off), *_f64 =
+ * self-check mode (closed forms, finite differences).  Gradients are accumulated and returned
+ * in fp64 in both modes.
+ *
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1 closed form single Gaussian, P2
+ * transmittance/opacity invariants, P3 brute-force binning, P4 tiling invariance, P5 sort
+ * invariants, P6 central finite differences (fp64), P7 UT exact for affine maps, P8 UT~EWA limit,
+ * P9 fisheye special cases, P10 SH orthonormality/degree-0, P11 linearity, P12 fp32-vs-fp64.
+ * No function here is "parity unpinned".
+ */
+#ifndef XPR_ORACLE_H
+#define XPR_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+    int32_t model;              /* 0 pinhole, 1 fisheye-equidistant, 2 affine/orthographic (pin P7 only) */
+    int32_t width, height;
+    double fx, fy, cx, cy;
+    double k[4];
+    double w2c[12];             /* row-major [W|t] */
+} xo_camera;
+
+typedef struct {
+    int32_t projection;         /* 0 EWA, 1 UT */
+    int32_t sh_degree;          /* 0..3 */
+    int32_t tile;               /* tile edge in pixels (16; 8 allowed for pin P4) */
+    int32_t antialias;          /* Mip-Splatting opacity factor */
+    double alpha_thresh, alpha_max, t_min, z_near, lowpass;
+    double ut_alpha, ut_beta, ut_kappa;
+    double bg[3];
+    double fragile_rel;         /* relative margin of the fragile-pixel protocol */
+} xo_config;
+
+/* flags byte written by project */
+enum { XO_VISIBLE = 1, XO_CLAMP_U = 2, XO_CLAMP_V = 4, XO_RGB_POS_R = 8, XO_RGB_POS_G = 16, XO_RGB_POS_B = 32 };
+/* fragile bits written by rasterize_fwd */
+enum { XO_FRAG_EXIT = 1, XO_FRAG_CLAMP = 2, XO_FRAG_GATE = 4 };
+
+#define XO_DECL(S, T)                                                                                   \
+    /* Preprocess (Listing 1; UT: L437, Listing 3). */         \
+    void xpr_oracle_project_##S(int64_t N, const T* means, const T* scales, const T* quats,             \
+                                const T* opacities, const T* sh, const xo_camera* cam,                  \
+                                const xo_config* cfg, T* mean2d, T* conic, T* opac_eff, T* rgb,         \
+                                T* depth, T* lnv, int32_t* tile_rect, uint32_t* tile_count,             \
+                                uint8_t* flags);                                                        \
+    /* Shader, Algorithm 1 (Listing 1), tile lists from bin_sort. */      \
+    void xpr_oracle_rasterize_fwd_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,            \
+                                      const T* mean2d, const T* conic, const T* opac_eff, const T* rgb, \
+                                      const T* lnv, const uint32_t* vals_sorted,                        \
+                                      const uint32_t* tile_ranges, T* image, T* final_T,                \
+                                      uint32_t* n_contrib, uint8_t* fragile, int64_t* counters);        \
+    /* Strict per-pixel mode: each pixel's own list sorted by (depth, index); no binning used. */       \
+    void xpr_oracle_rasterize_fwd_strict_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,     \
+                                             const T* mean2d, const T* conic, const T* opac_eff,        \
+                                             const T* rgb, const T* lnv, const T* depth,                \
+                                             const int32_t* tile_rect, const uint32_t* tile_count,      \
+                                             T* image, T* final_T, uint32_t* n_contrib);                \
+    /* Reverse mode through compositing (hand-derived; the paper relies on AD, L106). */                \
+    void xpr_oracle_rasterize_bwd_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,            \
+                                      const T* mean2d, const T* conic, const T* opac_eff, const T* rgb, \
+                                      const T* lnv, const uint32_t* vals_sorted,                        \
+                                      const uint32_t* tile_ranges, const uint32_t* n_contrib,           \
+                                      const T* dL_dimage, double* g_mean2d, double* g_conic,            \
+                                      double* g_opac_eff, double* g_rgb);                               \
+    /* Reverse mode through projection + SH (hand-derived). */                                          \
+    void xpr_oracle_project_bwd_##S(int64_t N, const T* means, const T* scales, const T* quats,         \
+                                    const T* opacities, const T* sh, const xo_camera* cam,              \
+                                    const xo_config* cfg, const double* g_mean2d, const double* g_conic,\
+                                    const double* g_opac_eff, const double* g_rgb, double* g_means,     \
+                                    double* g_scales, double* g_quats, double* g_opacities,             \
+                                    double* g_sh);                                                      \
+    /* Real SH basis, degree <= 3 (reading C5); out[16]. */                                             \
+    void xpr_oracle_sh_basis_##S(const T* dir, T* out16);                                               \
+    /* Camera model pi: camera-space point -> pixel (readings C1, C2, C18). */                          \
+    void xpr_oracle_camera_project_##S(const xo_camera* cam, const T* p_cam, T* pix2);
+
+XO_DECL(f32, float)
+XO_DECL(f64, double)
+
+/* Rasterizer: replicate, assign tile id, stable sort by (tile, depth), bounds.
+ * depth is fp32 (its bit pattern is the low key word, BASELINE.json:north_star).  Returns the
+ * number of pairs I; writes at most `capacity` entries (pass capacity=0 to count only). */
+int64_t xpr_oracle_bin_sort(int64_t N, const float* depth, const int32_t* tile_rect,
+                            const uint32_t* tile_count, int32_t tiles_x, int32_t tiles_y,
+                            int64_t capacity, uint64_t* keys_sorted, uint32_t* vals_sorted,
+                            uint32_t* tile_ranges);
+
+/* Unsorted emission only (pin P3 / parity of the emit step). */
+int64_t xpr_oracle_emit(int64_t N, const float* depth, const int32_t* tile_rect,
+                        const uint32_t* tile_count, int32_t tiles_x, int64_t capacity,
+                        uint64_t* keys, uint32_t* vals);
+
+int32_t xpr_oracle_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,217 @@
+"""ctypes binding of the CPU oracle (TEST INFRASTRUCTURE, not the product; see xpr_oracle.h).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It imports nothing from paper_2606_11529_b200 except (optionally, by the
+caller) the seeded scene containers, which carry no arithmetic of the method.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+if _HERE not in sys.path:
+    sys.path.insert(0, _HERE)
+import build as _build  # noqa: E402  (oracle/build.py)
+
+
+class XoCamera(C.Structure):
+    _fields_ = [("model", C.c_int32), ("width", C.c_int32), ("height", C.c_int32),
+                ("fx", C.c_double), ("fy", C.c_double), ("cx", C.c_double), ("cy", C.c_double),
+                ("k", C.c_double * 4), ("w2c", C.c_double * 12)]
+
+
+class XoConfig(C.Structure):
+    _fields_ = [("projection", C.c_int32), ("sh_degree", C.c_int32), ("tile", C.c_int32), ("antialias", C.c_int32),
+                ("alpha_thresh", C.c_double), ("alpha_max", C.c_double), ("t_min", C.c_double),
+                ("z_near", C.c_double), ("lowpass", C.c_double),
+                ("ut_alpha", C.c_double), ("ut_beta", C.c_double), ("ut_kappa", C.c_double),
+                ("bg", C.c_double * 3), ("fragile_rel", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.xpr_oracle_bin_sort.restype = C.c_int64
+        _lib.xpr_oracle_emit.restype = C.c_int64
+        _lib.xpr_oracle_num_threads.restype = C.c_int32
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().xpr_oracle_num_threads())
+
+
+def make_camera(cam) -> XoCamera:
+    """cam: any object with model,width,height,fx,fy,cx,cy,k,w2c (e.g. scenes.Camera)."""
+    c = XoCamera()
+    c.model, c.width, c.height = int(cam.model), int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    for i in range(4):
+        c.k[i] = float(cam.k[i])
+    w = np.asarray(cam.w2c, np.float64).reshape(12)
+    for i in range(12):
+        c.w2c[i] = float(w[i])
+    return c
+
+
+def make_config(d: dict, fragile_rel: float = 2e-5) -> XoConfig:
+    c = XoConfig()
+    c.projection, c.sh_degree, c.tile, c.antialias = int(d["projection"]), int(d["sh_degree"]), int(d["tile"]), int(d["antialias"])
+    c.alpha_thresh, c.alpha_max, c.t_min = float(d["alpha_thresh"]), float(d["alpha_max"]), float(d["t_min"])
+    c.z_near, c.lowpass = float(d["z_near"]), float(d["lowpass"])
+    c.ut_alpha, c.ut_beta, c.ut_kappa = float(d["ut_alpha"]), float(d["ut_beta"]), float(d["ut_kappa"])
+    for i in range(3):
+        c.bg[i] = float(d["bg"][i])
+    c.fragile_rel = float(fragile_rel)
+    return c
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _sfx(dtype):
+    return {np.dtype(np.float32): "f32", np.dtype(np.float64): "f64"}[np.dtype(dtype)]
+
+
+def tiles(cam, cfg):
+    ts = int(cfg.tile)
+    return (int(cam.width) + ts - 1) // ts, (int(cam.height) + ts - 1) // ts
+
+
+def project(means, scales, quats, opacities, sh, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    N = int(means.shape[0])
+    a = [np.ascontiguousarray(x, dt) for x in (means, scales, quats, opacities, sh)]
+    out = dict(mean2d=np.empty((N, 2), dt), conic=np.empty((N, 3), dt), opac_eff=np.empty(N, dt),
+               rgb=np.empty((N, 3), dt), depth=np.empty(N, dt), lnv=np.empty(N, dt),
+               tile_rect=np.empty((N, 4), np.int32), tile_count=np.empty(N, np.uint32), flags=np.empty(N, np.uint8))
+    fn = getattr(lib(), "xpr_oracle_project_" + _sfx(dt))
+    fn(C.c_int64(N), *[_p(x) for x in a], C.byref(cam), C.byref(cfg),
+       *[_p(out[k]) for k in ("mean2d", "conic", "opac_eff", "rgb", "depth", "lnv", "tile_rect", "tile_count", "flags")])
+    return out
+
+
+def emit(proj: dict, cam: XoCamera, cfg: XoConfig):
+    tx, _ = tiles(cam, cfg)
+    N = int(proj["tile_count"].shape[0])
+    depth = np.ascontiguousarray(proj["depth"], np.float32)
+    I = int(proj["tile_count"].astype(np.int64).sum())
+    keys = np.empty(I, np.uint64)
+    vals = np.empty(I, np.uint32)
+    n = lib().xpr_oracle_emit(C.c_int64(N), _p(depth), _p(proj["tile_rect"]), _p(proj["tile_count"]), C.c_int32(tx),
+                              C.c_int64(I), _p(keys), _p(vals))
+    assert n == I
+    return keys, vals
+
+
+def bin_sort(proj: dict, cam: XoCamera, cfg: XoConfig) -> dict:
+    tx, ty = tiles(cam, cfg)
+    N = int(proj["tile_count"].shape[0])
+    depth = np.ascontiguousarray(proj["depth"], np.float32)
+    I = int(proj["tile_count"].astype(np.int64).sum())
+    keys = np.empty(I, np.uint64)
+    vals = np.empty(I, np.uint32)
+    ranges = np.zeros((tx * ty, 2), np.uint32)
+    n = lib().xpr_oracle_bin_sort(C.c_int64(N), _p(depth), _p(proj["tile_rect"]), _p(proj["tile_count"]),
+                                  C.c_int32(tx), C.c_int32(ty), C.c_int64(I), _p(keys), _p(vals), _p(ranges))
+    assert n == I, (n, I)
+    return dict(keys=keys, vals=vals, ranges=ranges, num_pairs=I)
+
+
+def rasterize_fwd(proj: dict, binned: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    H, W = int(cam.height), int(cam.width)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv")]
+    out = dict(image=np.empty((H, W, 3), dt), final_T=np.empty((H, W), dt), n_contrib=np.empty((H, W), np.uint32),
+               fragile=np.empty((H, W), np.uint8))
+    counters = np.zeros(2, np.int64)
+    fn = getattr(lib(), "xpr_oracle_rasterize_fwd_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+       _p(out["image"]), _p(out["final_T"]), _p(out["n_contrib"]), _p(out["fragile"]), _p(counters))
+    out["pp_visit"], out["pp_pass"] = int(counters[0]), int(counters[1])
+    return out
+
+
+def rasterize_fwd_strict(proj: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    H, W = int(cam.height), int(cam.width)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv", "depth")]
+    out = dict(image=np.empty((H, W, 3), dt), final_T=np.empty((H, W), dt), n_contrib=np.empty((H, W), np.uint32))
+    fn = getattr(lib(), "xpr_oracle_rasterize_fwd_strict_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(proj["tile_rect"]), _p(proj["tile_count"]),
+       _p(out["image"]), _p(out["final_T"]), _p(out["n_contrib"]))
+    return out
+
+
+def rasterize_bwd(proj: dict, binned: dict, fwd: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv")]
+    dL = np.ascontiguousarray(dL_dimage, dt)
+    out = dict(g_mean2d=np.empty((N, 2), np.float64), g_conic=np.empty((N, 3), np.float64),
+               g_opac_eff=np.empty(N, np.float64), g_rgb=np.empty((N, 3), np.float64))
+    fn = getattr(lib(), "xpr_oracle_rasterize_bwd_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+       _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), _p(dL),
+       _p(out["g_mean2d"]), _p(out["g_conic"]), _p(out["g_opac_eff"]), _p(out["g_rgb"]))
+    return out
+
+
+def project_bwd(means, scales, quats, opacities, sh, cam: XoCamera, cfg: XoConfig, grads: dict, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    N = int(means.shape[0])
+    K = (int(cfg.sh_degree) + 1) ** 2
+    a = [np.ascontiguousarray(x, dt) for x in (means, scales, quats, opacities, sh)]
+    g = [np.ascontiguousarray(grads[k], np.float64) for k in ("g_mean2d", "g_conic", "g_opac_eff", "g_rgb")]
+    out = dict(g_means=np.empty((N, 3), np.float64), g_scales=np.empty((N, 3), np.float64),
+               g_quats=np.empty((N, 4), np.float64), g_opacities=np.empty(N, np.float64),
+               g_sh=np.empty((N, K, 3), np.float64))
+    fn = getattr(lib(), "xpr_oracle_project_bwd_" + _sfx(dt))
+    fn(C.c_int64(N), *[_p(x) for x in a], C.byref(cam), C.byref(cfg), *[_p(x) for x in g],
+       *[_p(out[k]) for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")])
+    return out
+
+
+def sh_basis(d, dtype=np.float64):
+    dt = np.dtype(dtype)
+    d = np.ascontiguousarray(d, dt)
+    out = np.empty(16, dt)
+    getattr(lib(), "xpr_oracle_sh_basis_" + _sfx(dt))(_p(d), _p(out))
+    return out
+
+
+def camera_project(cam: XoCamera, p, dtype=np.float64):
+    dt = np.dtype(dtype)
+    p = np.ascontiguousarray(p, dt)
+    out = np.empty(2, dt)
+    getattr(lib(), "xpr_oracle_camera_project_" + _sfx(dt))(C.byref(cam), _p(p), _p(out))
+    return out
+
+
+def render(scene_arrays: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """Full forward: project -> bin_sort -> rasterize_fwd. scene_arrays: means,scales,quats,opacities,sh."""
+    s = scene_arrays
+    proj = project(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, dtype)
+    binned = bin_sort(proj, cam, cfg)
+    fwd = rasterize_fwd(proj, binned, cam, cfg, dtype)
+    return dict(proj=proj, binned=binned, fwd=fwd)
+
+
+def backward(scene_arrays: dict, r: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """Full backward given render() output and dL/dimage; returns parameter gradients (fp64)."""
+    s = scene_arrays
+    g2 = rasterize_bwd(r["proj"], r["binned"], r["fwd"], dL_dimage, cam, cfg, dtype)
+    g3 = project_bwd(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, g2, dtype)
+    g3.update(g2)
+    return g3
