@@ -1,0 +1,147 @@
+/*
+ * xpr.h -- C-ABI boundary of libxpr.so: the tile-based splatting forward + backward hot path of
+ * "XPR: An Extensible Cross-Platform Point-Based Differentiable Renderer" (arxiv 2606.11529),
+ * hand-written CUDA for NVIDIA B200 (sm_100a).  Citations are PAPER.md line numbers ("PAPER L..")
+ * plus the readings C1..C26 and arithmetic rules R1..R3 listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *  - Every function returns an int32_t status (XPR_OK == 0).  No exceptions, no global state other
+ *    than the last CUDA error code (thread-local), re-entrant.
+ *  - Unless a parameter says HOST, every array pointer is a DEVICE pointer owned by the caller
+ *    (e.g. a PyTorch allocation), contiguous, row-major, 16-byte aligned.  The library allocates
+ *    no persistent device memory; scratch comes from the caller-provided workspace.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
+ *    enqueued on it.  The only call that synchronises the stream is xpr_bin_sort (8-byte read-back
+ *    of the pair count I).
+ *  - xpr_camera / xpr_config are HOST structs, read during the call.
+ *  - Arguments are validated before any launch: NULL or misaligned pointer, negative size, bad
+ *    enum -> XPR_ERR_INVALID_ARG; tile != 16, sh_degree > 3 -> XPR_ERR_UNSUPPORTED; a CUDA runtime
+ *    failure -> XPR_ERR_CUDA (code via xpr_last_cuda_error()).
+ *  - `scales`, `opacities`, `quats` are ACTIVATED values (positive scales, opacity in (0,1), unit
+ *    quaternion (w,x,y,z), not renormalised inside) exactly as the paper's PrimitiveParams
+ *    (PAPER L425-431).  Activations and the loss live outside the library.
+ *  - Pixel (i,j) is sampled at (i+0.5, j+0.5); mean2d is in continuous pixel coordinates (C1).
+ *    Tile t = ty*tiles_x + tx covers pixels [16 tx, 16 tx+16) x [16 ty, 16 ty+16).
+ */
+#ifndef XPR_H
+#define XPR_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { XPR_OK = 0, XPR_ERR_INVALID_ARG = 1, XPR_ERR_CAPACITY = 2, XPR_ERR_CUDA = 3, XPR_ERR_UNSUPPORTED = 4 };
+
+/* flags byte written per Gaussian by xpr_project */
+enum { XPR_FLAG_VISIBLE = 1, XPR_FLAG_CLAMP_U = 2, XPR_FLAG_CLAMP_V = 4,
+       XPR_FLAG_RGB_POS_R = 8, XPR_FLAG_RGB_POS_G = 16, XPR_FLAG_RGB_POS_B = 32 };
+
+typedef struct {
+    int32_t model;          /* 0 pinhole, 1 fisheye-equidistant (C18) */
+    int32_t width, height;  /* pixels */
+    float fx, fy, cx, cy;   /* intrinsics (C2) */
+    float k[4];             /* fisheye radial distortion k1..k4 */
+    float w2c[12];          /* row-major 3x4 [W|t]: x_cam = W x_world + t, +z forward, x right, y down */
+} xpr_camera;
+
+typedef struct {
+    int32_t projection;     /* 0 EWA (PAPER Listing 1), 1 UT with 7 sigma points */
+    int32_t sh_degree;      /* 0..3, K = (sh_degree+1)^2 coefficients per channel */
+    int32_t tile;           /* tile edge in pixels; must be 16 */
+    int32_t antialias;      /* Mip-Splatting opacity factor (C19) */
+    float alpha_thresh;     /* 1/255 */
+    float alpha_max;        /* 0.99 (C11) */
+    float t_min;            /* 1e-4 transmittance exit (C12) */
+    float z_near;           /* 0.2 (C9) */
+    float lowpass;          /* 0.3 added to the 2D covariance diagonal (C4) */
+    float ut_alpha, ut_beta, ut_kappa;  /* unscented-transform weights: 1, 2, 0 */
+    float bg[3];            /* background colour (C13) */
+} xpr_config;
+
+const char* xpr_status_string(int32_t status);
+int32_t xpr_last_cuda_error(void);   /* cudaError_t of the last XPR_ERR_CUDA on this thread */
+int32_t xpr_version(void);           /* 10000*major + 100*minor + patch */
+
+/*
+ * xpr_project -- Preprocess stage (Listing 1; A.1.1 L435; UT: L437,
+ * Listing 3) fused with SH -> RGB (C5).  One thread per Gaussian.
+ *   in : means[N,3] scales[N,3] quats[N,4] opacities[N] sh[N,K,3]  (fp32)
+ *   out: mean2d[N,2], conic_opac[N,4] = (A,B,C,o_eff) with (A,B,C) the inverse of the low-passed
+ *        2D covariance, rgb[N,3], depth[N] (camera z of the mean), lnv[N] = ln(o_eff/alpha_thresh),
+ *        tile_rect[N,4] = (x_min,y_min,x_max,y_max) half-open in tile units,
+ *        tile_count[N] = rectangle area if visible else 0, flags[N].
+ *   For a culled Gaussian only tile_count (=0) and flags (=0) are written; its other outputs are
+ *   left untouched (they are never read downstream).
+ *   Arithmetic follows rule R1: fp32, every operation individually rounded, no FMA contraction,
+ *   so that depth bits, rectangles and tile counts are bit-reproducible.
+ */
+int32_t xpr_project(int64_t N, const float* means, const float* scales, const float* quats,
+                    const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
+                    float* mean2d, float* conic_opac, float* rgb, float* depth, float* lnv,
+                    int32_t* tile_rect, uint32_t* tile_count, uint8_t* flags, void* stream);
+
+/*
+ * xpr_bin_sort -- Rasterizer stage: prefix-sum of tile counts, replication,
+ * tile-id assignment  x = x_min + (r mod w), y = y_min + floor(r / w), t = y*tiles_x + x,
+ * key = (uint64)t << 32 | float_bits(depth) (BASELINE.json:north_star, C10), value = Gaussian
+ * index; stable LSD radix sort by key (hand-written onesweep); per-tile bounds.
+ *   in : depth[N], tile_rect[N,4], tile_count[N] from xpr_project; pair_capacity = length of the
+ *        output arrays (must be < 2^30).
+ *   out: keys_sorted[I] u64, vals_sorted[I] u32, tile_ranges[T,2] = (start,end) per tile, (0,0)
+ *        for an empty tile; *num_pairs_host (HOST int64) = I.
+ *   I > pair_capacity -> XPR_ERR_CAPACITY, *num_pairs_host = required I, nothing out of bounds
+ *   is written and the outputs are unspecified.
+ *   workspace: DEVICE scratch of at least xpr_bin_sort_workspace() bytes, 256-byte aligned.
+ *   Equal keys keep emission order = ascending Gaussian index.
+ */
+int32_t xpr_bin_sort_workspace(int64_t N, int64_t pair_capacity, int32_t num_tiles, size_t* bytes);
+int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
+                     const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
+                     uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
+                     int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * xpr_rasterize_fwd -- Shader stage (Algorithm 1, Listing 1).
+ * Per pixel, front to back over its tile's list:
+ *   power = -1/2 (A dx^2 + C dy^2) - B dx dy   (order fixed by R3);
+ *   skip if power > 0 (L289) or power < -lnv (alpha < alpha_thresh, L679, C12);
+ *   alpha = min(alpha_max, o_eff exp(power));  T' = T (1 - alpha);  stop WITHOUT blending if
+ *   T' < t_min;  C += rgb alpha T;  T = T'.   Finally C += T bg.
+ *   out: image[H,W,3], final_T[H,W], n_contrib[H,W] = 1 + list position of the last blended entry.
+ */
+int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                          const float* conic_opac, const float* rgb, const float* lnv,
+                          const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                          float* image, float* final_T, uint32_t* n_contrib, void* stream);
+
+/*
+ * xpr_rasterize_bwd -- reverse mode through compositing (the paper relies on AD, L106; formulas
+ * in DESIGN.md section 3, readings C14-C15).  Replays each tile back to front from n_contrib.
+ *   in : forward inputs + final_T, n_contrib, dL_dimage[H,W,3].
+ *   out: g_mean2d[N,2], g_conic[N,3] (w.r.t. A,B,C), g_opac[N] (w.r.t. o_eff), g_rgb[N,3];
+ *        ACCUMULATED with fp32 atomics; zero-filled first by this call when zero_init != 0.
+ */
+int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                          const float* conic_opac, const float* rgb, const float* lnv,
+                          const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                          const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
+                          float* g_mean2d, float* g_conic, float* g_opac, float* g_rgb,
+                          int32_t zero_init, void* stream);
+
+/*
+ * xpr_project_bwd -- reverse mode through projection (EWA or UT) and SH (DESIGN.md section 3,
+ * readings C16-C19).  One thread per Gaussian; a culled Gaussian (tile_count == 0) gets zeros.
+ *   out (fully overwritten): g_means[N,3] g_scales[N,3] g_quats[N,4] g_opacities[N] g_sh[N,K,3].
+ */
+int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, const float* quats,
+                        const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
+                        const uint32_t* tile_count, const uint8_t* flags,
+                        const float* g_mean2d, const float* g_conic, const float* g_opac, const float* g_rgb,
+                        float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh,
+                        void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XPR_H */

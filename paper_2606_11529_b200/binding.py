@@ -1,0 +1,171 @@
+"""Thin ctypes binding of libxpr.so (include/xpr.h): same names, argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library; PyTorch is used for device memory and
+streams.  There is no CPU fallback: if libxpr.so is missing or a call fails, an exception is raised.
+Nothing here imports ``oracle/``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libxpr.so")
+
+XPR_OK, XPR_ERR_INVALID_ARG, XPR_ERR_CAPACITY, XPR_ERR_CUDA, XPR_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
+FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_RGB_POS_B = 1, 2, 4, 8, 16, 32
+
+SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
+           "xpr_bin_sort", "xpr_rasterize_fwd", "xpr_rasterize_bwd", "xpr_project_bwd")
+
+
+class XprCamera(C.Structure):
+    _fields_ = [("model", C.c_int32), ("width", C.c_int32), ("height", C.c_int32),
+                ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float), ("cy", C.c_float),
+                ("k", C.c_float * 4), ("w2c", C.c_float * 12)]
+
+
+class XprConfig(C.Structure):
+    _fields_ = [("projection", C.c_int32), ("sh_degree", C.c_int32), ("tile", C.c_int32), ("antialias", C.c_int32),
+                ("alpha_thresh", C.c_float), ("alpha_max", C.c_float), ("t_min", C.c_float), ("z_near", C.c_float),
+                ("lowpass", C.c_float), ("ut_alpha", C.c_float), ("ut_beta", C.c_float), ("ut_kappa", C.c_float),
+                ("bg", C.c_float * 3)]
+
+
+class XprError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().xpr_status_string(C.c_int32(status)).decode()
+        if status == XPR_ERR_CUDA:
+            msg += f" [cudaError {lib().xpr_last_cuda_error()}]"
+        super().__init__(f"{where}: {msg}")
+
+
+_lib = None
+
+
+def lib():
+    """Load libxpr.so (built in-tree by ``python -m paper_2606_11529_b200.build``); fail loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_2606_11529_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.xpr_status_string.restype = C.c_char_p
+        for name in SYMBOLS[1:]:
+            getattr(L, name).restype = C.c_int32
+        _lib = L
+    return _lib
+
+
+def make_camera(cam) -> XprCamera:
+    """cam: any object with model,width,height,fx,fy,cx,cy,k,w2c (e.g. scenes.Camera)."""
+    c = XprCamera()
+    c.model, c.width, c.height = int(cam.model), int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    for i in range(4):
+        c.k[i] = float(cam.k[i])
+    w = [float(v) for row in cam.w2c for v in row]
+    for i in range(12):
+        c.w2c[i] = w[i]
+    return c
+
+
+def make_config(d: dict) -> XprConfig:
+    c = XprConfig()
+    c.projection, c.sh_degree, c.tile, c.antialias = int(d["projection"]), int(d["sh_degree"]), int(d["tile"]), int(d["antialias"])
+    c.alpha_thresh, c.alpha_max, c.t_min = float(d["alpha_thresh"]), float(d["alpha_max"]), float(d["t_min"])
+    c.z_near, c.lowpass = float(d["z_near"]), float(d["lowpass"])
+    c.ut_alpha, c.ut_beta, c.ut_kappa = float(d["ut_alpha"]), float(d["ut_beta"]), float(d["ut_kappa"])
+    for i in range(3):
+        c.bg[i] = float(d["bg"][i])
+    return c
+
+
+def num_tiles(cam: XprCamera, cfg: XprConfig):
+    ts = int(cfg.tile)
+    return (int(cam.width) + ts - 1) // ts, (int(cam.height) + ts - 1) // ts
+
+
+def _p(t):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return C.c_void_p(0)
+    if not t.is_cuda:
+        raise TypeError("xpr: expected a CUDA tensor (the library takes device pointers; no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError("xpr: tensor must be contiguous")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check(status: int, where: str):
+    if status != XPR_OK:
+        raise XprError(status, where)
+
+
+def xpr_version() -> int:
+    return int(lib().xpr_version())
+
+
+def xpr_project(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, depth,
+                lnv, tile_rect, tile_count, flags, stream=None):
+    N = int(means.shape[0])
+    _check(lib().xpr_project(C.c_int64(N), _p(means), _p(scales), _p(quats), _p(opacities), _p(sh), C.byref(cam),
+                             C.byref(cfg), _p(mean2d), _p(conic_opac), _p(rgb), _p(depth), _p(lnv), _p(tile_rect),
+                             _p(tile_count), _p(flags), _stream(stream)), "xpr_project")
+
+
+def xpr_bin_sort_workspace(N: int, pair_capacity: int, n_tiles: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().xpr_bin_sort_workspace(C.c_int64(N), C.c_int64(pair_capacity), C.c_int32(n_tiles), C.byref(out)),
+           "xpr_bin_sort_workspace")
+    return int(out.value)
+
+
+def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, pair_capacity: int, keys_sorted,
+                 vals_sorted, tile_ranges, workspace, stream=None, raise_on_capacity: bool = True):
+    """Returns (status, I).  On XPR_ERR_CAPACITY I is the required capacity."""
+    N = int(tile_count.shape[0])
+    n_pairs = C.c_int64(0)
+    st = lib().xpr_bin_sort(C.c_int64(N), _p(depth), _p(tile_rect), _p(tile_count), C.byref(cam), C.byref(cfg),
+                            C.c_int64(pair_capacity), _p(keys_sorted), _p(vals_sorted), _p(tile_ranges),
+                            C.byref(n_pairs), _p(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+                            _stream(stream))
+    if st == XPR_ERR_CAPACITY and not raise_on_capacity:
+        return st, int(n_pairs.value)
+    _check(st, "xpr_bin_sort")
+    return st, int(n_pairs.value)
+
+
+def xpr_rasterize_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, image,
+                      final_T, n_contrib, stream=None):
+    N = int(mean2d.shape[0])
+    _check(lib().xpr_rasterize_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
+                                   _p(lnv), _p(vals_sorted), _p(tile_ranges), _p(image), _p(final_T), _p(n_contrib),
+                                   _stream(stream)), "xpr_rasterize_fwd")
+
+
+def xpr_rasterize_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, final_T,
+                      n_contrib, dL_dimage, g_mean2d, g_conic, g_opac, g_rgb, zero_init: bool = True, stream=None):
+    N = int(mean2d.shape[0])
+    _check(lib().xpr_rasterize_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
+                                   _p(lnv), _p(vals_sorted), _p(tile_ranges), _p(final_T), _p(n_contrib),
+                                   _p(dL_dimage), _p(g_mean2d), _p(g_conic), _p(g_opac), _p(g_rgb),
+                                   C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_bwd")
+
+
+def xpr_project_bwd(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, tile_count, flags, g_mean2d,
+                    g_conic, g_opac, g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None):
+    N = int(means.shape[0])
+    _check(lib().xpr_project_bwd(C.c_int64(N), _p(means), _p(scales), _p(quats), _p(opacities), _p(sh), C.byref(cam),
+                                 C.byref(cfg), _p(tile_count), _p(flags), _p(g_mean2d), _p(g_conic), _p(g_opac),
+                                 _p(g_rgb), _p(g_means), _p(g_scales), _p(g_quats), _p(g_opacities), _p(g_sh),
+                                 _stream(stream)), "xpr_project_bwd")

@@ -1,0 +1,257 @@
+// rasterize.cu -- xpr_rasterize_fwd / xpr_rasterize_bwd: per-tile front-to-back alpha compositing
+// (Algorithm 1, Listing 1) and its reverse-mode pass.
+//
+// One CTA per 16x16 tile, one thread per pixel.  The tile's list vals_sorted[start..end) is
+// staged through shared memory in batches; every thread walks the batch with warp-broadcast
+// LDS.128 reads.  Decisions (the power > 0 guard and the alpha gate) are taken on `power`,
+// computed in the fixed fp32 order of rule R3 with explicit _rn intrinsics, never on exp().
+#include "common.cuh"
+
+namespace xpr {
+namespace {
+
+constexpr int BLOCK = TILE * TILE;   // 256 threads = 256 pixels
+
+struct RasterParams {
+    int W, H, TW;
+    float amax, tmin;
+    float bg[3];
+};
+
+// power = fma(fma(qa, dx, qb*dy), dx, (qc*dy)*dy) with qa = -A/2, qb = -B, qc = -C/2 (R3, C25)
+__device__ __forceinline__ float eval_power(float qa, float qb, float qc, float dx, float dy) {
+    return __fmaf_rn(__fmaf_rn(qa, dx, __fmul_rn(qb, dy)), dx, __fmul_rn(__fmul_rn(qc, dy), dy));
+}
+
+__device__ __forceinline__ float fast_exp(float x) {   // ex2.approx(x * log2 e); x in [-lnv, 0]
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x * 1.4426950408889634f));
+    return y;
+}
+
+__global__ void __launch_bounds__(BLOCK)
+rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
+                     const float* __restrict__ rgb, const float* __restrict__ lnv,
+                     const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
+                     float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
+    __shared__ float4 s_geo[BLOCK];   // mx, my, qa, qb
+    __shared__ float4 s_gate[BLOCK];  // qc, thr = -lnv, o, unused
+    __shared__ float4 s_col[BLOCK];   // r, g, b, unused
+    const int tile = blockIdx.x;
+    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int px = tx * TILE + (threadIdx.x & (TILE - 1)), py = ty * TILE + (threadIdx.x >> 4);
+    const bool inside = (px < P.W) && (py < P.H);
+    const float pxc = (float)px + 0.5f, pyc = (float)py + 0.5f;
+    const uint2 rg = ranges[tile];
+    const uint32_t len = rg.y - rg.x;
+
+    float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
+    uint32_t last = 0;
+    bool done = !inside;
+
+    for (uint32_t base = 0; base < len; base += BLOCK) {
+        if (__syncthreads_count(done) == BLOCK) break;
+        const uint32_t cnt = min((uint32_t)BLOCK, len - base);
+        if (threadIdx.x < cnt) {
+            const uint32_t g = vals[rg.x + base + threadIdx.x];
+            const float2 m = mean2d[g];
+            const float4 co = conic_opac[g];
+            s_geo[threadIdx.x] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
+            s_gate[threadIdx.x] = make_float4(-0.5f * co.z, -lnv[g], co.w, 0.0f);
+            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
+        }
+        __syncthreads();
+        if (!done) {
+            for (uint32_t j = 0; j < cnt; ++j) {
+                const float4 ge = s_geo[j];
+                const float4 ga = s_gate[j];
+                const float dx = pxc - ge.x, dy = pyc - ge.y;
+                const float power = eval_power(ge.z, ge.w, ga.x, dx, dy);
+                if (power > 0.0f) continue;       // valid = power <= 0 (L289, C20)
+                if (power < ga.y) continue;       // alpha < alpha_thresh (L679, C12)
+                const float og = ga.z * fast_exp(power);
+                const float alpha = fminf(P.amax, og);          // C11
+                const float Tn = T * (1.0f - alpha);
+                if (Tn < P.tmin) { done = true; break; }        // C12: stop without blending
+                const float4 c = s_col[j];
+                const float w = alpha * T;
+                C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+                T = Tn;
+                last = base + j + 1;
+            }
+        }
+    }
+    if (inside) {
+        const int64_t pid = (int64_t)py * P.W + px;
+        image[3 * pid] = fmaf(T, P.bg[0], C0);
+        image[3 * pid + 1] = fmaf(T, P.bg[1], C1);
+        image[3 * pid + 2] = fmaf(T, P.bg[2], C2);
+        final_T[pid] = T;
+        n_contrib[pid] = last;
+    }
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void __launch_bounds__(BLOCK)
+rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
+                     const float* __restrict__ rgb, const float* __restrict__ lnv,
+                     const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
+                     const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
+                     const float* __restrict__ dL, float* __restrict__ g_mean2d, float* __restrict__ g_conic,
+                     float* __restrict__ g_opac, float* __restrict__ g_rgb) {
+    __shared__ float4 s_geo[BLOCK];   // mx, my, A, B
+    __shared__ float4 s_gate[BLOCK];  // C, thr, o, unused
+    __shared__ float4 s_col[BLOCK];   // r, g, b, index (bits)
+    __shared__ uint32_t s_max[BLOCK / 32];
+    const int tile = blockIdx.x;
+    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int px = tx * TILE + (threadIdx.x & (TILE - 1)), py = ty * TILE + (threadIdx.x >> 4);
+    const bool inside = (px < P.W) && (py < P.H);
+    const float pxc = (float)px + 0.5f, pyc = (float)py + 0.5f;
+    const uint2 rg = ranges[tile];
+    const int lane = threadIdx.x & 31;
+
+    uint32_t n = 0;
+    float T = 0.0f, g0 = 0.0f, g1 = 0.0f, g2 = 0.0f;
+    if (inside) {
+        const int64_t pid = (int64_t)py * P.W + px;
+        n = n_contrib[pid];
+        T = final_T[pid];
+        g0 = dL[3 * pid]; g1 = dL[3 * pid + 1]; g2 = dL[3 * pid + 2];
+    }
+    // colour behind the current entry, S_k = sum_{j>k} c_j alpha_j T_j + T_final bg (C13)
+    float S0 = T * P.bg[0], S1 = T * P.bg[1], S2 = T * P.bg[2];
+    uint32_t wmax = n;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+    if (lane == 0) s_max[threadIdx.x >> 5] = wmax;
+    __syncthreads();
+    uint32_t max_n = 0;
+#pragma unroll
+    for (int w = 0; w < BLOCK / 32; ++w) max_n = max(max_n, s_max[w]);
+
+    for (uint32_t hi = max_n; hi > 0;) {
+        const uint32_t cnt = min((uint32_t)BLOCK, hi);
+        __syncthreads();
+        if (threadIdx.x < cnt) {      // slot j holds list position hi-1-j (descending)
+            const uint32_t g = vals[rg.x + hi - 1 - threadIdx.x];
+            const float2 m = mean2d[g];
+            const float4 co = conic_opac[g];
+            s_geo[threadIdx.x] = make_float4(m.x, m.y, co.x, co.y);
+            s_gate[threadIdx.x] = make_float4(co.z, -lnv[g], co.w, 0.0f);
+            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], __uint_as_float(g));
+        }
+        __syncthreads();
+        for (uint32_t j = 0; j < cnt; ++j) {
+            const uint32_t pos = hi - 1 - j;
+            if (pos >= wmax) continue;     // warp-uniform: nobody in this warp got this far
+            const float4 ge = s_geo[j];
+            const float4 ga = s_gate[j];
+            const float dx = pxc - ge.x, dy = pyc - ge.y;
+            const float A = ge.z, Bc = ge.w, Cc = ga.x;
+            const float power = eval_power(-0.5f * A, -Bc, -0.5f * Cc, dx, dy);
+            const bool contrib = (pos < n) && !(power > 0.0f) && !(power < ga.y);
+            if (!__any_sync(0xffffffffu, contrib)) continue;
+            float v_mx = 0.f, v_my = 0.f, v_A = 0.f, v_B = 0.f, v_C = 0.f, v_o = 0.f, v_r = 0.f, v_g = 0.f, v_b = 0.f;
+            const float4 c = s_col[j];
+            if (contrib) {
+                const float G = fast_exp(power);
+                const float og = ga.z * G;
+                const float alpha = fminf(P.amax, og);
+                const float oma = 1.0f - alpha;
+                const float inv = 1.0f / oma;
+                T = T * inv;                       // transmittance in front of this entry
+                const float w = alpha * T;
+                v_r = w * g0; v_g = w * g1; v_b = w * g2;
+                const float dalpha = g0 * (c.x * T - S0 * inv) + g1 * (c.y * T - S1 * inv) + g2 * (c.z * T - S2 * inv);
+                S0 = fmaf(c.x, w, S0); S1 = fmaf(c.y, w, S1); S2 = fmaf(c.z, w, S2);
+                if (og < P.amax) {                 // C14: the clamp has zero derivative
+                    const float dpow = og * dalpha;
+                    v_o = G * dalpha;
+                    v_A = -0.5f * dx * dx * dpow; v_B = -dx * dy * dpow; v_C = -0.5f * dy * dy * dpow;
+                    v_mx = (A * dx + Bc * dy) * dpow; v_my = (Bc * dx + Cc * dy) * dpow;
+                }
+            }
+            v_mx = warp_sum(v_mx); v_my = warp_sum(v_my); v_A = warp_sum(v_A); v_B = warp_sum(v_B);
+            v_C = warp_sum(v_C); v_o = warp_sum(v_o); v_r = warp_sum(v_r); v_g = warp_sum(v_g); v_b = warp_sum(v_b);
+            if (lane == 0) {
+                const uint32_t g = __float_as_uint(c.w);
+                atomicAdd(g_mean2d + 2 * g, v_mx); atomicAdd(g_mean2d + 2 * g + 1, v_my);
+                atomicAdd(g_conic + 3 * g, v_A); atomicAdd(g_conic + 3 * g + 1, v_B); atomicAdd(g_conic + 3 * g + 2, v_C);
+                atomicAdd(g_opac + g, v_o);
+                atomicAdd(g_rgb + 3 * g, v_r); atomicAdd(g_rgb + 3 * g + 1, v_g); atomicAdd(g_rgb + 3 * g + 2, v_b);
+            }
+        }
+        hi -= cnt;
+    }
+}
+
+int32_t make_raster_params(const xpr_camera* cam, const xpr_config* cfg, RasterParams& P) {
+    P.W = cam->width; P.H = cam->height; P.TW = tiles_x(cam);
+    P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
+    for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
+    return XPR_OK;
+}
+
+}  // namespace
+}  // namespace xpr
+
+using namespace xpr;
+
+extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                     const float* conic_opac, const float* rgb, const float* lnv,
+                                     const uint32_t* vals_sorted, const uint32_t* tile_ranges, float* image,
+                                     float* final_T, uint32_t* n_contrib, void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+                  !aligned(vals_sorted, 4)))
+        return XPR_ERR_INVALID_ARG;
+    RasterParams P;
+    make_raster_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    rasterize_fwd_kernel<<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib);
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                     const float* conic_opac, const float* rgb, const float* lnv,
+                                     const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* final_T,
+                                     const uint32_t* n_contrib, const float* dL_dimage, float* g_mean2d,
+                                     float* g_conic, float* g_opac, float* g_rgb, int32_t zero_init, void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+        !aligned(vals_sorted, 4) || !aligned(g_mean2d, 4) || !aligned(g_conic, 4) || !aligned(g_opac, 4) ||
+        !aligned(g_rgb, 4))
+        return XPR_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (zero_init) {
+        XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 2 * (size_t)N, st));
+        XPR_CUDA(cudaMemsetAsync(g_conic, 0, sizeof(float) * 3 * (size_t)N, st));
+        XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * (size_t)N, st));
+        XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * (size_t)N, st));
+    }
+    RasterParams P;
+    make_raster_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    rasterize_bwd_kernel<<<T, BLOCK, 0, st>>>(
+        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_mean2d, g_conic,
+        g_opac, g_rgb);
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}

@@ -1,0 +1,105 @@
+"""Buffer plumbing around the five C-ABI calls: allocation (PyTorch), call order, capacity regrowth.
+
+No arithmetic of the method lives here -- each stage is one call into libxpr.so (binding.py).
+Call stack of one step:
+    xpr_project -> xpr_bin_sort -> xpr_rasterize_fwd -> [loss outside] -> xpr_rasterize_bwd -> xpr_project_bwd
+"""
+from __future__ import annotations
+
+import torch
+
+from . import binding as xb
+
+
+class SplatPipeline:
+    """Owns the intermediate device buffers for one (N, camera, config) and sequences the stages."""
+
+    def __init__(self, N: int, cam, cfg: dict, pair_capacity: int | None = None, device="cuda:0"):
+        self.N = int(N)
+        self.device = torch.device(device)
+        self.cam = cam if isinstance(cam, xb.XprCamera) else xb.make_camera(cam)
+        self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
+        self.K = (int(self.cfg.sh_degree) + 1) ** 2
+        self.W, self.H = int(self.cam.width), int(self.cam.height)
+        self.TW, self.TH = xb.num_tiles(self.cam, self.cfg)
+        self.T = self.TW * self.TH
+        d, f32, i32 = self.device, torch.float32, torch.int32
+        N = self.N
+        e = lambda *s, dtype=f32: torch.empty(*s, dtype=dtype, device=d)
+        # projection outputs (a1-a3)
+        self.mean2d, self.conic_opac, self.rgb = e(N, 2), e(N, 4), e(N, 3)
+        self.depth, self.lnv = e(N), e(N)
+        self.tile_rect, self.tile_count = e(N, 4, dtype=i32), e(N, dtype=i32)
+        self.flags = e(N, dtype=torch.uint8)
+        # binning / sort outputs (a4-a7)
+        self.tile_ranges = e(self.T, 2, dtype=i32)
+        self.num_pairs = 0
+        self._alloc_pairs(int(pair_capacity) if pair_capacity else max(1 << 16, 8 * N))
+        # compositing outputs (a8)
+        self.image, self.final_T = e(self.H, self.W, 3), e(self.H, self.W)
+        self.n_contrib = e(self.H, self.W, dtype=i32)
+        # gradients (a9, a10)
+        self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb = e(N, 2), e(N, 3), e(N), e(N, 3)
+        self.g_means, self.g_scales, self.g_quats = e(N, 3), e(N, 3), e(N, 4)
+        self.g_opacities, self.g_sh = e(N), e(N, self.K, 3)
+
+    def _alloc_pairs(self, cap: int):
+        cap = min(int(cap), (1 << 30) - 1)
+        self.pair_capacity = cap
+        d = self.device
+        self.keys_sorted = torch.empty(max(cap, 1), dtype=torch.int64, device=d)
+        self.vals_sorted = torch.empty(max(cap, 1), dtype=torch.int32, device=d)
+        ws = xb.xpr_bin_sort_workspace(self.N, cap, self.T)
+        self.workspace = torch.empty(ws, dtype=torch.uint8, device=d)
+
+    # ---- stages ------------------------------------------------------------------------------
+    def project(self, means, scales, quats, opacities, sh):
+        self._inputs = (means, scales, quats, opacities, sh)
+        xb.xpr_project(means, scales, quats, opacities, sh, self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb,
+                       self.depth, self.lnv, self.tile_rect, self.tile_count, self.flags)
+
+    def bin_sort(self):
+        while True:
+            st, n = xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg,
+                                    self.pair_capacity, self.keys_sorted, self.vals_sorted, self.tile_ranges,
+                                    self.workspace, raise_on_capacity=False)
+            if st == xb.XPR_OK:
+                self.num_pairs = n
+                return n
+            if n >= (1 << 30):
+                raise xb.XprError(st, "xpr_bin_sort (pair count exceeds 2^30)")
+            self._alloc_pairs(int(n * 1.25) + 1024)   # XPR_ERR_CAPACITY: regrow and redo
+
+    def rasterize_fwd(self):
+        xb.xpr_rasterize_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
+                             self.tile_ranges, self.image, self.final_T, self.n_contrib)
+
+    def rasterize_bwd(self, dL_dimage):
+        xb.xpr_rasterize_bwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
+                             self.tile_ranges, self.final_T, self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic,
+                             self.g_opac, self.g_rgb, zero_init=True)
+
+    def project_bwd(self):
+        means, scales, quats, opacities, sh = self._inputs
+        xb.xpr_project_bwd(means, scales, quats, opacities, sh, self.cam, self.cfg, self.tile_count, self.flags,
+                           self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb, self.g_means, self.g_scales,
+                           self.g_quats, self.g_opacities, self.g_sh)
+
+    # ---- whole passes -------------------------------------------------------------------------
+    def forward(self, means, scales, quats, opacities, sh):
+        self.project(means, scales, quats, opacities, sh)
+        self.bin_sort()
+        self.rasterize_fwd()
+        return self.image
+
+    def backward(self, dL_dimage):
+        self.rasterize_bwd(dL_dimage)
+        self.project_bwd()
+        return dict(g_means=self.g_means, g_scales=self.g_scales, g_quats=self.g_quats,
+                    g_opacities=self.g_opacities, g_sh=self.g_sh)
+
+
+def scene_to_device(scene, device="cuda:0"):
+    """Upload a scenes.Scene's parameter arrays; returns (means, scales, quats, opacities, sh)."""
+    t = lambda a: torch.from_numpy(a).to(device).contiguous()
+    return t(scene.means), t(scene.scales), t(scene.quats), t(scene.opacities), t(scene.sh)
