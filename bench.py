@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- fwd+bwd megapixels/s of the tile-based splatting hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--view 0]
+
+A "step" is one pass of the whole hot path over one view: xpr_project -> xpr_bin_sort ->
+xpr_rasterize_fwd -> (L1 loss gradient, torch) -> xpr_rasterize_bwd -> xpr_project_bwd.
+Workload: BASELINE.json configs[2] ("3DGS unbounded-scene scale": 1,000,000 Gaussians, 1920x1080),
+the configuration BASELINE.json:north_star quotes its target on.  Synthetic seeded scene.
+Multi-GPU: replicas only; each rank runs the same step, no data-path collective.
+One JSON line on stdout (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC, UNIT = "fwd_bwd_megapixels_per_s", "MP/s"
+WORKLOADS = {1: "configs[0] tiny 3DGS 1k Gaussians 64x64", 2: "configs[1] 3DGS object-scale 100k Gaussians 800x800",
+             3: "configs[2] 3DGS unbounded-scene 1M Gaussians 1920x1080",
+             4: "configs[3] 3DGUT fisheye 1M Gaussians 1920x1080", 5: "configs[4] 3DGS stress 3M Gaussians 1920x1080"}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--view", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--stages", action="store_true", help="also print per-stage times to stderr")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_step(xo, scenes, sc, view, np):
+    """One fwd+bwd step of the CPU oracle, as it stands (never tuned)."""
+    cam = xo.make_camera(sc.cameras[view])
+    cfg = xo.make_config(scenes.default_render_config(sc))
+    arrays = dict(means=sc.means, scales=sc.scales, quats=sc.quats, opacities=sc.opacities, sh=sc.sh)
+    t0 = time.perf_counter()
+    r = xo.render(arrays, cam, cfg, np.float32)
+    _, dL = scenes.loss_and_grad(sc.loss, r["fwd"]["image"], sc.target(view))
+    xo.backward(arrays, r, dL, cam, cfg, np.float32)
+    return time.perf_counter() - t0, r["binned"]["num_pairs"]
+
+
+def oracle_sample(args):
+    """Bounded sample of the bench workload for the CPU legs: same scene and Gaussian count, image at
+    1/4 linear resolution (same field of view), so that a step is ~10-30 s of CPU work."""
+    from paper_2606_11529_b200 import scenes
+    full = scenes.make_scene(args.config)
+    W, H = full.cameras[0].width, full.cameras[0].height
+    if args.config >= 3:
+        w, h = W // 4, H // 4
+        sc = scenes.make_scene(args.config, image_override=(w, h))
+        desc = f"same scene, all {sc.N} Gaussians, view {args.view}, {w}x{h} image (1/4 linear resolution, same FOV), 1 step"
+    else:
+        sc, w, h = full, W, H
+        desc = f"full workload, {sc.N} Gaussians, {w}x{h}, 1 step"
+    return sc, w, h, desc
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (this tier's reference arm)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import xpr_oracle as xo
+    from paper_2606_11529_b200 import scenes
+    sc, w, h, desc = oracle_sample(args)
+    for _ in range(args.warmup):
+        oracle_step(xo, scenes, sc, args.view, np)
+    t = 0.0
+    for _ in range(args.steps):
+        dt, I = oracle_step(xo, scenes, sc, args.view, np)
+        t += dt
+    ms = 1e3 * t / max(args.steps, 1)
+    val = (w * h / 1e6) / (ms / 1e3)
+    cores = xo.num_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config], "view": args.view, "sample": desc, "pairs": int(I)},
+            "gaussians_per_s": sc.N / (ms / 1e3),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# algorithmic work per unit: FP32 lane-ops per pixel-pair
+FWD_OPS_VISIT, FWD_OPS_PASS = 8, 9
+BWD_OPS_VISIT, BWD_OPS_PASS = 8, 45
+SMS, LANES_PER_SM = 148, 128
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2606_11529_b200 import binding as xb, pipeline, scenes
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --impl ours needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    xb.lib()   # fail loudly if libxpr.so is missing
+
+    sc = scenes.make_scene(args.config)
+    cam = sc.cameras[args.view]
+    cfg = scenes.default_render_config(sc)
+    params = pipeline.scene_to_device(sc, dev)
+    target = torch.from_numpy(sc.target(args.view)).to(dev)
+    pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def loss_grad(image):
+        if sc.loss == "l1":
+            return torch.sign(image - target)
+        return 2.0 * (image - target)
+
+    stage_names = ("project", "bin_sort", "rasterize_fwd", "loss_grad", "rasterize_bwd", "project_bwd")
+
+    def step(events=None):
+        ev = (lambda: None) if events is None else (lambda: events.append(_rec()))
+        ev(); pipe.project(*params)
+        ev(); pipe.bin_sort()
+        ev(); pipe.rasterize_fwd()
+        ev(); dL = loss_grad(pipe.image)
+        ev(); pipe.rasterize_bwd(dL)
+        ev(); pipe.project_bwd()
+        ev()
+
+    def _rec():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    n_pairs = pipe.num_pairs
+    # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
+    bits = max(1, (pipe.T - 1).bit_length()) if pipe.T > 1 else 0
+    passes = (32 + bits + 7) // 8
+    launches_per_step = 1 + 1 + passes + 1 + 1 + 1 + 1
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    all_events = []
+    barrier()
+    for _ in range(args.steps):
+        flush.fill_(1)                      # L2 flush between timed iterations (outside the event pairs)
+        evs = []
+        step(evs)
+        all_events.append(evs)
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [e[0].elapsed_time(e[-1]) for e in all_events]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms = total_ms / args.steps
+    stage_ms = {n: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in all_events])) for i, n in enumerate(stage_names)}
+    mp = cam.width * cam.height / 1e6
+    value = world * mp / (ms / 1e3)
+
+    # roofline of the dominant kernel (largest stage): pixel-pair counts from xpr_rasterize_stats
+    stats = torch.zeros(4, dtype=torch.int64, device=dev)
+    xb.xpr_rasterize_stats(pipe.cam, pipe.cfg, pipe.mean2d, pipe.conic_opac, pipe.rgb, pipe.lnv, pipe.vals_sorted,
+                           pipe.tile_ranges, stats)
+    visit, passed, blended, sum_n = [int(v) for v in stats.cpu().tolist()]
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    alu_peak = SMS * LANES_PER_SM * sm_max * 1e6 / 1e12          # T lane-ops/s (FMA = 1 lane-op)
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    dom = max(("rasterize_fwd", "rasterize_bwd", "bin_sort"), key=lambda n: stage_ms[n])
+    if dom == "rasterize_bwd":
+        ops = BWD_OPS_VISIT * sum_n + BWD_OPS_PASS * blended
+        roof = {"kernel": "rasterize_bwd_kernel", "bound": "alu", "achieved": ops / (stage_ms[dom] / 1e3) / 1e12,
+                "peak": alu_peak, "unit": "T lane-op/s"}
+    elif dom == "rasterize_fwd":
+        ops = FWD_OPS_VISIT * visit + FWD_OPS_PASS * passed
+        roof = {"kernel": "rasterize_fwd_kernel", "bound": "alu", "achieved": ops / (stage_ms[dom] / 1e3) / 1e12,
+                "peak": alu_peak, "unit": "T lane-op/s"}
+    else:
+        nbytes = n_pairs * (12 + 24 * passes + 8) + 24 * sc.N
+        roof = {"kernel": "bin_sort (emit + onesweep passes + ranges)", "bound": "hbm",
+                "achieved": nbytes / (stage_ms[dom] / 1e3) / 1e9, "peak": hbm_peak, "unit": "GB/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["peak_source"] = "MEASURED_PEAKS.json" if peaks else "fallback (B200_PROFILING.md)"
+    roof["ms_per_launch"] = stage_ms[dom]
+
+    # end to end through the public API with HOST buffers: H2D of the parameters, the step, D2H of results
+    e2e = None
+    if not args.no_e2e:
+        host_in = [torch.from_numpy(a).pin_memory() for a in (sc.means, sc.scales, sc.quats, sc.opacities, sc.sh)]
+        dev_in = [torch.empty_like(p) for p in params]
+        outs = [pipe.image, pipe.g_means, pipe.g_scales, pipe.g_quats, pipe.g_opacities, pipe.g_sh]
+        host_out = [torch.empty(o.shape, dtype=o.dtype).pin_memory() for o in outs]
+        h2d = sum(t.numel() * t.element_size() for t in host_in)
+        d2h = sum(t.numel() * t.element_size() for t in host_out)
+
+        def e2e_step():
+            for d, h in zip(dev_in, host_in):
+                d.copy_(h, non_blocking=True)
+            pipe.project(*dev_in); pipe.bin_sort(); pipe.rasterize_fwd()
+            pipe.rasterize_bwd(loss_grad(pipe.image)); pipe.project_bwd()
+            for h, o in zip(host_out, outs):
+                h.copy_(o, non_blocking=True)
+
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        k = max(3, min(args.steps, 10))
+        t_ms = 0.0
+        for _ in range(k):
+            flush.fill_(1)
+            a = _rec(); e2e_step(); b = _rec()
+            torch.cuda.synchronize()
+            t_ms += a.elapsed_time(b)
+        if world > 1:
+            t = torch.tensor([t_ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_ms = float(t.item())
+        e2e = {"value": world * mp / (t_ms / k / 1e3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "ms_per_step": t_ms / k}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sys.path.insert(0, os.path.join(ROOT, "oracle"))
+        import xpr_oracle as xo
+        osc, w, h, desc = oracle_sample(args)
+        dt, _ = oracle_step(xo, scenes, osc, args.view, np)
+        cpu = {"value": (w * h / 1e6) / dt, "unit": UNIT, "cores": xo.num_threads(), "kind": "oracle", "sample": desc,
+               "seconds": dt}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
+                           "image": [cam.width, cam.height], "pairs": n_pairs, "sort_passes": passes,
+                           "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",
+                           "parallelism": "replicas only" if world > 1 else "1 GPU"},
+                "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,
+                "pixel_pairs": {"visited": visit, "passed_gate": passed, "blended": blended, "sum_n_contrib": sum_n},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+                "roofline": roof, "cpu_baseline": cpu}
+        print(json.dumps(line), flush=True)
+        if args.stages:
+            print(json.dumps(stage_ms, indent=1), file=sys.stderr)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -116,6 +116,16 @@ int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t 
                           float* image, float* final_T, uint32_t* n_contrib, void* stream);
 
 /*
+ * xpr_rasterize_stats -- measurement aid (SURVEY.md 8(d) roofline accounting): the same walk as
+ * xpr_rasterize_fwd without writing an image; stats[0..3] (DEVICE uint64[4], overwritten) =
+ * {pixel-pairs visited, pixel-pairs passing both gates, pixel-pairs blended, sum of n_contrib}.
+ */
+int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                            const float* conic_opac, const float* rgb, const float* lnv,
+                            const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats,
+                            void* stream);
+
+/*
  * xpr_rasterize_bwd -- reverse mode through compositing (the paper relies on AD, L106; formulas
  * in DESIGN.md section 3, readings C14-C15).  Replays each tile back to front from n_contrib.
  *   in : forward inputs + final_T, n_contrib, dL_dimage[H,W,3].

@@ -18,7 +18,7 @@ XPR_OK, XPR_ERR_INVALID_ARG, XPR_ERR_CAPACITY, XPR_ERR_CUDA, XPR_ERR_UNSUPPORTED
 FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_RGB_POS_B = 1, 2, 4, 8, 16, 32
 
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
-           "xpr_bin_sort", "xpr_rasterize_fwd", "xpr_rasterize_bwd", "xpr_project_bwd")
+           "xpr_bin_sort", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd")
 
 
 class XprCamera(C.Structure):
@@ -151,6 +151,14 @@ def xpr_rasterize_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, l
     _check(lib().xpr_rasterize_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
                                    _p(lnv), _p(vals_sorted), _p(tile_ranges), _p(image), _p(final_T), _p(n_contrib),
                                    _stream(stream)), "xpr_rasterize_fwd")
+
+
+def xpr_rasterize_stats(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, stats,
+                        stream=None):
+    N = int(mean2d.shape[0])
+    _check(lib().xpr_rasterize_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
+                                     _p(lnv), _p(vals_sorted), _p(tile_ranges), _p(stats), _stream(stream)),
+           "xpr_rasterize_stats")
 
 
 def xpr_rasterize_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, final_T,

@@ -29,11 +29,15 @@ __device__ __forceinline__ float fast_exp(float x) {   // ex2.approx(x * log2 e)
     return y;
 }
 
+// STATS = true: the same walk, additionally counting pixel-pair events into stats[0..3] =
+// {visited, passed both gates, blended, sum of n_contrib} (xpr_rasterize_stats; roofline accounting).
+template <bool STATS>
 __global__ void __launch_bounds__(BLOCK)
 rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
-                     float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib) {
+                     float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
+                     unsigned long long* __restrict__ stats) {
     __shared__ float4 s_geo[BLOCK];   // mx, my, qa, qb
     __shared__ float4 s_gate[BLOCK];  // qc, thr = -lnv, o, unused
     __shared__ float4 s_col[BLOCK];   // r, g, b, unused
@@ -48,6 +52,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
     uint32_t last = 0;
     bool done = !inside;
+    uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
 
     for (uint32_t base = 0; base < len; base += BLOCK) {
         if (__syncthreads_count(done) == BLOCK) break;
@@ -67,8 +72,10 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                 const float4 ga = s_gate[j];
                 const float dx = pxc - ge.x, dy = pyc - ge.y;
                 const float power = eval_power(ge.z, ge.w, ga.x, dx, dy);
+                if (STATS) ++n_visit;
                 if (power > 0.0f) continue;       // valid = power <= 0 (L289, C20)
                 if (power < ga.y) continue;       // alpha < alpha_thresh (L679, C12)
+                if (STATS) ++n_pass;
                 const float og = ga.z * fast_exp(power);
                 const float alpha = fminf(P.amax, og);          // C11
                 const float Tn = T * (1.0f - alpha);
@@ -78,8 +85,14 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                 C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
                 T = Tn;
                 last = base + j + 1;
+                if (STATS) ++n_blend;
             }
         }
+    }
+    if (STATS) {
+        atomicAdd(stats + 0, (unsigned long long)n_visit); atomicAdd(stats + 1, (unsigned long long)n_pass);
+        atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)last);
+        return;
     }
     if (inside) {
         const int64_t pid = (int64_t)py * P.W + px;
@@ -217,9 +230,30 @@ extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cf
     RasterParams P;
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
-    rasterize_fwd_kernel<<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+    rasterize_fwd_kernel<false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
         P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib);
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                       const float* conic_opac, const float* rgb, const float* lnv,
+                                       const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats,
+                                       void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0 || !aligned(tile_ranges, 8) || !aligned(stats, 8)) return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+                  !aligned(vals_sorted, 4)))
+        return XPR_ERR_INVALID_ARG;
+    RasterParams P;
+    make_raster_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
+    rasterize_fwd_kernel<true><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr, nullptr, nullptr,
+        reinterpret_cast<unsigned long long*>(stats));
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }

@@ -1,0 +1,106 @@
+"""Helpers shared by the GPU parity tests: run the CUDA path (through the C-ABI binding) and the
+CPU oracle on the same seeded scene and compare stage by stage.  Test infrastructure only."""
+from __future__ import annotations
+
+import numpy as np
+
+import xpr_oracle as xo
+from paper_2606_11529_b200 import scenes
+
+IMG_TOL = 1e-4          # BASELINE.json:north_star: images within 1e-4 max abs in fp32
+GRAD_RTOL, GRAD_ATOL = 1e-3, 1e-6   # gradients within 1e-3 relative (plus 1e-6 absolute)
+FRAG_EXIT, FRAG_CLAMP, FRAG_GATE = 1, 2, 4   # xpr_oracle.h XO_FRAG_*
+
+
+def u32(t):
+    return t.detach().cpu().numpy().view(np.uint32)
+
+
+def run_gpu(scene, view=0, cfg_over=None, pair_capacity=None, dL=None):
+    import torch
+    from paper_2606_11529_b200 import pipeline
+    cfg = scenes.default_render_config(scene)
+    if cfg_over:
+        cfg.update(cfg_over)
+    cam = scene.cameras[view]
+    params = pipeline.scene_to_device(scene)
+    pipe = pipeline.SplatPipeline(scene.N, cam, cfg, pair_capacity=pair_capacity)
+    pipe.forward(*params)
+    torch.cuda.synchronize()
+    out = dict(pipe=pipe, params=params, cfg=cfg)
+    I = pipe.num_pairs
+    out["proj"] = dict(mean2d=pipe.mean2d.cpu().numpy(), conic_opac=pipe.conic_opac.cpu().numpy(),
+                       rgb=pipe.rgb.cpu().numpy(), depth=pipe.depth.cpu().numpy(), lnv=pipe.lnv.cpu().numpy(),
+                       tile_rect=pipe.tile_rect.cpu().numpy(), tile_count=u32(pipe.tile_count),
+                       flags=pipe.flags.cpu().numpy())
+    out["binned"] = dict(keys=pipe.keys_sorted[:I].cpu().numpy().view(np.uint64), vals=u32(pipe.vals_sorted[:I]),
+                         ranges=u32(pipe.tile_ranges), num_pairs=I)
+    out["fwd"] = dict(image=pipe.image.cpu().numpy(), final_T=pipe.final_T.cpu().numpy(), n_contrib=u32(pipe.n_contrib))
+    return out
+
+
+def run_gpu_backward(g, dL_np):
+    import torch
+    pipe = g["pipe"]
+    dL = torch.from_numpy(np.ascontiguousarray(dL_np, np.float32)).to(pipe.device)
+    pipe.backward(dL)
+    torch.cuda.synchronize()
+    names = ("g_mean2d", "g_conic", "g_opac", "g_rgb", "g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
+    return {k: getattr(pipe, k).cpu().numpy() for k in names}
+
+
+def run_oracle(scene, view=0, cfg_over=None, fragile_rel=2e-5):
+    cfg = scenes.default_render_config(scene)
+    if cfg_over:
+        cfg.update(cfg_over)
+    cam = xo.make_camera(scene.cameras[view])
+    ocfg = xo.make_config(cfg, fragile_rel=fragile_rel)
+    arrays = dict(means=scene.means, scales=scene.scales, quats=scene.quats, opacities=scene.opacities, sh=scene.sh)
+    r = xo.render(arrays, cam, ocfg, np.float32)
+    r.update(cam=cam, cfg=ocfg, arrays=arrays)
+    return r
+
+
+def compare_projection(g, o):
+    """Bit-exact on what feeds integers; returns the visible mask."""
+    gp, op = g["proj"], o["proj"]
+    np.testing.assert_array_equal(gp["tile_count"], op["tile_count"])
+    np.testing.assert_array_equal(gp["flags"], op["flags"])
+    vis = op["tile_count"] > 0
+    np.testing.assert_array_equal(gp["tile_rect"][vis], op["tile_rect"][vis])
+    np.testing.assert_array_equal(gp["depth"][vis].view(np.uint32), op["depth"][vis].view(np.uint32))
+    np.testing.assert_array_equal(gp["mean2d"][vis].view(np.uint32), op["mean2d"][vis].view(np.uint32))
+    np.testing.assert_array_equal(gp["conic_opac"][vis, :3].view(np.uint32), op["conic"][vis].view(np.uint32))
+    np.testing.assert_array_equal(gp["conic_opac"][vis, 3].view(np.uint32), op["opac_eff"][vis].view(np.uint32))
+    np.testing.assert_array_equal(gp["lnv"][vis].view(np.uint32), op["lnv"][vis].view(np.uint32))
+    np.testing.assert_array_equal(gp["rgb"][vis].view(np.uint32), op["rgb"][vis].view(np.uint32))
+    return vis
+
+
+def compare_binning(g, o):
+    gb, ob = g["binned"], o["binned"]
+    assert gb["num_pairs"] == ob["num_pairs"]
+    np.testing.assert_array_equal(gb["keys"], ob["keys"])
+    np.testing.assert_array_equal(gb["vals"], ob["vals"])
+    np.testing.assert_array_equal(gb["ranges"], ob["ranges"])
+
+
+def compare_forward(g, o):
+    """Image within 1e-4 max abs outside fragile pixels (exit decision within 2e-5 of t_min);
+    returns (n_fragile, max_err_all)."""
+    gf, of = g["fwd"], o["fwd"]
+    frag = (of["fragile"] & FRAG_EXIT) != 0
+    ok = ~frag
+    err = np.abs(gf["image"].astype(np.float64) - of["image"].astype(np.float64)).max(axis=2)
+    assert err[ok].max(initial=0.0) <= IMG_TOL, f"image max err {err[ok].max()}"
+    np.testing.assert_array_equal(gf["n_contrib"][ok], of["n_contrib"][ok])
+    dT = np.abs(gf["final_T"].astype(np.float64) - of["final_T"].astype(np.float64))
+    assert dT[ok].max(initial=0.0) <= 1e-5
+    return int(frag.sum()), float(err.max(initial=0.0))
+
+
+def grad_violations(got, ref):
+    got = np.asarray(got, np.float64).ravel()
+    ref = np.asarray(ref, np.float64).ravel()
+    bad = np.abs(got - ref) > GRAD_RTOL * np.abs(ref) + GRAD_ATOL
+    return bad, np.abs(got - ref)

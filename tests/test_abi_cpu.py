@@ -1,0 +1,111 @@
+"""CPU-only checks of the boundary: libxpr.so builds (nvcc cross-compiles sm_100a), loads, exports
+every symbol include/xpr.h declares, and rejects bad arguments before any launch (no GPU needed)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_11529_b200 import build, binding
+    build.build()
+    return binding.lib()
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "xpr.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(xpr_[a-z_]+)\s*\(", src)))
+
+
+def test_header_symbols_all_exported(lib):
+    from paper_2606_11529_b200 import binding
+    names = declared_symbols()
+    assert set(names) == set(binding.SYMBOLS), (names, binding.SYMBOLS)
+    for n in names:
+        assert hasattr(lib, n), n
+    for n in ("xpr_project", "xpr_bin_sort", "xpr_rasterize_fwd", "xpr_rasterize_bwd", "xpr_project_bwd"):
+        assert n in names   # BASELINE.json:north_star's five calls
+
+
+def test_struct_layout_matches_header():
+    from paper_2606_11529_b200 import binding
+    assert C.sizeof(binding.XprCamera) == 3 * 4 + 4 * 4 + 4 * 4 + 12 * 4
+    assert C.sizeof(binding.XprConfig) == 4 * 4 + 8 * 4 + 3 * 4
+
+
+def test_status_strings_and_version(lib):
+    assert lib.xpr_version() >= 100
+    for s in range(5):
+        assert lib.xpr_status_string(C.c_int32(s)).decode().startswith("XPR_")
+
+
+def _cam_cfg(**over):
+    from paper_2606_11529_b200 import binding, scenes
+    sc = scenes.make_scene(1, n_override=8)
+    d = scenes.default_render_config(sc)
+    d.update(over)
+    return binding.make_camera(sc.cameras[0]), binding.make_config(d)
+
+
+def test_invalid_arguments_rejected_before_launch(lib):
+    from paper_2606_11529_b200 import binding as xb
+    cam, cfg = _cam_cfg()
+    null = C.c_void_p(0)
+    # NULL pointers with N > 0
+    st = lib.xpr_project(C.c_int64(4), null, null, null, null, null, C.byref(cam), C.byref(cfg), null, null, null,
+                         null, null, null, null, null, null)
+    assert st == xb.XPR_ERR_INVALID_ARG
+    # negative N
+    st = lib.xpr_project(C.c_int64(-1), null, null, null, null, null, C.byref(cam), C.byref(cfg), null, null, null,
+                         null, null, null, null, null, null)
+    assert st == xb.XPR_ERR_INVALID_ARG
+    # tile != 16 and sh_degree > 3 are unsupported
+    cam2, cfg2 = _cam_cfg(tile=8)
+    st = lib.xpr_project(C.c_int64(0), null, null, null, null, null, C.byref(cam2), C.byref(cfg2), null, null, null,
+                         null, null, null, null, null, null)
+    assert st == xb.XPR_ERR_UNSUPPORTED
+    cam3, cfg3 = _cam_cfg(sh_degree=4)
+    st = lib.xpr_rasterize_fwd(C.byref(cam3), C.byref(cfg3), C.c_int64(0), null, null, null, null, null, null, null,
+                               null, null, null)
+    assert st == xb.XPR_ERR_UNSUPPORTED
+    # bad enum
+    cam4, cfg4 = _cam_cfg(projection=7)
+    st = lib.xpr_project_bwd(C.c_int64(0), null, null, null, null, null, C.byref(cam4), C.byref(cfg4), null, null,
+                             null, null, null, null, null, null, null, null, null, null)
+    assert st == xb.XPR_ERR_INVALID_ARG
+    # misaligned workspace
+    n = C.c_int64(0)
+    st = lib.xpr_bin_sort(C.c_int64(0), null, null, null, C.byref(cam), C.byref(cfg), C.c_int64(0), null, null,
+                          C.c_void_p(8), C.byref(n), C.c_void_p(100), C.c_size_t(1 << 20), null)
+    assert st == xb.XPR_ERR_INVALID_ARG
+
+
+def test_workspace_size_monotone(lib):
+    from paper_2606_11529_b200 import binding as xb
+    a = xb.xpr_bin_sort_workspace(1000, 10_000, 16)
+    b = xb.xpr_bin_sort_workspace(1000, 1_000_000, 8160)
+    assert 0 < a < b
+    assert b >= 12 * 1_000_000       # double buffer for keys (8 B) and values (4 B)
+    with pytest.raises(xb.XprError):
+        xb.xpr_bin_sort_workspace(1000, 1 << 30, 16)
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+    from paper_2606_11529_b200 import binding as xb
+    with pytest.raises(TypeError):
+        xb._p(torch.zeros(4))
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_11529_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "xpr_oracle" not in txt and "import oracle" not in txt, f

@@ -1,0 +1,102 @@
+"""GPU edge cases of the hot path: empty input, everything culled, capacity overflow and regrowth,
+a full-screen Gaussian, exact depth ties (stable order), huge pair counts per Gaussian."""
+import numpy as np
+import pytest
+
+import parity_util as pu
+import xpr_oracle as xo
+from paper_2606_11529_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+
+def _subset(sc, idx):
+    sc.means, sc.scales, sc.quats = sc.means[idx].copy(), sc.scales[idx].copy(), sc.quats[idx].copy()
+    sc.opacities, sc.sh = sc.opacities[idx].copy(), sc.sh[idx].copy()
+    return sc
+
+
+def test_empty_scene_renders_background():
+    import torch
+    from paper_2606_11529_b200 import pipeline
+    sc = _subset(scenes.make_scene(1), np.arange(0))
+    cfg = scenes.default_render_config(sc)
+    cfg["bg"] = (0.1, 0.2, 0.3)
+    pipe = pipeline.SplatPipeline(0, sc.cameras[0], cfg)
+    img = pipe.forward(*pipeline.scene_to_device(sc))
+    torch.cuda.synchronize()
+    assert pipe.num_pairs == 0
+    np.testing.assert_allclose(img.cpu().numpy(), np.broadcast_to(np.float32([0.1, 0.2, 0.3]), (64, 64, 3)))
+    assert (pipe.final_T.cpu().numpy() == 1).all() and (pipe.n_contrib.cpu().numpy() == 0).all()
+
+
+def test_everything_culled_behind_camera():
+    sc = scenes.make_scene(1, n_override=500)
+    sc.means[:, 2] -= 10.0          # all behind the camera at z = -4 looking +z
+    g = pu.run_gpu(sc)
+    o = pu.run_oracle(sc)
+    assert o["binned"]["num_pairs"] == 0 and g["binned"]["num_pairs"] == 0
+    assert (g["proj"]["tile_count"] == 0).all() and (g["proj"]["flags"] == 0).all()
+    assert (g["fwd"]["image"] == 0).all() and (g["binned"]["ranges"] == 0).all()
+    gg = pu.run_gpu_backward(g, np.ones((64, 64, 3), np.float32))
+    for k, v in gg.items():
+        assert not np.any(v), k
+
+
+def test_capacity_error_reports_required_pairs_then_regrows():
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline
+    sc = scenes.make_scene(1)
+    o = pu.run_oracle(sc)
+    I = o["binned"]["num_pairs"]
+    cfg = scenes.default_render_config(sc)
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg, pair_capacity=100)
+    pipe.project(*pipeline.scene_to_device(sc))
+    guard = torch.full((pipe.keys_sorted.numel(),), -7, dtype=torch.int64, device="cuda")
+    st, need = xb.xpr_bin_sort(pipe.depth, pipe.tile_rect, pipe.tile_count, pipe.cam, pipe.cfg, 50, guard,
+                               pipe.vals_sorted, pipe.tile_ranges, pipe.workspace, raise_on_capacity=False)
+    torch.cuda.synchronize()
+    assert st == xb.XPR_ERR_CAPACITY and need == I
+    assert (guard[50:] == -7).all()          # nothing written beyond the stated capacity
+    with pytest.raises(xb.XprError):
+        xb.xpr_bin_sort(pipe.depth, pipe.tile_rect, pipe.tile_count, pipe.cam, pipe.cfg, 50, guard,
+                        pipe.vals_sorted, pipe.tile_ranges, pipe.workspace)
+    assert pipe.bin_sort() == I and pipe.pair_capacity >= I     # pipeline regrows and redoes
+    np.testing.assert_array_equal(pu.u32(pipe.vals_sorted[:I]), o["binned"]["vals"])
+
+
+def test_fullscreen_gaussian_and_depth_ties():
+    """One Gaussian covering every tile plus exact duplicates (equal keys): the stable order of equal
+    keys is ascending Gaussian index (C10), so sorted values must match bit-exactly."""
+    sc = scenes.make_scene(2, n_override=4000, image_override=(320, 240))
+    sc.means[0] = (0.0, 0.0, 0.0)
+    sc.scales[0] = (5.0, 5.0, 5.0)       # covers the whole image
+    sc.opacities[0] = 0.9
+    for dup in range(1, 40):             # 39 exact copies of Gaussian 100 scattered over the index range
+        j = 100 * dup
+        sc.means[j], sc.scales[j], sc.quats[j] = sc.means[100], sc.scales[100] * 3, sc.quats[100]
+    g = pu.run_gpu(sc)
+    o = pu.run_oracle(sc)
+    TW, TH = 20, 15
+    assert o["proj"]["tile_count"][0] == TW * TH
+    pu.compare_projection(g, o)
+    pu.compare_binning(g, o)
+    keys = o["binned"]["keys"]
+    assert (np.diff(keys.astype(np.int64)) == 0).sum() >= 38       # the ties are really there
+    pu.compare_forward(g, o)
+
+
+def test_many_sort_tiles_and_all_digit_passes():
+    """> 100 onesweep tiles (4096 pairs each) so that the decoupled look-back chains are exercised,
+    and a 1920x1080 tile grid so that all six 8-bit digit passes carry information."""
+    sc = scenes.make_scene(5, n_override=40000)
+    g = pu.run_gpu(sc)
+    o = pu.run_oracle(sc)
+    assert o["binned"]["num_pairs"] > 100 * 4096
+    pu.compare_projection(g, o)
+    pu.compare_binning(g, o)
+    keys = g["binned"]["keys"]
+    assert (keys[1:] >= keys[:-1]).all()
+    r = g["binned"]["ranges"].astype(np.int64)
+    nz = r[:, 1] > r[:, 0]
+    assert (r[nz, 1] - r[nz, 0]).sum() == o["binned"]["num_pairs"]     # ranges partition [0, I)
