@@ -97,12 +97,12 @@ def oracle_step(xo, scenes, sc, view, np):
 
 
 def oracle_sample(args):
-    """Bounded sample of the bench workload for the CPU legs: same scene and Gaussian count, image at
-    1/4 linear resolution (same field of view), so that a step is ~10-30 s of CPU work."""
+    """Bounded sample of the bench workload for the CPU legs, sized so that a step is seconds of CPU
+    work: the full workload for configs 1-4; for config 5 the same scene at 1/4 linear resolution."""
     from paper_2606_11529_b200 import scenes
     full = scenes.make_scene(args.config)
     W, H = full.cameras[0].width, full.cameras[0].height
-    if args.config >= 3:
+    if args.config >= 5:
         w, h = W // 4, H // 4
         sc = scenes.make_scene(args.config, image_override=(w, h))
         desc = f"same scene, all {sc.N} Gaussians, view {args.view}, {w}x{h} image (1/4 linear resolution, same FOV), 1 step"

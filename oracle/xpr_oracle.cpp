@@ -452,7 +452,10 @@ void rasterize_fwd_strict(const xo_camera* cam, const xo_config* cfg, int64_t N,
 //   dL/dA = -1/2 dx^2 dL/dpower, dL/dB = -dx dy dL/dpower, dL/dC = -1/2 dy^2 dL/dpower,
 //   dL/dm_x = (A dx + B dy) dL/dpower, dL/dm_y = (B dx + C dy) dL/dpower.
 // Gates and the exit are piecewise constant (C15).
-template <class S>
+// MASS = true accumulates |addend| instead of the addend: the "mass" sum_pixels |term| of every
+// gradient element, i.e. the scale an fp32 sum of those terms is conditioned on (used only to
+// derive the cancellation-aware part of the gradient tolerance).
+template <class S, bool MASS = false>
 void rasterize_bwd(const xo_camera* cam, const xo_config* cfg, int64_t N, const S* mean2d, const S* conic, const S* opac,
                    const S* rgb, const S* lnv, const uint32_t* vals, const uint32_t* ranges, const uint32_t* n_contrib,
                    const S* dL, double* g_mean2d, double* g_conic, double* g_opac, double* g_rgb) {
@@ -483,7 +486,7 @@ void rasterize_bwd(const xo_camera* cam, const xo_config* cfg, int64_t N, const 
                     double dalpha = 0.0;
                     for (int ch = 0; ch < 3; ++ch) {
                         const double ck = (double)rgb[3 * q.g + ch];
-                        a9[6 + ch] += al * Tk * g[ch];
+                        a9[6 + ch] += MASS ? std::fabs(al * Tk * g[ch]) : al * Tk * g[ch];
                         dalpha += g[ch] * (ck * Tk - Sb[ch] / (1.0 - al));
                     }
                     for (int ch = 0; ch < 3; ++ch) Sb[ch] += (double)rgb[3 * q.g + ch] * al * Tk;
@@ -492,10 +495,9 @@ void rasterize_bwd(const xo_camera* cam, const xo_config* cfg, int64_t N, const 
                     const double dpow = o * G * dalpha;
                     const double A = (double)conic[3 * q.g], B = (double)conic[3 * q.g + 1], C = (double)conic[3 * q.g + 2];
                     const double dx = (double)q.dx, dy = (double)q.dy;
-                    a9[5] += G * dalpha;
-                    a9[2] += -0.5 * dx * dx * dpow; a9[3] += -dx * dy * dpow; a9[4] += -0.5 * dy * dy * dpow;
-                    // d power / d m_x = -d power / d dx = A dx + B dy
-                    a9[0] += (A * dx + B * dy) * dpow; a9[1] += (B * dx + C * dy) * dpow;
+                    const double add[6] = {(A * dx + B * dy) * dpow, (B * dx + C * dy) * dpow,   // d power / d m = A dx + B dy, ..
+                                           -0.5 * dx * dx * dpow, -dx * dy * dpow, -0.5 * dy * dy * dpow, G * dalpha};
+                    for (int j = 0; j < 6; ++j) a9[j] += MASS ? std::fabs(add[j]) : add[j];
                 }
             }
         for (uint32_t k = 0; k < e - b; ++k) {
@@ -691,6 +693,14 @@ inline uint32_t float_bits(float f) { uint32_t u; std::memcpy(&u, &f, 4); return
         double* g_rgb) {                                                                                            \
         rasterize_bwd<T>(cam, cfg, N, mean2d, conic, opac_eff, rgb, lnv, vals_sorted, tile_ranges, n_contrib,       \
                          dL_dimage, g_mean2d, g_conic, g_opac_eff, g_rgb);                                          \
+    }                                                                                                               \
+    extern "C" void xpr_oracle_rasterize_bwd_mass_##SFX(                                                            \
+        const xo_camera* cam, const xo_config* cfg, int64_t N, const T* mean2d, const T* conic, const T* opac_eff,  \
+        const T* rgb, const T* lnv, const uint32_t* vals_sorted, const uint32_t* tile_ranges,                       \
+        const uint32_t* n_contrib, const T* dL_dimage, double* g_mean2d, double* g_conic, double* g_opac_eff,       \
+        double* g_rgb) {                                                                                            \
+        rasterize_bwd<T, true>(cam, cfg, N, mean2d, conic, opac_eff, rgb, lnv, vals_sorted, tile_ranges, n_contrib, \
+                               dL_dimage, g_mean2d, g_conic, g_opac_eff, g_rgb);                                    \
     }                                                                                                               \
     extern "C" void xpr_oracle_project_bwd_##SFX(                                                                   \
         int64_t N, const T* means, const T* scales, const T* quats, const T* opacities, const T* sh,                \

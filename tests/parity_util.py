@@ -99,8 +99,15 @@ def compare_forward(g, o):
     return int(frag.sum()), float(err.max(initial=0.0))
 
 
-def grad_violations(got, ref):
+GRAD_KAPPA = 2e-6   # 32 fp32 ulps of the element's mass sum|term| (fp32 summation floor)
+
+
+def grad_violations(got, ref, mass=None):
+    """|got - ref| <= 1e-3 |ref| + 1e-6 (+ GRAD_KAPPA * mass when the oracle's mass is given)."""
     got = np.asarray(got, np.float64).ravel()
     ref = np.asarray(ref, np.float64).ravel()
-    bad = np.abs(got - ref) > GRAD_RTOL * np.abs(ref) + GRAD_ATOL
+    tol = GRAD_RTOL * np.abs(ref) + GRAD_ATOL
+    if mass is not None:
+        tol = tol + GRAD_KAPPA * np.asarray(mass, np.float64).ravel()
+    bad = np.abs(got - ref) > tol
     return bad, np.abs(got - ref)

@@ -189,3 +189,25 @@ def test_p11_linearity_and_exact_zero_for_culled():
     b64 = xo.backward(arr, r, G1 * mask, cam, cfg, np.float64)
     for k in ("g_means", "g_sh", "g_opacities"):
         np.testing.assert_allclose(b32[k], b64[k], rtol=2e-2, atol=2e-3 * np.abs(b64[k]).max())
+
+
+def test_gradient_mass_bounds_gradient_and_equals_it_for_sign_definite_terms():
+    """The mass output (sum over pixels of |term|, used only as the scale of the fp32 summation
+    tolerance) must dominate |gradient| element-wise, and for g_rgb with dL >= 0 every term
+    alpha T g is non-negative, so mass == gradient there (c = sum c_i alpha_i T_i)."""
+    sc = scenes.make_scene(1, n_override=300)
+    cam = xo.make_camera(sc.cameras[0])
+    cfg = xo.make_config(scenes.default_render_config(sc))
+    arrays = dict(means=sc.means, scales=sc.scales, quats=sc.quats, opacities=sc.opacities, sh=sc.sh)
+    r = xo.render(arrays, cam, cfg, np.float64)
+    rng = np.random.default_rng(5)
+    dL = rng.standard_normal((64, 64, 3))
+    g = xo.rasterize_bwd(r["proj"], r["binned"], r["fwd"], dL, cam, cfg, np.float64)
+    m = xo.rasterize_bwd(r["proj"], r["binned"], r["fwd"], dL, cam, cfg, np.float64, mass=True)
+    for k in ("g_mean2d", "g_conic", "g_opac_eff", "g_rgb"):
+        assert (m[k] >= np.abs(g[k]) * (1 - 1e-12) - 1e-300).all(), k
+        assert (m[k] > np.abs(g[k]) * 1.01).any(), k          # cancellation really occurs
+    gp = xo.rasterize_bwd(r["proj"], r["binned"], r["fwd"], np.abs(dL), cam, cfg, np.float64)
+    mp = xo.rasterize_bwd(r["proj"], r["binned"], r["fwd"], np.abs(dL), cam, cfg, np.float64, mass=True)
+    np.testing.assert_allclose(mp["g_rgb"], gp["g_rgb"], rtol=1e-13, atol=0)
+    np.testing.assert_allclose(m["g_rgb"], gp["g_rgb"], rtol=1e-13, atol=0)   # mass depends on |dL| only
