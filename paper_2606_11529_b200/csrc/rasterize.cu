@@ -110,54 +110,96 @@ __device__ __forceinline__ float warp_sum(float v) {
     return v;
 }
 
-__global__ void __launch_bounds__(BLOCK)
+// Transposed butterfly: reduces 8 per-lane values across the warp with 9 shuffles (4+2+1+1+1)
+// instead of 40.  On return lane L with (L & 3) == 0 holds the warp total of value (L >> 2).
+__device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
+    float w[4], x[2];
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float send = b4 ? v[i] : v[i + 4], keep = b4 ? v[i + 4] : v[i];
+        w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const float send = b3 ? w[i] : w[i + 2], keep = b3 ? w[i + 2] : w[i];
+        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    const float send = b2 ? x[0] : x[1], keep = b2 ? x[1] : x[0];
+    float y = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    y += __shfl_xor_sync(0xffffffffu, y, 2);
+    y += __shfl_xor_sync(0xffffffffu, y, 1);
+    return y;
+}
+
+// Backward compositing (a9).  One CTA of 64 threads per 16x16 tile, 4 pixels per thread (rows
+// 4q..4q+3 of one column), so that a Gaussian's record is read from shared memory once per 4
+// pixel-pairs and the per-Gaussian reduction runs once per 128 pixel-pairs: each lane first sums
+// its own pixels in registers, then one transposed butterfly (14 shuffles for the 9 gradients)
+// leaves the totals spread over lanes, which issue two RED instructions (8 lanes + 1 lane).
+constexpr int BWD_THREADS = 64, BWD_PPT = 4, BWD_BATCH = 64;
+
+__global__ void __launch_bounds__(BWD_THREADS)
 rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                      const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                      const float* __restrict__ dL, float* __restrict__ g_mean2d, float* __restrict__ g_conic,
                      float* __restrict__ g_opac, float* __restrict__ g_rgb) {
-    __shared__ float4 s_geo[BLOCK];   // mx, my, A, B
-    __shared__ float4 s_gate[BLOCK];  // C, thr, o, unused
-    __shared__ float4 s_col[BLOCK];   // r, g, b, index (bits)
-    __shared__ uint32_t s_max[BLOCK / 32];
+    __shared__ float4 s_geo[BWD_BATCH];   // mx, my, A, B
+    __shared__ float4 s_gate[BWD_BATCH];  // C, thr, o, index (bits)
+    __shared__ float4 s_col[BWD_BATCH];   // r, g, b, unused
+    __shared__ uint32_t s_max[BWD_THREADS / 32];
     const int tile = blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
-    const int px = tx * TILE + (threadIdx.x & (TILE - 1)), py = ty * TILE + (threadIdx.x >> 4);
-    const bool inside = (px < P.W) && (py < P.H);
-    const float pxc = (float)px + 0.5f, pyc = (float)py + 0.5f;
-    const uint2 rg = ranges[tile];
     const int lane = threadIdx.x & 31;
+    const int px = tx * TILE + (threadIdx.x & (TILE - 1));
+    const int py0 = ty * TILE + (threadIdx.x >> 4) * BWD_PPT;
+    const float pxc = (float)px + 0.5f;
+    const uint2 rg = ranges[tile];
 
-    uint32_t n = 0;
-    float T = 0.0f, g0 = 0.0f, g1 = 0.0f, g2 = 0.0f;
-    if (inside) {
-        const int64_t pid = (int64_t)py * P.W + px;
-        n = n_contrib[pid];
-        T = final_T[pid];
-        g0 = dL[3 * pid]; g1 = dL[3 * pid + 1]; g2 = dL[3 * pid + 2];
+    uint32_t n[BWD_PPT];
+    float T[BWD_PPT], S0[BWD_PPT], S1[BWD_PPT], S2[BWD_PPT], g0[BWD_PPT], g1[BWD_PPT], g2[BWD_PPT], pyc[BWD_PPT];
+    uint32_t wmax = 0;
+#pragma unroll
+    for (int k = 0; k < BWD_PPT; ++k) {
+        const int py = py0 + k;
+        pyc[k] = (float)py + 0.5f;
+        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = 0.0f;
+        if (px < P.W && py < P.H) {
+            const int64_t pid = (int64_t)py * P.W + px;
+            n[k] = n_contrib[pid];
+            T[k] = final_T[pid];
+            g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
+        }
+        // colour behind the current entry, S_k = sum_{j>k} c_j alpha_j T_j + T_final bg (C13)
+        S0[k] = T[k] * P.bg[0]; S1[k] = T[k] * P.bg[1]; S2[k] = T[k] * P.bg[2];
+        wmax = max(wmax, n[k]);
     }
-    // colour behind the current entry, S_k = sum_{j>k} c_j alpha_j T_j + T_final bg (C13)
-    float S0 = T * P.bg[0], S1 = T * P.bg[1], S2 = T * P.bg[2];
-    uint32_t wmax = n;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
     if (lane == 0) s_max[threadIdx.x >> 5] = wmax;
     __syncthreads();
     uint32_t max_n = 0;
 #pragma unroll
-    for (int w = 0; w < BLOCK / 32; ++w) max_n = max(max_n, s_max[w]);
+    for (int w = 0; w < BWD_THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
+
+    // lane (4 i) owns gradient i of the 8-value butterfly: its base pointer and per-Gaussian stride
+    const int vi = lane >> 2;
+    float* const red_base = (vi < 2) ? (g_mean2d + vi) : (vi < 5) ? (g_conic + (vi - 2)) : (g_rgb + (vi - 5));
+    const uint32_t red_stride = (vi < 2) ? 2u : 3u;
+    const bool red_lane = (lane & 3) == 0;
 
     for (uint32_t hi = max_n; hi > 0;) {
-        const uint32_t cnt = min((uint32_t)BLOCK, hi);
+        const uint32_t cnt = min((uint32_t)BWD_BATCH, hi);
         __syncthreads();
         if (threadIdx.x < cnt) {      // slot j holds list position hi-1-j (descending)
             const uint32_t g = vals[rg.x + hi - 1 - threadIdx.x];
             const float2 m = mean2d[g];
             const float4 co = conic_opac[g];
             s_geo[threadIdx.x] = make_float4(m.x, m.y, co.x, co.y);
-            s_gate[threadIdx.x] = make_float4(co.z, -lnv[g], co.w, 0.0f);
-            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], __uint_as_float(g));
+            s_gate[threadIdx.x] = make_float4(co.z, -lnv[g], co.w, __uint_as_float(g));
+            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
         }
         __syncthreads();
         for (uint32_t j = 0; j < cnt; ++j) {
@@ -165,40 +207,49 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             if (pos >= wmax) continue;     // warp-uniform: nobody in this warp got this far
             const float4 ge = s_geo[j];
             const float4 ga = s_gate[j];
-            const float dx = pxc - ge.x, dy = pyc - ge.y;
             const float A = ge.z, Bc = ge.w, Cc = ga.x;
-            const float power = eval_power(-0.5f * A, -Bc, -0.5f * Cc, dx, dy);
-            const bool contrib = (pos < n) && !(power > 0.0f) && !(power < ga.y);
-            if (!__any_sync(0xffffffffu, contrib)) continue;
-            float v_mx = 0.f, v_my = 0.f, v_A = 0.f, v_B = 0.f, v_C = 0.f, v_o = 0.f, v_r = 0.f, v_g = 0.f, v_b = 0.f;
+            const float qa = -0.5f * A, qb = -Bc, qc = -0.5f * Cc;
+            const float dx = pxc - ge.x;
+            float dy[BWD_PPT], power[BWD_PPT];
+            bool contrib[BWD_PPT], any_c = false;
+#pragma unroll
+            for (int k = 0; k < BWD_PPT; ++k) {
+                dy[k] = pyc[k] - ge.y;
+                power[k] = eval_power(qa, qb, qc, dx, dy[k]);
+                contrib[k] = (pos < n[k]) && !(power[k] > 0.0f) && !(power[k] < ga.y);
+                any_c |= contrib[k];
+            }
+            if (!__any_sync(0xffffffffu, any_c)) continue;
             const float4 c = s_col[j];
-            if (contrib) {
-                const float G = fast_exp(power);
-                const float og = ga.z * G;
-                const float alpha = fminf(P.amax, og);
-                const float oma = 1.0f - alpha;
-                const float inv = 1.0f / oma;
-                T = T * inv;                       // transmittance in front of this entry
-                const float w = alpha * T;
-                v_r = w * g0; v_g = w * g1; v_b = w * g2;
-                const float dalpha = g0 * (c.x * T - S0 * inv) + g1 * (c.y * T - S1 * inv) + g2 * (c.z * T - S2 * inv);
-                S0 = fmaf(c.x, w, S0); S1 = fmaf(c.y, w, S1); S2 = fmaf(c.z, w, S2);
-                if (og < P.amax) {                 // C14: the clamp has zero derivative
-                    const float dpow = og * dalpha;
-                    v_o = G * dalpha;
-                    v_A = -0.5f * dx * dx * dpow; v_B = -dx * dy * dpow; v_C = -0.5f * dy * dy * dpow;
-                    v_mx = (A * dx + Bc * dy) * dpow; v_my = (Bc * dx + Cc * dy) * dpow;
+            float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // mx my A B C r g b
+            float v_o = 0.f;
+#pragma unroll
+            for (int k = 0; k < BWD_PPT; ++k) {
+                if (contrib[k]) {
+                    const float G = fast_exp(power[k]);
+                    const float og = ga.z * G;
+                    const float alpha = fminf(P.amax, og);
+                    const float inv = 1.0f / (1.0f - alpha);
+                    T[k] = T[k] * inv;                 // transmittance in front of this entry
+                    const float w = alpha * T[k];
+                    v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
+                    const float dalpha = g0[k] * (c.x * T[k] - S0[k] * inv) + g1[k] * (c.y * T[k] - S1[k] * inv) +
+                                         g2[k] * (c.z * T[k] - S2[k] * inv);
+                    S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
+                    if (og < P.amax) {                 // C14: the clamp has zero derivative
+                        const float dpow = og * dalpha;
+                        v_o = fmaf(G, dalpha, v_o);
+                        const float dxp = dx * dpow, dyp = dy[k] * dpow;
+                        v[2] = fmaf(-0.5f * dx, dxp, v[2]); v[3] = fmaf(-dx, dyp, v[3]); v[4] = fmaf(-0.5f * dy[k], dyp, v[4]);
+                        v[0] = fmaf(A, dxp, fmaf(Bc, dyp, v[0])); v[1] = fmaf(Bc, dxp, fmaf(Cc, dyp, v[1]));
+                    }
                 }
             }
-            v_mx = warp_sum(v_mx); v_my = warp_sum(v_my); v_A = warp_sum(v_A); v_B = warp_sum(v_B);
-            v_C = warp_sum(v_C); v_o = warp_sum(v_o); v_r = warp_sum(v_r); v_g = warp_sum(v_g); v_b = warp_sum(v_b);
-            if (lane == 0) {
-                const uint32_t g = __float_as_uint(c.w);
-                atomicAdd(g_mean2d + 2 * g, v_mx); atomicAdd(g_mean2d + 2 * g + 1, v_my);
-                atomicAdd(g_conic + 3 * g, v_A); atomicAdd(g_conic + 3 * g + 1, v_B); atomicAdd(g_conic + 3 * g + 2, v_C);
-                atomicAdd(g_opac + g, v_o);
-                atomicAdd(g_rgb + 3 * g, v_r); atomicAdd(g_rgb + 3 * g + 1, v_g); atomicAdd(g_rgb + 3 * g + 2, v_b);
-            }
+            const float tot = warp_reduce8(v, lane);
+            v_o = warp_sum(v_o);
+            const uint32_t g = __float_as_uint(ga.w);
+            if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
+            if (lane == 0) atomicAdd(g_opac + g, v_o);
         }
         hi -= cnt;
     }
@@ -282,7 +333,7 @@ extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cf
     RasterParams P;
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
-    rasterize_bwd_kernel<<<T, BLOCK, 0, st>>>(
+    rasterize_bwd_kernel<<<T, BWD_THREADS, 0, st>>>(
         P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
         vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_mean2d, g_conic,
         g_opac, g_rgb);
