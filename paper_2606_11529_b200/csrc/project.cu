@@ -354,8 +354,11 @@ __device__ __forceinline__ void store_sh_grad(float* __restrict__ g_sh, int64_t 
     }
 }
 
+#ifndef XPR_PBWD_MINB
+#define XPR_PBWD_MINB 4
+#endif
 template <int K>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, XPR_PBWD_MINB)
 project_bwd_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const float* __restrict__ scales,
                    const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
                    const uint32_t* __restrict__ tcount, const uint8_t* __restrict__ flags,
