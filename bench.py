@@ -207,7 +207,7 @@ def run_ours(args):
     # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
     bits = max(1, (pipe.T - 1).bit_length()) if pipe.T > 1 else 0
     passes = (32 + bits + 7) // 8
-    launches_per_step = 1 + 1 + passes + 1 + 1 + 1 + 1
+    launches_per_step = 1 + (1 + 4 + 2 + (passes - 4) + 1) + 1 + 1 + 1   # project, bin_sort(compact, 4 depth passes, emit, tile passes, ranges), fwd, bwd, project_bwd
 
     sampler = ClockSampler(local)
     sampler.start()
