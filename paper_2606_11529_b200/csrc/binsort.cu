@@ -420,10 +420,10 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
         const uint32_t* p = my - RADIX;
         uint32_t remaining = tile;
         bool found = false;
-        {   // first round: 4 predecessors in flight (in steady state the nearest one is already inclusive)
+        while (!found) {   // 4 predecessors in flight per round; before tile 0: virtual inclusive 0
             uint32_t sv[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k)    // before tile 0: virtual inclusive 0
+            for (int k = 0; k < 4; ++k)
                 sv[k] = ((uint32_t)k < remaining) ? ld_relaxed(p - k * RADIX) : FLAG_INCLUSIVE;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
@@ -434,21 +434,6 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
             }
             p -= 4 * RADIX;
             remaining = (remaining > 4u) ? remaining - 4u : 0u;
-        }
-        while (!found) {   // first wave of CTAs: long runs of partial predecessors -> 16 in flight
-            uint32_t sv[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k)
-                sv[k] = ((uint32_t)k < remaining) ? ld_relaxed(p - k * RADIX) : FLAG_INCLUSIVE;
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                if (found) break;
-                while ((sv[k] & FLAG_MASK) == 0u) sv[k] = ld_relaxed(p - k * RADIX);
-                excl_prev += sv[k] & VALUE_MASK;
-                found = (sv[k] & FLAG_MASK) == FLAG_INCLUSIVE;
-            }
-            p -= 16 * RADIX;
-            remaining = (remaining > 16u) ? remaining - 16u : 0u;
         }
         st_relaxed(my, FLAG_INCLUSIVE | (excl_prev + real_count));
     }
