@@ -84,6 +84,28 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def rank_env():
+    """(world, rank, local_rank) from the torchrun environment; (1, 0, 0) when launched plainly."""
+    return (int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def max_over_ranks(value_ms: float, world: int, device):
+    """Replicas only: the job's time is the slowest rank's.  One all-reduce(MAX) of a scalar."""
+    if world <= 1:
+        return float(value_ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value_ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world: int, megapixels: float, ms_per_step: float) -> float:
+    """Whole-job MP/s of `world` replicas that each render `megapixels` per step in `ms_per_step` (max over ranks)."""
+    return world * megapixels / (ms_per_step / 1e3)
+
+
 def oracle_step(xo, scenes, sc, view, np):
     """One fwd+bwd step of the CPU oracle, as it stands (never tuned)."""
     cam = xo.make_camera(sc.cameras[view])
@@ -114,8 +136,7 @@ def oracle_sample(args):
 
 def run_reference(args):
     """--impl reference: the oracle on the host cores (this tier's reference arm)."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    if rank_env()[1] != 0:
         return
     import numpy as np
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
@@ -154,9 +175,7 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_2606_11529_b200 import binding as xb, pipeline, scenes
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local = rank_env()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py --impl ours needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
@@ -206,8 +225,11 @@ def run_ours(args):
     n_pairs = pipe.num_pairs
     # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
     bits = max(1, (pipe.T - 1).bit_length()) if pipe.T > 1 else 0
-    passes = (32 + bits + 7) // 8
-    launches_per_step = 1 + (1 + 4 + 2 + (passes - 4) + 1) + 1 + 1 + 1   # project, bin_sort(compact, 4 depth passes, emit, tile passes, ranges), fwd, bwd, project_bwd
+    tile_passes = (bits + 7) // 8
+    passes = 4 + tile_passes              # 8-bit digits: 4 on the depth bits (run on Gaussians) + tile digits (on pairs)
+    # project, bin_sort (compact, 4 depth passes, offsets, emit, tile passes, ranges), fwd, bwd, project_bwd
+    launches_per_step = 1 + (1 + 4 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1
+    n_vis = int(torch.count_nonzero(pipe.tile_count).item())
 
     sampler = ClockSampler(local)
     sampler.start()
@@ -221,15 +243,11 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop()
     step_ms = [e[0].elapsed_time(e[-1]) for e in all_events]
-    total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(float(sum(step_ms)), world, dev)
     ms = total_ms / args.steps
     stage_ms = {n: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in all_events])) for i, n in enumerate(stage_names)}
     mp = cam.width * cam.height / 1e6
-    value = world * mp / (ms / 1e3)
+    value = aggregate_value(world, mp, ms)
 
     # roofline of the dominant kernel (largest stage): pixel-pair counts from xpr_rasterize_stats
     stats = torch.zeros(4, dtype=torch.int64, device=dev)
@@ -254,8 +272,11 @@ def run_ours(args):
         roof = {"kernel": "rasterize_fwd_kernel", "bound": "alu", "achieved": ops / (stage_ms[dom] / 1e3) / 1e12,
                 "peak": alu_peak, "unit": "T lane-op/s"}
     else:
-        nbytes = n_pairs * (12 + 24 * passes + 8) + 24 * sc.N
-        roof = {"kernel": "bin_sort (emit + onesweep passes + ranges)", "bound": "hbm",
+        # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + per pair
+        # 12 B emitted, 24 B per tile-digit pass, 8 B read by ranges
+        nbytes = 8 * sc.N + 4 * 16 * n_vis + n_pairs * (12 + 24 * tile_passes + 8)
+        roof = {"kernel": "xpr_bin_sort (compact, 4 depth passes, offsets, emit, %d tile passes, ranges)" % tile_passes,
+                "bound": "hbm",
                 "achieved": nbytes / (stage_ms[dom] / 1e3) / 1e9, "peak": hbm_peak, "unit": "GB/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["traffic"] = None
@@ -290,11 +311,8 @@ def run_ours(args):
             a = _rec(); e2e_step(); b = _rec()
             torch.cuda.synchronize()
             t_ms += a.elapsed_time(b)
-        if world > 1:
-            t = torch.tensor([t_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_ms = float(t.item())
-        e2e = {"value": world * mp / (t_ms / k / 1e3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        t_ms = max_over_ranks(t_ms, world, dev)
+        e2e = {"value": aggregate_value(world, mp, t_ms / k), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "ms_per_step": t_ms / k}
 
     cpu = None
@@ -311,7 +329,8 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "pairs": n_pairs, "sort_passes": passes,
+                           "image": [cam.width, cam.height], "pairs": n_pairs, "visible_gaussians": n_vis,
+                           "sort_passes": {"depth_digits_on_gaussians": 4, "tile_digits_on_pairs": tile_passes},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},
                 "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,
