@@ -20,6 +20,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 COMMON = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
           "-Xcompiler", "-fPIC,-ffp-contract=off", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+COMMON += os.environ.get("XPR_NVCC_FLAGS", "").split()   # e.g. -DXPR_PBWD_MINB=3 for tuning experiments
 SOURCES = {
     "api.cu": [],
     "project.cu": ["-fmad=false"],

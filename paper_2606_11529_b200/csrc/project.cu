@@ -354,41 +354,63 @@ __device__ __forceinline__ void store_sh_grad(float* __restrict__ g_sh, int64_t 
     }
 }
 
-#ifndef XPR_PBWD_MINB
-#define XPR_PBWD_MINB 4
-#endif
+// One visible Gaussian: recompute the forward, chain rule in fp64, store its 59 gradient floats.
 template <int K>
-__global__ void __launch_bounds__(128, XPR_PBWD_MINB)
-project_bwd_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const float* __restrict__ scales,
-                   const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
-                   const uint32_t* __restrict__ tcount, const uint8_t* __restrict__ flags,
-                   const float* __restrict__ g_mean2d, const float* __restrict__ g_conic,
-                   const float* __restrict__ g_opac, const float* __restrict__ g_rgb, float* __restrict__ g_means,
-                   float* __restrict__ g_scales, float* __restrict__ g_quats, float* __restrict__ g_opacities,
-                   float* __restrict__ g_sh) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    float gsh[3 * K];
-#pragma unroll
-    for (int j = 0; j < 3 * K; ++j) gsh[j] = 0.0f;
+__device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, const float* __restrict__ means,
+                                                const float* __restrict__ scales, const float* __restrict__ quats,
+                                                const float* __restrict__ opac, const float* __restrict__ sh,
+                                                const uint8_t* __restrict__ flags, const float* __restrict__ g_mean2d,
+                                                const float* __restrict__ g_conic, const float* __restrict__ g_opac,
+                                                const float* __restrict__ g_rgb, float* __restrict__ g_means,
+                                                float* __restrict__ g_scales, float* __restrict__ g_quats,
+                                                float* __restrict__ g_opacities, float* __restrict__ g_sh) {
     B g_mu[3] = {0, 0, 0}, g_s[3] = {0, 0, 0}, g_q[4] = {0, 0, 0, 0}, g_o = 0;
+    // every load of this Gaussian is issued up front (the kernel is latency-bound: DESIGN.md 6.1)
     const uint8_t fl = flags[i];
-    bool vis = (tcount[i] != 0u) && (fl & XPR_FLAG_VISIBLE);
     Fwd F;
-    float mu[3], sc[3], q[4], o = 0.0f;
-    if (vis) {
-        mu[0] = __ldg(means + 3 * i); mu[1] = __ldg(means + 3 * i + 1); mu[2] = __ldg(means + 3 * i + 2);
-        sc[0] = __ldg(scales + 3 * i); sc[1] = __ldg(scales + 3 * i + 1); sc[2] = __ldg(scales + 3 * i + 2);
-        const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
-        q[0] = q4.x; q[1] = q4.y; q[2] = q4.z; q[3] = q4.w;
-        o = __ldg(opac + i);
-        vis = project_geometry(P, mu, sc, q, o, F);   // recompute; same decisions as forward
+    float mu[3], sc[3], q[4], o;
+    mu[0] = __ldg(means + 3 * i); mu[1] = __ldg(means + 3 * i + 1); mu[2] = __ldg(means + 3 * i + 2);
+    sc[0] = __ldg(scales + 3 * i); sc[1] = __ldg(scales + 3 * i + 1); sc[2] = __ldg(scales + 3 * i + 2);
+    const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
+    q[0] = q4.x; q[1] = q4.y; q[2] = q4.z; q[3] = q4.w;
+    o = __ldg(opac + i);
+    const float2 gm_f = __ldg(reinterpret_cast<const float2*>(g_mean2d) + i);
+    const float gK_f[3] = {__ldg(g_conic + 3 * i), __ldg(g_conic + 3 * i + 1), __ldg(g_conic + 3 * i + 2)};
+    const float go_f = __ldg(g_opac + i);
+    const float grgb_f[3] = {__ldg(g_rgb + 3 * i), __ldg(g_rgb + 3 * i + 1), __ldg(g_rgb + 3 * i + 2)};
+    {   // colour first: rgb = max(0, 1/2 + sum_k Y_k(d) sh_k), d = (mu - cam_pos)/|mu - cam_pos|.  Its 3K
+        // coefficient gradients are stored at once, so they do not occupy registers during the chain rule.
+        float c[3 * K];
+        load_sh<K>(sh, i, c);
+        const B grgb[3] = {(B)grgb_f[0], (B)grgb_f[1], (B)grgb_f[2]};
+        float dir[3], dnorm, Y[16];
+        view_dir(P, mu, dir, dnorm);
+        sh_basis(dir[0], dir[1], dir[2], Y);
+        B dY[16][3];
+        sh_basis_grad((B)dir[0], (B)dir[1], (B)dir[2], dY);
+        B gd[3] = {0, 0, 0};
+        float gsh[3 * K];
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) {
+            const bool on = (fl & (XPR_FLAG_RGB_POS_R << ch)) != 0;   // C16 mask saved by the forward
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                gsh[3 * k + ch] = on ? Y[k] * grgb_f[ch] : 0.0f;
+                const B cg = on ? (B)c[3 * k + ch] * grgb[ch] : 0.0;
+#pragma unroll
+                for (int j = 0; j < 3; ++j) gd[j] += dY[k][j] * cg;
+            }
+        }
+        store_sh_grad<K>(g_sh, i, gsh);
+        const B dot = (B)dir[0] * gd[0] + (B)dir[1] * gd[1] + (B)dir[2] * gd[2];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) g_mu[j] = (gd[j] - (B)dir[j] * dot) / (B)dnorm;
     }
+    const bool vis = project_geometry(P, mu, sc, q, o, F);   // recompute; same decisions as forward
     if (vis) {
-        const B gm[2] = {(B)g_mean2d[2 * i], (B)g_mean2d[2 * i + 1]};
-        const B gK[3] = {(B)g_conic[3 * i], (B)g_conic[3 * i + 1], (B)g_conic[3 * i + 2]};
-        const B go_eff = (B)g_opac[i];
-        const B grgb[3] = {(B)g_rgb[3 * i], (B)g_rgb[3 * i + 1], (B)g_rgb[3 * i + 2]};
+        const B gm[2] = {(B)gm_f.x, (B)gm_f.y};
+        const B gK[3] = {(B)gK_f[0], (B)gK_f[1], (B)gK_f[2]};
+        const B go_eff = (B)go_f;
         const float* W = P.W;
         // conic -> filtered covariance: G2 = -K G_K K (symmetric-matrix gradients)
         const B A = F.A, Bc = F.B, C = F.C;
@@ -507,35 +529,98 @@ project_bwd_kernel(int64_t N, ProjParams P, const float* __restrict__ means, con
             g_q[2] = 2.0 * (-2.0 * y * gR[0][0] + x * gR[0][1] + w * gR[0][2] + x * gR[1][0] + z * gR[1][2] - w * gR[2][0] + z * gR[2][1] - 2.0 * y * gR[2][2]);
             g_q[3] = 2.0 * (-2.0 * z * gR[0][0] - w * gR[0][1] + x * gR[0][2] + w * gR[1][0] - 2.0 * z * gR[1][1] + y * gR[1][2] + x * gR[2][0] + y * gR[2][1]);
         }
-        // colour: rgb = max(0, 1/2 + sum_k Y_k(d) sh_k), d = (mu - cam_pos)/|mu - cam_pos|
-        float dir[3], dnorm, Y[16];
-        view_dir(P, mu, dir, dnorm);
-        sh_basis(dir[0], dir[1], dir[2], Y);
-        float c[3 * K];
-        load_sh<K>(sh, i, c);
-        B dY[16][3];
-        sh_basis_grad((B)dir[0], (B)dir[1], (B)dir[2], dY);
-        B gd[3] = {0, 0, 0};
+    } else {   // cannot happen for a Gaussian the forward flagged visible (same arithmetic); keep the contract anyway
+        float z[3 * K];
 #pragma unroll
-        for (int ch = 0; ch < 3; ++ch) {
-            if (!(fl & (XPR_FLAG_RGB_POS_R << ch))) continue;   // C16 mask saved by the forward
-#pragma unroll
-            for (int k = 0; k < K; ++k) {
-                gsh[3 * k + ch] = (float)((B)Y[k] * grgb[ch]);
-                const B cg = (B)c[3 * k + ch] * grgb[ch];
-#pragma unroll
-                for (int j = 0; j < 3; ++j) gd[j] += dY[k][j] * cg;
-            }
-        }
-        const B dot = (B)dir[0] * gd[0] + (B)dir[1] * gd[1] + (B)dir[2] * gd[2];
-#pragma unroll
-        for (int j = 0; j < 3; ++j) g_mu[j] += (gd[j] - (B)dir[j] * dot) / (B)dnorm;
+        for (int j = 0; j < 3 * K; ++j) z[j] = 0.0f;
+        store_sh_grad<K>(g_sh, i, z);
+        g_mu[0] = g_mu[1] = g_mu[2] = 0;
     }
     g_means[3 * i] = (float)g_mu[0]; g_means[3 * i + 1] = (float)g_mu[1]; g_means[3 * i + 2] = (float)g_mu[2];
     g_scales[3 * i] = (float)g_s[0]; g_scales[3 * i + 1] = (float)g_s[1]; g_scales[3 * i + 2] = (float)g_s[2];
     reinterpret_cast<float4*>(g_quats)[i] = make_float4((float)g_q[0], (float)g_q[1], (float)g_q[2], (float)g_q[3]);
     g_opacities[i] = (float)g_o;
-    store_sh_grad<K>(g_sh, i, gsh);
+}
+
+// Backward kernel.  Only a fraction of the Gaussians is visible (26 % in config 3) and they are
+// scattered, so one thread per Gaussian would run the heavy chain rule with a handful of active lanes
+// per warp.  Each CTA therefore owns PBWD_THREADS * ipt consecutive Gaussians and works in three
+// phases: (1) read tile_count / flags coalesced and compact the visible indices into shared memory,
+// (2) run the chain rule over the dense list, (3) write zeros for the culled ones, coalesced, skipping
+// the visible ones (every output element is written exactly once).
+constexpr int PBWD_THREADS = 128, PBWD_MAX_IPT = 16;
+
+#ifndef XPR_PBWD_MINB
+#define XPR_PBWD_MINB 3
+#endif
+template <int K>
+__global__ void __launch_bounds__(PBWD_THREADS, XPR_PBWD_MINB)
+project_bwd_kernel(int64_t N, ProjParams P, int ipt, const float* __restrict__ means, const float* __restrict__ scales,
+                   const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
+                   const uint32_t* __restrict__ tcount, const uint8_t* __restrict__ flags,
+                   const float* __restrict__ g_mean2d, const float* __restrict__ g_conic,
+                   const float* __restrict__ g_opac, const float* __restrict__ g_rgb, float* __restrict__ g_means,
+                   float* __restrict__ g_scales, float* __restrict__ g_quats, float* __restrict__ g_opacities,
+                   float* __restrict__ g_sh) {
+    __shared__ uint16_t s_list[PBWD_THREADS * PBWD_MAX_IPT];
+    __shared__ uint32_t s_vis[PBWD_THREADS * PBWD_MAX_IPT / 32];   // bit j: Gaussian base + j is visible
+    __shared__ uint32_t s_cnt;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int chunk = PBWD_THREADS * ipt;
+    const int64_t base = (int64_t)blockIdx.x * chunk;
+    const int n_here = (int)min((int64_t)chunk, N - base);
+    if (tid == 0) s_cnt = 0u;
+    __syncthreads();
+    uint32_t tc[PBWD_MAX_IPT];                           // independent loads first (tile_count != 0 <=> visible)
+#pragma unroll
+    for (int k = 0; k < PBWD_MAX_IPT; ++k) {
+        const int j = k * PBWD_THREADS + tid;
+        tc[k] = (k < ipt && j < n_here) ? __ldg(tcount + base + j) : 0u;
+    }
+    uint32_t vbits = 0;
+#pragma unroll
+    for (int k = 0; k < PBWD_MAX_IPT; ++k) vbits |= (tc[k] != 0u ? 1u : 0u) << k;
+    for (int k = 0; k < ipt; ++k) {
+        const int j = k * PBWD_THREADS + tid;
+        const bool vis = (vbits >> k) & 1u;
+        const uint32_t m = __ballot_sync(0xffffffffu, vis);
+        uint32_t pos = 0;
+        if (lane == 0) {
+            s_vis[k * (PBWD_THREADS / 32) + warp] = m;
+            if (m) pos = atomicAdd(&s_cnt, (uint32_t)__popc(m));
+        }
+        pos = __shfl_sync(0xffffffffu, pos, 0);
+        if (vis) s_list[pos + __popc(m & ((1u << lane) - 1u))] = (uint16_t)j;
+    }
+    __syncthreads();
+    const int cnt = (int)s_cnt;
+    // zeros for the culled Gaussians first: the stores drain while the dense phase waits on its gathers
+    auto culled = [&](int j) { return !((s_vis[j >> 5] >> (j & 31)) & 1u); };
+#pragma unroll 4
+    for (int e = tid; e < 3 * n_here; e += PBWD_THREADS) {
+        if (culled(e / 3)) { g_means[3 * base + e] = 0.0f; g_scales[3 * base + e] = 0.0f; }
+    }
+#pragma unroll 4
+    for (int j = tid; j < n_here; j += PBWD_THREADS) {
+        if (culled(j)) {
+            reinterpret_cast<float4*>(g_quats)[base + j] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            g_opacities[base + j] = 0.0f;
+        }
+    }
+    if constexpr ((3 * K) % 4 == 0) {
+        constexpr int V = (3 * K) / 4;                 // float4 per Gaussian
+        float4* p4 = reinterpret_cast<float4*>(g_sh) + base * V;
+#pragma unroll 8
+        for (int e = tid; e < V * n_here; e += PBWD_THREADS)
+            if (culled(e / V)) p4[e] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    } else {
+        float* p = g_sh + base * (3 * K);
+        for (int e = tid; e < 3 * K * n_here; e += PBWD_THREADS)
+            if (culled(e / (3 * K))) p[e] = 0.0f;
+    }
+    for (int idx = tid; idx < cnt; idx += PBWD_THREADS)
+        project_bwd_one<K>(base + s_list[idx], P, means, scales, quats, opac, sh, flags, g_mean2d, g_conic, g_opac,
+                           g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh);
 }
 
 int32_t make_params(const xpr_camera* cam, const xpr_config* cfg, ProjParams& P) {
@@ -621,19 +706,25 @@ extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* s
     if (N < 0 || N > 0x7fffffffLL) return XPR_ERR_INVALID_ARG;
     if (N == 0) return XPR_OK;
     if (!aligned(means, 4) || !aligned(scales, 4) || !aligned(quats, 16) || !aligned(opacities, 4) ||
-        !aligned(sh, 16) || !aligned(tile_count, 4) || !flags || !aligned(g_mean2d, 4) || !aligned(g_conic, 4) ||
+        !aligned(sh, 16) || !aligned(tile_count, 4) || !flags || !aligned(g_mean2d, 8) || !aligned(g_conic, 4) ||
         !aligned(g_opac, 4) || !aligned(g_rgb, 4) || !aligned(g_means, 4) || !aligned(g_scales, 4) ||
         !aligned(g_quats, 16) || !aligned(g_opacities, 4) || !aligned(g_sh, 16))
         return XPR_ERR_INVALID_ARG;
     ProjParams P;
     if (int32_t s = make_params(cam, cfg, P)) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    const int threads = 128;
-    const unsigned blocks = (unsigned)((N + threads - 1) / threads);
-#define XPR_GO(KK)                                                                                               \
-    project_bwd_kernel<KK><<<blocks, threads, 0, st>>>(N, P, means, scales, quats, opacities, sh, tile_count, flags, \
-                                                       g_mean2d, g_conic, g_opac, g_rgb, g_means, g_scales, g_quats, \
-                                                       g_opacities, g_sh)
+    // Gaussians per CTA: enough CTAs for one full wave (148 SMs x 4 CTAs) before growing the chunk
+#ifndef XPR_PBWD_WAVES
+#define XPR_PBWD_WAVES 2
+#endif
+    int ipt = (int)(N / ((int64_t)148 * 4 * PBWD_THREADS * XPR_PBWD_WAVES));
+    ipt = ipt < 1 ? 1 : (ipt > PBWD_MAX_IPT ? PBWD_MAX_IPT : ipt);
+    const int64_t chunk = (int64_t)PBWD_THREADS * ipt;
+    const unsigned blocks = (unsigned)((N + chunk - 1) / chunk);
+#define XPR_GO(KK)                                                                                                  \
+    project_bwd_kernel<KK><<<blocks, PBWD_THREADS, 0, st>>>(N, P, ipt, means, scales, quats, opacities, sh, tile_count, \
+                                                            flags, g_mean2d, g_conic, g_opac, g_rgb, g_means, g_scales, \
+                                                            g_quats, g_opacities, g_sh)
     switch (cfg->sh_degree) {
         case 0: XPR_GO(1); break;
         case 1: XPR_GO(4); break;
