@@ -5,12 +5,18 @@
 // lexicographically by (tile id, depth)", "identify bounds".  Key packing tile << 32 | depth bits
 // is BASELINE.json:north_star (reading C10); ties keep ascending Gaussian index.
 //
-// The sort is one stable LSD radix sort of the 64-bit keys, 8 bits per pass, with one observation
-// (DESIGN.md section 6): the four low digits are the depth bits, which all pairs of a Gaussian
-// share, and replication preserves order.  So the four depth passes run on the visible Gaussians
-// (N_vis keys) BEFORE replication, pairs are emitted in that order, and only the tile-id digits
-// (2 passes at 1080p) run on the I replicated pairs.  The result is bit-identical to sorting the
-// I keys by all digits; HBM traffic per pair drops from 12 + 6*24 + 8 to 12 + 2*24 + 8 bytes.
+// The sort is one stable LSD radix sort of the 64-bit keys, 8 bits per pass, reorganised around two
+// observations:
+//  (1) the four low digits are the depth bits, which all pairs of a Gaussian share, and replication
+//      preserves order.  So the four depth passes run on the visible Gaussians (N_vis keys) BEFORE
+//      replication, pairs are emitted in that order, and only the tile-id digits (2 passes at 1080p)
+//      run on the I replicated pairs.
+//  (2) once the Gaussians are in (depth, index) order, a pair only has to carry its tile id and the
+//      RANK of its Gaussian in that order: the tile passes move 8-byte words (tile << 32 | rank), and
+//      the last pass expands them to the 64-bit key (tile << 32 | depth bits) and the 32-bit value
+//      (Gaussian index) through two small L2-resident tables.
+// The result is bit-identical to sorting the I (key, value) pairs by all digits; HBM traffic per pair
+// drops from 12 + 6*24 + 8 = 164 bytes to 8 + 16 + 20 = 44 bytes.
 //
 // Kernels (all hand-written, no CUB):
 //   compact_kernel   single-pass chained scan (decoupled look-back) of the visibility flags; writes
@@ -18,12 +24,14 @@
 //                    histograms.
 //   onesweep_kernel  one launch per 8-bit digit, least significant first: warp-striped loads,
 //                    stable in-warp ranking (match.any or ballot), shared-memory digit counts,
-//                    per-digit decoupled look-back across CTAs, shared-memory staged scatter.
-//                    Instantiated for 32-bit keys (Gaussians) and 64-bit keys (pairs).
+//                    per-digit decoupled look-back across tiles, shared-memory staged scatter.
+//                    Persistent CTAs draw tiles from a ticket counter.  Instantiated for 32-bit
+//                    keys + values (Gaussians) and for 64-bit packed words (pairs).
 //   offsets_kernel   chained scan of the tile counts in depth order -> pair offsets and I.
-//   emit_kernel      pair-parallel, load-balanced replication (each CTA writes 1024 consecutive pairs:
-//                    coalesced 8-byte key / 4-byte value stores) + the tile-digit histograms.
-//   ranges_kernel    per-tile (start, end) from the sorted keys.
+//   emit_kernel      pair-parallel, load-balanced replication: a CTA writes 2048 consecutive pairs
+//                    whatever Gaussians they belong to (segment heads scattered into shared memory,
+//                    max-scan, then one coalesced 8-byte store per pair) + the tile-digit histograms.
+//   ranges_kernel    per-tile (start, end): one warp per tile, 32-ary search in the sorted keys.
 #include "common.cuh"
 
 namespace xpr {
@@ -34,12 +42,16 @@ constexpr int RADIX = 1 << RADIX_BITS;
 constexpr int DEPTH_PASSES = 4;             // 32 depth bits
 constexpr int MAX_TILE_PASSES = 4;          // up to 2^31 tiles
 
-constexpr int SCAN_THREADS = 256;           // Gaussians per compact / emit block (one per thread)
+constexpr int SCAN_THREADS = 256;           // compact / offsets: 8 warps x 256 items
+constexpr int SCAN_WARPS = SCAN_THREADS / 32;
+constexpr int SCAN_ROUNDS = 8;              // items per lane
+constexpr int SCAN_ITEMS = SCAN_THREADS * SCAN_ROUNDS;
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 static_assert(SORT_THREADS == RADIX, "one thread per digit");
-constexpr int IPT32 = 4;                    // Gaussian-level passes: 1024 keys per CTA (N_vis is small)
-constexpr int IPT64 = 16;                   // pair-level passes: 4096 pairs per CTA
+constexpr int IPT32 = 4;                    // Gaussian-level passes: 1024 keys per tile (N_vis is small)
+constexpr int IPT64 = 16;                   // pair-level passes: 4096 pairs per tile
+constexpr int PERSIST_CTAS = 148 * 4;       // upper bound of the persistent grids
 
 constexpr uint32_t FLAG_PARTIAL = 1u << 30, FLAG_INCLUSIVE = 2u << 30, FLAG_MASK = 3u << 30, VALUE_MASK = ~FLAG_MASK;
 constexpr unsigned long long SFLAG_PARTIAL = 1ull << 62, SFLAG_INCLUSIVE = 2ull << 62, SFLAG_MASK = 3ull << 62;
@@ -55,24 +67,25 @@ struct Header {
 };
 
 struct Layout {
-    size_t header, scan_status, vkey0, vidx0, vkey1, vidx1, status32, keys_tmp, vals_tmp, status64, total;
+    size_t header, scan_status, vkey0, vidx0, vkey1, vidx1, status32, keys_tmp, status64, total;
 };
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-inline int tile_passes_for(int32_t num_tiles) {
+inline int tile_passes_for(int32_t num_tiles) {   // at least one: the last pass also expands the packed words
     int bits = 0;
     while (bits < 31 && ((int64_t)1 << bits) < (int64_t)num_tiles) ++bits;
-    return (bits + RADIX_BITS - 1) / RADIX_BITS;
+    const int p = (bits + RADIX_BITS - 1) / RADIX_BITS;
+    return p < 1 ? 1 : p;
 }
 
 inline Layout make_layout(int64_t N, int64_t cap, int32_t num_tiles) {
     Layout L;
     size_t off = 0;
     const size_t n = (size_t)N, c = (size_t)cap;
-    const size_t scan_blocks = (n + SCAN_THREADS - 1) / SCAN_THREADS;
+    const size_t scan_blocks = (n + SCAN_ITEMS - 1) / SCAN_ITEMS;
     L.header = off; off = align_up(off + sizeof(Header), 256);
-    L.scan_status = off; off = align_up(off + 8 * 2 * (scan_blocks + 1), 256);      // compact + emit chains
+    L.scan_status = off; off = align_up(off + 8 * 2 * (scan_blocks + 1), 256);      // compact + offsets chains
     const size_t tiles32 = (n + SORT_THREADS * IPT32 - 1) / (SORT_THREADS * IPT32);
     L.status32 = off; off = align_up(off + 4 * (size_t)RADIX * tiles32 * DEPTH_PASSES, 256);
     // everything up to here is zeroed with one memset
@@ -81,7 +94,6 @@ inline Layout make_layout(int64_t N, int64_t cap, int32_t num_tiles) {
     L.vkey1 = off; off = align_up(off + 4 * n, 256);
     L.vidx1 = off; off = align_up(off + 4 * n, 256);
     L.keys_tmp = off; off = align_up(off + 8 * c, 256);
-    L.vals_tmp = off; off = align_up(off + 4 * c, 256);
     const size_t tiles64 = (c + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
     L.status64 = off; off = align_up(off + 4 * (size_t)RADIX * tiles64 * (size_t)tile_passes_for(num_tiles), 256);
     L.total = off;
@@ -105,90 +117,100 @@ __device__ __forceinline__ void st_relaxed64(unsigned long long* p, unsigned lon
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-// Block-wide exclusive scan of one value per thread (SCAN_THREADS threads) followed by the chained
-// scan across blocks (decoupled look-back; `block` is a ticket, so predecessors are running or done).
-// Returns the block-local exclusive offset; *block_total and *global_base are block-uniform.
-__device__ __forceinline__ uint32_t chained_scan(uint32_t x, uint32_t block, unsigned long long* __restrict__ status,
-                                                 uint32_t* s_warp, unsigned long long* s_base, uint32_t* block_total,
-                                                 unsigned long long* global_base) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    uint32_t incl = x;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += v;
+// Chained scan across blocks (decoupled look-back), executed by warp 0 of a ticketed block: publishes
+// the block's total and returns (to every lane of warp 0) the sum of the totals of all earlier blocks.
+// `block` is a ticket, so every predecessor is running or done (forward progress).
+__device__ __forceinline__ unsigned long long chain_lookback(uint32_t block, uint32_t btotal,
+                                                             unsigned long long* __restrict__ status, int lane) {
+    unsigned long long excl = 0;
+    if (block == 0) {
+        if (lane == 0) st_relaxed64(&status[0], SFLAG_INCLUSIVE | (unsigned long long)btotal);
+        return 0;
     }
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    uint32_t wbase = 0, btotal = 0;
+    if (lane == 0) st_relaxed64(&status[block], SFLAG_PARTIAL | (unsigned long long)btotal);
+    int64_t top = (int64_t)block - 1;          // lane l inspects predecessor top - l
+    while (true) {
+        const int64_t t = top - lane;
+        unsigned long long sv = SFLAG_INCLUSIVE;   // virtual predecessors before block 0: inclusive 0
+        if (t >= 0) { do { sv = ld_relaxed64(&status[t]); } while ((sv & SFLAG_MASK) == 0); }
+        const uint32_t incl_mask = __ballot_sync(0xffffffffu, (sv & SFLAG_MASK) == SFLAG_INCLUSIVE);
+        const int first = incl_mask ? (__ffs(incl_mask) - 1) : 32;     // nearest inclusive predecessor
+        unsigned long long v = (lane <= first) ? (sv & ~SFLAG_MASK) : 0ull;
 #pragma unroll
-    for (int w = 0; w < SCAN_THREADS / 32; ++w) {
-        const uint32_t v = s_warp[w];
-        if (w < warp) wbase += v;
-        btotal += v;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        excl += v;
+        if (incl_mask) break;
+        top -= 32;
     }
-    if (warp == 0) {
-        // decoupled look-back by one warp: 32 predecessors per step
-        unsigned long long excl = 0;
-        if (block == 0) {
-            if (lane == 0) st_relaxed64(&status[0], SFLAG_INCLUSIVE | (unsigned long long)btotal);
-        } else {
-            if (lane == 0) st_relaxed64(&status[block], SFLAG_PARTIAL | (unsigned long long)btotal);
-            int64_t top = (int64_t)block - 1;          // lane l inspects predecessor top - l
-            while (true) {
-                const int64_t t = top - lane;
-                unsigned long long sv = SFLAG_INCLUSIVE;   // virtual predecessors before block 0: inclusive 0
-                if (t >= 0) { do { sv = ld_relaxed64(&status[t]); } while ((sv & SFLAG_MASK) == 0); }
-                const uint32_t incl_mask = __ballot_sync(0xffffffffu, (sv & SFLAG_MASK) == SFLAG_INCLUSIVE);
-                const int first = incl_mask ? (__ffs(incl_mask) - 1) : 32;     // nearest inclusive predecessor
-                unsigned long long v = (lane <= first) ? (sv & ~SFLAG_MASK) : 0ull;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                excl += v;
-                if (incl_mask) break;
-                top -= 32;
-            }
-            if (lane == 0) st_relaxed64(&status[block], SFLAG_INCLUSIVE | (excl + btotal));
-        }
-        if (lane == 0) *s_base = excl;
-    }
-    __syncthreads();
-    *block_total = btotal;
-    *global_base = *s_base;
-    return wbase + incl - x;
+    if (lane == 0) st_relaxed64(&status[block], SFLAG_INCLUSIVE | (excl + btotal));
+    return excl;
 }
 
 // ---------------------------------------------------------------------------------------------
-// compact: visible Gaussians in index order -> (depth bits, index), + depth-digit histograms
+// compact: visible Gaussians in index order -> (depth bits, index), + depth-digit histograms.
+// A block owns SCAN_ITEMS consecutive Gaussians; warp w owns 256 of them and reads them in 8 coalesced
+// rounds, so the in-warp prefix is just ballots and popcounts.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(SCAN_THREADS)
 compact_kernel(int64_t N, const float* __restrict__ depth, const uint32_t* __restrict__ tcount,
                Header* __restrict__ hdr, unsigned long long* __restrict__ status, uint32_t* __restrict__ vkey,
                uint32_t* __restrict__ vidx) {
-    __shared__ uint32_t s_warp[SCAN_THREADS / 32];
+    __shared__ uint32_t s_warp[SCAN_WARPS];
     __shared__ uint32_t s_hist[DEPTH_PASSES * RADIX];
     __shared__ uint32_t s_block;
     __shared__ unsigned long long s_base;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_block = atomicAdd(&hdr->compact_ticket, 1u);
     for (int b = tid; b < DEPTH_PASSES * RADIX; b += SCAN_THREADS) s_hist[b] = 0u;
     __syncthreads();
     const uint32_t block = s_block;
-    const int64_t i = (int64_t)block * SCAN_THREADS + tid;
-    const bool vis = (i < N) && (tcount[i] != 0u);
-    uint32_t db = 0;
-    if (vis) {
-        db = __float_as_uint(depth[i]);
+    const int64_t i0 = (int64_t)block * SCAN_ITEMS + warp * (32 * SCAN_ROUNDS) + lane;
+    uint32_t tc[SCAN_ROUNDS], db[SCAN_ROUNDS];
 #pragma unroll
-        for (int d = 0; d < DEPTH_PASSES; ++d) atomicAdd(&s_hist[d * RADIX + ((db >> (8 * d)) & 255u)], 1u);
+    for (int r = 0; r < SCAN_ROUNDS; ++r) {
+        const int64_t i = i0 + r * 32;
+        tc[r] = (i < N) ? __ldg(tcount + i) : 0u;
+        db[r] = (i < N) ? __float_as_uint(__ldg(depth + i)) : 0u;   // never-written for a culled Gaussian; unused then
     }
-    uint32_t btotal; unsigned long long base;
-    const uint32_t off = chained_scan(vis ? 1u : 0u, block, status, s_warp, &s_base, &btotal, &base);
-    if (vis) {
-        vkey[base + off] = db;
-        vidx[base + off] = (uint32_t)i;
+    uint32_t pos[SCAN_ROUNDS], wtotal = 0;
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int r = 0; r < SCAN_ROUNDS; ++r) {
+        const uint32_t m = __ballot_sync(0xffffffffu, tc[r] != 0u);
+        pos[r] = wtotal + (uint32_t)__popc(m & lt);
+        wtotal += (uint32_t)__popc(m);
     }
-    if (tid == 0 && (int64_t)(block + 1) * SCAN_THREADS >= N) hdr->n_vis = (uint32_t)(base + btotal);
+    if (lane == 0) s_warp[warp] = wtotal;
+    __syncthreads();
+    uint32_t wbase = 0, btotal = 0;
+#pragma unroll
+    for (int w = 0; w < SCAN_WARPS; ++w) {
+        const uint32_t v = s_warp[w];
+        if (w < warp) wbase += v;
+        btotal += v;
+    }
+    if (warp == 0) {
+        const unsigned long long e = chain_lookback(block, btotal, status, lane);
+        if (lane == 0) s_base = e;
+    }
+#pragma unroll
+    for (int r = 0; r < SCAN_ROUNDS; ++r) {
+        if (tc[r] != 0u) {
+#pragma unroll
+            for (int d = 0; d < DEPTH_PASSES; ++d) atomicAdd(&s_hist[d * RADIX + ((db[r] >> (8 * d)) & 255u)], 1u);
+        }
+    }
+    __syncthreads();
+    const unsigned long long base = s_base;
+#pragma unroll
+    for (int r = 0; r < SCAN_ROUNDS; ++r) {
+        if (tc[r] != 0u) {
+            const unsigned long long p = base + wbase + pos[r];
+            vkey[p] = db[r];
+            vidx[p] = (uint32_t)(i0 + r * 32);
+        }
+    }
+    if (tid == 0 && (int64_t)(block + 1) * SCAN_ITEMS >= N) hdr->n_vis = (uint32_t)(base + btotal);
     for (int b = tid; b < DEPTH_PASSES * RADIX; b += SCAN_THREADS) {
         const uint32_t v = s_hist[b];
         if (v) atomicAdd(&hdr->hist[b], v);
@@ -201,96 +223,176 @@ compact_kernel(int64_t N, const float* __restrict__ depth, const uint32_t* __res
 __global__ void __launch_bounds__(SCAN_THREADS)
 offsets_kernel(const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ tcount, Header* __restrict__ hdr,
                unsigned long long* __restrict__ status, uint32_t* __restrict__ voff) {
-    __shared__ uint32_t s_warp[SCAN_THREADS / 32];
+    __shared__ uint32_t s_warp[SCAN_WARPS];
     __shared__ uint32_t s_block;
     __shared__ unsigned long long s_base;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n_vis = hdr->n_vis;
     if (tid == 0) s_block = atomicAdd(&hdr->emit_ticket, 1u);   // ticket order = look-back order
     __syncthreads();
     const uint32_t block = s_block;
-    if ((uint64_t)block * SCAN_THREADS >= n_vis && block != 0) return;   // beyond the visible list: nobody waits on us
-    const uint32_t s = block * SCAN_THREADS + tid;       // position in depth order
-    const uint32_t tc = (s < n_vis) ? tcount[vidx[s]] : 0u;
-    uint32_t btotal; unsigned long long base;
-    const uint32_t off = chained_scan(tc, block, status, s_warp, &s_base, &btotal, &base);
-    if (s < n_vis) voff[s] = (uint32_t)(base + off);     // only used when I <= pair_capacity < 2^30
-    if (tid == 0 && (uint64_t)(block + 1) * SCAN_THREADS >= n_vis) hdr->total_pairs = base + btotal;   // I
+    if ((uint64_t)block * SCAN_ITEMS >= n_vis && block != 0) return;   // beyond the visible list: nobody waits on us
+    const uint32_t s0 = block * (uint32_t)SCAN_ITEMS + (uint32_t)warp * (32 * SCAN_ROUNDS) + (uint32_t)lane;
+    uint32_t tc[SCAN_ROUNDS];
+#pragma unroll
+    for (int r = 0; r < SCAN_ROUNDS; ++r) {
+        const uint32_t s = s0 + r * 32;
+        tc[r] = (s < n_vis) ? __ldg(tcount + __ldg(vidx + s)) : 0u;
+    }
+    uint32_t excl[SCAN_ROUNDS], wtotal = 0;
+#pragma unroll
+    for (int r = 0; r < SCAN_ROUNDS; ++r) {
+        uint32_t incl = tc[r];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        excl[r] = wtotal + incl - tc[r];
+        wtotal += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (lane == 0) s_warp[warp] = wtotal;
+    __syncthreads();
+    uint32_t wbase = 0, btotal = 0;
+#pragma unroll
+    for (int w = 0; w < SCAN_WARPS; ++w) {
+        const uint32_t v = s_warp[w];
+        if (w < warp) wbase += v;
+        btotal += v;
+    }
+    if (warp == 0) {
+        const unsigned long long e = chain_lookback(block, btotal, status, lane);
+        if (lane == 0) s_base = e;
+    }
+    __syncthreads();
+    const unsigned long long base = s_base;
+#pragma unroll
+    for (int r = 0; r < SCAN_ROUNDS; ++r) {
+        const uint32_t s = s0 + r * 32;
+        if (s < n_vis) voff[s] = (uint32_t)(base + wbase + excl[r]);   // only used when I <= pair_capacity < 2^30
+    }
+    if (tid == 0 && (uint64_t)(block + 1) * SCAN_ITEMS >= n_vis) hdr->total_pairs = base + btotal;   // I
+}
+
+// 32-ary search by one warp in a sorted u32 array: first index in [0, n) whose element is > x
+// (n if none).  ~log32(n) dependent loads instead of log2(n).
+__device__ __forceinline__ uint32_t warp_upper_bound(const uint32_t* __restrict__ a, uint32_t n, uint32_t x, int lane) {
+    uint32_t lo = 0, hi = n;                   // answer in [lo, hi]; hi == n or a[hi] > x
+    while (hi > lo) {
+        const uint32_t len = hi - lo, stride = (len + 31u) / 32u;
+        const uint32_t probe = min(lo + ((uint32_t)lane + 1u) * stride - 1u, hi - 1u);
+        const uint32_t b = __ballot_sync(0xffffffffu, a[probe] > x);
+        if (b == 0u) { lo = hi; break; }
+        const uint32_t f = (uint32_t)__ffs(b) - 1u;
+        hi = min(lo + (f + 1u) * stride - 1u, hi - 1u);
+        lo = lo + f * stride;
+    }
+    return lo;
 }
 
 // ---------------------------------------------------------------------------------------------
-// emit: replicate + assign tile id, pair-parallel and load-balanced: CTA b writes the
-// pairs [b*EMIT_PAIRS, (b+1)*EMIT_PAIRS) whatever Gaussians they belong to (a near Gaussian may
-// cover thousands of tiles, and in depth order those come first).  + tile-digit histograms.
+// emit: replicate + assign tile id, pair-parallel and load-balanced.  A unit of work is
+// EMIT_PAIRS consecutive pairs [p0, p1), whatever Gaussians they belong to (a near Gaussian covers
+// thousands of tiles, and in depth order those come first):
+//   1. warp 0 finds the Gaussian (in depth order) that owns pair p0 by a 32-ary search in voff;
+//   2. the Gaussians that start inside [p0, p1) are loaded one per thread into shared memory
+//      (offset, first tile id, rectangle width, 1/width) and their slot number is written at the
+//      position of their first pair;
+//   3. a max-scan over the positions gives every pair its slot;
+//   4. pair j of a slot: r = j - offset, (ry, rx) = divmod(r, w), tile = tile0 + ry * TW + rx; one
+//      coalesced 8-byte store of tile << 32 | rank; shared-memory histograms of the tile digits.
+// CTAs are persistent (grid <= PERSIST_CTAS) so that the digit histograms are flushed to global
+// memory once per CTA, not once per 2048 pairs.
 // ---------------------------------------------------------------------------------------------
-constexpr int EMIT_THREADS = 256, EMIT_PPT = 4, EMIT_PAIRS = EMIT_THREADS * EMIT_PPT;
+constexpr int EMIT_THREADS = 256, EMIT_PPT = 8, EMIT_PAIRS = EMIT_THREADS * EMIT_PPT;
+constexpr int EMIT_WARPS = EMIT_THREADS / 32;
 
 __global__ void __launch_bounds__(EMIT_THREADS)
-emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vkey, const uint32_t* __restrict__ vidx,
-            const uint32_t* __restrict__ voff, const int4* __restrict__ rect, Header* __restrict__ hdr,
-            uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
-    __shared__ uint32_t s_off[EMIT_PAIRS + 1];       // pair offsets of the Gaussians this CTA touches
-    __shared__ int s_x0[EMIT_PAIRS], s_y0[EMIT_PAIRS], s_w[EMIT_PAIRS];
-    __shared__ uint32_t s_dbits[EMIT_PAIRS], s_gid[EMIT_PAIRS];
+emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
+            const int4* __restrict__ rect, Header* __restrict__ hdr, uint64_t* __restrict__ words) {
+    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, tile0, w, bits(1/w) (0: use integer division)
+    __shared__ __align__(16) uint16_t s_mark[EMIT_PAIRS];
     __shared__ uint32_t s_hist[MAX_TILE_PASSES * RADIX];
+    __shared__ uint32_t s_wmax[EMIT_WARPS];
     __shared__ uint32_t s_first;
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n_vis = hdr->n_vis;
-    const uint32_t p0 = blockIdx.x * (uint32_t)EMIT_PAIRS, p1 = min(I, p0 + (uint32_t)EMIT_PAIRS);
+    const uint32_t units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
     for (int b = tid; b < tile_passes * RADIX; b += EMIT_THREADS) s_hist[b] = 0u;
-    if (tid == 0) {      // last Gaussian (in depth order) whose offset is <= p0
-        uint32_t lo = 0, hi = n_vis;                 // invariant: voff[lo] <= p0, (hi == n_vis or voff[hi] > p0)
-        while (hi - lo > 1) {
-            const uint32_t mid = (lo + hi) >> 1;
-            if (voff[mid] <= p0) lo = mid; else hi = mid;
+
+    for (uint32_t unit = blockIdx.x; unit < units; unit += gridDim.x) {
+        const uint32_t p0 = unit * (uint32_t)EMIT_PAIRS, p1 = min(I, p0 + (uint32_t)EMIT_PAIRS);
+        __syncthreads();                              // previous unit done with the shared arrays
+        reinterpret_cast<uint4*>(s_mark)[tid] = make_uint4(0u, 0u, 0u, 0u);      // 8 marks per thread
+        if (warp == 0) {                              // last Gaussian (in depth order) whose offset is <= p0
+            const uint32_t ub = warp_upper_bound(voff, n_vis, p0, lane);
+            if (lane == 0) s_first = ub - 1u;         // voff[0] == 0 <= p0, so ub >= 1
         }
-        s_first = lo;
-    }
-    __syncthreads();
-    const uint32_t first = s_first;
-    // Gaussians first .. first+cnt-1 cover [p0, p1); cnt <= EMIT_PAIRS because every listed Gaussian
-    // after the first starts inside the range
-    uint32_t cnt = 0;
-    for (uint32_t k = tid; k < (uint32_t)EMIT_PAIRS; k += EMIT_THREADS) {
-        const uint32_t s = first + k;
-        uint32_t off = 0xffffffffu;
-        if (s < n_vis) off = voff[s];
-        if (s < n_vis && off < p1) {
-            const uint32_t g = vidx[s];
-            const int4 r = rect[g];
-            s_off[k] = off; s_x0[k] = r.x; s_y0[k] = r.y; s_w[k] = r.z - r.x; s_dbits[k] = vkey[s]; s_gid[k] = g;
-        } else {
-            s_off[k] = 0xffffffffu;                  // sentinel: never <= a pair index
+        __syncthreads();
+        const uint32_t first = s_first;
+        // Gaussians first .. first+cnt-1 cover [p0, p1); cnt <= EMIT_PAIRS because every listed Gaussian
+        // after the first starts inside the range (each owns at least one pair)
+        for (uint32_t k = tid; k < (uint32_t)EMIT_PAIRS; k += EMIT_THREADS) {
+            const uint32_t s = first + k;
+            if (s >= n_vis) break;
+            const uint32_t off = voff[s];
+            if (off >= p1) break;
+            const int4 r = rect[vidx[s]];
+            const uint32_t w = (uint32_t)(r.z - r.x), h = (uint32_t)(r.w - r.y);
+            // r / w by a reciprocal (one fix-up step) is exact while the quotient is below 2^22
+            const float rcp = (h < (1u << 22)) ? __frcp_rz((float)w) : 0.0f;
+            s_slot[k] = make_uint4(off, (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, w, __float_as_uint(rcp));
+            s_mark[off > p0 ? off - p0 : 0u] = (uint16_t)k;
         }
-    }
-    if (tid == 0) s_off[EMIT_PAIRS] = 0xffffffffu;
-    __syncthreads();
-    (void)cnt;
+        __syncthreads();
+        {   // inclusive max-scan of the marks (thread t owns positions 8t .. 8t+7): slot of every pair
+            uint4 mv = reinterpret_cast<uint4*>(s_mark)[tid];
+            uint32_t m[8] = {mv.x & 0xffffu, mv.x >> 16, mv.y & 0xffffu, mv.y >> 16,
+                             mv.z & 0xffffu, mv.z >> 16, mv.w & 0xffffu, mv.w >> 16};
 #pragma unroll
-    for (int it = 0; it < EMIT_PPT; ++it) {
-        const uint32_t j = p0 + (uint32_t)it * EMIT_THREADS + tid;
-        const bool valid = j < p1;
-        uint32_t tile = 0;
-        if (valid) {
-            int lo = 0, hi = EMIT_PAIRS;             // invariant: s_off[lo] <= j < s_off[hi]
+            for (int q = 1; q < 8; ++q) m[q] = max(m[q], m[q - 1]);
+            uint32_t incl = m[7];
 #pragma unroll
-            for (int q = 0; q < 10; ++q) {
-                const int mid = (lo + hi) >> 1;
-                if (s_off[mid] <= j) lo = mid; else hi = mid;
+            for (int o = 1; o < 32; o <<= 1) incl = max(incl, __shfl_up_sync(0xffffffffu, incl, o));
+            if (lane == 31) s_wmax[warp] = incl;
+            uint32_t excl = __shfl_up_sync(0xffffffffu, incl, 1);
+            if (lane == 0) excl = 0u;
+            __syncthreads();
+#pragma unroll
+            for (int w = 0; w < EMIT_WARPS; ++w)
+                if (w < warp) excl = max(excl, s_wmax[w]);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) m[q] = max(m[q], excl);
+            reinterpret_cast<uint4*>(s_mark)[tid] = make_uint4(m[0] | (m[1] << 16), m[2] | (m[3] << 16),
+                                                               m[4] | (m[5] << 16), m[6] | (m[7] << 16));
+        }
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < EMIT_PPT; ++it) {
+            const uint32_t j = p0 + (uint32_t)it * EMIT_THREADS + (uint32_t)tid;
+            const bool valid = j < p1;
+            uint32_t tile = 0;
+            if (valid) {
+                const uint32_t k = s_mark[j - p0];
+                const uint4 sl = s_slot[k];
+                const uint32_t r = j - sl.x, w = sl.z;
+                uint32_t ry;
+                if (sl.w != 0u) {
+                    ry = (uint32_t)__float2uint_rz(__fmul_rz(__uint2float_rz(r), __uint_as_float(sl.w)));   // ry or ry - 1
+                    if (r - ry * w >= w) ++ry;
+                } else {
+                    ry = r / w;
+                }
+                tile = sl.y + ry * (uint32_t)TW + (r - ry * w);
+                words[j] = ((uint64_t)tile << 32) | (uint64_t)(first + k);
+                atomicAdd(&s_hist[tile & 255u], 1u);      // consecutive tiles -> distinct banks
             }
-            const uint32_t r = j - s_off[lo];
-            const uint32_t w = (uint32_t)s_w[lo];
-            const uint32_t ry = r / w, rx = r - ry * w;
-            tile = (uint32_t)(s_y0[lo] + (int)ry) * (uint32_t)TW + (uint32_t)(s_x0[lo] + (int)rx);
-            keys[j] = ((uint64_t)tile << 32) | (uint64_t)s_dbits[lo];
-            vals[j] = s_gid[lo];
-            if (tile_passes > 0) atomicAdd(&s_hist[tile & 255u], 1u);   // consecutive tiles -> distinct banks
-        }
-        // higher tile digits are nearly warp-uniform: aggregate with match.any before the atomic
-        for (int d = 1; d < tile_passes; ++d) {
-            const uint32_t dig = valid ? ((tile >> (8 * d)) & 255u) : 0xffffffffu;
-            const uint32_t peers = __match_any_sync(0xffffffffu, dig);
-            if (valid && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_hist[d * RADIX + dig], (uint32_t)__popc(peers));
+            // higher tile digits are nearly warp-uniform: aggregate with match.any before the atomic
+            for (int d = 1; d < tile_passes; ++d) {
+                const uint32_t dig = valid ? ((tile >> (8 * d)) & 255u) : 0xffffffffu;
+                const uint32_t peers = __match_any_sync(0xffffffffu, dig);
+                if (valid && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_hist[d * RADIX + dig], (uint32_t)__popc(peers));
+            }
         }
     }
     __syncthreads();
@@ -301,12 +403,14 @@ emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vk
 }
 
 // ---------------------------------------------------------------------------------------------
-// onesweep digit pass (KeyT = uint32_t for Gaussians, uint64_t for pairs)
+// onesweep digit pass.  MODE 0: 32-bit keys + 32-bit values (the depth passes on Gaussians);
+// MODE 1: 64-bit packed words tile << 32 | rank, no value; MODE 2: like 1, and the scatter expands
+// each word to key = tile << 32 | tab_key[rank], value = tab_val[rank] (the last tile pass).
 // ---------------------------------------------------------------------------------------------
-template <class KeyT, int IPT>
+template <class KeyT, int IPT, bool HAS_VAL>
 struct SortSmem {
     KeyT keys[SORT_THREADS * IPT];
-    uint32_t vals[SORT_THREADS * IPT];
+    uint32_t vals[HAS_VAL ? SORT_THREADS * IPT : 1];
     uint32_t warp_hist[SORT_WARPS][RADIX];
     uint32_t cta_excl[RADIX];     // exclusive digit offsets inside the tile
     uint32_t gbase[RADIX];        // global position of digit d's first key of this tile, minus cta_excl[d]
@@ -316,162 +420,206 @@ struct SortSmem {
 
 // BALLOT = true: peer mask from 8 ballots (cost independent of the digit distribution);
 // false: match.any (fast when a warp holds few distinct digits, slow when it holds 32).
-template <class KeyT, int IPT, bool BALLOT>
-__global__ void __launch_bounds__(SORT_THREADS)
+#ifndef XPR_SORT_MINB64
+#define XPR_SORT_MINB64 3
+#endif
+template <class KeyT, int IPT, bool BALLOT, int MODE>
+__global__ void __launch_bounds__(SORT_THREADS, sizeof(KeyT) == 8 ? XPR_SORT_MINB64 : 4)
 onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* __restrict__ n_dev64, int shift,
                 int hist_row, int ticket_row, const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                 KeyT* __restrict__ keys_out, uint32_t* __restrict__ vals_out, Header* __restrict__ hdr,
-                uint32_t* __restrict__ status /* [tiles][RADIX] of this pass */) {
+                uint32_t* __restrict__ status /* [tiles][RADIX] of this pass */,
+                const uint32_t* __restrict__ tab_key, const uint32_t* __restrict__ tab_val) {
     constexpr int TILE_KEYS = SORT_THREADS * IPT;
+    constexpr bool HAS_VAL = (MODE == 0);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    SortSmem<KeyT, IPT>& S = *reinterpret_cast<SortSmem<KeyT, IPT>*>(smem_raw);
+    SortSmem<KeyT, IPT, HAS_VAL>& S = *reinterpret_cast<SortSmem<KeyT, IPT, HAS_VAL>*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n = n_dev32 ? *n_dev32 : (uint32_t)*n_dev64;
 
-    if (tid == 0) S.tile_id = atomicAdd(&hdr->sort_ticket[ticket_row], 1u);
+    // global position of digit tid's first key: exclusive scan of the global histogram (same for every tile)
+    uint32_t bin_base;
+    {
+        const uint32_t gh = hdr->hist[hist_row * RADIX + tid];
+        uint32_t inc = gh;
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w) S.warp_hist[w][tid] = 0u;    // SORT_THREADS == RADIX
-    __syncthreads();
-    const uint32_t tile = S.tile_id;
-    if ((uint64_t)tile * TILE_KEYS >= n) return;                      // grid is sized for an upper bound of n
-    const uint32_t tile_base = tile * (uint32_t)TILE_KEYS;
-    const uint32_t tile_n = min((uint32_t)TILE_KEYS, n - tile_base);
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t a = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += a;
+        }
+        if (lane == 31) S.scan_tmp[warp] = inc;
+        __syncthreads();
+        uint32_t pre = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w)
+            if (w < warp) pre += S.scan_tmp[w];
+        bin_base = pre + inc - gh;
+    }
 
-    // warp-striped load: item `it` of lane l of warp w sits at tile_base + w*32*IPT + it*32 + l
-    KeyT key[IPT];
-    uint32_t val[IPT];
-    const uint32_t wofs = (uint32_t)warp * 32u * IPT + (uint32_t)lane;
+    while (true) {
+        __syncthreads();                                                  // previous tile done with shared memory
+        if (tid == 0) S.tile_id = atomicAdd(&hdr->sort_ticket[ticket_row], 1u);
 #pragma unroll
-    for (int it = 0; it < IPT; ++it) {
-        const uint32_t loc = wofs + (uint32_t)it * 32u;
-        if (loc < tile_n) {
-            key[it] = keys_in[tile_base + loc];
-            val[it] = vals_in[tile_base + loc];
-        } else {
-            key[it] = ~(KeyT)0;    // padding: highest digit, ranks after every real key of the tile
-            val[it] = 0u;
+        for (int w = 0; w < SORT_WARPS; ++w) S.warp_hist[w][tid] = 0u;    // SORT_THREADS == RADIX
+        __syncthreads();
+        const uint32_t tile = S.tile_id;
+        if ((uint64_t)tile * TILE_KEYS >= n) break;                       // tickets exhausted
+        const uint32_t tile_base = tile * (uint32_t)TILE_KEYS;
+        const uint32_t tile_n = min((uint32_t)TILE_KEYS, n - tile_base);
+
+        // warp-striped load: item `it` of lane l of warp w sits at tile_base + w*32*IPT + it*32 + l
+        KeyT key[IPT];
+        const uint32_t wofs = (uint32_t)warp * 32u * IPT + (uint32_t)lane;
+#pragma unroll
+        for (int it = 0; it < IPT; ++it) {
+            const uint32_t loc = wofs + (uint32_t)it * 32u;
+            key[it] = (loc < tile_n) ? keys_in[tile_base + loc]
+                                     : ~(KeyT)0;    // padding: highest digit, ranks after every real key of the tile
         }
-    }
-    // stable in-warp ranking: rank = #earlier items of this warp with the same digit
-    uint32_t rank[IPT];
-    const uint32_t lt_mask = (1u << lane) - 1u;
+        // stable in-warp ranking: rank = #earlier items of this warp with the same digit
+        uint16_t rank[IPT];
+        const uint32_t lt_mask = (1u << lane) - 1u;
 #pragma unroll
-    for (int it = 0; it < IPT; ++it) {
-        const uint32_t d = (uint32_t)(key[it] >> shift) & (RADIX - 1);
-        uint32_t peers;
-        if (BALLOT) {
-            peers = 0xffffffffu;
+        for (int it = 0; it < IPT; ++it) {
+            const uint32_t d = (uint32_t)(key[it] >> shift) & (RADIX - 1);
+            uint32_t peers;
+            if (BALLOT) {
+                peers = 0xffffffffu;
 #pragma unroll
-            for (int b = 0; b < RADIX_BITS; ++b) {
-                const bool bit = (d >> b) & 1u;
-                const uint32_t m = __ballot_sync(0xffffffffu, bit);
-                peers &= bit ? m : ~m;
+                for (int b = 0; b < RADIX_BITS; ++b) {
+                    const bool bit = (d >> b) & 1u;
+                    const uint32_t m = __ballot_sync(0xffffffffu, bit);
+                    peers &= bit ? m : ~m;
+                }
+            } else {
+                peers = __match_any_sync(0xffffffffu, d);
             }
-        } else {
-            peers = __match_any_sync(0xffffffffu, d);
-        }
-        const uint32_t lt = peers & lt_mask;
-        uint32_t prev = 0;
-        if (lt == 0u) {                                  // lowest lane of the peer group
-            prev = S.warp_hist[warp][d];
-            S.warp_hist[warp][d] = prev + (uint32_t)__popc(peers);
-        }
-        __syncwarp();
-        prev = __shfl_sync(0xffffffffu, prev, __ffs(peers) - 1);
-        rank[it] = prev + (uint32_t)__popc(lt);
-    }
-    __syncthreads();
-    // per digit (thread tid == digit): exclusive scan over warps, CTA count
-    uint32_t count = 0;
-#pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w) {
-        const uint32_t v = S.warp_hist[w][tid];
-        S.warp_hist[w][tid] = count;
-        count += v;
-    }
-    // the last tile's padding was counted in digit RADIX-1: remove it from what look-back publishes
-    uint32_t real_count = count;
-    if (tid == RADIX - 1) real_count -= (uint32_t)TILE_KEYS - tile_n;
-    // block exclusive scan over digits of `count` -> cta_excl; and of the global histogram -> bin base
-    const uint32_t gh = hdr->hist[hist_row * RADIX + tid];
-    uint32_t inc_c = count, inc_g = gh;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t a = __shfl_up_sync(0xffffffffu, inc_c, o), b = __shfl_up_sync(0xffffffffu, inc_g, o);
-        if (lane >= o) { inc_c += a; inc_g += b; }
-    }
-    if (lane == 31) { S.scan_tmp[warp] = inc_c; S.cta_excl[warp] = inc_g; }   // cta_excl reused as scratch
-    __syncthreads();
-    uint32_t pre_c = 0, pre_g = 0;
-#pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w)
-        if (w < warp) { pre_c += S.scan_tmp[w]; pre_g += S.cta_excl[w]; }
-    __syncthreads();
-    const uint32_t excl_c = pre_c + inc_c - count;        // position of digit tid inside the tile
-    const uint32_t bin_base = pre_g + inc_g - gh;         // global position of digit tid's first key
-    S.cta_excl[tid] = excl_c;
-    // decoupled look-back over earlier tiles, one thread per digit
-    uint32_t* my = status + (size_t)tile * RADIX + tid;
-    uint32_t excl_prev = 0;
-    if (tile == 0) {
-        st_relaxed(my, FLAG_INCLUSIVE | real_count);
-    } else {
-        st_relaxed(my, FLAG_PARTIAL | real_count);
-        const uint32_t* p = my - RADIX;
-        uint32_t remaining = tile;
-        bool found = false;
-        while (!found) {   // 4 predecessors in flight per round; before tile 0: virtual inclusive 0
-            uint32_t sv[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-                sv[k] = ((uint32_t)k < remaining) ? ld_relaxed(p - k * RADIX) : FLAG_INCLUSIVE;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                if (found) break;
-                while ((sv[k] & FLAG_MASK) == 0u) sv[k] = ld_relaxed(p - k * RADIX);
-                excl_prev += sv[k] & VALUE_MASK;
-                found = (sv[k] & FLAG_MASK) == FLAG_INCLUSIVE;
+            const uint32_t lt = peers & lt_mask;
+            uint32_t prev = 0;
+            if (lt == 0u) {                                  // lowest lane of the peer group
+                prev = S.warp_hist[warp][d];
+                S.warp_hist[warp][d] = prev + (uint32_t)__popc(peers);
             }
-            p -= 4 * RADIX;
-            remaining = (remaining > 4u) ? remaining - 4u : 0u;
+            __syncwarp();
+            prev = __shfl_sync(0xffffffffu, prev, __ffs(peers) - 1);
+            rank[it] = (uint16_t)(prev + (uint32_t)__popc(lt));
         }
-        st_relaxed(my, FLAG_INCLUSIVE | (excl_prev + real_count));
-    }
-    S.gbase[tid] = bin_base + excl_prev - excl_c;
-    __syncthreads();
-    // scatter into shared memory in tile-sorted order
+        __syncthreads();
+        // per digit (thread tid == digit): exclusive scan over warps, CTA count
+        uint32_t count = 0;
 #pragma unroll
-    for (int it = 0; it < IPT; ++it) {
-        const uint32_t d = (uint32_t)(key[it] >> shift) & (RADIX - 1);
-        const uint32_t pos = S.cta_excl[d] + S.warp_hist[warp][d] + rank[it];
-        S.keys[pos] = key[it];
-        S.vals[pos] = val[it];
-    }
-    __syncthreads();
-    // coalesced runs to global memory (padding sits at positions >= tile_n)
+        for (int w = 0; w < SORT_WARPS; ++w) {
+            const uint32_t v = S.warp_hist[w][tid];
+            S.warp_hist[w][tid] = count;
+            count += v;
+        }
+        // the last tile's padding was counted in digit RADIX-1: remove it from what look-back publishes
+        uint32_t real_count = count;
+        if (tid == RADIX - 1) real_count -= (uint32_t)TILE_KEYS - tile_n;
+        // block exclusive scan over digits of `count` -> cta_excl
+        uint32_t inc_c = count;
 #pragma unroll
-    for (int it = 0; it < IPT; ++it) {
-        const uint32_t p = (uint32_t)it * SORT_THREADS + (uint32_t)tid;
-        if (p < tile_n) {
-            const KeyT k = S.keys[p];
-            const uint32_t d = (uint32_t)(k >> shift) & (RADIX - 1);
-            const uint32_t dst = S.gbase[d] + p;
-            keys_out[dst] = k;
-            vals_out[dst] = S.vals[p];
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t a = __shfl_up_sync(0xffffffffu, inc_c, o);
+            if (lane >= o) inc_c += a;
+        }
+        if (lane == 31) S.scan_tmp[warp] = inc_c;
+        // decoupled look-back over earlier tiles, one thread per digit (overlaps the scan's barrier)
+        uint32_t* my = status + (size_t)tile * RADIX + tid;
+        uint32_t excl_prev = 0;
+        if (tile == 0) {
+            st_relaxed(my, FLAG_INCLUSIVE | real_count);
+        } else {
+            st_relaxed(my, FLAG_PARTIAL | real_count);
+            const uint32_t* p = my - RADIX;
+            uint32_t remaining = tile;
+            bool found = false;
+            while (!found) {   // 4 predecessors in flight per round; before tile 0: virtual inclusive 0
+                uint32_t sv[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    sv[k] = ((uint32_t)k < remaining) ? ld_relaxed(p - k * RADIX) : FLAG_INCLUSIVE;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    if (found) break;
+                    while ((sv[k] & FLAG_MASK) == 0u) sv[k] = ld_relaxed(p - k * RADIX);
+                    excl_prev += sv[k] & VALUE_MASK;
+                    found = (sv[k] & FLAG_MASK) == FLAG_INCLUSIVE;
+                }
+                p -= 4 * RADIX;
+                remaining = (remaining > 4u) ? remaining - 4u : 0u;
+            }
+            st_relaxed(my, FLAG_INCLUSIVE | (excl_prev + real_count));
+        }
+        __syncthreads();
+        uint32_t pre_c = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w)
+            if (w < warp) pre_c += S.scan_tmp[w];
+        const uint32_t excl_c = pre_c + inc_c - count;        // position of digit tid inside the tile
+        S.cta_excl[tid] = excl_c;
+        S.gbase[tid] = bin_base + excl_prev - excl_c;
+        __syncthreads();
+        // scatter into shared memory in tile-sorted order (values are loaded only now: fewer live registers)
+#pragma unroll
+        for (int it = 0; it < IPT; ++it) {
+            const uint32_t d = (uint32_t)(key[it] >> shift) & (RADIX - 1);
+            const uint32_t pos = S.cta_excl[d] + S.warp_hist[warp][d] + rank[it];
+            S.keys[pos] = key[it];
+            if constexpr (HAS_VAL) {
+                const uint32_t loc = wofs + (uint32_t)it * 32u;
+                S.vals[pos] = (loc < tile_n) ? vals_in[tile_base + loc] : 0u;
+            }
+        }
+        __syncthreads();
+        // coalesced runs to global memory (padding sits at positions >= tile_n)
+#pragma unroll
+        for (int it = 0; it < IPT; ++it) {
+            const uint32_t p = (uint32_t)it * SORT_THREADS + (uint32_t)tid;
+            if (p < tile_n) {
+                const KeyT k = S.keys[p];
+                const uint32_t d = (uint32_t)(k >> shift) & (RADIX - 1);
+                const uint32_t dst = S.gbase[d] + p;
+                if constexpr (MODE == 2) {
+                    const uint32_t r = (uint32_t)k;
+                    keys_out[dst] = (k & ~(KeyT)0xffffffffu) | (KeyT)__ldg(tab_key + r);
+                    vals_out[dst] = __ldg(tab_val + r);
+                } else {
+                    keys_out[dst] = k;
+                    if constexpr (HAS_VAL) vals_out[dst] = S.vals[p];
+                }
+            }
         }
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// per-tile bounds ("records each segment's start b_j and count c_j")
+// per-tile bounds ("records each segment's start b_j and count c_j"): one warp per tile
+// finds the first sorted key of tile t and of tile t+1 by a 32-ary search; an empty tile gets (0, 0).
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t warp_lower_bound_tile(const uint64_t* __restrict__ keys, uint32_t n, uint32_t t,
+                                                          int lane) {
+    uint32_t lo = 0, hi = n;                   // answer in [lo, hi]; hi == n or tile(keys[hi]) >= t
+    while (hi > lo) {
+        const uint32_t len = hi - lo, stride = (len + 31u) / 32u;
+        const uint32_t probe = min(lo + ((uint32_t)lane + 1u) * stride - 1u, hi - 1u);
+        const uint32_t b = __ballot_sync(0xffffffffu, (uint32_t)(keys[probe] >> 32) >= t);
+        if (b == 0u) { lo = hi; break; }
+        const uint32_t f = (uint32_t)__ffs(b) - 1u;
+        hi = min(lo + (f + 1u) * stride - 1u, hi - 1u);
+        lo = lo + f * stride;
+    }
+    return lo;
+}
+
 __global__ void __launch_bounds__(256)
-ranges_kernel(uint32_t I, const uint64_t* __restrict__ keys, uint32_t* __restrict__ ranges) {
-    const uint32_t j = blockIdx.x * 256u + threadIdx.x;
-    if (j >= I) return;
-    const uint32_t t = (uint32_t)(keys[j] >> 32);
-    if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != t) ranges[2 * t] = j;
-    if (j == I - 1 || (uint32_t)(keys[j + 1] >> 32) != t) ranges[2 * t + 1] = j + 1;
+ranges_kernel(uint32_t I, uint32_t T, const uint64_t* __restrict__ keys, uint32_t* __restrict__ ranges) {
+    const uint32_t t = blockIdx.x * 8u + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (t >= T) return;
+    const uint32_t b = warp_lower_bound_tile(keys, I, t, lane);
+    const uint32_t e = warp_lower_bound_tile(keys, I, t + 1u, lane);
+    if (lane == 0) reinterpret_cast<uint2*>(ranges)[t] = (e > b) ? make_uint2(b, e) : make_uint2(0u, 0u);
 }
 
 }  // namespace
@@ -486,18 +634,19 @@ extern "C" int32_t xpr_bin_sort_workspace(int64_t N, int64_t pair_capacity, int3
     return XPR_OK;
 }
 
-template <class KeyT, int IPT, bool BALLOT>
-static cudaError_t launch_pass(unsigned grid, cudaStream_t st, const uint32_t* n32, const unsigned long long* n64,
+template <class KeyT, int IPT, bool BALLOT, int MODE>
+static cudaError_t launch_pass(unsigned tiles, cudaStream_t st, const uint32_t* n32, const unsigned long long* n64,
                                int shift, int row, const KeyT* kin, const uint32_t* vin, KeyT* kout, uint32_t* vout,
-                               Header* hdr, uint32_t* status) {
-    const size_t smem = sizeof(SortSmem<KeyT, IPT>);
+                               Header* hdr, uint32_t* status, const uint32_t* tab_key, const uint32_t* tab_val) {
+    const size_t smem = sizeof(SortSmem<KeyT, IPT, MODE == 0>);
     if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(onesweep_kernel<KeyT, IPT, BALLOT>,
+        cudaError_t e = cudaFuncSetAttribute(onesweep_kernel<KeyT, IPT, BALLOT, MODE>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    onesweep_kernel<KeyT, IPT, BALLOT><<<grid, SORT_THREADS, smem, st>>>(n32, n64, shift, row, row, kin, vin, kout,
-                                                                        vout, hdr, status);
+    const unsigned grid = tiles < (unsigned)PERSIST_CTAS ? tiles : (unsigned)PERSIST_CTAS;
+    onesweep_kernel<KeyT, IPT, BALLOT, MODE><<<grid, SORT_THREADS, smem, st>>>(n32, n64, shift, row, row, kin, vin, kout,
+                                                                              vout, hdr, status, tab_key, tab_val);
     return cudaGetLastError();
 }
 
@@ -520,68 +669,76 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     cudaStream_t st = (cudaStream_t)stream;
     unsigned char* ws = static_cast<unsigned char*>(workspace);
     Header* hdr = reinterpret_cast<Header*>(ws + L.header);
-    const size_t scan_blocks = ((size_t)N + SCAN_THREADS - 1) / SCAN_THREADS;
+    const size_t scan_blocks = ((size_t)N + SCAN_ITEMS - 1) / SCAN_ITEMS;
     unsigned long long* compact_status = reinterpret_cast<unsigned long long*>(ws + L.scan_status);
-    unsigned long long* emit_status = compact_status + scan_blocks + 1;
+    unsigned long long* offsets_status = compact_status + scan_blocks + 1;
     uint32_t* vkey[2] = {reinterpret_cast<uint32_t*>(ws + L.vkey0), reinterpret_cast<uint32_t*>(ws + L.vkey1)};
     uint32_t* vidx[2] = {reinterpret_cast<uint32_t*>(ws + L.vidx0), reinterpret_cast<uint32_t*>(ws + L.vidx1)};
     uint32_t* status32 = reinterpret_cast<uint32_t*>(ws + L.status32);
     uint64_t* keys_tmp = reinterpret_cast<uint64_t*>(ws + L.keys_tmp);
-    uint32_t* vals_tmp = reinterpret_cast<uint32_t*>(ws + L.vals_tmp);
     uint32_t* status64 = reinterpret_cast<uint32_t*>(ws + L.status64);
     const int tpasses = tile_passes_for(T);
 
-    XPR_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)T, st));
     *num_pairs_host = 0;
-    if (N == 0) return XPR_OK;
+    if (N == 0) {
+        XPR_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)T, st));
+        return XPR_OK;
+    }
     XPR_CUDA(cudaMemsetAsync(ws + L.header, 0, L.vkey0 - L.header, st));   // header, scan chains, status32
     // 1. visible Gaussians (index order) + depth-digit histograms
     compact_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(N, depth, tile_count, hdr, compact_status, vkey[0],
                                                                    vidx[0]);
     XPR_LAUNCH_CHECK();
-    // 2. the four depth digits, on the N_vis Gaussians (grid sized for N; surplus CTAs exit)
+    // 2. the four depth digits, on the N_vis Gaussians (tiles counted for N; surplus tickets end the loop)
     const unsigned tiles32 = (unsigned)(((size_t)N + SORT_THREADS * IPT32 - 1) / (SORT_THREADS * IPT32));
     for (int p = 0; p < DEPTH_PASSES; ++p) {
         uint32_t* status = status32 + (size_t)p * RADIX * tiles32;
         const int a = p & 1, b = a ^ 1;
         cudaError_t e = (p < 3)   // mantissa bytes: ~32 distinct digits per warp -> ballot ranking
-            ? launch_pass<uint32_t, IPT32, true>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status)
-            : launch_pass<uint32_t, IPT32, false>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status);
+            ? launch_pass<uint32_t, IPT32, true, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr)
+            : launch_pass<uint32_t, IPT32, false, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr);
         XPR_CUDA(e);
     }   // DEPTH_PASSES is even: the sorted list is back in vkey[0] / vidx[0]
     // 3. pair offsets in depth order and the pair count I (the one host read-back)
     uint32_t* voff = vkey[1];                          // free after the depth passes
-    offsets_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], tile_count, hdr, emit_status, voff);
+    offsets_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], tile_count, hdr, offsets_status, voff);
     XPR_LAUNCH_CHECK();
     unsigned long long total = 0;
     XPR_CUDA(cudaMemcpyAsync(&total, &hdr->total_pairs, sizeof(total), cudaMemcpyDeviceToHost, st));
     XPR_CUDA(cudaStreamSynchronize(st));
     *num_pairs_host = (int64_t)total;
     if ((int64_t)total > pair_capacity) return XPR_ERR_CAPACITY;
-    if (total == 0) return XPR_OK;
+    if (total == 0) {
+        XPR_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)T, st));
+        return XPR_OK;
+    }
     const uint32_t I = (uint32_t)total;
-    // replicate in depth order; an even number of tile passes ends in the buffer emission wrote to
-    uint64_t* k0 = (tpasses % 2 == 0) ? keys_sorted : keys_tmp;
-    uint32_t* v0 = (tpasses % 2 == 0) ? vals_sorted : vals_tmp;
-    uint64_t* k1 = (tpasses % 2 == 0) ? keys_tmp : keys_sorted;
-    uint32_t* v1 = (tpasses % 2 == 0) ? vals_tmp : vals_sorted;
-    emit_kernel<<<(I + EMIT_PAIRS - 1) / EMIT_PAIRS, EMIT_THREADS, 0, st>>>(
-        I, TW, tpasses, vkey[0], vidx[0], voff, reinterpret_cast<const int4*>(tile_rect), hdr, k0, v0);
+    // 4. replicate in depth order as packed words; pass p reads buffer p and writes buffer p+1, the last
+    //    one writes keys_sorted / vals_sorted, so emission starts in keys_sorted when tpasses is even
+    uint64_t* w0 = (tpasses % 2 == 0) ? keys_sorted : keys_tmp;
+    uint64_t* w1 = (tpasses % 2 == 0) ? keys_tmp : keys_sorted;
+    const unsigned units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
+    emit_kernel<<<units < (unsigned)PERSIST_CTAS ? units : (unsigned)PERSIST_CTAS, EMIT_THREADS, 0, st>>>(
+        I, TW, tpasses, vidx[0], voff, reinterpret_cast<const int4*>(tile_rect), hdr, w0);
     XPR_LAUNCH_CHECK();
-    // 4. the tile-id digits, on the I pairs
+    // 5. the tile-id digits, on the I pairs
     const unsigned tiles64 = (I + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
-    if (tpasses > 0) XPR_CUDA(cudaMemsetAsync(status64, 0, sizeof(uint32_t) * (size_t)RADIX * tiles64 * (size_t)tpasses, st));
+    XPR_CUDA(cudaMemsetAsync(status64, 0, sizeof(uint32_t) * (size_t)RADIX * tiles64 * (size_t)tpasses, st));
     for (int p = 0; p < tpasses; ++p) {
         uint32_t* status = status64 + (size_t)p * RADIX * tiles64;
-        const int row = DEPTH_PASSES + p;
-        cudaError_t e = (p == 0)  // consecutive pairs of a Gaussian are consecutive tiles -> ballot ranking
-            ? launch_pass<uint64_t, IPT64, true>(tiles64, st, nullptr, &hdr->total_pairs, 32 + 8 * p, row, k0, v0, k1, v1, hdr, status)
-            : launch_pass<uint64_t, IPT64, false>(tiles64, st, nullptr, &hdr->total_pairs, 32 + 8 * p, row, k0, v0, k1, v1, hdr, status);
+        const int row = DEPTH_PASSES + p, shift = 32 + 8 * p;
+        const bool last = (p == tpasses - 1);
+        cudaError_t e;
+        // digit 0: consecutive pairs of a Gaussian are consecutive tiles -> ballot ranking
+        if (!last)       e = (p == 0) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
+                                      : launch_pass<uint64_t, IPT64, false, 1>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr);
+        else             e = (p == 0) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
+                                      : launch_pass<uint64_t, IPT64, false, 2>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0]);
         XPR_CUDA(e);
-        uint64_t* tk = k0; k0 = k1; k1 = tk;
-        uint32_t* tv = v0; v0 = v1; v1 = tv;
+        uint64_t* t = w0; w0 = w1; w1 = t;
     }
-    ranges_kernel<<<(I + 255) / 256, 256, 0, st>>>(I, keys_sorted, tile_ranges);
+    // 6. per-tile ranges
+    ranges_kernel<<<((unsigned)T + 7) / 8, 256, 0, st>>>(I, (uint32_t)T, keys_sorted, tile_ranges);
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }
