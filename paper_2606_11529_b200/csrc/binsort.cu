@@ -14,7 +14,9 @@
 //  (2) once the Gaussians are in (depth, index) order, a pair only has to carry its tile id and the
 //      RANK of its Gaussian in that order: the tile passes move 8-byte words (tile << 32 | rank), and
 //      the last pass expands them to the 64-bit key (tile << 32 | depth bits) and the 32-bit value
-//      (Gaussian index) through two small L2-resident tables.
+//      (Gaussian index) through two rank-indexed tables.  The expansion happens while the words are
+//      still in the INPUT order of that pass, where neighbouring lanes hold neighbouring ranks, so
+//      the gathers are coalesced (a gather in output order costs one 32-byte sector per pair).
 // The result is bit-identical to sorting the I (key, value) pairs by all digits; HBM traffic per pair
 // drops from 12 + 6*24 + 8 = 164 bytes to 8 + 16 + 20 = 44 bytes.
 //
@@ -310,7 +312,7 @@ constexpr int EMIT_WARPS = EMIT_THREADS / 32;
 __global__ void __launch_bounds__(EMIT_THREADS)
 emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
             const int4* __restrict__ rect, Header* __restrict__ hdr, uint64_t* __restrict__ words) {
-    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, tile0, w, bits(1/w) (0: use integer division)
+    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, first tile id, rectangle width, unused
     __shared__ __align__(16) uint16_t s_mark[EMIT_PAIRS];
     __shared__ uint32_t s_hist[MAX_TILE_PASSES * RADIX];
     __shared__ uint32_t s_wmax[EMIT_WARPS];
@@ -338,10 +340,7 @@ emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vi
             const uint32_t off = voff[s];
             if (off >= p1) break;
             const int4 r = rect[vidx[s]];
-            const uint32_t w = (uint32_t)(r.z - r.x), h = (uint32_t)(r.w - r.y);
-            // r / w by a reciprocal (one fix-up step) is exact while the quotient is below 2^22
-            const float rcp = (h < (1u << 22)) ? __frcp_rz((float)w) : 0.0f;
-            s_slot[k] = make_uint4(off, (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, w, __float_as_uint(rcp));
+            s_slot[k] = make_uint4(off, (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, (uint32_t)(r.z - r.x), 0u);
             s_mark[off > p0 ? off - p0 : 0u] = (uint16_t)k;
         }
         __syncthreads();
@@ -376,9 +375,10 @@ emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vi
                 const uint32_t k = s_mark[j - p0];
                 const uint4 sl = s_slot[k];
                 const uint32_t r = j - sl.x, w = sl.z;
+                // r / w by a reciprocal (one fix-up step): exact while the quotient is below 2^22
                 uint32_t ry;
-                if (sl.w != 0u) {
-                    ry = (uint32_t)__float2uint_rz(__fmul_rz(__uint2float_rz(r), __uint_as_float(sl.w)));   // ry or ry - 1
+                if (r < (1u << 22)) {
+                    ry = (uint32_t)__float2uint_rz(__fmul_rz(__uint2float_rz(r), __frcp_rz(__uint2float_rz(w))));   // ry or ry - 1
                     if (r - ry * w >= w) ++ry;
                 } else {
                     ry = r / w;
@@ -404,39 +404,53 @@ emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vi
 
 // ---------------------------------------------------------------------------------------------
 // onesweep digit pass.  MODE 0: 32-bit keys + 32-bit values (the depth passes on Gaussians);
-// MODE 1: 64-bit packed words tile << 32 | rank, no value; MODE 2: like 1, and the scatter expands
-// each word to key = tile << 32 | tab_key[rank], value = tab_val[rank] (the last tile pass).
+// MODE 1: 64-bit packed words tile << 32 | rank, no value; MODE 2: the last tile pass: reads words and,
+// when staging them in shared memory, expands each to key = tile << 32 | tab_key[rank], value = tab_val[rank].
 // ---------------------------------------------------------------------------------------------
 template <class KeyT, int IPT, bool HAS_VAL>
 struct SortSmem {
     KeyT keys[SORT_THREADS * IPT];
     uint32_t vals[HAS_VAL ? SORT_THREADS * IPT : 1];
     uint32_t warp_hist[SORT_WARPS][RADIX];
+    uint32_t bitmap[SORT_WARPS][RADIX];   // BITMAP ranking: bit l of bitmap[w][d] = lane l of warp w holds digit d
     uint32_t cta_excl[RADIX];     // exclusive digit offsets inside the tile
     uint32_t gbase[RADIX];        // global position of digit d's first key of this tile, minus cta_excl[d]
     uint32_t scan_tmp[SORT_WARPS];
     uint32_t tile_id;
 };
 
-// BALLOT = true: peer mask from 8 ballots (cost independent of the digit distribution);
-// false: match.any (fast when a warp holds few distinct digits, slow when it holds 32).
-#ifndef XPR_SORT_MINB64
-#define XPR_SORT_MINB64 3
+// BITMAP = true: the peer mask of a lane (lanes of its warp holding the same digit) is built in shared
+// memory: every lane ORs its bit into bitmap[warp][digit] and reads the word back -- 3 shared-memory
+// instructions instead of 8 ballots x 5 ALU instructions; conflict-free when the digits of a warp are
+// distinct (mantissa bytes, consecutive tile ids), 32-way serialised when they are all equal.
+// false: match.any (fast when a warp holds few distinct digits: the high tile digit).
+#ifndef XPR_P2_BITMAP
+#define XPR_P2_BITMAP 0
 #endif
-template <class KeyT, int IPT, bool BALLOT, int MODE>
-__global__ void __launch_bounds__(SORT_THREADS, sizeof(KeyT) == 8 ? XPR_SORT_MINB64 : 4)
+#ifndef XPR_P1_BITMAP
+#define XPR_P1_BITMAP 1
+#endif
+#ifndef XPR_SORT_MINB64
+#define XPR_SORT_MINB64 4
+#endif
+template <class KeyT, int IPT, bool BITMAP, int MODE>
+__global__ void __launch_bounds__(SORT_THREADS, MODE == 2 ? 3 : (sizeof(KeyT) == 8 ? XPR_SORT_MINB64 : 4))   // MODE 2: 66 KB of shared memory
 onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* __restrict__ n_dev64, int shift,
                 int hist_row, int ticket_row, const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                 KeyT* __restrict__ keys_out, uint32_t* __restrict__ vals_out, Header* __restrict__ hdr,
                 uint32_t* __restrict__ status /* [tiles][RADIX] of this pass */,
                 const uint32_t* __restrict__ tab_key, const uint32_t* __restrict__ tab_val) {
     constexpr int TILE_KEYS = SORT_THREADS * IPT;
-    constexpr bool HAS_VAL = (MODE == 0);
+    constexpr bool HAS_VAL = (MODE != 1);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     SortSmem<KeyT, IPT, HAS_VAL>& S = *reinterpret_cast<SortSmem<KeyT, IPT, HAS_VAL>*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n = n_dev32 ? *n_dev32 : (uint32_t)*n_dev64;
 
+    if (BITMAP) {
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) S.bitmap[w][tid] = 0u;
+    }
     // global position of digit tid's first key: exclusive scan of the global histogram (same for every tile)
     uint32_t bin_base;
     {
@@ -483,14 +497,11 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
         for (int it = 0; it < IPT; ++it) {
             const uint32_t d = (uint32_t)(key[it] >> shift) & (RADIX - 1);
             uint32_t peers;
-            if (BALLOT) {
-                peers = 0xffffffffu;
-#pragma unroll
-                for (int b = 0; b < RADIX_BITS; ++b) {
-                    const bool bit = (d >> b) & 1u;
-                    const uint32_t m = __ballot_sync(0xffffffffu, bit);
-                    peers &= bit ? m : ~m;
-                }
+            if (BITMAP) {
+                atomicOr(&S.bitmap[warp][d], 1u << lane);
+                __syncwarp();
+                peers = S.bitmap[warp][d];
+                __syncwarp();                                // everyone has read before the leader clears the word
             } else {
                 peers = __match_any_sync(0xffffffffu, d);
             }
@@ -499,6 +510,7 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
             if (lt == 0u) {                                  // lowest lane of the peer group
                 prev = S.warp_hist[warp][d];
                 S.warp_hist[warp][d] = prev + (uint32_t)__popc(peers);
+                if (BITMAP) S.bitmap[warp][d] = 0u;          // left zero for the next item / tile
             }
             __syncwarp();
             prev = __shfl_sync(0xffffffffu, prev, __ffs(peers) - 1);
@@ -524,13 +536,39 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
             if (lane >= o) inc_c += a;
         }
         if (lane == 31) S.scan_tmp[warp] = inc_c;
-        // decoupled look-back over earlier tiles, one thread per digit (overlaps the scan's barrier)
+        // publish this tile's digit counts at once; the look-back itself runs after the shared-memory
+        // scatter, which gives the predecessors time to publish theirs
         uint32_t* my = status + (size_t)tile * RADIX + tid;
+        st_relaxed(my, (tile == 0 ? FLAG_INCLUSIVE : FLAG_PARTIAL) | real_count);
+        __syncthreads();
+        uint32_t pre_c = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w)
+            if (w < warp) pre_c += S.scan_tmp[w];
+        const uint32_t excl_c = pre_c + inc_c - count;        // position of digit tid inside the tile
+        S.cta_excl[tid] = excl_c;
+        __syncthreads();
+        // scatter into shared memory in tile-sorted order (values are loaded only now: fewer live registers)
+#pragma unroll
+        for (int it = 0; it < IPT; ++it) {
+            const uint32_t d = (uint32_t)(key[it] >> shift) & (RADIX - 1);
+            const uint32_t pos = S.cta_excl[d] + S.warp_hist[warp][d] + rank[it];
+            if constexpr (MODE == 2) {
+                const uint32_t loc = wofs + (uint32_t)it * 32u;
+                const uint32_t r = (loc < tile_n) ? (uint32_t)key[it] : 0u;     // rank; 0 for the padding
+                S.keys[pos] = (key[it] & ~(KeyT)0xffffffffu) | (KeyT)__ldg(tab_key + r);
+                S.vals[pos] = __ldg(tab_val + r);
+            } else {
+                S.keys[pos] = key[it];
+                if constexpr (HAS_VAL) {
+                    const uint32_t loc = wofs + (uint32_t)it * 32u;
+                    S.vals[pos] = (loc < tile_n) ? vals_in[tile_base + loc] : 0u;
+                }
+            }
+        }
+        // decoupled look-back over earlier tiles, one thread per digit
         uint32_t excl_prev = 0;
-        if (tile == 0) {
-            st_relaxed(my, FLAG_INCLUSIVE | real_count);
-        } else {
-            st_relaxed(my, FLAG_PARTIAL | real_count);
+        if (tile != 0) {
             const uint32_t* p = my - RADIX;
             uint32_t remaining = tile;
             bool found = false;
@@ -551,26 +589,7 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
             }
             st_relaxed(my, FLAG_INCLUSIVE | (excl_prev + real_count));
         }
-        __syncthreads();
-        uint32_t pre_c = 0;
-#pragma unroll
-        for (int w = 0; w < SORT_WARPS; ++w)
-            if (w < warp) pre_c += S.scan_tmp[w];
-        const uint32_t excl_c = pre_c + inc_c - count;        // position of digit tid inside the tile
-        S.cta_excl[tid] = excl_c;
         S.gbase[tid] = bin_base + excl_prev - excl_c;
-        __syncthreads();
-        // scatter into shared memory in tile-sorted order (values are loaded only now: fewer live registers)
-#pragma unroll
-        for (int it = 0; it < IPT; ++it) {
-            const uint32_t d = (uint32_t)(key[it] >> shift) & (RADIX - 1);
-            const uint32_t pos = S.cta_excl[d] + S.warp_hist[warp][d] + rank[it];
-            S.keys[pos] = key[it];
-            if constexpr (HAS_VAL) {
-                const uint32_t loc = wofs + (uint32_t)it * 32u;
-                S.vals[pos] = (loc < tile_n) ? vals_in[tile_base + loc] : 0u;
-            }
-        }
         __syncthreads();
         // coalesced runs to global memory (padding sits at positions >= tile_n)
 #pragma unroll
@@ -580,14 +599,8 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
                 const KeyT k = S.keys[p];
                 const uint32_t d = (uint32_t)(k >> shift) & (RADIX - 1);
                 const uint32_t dst = S.gbase[d] + p;
-                if constexpr (MODE == 2) {
-                    const uint32_t r = (uint32_t)k;
-                    keys_out[dst] = (k & ~(KeyT)0xffffffffu) | (KeyT)__ldg(tab_key + r);
-                    vals_out[dst] = __ldg(tab_val + r);
-                } else {
-                    keys_out[dst] = k;
-                    if constexpr (HAS_VAL) vals_out[dst] = S.vals[p];
-                }
+                keys_out[dst] = k;
+                if constexpr (HAS_VAL) vals_out[dst] = S.vals[p];
             }
         }
     }
@@ -634,18 +647,18 @@ extern "C" int32_t xpr_bin_sort_workspace(int64_t N, int64_t pair_capacity, int3
     return XPR_OK;
 }
 
-template <class KeyT, int IPT, bool BALLOT, int MODE>
+template <class KeyT, int IPT, bool BITMAP, int MODE>
 static cudaError_t launch_pass(unsigned tiles, cudaStream_t st, const uint32_t* n32, const unsigned long long* n64,
                                int shift, int row, const KeyT* kin, const uint32_t* vin, KeyT* kout, uint32_t* vout,
                                Header* hdr, uint32_t* status, const uint32_t* tab_key, const uint32_t* tab_val) {
-    const size_t smem = sizeof(SortSmem<KeyT, IPT, MODE == 0>);
+    const size_t smem = sizeof(SortSmem<KeyT, IPT, MODE != 1>);
     if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(onesweep_kernel<KeyT, IPT, BALLOT, MODE>,
+        cudaError_t e = cudaFuncSetAttribute(onesweep_kernel<KeyT, IPT, BITMAP, MODE>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
     const unsigned grid = tiles < (unsigned)PERSIST_CTAS ? tiles : (unsigned)PERSIST_CTAS;
-    onesweep_kernel<KeyT, IPT, BALLOT, MODE><<<grid, SORT_THREADS, smem, st>>>(n32, n64, shift, row, row, kin, vin, kout,
+    onesweep_kernel<KeyT, IPT, BITMAP, MODE><<<grid, SORT_THREADS, smem, st>>>(n32, n64, shift, row, row, kin, vin, kout,
                                                                               vout, hdr, status, tab_key, tab_val);
     return cudaGetLastError();
 }
@@ -694,7 +707,7 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     for (int p = 0; p < DEPTH_PASSES; ++p) {
         uint32_t* status = status32 + (size_t)p * RADIX * tiles32;
         const int a = p & 1, b = a ^ 1;
-        cudaError_t e = (p < 3)   // mantissa bytes: ~32 distinct digits per warp -> ballot ranking
+        cudaError_t e = (p < 3)   // mantissa bytes: ~32 distinct digits per warp -> bitmap ranking
             ? launch_pass<uint32_t, IPT32, true, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr)
             : launch_pass<uint32_t, IPT32, false, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr);
         XPR_CUDA(e);
@@ -729,10 +742,10 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
         const int row = DEPTH_PASSES + p, shift = 32 + 8 * p;
         const bool last = (p == tpasses - 1);
         cudaError_t e;
-        // digit 0: consecutive pairs of a Gaussian are consecutive tiles -> ballot ranking
-        if (!last)       e = (p == 0) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
+        // digit 0: consecutive pairs of a Gaussian are consecutive tiles -> bitmap ranking
+        if (!last)       e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
                                       : launch_pass<uint64_t, IPT64, false, 1>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr);
-        else             e = (p == 0) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
+        else             e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
                                       : launch_pass<uint64_t, IPT64, false, 2>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0]);
         XPR_CUDA(e);
         uint64_t* t = w0; w0 = w1; w1 = t;
