@@ -38,9 +38,8 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                      float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                      unsigned long long* __restrict__ stats) {
-    __shared__ float4 s_geo[BLOCK];   // mx, my, qa, qb
-    __shared__ float4 s_gate[BLOCK];  // qc, thr = -lnv, o, unused
-    __shared__ float4 s_col[BLOCK];   // r, g, b, unused
+    // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, o, - | r, g, b, -)
+    __shared__ float4 s_rec[3 * BLOCK];
     const int tile = blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
     const int px = tx * TILE + (threadIdx.x & (TILE - 1)), py = ty * TILE + (threadIdx.x >> 4);
@@ -54,6 +53,29 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     bool done = !inside;
     uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
 
+    // one list entry against this thread's pixel; `rp` points at its record, `pos` = list position + 1
+#define XPR_FWD_ENTRY(rp, pos)                                                                       \
+    {                                                                                                \
+        const float4 ge = (rp)[0];                                                                   \
+        const float4 ga = (rp)[1];                                                                   \
+        const float dx = pxc - ge.x, dy = pyc - ge.y;                                                \
+        const float power = eval_power(ge.z, ge.w, ga.x, dx, dy);                                    \
+        if (STATS) ++n_visit;                                                                        \
+        /* valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12) */    \
+        if (!(power > 0.0f) && !(power < ga.y)) {                                                    \
+            if (STATS) ++n_pass;                                                                     \
+            const float alpha = fminf(P.amax, ga.z * fast_exp(power));      /* C11 */                \
+            const float Tn = T * (1.0f - alpha);                                                     \
+            if (Tn < P.tmin) { done = true; break; }                        /* C12: stop, no blend */\
+            const float4 c = (rp)[2];                                                                \
+            const float w = alpha * T;                                                               \
+            C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);                     \
+            T = Tn;                                                                                  \
+            last = (pos);                                                                            \
+            if (STATS) ++n_blend;                                                                    \
+        }                                                                                            \
+    }
+
     for (uint32_t base = 0; base < len; base += BLOCK) {
         if (__syncthreads_count(done) == BLOCK) break;
         const uint32_t cnt = min((uint32_t)BLOCK, len - base);
@@ -61,34 +83,28 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             const uint32_t g = vals[rg.x + base + threadIdx.x];
             const float2 m = mean2d[g];
             const float4 co = conic_opac[g];
-            s_geo[threadIdx.x] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-            s_gate[threadIdx.x] = make_float4(-0.5f * co.z, -lnv[g], co.w, 0.0f);
-            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
+            float4* rec = s_rec + 3 * threadIdx.x;
+            rec[0] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
+            rec[1] = make_float4(-0.5f * co.z, -lnv[g], co.w, 0.0f);
+            rec[2] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
         }
         __syncthreads();
         if (!done) {
-            for (uint32_t j = 0; j < cnt; ++j) {
-                const float4 ge = s_geo[j];
-                const float4 ga = s_gate[j];
-                const float dx = pxc - ge.x, dy = pyc - ge.y;
-                const float power = eval_power(ge.z, ge.w, ga.x, dx, dy);
-                if (STATS) ++n_visit;
-                if (power > 0.0f) continue;       // valid = power <= 0 (L289, C20)
-                if (power < ga.y) continue;       // alpha < alpha_thresh (L679, C12)
-                if (STATS) ++n_pass;
-                const float og = ga.z * fast_exp(power);
-                const float alpha = fminf(P.amax, og);          // C11
-                const float Tn = T * (1.0f - alpha);
-                if (Tn < P.tmin) { done = true; break; }        // C12: stop without blending
-                const float4 c = s_col[j];
-                const float w = alpha * T;
-                C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
-                T = Tn;
-                last = base + j + 1;
-                if (STATS) ++n_blend;
-            }
+            const float4* rp = s_rec;
+            uint32_t j = 0;
+            do {                                      // `break` inside XPR_FWD_ENTRY leaves this do-while
+                for (; j + 4 <= cnt; j += 4, rp += 12) {
+                    XPR_FWD_ENTRY(rp, base + j + 1)
+                    XPR_FWD_ENTRY(rp + 3, base + j + 2)
+                    XPR_FWD_ENTRY(rp + 6, base + j + 3)
+                    XPR_FWD_ENTRY(rp + 9, base + j + 4)
+                }
+                if (done) break;
+                for (; j < cnt; ++j, rp += 3) XPR_FWD_ENTRY(rp, base + j + 1)
+            } while (false);
         }
     }
+#undef XPR_FWD_ENTRY
     if (STATS) {
         atomicAdd(stats + 0, (unsigned long long)n_visit); atomicAdd(stats + 1, (unsigned long long)n_pass);
         atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)last);
