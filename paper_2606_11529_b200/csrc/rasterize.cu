@@ -120,6 +120,12 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     }
 }
 
+__device__ __forceinline__ float fast_rcp(float x) {   // rcp.approx (1 ulp); x = 1 - alpha in [0.01, 1]
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -245,7 +251,7 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                     const float G = fast_exp(power[k]);
                     const float og = ga.z * G;
                     const float alpha = fminf(P.amax, og);
-                    const float inv = 1.0f / (1.0f - alpha);
+                    const float inv = fast_rcp(1.0f - alpha);
                     T[k] = T[k] * inv;                 // transmittance in front of this entry
                     const float w = alpha * T[k];
                     v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
