@@ -424,8 +424,43 @@ struct SortSmem {
 // instructions instead of 8 ballots x 5 ALU instructions; conflict-free when the digits of a warp are
 // distinct (mantissa bytes, consecutive tile ids), 32-way serialised when they are all equal.
 // false: match.any (fast when a warp holds few distinct digits: the high tile digit).
+#ifndef XPR_LB
+#define XPR_LB 4
+#endif
+constexpr int LB = XPR_LB;   // look-back loads in flight per digit thread
+#ifndef XPR_LB_EARLY
+#define XPR_LB_EARLY 0
+#endif
+// Decoupled look-back over earlier tiles by the thread that owns one digit: sums the published counts
+// of the predecessors down to the nearest one whose inclusive prefix is known, then publishes its own.
+__device__ __forceinline__ uint32_t look_back(uint32_t* my, uint32_t tile, uint32_t real_count) {
+    uint32_t excl_prev = 0;
+    if (tile != 0) {
+        const uint32_t* p = my - RADIX;
+        uint32_t remaining = tile;
+        bool found = false;
+        while (!found) {   // LB predecessors in flight per round; before tile 0: virtual inclusive 0
+            uint32_t sv[LB];
+#pragma unroll
+            for (int k = 0; k < LB; ++k)
+                sv[k] = ((uint32_t)k < remaining) ? ld_relaxed(p - k * RADIX) : FLAG_INCLUSIVE;
+#pragma unroll
+            for (int k = 0; k < LB; ++k) {
+                if (found) break;
+                while ((sv[k] & FLAG_MASK) == 0u) sv[k] = ld_relaxed(p - k * RADIX);
+                excl_prev += sv[k] & VALUE_MASK;
+                found = (sv[k] & FLAG_MASK) == FLAG_INCLUSIVE;
+            }
+            p -= LB * RADIX;
+            remaining = (remaining > (uint32_t)LB) ? remaining - (uint32_t)LB : 0u;
+        }
+        st_relaxed(my, FLAG_INCLUSIVE | (excl_prev + real_count));
+    }
+    return excl_prev;
+}
+
 #ifndef XPR_P2_BITMAP
-#define XPR_P2_BITMAP 0
+#define XPR_P2_BITMAP 1
 #endif
 #ifndef XPR_P1_BITMAP
 #define XPR_P1_BITMAP 1
@@ -536,10 +571,11 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
             if (lane >= o) inc_c += a;
         }
         if (lane == 31) S.scan_tmp[warp] = inc_c;
-        // publish this tile's digit counts at once; the look-back itself runs after the shared-memory
-        // scatter, which gives the predecessors time to publish theirs
+        // publish this tile's digit counts at once
         uint32_t* my = status + (size_t)tile * RADIX + tid;
         st_relaxed(my, (tile == 0 ? FLAG_INCLUSIVE : FLAG_PARTIAL) | real_count);
+        uint32_t excl_prev = 0;
+        if (XPR_LB_EARLY) excl_prev = look_back(my, tile, real_count);
         __syncthreads();
         uint32_t pre_c = 0;
 #pragma unroll
@@ -566,29 +602,7 @@ onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* 
                 }
             }
         }
-        // decoupled look-back over earlier tiles, one thread per digit
-        uint32_t excl_prev = 0;
-        if (tile != 0) {
-            const uint32_t* p = my - RADIX;
-            uint32_t remaining = tile;
-            bool found = false;
-            while (!found) {   // 4 predecessors in flight per round; before tile 0: virtual inclusive 0
-                uint32_t sv[4];
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    sv[k] = ((uint32_t)k < remaining) ? ld_relaxed(p - k * RADIX) : FLAG_INCLUSIVE;
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    if (found) break;
-                    while ((sv[k] & FLAG_MASK) == 0u) sv[k] = ld_relaxed(p - k * RADIX);
-                    excl_prev += sv[k] & VALUE_MASK;
-                    found = (sv[k] & FLAG_MASK) == FLAG_INCLUSIVE;
-                }
-                p -= 4 * RADIX;
-                remaining = (remaining > 4u) ? remaining - 4u : 0u;
-            }
-            st_relaxed(my, FLAG_INCLUSIVE | (excl_prev + real_count));
-        }
+        if (!XPR_LB_EARLY) excl_prev = look_back(my, tile, real_count);
         S.gbase[tid] = bin_base + excl_prev - excl_c;
         __syncthreads();
         // coalesced runs to global memory (padding sits at positions >= tile_n)
