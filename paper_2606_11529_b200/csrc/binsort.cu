@@ -54,6 +54,10 @@ static_assert(SORT_THREADS == RADIX, "one thread per digit");
 constexpr int IPT32 = 4;                    // Gaussian-level passes: 1024 keys per tile (N_vis is small)
 constexpr int IPT64 = 16;                   // pair-level passes: 4096 pairs per tile
 constexpr int PERSIST_CTAS = 148 * 4;       // upper bound of the persistent grids
+constexpr int EMIT_THREADS = 256, EMIT_PPT = 8, EMIT_PAIRS = EMIT_THREADS * EMIT_PPT;   // emit: 2048 pairs per unit
+constexpr int EMIT_WARPS = EMIT_THREADS / 32;
+constexpr int EMIT_SHIFT = 11;
+static_assert(EMIT_PAIRS == 1 << EMIT_SHIFT, "unit_first is indexed by pair offset >> EMIT_SHIFT");
 
 constexpr uint32_t FLAG_PARTIAL = 1u << 30, FLAG_INCLUSIVE = 2u << 30, FLAG_MASK = 3u << 30, VALUE_MASK = ~FLAG_MASK;
 constexpr unsigned long long SFLAG_PARTIAL = 1ull << 62, SFLAG_INCLUSIVE = 2ull << 62, SFLAG_MASK = 3ull << 62;
@@ -69,7 +73,7 @@ struct Header {
 };
 
 struct Layout {
-    size_t header, scan_status, vkey0, vidx0, vkey1, vidx1, status32, keys_tmp, status64, total;
+    size_t header, scan_status, vkey0, vidx0, vkey1, vidx1, status32, keys_tmp, status64, unit_first, total;
 };
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -98,6 +102,7 @@ inline Layout make_layout(int64_t N, int64_t cap, int32_t num_tiles) {
     L.keys_tmp = off; off = align_up(off + 8 * c, 256);
     const size_t tiles64 = (c + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
     L.status64 = off; off = align_up(off + 4 * (size_t)RADIX * tiles64 * (size_t)tile_passes_for(num_tiles), 256);
+    L.unit_first = off; off = align_up(off + 4 * (c / EMIT_PAIRS + 2), 256);   // one entry per EMIT_PAIRS pairs
     L.total = off;
     return L;
 }
@@ -224,7 +229,8 @@ compact_kernel(int64_t N, const float* __restrict__ depth, const uint32_t* __res
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(SCAN_THREADS)
 offsets_kernel(const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ tcount, Header* __restrict__ hdr,
-               unsigned long long* __restrict__ status, uint32_t* __restrict__ voff) {
+               unsigned long long* __restrict__ status, uint32_t* __restrict__ voff, uint32_t* __restrict__ unit_first,
+               uint32_t units_cap) {
     __shared__ uint32_t s_warp[SCAN_WARPS];
     __shared__ uint32_t s_block;
     __shared__ unsigned long long s_base;
@@ -271,7 +277,14 @@ offsets_kernel(const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ t
 #pragma unroll
     for (int r = 0; r < SCAN_ROUNDS; ++r) {
         const uint32_t s = s0 + r * 32;
-        if (s < n_vis) voff[s] = (uint32_t)(base + wbase + excl[r]);   // only used when I <= pair_capacity < 2^30
+        if (s < n_vis) {
+            const unsigned long long off = base + wbase + excl[r], end = off + tc[r];
+            voff[s] = (uint32_t)off;                   // only used when I <= pair_capacity < 2^30
+            // emit works in units of EMIT_PAIRS consecutive pairs: unit u starts inside this Gaussian's pairs
+            // iff off <= EMIT_PAIRS u < end; then this Gaussian is the first one the unit needs
+            for (unsigned long long u = (off + (EMIT_PAIRS - 1)) >> EMIT_SHIFT; (u << EMIT_SHIFT) < end && u < units_cap; ++u)
+                unit_first[u] = s;
+        }
     }
     if (tid == 0 && (uint64_t)(block + 1) * SCAN_ITEMS >= n_vis) hdr->total_pairs = base + btotal;   // I
 }
@@ -306,43 +319,76 @@ __device__ __forceinline__ uint32_t warp_upper_bound(const uint32_t* __restrict_
 // CTAs are persistent (grid <= PERSIST_CTAS) so that the digit histograms are flushed to global
 // memory once per CTA, not once per 2048 pairs.
 // ---------------------------------------------------------------------------------------------
-constexpr int EMIT_THREADS = 256, EMIT_PPT = 8, EMIT_PAIRS = EMIT_THREADS * EMIT_PPT;
-constexpr int EMIT_WARPS = EMIT_THREADS / 32;
+constexpr int EMIT_CAND = 2;                 // prefetched candidate Gaussians per thread and unit
 
+__device__ __forceinline__ uint32_t slot_rcp(uint32_t w) {   // bits of ~1/w (rcp.approx, 1 ulp)
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(__uint2float_rn(w)));
+    return __float_as_uint(y);
+}
+
+template <int TILE_PASSES>
 __global__ void __launch_bounds__(EMIT_THREADS)
-emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
-            const int4* __restrict__ rect, Header* __restrict__ hdr, uint64_t* __restrict__ words) {
-    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, first tile id, rectangle width, unused
+emit_kernel(uint32_t I, int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
+            const uint32_t* __restrict__ unit_first, const int4* __restrict__ rect, Header* __restrict__ hdr,
+            uint64_t* __restrict__ words) {
+    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, first tile id, rectangle width, bits(~1/width)
     __shared__ __align__(16) uint16_t s_mark[EMIT_PAIRS];
     __shared__ uint32_t s_hist[MAX_TILE_PASSES * RADIX];
     __shared__ uint32_t s_wmax[EMIT_WARPS];
-    __shared__ uint32_t s_first;
+    constexpr int tile_passes = TILE_PASSES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n_vis = hdr->n_vis;
     const uint32_t units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
     for (int b = tid; b < tile_passes * RADIX; b += EMIT_THREADS) s_hist[b] = 0u;
+    // the first Gaussian of every unit was recorded by offsets_kernel (unit_first), so a unit needs no
+    // search; the candidates of the CTA's NEXT unit are prefetched into registers while the current
+    // one is expanded (the dependent loads voff -> vidx -> rect are off the critical path)
+    uint32_t c_off[EMIT_CAND];
+    int4 c_rect[EMIT_CAND];
+    auto load_candidates = [&](uint32_t first) {
+#pragma unroll
+        for (int c = 0; c < EMIT_CAND; ++c) {
+            const uint32_t s = first + (uint32_t)c * EMIT_THREADS + (uint32_t)tid;
+            c_off[c] = 0xffffffffu;                   // beyond the list: never < a pair index
+            if (s < n_vis) { c_off[c] = voff[s]; c_rect[c] = rect[vidx[s]]; }
+        }
+    };
+    uint32_t first = 0, next_first = 0;
+    if (blockIdx.x < units) { first = unit_first[blockIdx.x]; load_candidates(first); }
 
     for (uint32_t unit = blockIdx.x; unit < units; unit += gridDim.x) {
         const uint32_t p0 = unit * (uint32_t)EMIT_PAIRS, p1 = min(I, p0 + (uint32_t)EMIT_PAIRS);
+        const bool has_next = unit + gridDim.x < units;
+        if (has_next) next_first = unit_first[unit + gridDim.x];
         __syncthreads();                              // previous unit done with the shared arrays
         reinterpret_cast<uint4*>(s_mark)[tid] = make_uint4(0u, 0u, 0u, 0u);      // 8 marks per thread
-        if (warp == 0) {                              // last Gaussian (in depth order) whose offset is <= p0
-            const uint32_t ub = warp_upper_bound(voff, n_vis, p0, lane);
-            if (lane == 0) s_first = ub - 1u;         // voff[0] == 0 <= p0, so ub >= 1
-        }
-        __syncthreads();
-        const uint32_t first = s_first;
         // Gaussians first .. first+cnt-1 cover [p0, p1); cnt <= EMIT_PAIRS because every listed Gaussian
         // after the first starts inside the range (each owns at least one pair)
-        for (uint32_t k = tid; k < (uint32_t)EMIT_PAIRS; k += EMIT_THREADS) {
-            const uint32_t s = first + k;
-            if (s >= n_vis) break;
-            const uint32_t off = voff[s];
-            if (off >= p1) break;
-            const int4 r = rect[vidx[s]];
-            s_slot[k] = make_uint4(off, (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, (uint32_t)(r.z - r.x), 0u);
-            s_mark[off > p0 ? off - p0 : 0u] = (uint16_t)k;
+        const int overflow = __syncthreads_or(c_off[EMIT_CAND - 1] < p1 && tid == EMIT_THREADS - 1);
+#pragma unroll
+        for (int c = 0; c < EMIT_CAND; ++c) {
+            if (c_off[c] < p1) {
+                const uint32_t k = (uint32_t)c * EMIT_THREADS + (uint32_t)tid;
+                const int4 r = c_rect[c];
+                s_slot[k] = make_uint4(c_off[c], (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, (uint32_t)(r.z - r.x), slot_rcp((uint32_t)(r.z - r.x)));
+                s_mark[c_off[c] > p0 ? c_off[c] - p0 : 0u] = (uint16_t)k;
+            }
         }
+        if (overflow) {
+            // more Gaussians start in this unit than were prefetched (tiny Gaussians): load the rest now
+            for (uint32_t k = (uint32_t)(EMIT_CAND * EMIT_THREADS) + tid; k < (uint32_t)EMIT_PAIRS; k += EMIT_THREADS) {
+                const uint32_t s = first + k;
+                if (s >= n_vis) break;
+                const uint32_t off = voff[s];
+                if (off >= p1) break;
+                const int4 r = rect[vidx[s]];
+                s_slot[k] = make_uint4(off, (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, (uint32_t)(r.z - r.x), slot_rcp((uint32_t)(r.z - r.x)));
+                s_mark[off - p0] = (uint16_t)k;
+            }
+        }
+        const uint32_t cur_first = first;             // rank of a pair = cur_first + slot
+        if (has_next) { first = next_first; load_candidates(first); }   // consumed in the next iteration
         __syncthreads();
         {   // inclusive max-scan of the marks (thread t owns positions 8t .. 8t+7): slot of every pair
             uint4 mv = reinterpret_cast<uint4*>(s_mark)[tid];
@@ -375,19 +421,23 @@ emit_kernel(uint32_t I, int TW, int tile_passes, const uint32_t* __restrict__ vi
                 const uint32_t k = s_mark[j - p0];
                 const uint4 sl = s_slot[k];
                 const uint32_t r = j - sl.x, w = sl.z;
-                // r / w by a reciprocal (one fix-up step): exact while the quotient is below 2^22
+                // r / w by an approximate reciprocal: the estimate is within 1 of the quotient while
+                // r < 2^22 (relative error of the product < 2^-21), fixed up on both sides
                 uint32_t ry;
                 if (r < (1u << 22)) {
-                    ry = (uint32_t)__float2uint_rz(__fmul_rz(__uint2float_rz(r), __frcp_rz(__uint2float_rz(w))));   // ry or ry - 1
-                    if (r - ry * w >= w) ++ry;
+                    ry = (uint32_t)__float2uint_rz(__uint2float_rn(r) * __uint_as_float(sl.w));
+                    const int rem = (int)(r - ry * w);
+                    if (rem < 0) --ry;
+                    else if (rem >= (int)w) ++ry;
                 } else {
                     ry = r / w;
                 }
                 tile = sl.y + ry * (uint32_t)TW + (r - ry * w);
-                words[j] = ((uint64_t)tile << 32) | (uint64_t)(first + k);
+                words[j] = ((uint64_t)tile << 32) | (uint64_t)(cur_first + k);
                 atomicAdd(&s_hist[tile & 255u], 1u);      // consecutive tiles -> distinct banks
             }
             // higher tile digits are nearly warp-uniform: aggregate with match.any before the atomic
+#pragma unroll
             for (int d = 1; d < tile_passes; ++d) {
                 const uint32_t dig = valid ? ((tile >> (8 * d)) & 255u) : 0xffffffffu;
                 const uint32_t peers = __match_any_sync(0xffffffffu, dig);
@@ -728,7 +778,9 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     }   // DEPTH_PASSES is even: the sorted list is back in vkey[0] / vidx[0]
     // 3. pair offsets in depth order and the pair count I (the one host read-back)
     uint32_t* voff = vkey[1];                          // free after the depth passes
-    offsets_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], tile_count, hdr, offsets_status, voff);
+    uint32_t* unit_first = reinterpret_cast<uint32_t*>(ws + L.unit_first);
+    offsets_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], tile_count, hdr, offsets_status, voff, unit_first,
+                                                                   (uint32_t)(pair_capacity / EMIT_PAIRS + 1));
     XPR_LAUNCH_CHECK();
     unsigned long long total = 0;
     XPR_CUDA(cudaMemcpyAsync(&total, &hdr->total_pairs, sizeof(total), cudaMemcpyDeviceToHost, st));
@@ -745,8 +797,17 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     uint64_t* w0 = (tpasses % 2 == 0) ? keys_sorted : keys_tmp;
     uint64_t* w1 = (tpasses % 2 == 0) ? keys_tmp : keys_sorted;
     const unsigned units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
-    emit_kernel<<<units < (unsigned)PERSIST_CTAS ? units : (unsigned)PERSIST_CTAS, EMIT_THREADS, 0, st>>>(
-        I, TW, tpasses, vidx[0], voff, reinterpret_cast<const int4*>(tile_rect), hdr, w0);
+    const unsigned egrid = units < (unsigned)PERSIST_CTAS ? units : (unsigned)PERSIST_CTAS;
+#define XPR_EMIT(TP)                                                                                             \
+    emit_kernel<TP><<<egrid, EMIT_THREADS, 0, st>>>(I, TW, vidx[0], voff, unit_first,                             \
+                                                    reinterpret_cast<const int4*>(tile_rect), hdr, w0)
+    switch (tpasses) {
+        case 1: XPR_EMIT(1); break;
+        case 2: XPR_EMIT(2); break;
+        case 3: XPR_EMIT(3); break;
+        default: XPR_EMIT(4); break;
+    }
+#undef XPR_EMIT
     XPR_LAUNCH_CHECK();
     // 5. the tile-id digits, on the I pairs
     const unsigned tiles64 = (I + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
