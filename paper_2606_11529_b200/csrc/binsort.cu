@@ -412,28 +412,28 @@ emit_kernel(uint32_t I, int TW, const uint32_t* __restrict__ vidx, const uint32_
                                                                m[4] | (m[5] << 16), m[6] | (m[7] << 16));
         }
         __syncthreads();
+        // pair j of slot k: r = j - offset, (ry, rx) = divmod(r, w), tile = tile0 + ry * TW + rx.  The loads of
+        // the 8 pairs of a thread are issued together and the arithmetic is branch-free (8 independent chains).
+        // r / w by an approximate reciprocal: the estimate is within 1 of the quotient while r < 2^22
+        // (relative error of the product < 2^-21) and is fixed up on both sides; beyond that, integer division.
+        uint32_t kk[EMIT_PPT];
+        uint4 sl[EMIT_PPT];
+#pragma unroll
+        for (int it = 0; it < EMIT_PPT; ++it) kk[it] = s_mark[min((uint32_t)it * EMIT_THREADS + (uint32_t)tid, p1 - p0 - 1u)];
+#pragma unroll
+        for (int it = 0; it < EMIT_PPT; ++it) sl[it] = s_slot[kk[it]];
 #pragma unroll
         for (int it = 0; it < EMIT_PPT; ++it) {
             const uint32_t j = p0 + (uint32_t)it * EMIT_THREADS + (uint32_t)tid;
-            const bool valid = j < p1;
-            uint32_t tile = 0;
+            const bool valid = j < p1;                 // false only in the tail of the last unit
+            const uint32_t r = j - sl[it].x, w = sl[it].z;
+            uint32_t ry = (uint32_t)__float2uint_rz(__uint2float_rn(r) * __uint_as_float(sl[it].w));
+            const int rem = (int)(r - ry * w);
+            ry += (rem >= (int)w ? 1u : 0u) - (rem < 0 ? 1u : 0u);
+            if (r >= (1u << 22)) ry = r / w;           // a Gaussian covering more than 4M tiles
+            const uint32_t tile = sl[it].y + ry * (uint32_t)TW + (r - ry * w);
             if (valid) {
-                const uint32_t k = s_mark[j - p0];
-                const uint4 sl = s_slot[k];
-                const uint32_t r = j - sl.x, w = sl.z;
-                // r / w by an approximate reciprocal: the estimate is within 1 of the quotient while
-                // r < 2^22 (relative error of the product < 2^-21), fixed up on both sides
-                uint32_t ry;
-                if (r < (1u << 22)) {
-                    ry = (uint32_t)__float2uint_rz(__uint2float_rn(r) * __uint_as_float(sl.w));
-                    const int rem = (int)(r - ry * w);
-                    if (rem < 0) --ry;
-                    else if (rem >= (int)w) ++ry;
-                } else {
-                    ry = r / w;
-                }
-                tile = sl.y + ry * (uint32_t)TW + (r - ry * w);
-                words[j] = ((uint64_t)tile << 32) | (uint64_t)(cur_first + k);
+                words[j] = ((uint64_t)tile << 32) | (uint64_t)(cur_first + kk[it]);
                 atomicAdd(&s_hist[tile & 255u], 1u);      // consecutive tiles -> distinct banks
             }
             // higher tile digits are nearly warp-uniform: aggregate with match.any before the atomic
