@@ -29,94 +29,140 @@ __device__ __forceinline__ float fast_exp(float x) {   // ex2.approx(x * log2 e)
     return y;
 }
 
+// Forward compositing (a8).  One CTA per 16x16 tile, in two shapes:
+//   PPT = 2: 128 threads, a thread owns the two pixels (x, y) and (x + 8, y) of one row, so the row terms
+//            of `power` (dy, qb*dy, (qc*dy)*dy) and the shared-memory reads of a list entry are paid once
+//            per two pixels -- fewer instructions per pixel-pair (throughput shape, large images);
+//   PPT = 1: 256 threads, one pixel each -- twice the warps on a tile, i.e. half the critical path of a
+//            heavy tile (latency shape, images with few tiles where the longest list bounds the kernel).
+// The arithmetic per pixel is exactly eval_power's (rule R3) in both.
 // STATS = true: the same walk, additionally counting pixel-pair events into stats[0..3] =
 // {visited, passed both gates, blended, sum of n_contrib} (xpr_rasterize_stats; roofline accounting).
-template <bool STATS>
-__global__ void __launch_bounds__(BLOCK)
+#ifndef XPR_FWD_PPT2_MIN_TILES
+#define XPR_FWD_PPT2_MIN_TILES 4096
+#endif
+constexpr int FWD_PPT2_MIN_TILES = XPR_FWD_PPT2_MIN_TILES;
+
+template <bool STATS, int PPT>
+__global__ void __launch_bounds__(BLOCK / PPT)
 rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                      float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                      unsigned long long* __restrict__ stats) {
     // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, o, - | r, g, b, -)
-    __shared__ float4 s_rec[3 * BLOCK];
+    constexpr int FWD_BATCH = BLOCK / PPT;          // one list entry staged per thread
+    __shared__ float4 s_rec[3 * FWD_BATCH];
     const int tile = blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
-    const int px = tx * TILE + (threadIdx.x & (TILE - 1)), py = ty * TILE + (threadIdx.x >> 4);
-    const bool inside = (px < P.W) && (py < P.H);
-    const float pxc = (float)px + 0.5f, pyc = (float)py + 0.5f;
+    constexpr int FWD_THREADS = BLOCK / PPT, ROW = TILE / PPT;
+    const int px0 = tx * TILE + (threadIdx.x % ROW), px1 = px0 + 8, py = ty * TILE + (threadIdx.x / ROW);
+    const bool in0 = (px0 < P.W) && (py < P.H), in1 = (PPT == 2) && (px1 < P.W) && (py < P.H);
+    const float pxc0 = (float)px0 + 0.5f, pxc1 = (float)px1 + 0.5f, pyc = (float)py + 0.5f;
     const uint2 rg = ranges[tile];
     const uint32_t len = rg.y - rg.x;
 
-    float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
-    uint32_t last = 0;
-    bool done = !inside;
+    float Ta = 1.0f, Ca0 = 0.0f, Ca1 = 0.0f, Ca2 = 0.0f;     // pixel (px0, py)
+    float Tb = 1.0f, Cb0 = 0.0f, Cb1 = 0.0f, Cb2 = 0.0f;     // pixel (px1, py)
+    uint32_t last_a = 0, last_b = 0;
+    bool act_a = in0, act_b = in1;                            // still compositing
     uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
 
-    // one list entry against this thread's pixel; `rp` points at its record, `pos` = list position + 1
-#define XPR_FWD_ENTRY(rp, pos)                                                                       \
+    // The list is walked in groups of 4 entries.  Phase 1 of a group computes the 4 (x PPT) values of
+    // `power` -- independent of each other and of the transmittance, so their latencies overlap -- and
+    // phase 2 runs the sequential part (gate, alpha, T' = T (1 - alpha), exit test, blend).
+#define XPR_FWD_POWER(u, rp)                                                                          \
     {                                                                                                \
         const float4 ge = (rp)[0];                                                                   \
         const float4 ga = (rp)[1];                                                                   \
-        const float dx = pxc - ge.x, dy = pyc - ge.y;                                                \
-        const float power = eval_power(ge.z, ge.w, ga.x, dx, dy);                                    \
+        const float dy = pyc - ge.y;                                                                 \
+        const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);               \
+        const float dxa = pxc0 - ge.x;                                                               \
+        pw_a[u] = __fmaf_rn(__fmaf_rn(ge.z, dxa, t1), dxa, t2);                                      \
+        if (PPT == 2) {                                                                              \
+            const float dxb = pxc1 - ge.x;                                                           \
+            pw_b[u] = __fmaf_rn(__fmaf_rn(ge.z, dxb, t1), dxb, t2);                                  \
+        }                                                                                            \
+        thr[u] = ga.y; op[u] = ga.z;                                                                 \
+    }
+    // valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12)
+#define XPR_FWD_BLEND(act, power, u, rp, T, C0, C1, C2, last, pos)                                    \
+    if (act) {                                                                                       \
         if (STATS) ++n_visit;                                                                        \
-        /* valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12) */    \
-        if (!(power > 0.0f) && !(power < ga.y)) {                                                    \
+        if (!((power) > 0.0f) && !((power) < thr[u])) {                                              \
             if (STATS) ++n_pass;                                                                     \
-            const float alpha = fminf(P.amax, ga.z * fast_exp(power));      /* C11 */                \
+            const float alpha = fminf(amax, op[u] * fast_exp(power));       /* C11 */                \
             const float Tn = T * (1.0f - alpha);                                                     \
-            if (Tn < P.tmin) { done = true; break; }                        /* C12: stop, no blend */\
-            const float4 c = (rp)[2];                                                                \
-            const float w = alpha * T;                                                               \
-            C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);                     \
-            T = Tn;                                                                                  \
-            last = (pos);                                                                            \
-            if (STATS) ++n_blend;                                                                    \
+            if (Tn < tmin) {                                                /* C12: stop, no blend */\
+                act = false;                                                                         \
+            } else {                                                                                 \
+                const float4 c = (rp)[2];                                                            \
+                const float w = alpha * T;                                                           \
+                C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);                 \
+                T = Tn;                                                                              \
+                last = (pos);                                                                        \
+                if (STATS) ++n_blend;                                                                \
+            }                                                                                        \
         }                                                                                            \
     }
+#define XPR_FWD_STEP(u, rp, pos)                                                                      \
+    XPR_FWD_BLEND(act_a, pw_a[u], u, rp, Ta, Ca0, Ca1, Ca2, last_a, pos)                              \
+    if (PPT == 2) XPR_FWD_BLEND(act_b, pw_b[u], u, rp, Tb, Cb0, Cb1, Cb2, last_b, pos)
 
-    for (uint32_t base = 0; base < len; base += BLOCK) {
-        if (__syncthreads_count(done) == BLOCK) break;
-        const uint32_t cnt = min((uint32_t)BLOCK, len - base);
-        if (threadIdx.x < cnt) {
-            const uint32_t g = vals[rg.x + base + threadIdx.x];
+    const float amax = P.amax, tmin = P.tmin;
+    float pw_a[4], pw_b[4], thr[4], op[4];
+    for (uint32_t base = 0; base < len; base += FWD_BATCH) {
+        if (__syncthreads_or(act_a || act_b) == 0) break;
+        const uint32_t cnt = min((uint32_t)FWD_BATCH, len - base);
+        for (uint32_t e = threadIdx.x; e < cnt; e += FWD_THREADS) {
+            const uint32_t g = vals[rg.x + base + e];
             const float2 m = mean2d[g];
             const float4 co = conic_opac[g];
-            float4* rec = s_rec + 3 * threadIdx.x;
+            float4* rec = s_rec + 3 * e;
             rec[0] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
             rec[1] = make_float4(-0.5f * co.z, -lnv[g], co.w, 0.0f);
             rec[2] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
         }
         __syncthreads();
-        if (!done) {
-            const float4* rp = s_rec;
+        if (act_a || act_b) {
+            const float4* rq = s_rec;
             uint32_t j = 0;
-            do {                                      // `break` inside XPR_FWD_ENTRY leaves this do-while
-                for (; j + 4 <= cnt; j += 4, rp += 12) {
-                    XPR_FWD_ENTRY(rp, base + j + 1)
-                    XPR_FWD_ENTRY(rp + 3, base + j + 2)
-                    XPR_FWD_ENTRY(rp + 6, base + j + 3)
-                    XPR_FWD_ENTRY(rp + 9, base + j + 4)
-                }
-                if (done) break;
-                for (; j < cnt; ++j, rp += 3) XPR_FWD_ENTRY(rp, base + j + 1)
-            } while (false);
+            for (; j + 4 <= cnt && (act_a || act_b); j += 4, rq += 12) {
+                XPR_FWD_POWER(0, rq) XPR_FWD_POWER(1, rq + 3) XPR_FWD_POWER(2, rq + 6) XPR_FWD_POWER(3, rq + 9)
+                XPR_FWD_STEP(0, rq, base + j + 1)
+                XPR_FWD_STEP(1, rq + 3, base + j + 2)
+                XPR_FWD_STEP(2, rq + 6, base + j + 3)
+                XPR_FWD_STEP(3, rq + 9, base + j + 4)
+            }
+            for (; j < cnt && (act_a || act_b); ++j, rq += 3) {
+                XPR_FWD_POWER(0, rq)
+                XPR_FWD_STEP(0, rq, base + j + 1)
+            }
         }
     }
-#undef XPR_FWD_ENTRY
+#undef XPR_FWD_POWER
+#undef XPR_FWD_BLEND
+#undef XPR_FWD_STEP
     if (STATS) {
         atomicAdd(stats + 0, (unsigned long long)n_visit); atomicAdd(stats + 1, (unsigned long long)n_pass);
-        atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)last);
+        atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)(last_a + last_b));
         return;
     }
-    if (inside) {
-        const int64_t pid = (int64_t)py * P.W + px;
-        image[3 * pid] = fmaf(T, P.bg[0], C0);
-        image[3 * pid + 1] = fmaf(T, P.bg[1], C1);
-        image[3 * pid + 2] = fmaf(T, P.bg[2], C2);
-        final_T[pid] = T;
-        n_contrib[pid] = last;
+    if (in0) {
+        const int64_t pid = (int64_t)py * P.W + px0;
+        image[3 * pid] = fmaf(Ta, P.bg[0], Ca0);
+        image[3 * pid + 1] = fmaf(Ta, P.bg[1], Ca1);
+        image[3 * pid + 2] = fmaf(Ta, P.bg[2], Ca2);
+        final_T[pid] = Ta;
+        n_contrib[pid] = last_a;
+    }
+    if (in1) {
+        const int64_t pid = (int64_t)py * P.W + px1;
+        image[3 * pid] = fmaf(Tb, P.bg[0], Cb0);
+        image[3 * pid + 1] = fmaf(Tb, P.bg[1], Cb1);
+        image[3 * pid + 2] = fmaf(Tb, P.bg[2], Cb2);
+        final_T[pid] = Tb;
+        n_contrib[pid] = last_b;
     }
 }
 
@@ -303,9 +349,15 @@ extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cf
     RasterParams P;
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
-    rasterize_fwd_kernel<false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
-        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    // throughput shape once the image has enough tiles for several waves of every SM
+    if (T >= FWD_PPT2_MIN_TILES)
+        rasterize_fwd_kernel<false, 2><<<T, BLOCK / 2, 0, (cudaStream_t)stream>>>(
+            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    else
+        rasterize_fwd_kernel<false, 1><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }
@@ -323,7 +375,7 @@ extern "C" int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* 
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
     XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
-    rasterize_fwd_kernel<true><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+    rasterize_fwd_kernel<true, 1><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
         P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
         vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr, nullptr, nullptr,
         reinterpret_cast<unsigned long long*>(stats));
