@@ -225,7 +225,7 @@ def run_ours(args):
     n_pairs = pipe.num_pairs
     # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
     bits = max(1, (pipe.T - 1).bit_length()) if pipe.T > 1 else 0
-    tile_passes = (bits + 7) // 8
+    tile_passes = max(1, (bits + 7) // 8)
     passes = 4 + tile_passes              # 8-bit digits: 4 on the depth bits (run on Gaussians) + tile digits (on pairs)
     # project, bin_sort (compact, 4 depth passes, offsets, emit, tile passes, ranges), fwd, bwd, project_bwd
     launches_per_step = 1 + (1 + 4 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1
@@ -262,26 +262,31 @@ def run_ours(args):
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     alu_peak = SMS * LANES_PER_SM * sm_max * 1e6 / 1e12          # T lane-ops/s (FMA = 1 lane-op)
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    dom = max(("rasterize_fwd", "rasterize_bwd", "bin_sort"), key=lambda n: stage_ms[n])
-    if dom == "rasterize_bwd":
-        ops = BWD_OPS_VISIT * sum_n + BWD_OPS_PASS * blended
-        roof = {"kernel": "rasterize_bwd_kernel", "bound": "alu", "achieved": ops / (stage_ms[dom] / 1e3) / 1e12,
-                "peak": alu_peak, "unit": "T lane-op/s"}
-    elif dom == "rasterize_fwd":
-        ops = FWD_OPS_VISIT * visit + FWD_OPS_PASS * passed
-        roof = {"kernel": "rasterize_fwd_kernel", "bound": "alu", "achieved": ops / (stage_ms[dom] / 1e3) / 1e12,
-                "peak": alu_peak, "unit": "T lane-op/s"}
-    else:
-        # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + per pair
-        # 12 B emitted, 24 B per tile-digit pass, 8 B read by ranges
-        nbytes = 8 * sc.N + 4 * 16 * n_vis + n_pairs * (12 + 24 * tile_passes + 8)
-        roof = {"kernel": "xpr_bin_sort (compact, 4 depth passes, offsets, emit, %d tile passes, ranges)" % tile_passes,
-                "bound": "hbm",
-                "achieved": nbytes / (stage_ms[dom] / 1e3) / 1e9, "peak": hbm_peak, "unit": "GB/s"}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
-    roof["peak_source"] = "MEASURED_PEAKS.json" if peaks else "fallback (B200_PROFILING.md)"
-    roof["ms_per_launch"] = stage_ms[dom]
+    sec = lambda n: stage_ms[n] / 1e3
+    # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + per pair: 8 B
+    # emitted, 16 B per intermediate tile pass, 8 B read + 12 B written by the last one
+    sort_bytes = 8 * sc.N + 4 * 16 * n_vis + n_pairs * (8 + 16 * (tile_passes - 1) + 20)
+    rooflines = {
+        "rasterize_fwd": {"kernel": "rasterize_fwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
+                          "achieved": (FWD_OPS_VISIT * visit + FWD_OPS_PASS * passed) / sec("rasterize_fwd") / 1e12},
+        "rasterize_bwd": {"kernel": "rasterize_bwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
+                          "achieved": (BWD_OPS_VISIT * sum_n + BWD_OPS_PASS * blended) / sec("rasterize_bwd") / 1e12},
+        "bin_sort": {"kernel": "xpr_bin_sort (compact, 4 depth passes on Gaussians, offsets, emit, %d tile passes "
+                               "on pairs, ranges)" % tile_passes, "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
+                     "achieved": sort_bytes / sec("bin_sort") / 1e9, "algorithmic_bytes": sort_bytes},
+    }
+    traffic = {}
+    try:   # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu --set full capture
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get("config%d" % args.config, {})
+    except Exception:
+        pass
+    for name, r in rooflines.items():
+        r["frac"] = r["achieved"] / r["peak"]
+        r["traffic"] = traffic.get(name)
+        r["peak_source"] = "MEASURED_PEAKS.json" if peaks else "fallback (B200_PROFILING.md)"
+        r["ms_per_launch"] = stage_ms[name]
+    dom = max(rooflines, key=lambda n: stage_ms[n])
+    roof = rooflines[dom]
 
     # end to end through the public API with HOST buffers: H2D of the parameters, the step, D2H of results
     e2e = None
@@ -336,7 +341,7 @@ def run_ours(args):
                 "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,
                 "pixel_pairs": {"visited": visit, "passed_gate": passed, "blended": blended, "sum_n_contrib": sum_n},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-                "roofline": roof, "cpu_baseline": cpu}
+                "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
         if args.stages:
             print(json.dumps(stage_ms, indent=1), file=sys.stderr)
