@@ -124,3 +124,22 @@ def test_config3_full_size_bench_configuration():
     bench.py times: every stage against the oracle, every element."""
     g, o = full_parity(scenes.make_scene(3))
     assert o["binned"]["num_pairs"] > 5_000_000
+
+
+def test_config5_full_size_stress_view():
+    """BASELINE.json configs[4] at full size (3M Gaussians, 1920x1080, > 10^8 tile-Gaussian pairs in one
+    view): every stage against the oracle, every element (the oracle needs about a minute)."""
+    g, o = full_parity(scenes.make_scene(5), view=0)
+    assert o["binned"]["num_pairs"] > 50_000_000
+
+
+@pytest.mark.parametrize("view", [0, 1])
+def test_config4_full_size_ut_fisheye(view):
+    """BASELINE.json configs[3] at full size (1M Gaussians, UT with 7 sigma points through the seeded
+    fisheye camera, 1920x1080), both poses."""
+    g, o = full_parity(scenes.make_scene(4), view=view)
+    assert o["binned"]["num_pairs"] > 1_000_000
+
+
+def test_config3_full_size_second_pose():
+    full_parity(scenes.make_scene(3), view=1)
