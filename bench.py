@@ -39,6 +39,7 @@ def parse():
     ap.add_argument("--view", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--stages", action="store_true", help="also print per-stage times to stderr")
     return ap.parse_args()
 
@@ -199,10 +200,13 @@ def run_ours(args):
 
     stage_names = ("project", "bin_sort", "rasterize_fwd", "loss_grad", "rasterize_bwd", "project_bwd")
 
-    def step(events=None):
+    def step(events=None, sync_count=False):
+        """One fwd+bwd step.  sync_count=True: xpr_bin_sort reads the pair count back (and regrows the pair
+        buffers if needed) -- used for the warm-up; the timed steps run fully asynchronously and the count is
+        checked against the capacity after the timed region."""
         ev = (lambda: None) if events is None else (lambda: events.append(_rec()))
         ev(); pipe.project(*params)
-        ev(); pipe.bin_sort()
+        ev(); pipe.bin_sort() if sync_count else pipe.bin_sort_async()
         ev(); pipe.rasterize_fwd()
         ev(); dL = loss_grad(pipe.image)
         ev(); pipe.rasterize_bwd(dL)
@@ -220,7 +224,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     for _ in range(max(args.warmup, 3)):
-        step()
+        step(sync_count=True)
     barrier()
     n_pairs = pipe.num_pairs
     # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
@@ -242,6 +246,7 @@ def run_ours(args):
         all_events.append(evs)
     barrier()
     clocks = sampler.stop()
+    assert pipe.check_capacity() == n_pairs          # the asynchronous steps produced the same, fitting, pair count
     step_ms = [e[0].elapsed_time(e[-1]) for e in all_events]
     total_ms = max_over_ranks(float(sum(step_ms)), world, dev)
     ms = total_ms / args.steps
@@ -288,6 +293,32 @@ def run_ours(args):
     dom = max(rooflines, key=lambda n: stage_ms[n])
     roof = rooflines[dom]
 
+    # the same step captured once in a CUDA graph and replayed (no host work between the 15 launches)
+    graph_ms = None
+    if not args.no_graph:
+        try:
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                step()
+            torch.cuda.current_stream().wait_stream(side)
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                step()
+            for _ in range(3):
+                g.replay()
+            barrier()
+            t_ms = 0.0
+            for _ in range(args.steps):
+                flush.fill_(1)
+                a = _rec(); g.replay(); b = _rec()
+                torch.cuda.synchronize()
+                t_ms += a.elapsed_time(b)
+            assert pipe.check_capacity() == n_pairs
+            graph_ms = max_over_ranks(t_ms, world, dev) / args.steps
+        except Exception as e:      # capture unsupported in this environment: report, do not hide
+            graph_ms = "unavailable: %s" % (str(e).splitlines()[0][:120],)
+
     # end to end through the public API with HOST buffers: H2D of the parameters, the step, D2H of results
     e2e = None
     if not args.no_e2e:
@@ -301,7 +332,7 @@ def run_ours(args):
         def e2e_step():
             for d, h in zip(dev_in, host_in):
                 d.copy_(h, non_blocking=True)
-            pipe.project(*dev_in); pipe.bin_sort(); pipe.rasterize_fwd()
+            pipe.project(*dev_in); pipe.bin_sort_async(); pipe.rasterize_fwd()
             pipe.rasterize_bwd(loss_grad(pipe.image)); pipe.project_bwd()
             for h, o in zip(host_out, outs):
                 h.copy_(o, non_blocking=True)
@@ -341,7 +372,7 @@ def run_ours(args):
                 "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,
                 "pixel_pairs": {"visited": visit, "passed_gate": passed, "blended": blended, "sum_n_contrib": sum_n},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-                "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}
+                "cuda_graph_ms_per_step": graph_ms, "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
         if args.stages:
             print(json.dumps(stage_ms, indent=1), file=sys.stderr)

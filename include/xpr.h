@@ -11,8 +11,8 @@
  *    (e.g. a PyTorch allocation), contiguous, row-major, 16-byte aligned.  The library allocates
  *    no persistent device memory; scratch comes from the caller-provided workspace.
  *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
- *    enqueued on it.  The only call that synchronises the stream is xpr_bin_sort (8-byte read-back
- *    of the pair count I).
+ *    enqueued on it.  The only call that synchronises the stream is xpr_bin_sort, at its end (8-byte
+ *    read-back of the pair count I), and only when num_pairs_host != NULL.
  *  - xpr_camera / xpr_config are HOST structs, read during the call.
  *  - Arguments are validated before any launch: NULL or misaligned pointer, negative size, bad
  *    enum -> XPR_ERR_INVALID_ARG; tile != 16, sh_degree > 3 -> XPR_ERR_UNSUPPORTED; a CUDA runtime
@@ -90,8 +90,14 @@ int32_t xpr_project(int64_t N, const float* means, const float* scales, const fl
  *        output arrays (must be < 2^30).
  *   out: keys_sorted[I] u64, vals_sorted[I] u32, tile_ranges[T,2] = (start,end) per tile, (0,0)
  *        for an empty tile; *num_pairs_host (HOST int64) = I.
- *   I > pair_capacity -> XPR_ERR_CAPACITY, *num_pairs_host = required I, nothing out of bounds
- *   is written and the outputs are unspecified.
+ *   Nothing inside the call waits for the host: I stays on the device and every kernel reads it
+ *   there.  With num_pairs_host != NULL the call ends with an 8-byte read-back of I and a stream
+ *   synchronisation; I > pair_capacity -> XPR_ERR_CAPACITY with *num_pairs_host = required I.
+ *   With num_pairs_host == NULL the call is fully asynchronous (capturable in a CUDA graph): it
+ *   returns XPR_OK after enqueueing, and the first 8 bytes of `workspace` hold I (uint64) once the
+ *   stream has run; the caller must compare it with pair_capacity before trusting the outputs.
+ *   In both modes, when I > pair_capacity nothing out of bounds is written, tile_ranges is (0,0) for
+ *   every tile (a following xpr_rasterize_fwd renders the background) and keys/vals are unspecified.
  *   workspace: DEVICE scratch of at least xpr_bin_sort_workspace() bytes, 256-byte aligned.
  *   Equal keys keep emission order = ascending Gaussian index.
  */

@@ -131,14 +131,19 @@ def xpr_bin_sort_workspace(N: int, pair_capacity: int, n_tiles: int) -> int:
 
 
 def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, pair_capacity: int, keys_sorted,
-                 vals_sorted, tile_ranges, workspace, stream=None, raise_on_capacity: bool = True):
-    """Returns (status, I).  On XPR_ERR_CAPACITY I is the required capacity."""
+                 vals_sorted, tile_ranges, workspace, stream=None, raise_on_capacity: bool = True, sync: bool = True):
+    """Returns (status, I).  On XPR_ERR_CAPACITY I is the required capacity.
+    sync=False: num_pairs_host = NULL -- nothing waits for the host, I is returned as None and stays in the
+    first 8 bytes of `workspace` (xpr.h); the caller checks it against pair_capacity later."""
     N = int(tile_count.shape[0])
     n_pairs = C.c_int64(0)
     st = lib().xpr_bin_sort(C.c_int64(N), _p(depth), _p(tile_rect), _p(tile_count), C.byref(cam), C.byref(cfg),
                             C.c_int64(pair_capacity), _p(keys_sorted), _p(vals_sorted), _p(tile_ranges),
-                            C.byref(n_pairs), _p(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
-                            _stream(stream))
+                            C.byref(n_pairs) if sync else None, _p(workspace),
+                            C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    if not sync:
+        _check(st, "xpr_bin_sort")
+        return st, None
     if st == XPR_ERR_CAPACITY and not raise_on_capacity:
         return st, int(n_pairs.value)
     _check(st, "xpr_bin_sort")

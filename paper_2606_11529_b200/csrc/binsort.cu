@@ -64,11 +64,12 @@ constexpr unsigned long long SFLAG_PARTIAL = 1ull << 62, SFLAG_INCLUSIVE = 2ull 
 
 // Header at the start of the workspace (zeroed every call).
 struct Header {
-    unsigned long long total_pairs;          // I
+    unsigned long long total_pairs;          // I (first 8 bytes of the workspace: readable by the caller)
+    unsigned long long pairs_eff;            // I if it fits pair_capacity, else 0: what the pair kernels process
     uint32_t n_vis;                          // visible Gaussians
     uint32_t compact_ticket, emit_ticket;
     uint32_t sort_ticket[DEPTH_PASSES + MAX_TILE_PASSES];
-    uint32_t pad[5];
+    uint32_t pad[3];
     uint32_t hist[(DEPTH_PASSES + MAX_TILE_PASSES) * RADIX];   // global digit histograms
 };
 
@@ -94,14 +95,14 @@ inline Layout make_layout(int64_t N, int64_t cap, int32_t num_tiles) {
     L.scan_status = off; off = align_up(off + 8 * 2 * (scan_blocks + 1), 256);      // compact + offsets chains
     const size_t tiles32 = (n + SORT_THREADS * IPT32 - 1) / (SORT_THREADS * IPT32);
     L.status32 = off; off = align_up(off + 4 * (size_t)RADIX * tiles32 * DEPTH_PASSES, 256);
+    const size_t tiles64 = (c + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
+    L.status64 = off; off = align_up(off + 4 * (size_t)RADIX * tiles64 * (size_t)tile_passes_for(num_tiles), 256);
     // everything up to here is zeroed with one memset
     L.vkey0 = off; off = align_up(off + 4 * n, 256);
     L.vidx0 = off; off = align_up(off + 4 * n, 256);
     L.vkey1 = off; off = align_up(off + 4 * n, 256);
     L.vidx1 = off; off = align_up(off + 4 * n, 256);
     L.keys_tmp = off; off = align_up(off + 8 * c, 256);
-    const size_t tiles64 = (c + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
-    L.status64 = off; off = align_up(off + 4 * (size_t)RADIX * tiles64 * (size_t)tile_passes_for(num_tiles), 256);
     L.unit_first = off; off = align_up(off + 4 * (c / EMIT_PAIRS + 2), 256);   // one entry per EMIT_PAIRS pairs
     L.total = off;
     return L;
@@ -230,7 +231,7 @@ compact_kernel(int64_t N, const float* __restrict__ depth, const uint32_t* __res
 __global__ void __launch_bounds__(SCAN_THREADS)
 offsets_kernel(const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ tcount, Header* __restrict__ hdr,
                unsigned long long* __restrict__ status, uint32_t* __restrict__ voff, uint32_t* __restrict__ unit_first,
-               uint32_t units_cap) {
+               uint32_t units_cap, unsigned long long pair_capacity) {
     __shared__ uint32_t s_warp[SCAN_WARPS];
     __shared__ uint32_t s_block;
     __shared__ unsigned long long s_base;
@@ -286,7 +287,11 @@ offsets_kernel(const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ t
                 unit_first[u] = s;
         }
     }
-    if (tid == 0 && (uint64_t)(block + 1) * SCAN_ITEMS >= n_vis) hdr->total_pairs = base + btotal;   // I
+    if (tid == 0 && (uint64_t)(block + 1) * SCAN_ITEMS >= n_vis) {
+        const unsigned long long I = base + btotal;
+        hdr->total_pairs = I;
+        hdr->pairs_eff = (I <= pair_capacity) ? I : 0ull;     // over capacity: the pair kernels do nothing
+    }
 }
 
 // 32-ary search by one warp in a sorted u32 array: first index in [0, n) whose element is > x
@@ -329,7 +334,7 @@ __device__ __forceinline__ uint32_t slot_rcp(uint32_t w) {   // bits of ~1/w (rc
 
 template <int TILE_PASSES>
 __global__ void __launch_bounds__(EMIT_THREADS)
-emit_kernel(uint32_t I, int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
+emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
             const uint32_t* __restrict__ unit_first, const int4* __restrict__ rect, Header* __restrict__ hdr,
             uint64_t* __restrict__ words) {
     __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, first tile id, rectangle width, bits(~1/width)
@@ -339,6 +344,7 @@ emit_kernel(uint32_t I, int TW, const uint32_t* __restrict__ vidx, const uint32_
     constexpr int tile_passes = TILE_PASSES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n_vis = hdr->n_vis;
+    const uint32_t I = (uint32_t)hdr->pairs_eff;
     const uint32_t units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
     for (int b = tid; b < tile_passes * RADIX; b += EMIT_THREADS) s_hist[b] = 0u;
     // the first Gaussian of every unit was recorded by offsets_kernel (unit_first), so a unit needs no
@@ -690,7 +696,9 @@ __device__ __forceinline__ uint32_t warp_lower_bound_tile(const uint64_t* __rest
 }
 
 __global__ void __launch_bounds__(256)
-ranges_kernel(uint32_t I, uint32_t T, const uint64_t* __restrict__ keys, uint32_t* __restrict__ ranges) {
+ranges_kernel(const unsigned long long* __restrict__ pairs_eff, uint32_t T, const uint64_t* __restrict__ keys,
+              uint32_t* __restrict__ ranges) {
+    const uint32_t I = (uint32_t)*pairs_eff;
     const uint32_t t = blockIdx.x * 8u + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (t >= T) return;
@@ -732,7 +740,7 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
                                 uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
                                 int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
-    if (N < 0 || N > 0x7fffffffLL || pair_capacity < 0 || pair_capacity >= (1LL << 30) || !num_pairs_host)
+    if (N < 0 || N > 0x7fffffffLL || pair_capacity < 0 || pair_capacity >= (1LL << 30))
         return XPR_ERR_INVALID_ARG;
     const int TW = tiles_x(cam), TH = tiles_y(cam);
     const int64_t T64 = (int64_t)TW * TH;
@@ -756,12 +764,13 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     uint32_t* status64 = reinterpret_cast<uint32_t*>(ws + L.status64);
     const int tpasses = tile_passes_for(T);
 
-    *num_pairs_host = 0;
+    if (num_pairs_host) *num_pairs_host = 0;
     if (N == 0) {
         XPR_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)T, st));
+        XPR_CUDA(cudaMemsetAsync(ws + L.header, 0, sizeof(Header), st));       // pair count 0 for an asynchronous caller
         return XPR_OK;
     }
-    XPR_CUDA(cudaMemsetAsync(ws + L.header, 0, L.vkey0 - L.header, st));   // header, scan chains, status32
+    XPR_CUDA(cudaMemsetAsync(ws + L.header, 0, L.vkey0 - L.header, st));   // header, scan chains, look-back status words
     // 1. visible Gaussians (index order) + depth-digit histograms
     compact_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(N, depth, tile_count, hdr, compact_status, vkey[0],
                                                                    vidx[0]);
@@ -776,57 +785,56 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
             : launch_pass<uint32_t, IPT32, false, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr);
         XPR_CUDA(e);
     }   // DEPTH_PASSES is even: the sorted list is back in vkey[0] / vidx[0]
-    // 3. pair offsets in depth order and the pair count I (the one host read-back)
+    // 3. pair offsets in depth order and the pair count I.  I stays on the device: every later kernel reads
+    //    it there (grids are persistent and sized for pair_capacity), so nothing waits for the host.
     uint32_t* voff = vkey[1];                          // free after the depth passes
     uint32_t* unit_first = reinterpret_cast<uint32_t*>(ws + L.unit_first);
     offsets_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], tile_count, hdr, offsets_status, voff, unit_first,
-                                                                   (uint32_t)(pair_capacity / EMIT_PAIRS + 1));
+                                                                   (uint32_t)(pair_capacity / EMIT_PAIRS + 1),
+                                                                   (unsigned long long)pair_capacity);
     XPR_LAUNCH_CHECK();
-    unsigned long long total = 0;
-    XPR_CUDA(cudaMemcpyAsync(&total, &hdr->total_pairs, sizeof(total), cudaMemcpyDeviceToHost, st));
-    XPR_CUDA(cudaStreamSynchronize(st));
-    *num_pairs_host = (int64_t)total;
-    if ((int64_t)total > pair_capacity) return XPR_ERR_CAPACITY;
-    if (total == 0) {
-        XPR_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)T, st));
-        return XPR_OK;
-    }
-    const uint32_t I = (uint32_t)total;
     // 4. replicate in depth order as packed words; pass p reads buffer p and writes buffer p+1, the last
     //    one writes keys_sorted / vals_sorted, so emission starts in keys_sorted when tpasses is even
     uint64_t* w0 = (tpasses % 2 == 0) ? keys_sorted : keys_tmp;
     uint64_t* w1 = (tpasses % 2 == 0) ? keys_tmp : keys_sorted;
-    const unsigned units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
-    const unsigned egrid = units < (unsigned)PERSIST_CTAS ? units : (unsigned)PERSIST_CTAS;
+    const unsigned units_cap = (unsigned)((pair_capacity + EMIT_PAIRS - 1) / EMIT_PAIRS);
+    const unsigned tiles64 = (unsigned)((pair_capacity + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64));
+    if (pair_capacity > 0) {
+        const unsigned egrid = units_cap < (unsigned)PERSIST_CTAS ? units_cap : (unsigned)PERSIST_CTAS;
 #define XPR_EMIT(TP)                                                                                             \
-    emit_kernel<TP><<<egrid, EMIT_THREADS, 0, st>>>(I, TW, vidx[0], voff, unit_first,                             \
+    emit_kernel<TP><<<egrid, EMIT_THREADS, 0, st>>>(TW, vidx[0], voff, unit_first,                                \
                                                     reinterpret_cast<const int4*>(tile_rect), hdr, w0)
-    switch (tpasses) {
-        case 1: XPR_EMIT(1); break;
-        case 2: XPR_EMIT(2); break;
-        case 3: XPR_EMIT(3); break;
-        default: XPR_EMIT(4); break;
-    }
+        switch (tpasses) {
+            case 1: XPR_EMIT(1); break;
+            case 2: XPR_EMIT(2); break;
+            case 3: XPR_EMIT(3); break;
+            default: XPR_EMIT(4); break;
+        }
 #undef XPR_EMIT
-    XPR_LAUNCH_CHECK();
-    // 5. the tile-id digits, on the I pairs
-    const unsigned tiles64 = (I + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
-    XPR_CUDA(cudaMemsetAsync(status64, 0, sizeof(uint32_t) * (size_t)RADIX * tiles64 * (size_t)tpasses, st));
-    for (int p = 0; p < tpasses; ++p) {
-        uint32_t* status = status64 + (size_t)p * RADIX * tiles64;
-        const int row = DEPTH_PASSES + p, shift = 32 + 8 * p;
-        const bool last = (p == tpasses - 1);
-        cudaError_t e;
-        // digit 0: consecutive pairs of a Gaussian are consecutive tiles -> bitmap ranking
-        if (!last)       e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
-                                      : launch_pass<uint64_t, IPT64, false, 1>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr);
-        else             e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
-                                      : launch_pass<uint64_t, IPT64, false, 2>(tiles64, st, nullptr, &hdr->total_pairs, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0]);
-        XPR_CUDA(e);
-        uint64_t* t = w0; w0 = w1; w1 = t;
+        XPR_LAUNCH_CHECK();
+        // 5. the tile-id digits, on the I pairs
+        for (int p = 0; p < tpasses; ++p) {
+            uint32_t* status = status64 + (size_t)p * RADIX * tiles64;
+            const int row = DEPTH_PASSES + p, shift = 32 + 8 * p;
+            const bool last = (p == tpasses - 1);
+            cudaError_t e;
+            // bitmap ranking: consecutive pairs of a Gaussian are consecutive tiles (digit 0); after pass 1 a
+            // warp holds many distinct high digits
+            if (!last)       e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
+                                          : launch_pass<uint64_t, IPT64, false, 1>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr);
+            else             e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
+                                          : launch_pass<uint64_t, IPT64, false, 2>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0]);
+            XPR_CUDA(e);
+            uint64_t* t = w0; w0 = w1; w1 = t;
+        }
     }
-    // 6. per-tile ranges
-    ranges_kernel<<<((unsigned)T + 7) / 8, 256, 0, st>>>(I, (uint32_t)T, keys_sorted, tile_ranges);
+    // 6. per-tile ranges ((0, 0) for every tile when there are no pairs or they exceed the capacity)
+    ranges_kernel<<<((unsigned)T + 7) / 8, 256, 0, st>>>(&hdr->pairs_eff, (uint32_t)T, keys_sorted, tile_ranges);
     XPR_LAUNCH_CHECK();
-    return XPR_OK;
+    if (!num_pairs_host) return XPR_OK;                // asynchronous mode: the caller reads the count later
+    unsigned long long total = 0;
+    XPR_CUDA(cudaMemcpyAsync(&total, &hdr->total_pairs, sizeof(total), cudaMemcpyDeviceToHost, st));
+    XPR_CUDA(cudaStreamSynchronize(st));
+    *num_pairs_host = (int64_t)total;
+    return ((int64_t)total > pair_capacity) ? XPR_ERR_CAPACITY : XPR_OK;
 }

@@ -70,6 +70,24 @@ class SplatPipeline:
                 raise xb.XprError(st, "xpr_bin_sort (pair count exceeds 2^30)")
             self._alloc_pairs(int(n * 1.25) + 1024)   # XPR_ERR_CAPACITY: regrow and redo
 
+    def bin_sort_async(self):
+        """xpr_bin_sort without the host read-back of I (num_pairs_host = NULL): nothing in the step waits for
+        the host, so the whole step can be enqueued ahead or captured in a CUDA graph.  The buffers must have
+        been sized by an earlier bin_sort(); pairs_on_device() / check_capacity() read the count afterwards."""
+        xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg, self.pair_capacity,
+                        self.keys_sorted, self.vals_sorted, self.tile_ranges, self.workspace, sync=False)
+
+    def pairs_on_device(self) -> int:
+        """I of the last bin_sort call, from the first 8 bytes of the workspace (synchronises)."""
+        return int(self.workspace[:8].view(torch.int64).item())
+
+    def check_capacity(self):
+        n = self.pairs_on_device()
+        if n > self.pair_capacity:
+            raise xb.XprError(xb.XPR_ERR_CAPACITY, f"xpr_bin_sort (asynchronous): {n} pairs > capacity {self.pair_capacity}")
+        self.num_pairs = n
+        return n
+
     def rasterize_fwd(self):
         xb.xpr_rasterize_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
                              self.tile_ranges, self.image, self.final_T, self.n_contrib)

@@ -90,7 +90,7 @@ def test_workspace_size_monotone(lib):
     a = xb.xpr_bin_sort_workspace(1000, 10_000, 16)
     b = xb.xpr_bin_sort_workspace(1000, 1_000_000, 8160)
     assert 0 < a < b
-    assert b >= 12 * 1_000_000       # double buffer for keys (8 B) and values (4 B)
+    assert b >= 8 * 1_000_000        # the second buffer of 8-byte packed words (tile << 32 | rank)
     with pytest.raises(xb.XprError):
         xb.xpr_bin_sort_workspace(1000, 1 << 30, 16)
 

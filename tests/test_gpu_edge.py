@@ -100,3 +100,37 @@ def test_many_sort_tiles_and_all_digit_passes():
     r = g["binned"]["ranges"].astype(np.int64)
     nz = r[:, 1] > r[:, 0]
     assert (r[nz, 1] - r[nz, 0]).sum() == o["binned"]["num_pairs"]     # ranges partition [0, I)
+
+
+def test_async_bin_sort_matches_sync_and_overflow_renders_background():
+    """num_pairs_host = NULL: no host read-back; I is left in the first 8 bytes of the workspace.  Same outputs
+    as the synchronous call; over capacity every tile range is (0, 0) and nothing is written out of bounds."""
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline
+    sc = scenes.make_scene(2, n_override=20000, image_override=(200, 200))
+    cfg = scenes.default_render_config(sc)
+    params = pipeline.scene_to_device(sc)
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg)
+    pipe.project(*params)
+    I = pipe.bin_sort()
+    keys = pipe.keys_sorted[:I].clone(); vals = pipe.vals_sorted[:I].clone(); ranges = pipe.tile_ranges.clone()
+    pipe.keys_sorted.fill_(-1); pipe.vals_sorted.fill_(-1); pipe.tile_ranges.fill_(-1)
+    pipe.bin_sort_async()
+    assert pipe.check_capacity() == I
+    assert torch.equal(pipe.keys_sorted[:I], keys) and torch.equal(pipe.vals_sorted[:I], vals)
+    assert torch.equal(pipe.tile_ranges, ranges)
+    # over capacity, asynchronously
+    small = pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg, pair_capacity=4096)
+    small.project(*params)
+    guard = torch.full((8192,), -7, dtype=torch.int64, device="cuda")
+    xb.xpr_bin_sort(small.depth, small.tile_rect, small.tile_count, small.cam, small.cfg, 4096, guard,
+                    small.vals_sorted, small.tile_ranges, small.workspace, sync=False)
+    torch.cuda.synchronize()
+    assert small.pairs_on_device() == I
+    assert (guard[4096:] == -7).all()
+    assert not small.tile_ranges.any()
+    with pytest.raises(xb.XprError):
+        small.check_capacity()
+    small.rasterize_fwd()
+    torch.cuda.synchronize()
+    assert float(small.image.abs().max()) == 0.0 and float(small.final_T.min()) == 1.0
