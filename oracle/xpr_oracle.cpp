@@ -742,16 +742,92 @@ extern "C" int64_t xpr_oracle_emit(int64_t N, const float* depth, const int32_t*
     return I;
 }
 
+// ---------------------------------------------------------------------------------------------
+// tile_cull of XPR-3DGS ("Cull", Listing 1, A.1.1 L435; StopThePop): keep the pair
+// (primitive, tile) iff the maximum of alpha = o G_2D(x) over the tile reaches alpha_thresh, i.e. iff
+//   min_{x in tile} 1/2 (x - mu)^T K (x - mu) <= ln(o / alpha_thresh) = lnv,   K = [[A, B], [B, C]].
+// "Tile" is the hull of the tile's pixel centres [ts*tx + 1/2, ts*tx + ts - 1/2]^2 (reading C8, C1).
+// The minimiser is mu when mu is inside, else it lies on an edge facing mu (the response falls off
+// along every ray from mu, L435): on the vertical edge x = xe the minimiser over y is
+// dy = clamp(-B dx / C, ...), on the horizontal edge y = ye it is dx = clamp(-B dy / A, ...).
+// fp32 evaluation order and the conservative margin are fixed in DESIGN.md reading C8: a pair is
+// dropped only if q > lnv + 2^-18 (|a| + |b| + |c| + lnv), with q = (a + b) + c,
+// a = ((A/2) dx) dx, b = (B dx) dy, c = ((C/2) dy) dy.  Written so that a NaN keeps the pair.
+// ---------------------------------------------------------------------------------------------
+template <class S>
+bool tile_keep(S mx, S my, S A, S B, S C, S lnv, int32_t tx, int32_t ty, int32_t ts) {
+    const S x0 = S(ts) * S(tx) + S(0.5), x1 = (S(ts) * S(tx) + S(ts)) - S(0.5);
+    const S y0 = S(ts) * S(ty) + S(0.5), y1 = (S(ts) * S(ty) + S(ts)) - S(0.5);
+    const bool in_x = (mx >= x0) && (mx <= x1), in_y = (my >= y0) && (my <= y1);
+    if (in_x && in_y) return true;
+    const S margin = S(1.0 / 262144.0);   // 2^-18
+    auto drop = [&](S dx, S dy) {
+        const S a = ((S(0.5) * A) * dx) * dx, b = (B * dx) * dy, c = ((S(0.5) * C) * dy) * dy;
+        const S q = (a + b) + c;
+        const S mag = ((std::fabs(a) + std::fabs(b)) + std::fabs(c)) + lnv;
+        return q > lnv + mag * margin;
+    };
+    bool dropped = true;                   // dropped by every facing edge
+    if (!in_x) {
+        const S dx = ((mx < x0) ? x0 : x1) - mx;
+        S dy = (-(B * dx)) / C;
+        const S lo = y0 - my, hi = y1 - my;
+        dy = (dy < lo) ? lo : dy; dy = (hi < dy) ? hi : dy;
+        dropped = dropped && drop(dx, dy);
+    }
+    if (!in_y) {
+        const S dy = ((my < y0) ? y0 : y1) - my;
+        S dx = (-(B * dy)) / A;
+        const S lo = x0 - mx, hi = x1 - mx;
+        dx = (dx < lo) ? lo : dx; dx = (hi < dx) ? hi : dx;
+        dropped = dropped && drop(dx, dy);
+    }
+    return !dropped;
+}
+
+#define XO_KEEP(S, T)                                                                                     \
+    extern "C" void xpr_oracle_tile_keep_##S(int64_t n, const T* mean2d, const T* conic, const T* lnv,     \
+                                             const int32_t* tile_xy, int32_t ts, uint8_t* keep) {          \
+        for (int64_t i = 0; i < n; ++i)                                                                   \
+            keep[i] = tile_keep<T>(mean2d[2 * i], mean2d[2 * i + 1], conic[3 * i], conic[3 * i + 1],       \
+                                   conic[3 * i + 2], lnv[i], tile_xy[2 * i], tile_xy[2 * i + 1], ts) ? 1 : 0; \
+    }
+XO_KEEP(f32, float)
+XO_KEEP(f64, double)
+
+// Replicate + assign tile id + cull: as xpr_oracle_emit, but a pair that fails tile_cull
+// is not emitted (the paper keeps its slot with tile id T so that it sorts behind every tile and
+// belongs to no segment; dropping it gives the same per-tile segments).  Decisions in fp32.
+extern "C" int64_t xpr_oracle_emit_cull(int64_t N, const float* depth, const int32_t* rect, const uint32_t* tcount,
+                                        const float* mean2d, const float* conic, const float* lnv, int32_t tiles_x,
+                                        int32_t ts, int64_t capacity, uint64_t* keys, uint32_t* vals) {
+    int64_t I = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        const uint32_t tc = tcount[i];
+        if (tc == 0) continue;
+        const int32_t w = rect[4 * i + 2] - rect[4 * i];
+        for (uint32_t r = 0; r < tc; ++r) {
+            const int32_t x = rect[4 * i] + (int32_t)(r % (uint32_t)w);
+            const int32_t y = rect[4 * i + 1] + (int32_t)(r / (uint32_t)w);
+            if (!tile_keep<float>(mean2d[2 * i], mean2d[2 * i + 1], conic[3 * i], conic[3 * i + 1], conic[3 * i + 2],
+                                  lnv[i], x, y, ts))
+                continue;
+            if (I < capacity) {
+                const uint64_t t = (uint64_t)y * (uint64_t)tiles_x + (uint64_t)x;
+                keys[I] = (t << 32) | (uint64_t)float_bits(depth[i]);
+                vals[I] = (uint32_t)i;
+            }
+            ++I;
+        }
+    }
+    return I;
+}
+
 // Sort by (tile, depth) and identify bounds.  Stable sort on index-ordered emission
 // gives the tie-break "lower primitive index first" (C10).  Empty tiles get (0, 0).
-extern "C" int64_t xpr_oracle_bin_sort(int64_t N, const float* depth, const int32_t* rect, const uint32_t* tcount,
-                                       int32_t tiles_x, int32_t tiles_y, int64_t capacity, uint64_t* keys_sorted,
-                                       uint32_t* vals_sorted, uint32_t* ranges) {
-    const int64_t I = xpr_oracle_emit(N, depth, rect, tcount, tiles_x, 0, nullptr, nullptr);
-    if (capacity < I) return I;
-    std::vector<uint64_t> keys((size_t)I);
-    std::vector<uint32_t> vals((size_t)I);
-    xpr_oracle_emit(N, depth, rect, tcount, tiles_x, I, keys.data(), vals.data());
+static void sort_and_bounds(int64_t I, const std::vector<uint64_t>& keys, const std::vector<uint32_t>& vals,
+                            int32_t tiles_x, int32_t tiles_y, uint64_t* keys_sorted, uint32_t* vals_sorted,
+                            uint32_t* ranges) {
     std::vector<uint32_t> perm((size_t)I);
     std::iota(perm.begin(), perm.end(), 0u);
     std::stable_sort(perm.begin(), perm.end(), [&](uint32_t x, uint32_t y) { return keys[x] < keys[y]; });
@@ -763,6 +839,31 @@ extern "C" int64_t xpr_oracle_bin_sort(int64_t N, const float* depth, const int3
         if (j == 0 || (keys_sorted[j - 1] >> 32) != t) ranges[2 * t] = (uint32_t)j;
         if (j == I - 1 || (keys_sorted[j + 1] >> 32) != t) ranges[2 * t + 1] = (uint32_t)(j + 1);
     }
+}
+
+extern "C" int64_t xpr_oracle_bin_sort(int64_t N, const float* depth, const int32_t* rect, const uint32_t* tcount,
+                                       int32_t tiles_x, int32_t tiles_y, int64_t capacity, uint64_t* keys_sorted,
+                                       uint32_t* vals_sorted, uint32_t* ranges) {
+    const int64_t I = xpr_oracle_emit(N, depth, rect, tcount, tiles_x, 0, nullptr, nullptr);
+    if (capacity < I) return I;
+    std::vector<uint64_t> keys((size_t)I);
+    std::vector<uint32_t> vals((size_t)I);
+    xpr_oracle_emit(N, depth, rect, tcount, tiles_x, I, keys.data(), vals.data());
+    sort_and_bounds(I, keys, vals, tiles_x, tiles_y, keys_sorted, vals_sorted, ranges);
+    return I;
+}
+
+// The same with tile_cull ("Cull"): returns the number of surviving pairs.
+extern "C" int64_t xpr_oracle_bin_sort_cull(int64_t N, const float* depth, const int32_t* rect, const uint32_t* tcount,
+                                            const float* mean2d, const float* conic, const float* lnv, int32_t tiles_x,
+                                            int32_t tiles_y, int32_t ts, int64_t capacity, uint64_t* keys_sorted,
+                                            uint32_t* vals_sorted, uint32_t* ranges) {
+    const int64_t I = xpr_oracle_emit_cull(N, depth, rect, tcount, mean2d, conic, lnv, tiles_x, ts, 0, nullptr, nullptr);
+    if (capacity < I) return I;
+    std::vector<uint64_t> keys((size_t)I);
+    std::vector<uint32_t> vals((size_t)I);
+    xpr_oracle_emit_cull(N, depth, rect, tcount, mean2d, conic, lnv, tiles_x, ts, I, keys.data(), vals.data());
+    sort_and_bounds(I, keys, vals, tiles_x, tiles_y, keys_sorted, vals_sorted, ranges);
     return I;
 }
 

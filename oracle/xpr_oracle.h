@@ -17,7 +17,8 @@
  * Pins (tests/test_oracle_*.py, run with -m "not gpu"): P1 closed form single Gaussian, P2
  * transmittance/opacity invariants, P3 brute-force binning, P4 tiling invariance, P5 sort
  * invariants, P6 central finite differences (fp64), P7 UT exact for affine maps, P8 UT~EWA limit,
- * P9 fisheye special cases, P10 SH orthonormality/degree-0, P11 linearity, P12 fp32-vs-fp64.
+ * P9 fisheye special cases, P10 SH orthonormality/degree-0, P11 linearity, P12 fp32-vs-fp64,
+ * P13 tile_cull (dense-sampling maximum, no passing pixel in a dropped pair, image unchanged).
  * No function here is "parity unpinned".
  */
 #ifndef XPR_ORACLE_H
@@ -44,6 +45,7 @@ typedef struct {
     double ut_alpha, ut_beta, ut_kappa;
     double bg[3];
     double fragile_rel;         /* relative margin of the fragile-pixel protocol */
+    int32_t tile_cull;          /* 1: drop (primitive, tile) pairs that fail tile_cull */
 } xo_config;
 
 /* flags byte written by project */
@@ -111,6 +113,21 @@ int64_t xpr_oracle_bin_sort(int64_t N, const float* depth, const int32_t* tile_r
 int64_t xpr_oracle_emit(int64_t N, const float* depth, const int32_t* tile_rect,
                         const uint32_t* tile_count, int32_t tiles_x, int64_t capacity,
                         uint64_t* keys, uint32_t* vals);
+
+/* tile_cull of XPR-3DGS ("Cull", L268-281, L435): keep[i] = 1 iff the maximum of alpha over the
+ * hull of the pixel centres of tile tile_xy[i] reaches alpha_thresh (conservative margin: DESIGN.md C8). */
+void xpr_oracle_tile_keep_f32(int64_t n, const float* mean2d, const float* conic, const float* lnv,
+                              const int32_t* tile_xy, int32_t ts, uint8_t* keep);
+void xpr_oracle_tile_keep_f64(int64_t n, const double* mean2d, const double* conic, const double* lnv,
+                              const int32_t* tile_xy, int32_t ts, uint8_t* keep);
+/* Emission and binning with tile_cull: pairs that fail it are not emitted.  Return the surviving count. */
+int64_t xpr_oracle_emit_cull(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
+                             const float* mean2d, const float* conic, const float* lnv, int32_t tiles_x,
+                             int32_t ts, int64_t capacity, uint64_t* keys, uint32_t* vals);
+int64_t xpr_oracle_bin_sort_cull(int64_t N, const float* depth, const int32_t* tile_rect,
+                                 const uint32_t* tile_count, const float* mean2d, const float* conic,
+                                 const float* lnv, int32_t tiles_x, int32_t tiles_y, int32_t ts, int64_t capacity,
+                                 uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges);
 
 int32_t xpr_oracle_num_threads(void);
 

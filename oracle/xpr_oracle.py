@@ -29,7 +29,7 @@ class XoConfig(C.Structure):
                 ("alpha_thresh", C.c_double), ("alpha_max", C.c_double), ("t_min", C.c_double),
                 ("z_near", C.c_double), ("lowpass", C.c_double),
                 ("ut_alpha", C.c_double), ("ut_beta", C.c_double), ("ut_kappa", C.c_double),
-                ("bg", C.c_double * 3), ("fragile_rel", C.c_double)]
+                ("bg", C.c_double * 3), ("fragile_rel", C.c_double), ("tile_cull", C.c_int32)]
 
 
 _lib = None
@@ -41,6 +41,8 @@ def lib():
         _lib = C.CDLL(_build.build())
         _lib.xpr_oracle_bin_sort.restype = C.c_int64
         _lib.xpr_oracle_emit.restype = C.c_int64
+        _lib.xpr_oracle_emit_cull.restype = C.c_int64
+        _lib.xpr_oracle_bin_sort_cull.restype = C.c_int64
         _lib.xpr_oracle_num_threads.restype = C.c_int32
     return _lib
 
@@ -71,6 +73,7 @@ def make_config(d: dict, fragile_rel: float = 2e-5) -> XoConfig:
     for i in range(3):
         c.bg[i] = float(d["bg"][i])
     c.fragile_rel = float(fragile_rel)
+    c.tile_cull = int(d.get("tile_cull", 0))
     return c
 
 
@@ -100,6 +103,23 @@ def project(means, scales, quats, opacities, sh, cam: XoCamera, cfg: XoConfig, d
     return out
 
 
+def _cull_args(proj: dict):
+    """tile_cull data p_tcd: mean2d, conic, lnv -- always fp32, like depth (the decision is
+    taken on the fp32 projection outputs)."""
+    return (np.ascontiguousarray(proj["mean2d"], np.float32), np.ascontiguousarray(proj["conic"], np.float32),
+            np.ascontiguousarray(proj["lnv"], np.float32))
+
+
+def tile_keep(mean2d, conic, lnv, tile_xy, ts: int, dtype=np.float32):
+    """keep flags of (primitive, tile) pairs: arrays [n,2], [n,3], [n], int32 [n,2]."""
+    sfx = _sfx(dtype)
+    m, c, l = (np.ascontiguousarray(a, dtype) for a in (mean2d, conic, lnv))
+    t = np.ascontiguousarray(tile_xy, np.int32)
+    keep = np.zeros(len(l), np.uint8)
+    getattr(lib(), "xpr_oracle_tile_keep_" + sfx)(C.c_int64(len(l)), _p(m), _p(c), _p(l), _p(t), C.c_int32(ts), _p(keep))
+    return keep.astype(bool)
+
+
 def emit(proj: dict, cam: XoCamera, cfg: XoConfig):
     tx, _ = tiles(cam, cfg)
     N = int(proj["tile_count"].shape[0])
@@ -107,6 +127,12 @@ def emit(proj: dict, cam: XoCamera, cfg: XoConfig):
     I = int(proj["tile_count"].astype(np.int64).sum())
     keys = np.empty(I, np.uint64)
     vals = np.empty(I, np.uint32)
+    if cfg.tile_cull:
+        m, c, l = _cull_args(proj)
+        n = lib().xpr_oracle_emit_cull(C.c_int64(N), _p(depth), _p(proj["tile_rect"]), _p(proj["tile_count"]), _p(m),
+                                       _p(c), _p(l), C.c_int32(tx), C.c_int32(cfg.tile), C.c_int64(I), _p(keys), _p(vals))
+        assert n <= I
+        return keys[:n], vals[:n]
     n = lib().xpr_oracle_emit(C.c_int64(N), _p(depth), _p(proj["tile_rect"]), _p(proj["tile_count"]), C.c_int32(tx),
                               C.c_int64(I), _p(keys), _p(vals))
     assert n == I
@@ -121,10 +147,17 @@ def bin_sort(proj: dict, cam: XoCamera, cfg: XoConfig) -> dict:
     keys = np.empty(I, np.uint64)
     vals = np.empty(I, np.uint32)
     ranges = np.zeros((tx * ty, 2), np.uint32)
+    if cfg.tile_cull:
+        m, c, l = _cull_args(proj)
+        n = lib().xpr_oracle_bin_sort_cull(C.c_int64(N), _p(depth), _p(proj["tile_rect"]), _p(proj["tile_count"]),
+                                           _p(m), _p(c), _p(l), C.c_int32(tx), C.c_int32(ty), C.c_int32(cfg.tile),
+                                           C.c_int64(I), _p(keys), _p(vals), _p(ranges))
+        assert n <= I, (n, I)
+        return dict(keys=keys[:n].copy(), vals=vals[:n].copy(), ranges=ranges, num_pairs=int(n), num_candidates=I)
     n = lib().xpr_oracle_bin_sort(C.c_int64(N), _p(depth), _p(proj["tile_rect"]), _p(proj["tile_count"]),
                                   C.c_int32(tx), C.c_int32(ty), C.c_int64(I), _p(keys), _p(vals), _p(ranges))
     assert n == I, (n, I)
-    return dict(keys=keys, vals=vals, ranges=ranges, num_pairs=I)
+    return dict(keys=keys, vals=vals, ranges=ranges, num_pairs=I, num_candidates=I)
 
 
 def rasterize_fwd(proj: dict, binned: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:

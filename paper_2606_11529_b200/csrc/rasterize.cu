@@ -207,7 +207,10 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
 // leaves the totals spread over lanes, which issue two RED instructions (8 lanes + 1 lane).
 constexpr int BWD_THREADS = 64, BWD_PPT = 4, BWD_BATCH = 64;
 
-__global__ void __launch_bounds__(BWD_THREADS)
+#ifndef XPR_BWD_MINB
+#define XPR_BWD_MINB 1
+#endif
+__global__ void __launch_bounds__(BWD_THREADS, XPR_BWD_MINB)
 rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
