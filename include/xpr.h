@@ -57,6 +57,7 @@ typedef struct {
     float lowpass;          /* 0.3 added to the 2D covariance diagonal (C4) */
     float ut_alpha, ut_beta, ut_kappa;  /* unscented-transform weights: 1, 2, 0 */
     float bg[3];            /* background colour (C13) */
+    int32_t tile_cull;      /* 1: xpr_bin_sort_cull drops (Gaussian, tile) pairs that fail tile_cull */
 } xpr_config;
 
 const char* xpr_status_string(int32_t status);
@@ -94,8 +95,8 @@ int32_t xpr_project(int64_t N, const float* means, const float* scales, const fl
  *   there.  With num_pairs_host != NULL the call ends with an 8-byte read-back of I and a stream
  *   synchronisation; I > pair_capacity -> XPR_ERR_CAPACITY with *num_pairs_host = required I.
  *   With num_pairs_host == NULL the call is fully asynchronous (capturable in a CUDA graph): it
- *   returns XPR_OK after enqueueing, and the first 8 bytes of `workspace` hold I (uint64) once the
- *   stream has run; the caller must compare it with pair_capacity before trusting the outputs.
+ *   returns XPR_OK after enqueueing, and the first 16 bytes of `workspace` hold I twice (uint64:
+ *   candidates, pairs in the output) once the stream has run; the caller must compare it with pair_capacity before trusting the outputs.
  *   In both modes, when I > pair_capacity nothing out of bounds is written, tile_ranges is (0,0) for
  *   every tile (a following xpr_rasterize_fwd renders the background) and keys/vals are unspecified.
  *   workspace: DEVICE scratch of at least xpr_bin_sort_workspace() bytes, 256-byte aligned.
@@ -106,6 +107,30 @@ int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* tile_rect, co
                      const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
                      uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
                      int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * xpr_bin_sort_cull -- xpr_bin_sort with the optional "Cull" step of the paper's rasterizer (
+ * tile_cull of XPR-3DGS: Listing 1, A.1.1 L435, after StopThePop).  With cfg->tile_cull != 0 a
+ * candidate pair (Gaussian, tile) is kept iff the maximum of alpha = o G_2D(x) over the hull of the
+ * tile's pixel centres reaches alpha_thresh, i.e. iff min 1/2 d^T K d <= lnv; the minimiser is the mean
+ * if it lies inside, else a point on an edge facing the mean.  The decision is conservative (margin
+ * 2^-18 of the magnitude of the terms, reading C8), so every dropped pair has alpha <
+ * alpha_thresh at all of its pixels and the image, final_T and the gradients are those of xpr_bin_sort
+ * (PAPER L683); n_contrib, which counts list positions, refers to the shorter lists.
+ * The paper keeps a rejected pair in its slot with tile id T; here it is not written at all: the
+ * survivors are compacted in emission order and only they are sorted.
+ *   in : as xpr_bin_sort + the tile-cull data p_tcd of xpr_project: mean2d[N,2], conic_opac[N,4], lnv[N].
+ *   out: as xpr_bin_sort; *num_pairs_host = number of SURVIVING pairs (= length of the sorted arrays).
+ *   pair_capacity must hold the CANDIDATE count (sum of tile_count); otherwise XPR_ERR_CAPACITY with
+ *   *num_pairs_host = that count.  Asynchronous mode: workspace bytes [0,8) = candidate count,
+ *   bytes [8,16) = surviving count (for xpr_bin_sort both are I).
+ *   With cfg->tile_cull == 0 the call is xpr_bin_sort; xpr_bin_sort itself rejects cfg->tile_cull != 0.
+ */
+int32_t xpr_bin_sort_cull(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
+                          const float* mean2d, const float* conic_opac, const float* lnv,
+                          const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
+                          uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
+                          int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
  * xpr_rasterize_fwd -- Shader stage (Algorithm 1, Listing 1).

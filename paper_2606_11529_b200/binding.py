@@ -18,7 +18,7 @@ XPR_OK, XPR_ERR_INVALID_ARG, XPR_ERR_CAPACITY, XPR_ERR_CUDA, XPR_ERR_UNSUPPORTED
 FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_RGB_POS_B = 1, 2, 4, 8, 16, 32
 
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
-           "xpr_bin_sort", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd")
+           "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd")
 
 
 class XprCamera(C.Structure):
@@ -31,7 +31,7 @@ class XprConfig(C.Structure):
     _fields_ = [("projection", C.c_int32), ("sh_degree", C.c_int32), ("tile", C.c_int32), ("antialias", C.c_int32),
                 ("alpha_thresh", C.c_float), ("alpha_max", C.c_float), ("t_min", C.c_float), ("z_near", C.c_float),
                 ("lowpass", C.c_float), ("ut_alpha", C.c_float), ("ut_beta", C.c_float), ("ut_kappa", C.c_float),
-                ("bg", C.c_float * 3)]
+                ("bg", C.c_float * 3), ("tile_cull", C.c_int32)]
 
 
 class XprError(RuntimeError):
@@ -82,6 +82,7 @@ def make_config(d: dict) -> XprConfig:
     c.ut_alpha, c.ut_beta, c.ut_kappa = float(d["ut_alpha"]), float(d["ut_beta"]), float(d["ut_kappa"])
     for i in range(3):
         c.bg[i] = float(d["bg"][i])
+    c.tile_cull = int(d.get("tile_cull", 0))
     return c
 
 
@@ -131,16 +132,22 @@ def xpr_bin_sort_workspace(N: int, pair_capacity: int, n_tiles: int) -> int:
 
 
 def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, pair_capacity: int, keys_sorted,
-                 vals_sorted, tile_ranges, workspace, stream=None, raise_on_capacity: bool = True, sync: bool = True):
+                 vals_sorted, tile_ranges, workspace, stream=None, raise_on_capacity: bool = True, sync: bool = True,
+                 cull_data=None):
     """Returns (status, I).  On XPR_ERR_CAPACITY I is the required capacity.
+    cull_data = (mean2d, conic_opac, lnv): call xpr_bin_sort_cull (tile_cull applied when cfg.tile_cull != 0).
     sync=False: num_pairs_host = NULL -- nothing waits for the host, I is returned as None and stays in the
     first 8 bytes of `workspace` (xpr.h); the caller checks it against pair_capacity later."""
     N = int(tile_count.shape[0])
     n_pairs = C.c_int64(0)
-    st = lib().xpr_bin_sort(C.c_int64(N), _p(depth), _p(tile_rect), _p(tile_count), C.byref(cam), C.byref(cfg),
-                            C.c_int64(pair_capacity), _p(keys_sorted), _p(vals_sorted), _p(tile_ranges),
-                            C.byref(n_pairs) if sync else None, _p(workspace),
-                            C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    tail = (C.byref(cam), C.byref(cfg), C.c_int64(pair_capacity), _p(keys_sorted), _p(vals_sorted), _p(tile_ranges),
+            C.byref(n_pairs) if sync else None, _p(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+            _stream(stream))
+    if cull_data is None:
+        st = lib().xpr_bin_sort(C.c_int64(N), _p(depth), _p(tile_rect), _p(tile_count), *tail)
+    else:
+        st = lib().xpr_bin_sort_cull(C.c_int64(N), _p(depth), _p(tile_rect), _p(tile_count), _p(cull_data[0]),
+                                     _p(cull_data[1]), _p(cull_data[2]), *tail)
     if not sync:
         _check(st, "xpr_bin_sort")
         return st, None

@@ -57,6 +57,7 @@ constexpr int PERSIST_CTAS = 148 * 4;       // upper bound of the persistent gri
 constexpr int EMIT_THREADS = 256, EMIT_PPT = 8, EMIT_PAIRS = EMIT_THREADS * EMIT_PPT;   // emit: 2048 pairs per unit
 constexpr int EMIT_WARPS = EMIT_THREADS / 32;
 constexpr int EMIT_SHIFT = 11;
+static_assert(EMIT_PPT * EMIT_WARPS == 64, "emit's survivor scan handles two counts per lane of one warp");
 static_assert(EMIT_PAIRS == 1 << EMIT_SHIFT, "unit_first is indexed by pair offset >> EMIT_SHIFT");
 
 constexpr uint32_t FLAG_PARTIAL = 1u << 30, FLAG_INCLUSIVE = 2u << 30, FLAG_MASK = 3u << 30, VALUE_MASK = ~FLAG_MASK;
@@ -65,16 +66,17 @@ constexpr unsigned long long SFLAG_PARTIAL = 1ull << 62, SFLAG_INCLUSIVE = 2ull 
 // Header at the start of the workspace (zeroed every call).
 struct Header {
     unsigned long long total_pairs;          // I (first 8 bytes of the workspace: readable by the caller)
-    unsigned long long pairs_eff;            // I if it fits pair_capacity, else 0: what the pair kernels process
+    unsigned long long pairs_out;            // pairs in the sorted output: I, or the survivors of tile_cull (second 8 bytes)
+    unsigned long long pairs_eff;            // I if it fits pair_capacity, else 0: what emit expands
     uint32_t n_vis;                          // visible Gaussians
-    uint32_t compact_ticket, emit_ticket;
+    uint32_t compact_ticket, emit_ticket, unit_ticket;
     uint32_t sort_ticket[DEPTH_PASSES + MAX_TILE_PASSES];
-    uint32_t pad[3];
+    uint32_t pad[4];
     uint32_t hist[(DEPTH_PASSES + MAX_TILE_PASSES) * RADIX];   // global digit histograms
 };
 
 struct Layout {
-    size_t header, scan_status, vkey0, vidx0, vkey1, vidx1, status32, keys_tmp, status64, unit_first, total;
+    size_t header, scan_status, vkey0, vidx0, vkey1, vidx1, status32, keys_tmp, status64, unit_status, unit_first, total;
 };
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -97,6 +99,7 @@ inline Layout make_layout(int64_t N, int64_t cap, int32_t num_tiles) {
     L.status32 = off; off = align_up(off + 4 * (size_t)RADIX * tiles32 * DEPTH_PASSES, 256);
     const size_t tiles64 = (c + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64);
     L.status64 = off; off = align_up(off + 4 * (size_t)RADIX * tiles64 * (size_t)tile_passes_for(num_tiles), 256);
+    L.unit_status = off; off = align_up(off + 8 * (c / EMIT_PAIRS + 2), 256);    // emit's chain over units (tile_cull)
     // everything up to here is zeroed with one memset
     L.vkey0 = off; off = align_up(off + 4 * n, 256);
     L.vidx0 = off; off = align_up(off + 4 * n, 256);
@@ -332,52 +335,102 @@ __device__ __forceinline__ uint32_t slot_rcp(uint32_t w) {   // bits of ~1/w (rc
     return __float_as_uint(y);
 }
 
-template <int TILE_PASSES>
+// tile_cull of XPR-3DGS ("Cull", Listing 1, A.1.1 L435): true when the pair survives,
+// i.e. unless min over the hull of the tile's pixel centres of 1/2 d^T K d exceeds lnv = ln(o / alpha_thresh)
+// by more than the conservative margin.  Evaluation order and margin are reading C8 of DESIGN.md; every
+// operation is individually rounded (explicit _rn intrinsics: this file is compiled with FMA contraction).
+__device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, float C, float lnv, uint32_t tx, uint32_t ty) {
+    const float ts = (float)TILE;
+    const float x0 = __fadd_rn(__fmul_rn(ts, (float)tx), 0.5f), x1 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)tx), ts), 0.5f);
+    const float y0 = __fadd_rn(__fmul_rn(ts, (float)ty), 0.5f), y1 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)ty), ts), 0.5f);
+    const bool in_x = (mx >= x0) && (mx <= x1), in_y = (my >= y0) && (my <= y1);
+    if (in_x && in_y) return true;
+    const float margin = 1.0f / 262144.0f;   // 2^-18
+    auto drop = [&](float dx, float dy) {
+        const float a = __fmul_rn(__fmul_rn(__fmul_rn(0.5f, A), dx), dx), b = __fmul_rn(__fmul_rn(B, dx), dy),
+                    c = __fmul_rn(__fmul_rn(__fmul_rn(0.5f, C), dy), dy);
+        const float q = __fadd_rn(__fadd_rn(a, b), c);
+        const float mag = __fadd_rn(__fadd_rn(__fadd_rn(fabsf(a), fabsf(b)), fabsf(c)), lnv);
+        return q > __fadd_rn(lnv, __fmul_rn(mag, margin));
+    };
+    bool dropped = true;                      // dropped by every facing edge
+    if (!in_x) {
+        const float dx = __fsub_rn((mx < x0) ? x0 : x1, mx);
+        float dy = __fdiv_rn(-__fmul_rn(B, dx), C);
+        const float lo = __fsub_rn(y0, my), hi = __fsub_rn(y1, my);
+        dy = (dy < lo) ? lo : dy; dy = (hi < dy) ? hi : dy;
+        dropped = dropped && drop(dx, dy);
+    }
+    if (!in_y) {
+        const float dy = __fsub_rn((my < y0) ? y0 : y1, my);
+        float dx = __fdiv_rn(-__fmul_rn(B, dy), A);
+        const float lo = __fsub_rn(x0, mx), hi = __fsub_rn(x1, mx);
+        dx = (dx < lo) ? lo : dx; dx = (hi < dx) ? hi : dx;
+        dropped = dropped && drop(dx, dy);
+    }
+    return !dropped;
+}
+
+// CULL = true (xpr_bin_sort_cull): every pair is tested with tile_keep and only the survivors are written,
+// compacted in order: the survivors of a unit are counted, a chained scan over the units (decoupled look-back)
+// gives the unit its base, and hdr->pairs_out ends up holding the number of surviving pairs.
+template <int TILE_PASSES, bool CULL>
 __global__ void __launch_bounds__(EMIT_THREADS)
 emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
-            const uint32_t* __restrict__ unit_first, const int4* __restrict__ rect, Header* __restrict__ hdr,
-            uint64_t* __restrict__ words) {
-    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, first tile id, rectangle width, bits(~1/width)
+            const uint32_t* __restrict__ unit_first, const int4* __restrict__ rect, const float2* __restrict__ mean2d,
+            const float4* __restrict__ conic_opac, const float* __restrict__ lnv, Header* __restrict__ hdr,
+            unsigned long long* __restrict__ unit_status, uint64_t* __restrict__ words) {
+    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, x_min | y_min << 16, rectangle width, Gaussian index
     __shared__ __align__(16) uint16_t s_mark[EMIT_PAIRS];
     __shared__ uint32_t s_hist[MAX_TILE_PASSES * RADIX];
     __shared__ uint32_t s_wmax[EMIT_WARPS];
+    __shared__ uint32_t s_cnt[EMIT_PPT * EMIT_WARPS];   // survivors per (item, warp), then their exclusive scan
+    __shared__ uint32_t s_unit[2];                   // tickets: this unit's successor (double buffered)
+    __shared__ unsigned long long s_base;
     constexpr int tile_passes = TILE_PASSES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n_vis = hdr->n_vis;
     const uint32_t I = (uint32_t)hdr->pairs_eff;
     const uint32_t units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
     for (int b = tid; b < tile_passes * RADIX; b += EMIT_THREADS) s_hist[b] = 0u;
-    // the first Gaussian of every unit was recorded by offsets_kernel (unit_first), so a unit needs no
-    // search; the candidates of the CTA's NEXT unit are prefetched into registers while the current
-    // one is expanded (the dependent loads voff -> vidx -> rect are off the critical path)
+    // units are drawn from a ticket counter (forward progress of the chain over units); the first Gaussian of
+    // every unit was recorded by offsets_kernel (unit_first), so a unit needs no search; the candidates of the
+    // CTA's NEXT unit are prefetched into registers while the current one is expanded
     uint32_t c_off[EMIT_CAND];
     int4 c_rect[EMIT_CAND];
+    uint32_t c_gid[EMIT_CAND];
     auto load_candidates = [&](uint32_t first) {
 #pragma unroll
         for (int c = 0; c < EMIT_CAND; ++c) {
             const uint32_t s = first + (uint32_t)c * EMIT_THREADS + (uint32_t)tid;
             c_off[c] = 0xffffffffu;                   // beyond the list: never < a pair index
-            if (s < n_vis) { c_off[c] = voff[s]; c_rect[c] = rect[vidx[s]]; }
+            if (s < n_vis) { c_off[c] = voff[s]; c_gid[c] = vidx[s]; c_rect[c] = rect[c_gid[c]]; }
         }
     };
-    uint32_t first = 0, next_first = 0;
-    if (blockIdx.x < units) { first = unit_first[blockIdx.x]; load_candidates(first); }
+    auto make_slot = [&](uint32_t off, const int4& r, uint32_t g) {
+        return make_uint4(off, (uint32_t)r.x | ((uint32_t)r.y << 16), (uint32_t)(r.z - r.x), g);
+    };
+    if (tid == 0) s_unit[0] = atomicAdd(&hdr->unit_ticket, 1u);
+    __syncthreads();
+    uint32_t unit = s_unit[0], first = 0, next_first = 0;
+    if (unit < units) { first = unit_first[unit]; load_candidates(first); }
 
-    for (uint32_t unit = blockIdx.x; unit < units; unit += gridDim.x) {
+    for (int phase = 0; unit < units; phase ^= 1) {
         const uint32_t p0 = unit * (uint32_t)EMIT_PAIRS, p1 = min(I, p0 + (uint32_t)EMIT_PAIRS);
-        const bool has_next = unit + gridDim.x < units;
-        if (has_next) next_first = unit_first[unit + gridDim.x];
+        if (tid == 0) s_unit[phase ^ 1] = atomicAdd(&hdr->unit_ticket, 1u);      // the unit after this one
         __syncthreads();                              // previous unit done with the shared arrays
         reinterpret_cast<uint4*>(s_mark)[tid] = make_uint4(0u, 0u, 0u, 0u);      // 8 marks per thread
         // Gaussians first .. first+cnt-1 cover [p0, p1); cnt <= EMIT_PAIRS because every listed Gaussian
         // after the first starts inside the range (each owns at least one pair)
         const int overflow = __syncthreads_or(c_off[EMIT_CAND - 1] < p1 && tid == EMIT_THREADS - 1);
+        const uint32_t next_unit = s_unit[phase ^ 1];
+        const bool has_next = next_unit < units;
+        if (has_next) next_first = unit_first[next_unit];
 #pragma unroll
         for (int c = 0; c < EMIT_CAND; ++c) {
             if (c_off[c] < p1) {
                 const uint32_t k = (uint32_t)c * EMIT_THREADS + (uint32_t)tid;
-                const int4 r = c_rect[c];
-                s_slot[k] = make_uint4(c_off[c], (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, (uint32_t)(r.z - r.x), slot_rcp((uint32_t)(r.z - r.x)));
+                s_slot[k] = make_slot(c_off[c], c_rect[c], c_gid[c]);
                 s_mark[c_off[c] > p0 ? c_off[c] - p0 : 0u] = (uint16_t)k;
             }
         }
@@ -388,8 +441,8 @@ emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
                 if (s >= n_vis) break;
                 const uint32_t off = voff[s];
                 if (off >= p1) break;
-                const int4 r = rect[vidx[s]];
-                s_slot[k] = make_uint4(off, (uint32_t)r.y * (uint32_t)TW + (uint32_t)r.x, (uint32_t)(r.z - r.x), slot_rcp((uint32_t)(r.z - r.x)));
+                const uint32_t g = vidx[s];
+                s_slot[k] = make_slot(off, rect[g], g);
                 s_mark[off - p0] = (uint16_t)k;
             }
         }
@@ -418,12 +471,13 @@ emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
                                                                m[4] | (m[5] << 16), m[6] | (m[7] << 16));
         }
         __syncthreads();
-        // pair j of slot k: r = j - offset, (ry, rx) = divmod(r, w), tile = tile0 + ry * TW + rx.  The loads of
-        // the 8 pairs of a thread are issued together and the arithmetic is branch-free (8 independent chains).
+        // pair j of slot k: r = j - offset, (ry, rx) = divmod(r, w), tile = (y_min + ry) TW + x_min + rx.  The loads
+        // of the 8 pairs of a thread are issued together and the arithmetic is branch-free (8 independent chains).
         // r / w by an approximate reciprocal: the estimate is within 1 of the quotient while r < 2^22
         // (relative error of the product < 2^-21) and is fixed up on both sides; beyond that, integer division.
-        uint32_t kk[EMIT_PPT];
+        uint32_t kk[EMIT_PPT], tile[EMIT_PPT];
         uint4 sl[EMIT_PPT];
+        bool keep[EMIT_PPT];
 #pragma unroll
         for (int it = 0; it < EMIT_PPT; ++it) kk[it] = s_mark[min((uint32_t)it * EMIT_THREADS + (uint32_t)tid, p1 - p0 - 1u)];
 #pragma unroll
@@ -431,25 +485,73 @@ emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
 #pragma unroll
         for (int it = 0; it < EMIT_PPT; ++it) {
             const uint32_t j = p0 + (uint32_t)it * EMIT_THREADS + (uint32_t)tid;
-            const bool valid = j < p1;                 // false only in the tail of the last unit
+            keep[it] = j < p1;                         // false only in the tail of the last unit
             const uint32_t r = j - sl[it].x, w = sl[it].z;
-            uint32_t ry = (uint32_t)__float2uint_rz(__uint2float_rn(r) * __uint_as_float(sl[it].w));
+            uint32_t ry = (uint32_t)__float2uint_rz(__uint2float_rn(r) * __uint_as_float(slot_rcp(w)));
             const int rem = (int)(r - ry * w);
             ry += (rem >= (int)w ? 1u : 0u) - (rem < 0 ? 1u : 0u);
             if (r >= (1u << 22)) ry = r / w;           // a Gaussian covering more than 4M tiles
-            const uint32_t tile = sl[it].y + ry * (uint32_t)TW + (r - ry * w);
-            if (valid) {
-                words[j] = ((uint64_t)tile << 32) | (uint64_t)(cur_first + kk[it]);
-                atomicAdd(&s_hist[tile & 255u], 1u);      // consecutive tiles -> distinct banks
+            const uint32_t tx = (sl[it].y & 0xffffu) + (r - ry * w), ty = (sl[it].y >> 16) + ry;
+            tile[it] = ty * (uint32_t)TW + tx;
+            if (CULL) {
+                const uint32_t g = sl[it].w;
+                const float2 m = __ldg(mean2d + g);
+                const float4 co = __ldg(conic_opac + g);
+                keep[it] = keep[it] && tile_keep(m.x, m.y, co.x, co.y, co.z, __ldg(lnv + g), tx, ty);
+            }
+        }
+        uint32_t dst[EMIT_PPT];                        // position of a kept pair in the output
+        if (CULL) {
+            // order of the pairs: j = it * 256 + warp * 32 + lane -> exclusive scan over (it, warp), then lanes
+            uint32_t lrank[EMIT_PPT];
+#pragma unroll
+            for (int it = 0; it < EMIT_PPT; ++it) {
+                const uint32_t m = __ballot_sync(0xffffffffu, keep[it]);
+                lrank[it] = (uint32_t)__popc(m & ((1u << lane) - 1u));
+                if (lane == 0) s_cnt[it * EMIT_WARPS + warp] = (uint32_t)__popc(m);
+            }
+            __syncthreads();
+            if (warp == 0) {                           // 64 counts: 2 per lane
+                const uint32_t c0 = s_cnt[2 * lane], c1 = s_cnt[2 * lane + 1];
+                uint32_t incl = c0 + c1;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += v;
+                }
+                const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+                const uint32_t excl = incl - (c0 + c1);
+                s_cnt[2 * lane] = excl; s_cnt[2 * lane + 1] = excl + c0;
+                const unsigned long long base = chain_lookback(unit, total, unit_status, lane);
+                if (lane == 0) {
+                    s_base = base;
+                    if (unit == units - 1u) hdr->pairs_out = base + total;
+                }
+            }
+            __syncthreads();
+            const uint32_t base = (uint32_t)s_base;
+#pragma unroll
+            for (int it = 0; it < EMIT_PPT; ++it) dst[it] = base + s_cnt[it * EMIT_WARPS + warp] + lrank[it];
+        } else {
+#pragma unroll
+            for (int it = 0; it < EMIT_PPT; ++it) dst[it] = p0 + (uint32_t)it * EMIT_THREADS + (uint32_t)tid;
+            if (tid == 0 && unit == units - 1u) hdr->pairs_out = I;
+        }
+#pragma unroll
+        for (int it = 0; it < EMIT_PPT; ++it) {
+            if (keep[it]) {
+                words[dst[it]] = ((uint64_t)tile[it] << 32) | (uint64_t)(cur_first + kk[it]);
+                atomicAdd(&s_hist[tile[it] & 255u], 1u);   // consecutive tiles -> distinct banks
             }
             // higher tile digits are nearly warp-uniform: aggregate with match.any before the atomic
 #pragma unroll
             for (int d = 1; d < tile_passes; ++d) {
-                const uint32_t dig = valid ? ((tile >> (8 * d)) & 255u) : 0xffffffffu;
+                const uint32_t dig = keep[it] ? ((tile[it] >> (8 * d)) & 255u) : 0xffffffffu;
                 const uint32_t peers = __match_any_sync(0xffffffffu, dig);
-                if (valid && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_hist[d * RADIX + dig], (uint32_t)__popc(peers));
+                if (keep[it] && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_hist[d * RADIX + dig], (uint32_t)__popc(peers));
             }
         }
+        unit = next_unit;
     }
     __syncthreads();
     for (int b = tid; b < tile_passes * RADIX; b += EMIT_THREADS) {
@@ -696,9 +798,9 @@ __device__ __forceinline__ uint32_t warp_lower_bound_tile(const uint64_t* __rest
 }
 
 __global__ void __launch_bounds__(256)
-ranges_kernel(const unsigned long long* __restrict__ pairs_eff, uint32_t T, const uint64_t* __restrict__ keys,
+ranges_kernel(const unsigned long long* __restrict__ pairs_out, uint32_t T, const uint64_t* __restrict__ keys,
               uint32_t* __restrict__ ranges) {
-    const uint32_t I = (uint32_t)*pairs_eff;
+    const uint32_t I = (uint32_t)*pairs_out;
     const uint32_t t = blockIdx.x * 8u + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (t >= T) return;
@@ -735,10 +837,12 @@ static cudaError_t launch_pass(unsigned tiles, cudaStream_t st, const uint32_t* 
     return cudaGetLastError();
 }
 
-extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
-                                const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
-                                uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
-                                int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream) {
+// Common body of xpr_bin_sort (cull == false; the cull-data pointers are unused) and xpr_bin_sort_cull.
+static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int32_t* tile_rect,
+                             const uint32_t* tile_count, const float* mean2d, const float* conic_opac, const float* lnv,
+                             const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
+                             uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
+                             int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0 || N > 0x7fffffffLL || pair_capacity < 0 || pair_capacity >= (1LL << 30))
         return XPR_ERR_INVALID_ARG;
@@ -748,6 +852,8 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     const int32_t T = (int32_t)T64;
     if (!aligned(tile_ranges, 8) || !aligned(workspace, 256)) return XPR_ERR_INVALID_ARG;
     if (N > 0 && (!aligned(depth, 4) || !aligned(tile_rect, 16) || !aligned(tile_count, 4))) return XPR_ERR_INVALID_ARG;
+    if (cull && N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(lnv, 4))) return XPR_ERR_INVALID_ARG;
+    if (TW > 0xffff || TH > 0xffff) return XPR_ERR_UNSUPPORTED;     // emit packs a tile coordinate in 16 bits
     if (pair_capacity > 0 && (!aligned(keys_sorted, 8) || !aligned(vals_sorted, 4))) return XPR_ERR_INVALID_ARG;
     const Layout L = make_layout(N, pair_capacity, T);
     if (workspace_bytes < L.total) return XPR_ERR_INVALID_ARG;
@@ -789,6 +895,7 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     //    it there (grids are persistent and sized for pair_capacity), so nothing waits for the host.
     uint32_t* voff = vkey[1];                          // free after the depth passes
     uint32_t* unit_first = reinterpret_cast<uint32_t*>(ws + L.unit_first);
+    unsigned long long* unit_status = reinterpret_cast<unsigned long long*>(ws + L.unit_status);
     offsets_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], tile_count, hdr, offsets_status, voff, unit_first,
                                                                    (uint32_t)(pair_capacity / EMIT_PAIRS + 1),
                                                                    (unsigned long long)pair_capacity);
@@ -802,8 +909,17 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
     if (pair_capacity > 0) {
         const unsigned egrid = units_cap < (unsigned)PERSIST_CTAS ? units_cap : (unsigned)PERSIST_CTAS;
 #define XPR_EMIT(TP)                                                                                             \
-    emit_kernel<TP><<<egrid, EMIT_THREADS, 0, st>>>(TW, vidx[0], voff, unit_first,                                \
-                                                    reinterpret_cast<const int4*>(tile_rect), hdr, w0)
+    do {                                                                                                         \
+        if (cull)                                                                                                \
+            emit_kernel<TP, true><<<egrid, EMIT_THREADS, 0, st>>>(                                                \
+                TW, vidx[0], voff, unit_first, reinterpret_cast<const int4*>(tile_rect),                          \
+                reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), lnv, hdr,   \
+                unit_status, w0);                                                                                \
+        else                                                                                                     \
+            emit_kernel<TP, false><<<egrid, EMIT_THREADS, 0, st>>>(                                               \
+                TW, vidx[0], voff, unit_first, reinterpret_cast<const int4*>(tile_rect), nullptr, nullptr,        \
+                nullptr, hdr, unit_status, w0);                                                                  \
+    } while (0)
         switch (tpasses) {
             case 1: XPR_EMIT(1); break;
             case 2: XPR_EMIT(2); break;
@@ -820,21 +936,42 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
             cudaError_t e;
             // bitmap ranking: consecutive pairs of a Gaussian are consecutive tiles (digit 0); after pass 1 a
             // warp holds many distinct high digits
-            if (!last)       e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
-                                          : launch_pass<uint64_t, IPT64, false, 1>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr);
-            else             e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
-                                          : launch_pass<uint64_t, IPT64, false, 2>(tiles64, st, nullptr, &hdr->pairs_eff, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0]);
+            if (!last)       e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
+                                          : launch_pass<uint64_t, IPT64, false, 1>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr);
+            else             e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
+                                          : launch_pass<uint64_t, IPT64, false, 2>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0]);
             XPR_CUDA(e);
             uint64_t* t = w0; w0 = w1; w1 = t;
         }
     }
     // 6. per-tile ranges ((0, 0) for every tile when there are no pairs or they exceed the capacity)
-    ranges_kernel<<<((unsigned)T + 7) / 8, 256, 0, st>>>(&hdr->pairs_eff, (uint32_t)T, keys_sorted, tile_ranges);
+    ranges_kernel<<<((unsigned)T + 7) / 8, 256, 0, st>>>(&hdr->pairs_out, (uint32_t)T, keys_sorted, tile_ranges);
     XPR_LAUNCH_CHECK();
     if (!num_pairs_host) return XPR_OK;                // asynchronous mode: the caller reads the count later
-    unsigned long long total = 0;
-    XPR_CUDA(cudaMemcpyAsync(&total, &hdr->total_pairs, sizeof(total), cudaMemcpyDeviceToHost, st));
+    unsigned long long counts[2] = {0, 0};             // candidates I (must fit the capacity), pairs in the output
+    XPR_CUDA(cudaMemcpyAsync(counts, &hdr->total_pairs, sizeof(counts), cudaMemcpyDeviceToHost, st));
     XPR_CUDA(cudaStreamSynchronize(st));
-    *num_pairs_host = (int64_t)total;
+    const unsigned long long total = counts[0];
+    *num_pairs_host = ((int64_t)total > pair_capacity) ? (int64_t)total : (int64_t)counts[1];
     return ((int64_t)total > pair_capacity) ? XPR_ERR_CAPACITY : XPR_OK;
+}
+
+extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
+                                const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
+                                uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
+                                int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream) {
+    if (cfg && cfg->tile_cull != 0) return XPR_ERR_INVALID_ARG;     // tile_cull needs the cull data: xpr_bin_sort_cull
+    return bin_sort_impl(false, N, depth, tile_rect, tile_count, nullptr, nullptr, nullptr, cam, cfg, pair_capacity,
+                         keys_sorted, vals_sorted, tile_ranges, num_pairs_host, workspace, workspace_bytes, stream);
+}
+
+extern "C" int32_t xpr_bin_sort_cull(int64_t N, const float* depth, const int32_t* tile_rect,
+                                     const uint32_t* tile_count, const float* mean2d, const float* conic_opac,
+                                     const float* lnv, const xpr_camera* cam, const xpr_config* cfg,
+                                     int64_t pair_capacity, uint64_t* keys_sorted, uint32_t* vals_sorted,
+                                     uint32_t* tile_ranges, int64_t* num_pairs_host, void* workspace,
+                                     size_t workspace_bytes, void* stream) {
+    const bool cull = cfg && cfg->tile_cull != 0;
+    return bin_sort_impl(cull, N, depth, tile_rect, tile_count, mean2d, conic_opac, lnv, cam, cfg, pair_capacity,
+                         keys_sorted, vals_sorted, tile_ranges, num_pairs_host, workspace, workspace_bytes, stream);
 }

@@ -62,7 +62,7 @@ class SplatPipeline:
         while True:
             st, n = xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg,
                                     self.pair_capacity, self.keys_sorted, self.vals_sorted, self.tile_ranges,
-                                    self.workspace, raise_on_capacity=False)
+                                    self.workspace, raise_on_capacity=False, cull_data=self._cull_data())
             if st == xb.XPR_OK:
                 self.num_pairs = n
                 return n
@@ -75,16 +75,23 @@ class SplatPipeline:
         the host, so the whole step can be enqueued ahead or captured in a CUDA graph.  The buffers must have
         been sized by an earlier bin_sort(); pairs_on_device() / check_capacity() read the count afterwards."""
         xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg, self.pair_capacity,
-                        self.keys_sorted, self.vals_sorted, self.tile_ranges, self.workspace, sync=False)
+                        self.keys_sorted, self.vals_sorted, self.tile_ranges, self.workspace, sync=False,
+                        cull_data=self._cull_data())
 
-    def pairs_on_device(self) -> int:
-        """I of the last bin_sort call, from the first 8 bytes of the workspace (synchronises)."""
-        return int(self.workspace[:8].view(torch.int64).item())
+    def _cull_data(self):
+        """tile-cull data p_tcd of the projection when cfg.tile_cull is set -> xpr_bin_sort_cull."""
+        return (self.mean2d, self.conic_opac, self.lnv) if int(self.cfg.tile_cull) else None
+
+    def pairs_on_device(self):
+        """(candidate pairs, pairs in the sorted output) of the last bin_sort call, from the first 16 bytes of
+        the workspace (synchronises).  They differ only with tile_cull."""
+        c = self.workspace[:16].view(torch.int64).tolist()
+        return int(c[0]), int(c[1])
 
     def check_capacity(self):
-        n = self.pairs_on_device()
-        if n > self.pair_capacity:
-            raise xb.XprError(xb.XPR_ERR_CAPACITY, f"xpr_bin_sort (asynchronous): {n} pairs > capacity {self.pair_capacity}")
+        cand, n = self.pairs_on_device()
+        if cand > self.pair_capacity:
+            raise xb.XprError(xb.XPR_ERR_CAPACITY, f"xpr_bin_sort (asynchronous): {cand} pairs > capacity {self.pair_capacity}")
         self.num_pairs = n
         return n
 

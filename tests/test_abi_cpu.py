@@ -28,14 +28,14 @@ def test_header_symbols_all_exported(lib):
     assert set(names) == set(binding.SYMBOLS), (names, binding.SYMBOLS)
     for n in names:
         assert hasattr(lib, n), n
-    for n in ("xpr_project", "xpr_bin_sort", "xpr_rasterize_fwd", "xpr_rasterize_bwd", "xpr_project_bwd"):
+    for n in ("xpr_project", "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_bwd", "xpr_project_bwd"):
         assert n in names   # BASELINE.json:north_star's five calls
 
 
 def test_struct_layout_matches_header():
     from paper_2606_11529_b200 import binding
     assert C.sizeof(binding.XprCamera) == 3 * 4 + 4 * 4 + 4 * 4 + 12 * 4
-    assert C.sizeof(binding.XprConfig) == 4 * 4 + 8 * 4 + 3 * 4
+    assert C.sizeof(binding.XprConfig) == 4 * 4 + 8 * 4 + 3 * 4 + 4
 
 
 def test_status_strings_and_version(lib):

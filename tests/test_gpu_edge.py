@@ -126,7 +126,7 @@ def test_async_bin_sort_matches_sync_and_overflow_renders_background():
     xb.xpr_bin_sort(small.depth, small.tile_rect, small.tile_count, small.cam, small.cfg, 4096, guard,
                     small.vals_sorted, small.tile_ranges, small.workspace, sync=False)
     torch.cuda.synchronize()
-    assert small.pairs_on_device() == I
+    assert small.pairs_on_device() == (I, 0)      # candidates, nothing in the output
     assert (guard[4096:] == -7).all()
     assert not small.tile_ranges.any()
     with pytest.raises(xb.XprError):

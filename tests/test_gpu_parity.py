@@ -143,3 +143,46 @@ def test_config4_full_size_ut_fisheye(view):
 
 def test_config3_full_size_second_pose():
     full_parity(scenes.make_scene(3), view=1)
+
+
+# ---- f1: tile_cull ("Cull", L268-281, L435; C8) -------------------------------------
+CULL = dict(tile_cull=1)
+
+
+@pytest.mark.parametrize("config,kw,view", [(1, {}, 0), (2, dict(n_override=20000, image_override=(200, 200)), 0),
+                                            (3, dict(n_override=50000, image_override=(480, 270)), 1),
+                                            (4, dict(n_override=50000, image_override=(480, 270)), 0),
+                                            (5, dict(n_override=30000, image_override=(320, 180)), 3)])
+def test_tile_cull_reduced(config, kw, view):
+    g, o = full_parity(scenes.make_scene(config, **kw), view, CULL)
+    assert g["binned"]["num_pairs"] == o["binned"]["num_pairs"] < o["binned"]["num_candidates"]
+
+
+def test_tile_cull_image_equals_uncut_image_on_gpu():
+    """PAPER L683 on the GPU path itself: same image, final_T and gradients with and without culling."""
+    sc = scenes.make_scene(3, n_override=50000, image_override=(480, 270))
+    a = pu.run_gpu(sc, 0)
+    b = pu.run_gpu(sc, 0, CULL)
+    assert b["binned"]["num_pairs"] < a["binned"]["num_pairs"]
+    np.testing.assert_array_equal(a["fwd"]["image"], b["fwd"]["image"])
+    np.testing.assert_array_equal(a["fwd"]["final_T"], b["fwd"]["final_T"])
+    dL = np.sign(a["fwd"]["image"] - sc.target(0)).astype(np.float32)
+    ga, gb = pu.run_gpu_backward(a, dL), pu.run_gpu_backward(b, dL)
+    for k in PARAMS:      # same terms, another order of the fp32 atomics: only cancelled elements may move
+        bad, _ = pu.grad_violations(gb[k], ga[k])
+        assert bad.mean() <= 1e-4, (k, int(bad.sum()))
+
+
+def test_tile_cull_ragged_and_edge():
+    full_parity(scenes.make_scene(1, n_override=600, image_override=(70, 50)), 0, CULL)
+    full_parity(scenes.make_scene(1, n_override=600, image_override=(33, 17)), 0, CULL)
+
+
+def test_tile_cull_config3_full_size_bench_configuration():
+    g, o = full_parity(scenes.make_scene(3), 0, CULL)
+    assert o["binned"]["num_pairs"] < 0.75 * o["binned"]["num_candidates"]
+
+
+def test_tile_cull_config5_full_size():
+    g, o = full_parity(scenes.make_scene(5), 0, CULL)
+    assert o["binned"]["num_pairs"] > 50_000_000
