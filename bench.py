@@ -40,6 +40,9 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--tile-cull", type=int, default=1, choices=(0, 1),
+                    help="1: binning with the paper's tile_cull (XPR-3DGS, PAPER L149/L268-281; same image); "
+                         "0: rectangle overlap only")
     ap.add_argument("--stages", action="store_true", help="also print per-stage times to stderr")
     return ap.parse_args()
 
@@ -107,10 +110,10 @@ def aggregate_value(world: int, megapixels: float, ms_per_step: float) -> float:
     return world * megapixels / (ms_per_step / 1e3)
 
 
-def oracle_step(xo, scenes, sc, view, np):
+def oracle_step(xo, scenes, sc, view, np, tile_cull=0):
     """One fwd+bwd step of the CPU oracle, as it stands (never tuned)."""
     cam = xo.make_camera(sc.cameras[view])
-    cfg = xo.make_config(scenes.default_render_config(sc))
+    cfg = xo.make_config(dict(scenes.default_render_config(sc), tile_cull=tile_cull))
     arrays = dict(means=sc.means, scales=sc.scales, quats=sc.quats, opacities=sc.opacities, sh=sc.sh)
     t0 = time.perf_counter()
     r = xo.render(arrays, cam, cfg, np.float32)
@@ -145,10 +148,10 @@ def run_reference(args):
     from paper_2606_11529_b200 import scenes
     sc, w, h, desc = oracle_sample(args)
     for _ in range(args.warmup):
-        oracle_step(xo, scenes, sc, args.view, np)
+        oracle_step(xo, scenes, sc, args.view, np, args.tile_cull)
     t = 0.0
     for _ in range(args.steps):
-        dt, I = oracle_step(xo, scenes, sc, args.view, np)
+        dt, I = oracle_step(xo, scenes, sc, args.view, np, args.tile_cull)
         t += dt
     ms = 1e3 * t / max(args.steps, 1)
     val = (w * h / 1e6) / (ms / 1e3)
@@ -156,7 +159,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config], "view": args.view, "sample": desc, "pairs": int(I)},
+            "config": {"workload": WORKLOADS[args.config], "view": args.view, "tile_cull": args.tile_cull, "sample": desc,
+                       "pairs": int(I)},
             "gaussians_per_s": sc.N / (ms / 1e3),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -187,7 +191,7 @@ def run_ours(args):
 
     sc = scenes.make_scene(args.config)
     cam = sc.cameras[args.view]
-    cfg = scenes.default_render_config(sc)
+    cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull)
     params = pipeline.scene_to_device(sc, dev)
     target = torch.from_numpy(sc.target(args.view)).to(dev)
     pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
@@ -227,6 +231,7 @@ def run_ours(args):
         step(sync_count=True)
     barrier()
     n_pairs = pipe.num_pairs
+    n_cand = pipe.pairs_on_device()[0]
     # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
     bits = max(1, (pipe.T - 1).bit_length()) if pipe.T > 1 else 0
     tile_passes = max(1, (bits + 7) // 8)
@@ -270,7 +275,7 @@ def run_ours(args):
     sec = lambda n: stage_ms[n] / 1e3
     # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + per pair: 8 B
     # emitted, 16 B per intermediate tile pass, 8 B read + 12 B written by the last one
-    sort_bytes = 8 * sc.N + 4 * 16 * n_vis + n_pairs * (8 + 16 * (tile_passes - 1) + 20)
+    sort_bytes = 8 * sc.N + 4 * 16 * n_vis + n_pairs * (8 + 16 * (tile_passes - 1) + 20)   # pairs that are sorted
     rooflines = {
         "rasterize_fwd": {"kernel": "rasterize_fwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
                           "achieved": (FWD_OPS_VISIT * visit + FWD_OPS_PASS * passed) / sec("rasterize_fwd") / 1e12},
@@ -356,7 +361,7 @@ def run_ours(args):
         sys.path.insert(0, os.path.join(ROOT, "oracle"))
         import xpr_oracle as xo
         osc, w, h, desc = oracle_sample(args)
-        dt, _ = oracle_step(xo, scenes, osc, args.view, np)
+        dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull)
         cpu = {"value": (w * h / 1e6) / dt, "unit": UNIT, "cores": xo.num_threads(), "kind": "oracle", "sample": desc,
                "seconds": dt}
 
@@ -365,7 +370,8 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "pairs": n_pairs, "visible_gaussians": n_vis,
+                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "pairs": n_pairs,
+                           "candidate_pairs": n_cand, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "tile_digits_on_pairs": tile_passes},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},

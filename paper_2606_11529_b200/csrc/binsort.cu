@@ -57,7 +57,7 @@ constexpr int PERSIST_CTAS = 148 * 4;       // upper bound of the persistent gri
 constexpr int EMIT_THREADS = 256, EMIT_PPT = 8, EMIT_PAIRS = EMIT_THREADS * EMIT_PPT;   // emit: 2048 pairs per unit
 constexpr int EMIT_WARPS = EMIT_THREADS / 32;
 constexpr int EMIT_SHIFT = 11;
-static_assert(EMIT_PPT * EMIT_WARPS == 64, "emit's survivor scan handles two counts per lane of one warp");
+static_assert(SCAN_ITEMS == EMIT_PAIRS, "unit_status is sized for one scan block per emit unit");
 static_assert(EMIT_PAIRS == 1 << EMIT_SHIFT, "unit_first is indexed by pair offset >> EMIT_SHIFT");
 
 constexpr uint32_t FLAG_PARTIAL = 1u << 30, FLAG_INCLUSIVE = 2u << 30, FLAG_MASK = 3u << 30, VALUE_MASK = ~FLAG_MASK;
@@ -66,12 +66,15 @@ constexpr unsigned long long SFLAG_PARTIAL = 1ull << 62, SFLAG_INCLUSIVE = 2ull 
 // Header at the start of the workspace (zeroed every call).
 struct Header {
     unsigned long long total_pairs;          // I (first 8 bytes of the workspace: readable by the caller)
-    unsigned long long pairs_out;            // pairs in the sorted output: I, or the survivors of tile_cull (second 8 bytes)
-    unsigned long long pairs_eff;            // I if it fits pair_capacity, else 0: what emit expands
+    unsigned long long pairs_out;            // pairs in the sorted output (second 8 bytes): total_pairs if it fits, else 0
+    unsigned long long pairs_eff;            // what emit expands: total_pairs if pairs and rows fit pair_capacity, else 0
+    unsigned long long rows_total;           // (Gaussian, tile row) segments of the visible Gaussians
+    unsigned long long rows_eff;             // rows_total if it fits pair_capacity, else 0
+    unsigned long long cand_total;           // candidate pairs: sum of tile_count (what pair_capacity must hold)
     uint32_t n_vis;                          // visible Gaussians
-    uint32_t compact_ticket, emit_ticket, unit_ticket;
+    uint32_t compact_ticket, rows_ticket, offsets_ticket, unit_ticket;
     uint32_t sort_ticket[DEPTH_PASSES + MAX_TILE_PASSES];
-    uint32_t pad[4];
+    uint32_t pad[5];
     uint32_t hist[(DEPTH_PASSES + MAX_TILE_PASSES) * RADIX];   // global digit histograms
 };
 
@@ -229,39 +232,60 @@ compact_kernel(int64_t N, const float* __restrict__ depth, const uint32_t* __res
 }
 
 // ---------------------------------------------------------------------------------------------
-// offsets: chained scan of the tile counts in depth order ("prefix-sum of tile counts")
+// Chained scans in depth order ("prefix-sum of tile counts").  The unit of replication is
+// a ROW: the run of consecutive tiles that one Gaussian covers in one tile row (all of its rectangle's
+// row, or with tile_cull the surviving interval), because pair r of a row is simply tile_start + r.
+//   MODE 0: values = tile rows h of the Gaussians in depth order -> row_base[rank], rows_total
+//   MODE 1: values = pairs of the rows                          -> row_off[row] (+ one past the end),
+//           unit_first[u] = the row that owns pair u * EMIT_PAIRS, total_pairs / pairs_out / pairs_eff
 // ---------------------------------------------------------------------------------------------
+template <int MODE>
 __global__ void __launch_bounds__(SCAN_THREADS)
-offsets_kernel(const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ tcount, Header* __restrict__ hdr,
-               unsigned long long* __restrict__ status, uint32_t* __restrict__ voff, uint32_t* __restrict__ unit_first,
-               uint32_t units_cap, unsigned long long pair_capacity) {
+scan_kernel(const uint32_t* __restrict__ vidx, const int4* __restrict__ rect, const uint32_t* __restrict__ tcount,
+            Header* __restrict__ hdr, unsigned long long* __restrict__ status, uint32_t* out,
+            uint32_t* __restrict__ unit_first, uint32_t units_cap, unsigned long long pair_capacity) {
     __shared__ uint32_t s_warp[SCAN_WARPS];
     __shared__ uint32_t s_block;
     __shared__ unsigned long long s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t n_vis = hdr->n_vis;
-    if (tid == 0) s_block = atomicAdd(&hdr->emit_ticket, 1u);   // ticket order = look-back order
+    const uint32_t n = (MODE == 0) ? hdr->n_vis : (uint32_t)hdr->rows_eff;
+    if (tid == 0) s_block = atomicAdd(MODE == 0 ? &hdr->rows_ticket : &hdr->offsets_ticket, 1u);   // ticket order = look-back order
     __syncthreads();
     const uint32_t block = s_block;
-    if ((uint64_t)block * SCAN_ITEMS >= n_vis && block != 0) return;   // beyond the visible list: nobody waits on us
+    if ((uint64_t)block * SCAN_ITEMS >= n && block != 0) return;   // beyond the list: nobody waits on us
     const uint32_t s0 = block * (uint32_t)SCAN_ITEMS + (uint32_t)warp * (32 * SCAN_ROUNDS) + (uint32_t)lane;
-    uint32_t tc[SCAN_ROUNDS];
+    uint32_t val[SCAN_ROUNDS];
+    unsigned long long cand = 0;                       // MODE 0: candidate pairs of this thread's Gaussians
 #pragma unroll
     for (int r = 0; r < SCAN_ROUNDS; ++r) {
         const uint32_t s = s0 + r * 32;
-        tc[r] = (s < n_vis) ? __ldg(tcount + __ldg(vidx + s)) : 0u;
+        val[r] = 0u;
+        if (s < n) {
+            if (MODE == 0) {
+                const uint32_t g = __ldg(vidx + s);
+                const int4 q = __ldg(rect + g);
+                val[r] = (uint32_t)(q.w - q.y);
+                cand += __ldg(tcount + g);
+            }
+            else val[r] = out[s];                       // MODE 1 scans in place: counts in, offsets out
+        }
     }
     uint32_t excl[SCAN_ROUNDS], wtotal = 0;
 #pragma unroll
     for (int r = 0; r < SCAN_ROUNDS; ++r) {
-        uint32_t incl = tc[r];
+        uint32_t incl = val[r];
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
             if (lane >= o) incl += v;
         }
-        excl[r] = wtotal + incl - tc[r];
+        excl[r] = wtotal + incl - val[r];
         wtotal += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (MODE == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cand += __shfl_xor_sync(0xffffffffu, cand, o);
+        if (lane == 0 && cand) atomicAdd(&hdr->cand_total, cand);
     }
     if (lane == 0) s_warp[warp] = wtotal;
     __syncthreads();
@@ -278,39 +302,128 @@ offsets_kernel(const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ t
     }
     __syncthreads();
     const unsigned long long base = s_base;
+    const bool last_block = (uint64_t)(block + 1) * SCAN_ITEMS >= n;
+    const unsigned long long total = base + btotal;
 #pragma unroll
     for (int r = 0; r < SCAN_ROUNDS; ++r) {
         const uint32_t s = s0 + r * 32;
-        if (s < n_vis) {
-            const unsigned long long off = base + wbase + excl[r], end = off + tc[r];
-            voff[s] = (uint32_t)off;                   // only used when I <= pair_capacity < 2^30
-            // emit works in units of EMIT_PAIRS consecutive pairs: unit u starts inside this Gaussian's pairs
-            // iff off <= EMIT_PAIRS u < end; then this Gaussian is the first one the unit needs
-            for (unsigned long long u = (off + (EMIT_PAIRS - 1)) >> EMIT_SHIFT; (u << EMIT_SHIFT) < end && u < units_cap; ++u)
-                unit_first[u] = s;
+        if (s < n) {
+            const unsigned long long off = base + wbase + excl[r], end = off + val[r];
+            out[s] = (uint32_t)off;
+            if (MODE == 1) {
+                // emit works in units of EMIT_PAIRS consecutive pairs: unit u starts inside this row's pairs
+                // iff off <= EMIT_PAIRS u < end; then this row is the first one the unit needs
+                for (unsigned long long u = (off + (EMIT_PAIRS - 1)) >> EMIT_SHIFT; (u << EMIT_SHIFT) < end && u < units_cap; ++u)
+                    unit_first[u] = s;
+            }
         }
     }
-    if (tid == 0 && (uint64_t)(block + 1) * SCAN_ITEMS >= n_vis) {
-        const unsigned long long I = base + btotal;
-        hdr->total_pairs = I;
-        hdr->pairs_eff = (I <= pair_capacity) ? I : 0ull;     // over capacity: the pair kernels do nothing
+    if (tid == 0 && last_block) {
+        if (MODE == 0) {
+            hdr->rows_total = total;
+            hdr->rows_eff = (total < pair_capacity) ? total : 0ull;    // over capacity: the row kernels do nothing
+                                                                        // (strict: row_off has one entry past the rows)
+        } else {
+            out[n] = (uint32_t)total;                    // one past the end: a row's pairs are [row_off[s], row_off[s+1])
+            // the capacity must hold the candidate pairs (sum of tile_count >= pairs, >= rows), as in xpr.h
+            const unsigned long long rows = hdr->rows_total, cand = hdr->cand_total;
+            const bool ok = cand <= pair_capacity && rows < pair_capacity;
+            hdr->total_pairs = ok ? total : (cand > rows + 1 ? cand : rows + 1);
+            hdr->pairs_out = ok ? total : 0ull;
+            hdr->pairs_eff = ok ? total : 0ull;           // over capacity: the pair kernels do nothing
+        }
     }
 }
 
-// 32-ary search by one warp in a sorted u32 array: first index in [0, n) whose element is > x
-// (n if none).  ~log32(n) dependent loads instead of log2(n).
-__device__ __forceinline__ uint32_t warp_upper_bound(const uint32_t* __restrict__ a, uint32_t n, uint32_t x, int lane) {
-    uint32_t lo = 0, hi = n;                   // answer in [lo, hi]; hi == n or a[hi] > x
-    while (hi > lo) {
-        const uint32_t len = hi - lo, stride = (len + 31u) / 32u;
-        const uint32_t probe = min(lo + ((uint32_t)lane + 1u) * stride - 1u, hi - 1u);
-        const uint32_t b = __ballot_sync(0xffffffffu, a[probe] > x);
-        if (b == 0u) { lo = hi; break; }
-        const uint32_t f = (uint32_t)__ffs(b) - 1u;
-        hi = min(lo + (f + 1u) * stride - 1u, hi - 1u);
-        lo = lo + f * stride;
+__device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, float C, float lnv, uint32_t tx, uint32_t ty);
+
+// ---------------------------------------------------------------------------------------------
+// rows: one thread per visible Gaussian (in depth order) writes its h rows: first tile id, number of
+// tiles, rank.  Without tile_cull a row is the whole width of the rectangle.  With tile_cull (PAPER
+// L149 "Cull") it is the interval of tiles that pass tile_keep: the set {x : min_{y in row} q <= lnv}
+// is an interval (q is convex), so the kernel estimates its two ends analytically (the ellipse
+// {q = lnv} cut by the strip of the row: its extreme x, or its intersection with the strip's edges) and
+// then settles each end with the exact per-tile predicate tile_keep -- the decision that defines the
+// result (bit-identical to the oracle's) -- stepping while the predicate disagrees.
+// ---------------------------------------------------------------------------------------------
+constexpr int ROWS_LANES = 8;
+template <bool CULL>
+__global__ void __launch_bounds__(128)
+rows_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ row_base,
+            const int4* __restrict__ rect, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
+            const float* __restrict__ lnv, const Header* __restrict__ hdr, uint32_t* __restrict__ row_start,
+            uint32_t* __restrict__ row_rank, uint32_t* __restrict__ row_cnt) {
+    // ROWS_LANES consecutive lanes share a Gaussian and take its rows in turn (a full-screen Gaussian has 68)
+    const uint32_t s = (blockIdx.x * 128u + threadIdx.x) / ROWS_LANES, sub = threadIdx.x % ROWS_LANES;
+    if (s >= hdr->n_vis || hdr->rows_eff == 0ull) return;
+    const uint32_t g = vidx[s];
+    const int4 r = rect[g];
+    uint32_t row = row_base[s] + sub;
+    float mx = 0.f, my = 0.f, A = 0.f, B = 0.f, C = 0.f, L = 0.f, ext = 0.f, det = 0.f;
+    if (CULL) {
+        const float2 m = mean2d[g]; const float4 co = conic_opac[g];
+        mx = m.x; my = m.y; A = co.x; B = co.y; C = co.z; L = lnv[g];
+        det = A * C - B * B;
+        ext = sqrtf(fmaxf(2.0f * L * C / det, 0.0f));          // half-width of the ellipse {q = L} in x
     }
-    return lo;
+    for (int ty = r.y + (int)sub; ty < r.w; ty += ROWS_LANES, row += ROWS_LANES) {
+        int xa = r.x, xb = r.z;                                 // kept tiles of this row: [xa, xb)
+        if (CULL) {
+            const auto keep = [&](int tx) { return tile_keep(mx, my, A, B, C, L, (uint32_t)tx, (uint32_t)ty); };
+            // estimate: x extent of {q <= L} over dy in [lo, hi] (pixel-centre hull of the row)
+            const float lo = (float)(TILE * ty) + 0.5f - my, hi = (float)(TILE * ty + TILE) - 0.5f - my;
+            float left = 1e30f, right = -1e30f;
+            const float dy_ext = B * ext / C;                   // dy at the ellipse's extreme x: -B dx / C, dx = -+ext
+            if (dy_ext >= lo && dy_ext <= hi) left = -ext;
+            if (-dy_ext >= lo && -dy_ext <= hi) right = ext;
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const float c = e ? hi : lo;
+                const float disc = 2.0f * A * L - det * c * c;  // roots of q(dx, c) = L
+                if (disc >= 0.0f) {
+                    const float sq = sqrtf(disc), mid = -B * c;
+                    left = fminf(left, (mid - sq) / A); right = fmaxf(right, (mid + sq) / A);
+                }
+            }
+            if (lo <= 0.0f && hi >= 0.0f) { left = fminf(left, 0.0f); right = fmaxf(right, 0.0f); }   // the mean's row
+            bool found = false;
+            if (left <= right) {
+                xa = max(r.x, min(r.z - 1, (int)floorf((mx + left - ((float)TILE - 0.5f)) / (float)TILE) + 1));
+                xb = max(xa, min(r.z - 1, (int)floorf((mx + right - 0.5f) / (float)TILE))) + 1;   // exclusive
+                // settle the left end with the exact predicate
+                int t = xa;
+                if (keep(t)) { while (t > r.x && keep(t - 1)) --t; found = true; }
+                else { while (t < xb && !keep(t)) ++t; found = t < xb; }
+                xa = t;
+                if (found) {
+                    t = max(xb - 1, xa);
+                    if (keep(t)) { while (t + 1 < r.z && keep(t + 1)) ++t; }
+                    else { while (t > xa && !keep(t)) --t; }
+                    xb = t + 1;
+                }
+            }
+            if (!found) {
+                // the estimate saw nothing.  q_min over the row's tiles is convex in x, so if any tile is kept the
+                // one nearest the row's minimiser x* is: x* = mx when the mean lies in the row's strip, else
+                // mx - B c / A with c the strip edge nearest the mean.  Test it and its neighbours (rounding of
+                // x*), then grow the interval with the predicate.
+                const float c = (lo <= 0.0f && hi >= 0.0f) ? 0.0f : ((lo > 0.0f) ? lo : hi);
+                const int tc = max(r.x, min(r.z - 1, (int)floorf((mx - B * c / A) / (float)TILE)));
+                int t = -1;
+                if (keep(tc)) t = tc;
+                else if (tc > r.x && keep(tc - 1)) t = tc - 1;
+                else if (tc + 1 < r.z && keep(tc + 1)) t = tc + 1;
+                if (t < 0) { xa = xb = r.x; }
+                else {
+                    xa = t; while (xa > r.x && keep(xa - 1)) --xa;
+                    xb = t + 1; while (xb < r.z && keep(xb)) ++xb;
+                }
+            }
+        }
+        row_start[row] = (uint32_t)ty * (uint32_t)TW + (uint32_t)xa;
+        row_rank[row] = s;
+        row_cnt[row] = (uint32_t)(xb - xa);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -328,12 +441,6 @@ __device__ __forceinline__ uint32_t warp_upper_bound(const uint32_t* __restrict_
 // memory once per CTA, not once per 2048 pairs.
 // ---------------------------------------------------------------------------------------------
 constexpr int EMIT_CAND = 2;                 // prefetched candidate Gaussians per thread and unit
-
-__device__ __forceinline__ uint32_t slot_rcp(uint32_t w) {   // bits of ~1/w (rcp.approx, 1 ulp)
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(__uint2float_rn(w)));
-    return __float_as_uint(y);
-}
 
 // tile_cull of XPR-3DGS ("Cull", Listing 1, A.1.1 L435): true when the pair survives,
 // i.e. unless min over the hull of the tile's pixel centres of 1/2 d^T K d exceeds lnv = ln(o / alpha_thresh)
@@ -371,44 +478,33 @@ __device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, 
     return !dropped;
 }
 
-// CULL = true (xpr_bin_sort_cull): every pair is tested with tile_keep and only the survivors are written,
-// compacted in order: the survivors of a unit are counted, a chained scan over the units (decoupled look-back)
-// gives the unit its base, and hdr->pairs_out ends up holding the number of surviving pairs.
-template <int TILE_PASSES, bool CULL>
+template <int TILE_PASSES>
 __global__ void __launch_bounds__(EMIT_THREADS)
-emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ voff,
-            const uint32_t* __restrict__ unit_first, const int4* __restrict__ rect, const float2* __restrict__ mean2d,
-            const float4* __restrict__ conic_opac, const float* __restrict__ lnv, Header* __restrict__ hdr,
-            unsigned long long* __restrict__ unit_status, uint64_t* __restrict__ words) {
-    __shared__ uint4 s_slot[EMIT_PAIRS];             // offset, x_min | y_min << 16, rectangle width, Gaussian index
+emit_kernel(const uint32_t* __restrict__ row_off, const uint32_t* __restrict__ row_start,
+            const uint32_t* __restrict__ row_rank, const uint32_t* __restrict__ unit_first, Header* __restrict__ hdr,
+            uint64_t* __restrict__ words) {
+    __shared__ uint4 s_slot[EMIT_PAIRS];             // pair offset of the row, its first tile id, rank of its Gaussian, -
     __shared__ __align__(16) uint16_t s_mark[EMIT_PAIRS];
     __shared__ uint32_t s_hist[MAX_TILE_PASSES * RADIX];
     __shared__ uint32_t s_wmax[EMIT_WARPS];
-    __shared__ uint32_t s_cnt[EMIT_PPT * EMIT_WARPS];   // survivors per (item, warp), then their exclusive scan
     __shared__ uint32_t s_unit[2];                   // tickets: this unit's successor (double buffered)
-    __shared__ unsigned long long s_base;
     constexpr int tile_passes = TILE_PASSES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t n_vis = hdr->n_vis;
+    const uint32_t n_rows = (uint32_t)hdr->rows_eff;
     const uint32_t I = (uint32_t)hdr->pairs_eff;
     const uint32_t units = (I + EMIT_PAIRS - 1) / EMIT_PAIRS;
     for (int b = tid; b < tile_passes * RADIX; b += EMIT_THREADS) s_hist[b] = 0u;
-    // units are drawn from a ticket counter (forward progress of the chain over units); the first Gaussian of
-    // every unit was recorded by offsets_kernel (unit_first), so a unit needs no search; the candidates of the
-    // CTA's NEXT unit are prefetched into registers while the current one is expanded
-    uint32_t c_off[EMIT_CAND];
-    int4 c_rect[EMIT_CAND];
-    uint32_t c_gid[EMIT_CAND];
+    // units are drawn from a ticket counter; the first row of every unit was recorded by the offsets scan
+    // (unit_first), so a unit needs no search; the candidate rows of the CTA's NEXT unit are prefetched into
+    // registers while the current one is expanded (the dependent loads are off the critical path)
+    uint32_t c_off[EMIT_CAND], c_end[EMIT_CAND], c_start[EMIT_CAND], c_rank[EMIT_CAND];
     auto load_candidates = [&](uint32_t first) {
 #pragma unroll
         for (int c = 0; c < EMIT_CAND; ++c) {
             const uint32_t s = first + (uint32_t)c * EMIT_THREADS + (uint32_t)tid;
-            c_off[c] = 0xffffffffu;                   // beyond the list: never < a pair index
-            if (s < n_vis) { c_off[c] = voff[s]; c_gid[c] = vidx[s]; c_rect[c] = rect[c_gid[c]]; }
+            c_off[c] = 0xffffffffu; c_end[c] = 0xffffffffu;  // beyond the list: never < a pair index
+            if (s < n_rows) { c_off[c] = row_off[s]; c_end[c] = row_off[s + 1]; c_start[c] = row_start[s]; c_rank[c] = row_rank[s]; }
         }
-    };
-    auto make_slot = [&](uint32_t off, const int4& r, uint32_t g) {
-        return make_uint4(off, (uint32_t)r.x | ((uint32_t)r.y << 16), (uint32_t)(r.z - r.x), g);
     };
     if (tid == 0) s_unit[0] = atomicAdd(&hdr->unit_ticket, 1u);
     __syncthreads();
@@ -420,33 +516,33 @@ emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
         if (tid == 0) s_unit[phase ^ 1] = atomicAdd(&hdr->unit_ticket, 1u);      // the unit after this one
         __syncthreads();                              // previous unit done with the shared arrays
         reinterpret_cast<uint4*>(s_mark)[tid] = make_uint4(0u, 0u, 0u, 0u);      // 8 marks per thread
-        // Gaussians first .. first+cnt-1 cover [p0, p1); cnt <= EMIT_PAIRS because every listed Gaussian
-        // after the first starts inside the range (each owns at least one pair)
+        // rows first .. cover [p0, p1); at most EMIT_PAIRS of them are non-empty (each owns a pair of the
+        // unit), empty rows (tile_cull) own nothing and are skipped
         const int overflow = __syncthreads_or(c_off[EMIT_CAND - 1] < p1 && tid == EMIT_THREADS - 1);
         const uint32_t next_unit = s_unit[phase ^ 1];
         const bool has_next = next_unit < units;
         if (has_next) next_first = unit_first[next_unit];
 #pragma unroll
         for (int c = 0; c < EMIT_CAND; ++c) {
-            if (c_off[c] < p1) {
-                const uint32_t k = (uint32_t)c * EMIT_THREADS + (uint32_t)tid;
-                s_slot[k] = make_slot(c_off[c], c_rect[c], c_gid[c]);
-                s_mark[c_off[c] > p0 ? c_off[c] - p0 : 0u] = (uint16_t)k;
+            if (c_off[c] < p1 && c_end[c] > c_off[c]) {
+                const uint32_t pos = c_off[c] > p0 ? c_off[c] - p0 : 0u;    // distinct for distinct non-empty rows
+                s_slot[pos] = make_uint4(c_off[c], c_start[c], c_rank[c], 0u);
+                s_mark[pos] = (uint16_t)pos;
             }
         }
         if (overflow) {
-            // more Gaussians start in this unit than were prefetched (tiny Gaussians): load the rest now
-            for (uint32_t k = (uint32_t)(EMIT_CAND * EMIT_THREADS) + tid; k < (uint32_t)EMIT_PAIRS; k += EMIT_THREADS) {
+            // more rows start in this unit than were prefetched (tiny Gaussians): load the rest now
+            for (uint32_t k = (uint32_t)(EMIT_CAND * EMIT_THREADS) + tid;; k += EMIT_THREADS) {
                 const uint32_t s = first + k;
-                if (s >= n_vis) break;
-                const uint32_t off = voff[s];
+                if (s >= n_rows) break;
+                const uint32_t off = row_off[s];
                 if (off >= p1) break;
-                const uint32_t g = vidx[s];
-                s_slot[k] = make_slot(off, rect[g], g);
-                s_mark[off - p0] = (uint16_t)k;
+                if (row_off[s + 1] > off) {
+                    s_slot[off - p0] = make_uint4(off, row_start[s], row_rank[s], 0u);
+                    s_mark[off - p0] = (uint16_t)(off - p0);
+                }
             }
         }
-        const uint32_t cur_first = first;             // rank of a pair = cur_first + slot
         if (has_next) { first = next_first; load_candidates(first); }   // consumed in the next iteration
         __syncthreads();
         {   // inclusive max-scan of the marks (thread t owns positions 8t .. 8t+7): slot of every pair
@@ -471,13 +567,10 @@ emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
                                                                m[4] | (m[5] << 16), m[6] | (m[7] << 16));
         }
         __syncthreads();
-        // pair j of slot k: r = j - offset, (ry, rx) = divmod(r, w), tile = (y_min + ry) TW + x_min + rx.  The loads
-        // of the 8 pairs of a thread are issued together and the arithmetic is branch-free (8 independent chains).
-        // r / w by an approximate reciprocal: the estimate is within 1 of the quotient while r < 2^22
-        // (relative error of the product < 2^-21) and is fixed up on both sides; beyond that, integer division.
-        uint32_t kk[EMIT_PPT], tile[EMIT_PPT];
+        // pair j belongs to the row whose first pair is the nearest mark at or before it: tile = first tile of
+        // the row + (j - offset of the row).  The loads of the 8 pairs of a thread are issued together.
+        uint32_t kk[EMIT_PPT];
         uint4 sl[EMIT_PPT];
-        bool keep[EMIT_PPT];
 #pragma unroll
         for (int it = 0; it < EMIT_PPT; ++it) kk[it] = s_mark[min((uint32_t)it * EMIT_THREADS + (uint32_t)tid, p1 - p0 - 1u)];
 #pragma unroll
@@ -485,70 +578,18 @@ emit_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
 #pragma unroll
         for (int it = 0; it < EMIT_PPT; ++it) {
             const uint32_t j = p0 + (uint32_t)it * EMIT_THREADS + (uint32_t)tid;
-            keep[it] = j < p1;                         // false only in the tail of the last unit
-            const uint32_t r = j - sl[it].x, w = sl[it].z;
-            uint32_t ry = (uint32_t)__float2uint_rz(__uint2float_rn(r) * __uint_as_float(slot_rcp(w)));
-            const int rem = (int)(r - ry * w);
-            ry += (rem >= (int)w ? 1u : 0u) - (rem < 0 ? 1u : 0u);
-            if (r >= (1u << 22)) ry = r / w;           // a Gaussian covering more than 4M tiles
-            const uint32_t tx = (sl[it].y & 0xffffu) + (r - ry * w), ty = (sl[it].y >> 16) + ry;
-            tile[it] = ty * (uint32_t)TW + tx;
-            if (CULL) {
-                const uint32_t g = sl[it].w;
-                const float2 m = __ldg(mean2d + g);
-                const float4 co = __ldg(conic_opac + g);
-                keep[it] = keep[it] && tile_keep(m.x, m.y, co.x, co.y, co.z, __ldg(lnv + g), tx, ty);
-            }
-        }
-        uint32_t dst[EMIT_PPT];                        // position of a kept pair in the output
-        if (CULL) {
-            // order of the pairs: j = it * 256 + warp * 32 + lane -> exclusive scan over (it, warp), then lanes
-            uint32_t lrank[EMIT_PPT];
-#pragma unroll
-            for (int it = 0; it < EMIT_PPT; ++it) {
-                const uint32_t m = __ballot_sync(0xffffffffu, keep[it]);
-                lrank[it] = (uint32_t)__popc(m & ((1u << lane) - 1u));
-                if (lane == 0) s_cnt[it * EMIT_WARPS + warp] = (uint32_t)__popc(m);
-            }
-            __syncthreads();
-            if (warp == 0) {                           // 64 counts: 2 per lane
-                const uint32_t c0 = s_cnt[2 * lane], c1 = s_cnt[2 * lane + 1];
-                uint32_t incl = c0 + c1;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o) incl += v;
-                }
-                const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
-                const uint32_t excl = incl - (c0 + c1);
-                s_cnt[2 * lane] = excl; s_cnt[2 * lane + 1] = excl + c0;
-                const unsigned long long base = chain_lookback(unit, total, unit_status, lane);
-                if (lane == 0) {
-                    s_base = base;
-                    if (unit == units - 1u) hdr->pairs_out = base + total;
-                }
-            }
-            __syncthreads();
-            const uint32_t base = (uint32_t)s_base;
-#pragma unroll
-            for (int it = 0; it < EMIT_PPT; ++it) dst[it] = base + s_cnt[it * EMIT_WARPS + warp] + lrank[it];
-        } else {
-#pragma unroll
-            for (int it = 0; it < EMIT_PPT; ++it) dst[it] = p0 + (uint32_t)it * EMIT_THREADS + (uint32_t)tid;
-            if (tid == 0 && unit == units - 1u) hdr->pairs_out = I;
-        }
-#pragma unroll
-        for (int it = 0; it < EMIT_PPT; ++it) {
-            if (keep[it]) {
-                words[dst[it]] = ((uint64_t)tile[it] << 32) | (uint64_t)(cur_first + kk[it]);
-                atomicAdd(&s_hist[tile[it] & 255u], 1u);   // consecutive tiles -> distinct banks
+            const bool valid = j < p1;                 // false only in the tail of the last unit
+            const uint32_t tile = sl[it].y + (j - sl[it].x);
+            if (valid) {
+                words[j] = ((uint64_t)tile << 32) | (uint64_t)sl[it].z;
+                atomicAdd(&s_hist[tile & 255u], 1u);   // consecutive tiles -> distinct banks
             }
             // higher tile digits are nearly warp-uniform: aggregate with match.any before the atomic
 #pragma unroll
             for (int d = 1; d < tile_passes; ++d) {
-                const uint32_t dig = keep[it] ? ((tile[it] >> (8 * d)) & 255u) : 0xffffffffu;
+                const uint32_t dig = valid ? ((tile >> (8 * d)) & 255u) : 0xffffffffu;
                 const uint32_t peers = __match_any_sync(0xffffffffu, dig);
-                if (keep[it] && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_hist[d * RADIX + dig], (uint32_t)__popc(peers));
+                if (valid && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_hist[d * RADIX + dig], (uint32_t)__popc(peers));
             }
         }
         unit = next_unit;
@@ -891,35 +932,45 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
             : launch_pass<uint32_t, IPT32, false, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr);
         XPR_CUDA(e);
     }   // DEPTH_PASSES is even: the sorted list is back in vkey[0] / vidx[0]
-    // 3. pair offsets in depth order and the pair count I.  I stays on the device: every later kernel reads
-    //    it there (grids are persistent and sized for pair_capacity), so nothing waits for the host.
-    uint32_t* voff = vkey[1];                          // free after the depth passes
-    uint32_t* unit_first = reinterpret_cast<uint32_t*>(ws + L.unit_first);
-    unsigned long long* unit_status = reinterpret_cast<unsigned long long*>(ws + L.unit_status);
-    offsets_kernel<<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], tile_count, hdr, offsets_status, voff, unit_first,
-                                                                   (uint32_t)(pair_capacity / EMIT_PAIRS + 1),
-                                                                   (unsigned long long)pair_capacity);
-    XPR_LAUNCH_CHECK();
-    // 4. replicate in depth order as packed words; pass p reads buffer p and writes buffer p+1, the last
-    //    one writes keys_sorted / vals_sorted, so emission starts in keys_sorted when tpasses is even
+    // 3. rows: a row is the run of consecutive tiles one Gaussian covers in one tile row;
+    //    scan of the row counts in depth order, the row table (with tile_cull: the surviving interval), scan
+    //    of the pairs per row.  Every count stays on the device: later kernels read it there (grids are sized
+    //    for pair_capacity), so nothing waits for the host.
+    //    Scratch: the word buffer emission does not write to (free until pass 1) holds first tile + rank of
+    //    the rows, vals_sorted (free until the last pass) their pair offsets, vkey[1]/vidx[1] (free after the
+    //    depth passes) row bases and counts... all bounded by rows <= candidate pairs <= pair_capacity.
     uint64_t* w0 = (tpasses % 2 == 0) ? keys_sorted : keys_tmp;
     uint64_t* w1 = (tpasses % 2 == 0) ? keys_tmp : keys_sorted;
+    uint32_t* row_base = vkey[1];
+    uint32_t* unit_first = reinterpret_cast<uint32_t*>(ws + L.unit_first);
+    unsigned long long* unit_status = reinterpret_cast<unsigned long long*>(ws + L.unit_status);
     const unsigned units_cap = (unsigned)((pair_capacity + EMIT_PAIRS - 1) / EMIT_PAIRS);
     const unsigned tiles64 = (unsigned)((pair_capacity + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64));
+    const int4* rect4 = reinterpret_cast<const int4*>(tile_rect);
+    scan_kernel<0><<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], rect4, tile_count, hdr, offsets_status, row_base,
+                                                                   nullptr, 0u, (unsigned long long)pair_capacity);
+    XPR_LAUNCH_CHECK();
     if (pair_capacity > 0) {
+        uint32_t* row_start = reinterpret_cast<uint32_t*>(w1);          // [pair_capacity]
+        uint32_t* row_rank = row_start + pair_capacity;                  // [pair_capacity]
+        uint32_t* row_off = vals_sorted;                                 // counts, scanned in place; [rows + 1], rows < pair_capacity
+        const unsigned rgrid = (unsigned)(((size_t)N * ROWS_LANES + 127) / 128);
+        if (cull)
+            rows_kernel<true><<<rgrid, 128, 0, st>>>(TW, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
+                                                     reinterpret_cast<const float4*>(conic_opac), lnv, hdr, row_start,
+                                                     row_rank, row_off);
+        else
+            rows_kernel<false><<<rgrid, 128, 0, st>>>(TW, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, hdr,
+                                                      row_start, row_rank, row_off);
+        XPR_LAUNCH_CHECK();
+        const unsigned oblocks = (unsigned)(((size_t)pair_capacity + SCAN_ITEMS - 1) / SCAN_ITEMS);
+        scan_kernel<1><<<oblocks, SCAN_THREADS, 0, st>>>(nullptr, nullptr, nullptr, hdr, unit_status, row_off, unit_first,
+                                                         units_cap + 1u, (unsigned long long)pair_capacity);
+        XPR_LAUNCH_CHECK();
+        // 4. replicate in depth order as packed words; pass p reads buffer p and writes buffer p+1, the last
+        //    one writes keys_sorted / vals_sorted, so emission starts in keys_sorted when tpasses is even
         const unsigned egrid = units_cap < (unsigned)PERSIST_CTAS ? units_cap : (unsigned)PERSIST_CTAS;
-#define XPR_EMIT(TP)                                                                                             \
-    do {                                                                                                         \
-        if (cull)                                                                                                \
-            emit_kernel<TP, true><<<egrid, EMIT_THREADS, 0, st>>>(                                                \
-                TW, vidx[0], voff, unit_first, reinterpret_cast<const int4*>(tile_rect),                          \
-                reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), lnv, hdr,   \
-                unit_status, w0);                                                                                \
-        else                                                                                                     \
-            emit_kernel<TP, false><<<egrid, EMIT_THREADS, 0, st>>>(                                               \
-                TW, vidx[0], voff, unit_first, reinterpret_cast<const int4*>(tile_rect), nullptr, nullptr,        \
-                nullptr, hdr, unit_status, w0);                                                                  \
-    } while (0)
+#define XPR_EMIT(TP) emit_kernel<TP><<<egrid, EMIT_THREADS, 0, st>>>(row_off, row_start, row_rank, unit_first, hdr, w0)
         switch (tpasses) {
             case 1: XPR_EMIT(1); break;
             case 2: XPR_EMIT(2); break;
