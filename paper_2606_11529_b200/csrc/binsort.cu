@@ -243,13 +243,17 @@ template <int MODE>
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_kernel(const uint32_t* __restrict__ vidx, const int4* __restrict__ rect, const uint32_t* __restrict__ tcount,
             Header* __restrict__ hdr, unsigned long long* __restrict__ status, uint32_t* out,
-            uint32_t* __restrict__ unit_first, uint32_t units_cap, unsigned long long pair_capacity) {
+            uint32_t* __restrict__ aux /* MODE 1: unit_first */, uint32_t units_cap,
+            unsigned long long pair_capacity) {
     __shared__ uint32_t s_warp[SCAN_WARPS];
     __shared__ uint32_t s_block;
     __shared__ unsigned long long s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n = (MODE == 0) ? hdr->n_vis : (uint32_t)hdr->rows_eff;
-    if (tid == 0) s_block = atomicAdd(MODE == 0 ? &hdr->rows_ticket : &hdr->offsets_ticket, 1u);   // ticket order = look-back order
+    uint32_t* const unit_first = aux;
+    for (;;) {       // persistent: blocks of SCAN_ITEMS items are drawn from a ticket counter (= look-back order)
+    __syncthreads();
+    if (tid == 0) s_block = atomicAdd(MODE == 0 ? &hdr->rows_ticket : &hdr->offsets_ticket, 1u);
     __syncthreads();
     const uint32_t block = s_block;
     if ((uint64_t)block * SCAN_ITEMS >= n && block != 0) return;   // beyond the list: nobody waits on us
@@ -333,6 +337,8 @@ scan_kernel(const uint32_t* __restrict__ vidx, const int4* __restrict__ rect, co
             hdr->pairs_eff = ok ? total : 0ull;           // over capacity: the pair kernels do nothing
         }
     }
+    if (last_block) return;
+    }
 }
 
 __device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, float C, float lnv, uint32_t tx, uint32_t ty);
@@ -346,27 +352,32 @@ __device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, 
 // then settles each end with the exact per-tile predicate tile_keep -- the decision that defines the
 // result (bit-identical to the oracle's) -- stepping while the predicate disagrees.
 // ---------------------------------------------------------------------------------------------
-constexpr int ROWS_LANES = 8;
 template <bool CULL>
 __global__ void __launch_bounds__(128)
 rows_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ row_base,
             const int4* __restrict__ rect, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
             const float* __restrict__ lnv, const Header* __restrict__ hdr, uint32_t* __restrict__ row_start,
             uint32_t* __restrict__ row_rank, uint32_t* __restrict__ row_cnt) {
-    // ROWS_LANES consecutive lanes share a Gaussian and take its rows in turn (a full-screen Gaussian has 68)
-    const uint32_t s = (blockIdx.x * 128u + threadIdx.x) / ROWS_LANES, sub = threadIdx.x % ROWS_LANES;
-    if (s >= hdr->n_vis || hdr->rows_eff == 0ull) return;
-    const uint32_t g = vidx[s];
-    const int4 r = rect[g];
-    uint32_t row = row_base[s] + sub;
-    float mx = 0.f, my = 0.f, A = 0.f, B = 0.f, C = 0.f, L = 0.f, ext = 0.f, det = 0.f;
-    if (CULL) {
-        const float2 m = mean2d[g]; const float4 co = conic_opac[g];
-        mx = m.x; my = m.y; A = co.x; B = co.y; C = co.z; L = lnv[g];
-        det = A * C - B * B;
-        ext = sqrtf(fmaxf(2.0f * L * C / det, 0.0f));          // half-width of the ellipse {q = L} in x
-    }
-    for (int ty = r.y + (int)sub; ty < r.w; ty += ROWS_LANES, row += ROWS_LANES) {
+    // one thread per row (grid-stride); its Gaussian is the last one whose first row is <= row (binary search in
+    // the strictly increasing row_base; neighbouring threads follow the same path, so the loads coalesce)
+    const uint32_t n_rows = (uint32_t)hdr->rows_eff, n_vis = hdr->n_vis;
+    for (uint32_t row = blockIdx.x * 128u + threadIdx.x; row < n_rows; row += gridDim.x * 128u) {
+        uint32_t s = 0, hi_s = n_vis;                // invariant: row_base[s] <= row, (hi_s == n_vis or row_base[hi_s] > row)
+        while (hi_s - s > 1u) {
+            const uint32_t mid = (s + hi_s) >> 1;
+            if (__ldg(row_base + mid) <= row) s = mid; else hi_s = mid;
+        }
+        row_rank[row] = s;
+        const uint32_t g = vidx[s];
+        const int4 r = rect[g];
+        const int ty = r.y + (int)(row - row_base[s]);
+        float mx = 0.f, my = 0.f, A = 0.f, B = 0.f, C = 0.f, L = 0.f, ext = 0.f, det = 0.f;
+        if (CULL) {
+            const float2 m = mean2d[g]; const float4 co = conic_opac[g];
+            mx = m.x; my = m.y; A = co.x; B = co.y; C = co.z; L = lnv[g];
+            det = A * C - B * B;
+            ext = sqrtf(fmaxf(2.0f * L * C / det, 0.0f));          // half-width of the ellipse {q = L} in x
+        }
         int xa = r.x, xb = r.z;                                 // kept tiles of this row: [xa, xb)
         if (CULL) {
             const auto keep = [&](int tx) { return tile_keep(mx, my, A, B, C, L, (uint32_t)tx, (uint32_t)ty); };
@@ -421,7 +432,6 @@ rows_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
             }
         }
         row_start[row] = (uint32_t)ty * (uint32_t)TW + (uint32_t)xa;
-        row_rank[row] = s;
         row_cnt[row] = (uint32_t)(xb - xa);
     }
 }
@@ -947,14 +957,15 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     const unsigned units_cap = (unsigned)((pair_capacity + EMIT_PAIRS - 1) / EMIT_PAIRS);
     const unsigned tiles64 = (unsigned)((pair_capacity + SORT_THREADS * IPT64 - 1) / (SORT_THREADS * IPT64));
     const int4* rect4 = reinterpret_cast<const int4*>(tile_rect);
-    scan_kernel<0><<<(unsigned)scan_blocks, SCAN_THREADS, 0, st>>>(vidx[0], rect4, tile_count, hdr, offsets_status, row_base,
-                                                                   nullptr, 0u, (unsigned long long)pair_capacity);
+    uint32_t* row_start = reinterpret_cast<uint32_t*>(w1);          // [pair_capacity]
+    uint32_t* row_rank = row_start + pair_capacity;                  // [pair_capacity]
+    const unsigned sgrid0 = (unsigned)scan_blocks < 2u * PERSIST_CTAS ? (unsigned)scan_blocks : 2u * PERSIST_CTAS;
+    scan_kernel<0><<<sgrid0, SCAN_THREADS, 0, st>>>(vidx[0], rect4, tile_count, hdr, offsets_status, row_base, nullptr, 0u,
+                                                    (unsigned long long)pair_capacity);
     XPR_LAUNCH_CHECK();
     if (pair_capacity > 0) {
-        uint32_t* row_start = reinterpret_cast<uint32_t*>(w1);          // [pair_capacity]
-        uint32_t* row_rank = row_start + pair_capacity;                  // [pair_capacity]
         uint32_t* row_off = vals_sorted;                                 // counts, scanned in place; [rows + 1], rows < pair_capacity
-        const unsigned rgrid = (unsigned)(((size_t)N * ROWS_LANES + 127) / 128);
+        const unsigned rgrid = 148u * 16u;                               // grid-stride over the rows (count on the device)
         if (cull)
             rows_kernel<true><<<rgrid, 128, 0, st>>>(TW, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
                                                      reinterpret_cast<const float4*>(conic_opac), lnv, hdr, row_start,
@@ -964,8 +975,9 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
                                                       row_start, row_rank, row_off);
         XPR_LAUNCH_CHECK();
         const unsigned oblocks = (unsigned)(((size_t)pair_capacity + SCAN_ITEMS - 1) / SCAN_ITEMS);
-        scan_kernel<1><<<oblocks, SCAN_THREADS, 0, st>>>(nullptr, nullptr, nullptr, hdr, unit_status, row_off, unit_first,
-                                                         units_cap + 1u, (unsigned long long)pair_capacity);
+        const unsigned sgrid1 = oblocks < 2u * PERSIST_CTAS ? oblocks : 2u * PERSIST_CTAS;
+        scan_kernel<1><<<sgrid1, SCAN_THREADS, 0, st>>>(nullptr, nullptr, nullptr, hdr, unit_status, row_off, unit_first,
+                                                        units_cap + 1u, (unsigned long long)pair_capacity);
         XPR_LAUNCH_CHECK();
         // 4. replicate in depth order as packed words; pass p reads buffer p and writes buffer p+1, the last
         //    one writes keys_sorted / vals_sorted, so emission starts in keys_sorted when tpasses is even
