@@ -231,13 +231,15 @@ def run_ours(args):
         step(sync_count=True)
     barrier()
     n_pairs = pipe.num_pairs
-    n_cand = pipe.pairs_on_device()[0]
+    n_cand = pipe.candidates_on_device()
     # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
     bits = max(1, (pipe.T - 1).bit_length()) if pipe.T > 1 else 0
     tile_passes = max(1, (bits + 7) // 8)
     passes = 4 + tile_passes              # 8-bit digits: 4 on the depth bits (run on Gaussians) + tile digits (on pairs)
-    # project, bin_sort (compact, 4 depth passes, offsets, emit, tile passes, ranges), fwd, bwd, project_bwd
-    launches_per_step = 1 + (1 + 4 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1
+    # project, bin_sort (compact, 4 depth passes, row scan, rows, pair scan, emit, tile passes, ranges), fwd, bwd,
+    # project_bwd
+    launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1
+    n_rows = pipe.rows_on_device()
     n_vis = int(torch.count_nonzero(pipe.tile_count).item())
 
     sampler = ClockSampler(local)
@@ -273,16 +275,18 @@ def run_ours(args):
     alu_peak = SMS * LANES_PER_SM * sm_max * 1e6 / 1e12          # T lane-ops/s (FMA = 1 lane-op)
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     sec = lambda n: stage_ms[n] / 1e3
-    # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + per pair: 8 B
-    # emitted, 16 B per intermediate tile pass, 8 B read + 12 B written by the last one
-    sort_bytes = 8 * sc.N + 4 * 16 * n_vis + n_pairs * (8 + 16 * (tile_passes - 1) + 20)   # pairs that are sorted
+    # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + 20 B per visible
+    # Gaussian (row scan) + 36 B per row (table written, counts scanned in place, read by emit) + per sorted pair:
+    # 8 B emitted, 16 B per intermediate tile pass, 8 B read + 12 B written by the last one
+    sort_bytes = (8 * sc.N + (4 * 16 + 20) * n_vis + 36 * n_rows
+                  + n_pairs * (8 + 16 * (tile_passes - 1) + 20))
     rooflines = {
         "rasterize_fwd": {"kernel": "rasterize_fwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
                           "achieved": (FWD_OPS_VISIT * visit + FWD_OPS_PASS * passed) / sec("rasterize_fwd") / 1e12},
         "rasterize_bwd": {"kernel": "rasterize_bwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
                           "achieved": (BWD_OPS_VISIT * sum_n + BWD_OPS_PASS * blended) / sec("rasterize_bwd") / 1e12},
-        "bin_sort": {"kernel": "xpr_bin_sort (compact, 4 depth passes on Gaussians, offsets, emit, %d tile passes "
-                               "on pairs, ranges)" % tile_passes, "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
+        "bin_sort": {"kernel": "xpr_bin_sort%s (compact, 4 depth passes on Gaussians, row scan, rows, pair scan, emit, "
+                               "%d tile passes on pairs, ranges)" % ("_cull" if args.tile_cull else "", tile_passes), "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
                      "achieved": sort_bytes / sec("bin_sort") / 1e9, "algorithmic_bytes": sort_bytes},
     }
     traffic = {}
@@ -371,7 +375,7 @@ def run_ours(args):
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
                            "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "pairs": n_pairs,
-                           "candidate_pairs": n_cand, "visible_gaussians": n_vis,
+                           "candidate_pairs": n_cand, "rows": n_rows, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "tile_digits_on_pairs": tile_passes},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},

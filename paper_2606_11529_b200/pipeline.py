@@ -88,6 +88,14 @@ class SplatPipeline:
         c = self.workspace[:16].view(torch.int64).tolist()
         return int(c[0]), int(c[1])
 
+    def rows_on_device(self) -> int:
+        """Number of (Gaussian, tile row) segments of the last bin_sort call (workspace bytes [24, 32))."""
+        return int(self.workspace[24:32].view(torch.int64).item())
+
+    def candidates_on_device(self) -> int:
+        """Candidate pairs (sum of tile_count over the visible Gaussians) of the last call (workspace bytes [40, 48))."""
+        return int(self.workspace[40:48].view(torch.int64).item())
+
     def check_capacity(self):
         cand, n = self.pairs_on_device()
         if cand > self.pair_capacity:
