@@ -205,18 +205,22 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
 // pixel-pairs and the per-Gaussian reduction runs once per 128 pixel-pairs: each lane first sums
 // its own pixels in registers, then one transposed butterfly (14 shuffles for the 9 gradients)
 // leaves the totals spread over lanes, which issue two RED instructions (8 lanes + 1 lane).
-constexpr int BWD_THREADS = 64, BWD_PPT = 4, BWD_BATCH = 64;
+#ifndef XPR_BWD_PPT_SMALL
+#define XPR_BWD_PPT_SMALL 2
+#endif
 
 #ifndef XPR_BWD_MINB
 #define XPR_BWD_MINB 1
 #endif
-__global__ void __launch_bounds__(BWD_THREADS, XPR_BWD_MINB)
+template <int BWD_PPT>
+__global__ void __launch_bounds__(BLOCK / BWD_PPT, XPR_BWD_MINB)
 rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                      const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                      const float* __restrict__ dL, float* __restrict__ g_mean2d, float* __restrict__ g_conic,
                      float* __restrict__ g_opac, float* __restrict__ g_rgb) {
+    constexpr int BWD_THREADS = BLOCK / BWD_PPT, BWD_BATCH = BWD_THREADS;
     __shared__ float4 s_geo[BWD_BATCH];   // mx, my, A, B
     __shared__ float4 s_gate[BWD_BATCH];  // C, thr, o, index (bits)
     __shared__ float4 s_col[BWD_BATCH];   // r, g, b, unused
@@ -410,10 +414,18 @@ extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cf
     RasterParams P;
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
-    rasterize_bwd_kernel<<<T, BWD_THREADS, 0, st>>>(
-        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_mean2d, g_conic,
-        g_opac, g_rgb);
+    // 4 pixels per thread (64 threads) is the throughput shape; images with few tiles are bounded by their
+    // heaviest tile, where more warps per tile (2 pixels per thread) shorten the critical path
+    if (T >= FWD_PPT2_MIN_TILES)
+        rasterize_bwd_kernel<4><<<T, BLOCK / 4, 0, st>>>(
+            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_mean2d, g_conic,
+            g_opac, g_rgb);
+    else
+        rasterize_bwd_kernel<XPR_BWD_PPT_SMALL><<<T, BLOCK / XPR_BWD_PPT_SMALL, 0, st>>>(
+            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_mean2d, g_conic,
+            g_opac, g_rgb);
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }
