@@ -91,14 +91,20 @@ int32_t xpr_project(int64_t N, const float* means, const float* scales, const fl
  *        output arrays (must be < 2^30).
  *   out: keys_sorted[I] u64, vals_sorted[I] u32, tile_ranges[T,2] = (start,end) per tile, (0,0)
  *        for an empty tile; *num_pairs_host (HOST int64) = I.
- *   Nothing inside the call waits for the host: I stays on the device and every kernel reads it
- *   there.  With num_pairs_host != NULL the call ends with an 8-byte read-back of I and a stream
- *   synchronisation; I > pair_capacity -> XPR_ERR_CAPACITY with *num_pairs_host = required I.
+ *   Capacity: pair_capacity must hold I = sum of tile_count (the candidate pairs) and must exceed
+ *   the number of (Gaussian, tile-row) rows, which is <= I; practically: pair_capacity > I.
+ *   Nothing inside the call waits for the host: every count stays on the device and every kernel
+ *   reads it there.  With num_pairs_host != NULL the call ends with a 16-byte read-back of the counts
+ *   and a stream synchronisation; if the capacity does not suffice -> XPR_ERR_CAPACITY with
+ *   *num_pairs_host = the capacity that suffices (max(I, rows + 1)).
  *   With num_pairs_host == NULL the call is fully asynchronous (capturable in a CUDA graph): it
- *   returns XPR_OK after enqueueing, and the first 16 bytes of `workspace` hold I twice (uint64:
- *   candidates, pairs in the output) once the stream has run; the caller must compare it with pair_capacity before trusting the outputs.
- *   In both modes, when I > pair_capacity nothing out of bounds is written, tile_ranges is (0,0) for
- *   every tile (a following xpr_rasterize_fwd renders the background) and keys/vals are unspecified.
+ *   returns XPR_OK after enqueueing; once the stream has run, workspace bytes [0,8) hold (uint64) the
+ *   number of sorted pairs, or the capacity that suffices when it exceeds pair_capacity -- the caller
+ *   must compare it with pair_capacity before trusting the outputs -- and bytes [8,16) the number of
+ *   sorted pairs (0 on overflow).
+ *   In both modes, when the capacity does not suffice nothing out of bounds is written, tile_ranges
+ *   is (0,0) for every tile (a following xpr_rasterize_fwd renders the background) and keys/vals are
+ *   unspecified.  keys_sorted and vals_sorted are also used as scratch during the call.
  *   workspace: DEVICE scratch of at least xpr_bin_sort_workspace() bytes, 256-byte aligned.
  *   Equal keys keep emission order = ascending Gaussian index.
  */
@@ -121,9 +127,8 @@ int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* tile_rect, co
  * survivors are compacted in emission order and only they are sorted.
  *   in : as xpr_bin_sort + the tile-cull data p_tcd of xpr_project: mean2d[N,2], conic_opac[N,4], lnv[N].
  *   out: as xpr_bin_sort; *num_pairs_host = number of SURVIVING pairs (= length of the sorted arrays).
- *   pair_capacity must hold the CANDIDATE count (sum of tile_count); otherwise XPR_ERR_CAPACITY with
- *   *num_pairs_host = that count.  Asynchronous mode: workspace bytes [0,8) = candidate count,
- *   bytes [8,16) = surviving count (for xpr_bin_sort both are I).
+ *   pair_capacity as for xpr_bin_sort: it must hold the CANDIDATE count (sum of tile_count), not only
+ *   the survivors; otherwise XPR_ERR_CAPACITY with *num_pairs_host = the capacity that suffices.
  *   With cfg->tile_cull == 0 the call is xpr_bin_sort; xpr_bin_sort itself rejects cfg->tile_cull != 0.
  */
 int32_t xpr_bin_sort_cull(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,

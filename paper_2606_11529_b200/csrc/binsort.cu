@@ -904,7 +904,6 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     if (!aligned(tile_ranges, 8) || !aligned(workspace, 256)) return XPR_ERR_INVALID_ARG;
     if (N > 0 && (!aligned(depth, 4) || !aligned(tile_rect, 16) || !aligned(tile_count, 4))) return XPR_ERR_INVALID_ARG;
     if (cull && N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(lnv, 4))) return XPR_ERR_INVALID_ARG;
-    if (TW > 0xffff || TH > 0xffff) return XPR_ERR_UNSUPPORTED;     // emit packs a tile coordinate in 16 bits
     if (pair_capacity > 0 && (!aligned(keys_sorted, 8) || !aligned(vals_sorted, 4))) return XPR_ERR_INVALID_ARG;
     const Layout L = make_layout(N, pair_capacity, T);
     if (workspace_bytes < L.total) return XPR_ERR_INVALID_ARG;
