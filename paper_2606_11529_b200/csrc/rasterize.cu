@@ -298,6 +298,9 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             const float4 c = s_col[j];
             float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // mx my A B C r g b
             float v_o = 0.f;
+            // the thread's pixels share dx: accumulate sum dpow, sum dpow dy, sum dpow dy^2 and form the five
+            // geometric gradients once per entry (dpow = dL/dpower of a pixel)
+            float sp = 0.f, spy = 0.f, spyy = 0.f;
 #pragma unroll
             for (int k = 0; k < BWD_PPT; ++k) {
                 if (contrib[k]) {
@@ -308,17 +311,23 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                     T[k] = T[k] * inv;                 // transmittance in front of this entry
                     const float w = alpha * T[k];
                     v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
-                    const float dalpha = g0[k] * (c.x * T[k] - S0[k] * inv) + g1[k] * (c.y * T[k] - S1[k] * inv) +
-                                         g2[k] * (c.z * T[k] - S2[k] * inv);
+                    // dL/dalpha = sum_ch g_ch (c_ch T - S_ch / (1 - alpha)) = T (g . c) - (g . S) / (1 - alpha)
+                    const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
+                    const float gS = fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]));
+                    const float dalpha = fmaf(T[k], gc, -(inv * gS));
                     S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
                     if (og < P.amax) {                 // C14: the clamp has zero derivative
                         const float dpow = og * dalpha;
                         v_o = fmaf(G, dalpha, v_o);
-                        const float dxp = dx * dpow, dyp = dy[k] * dpow;
-                        v[2] = fmaf(-0.5f * dx, dxp, v[2]); v[3] = fmaf(-dx, dyp, v[3]); v[4] = fmaf(-0.5f * dy[k], dyp, v[4]);
-                        v[0] = fmaf(A, dxp, fmaf(Bc, dyp, v[0])); v[1] = fmaf(Bc, dxp, fmaf(Cc, dyp, v[1]));
+                        const float dyp = dy[k] * dpow;
+                        sp += dpow; spy += dyp; spyy = fmaf(dy[k], dyp, spyy);
                     }
                 }
+            }
+            {
+                const float sx = dx * sp;              // sum dpow dx
+                v[0] = fmaf(A, sx, Bc * spy); v[1] = fmaf(Bc, sx, Cc * spy);
+                v[2] = -0.5f * dx * sx; v[3] = -dx * spy; v[4] = -0.5f * spyy;
             }
             const float tot = warp_reduce8(v, lane);
             v_o = warp_sum(v_o);
