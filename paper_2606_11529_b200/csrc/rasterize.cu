@@ -205,6 +205,9 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
 // pixel-pairs and the per-Gaussian reduction runs once per 128 pixel-pairs: each lane first sums
 // its own pixels in registers, then one transposed butterfly (14 shuffles for the 9 gradients)
 // leaves the totals spread over lanes, which issue two RED instructions (8 lanes + 1 lane).
+#ifndef XPR_BWD_BRANCHFREE
+#define XPR_BWD_BRANCHFREE 1
+#endif
 #ifndef XPR_BWD_PPT_SMALL
 #define XPR_BWD_PPT_SMALL 2
 #endif
@@ -303,8 +306,10 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             float sp = 0.f, spy = 0.f, spyy = 0.f;
 #pragma unroll
             for (int k = 0; k < BWD_PPT; ++k) {
-                if (contrib[k]) {
-                    const float G = fast_exp(power[k]);
+                if (XPR_BWD_BRANCHFREE || contrib[k]) {
+                    // (branch-free variant: a pixel that does not contribute enters with o G = 0, hence alpha = 0,
+                    // 1/(1-alpha) = 1, w = 0: its T and S are unchanged and all its terms vanish)
+                    const float G = (XPR_BWD_BRANCHFREE && !contrib[k]) ? 0.0f : fast_exp(power[k]);
                     const float og = ga.z * G;
                     const float alpha = fminf(P.amax, og);
                     const float inv = fast_rcp(1.0f - alpha);
@@ -316,12 +321,11 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                     const float gS = fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]));
                     const float dalpha = fmaf(T[k], gc, -(inv * gS));
                     S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
-                    if (og < P.amax) {                 // C14: the clamp has zero derivative
-                        const float dpow = og * dalpha;
-                        v_o = fmaf(G, dalpha, v_o);
-                        const float dyp = dy[k] * dpow;
-                        sp += dpow; spy += dyp; spyy = fmaf(dy[k], dyp, spyy);
-                    }
+                    const float live = (og < P.amax) ? dalpha : 0.0f;   // C14: the clamp has zero derivative
+                    const float dpow = og * live;
+                    v_o = fmaf(G, live, v_o);
+                    const float dyp = dy[k] * dpow;
+                    sp += dpow; spy += dyp; spyy = fmaf(dy[k], dyp, spyy);
                 }
             }
             {
