@@ -200,14 +200,12 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
     return y;
 }
 
-// Backward compositing (a9).  One CTA of 64 threads per 16x16 tile, 4 pixels per thread (rows
-// 4q..4q+3 of one column), so that a Gaussian's record is read from shared memory once per 4
-// pixel-pairs and the per-Gaussian reduction runs once per 128 pixel-pairs: each lane first sums
-// its own pixels in registers, then one transposed butterfly (14 shuffles for the 9 gradients)
-// leaves the totals spread over lanes, which issue two RED instructions (8 lanes + 1 lane).
-#ifndef XPR_BWD_BRANCHFREE
-#define XPR_BWD_BRANCHFREE 1
-#endif
+// Backward compositing (a9).  One CTA per 16x16 tile; a thread owns BWD_PPT consecutive pixels of one row
+// (4 -> 64 threads, the throughput shape; 2 -> 128 threads for images with few tiles), so that a Gaussian's
+// record is read from shared memory once per BWD_PPT pixel-pairs, the row terms of `power` are shared, and
+// the per-Gaussian reduction runs once per 32 * BWD_PPT pixel-pairs: each lane first sums its own pixels in
+// registers, then one transposed butterfly (14 shuffles for the 9 gradients) leaves the totals spread over
+// lanes, which issue two RED instructions (8 lanes + 1 lane).
 #ifndef XPR_BWD_PPT_SMALL
 #define XPR_BWD_PPT_SMALL 2
 #endif
@@ -231,18 +229,20 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     const int tile = blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
     const int lane = threadIdx.x & 31;
-    const int px = tx * TILE + (threadIdx.x & (TILE - 1));
-    const int py0 = ty * TILE + (threadIdx.x >> 4) * BWD_PPT;
-    const float pxc = (float)px + 0.5f;
+    // a thread owns BWD_PPT consecutive pixels of one row: they share dy and the row terms of `power`
+    constexpr int TPR = TILE / BWD_PPT;                 // threads per tile row
+    const int px0 = tx * TILE + (threadIdx.x % TPR) * BWD_PPT;
+    const int py = ty * TILE + (threadIdx.x / TPR);
+    const float pyc = (float)py + 0.5f;
     const uint2 rg = ranges[tile];
 
     uint32_t n[BWD_PPT];
-    float T[BWD_PPT], S0[BWD_PPT], S1[BWD_PPT], S2[BWD_PPT], g0[BWD_PPT], g1[BWD_PPT], g2[BWD_PPT], pyc[BWD_PPT];
+    float T[BWD_PPT], S0[BWD_PPT], S1[BWD_PPT], S2[BWD_PPT], g0[BWD_PPT], g1[BWD_PPT], g2[BWD_PPT], pxc[BWD_PPT];
     uint32_t wmax = 0;
 #pragma unroll
     for (int k = 0; k < BWD_PPT; ++k) {
-        const int py = py0 + k;
-        pyc[k] = (float)py + 0.5f;
+        const int px = px0 + k;
+        pxc[k] = (float)px + 0.5f;
         n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = 0.0f;
         if (px < P.W && py < P.H) {
             const int64_t pid = (int64_t)py * P.W + px;
@@ -287,51 +287,51 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             const float4 ga = s_gate[j];
             const float A = ge.z, Bc = ge.w, Cc = ga.x;
             const float qa = -0.5f * A, qb = -Bc, qc = -0.5f * Cc;
-            const float dx = pxc - ge.x;
-            float dy[BWD_PPT], power[BWD_PPT];
+            const float dy = pyc - ge.y;
+            const float t1 = __fmul_rn(qb, dy), t2 = __fmul_rn(__fmul_rn(qc, dy), dy);   // row terms of eval_power
+            float dx[BWD_PPT], power[BWD_PPT];
             bool contrib[BWD_PPT], any_c = false;
 #pragma unroll
             for (int k = 0; k < BWD_PPT; ++k) {
-                dy[k] = pyc[k] - ge.y;
-                power[k] = eval_power(qa, qb, qc, dx, dy[k]);
+                dx[k] = pxc[k] - ge.x;
+                power[k] = __fmaf_rn(__fmaf_rn(qa, dx[k], t1), dx[k], t2);               // = eval_power(qa, qb, qc, dx, dy)
                 contrib[k] = (pos < n[k]) && !(power[k] > 0.0f) && !(power[k] < ga.y);
                 any_c |= contrib[k];
             }
             if (!__any_sync(0xffffffffu, any_c)) continue;
             const float4 c = s_col[j];
-            float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};   // mx my A B C r g b
+            float v[8];                                // mx my A B C r g b
+            v[5] = v[6] = v[7] = 0.f;
             float v_o = 0.f;
-            // the thread's pixels share dx: accumulate sum dpow, sum dpow dy, sum dpow dy^2 and form the five
-            // geometric gradients once per entry (dpow = dL/dpower of a pixel)
-            float sp = 0.f, spy = 0.f, spyy = 0.f;
+            // the thread's pixels share dy: accumulate sum dpow, sum dpow dx, sum dpow dx^2 and form the five
+            // geometric gradients once per entry (dpow = dL/dpower of a pixel).  Branch-free over the pixels:
+            // one that does not contribute enters with o G = 0, hence alpha = 0, 1/(1-alpha) = 1, w = 0 -- its T
+            // and S are unchanged and all its terms vanish.
+            float sp = 0.f, spx = 0.f, spxx = 0.f;
 #pragma unroll
             for (int k = 0; k < BWD_PPT; ++k) {
-                if (XPR_BWD_BRANCHFREE || contrib[k]) {
-                    // (branch-free variant: a pixel that does not contribute enters with o G = 0, hence alpha = 0,
-                    // 1/(1-alpha) = 1, w = 0: its T and S are unchanged and all its terms vanish)
-                    const float G = (XPR_BWD_BRANCHFREE && !contrib[k]) ? 0.0f : fast_exp(power[k]);
-                    const float og = ga.z * G;
-                    const float alpha = fminf(P.amax, og);
-                    const float inv = fast_rcp(1.0f - alpha);
-                    T[k] = T[k] * inv;                 // transmittance in front of this entry
-                    const float w = alpha * T[k];
-                    v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
-                    // dL/dalpha = sum_ch g_ch (c_ch T - S_ch / (1 - alpha)) = T (g . c) - (g . S) / (1 - alpha)
-                    const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
-                    const float gS = fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]));
-                    const float dalpha = fmaf(T[k], gc, -(inv * gS));
-                    S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
-                    const float live = (og < P.amax) ? dalpha : 0.0f;   // C14: the clamp has zero derivative
-                    const float dpow = og * live;
-                    v_o = fmaf(G, live, v_o);
-                    const float dyp = dy[k] * dpow;
-                    sp += dpow; spy += dyp; spyy = fmaf(dy[k], dyp, spyy);
-                }
+                const float G = contrib[k] ? fast_exp(power[k]) : 0.0f;
+                const float og = ga.z * G;
+                const float alpha = fminf(P.amax, og);
+                const float inv = fast_rcp(1.0f - alpha);
+                T[k] = T[k] * inv;                     // transmittance in front of this entry
+                const float w = alpha * T[k];
+                v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
+                // dL/dalpha = sum_ch g_ch (c_ch T - S_ch / (1 - alpha)) = T (g . c) - (g . S) / (1 - alpha)
+                const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
+                const float gS = fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]));
+                const float dalpha = fmaf(T[k], gc, -(inv * gS));
+                S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
+                const float live = (og < P.amax) ? dalpha : 0.0f;   // C14: the clamp has zero derivative
+                const float dpow = og * live;
+                v_o = fmaf(G, live, v_o);
+                const float dxp = dx[k] * dpow;
+                sp += dpow; spx += dxp; spxx = fmaf(dx[k], dxp, spxx);
             }
             {
-                const float sx = dx * sp;              // sum dpow dx
-                v[0] = fmaf(A, sx, Bc * spy); v[1] = fmaf(Bc, sx, Cc * spy);
-                v[2] = -0.5f * dx * sx; v[3] = -dx * spy; v[4] = -0.5f * spyy;
+                const float sy = dy * sp;              // sum dpow dy
+                v[0] = fmaf(A, spx, Bc * sy); v[1] = fmaf(Bc, spx, Cc * sy);
+                v[2] = -0.5f * spxx; v[3] = -dy * spx; v[4] = -0.5f * dy * sy;
             }
             const float tot = warp_reduce8(v, lane);
             v_o = warp_sum(v_o);
