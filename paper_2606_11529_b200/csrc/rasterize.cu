@@ -43,7 +43,7 @@ __device__ __forceinline__ float fast_exp(float x) {   // ex2.approx(x * log2 e)
 #endif
 constexpr int FWD_PPT2_MIN_TILES = XPR_FWD_PPT2_MIN_TILES;
 
-template <bool STATS, int PPT>
+template <bool STATS, int PPT, bool BF>
 __global__ void __launch_bounds__(BLOCK / PPT)
 rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
@@ -84,10 +84,28 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             pw_b[u] = __fmaf_rn(__fmaf_rn(ge.z, dxb, t1), dxb, t2);                                  \
         }                                                                                            \
         thr[u] = ga.y; op[u] = ga.z;                                                                 \
+        if (BF) c_##u = (rp)[2];                                                                     \
     }
     // valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12)
+    // BF (lists produced with tile_cull: > 90 % of the visited pairs pass the gate): branch-free -- a pixel that
+    // is done or gated enters with alpha = 0, so T' = T >= t_min and w = 0; otherwise the gated pairs are branched over
 #define XPR_FWD_BLEND(act, power, u, rp, T, C0, C1, C2, last, pos)                                    \
-    if (act) {                                                                                       \
+    if (BF) {                                                                                        \
+        if (STATS) {                                                                                 \
+            if (act) { ++n_visit; if (!((power) > 0.0f) && !((power) < thr[u])) ++n_pass; }          \
+        }                                                                                            \
+        const bool pass = act && !((power) > 0.0f) && !((power) < thr[u]);                           \
+        const float alpha = pass ? fminf(amax, op[u] * fast_exp(power)) : 0.0f;     /* C11 */        \
+        const float Tn = T * (1.0f - alpha);                                                         \
+        const bool stop = Tn < tmin;                                        /* C12: stop, no blend */\
+        const bool blend = pass && !stop;                                                            \
+        act = act && !stop;                                                                          \
+        const float w = blend ? alpha * T : 0.0f;                                                    \
+        C0 = fmaf(c_##u.x, w, C0); C1 = fmaf(c_##u.y, w, C1); C2 = fmaf(c_##u.z, w, C2);             \
+        T = blend ? Tn : T;                                                                          \
+        last = blend ? (pos) : last;                                                                 \
+        if (STATS && blend) ++n_blend;                                                               \
+    } else if (act) {                                                                                \
         if (STATS) ++n_visit;                                                                        \
         if (!((power) > 0.0f) && !((power) < thr[u])) {                                              \
             if (STATS) ++n_pass;                                                                     \
@@ -111,6 +129,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
 
     const float amax = P.amax, tmin = P.tmin;
     float pw_a[4], pw_b[4], thr[4], op[4];
+    float4 c_0, c_1, c_2, c_3;                         // colours of the group's entries
     for (uint32_t base = 0; base < len; base += FWD_BATCH) {
         if (__syncthreads_or(act_a || act_b) == 0) break;
         const uint32_t cnt = min((uint32_t)FWD_BATCH, len - base);
@@ -369,15 +388,16 @@ extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cf
     RasterParams P;
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
-    // throughput shape once the image has enough tiles for several waves of every SM
-    if (T >= FWD_PPT2_MIN_TILES)
-        rasterize_fwd_kernel<false, 2><<<T, BLOCK / 2, 0, (cudaStream_t)stream>>>(
-            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
-    else
-        rasterize_fwd_kernel<false, 1><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
-            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    // throughput shape once the image has enough tiles for several waves of every SM; branch-free blend when
+    // the lists were culled
+#define XPR_FWD(PPT_, BF_)                                                                                          \
+    rasterize_fwd_kernel<false, PPT_, BF_><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                             \
+        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,           \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr)
+    const bool bf = cfg->tile_cull != 0;
+    if (T >= FWD_PPT2_MIN_TILES) { if (bf) XPR_FWD(2, true); else XPR_FWD(2, false); }
+    else                         { XPR_FWD(1, false); }      // latency shape: the branchy blend is shorter
+#undef XPR_FWD
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }
@@ -395,7 +415,7 @@ extern "C" int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* 
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
     XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
-    rasterize_fwd_kernel<true, 1><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+    rasterize_fwd_kernel<true, 1, false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
         P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
         vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr, nullptr, nullptr,
         reinterpret_cast<unsigned long long*>(stats));
