@@ -1,38 +1,48 @@
-// binsort.cu -- xpr_bin_sort: tile binning and the hand-written device radix sort.
+// binsort.cu -- xpr_bin_sort / xpr_bin_sort_cull: tile binning and the hand-written device radix sort.
 //
 // Rasterizer stage of the paper: "prefix-sum of tile counts", "replicate",
-// "assign tile id" x = x_min + (r mod w), y = y_min + floor(r / w), t = y W' + x, "sort
-// lexicographically by (tile id, depth)", "identify bounds".  Key packing tile << 32 | depth bits
-// is BASELINE.json:north_star (reading C10); ties keep ascending Gaussian index.
+// "assign tile id" x = x_min + (r mod w), y = y_min + floor(r / w), t = y W' + x, optional "cull"
+// (tile_cull, Listing 1), "sort lexicographically by (tile id, depth)", "identify bounds".
+// Key packing tile << 32 | depth bits is BASELINE.json:north_star (reading C10); ties keep ascending
+// Gaussian index.
 //
-// The sort is one stable LSD radix sort of the 64-bit keys, 8 bits per pass, reorganised around two
+// The sort is one stable LSD radix sort of the 64-bit keys, 8 bits per pass, reorganised around three
 // observations:
 //  (1) the four low digits are the depth bits, which all pairs of a Gaussian share, and replication
 //      preserves order.  So the four depth passes run on the visible Gaussians (N_vis keys) BEFORE
 //      replication, pairs are emitted in that order, and only the tile-id digits (2 passes at 1080p)
-//      run on the I replicated pairs.
+//      run on the replicated pairs.
 //  (2) once the Gaussians are in (depth, index) order, a pair only has to carry its tile id and the
 //      RANK of its Gaussian in that order: the tile passes move 8-byte words (tile << 32 | rank), and
 //      the last pass expands them to the 64-bit key (tile << 32 | depth bits) and the 32-bit value
 //      (Gaussian index) through two rank-indexed tables.  The expansion happens while the words are
 //      still in the INPUT order of that pass, where neighbouring lanes hold neighbouring ranks, so
 //      the gathers are coalesced (a gather in output order costs one 32-byte sector per pair).
-// The result is bit-identical to sorting the I (key, value) pairs by all digits; HBM traffic per pair
-// drops from 12 + 6*24 + 8 = 164 bytes to 8 + 16 + 20 = 44 bytes.
+//  (3) the unit of replication is a ROW -- the run of consecutive tiles one Gaussian covers in one
+//      tile row: pair r of a row is tile_start + r (no divmod), and tile_cull reduces to one
+//      surviving interval per row (the kept tiles of a row are contiguous because the quadratic form
+//      is convex), found with 3-4 evaluations of the exact per-tile predicate instead of one per tile;
+//      pairs that fail tile_cull are never generated.
+// The result is bit-identical to sorting the (key, value) pairs by all digits; HBM traffic per pair
+// drops from 12 + 6*24 + 8 = 164 bytes to 8 + 16 + 20 = 44 bytes.  No count ever travels to the host
+// inside the call (persistent grids sized for the capacity; optional read-back at the end).
 //
 // Kernels (all hand-written, no CUB):
 //   compact_kernel   single-pass chained scan (decoupled look-back) of the visibility flags; writes
 //                    (depth bits, index) of the visible Gaussians in index order + the 4 depth-digit
 //                    histograms.
 //   onesweep_kernel  one launch per 8-bit digit, least significant first: warp-striped loads,
-//                    stable in-warp ranking (match.any or ballot), shared-memory digit counts,
-//                    per-digit decoupled look-back across tiles, shared-memory staged scatter.
+//                    stable in-warp ranking (shared-memory bitmap or match.any), shared-memory digit
+//                    counts, per-digit decoupled look-back across tiles, shared-memory staged scatter.
 //                    Persistent CTAs draw tiles from a ticket counter.  Instantiated for 32-bit
 //                    keys + values (Gaussians) and for 64-bit packed words (pairs).
-//   offsets_kernel   chained scan of the tile counts in depth order -> pair offsets and I.
-//   emit_kernel      pair-parallel, load-balanced replication: a CTA writes 2048 consecutive pairs
-//                    whatever Gaussians they belong to (segment heads scattered into shared memory,
-//                    max-scan, then one coalesced 8-byte store per pair) + the tile-digit histograms.
+//   scan_kernel<0>   chained scan of the row counts of the Gaussians in depth order -> row bases.
+//   rows_kernel      one thread per row: first tile, rank, number of tiles (whole width, or with
+//                    tile_cull the surviving interval settled by the per-tile predicate tile_keep).
+//   scan_kernel<1>   chained scan of the pairs per row -> pair offsets, I, first row of every emit unit.
+//   emit_kernel      pair-parallel, load-balanced replication: a unit is 2048 consecutive pairs
+//                    whatever rows they belong to (row heads scattered into shared memory, max-scan,
+//                    then one coalesced 8-byte store per pair) + the tile-digit histograms.
 //   ranges_kernel    per-tile (start, end): one warp per tile, 32-ary search in the sorted keys.
 #include "common.cuh"
 
@@ -52,7 +62,10 @@ constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 static_assert(SORT_THREADS == RADIX, "one thread per digit");
 constexpr int IPT32 = 4;                    // Gaussian-level passes: 1024 keys per tile (N_vis is small)
-constexpr int IPT64 = 16;                   // pair-level passes: 4096 pairs per tile
+#ifndef XPR_IPT64
+#define XPR_IPT64 16
+#endif
+constexpr int IPT64 = XPR_IPT64;            // pair-level passes: 4096 pairs per tile
 constexpr int PERSIST_CTAS = 148 * 4;       // upper bound of the persistent grids
 constexpr int EMIT_THREADS = 256, EMIT_PPT = 8, EMIT_PAIRS = EMIT_THREADS * EMIT_PPT;   // emit: 2048 pairs per unit
 constexpr int EMIT_WARPS = EMIT_THREADS / 32;
@@ -678,7 +691,10 @@ __device__ __forceinline__ uint32_t look_back(uint32_t* my, uint32_t tile, uint3
 #define XPR_SORT_MINB64 4
 #endif
 template <class KeyT, int IPT, bool BITMAP, int MODE>
-__global__ void __launch_bounds__(SORT_THREADS, MODE == 2 ? 3 : (sizeof(KeyT) == 8 ? XPR_SORT_MINB64 : 4))   // MODE 2: 66 KB of shared memory
+#ifndef XPR_SORT_MINB_M2
+#define XPR_SORT_MINB_M2 3
+#endif
+__global__ void __launch_bounds__(SORT_THREADS, MODE == 2 ? XPR_SORT_MINB_M2 : (sizeof(KeyT) == 8 ? XPR_SORT_MINB64 : 4))   // MODE 2: 66 KB of shared memory
 onesweep_kernel(const uint32_t* __restrict__ n_dev32, const unsigned long long* __restrict__ n_dev64, int shift,
                 int hist_row, int ticket_row, const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                 KeyT* __restrict__ keys_out, uint32_t* __restrict__ vals_out, Header* __restrict__ hdr,
