@@ -134,3 +134,17 @@ def test_async_bin_sort_matches_sync_and_overflow_renders_background():
     small.rasterize_fwd()
     torch.cuda.synchronize()
     assert float(small.image.abs().max()) == 0.0 and float(small.final_T.min()) == 1.0
+
+
+def test_more_than_65536_tiles_three_tile_digit_passes():
+    """4112 x 4112 pixels = 257 x 257 = 66049 tiles: tile ids need 17 bits -> three tile-digit passes on the pairs
+    (emit_kernel<3>), tile coordinates beyond 8 bits, ragged last tile row/column."""
+    sc = scenes.make_scene(1, n_override=400, image_override=(4112, 4112))
+    for over in (None, dict(tile_cull=1)):
+        g = pu.run_gpu(sc, 0, over)
+        o = pu.run_oracle(sc, 0, over)
+        pu.compare_projection(g, o)
+        pu.compare_binning(g, o)
+        n_frag, _ = pu.compare_forward(g, o)
+        assert n_frag <= 1e-3 * 4112 * 4112
+        assert int(g["binned"]["keys"].max() >> np.uint64(32)) > 65536
