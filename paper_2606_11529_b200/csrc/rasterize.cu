@@ -23,6 +23,13 @@ __device__ __forceinline__ float eval_power(float qa, float qb, float qc, float 
     return __fmaf_rn(__fmaf_rn(qa, dx, __fmul_rn(qb, dy)), dx, __fmul_rn(__fmul_rn(qc, dy), dy));
 }
 
+// o * exp(power) = ex2(power * log2 e + log2 o): one FFMA + one MUFU; l2o = log2 o is staged with the record
+__device__ __forceinline__ float opac_exp(float power, float l2o) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(fmaf(power, 1.4426950408889634f, l2o)));
+    return y;
+}
+
 __device__ __forceinline__ float fast_exp(float x) {   // ex2.approx(x * log2 e); x in [-lnv, 0]
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x * 1.4426950408889634f));
@@ -50,7 +57,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                      float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                      unsigned long long* __restrict__ stats) {
-    // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, o, - | r, g, b, -)
+    // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, log2 o, - | r, g, b, -)
     constexpr int FWD_BATCH = BLOCK / PPT;          // one list entry staged per thread
     __shared__ float4 s_rec[3 * FWD_BATCH];
     const int tile = blockIdx.x;
@@ -95,7 +102,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             if (act) { ++n_visit; if (!((power) > 0.0f) && !((power) < thr[u])) ++n_pass; }          \
         }                                                                                            \
         const bool pass = act && !((power) > 0.0f) && !((power) < thr[u]);                           \
-        const float alpha = pass ? fminf(amax, op[u] * fast_exp(power)) : 0.0f;     /* C11 */        \
+        const float alpha = pass ? fminf(amax, opac_exp(power, op[u])) : 0.0f;      /* C11 */        \
         const float Tn = T * (1.0f - alpha);                                                         \
         const bool stop = Tn < tmin;                                        /* C12: stop, no blend */\
         const bool blend = pass && !stop;                                                            \
@@ -109,7 +116,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
         if (STATS) ++n_visit;                                                                        \
         if (!((power) > 0.0f) && !((power) < thr[u])) {                                              \
             if (STATS) ++n_pass;                                                                     \
-            const float alpha = fminf(amax, op[u] * fast_exp(power));       /* C11 */                \
+            const float alpha = fminf(amax, opac_exp(power, op[u]));        /* C11 */                \
             const float Tn = T * (1.0f - alpha);                                                     \
             if (Tn < tmin) {                                                /* C12: stop, no blend */\
                 act = false;                                                                         \
@@ -139,7 +146,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             const float4 co = conic_opac[g];
             float4* rec = s_rec + 3 * e;
             rec[0] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-            rec[1] = make_float4(-0.5f * co.z, -lnv[g], co.w, 0.0f);
+            rec[1] = make_float4(-0.5f * co.z, -lnv[g], __log2f(co.w), 0.0f);
             rec[2] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
         }
         __syncthreads();
@@ -296,7 +303,7 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             const float4 co = conic_opac[g];
             s_geo[threadIdx.x] = make_float4(m.x, m.y, co.x, co.y);
             s_gate[threadIdx.x] = make_float4(co.z, -lnv[g], co.w, __uint_as_float(g));
-            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
+            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], __log2f(co.w));
         }
         __syncthreads();
         for (uint32_t j = 0; j < cnt; ++j) {
@@ -321,7 +328,6 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             const float4 c = s_col[j];
             float v[8];                                // mx my A B C r g b
             v[5] = v[6] = v[7] = 0.f;
-            float v_o = 0.f;
             // the thread's pixels share dy: accumulate sum dpow, sum dpow dx, sum dpow dx^2 and form the five
             // geometric gradients once per entry (dpow = dL/dpower of a pixel).  Branch-free over the pixels:
             // one that does not contribute enters with o G = 0, hence alpha = 0, 1/(1-alpha) = 1, w = 0 -- its T
@@ -329,8 +335,7 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             float sp = 0.f, spx = 0.f, spxx = 0.f;
 #pragma unroll
             for (int k = 0; k < BWD_PPT; ++k) {
-                const float G = contrib[k] ? fast_exp(power[k]) : 0.0f;
-                const float og = ga.z * G;
+                const float og = contrib[k] ? opac_exp(power[k], c.w) : 0.0f;          // o G
                 const float alpha = fminf(P.amax, og);
                 const float inv = fast_rcp(1.0f - alpha);
                 T[k] = T[k] * inv;                     // transmittance in front of this entry
@@ -342,8 +347,7 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                 const float dalpha = fmaf(T[k], gc, -(inv * gS));
                 S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
                 const float live = (og < P.amax) ? dalpha : 0.0f;   // C14: the clamp has zero derivative
-                const float dpow = og * live;
-                v_o = fmaf(G, live, v_o);
+                const float dpow = og * live;          // dL/dpower; dL/do = G live = dpow / o: summed as sp below
                 const float dxp = dx[k] * dpow;
                 sp += dpow; spx += dxp; spxx = fmaf(dx[k], dxp, spxx);
             }
@@ -353,10 +357,10 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                 v[2] = -0.5f * spxx; v[3] = -dy * spx; v[4] = -0.5f * dy * sy;
             }
             const float tot = warp_reduce8(v, lane);
-            v_o = warp_sum(v_o);
+            const float sp_tot = warp_sum(sp);         // dL/do = (sum dpow) / o, divided by the one lane that adds it
             const uint32_t g = __float_as_uint(ga.w);
             if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
-            if (lane == 0) atomicAdd(g_opac + g, v_o);
+            if (lane == 0) atomicAdd(g_opac + g, sp_tot * fast_rcp(ga.z));
         }
         hi -= cnt;
     }
