@@ -237,10 +237,10 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
 #endif
 
 #ifndef XPR_BWD_MINB
-#define XPR_BWD_MINB 1
+#define XPR_BWD_MINB 12      // 64-thread CTAs per SM in the throughput shape (85 registers)
 #endif
 template <int BWD_PPT>
-__global__ void __launch_bounds__(BLOCK / BWD_PPT, XPR_BWD_MINB)
+__global__ void __launch_bounds__(BLOCK / BWD_PPT, XPR_BWD_MINB * BWD_PPT / 4)
 rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
