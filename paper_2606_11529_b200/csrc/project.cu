@@ -382,7 +382,6 @@ __device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, 
         // coefficient gradients are stored at once, so they do not occupy registers during the chain rule.
         float c[3 * K];
         load_sh<K>(sh, i, c);
-        const B grgb[3] = {(B)grgb_f[0], (B)grgb_f[1], (B)grgb_f[2]};
         float dir[3], dnorm, Y[16];
         view_dir(P, mu, dir, dnorm);
         sh_basis(dir[0], dir[1], dir[2], Y);
@@ -390,16 +389,16 @@ __device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, 
         sh_basis_grad((B)dir[0], (B)dir[1], (B)dir[2], dY);
         B gd[3] = {0, 0, 0};
         float gsh[3 * K];
+        // C16 mask saved by the forward; dL/dd = sum_k grad Y_k(d) w_k with w_k = sum_ch sh[k][ch] g_ch (three fp32
+        // products per coefficient), accumulated over k in fp64
+        const float gr = (fl & XPR_FLAG_RGB_POS_R) ? grgb_f[0] : 0.0f, gg = (fl & XPR_FLAG_RGB_POS_G) ? grgb_f[1] : 0.0f,
+                    gb = (fl & XPR_FLAG_RGB_POS_B) ? grgb_f[2] : 0.0f;
 #pragma unroll
-        for (int ch = 0; ch < 3; ++ch) {
-            const bool on = (fl & (XPR_FLAG_RGB_POS_R << ch)) != 0;   // C16 mask saved by the forward
+        for (int k = 0; k < K; ++k) {
+            gsh[3 * k] = Y[k] * gr; gsh[3 * k + 1] = Y[k] * gg; gsh[3 * k + 2] = Y[k] * gb;
+            const B w = (B)fmaf(c[3 * k], gr, fmaf(c[3 * k + 1], gg, c[3 * k + 2] * gb));
 #pragma unroll
-            for (int k = 0; k < K; ++k) {
-                gsh[3 * k + ch] = on ? Y[k] * grgb_f[ch] : 0.0f;
-                const B cg = on ? (B)c[3 * k + ch] * grgb[ch] : 0.0;
-#pragma unroll
-                for (int j = 0; j < 3; ++j) gd[j] += dY[k][j] * cg;
-            }
+            for (int j = 0; j < 3; ++j) gd[j] += dY[k][j] * w;
         }
         store_sh_grad<K>(g_sh, i, gsh);
         const B dot = (B)dir[0] * gd[0] + (B)dir[1] * gd[1] + (B)dir[2] * gd[2];
