@@ -58,7 +58,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except Exception:
@@ -252,7 +252,6 @@ def run_ours(args):
         step(evs)
         all_events.append(evs)
     barrier()
-    clocks = sampler.stop()
     assert pipe.check_capacity() == n_pairs          # the asynchronous steps produced the same, fitting, pair count
     step_ms = [e[0].elapsed_time(e[-1]) for e in all_events]
     total_ms = max_over_ranks(float(sum(step_ms)), world, dev)
@@ -327,6 +326,8 @@ def run_ours(args):
             graph_ms = max_over_ranks(t_ms, world, dev) / args.steps
         except Exception as e:      # capture unsupported in this environment: report, do not hide
             graph_ms = "unavailable: %s" % (str(e).splitlines()[0][:120],)
+
+    clocks = sampler.stop()      # sampled (every 20 ms) over the timed steps and the graph replays
 
     # end to end through the public API with HOST buffers: H2D of the parameters, the step, D2H of results
     e2e = None
