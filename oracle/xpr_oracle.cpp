@@ -874,3 +874,6 @@ extern "C" int32_t xpr_oracle_num_threads(void) {
     return 1;
 #endif
 }
+
+// XPR-3DGUT ray evaluation
+#include "xpr_oracle_ray.inc"

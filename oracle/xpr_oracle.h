@@ -8,7 +8,7 @@
  *
  * What it computes: the plain definition of tile-based 3DGS rendering and its exact reverse-mode
  * derivative, written from /root/reference/PAPER.md (XPR, arxiv 2606.11529) and the readings
- * C1..C26 / rules R1..R3 in DESIGN.md.  Each function cites the passage it follows
+ * C1..C30 / rules R1..R3 in DESIGN.md.  Each function cites the passage it follows
  * ("PAPER L<line>").  Scalar type: *_f32 = parity mode (every operation individually rounded in
  * fp32, in the order DESIGN.md section 3 fixes; compiled with -ffp-contract=off), *_f64 =
  * self-check mode (closed forms, finite differences).  Gradients are accumulated and returned
@@ -18,7 +18,9 @@
  * transmittance/opacity invariants, P3 brute-force binning, P4 tiling invariance, P5 sort
  * invariants, P6 central finite differences (fp64), P7 UT exact for affine maps, P8 UT~EWA limit,
  * P9 fisheye special cases, P10 SH orthonormality/degree-0, P11 linearity, P12 fp32-vs-fp64,
- * P13 tile_cull (dense-sampling maximum, no passing pixel in a dropped pair, image unchanged).
+ * P13 tile_cull (dense-sampling maximum, no passing pixel in a dropped pair, image unchanged),
+ * P14 3DGUT ray evaluation (brute-force maximum along the ray in the world frame, isotropic closed form,
+ * pixel_info as the inverse of the camera model, finite differences).
  * No function here is "parity unpinned".
  */
 #ifndef XPR_ORACLE_H
@@ -128,6 +130,43 @@ int64_t xpr_oracle_bin_sort_cull(int64_t N, const float* depth, const int32_t* t
                                  const uint32_t* tile_count, const float* mean2d, const float* conic,
                                  const float* lnv, int32_t tiles_x, int32_t tiles_y, int32_t ts, int64_t capacity,
                                  uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges);
+
+/* ---- XPR-3DGUT evaluation, SURVEY 8(f) f2 (xpr_oracle_ray.inc; PAPER A.1.2 L437-444 Eq. 1, Listing 3).
+ * Reading C27: ray and Gaussian live in the camera frame.  pixel_rays [H*W*3]: unit ray directions (camera frame)
+ * through the pixel centres; ray_rec [N*12]: M_c = S^-1 (W R)^T row-major (9), o_c = -M_c p (3).  Pin P14. */
+#define XO_RAY_DECL(S, T)                                                                                \
+    void xpr_oracle_pixel_info_##S(const xo_camera* cam, T* pixel_rays);                                 \
+    void xpr_oracle_pixel_ray_##S(const xo_camera* cam, double u, double v, T* d3);                      \
+    void xpr_oracle_project_ray_##S(int64_t N, const T* means, const T* scales, const T* quats,          \
+                                    const xo_camera* cam, const uint32_t* tile_count, T* ray_rec);       \
+    /* out3 = {power = nhq/dd, nhq = -1/2 |o_c x d_c|^2, dd = |d_c|^2} for one record and one ray */     \
+    void xpr_oracle_ray_power_##S(const T* rec12, const T* d3, T* out3);                                 \
+    void xpr_oracle_rasterize_ray_fwd_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,         \
+                                          const T* ray_rec, const T* opac_eff, const T* rgb,             \
+                                          const T* lnv, const T* pixel_rays, const uint32_t* vals_sorted,\
+                                          const uint32_t* tile_ranges, T* image, T* final_T,             \
+                                          uint32_t* n_contrib, uint8_t* fragile, int64_t* counters);     \
+    /* g_ray_rec [N*12] = dL/dM_c (9), dL/do_c (3) */                                                    \
+    void xpr_oracle_rasterize_ray_bwd_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,         \
+                                          const T* ray_rec, const T* opac_eff, const T* rgb,             \
+                                          const T* lnv, const T* pixel_rays, const uint32_t* vals_sorted,\
+                                          const uint32_t* tile_ranges, const uint32_t* n_contrib,        \
+                                          const T* dL_dimage, double* g_ray_rec, double* g_opac_eff,     \
+                                          double* g_rgb);                                                \
+    void xpr_oracle_rasterize_ray_bwd_mass_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,    \
+                                          const T* ray_rec, const T* opac_eff, const T* rgb,             \
+                                          const T* lnv, const T* pixel_rays, const uint32_t* vals_sorted,\
+                                          const uint32_t* tile_ranges, const uint32_t* n_contrib,        \
+                                          const T* dL_dimage, double* g_ray_rec, double* g_opac_eff,     \
+                                          double* g_rgb);                                                \
+    /* chain rule record -> (mu, s, q); WRITES its outputs (the caller adds them to project_bwd's) */    \
+    void xpr_oracle_ray_bwd_##S(int64_t N, const T* means, const T* scales, const T* quats,              \
+                                const xo_camera* cam, const uint32_t* tile_count,                        \
+                                const double* g_ray_rec, double* g_means, double* g_scales,              \
+                                double* g_quats);
+
+XO_RAY_DECL(f32, float)
+XO_RAY_DECL(f64, double)
 
 int32_t xpr_oracle_num_threads(void);
 

@@ -249,3 +249,109 @@ def backward(scene_arrays: dict, r: dict, dL_dimage, cam: XoCamera, cfg: XoConfi
     g3 = project_bwd(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, g2, dtype)
     g3.update(g2)
     return g3
+
+
+# ---- XPR-3DGUT ray evaluation (xpr_oracle_ray.inc) -------------------------------------------
+
+def pixel_info(cam: XoCamera, dtype=np.float32):
+    dt = np.dtype(dtype)
+    if int(cam.model) not in (0, 1):
+        raise ValueError("ray evaluation is defined for the pinhole and fisheye models only")
+    rays = np.empty((int(cam.height), int(cam.width), 3), dt)
+    getattr(lib(), "xpr_oracle_pixel_info_" + _sfx(dt))(C.byref(cam), _p(rays))
+    return rays
+
+
+def pixel_ray(cam: XoCamera, u: float, v: float, dtype=np.float64):
+    dt = np.dtype(dtype)
+    d = np.empty(3, dt)
+    getattr(lib(), "xpr_oracle_pixel_ray_" + _sfx(dt))(C.byref(cam), C.c_double(u), C.c_double(v), _p(d))
+    return d
+
+
+def project_ray(means, scales, quats, tile_count, cam: XoCamera, dtype=np.float32):
+    dt = np.dtype(dtype)
+    N = int(means.shape[0])
+    a = [np.ascontiguousarray(x, dt) for x in (means, scales, quats)]
+    rec = np.empty((N, 12), dt)
+    getattr(lib(), "xpr_oracle_project_ray_" + _sfx(dt))(C.c_int64(N), *[_p(x) for x in a], C.byref(cam),
+                                                         _p(np.ascontiguousarray(tile_count, np.uint32)), _p(rec))
+    return rec
+
+
+def ray_power(rec12, d3, dtype=np.float64):
+    dt = np.dtype(dtype)
+    out = np.empty(3, dt)
+    getattr(lib(), "xpr_oracle_ray_power_" + _sfx(dt))(_p(np.ascontiguousarray(rec12, dt)), _p(np.ascontiguousarray(d3, dt)), _p(out))
+    return out
+
+
+def rasterize_ray_fwd(proj: dict, binned: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """proj additionally holds ray_rec [N,12] and pixel_rays [H,W,3]."""
+    dt = np.dtype(dtype)
+    H, W = int(cam.height), int(cam.width)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("ray_rec", "opac_eff", "rgb", "lnv", "pixel_rays")]
+    out = dict(image=np.empty((H, W, 3), dt), final_T=np.empty((H, W), dt), n_contrib=np.empty((H, W), np.uint32),
+               fragile=np.empty((H, W), np.uint8))
+    counters = np.zeros(2, np.int64)
+    fn = getattr(lib(), "xpr_oracle_rasterize_ray_fwd_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+       _p(out["image"]), _p(out["final_T"]), _p(out["n_contrib"]), _p(out["fragile"]), _p(counters))
+    out["pp_visit"], out["pp_pass"] = int(counters[0]), int(counters[1])
+    return out
+
+
+def rasterize_ray_bwd(proj: dict, binned: dict, fwd: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32,
+                      mass: bool = False) -> dict:
+    dt = np.dtype(dtype)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("ray_rec", "opac_eff", "rgb", "lnv", "pixel_rays")]
+    dL = np.ascontiguousarray(dL_dimage, dt)
+    out = dict(g_ray_rec=np.empty((N, 12), np.float64), g_opac_eff=np.empty(N, np.float64),
+               g_rgb=np.empty((N, 3), np.float64))
+    fn = getattr(lib(), ("xpr_oracle_rasterize_ray_bwd_mass_" if mass else "xpr_oracle_rasterize_ray_bwd_") + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+       _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), _p(dL),
+       _p(out["g_ray_rec"]), _p(out["g_opac_eff"]), _p(out["g_rgb"]))
+    return out
+
+
+def ray_bwd(means, scales, quats, tile_count, g_ray_rec, cam: XoCamera, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    N = int(means.shape[0])
+    a = [np.ascontiguousarray(x, dt) for x in (means, scales, quats)]
+    out = dict(g_means=np.empty((N, 3), np.float64), g_scales=np.empty((N, 3), np.float64),
+               g_quats=np.empty((N, 4), np.float64))
+    getattr(lib(), "xpr_oracle_ray_bwd_" + _sfx(dt))(
+        C.c_int64(N), *[_p(x) for x in a], C.byref(cam), _p(np.ascontiguousarray(tile_count, np.uint32)),
+        _p(np.ascontiguousarray(g_ray_rec, np.float64)), *[_p(out[k]) for k in ("g_means", "g_scales", "g_quats")])
+    return out
+
+
+def render_ray(scene_arrays: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """XPR-3DGUT forward (PAPER A.1.2): project (2D footprint for tiling / culling) -> shader record -> bin_sort ->
+    pixel_info -> compositing with the ray evaluation."""
+    s = scene_arrays
+    proj = project(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, dtype)
+    proj["ray_rec"] = project_ray(s["means"], s["scales"], s["quats"], proj["tile_count"], cam, dtype)
+    proj["pixel_rays"] = pixel_info(cam, dtype)
+    binned = bin_sort(proj, cam, cfg)
+    fwd = rasterize_ray_fwd(proj, binned, cam, cfg, dtype)
+    return dict(proj=proj, binned=binned, fwd=fwd)
+
+
+def backward_ray(scene_arrays: dict, r: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """Backward of render_ray: the 2D footprint only tiles (no gradient through mean2d / conic); the opacity
+    factor (C19) and the colour go through project_bwd, the record through ray_bwd."""
+    s = scene_arrays
+    g2 = rasterize_ray_bwd(r["proj"], r["binned"], r["fwd"], dL_dimage, cam, cfg, dtype)
+    N = int(s["means"].shape[0])
+    gz = dict(g_mean2d=np.zeros((N, 2)), g_conic=np.zeros((N, 3)), g_opac_eff=g2["g_opac_eff"], g_rgb=g2["g_rgb"])
+    g3 = project_bwd(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, gz, dtype)
+    gr = ray_bwd(s["means"], s["scales"], s["quats"], r["proj"]["tile_count"], g2["g_ray_rec"], cam, dtype)
+    for k in ("g_means", "g_scales", "g_quats"):
+        g3[k] = g3[k] + gr[k]
+    g3.update(g2)
+    g3["ray_part"] = gr
+    return g3
