@@ -2,7 +2,7 @@
  * xpr.h -- C-ABI boundary of libxpr.so: the tile-based splatting forward + backward hot path of
  * "XPR: An Extensible Cross-Platform Point-Based Differentiable Renderer" (arxiv 2606.11529),
  * hand-written CUDA for NVIDIA B200 (sm_100a).  Citations are PAPER.md line numbers ("PAPER L..")
- * plus the readings C1..C26 and arithmetic rules R1..R3 listed in DESIGN.md section 3.
+ * plus the readings C1..C30 and arithmetic rules R1..R3 listed in DESIGN.md section 3.
  *
  * Conventions
  *  - Every function returns an int32_t status (XPR_OK == 0).  No exceptions, no global state other
@@ -186,6 +186,47 @@ int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, cons
                         const float* g_mean2d, const float* g_conic, const float* g_opac, const float* g_rgb,
                         float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh,
                         void* stream);
+
+/*
+ * ---- XPR-3DGUT evaluation (PAPER A.1.2 L437-444 Eq. 1, Listing 3) -----------------
+ * The 2D footprint of xpr_project (UT or EWA) only tiles and culls; a pixel evaluates the 3D Gaussian at the
+ * point of maximum response along its camera ray.  Reading C27: ray and Gaussian are expressed in the camera
+ * frame (ray origin 0, p = W mu + t):  M_c = S^-1 (W R)^T,  o_c = -M_c p,  d_c = M_c d,
+ *   response = exp(-1/2 |o_c x d_c|^2 / |d_c|^2),  alpha = min(alpha_max, o_eff response),
+ *   valid = response > 0.0113 (L500) and alpha >= alpha_thresh, both decided on products (rule R3):
+ *   nhq = -1/2 |o_c x d_c|^2, dd = |d_c|^2:  nhq > ln(0.0113) dd  and  nhq >= -lnv dd.
+ *
+ * xpr_pixel_info -- pixel_info of Listing 3: pixel_rays[H,W,3] = unit direction (camera frame) of the ray through
+ *   the pixel centre (i+0.5, j+0.5), the inverse of the camera model (fisheye: 12 Newton steps on the radial
+ *   polynomial); fp64 inside, rounded to fp32 last (rule R2).  Depends on the intrinsics only.
+ * xpr_project_ray -- shader record p_sd: ray_rec[N,12] = M_c row-major (9), o_c (3); zeros for a culled Gaussian
+ *   (tile_count == 0) and for a record that is not finite (C30).  fp32, rule R1.
+ * xpr_rasterize_ray_fwd / _bwd -- xpr_rasterize_fwd / _bwd with this evaluation; opacity o_eff is read from
+ *   conic_opac[.,3].  bwd ACCUMULATES g_ray_rec[N,12] = dL/dM_c (9), dL/do_c (3), g_opac[N], g_rgb[N,3]
+ *   (zero-filled first when zero_init != 0).
+ * xpr_ray_bwd -- chain rule from g_ray_rec to (mu, s, q), fp64 inside; ADDS to g_means[N,3], g_scales[N,3],
+ *   g_quats[N,4] (call it after xpr_project_bwd, which is given zero g_mean2d / g_conic: the footprint carries
+ *   no gradient, the opacity factor and the colour do).
+ */
+int32_t xpr_pixel_info(const xpr_camera* cam, float* pixel_rays, void* stream);
+int32_t xpr_project_ray(int64_t N, const float* means, const float* scales, const float* quats,
+                        const xpr_camera* cam, const uint32_t* tile_count, float* ray_rec, void* stream);
+int32_t xpr_rasterize_ray_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                              const float* conic_opac, const float* rgb, const float* lnv, const float* pixel_rays,
+                              const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                              float* image, float* final_T, uint32_t* n_contrib, void* stream);
+int32_t xpr_rasterize_ray_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                const float* conic_opac, const float* rgb, const float* lnv, const float* pixel_rays,
+                                const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats,
+                                void* stream);
+int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                              const float* conic_opac, const float* rgb, const float* lnv, const float* pixel_rays,
+                              const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                              const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
+                              float* g_ray_rec, float* g_opac, float* g_rgb, int32_t zero_init, void* stream);
+int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const float* quats,
+                    const xpr_camera* cam, const uint32_t* tile_count, const float* g_ray_rec,
+                    float* g_means, float* g_scales, float* g_quats, void* stream);
 
 #ifdef __cplusplus
 }

@@ -18,7 +18,9 @@ XPR_OK, XPR_ERR_INVALID_ARG, XPR_ERR_CAPACITY, XPR_ERR_CUDA, XPR_ERR_UNSUPPORTED
 FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_RGB_POS_B = 1, 2, 4, 8, 16, 32
 
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
-           "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd")
+           "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
+           "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
+           "xpr_ray_bwd")
 
 
 class XprCamera(C.Structure):
@@ -189,3 +191,47 @@ def xpr_project_bwd(means, scales, quats, opacities, sh, cam: XprCamera, cfg: Xp
                                  C.byref(cfg), _p(tile_count), _p(flags), _p(g_mean2d), _p(g_conic), _p(g_opac),
                                  _p(g_rgb), _p(g_means), _p(g_scales), _p(g_quats), _p(g_opacities), _p(g_sh),
                                  _stream(stream)), "xpr_project_bwd")
+
+
+# ---- XPR-3DGUT ray evaluation (xpr.h) ----------------------------------------------------------
+
+def xpr_pixel_info(cam: XprCamera, pixel_rays, stream=None):
+    _check(lib().xpr_pixel_info(C.byref(cam), _p(pixel_rays), _stream(stream)), "xpr_pixel_info")
+
+
+def xpr_project_ray(means, scales, quats, cam: XprCamera, tile_count, ray_rec, stream=None):
+    N = int(means.shape[0])
+    _check(lib().xpr_project_ray(C.c_int64(N), _p(means), _p(scales), _p(quats), C.byref(cam), _p(tile_count),
+                                 _p(ray_rec), _stream(stream)), "xpr_project_ray")
+
+
+def xpr_rasterize_ray_fwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, pixel_rays, vals_sorted,
+                          tile_ranges, image, final_T, n_contrib, stream=None):
+    N = int(ray_rec.shape[0])
+    _check(lib().xpr_rasterize_ray_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec), _p(conic_opac), _p(rgb),
+                                       _p(lnv), _p(pixel_rays), _p(vals_sorted), _p(tile_ranges), _p(image),
+                                       _p(final_T), _p(n_contrib), _stream(stream)), "xpr_rasterize_ray_fwd")
+
+
+def xpr_rasterize_ray_stats(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, pixel_rays, vals_sorted,
+                            tile_ranges, stats, stream=None):
+    N = int(ray_rec.shape[0])
+    _check(lib().xpr_rasterize_ray_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec), _p(conic_opac),
+                                         _p(rgb), _p(lnv), _p(pixel_rays), _p(vals_sorted), _p(tile_ranges),
+                                         _p(stats), _stream(stream)), "xpr_rasterize_ray_stats")
+
+
+def xpr_rasterize_ray_bwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, pixel_rays, vals_sorted,
+                          tile_ranges, final_T, n_contrib, dL_dimage, g_ray_rec, g_opac, g_rgb, zero_init: bool = True,
+                          stream=None):
+    N = int(ray_rec.shape[0])
+    _check(lib().xpr_rasterize_ray_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec), _p(conic_opac), _p(rgb),
+                                       _p(lnv), _p(pixel_rays), _p(vals_sorted), _p(tile_ranges), _p(final_T),
+                                       _p(n_contrib), _p(dL_dimage), _p(g_ray_rec), _p(g_opac), _p(g_rgb),
+                                       C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_ray_bwd")
+
+
+def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_rec, g_means, g_scales, g_quats, stream=None):
+    N = int(means.shape[0])
+    _check(lib().xpr_ray_bwd(C.c_int64(N), _p(means), _p(scales), _p(quats), C.byref(cam), _p(tile_count),
+                             _p(g_ray_rec), _p(g_means), _p(g_scales), _p(g_quats), _stream(stream)), "xpr_ray_bwd")

@@ -2,7 +2,7 @@
 
     python -m paper_2606_11529_b200.build [--force]
 
-nvcc cross-compiles without a GPU.  project.cu is compiled with -fmad=false (rule R1 of
+nvcc cross-compiles without a GPU.  project.cu and ray.cu are compiled with -fmad=false (rule R1 of
 DESIGN.md: no FMA contraction in anything that feeds depth bits, rectangles or tile counts).
 """
 from __future__ import annotations
@@ -26,6 +26,8 @@ SOURCES = {
     "project.cu": ["-fmad=false"],
     "binsort.cu": [],
     "rasterize.cu": [],
+    "ray.cu": ["-fmad=false"],
+    "rasterize_ray.cu": [],
 }
 
 

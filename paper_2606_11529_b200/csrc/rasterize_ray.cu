@@ -1,0 +1,398 @@
+// rasterize_ray.cu -- xpr_rasterize_ray_fwd / _bwd: per-tile front-to-back compositing with the XPR-3DGUT
+// evaluation (PAPER A.1.2 L437-444 Eq. 1, Listing 3) and its reverse-mode pass.
+//
+// Same tile / list / batch structure as rasterize.cu; the per-entry evaluation is the maximum response of the 3D
+// Gaussian along the pixel's camera ray d (reading C27, camera frame):
+//   d_c = M_c d,  c = o_c x d_c,  nhq = -1/2 |c|^2,  dd = |d_c|^2,  response = exp(nhq / dd).
+// Decisions are taken on products in the fixed fp32 order of rule R3 (explicit _rn intrinsics), never on the
+// quotient or on exp():  valid <=> nhq > ln(0.0113) dd (L500),  gate <=> nhq >= -lnv dd (C12).
+#include <math.h>
+
+#include "common.cuh"
+
+namespace xpr {
+namespace {
+
+constexpr int BLOCK = TILE * TILE;
+
+struct RayRasterParams {
+    int W, H, TW;
+    float amax, tmin, lnr;     // lnr = (float) ln(0.0113)
+    float bg[3];
+};
+
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// evaluate (Listing 3) in the fixed fp32 order of DESIGN.md 3 (rule R3)
+struct RayEval { float dc0, dc1, dc2, c0, c1, c2, nhq, dd; };
+__device__ __forceinline__ RayEval eval_ray(const float4 r0, const float4 r1, const float4 r2, float d0, float d1,
+                                            float d2) {
+    RayEval e;
+    e.dc0 = __fmaf_rn(r0.z, d2, __fmaf_rn(r0.y, d1, __fmul_rn(r0.x, d0)));
+    e.dc1 = __fmaf_rn(r1.y, d2, __fmaf_rn(r1.x, d1, __fmul_rn(r0.w, d0)));
+    e.dc2 = __fmaf_rn(r2.x, d2, __fmaf_rn(r1.w, d1, __fmul_rn(r1.z, d0)));
+    const float o0 = r2.y, o1 = r2.z, o2 = r2.w;
+    e.c0 = __fmaf_rn(o1, e.dc2, -__fmul_rn(o2, e.dc1));
+    e.c1 = __fmaf_rn(o2, e.dc0, -__fmul_rn(o0, e.dc2));
+    e.c2 = __fmaf_rn(o0, e.dc1, -__fmul_rn(o1, e.dc0));
+    const float q = __fmaf_rn(e.c2, e.c2, __fmaf_rn(e.c1, e.c1, __fmul_rn(e.c0, e.c0)));
+    e.dd = __fmaf_rn(e.dc2, e.dc2, __fmaf_rn(e.dc1, e.dc1, __fmul_rn(e.dc0, e.dc0)));
+    e.nhq = __fmul_rn(-0.5f, q);
+    return e;
+}
+
+// Forward (a8 with the f2 evaluation).  One CTA per tile, one thread per pixel; record of a list entry in shared
+// memory: 5 x float4 = (M_c, o_c | thr = -lnv, log2 o, r, g | b).  STATS as in rasterize.cu.
+template <bool STATS>
+__global__ void __launch_bounds__(BLOCK)
+rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, const float4* __restrict__ conic_opac,
+                         const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ rays,
+                         const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
+                         float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
+                         unsigned long long* __restrict__ stats) {
+    __shared__ float4 s_geo[3 * BLOCK];
+    __shared__ float4 s_att[BLOCK];      // thr, log2 o, r, g
+    __shared__ float s_blue[BLOCK];
+    const int tile = blockIdx.x;
+    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int px = tx * TILE + (threadIdx.x % TILE), py = ty * TILE + (threadIdx.x / TILE);
+    const bool inside = (px < P.W) && (py < P.H);
+    const int64_t pid = (int64_t)py * P.W + px;
+    float d0 = 0.f, d1 = 0.f, d2 = 1.f;
+    if (inside) { d0 = rays[3 * pid]; d1 = rays[3 * pid + 1]; d2 = rays[3 * pid + 2]; }
+    const uint2 rg = ranges[tile];
+    const uint32_t len = rg.y - rg.x;
+    const float amax = P.amax, tmin = P.tmin, lnr = P.lnr;
+
+    float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
+    uint32_t last = 0;
+    bool act = inside;
+    uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
+
+    for (uint32_t base = 0; base < len; base += BLOCK) {
+        if (__syncthreads_or(act) == 0) break;
+        const uint32_t cnt = min((uint32_t)BLOCK, len - base);
+        if (threadIdx.x < cnt) {
+            const uint32_t g = vals[rg.x + base + threadIdx.x];
+            s_geo[3 * threadIdx.x] = ray_rec[3 * (size_t)g];
+            s_geo[3 * threadIdx.x + 1] = ray_rec[3 * (size_t)g + 1];
+            s_geo[3 * threadIdx.x + 2] = ray_rec[3 * (size_t)g + 2];
+            s_att[threadIdx.x] = make_float4(-lnv[g], __log2f(conic_opac[g].w), rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1]);
+            s_blue[threadIdx.x] = rgb[3 * (size_t)g + 2];
+        }
+        __syncthreads();
+        if (act) {
+            // groups of 4: the evaluations are independent of the transmittance, so their latencies overlap;
+            // the sequential part (gates, alpha, T' = T (1 - alpha), exit test, blend) follows
+            for (uint32_t j0 = 0; j0 < cnt && act; j0 += 4) {
+                float nhq[4], dd[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t j = min(j0 + u, cnt - 1);
+                    const RayEval e = eval_ray(s_geo[3 * j], s_geo[3 * j + 1], s_geo[3 * j + 2], d0, d1, d2);
+                    nhq[u] = e.nhq; dd[u] = e.dd;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t j = j0 + u;
+                    if (j < cnt && act) {
+                        if (STATS) ++n_visit;
+                        const float4 at = s_att[j];
+                        const float tv = __fmul_rn(lnr, dd[u]), tg = __fmul_rn(at.x, dd[u]);
+                        if ((nhq[u] > tv) && !(nhq[u] < tg)) {            // valid (L500) and alpha >= alpha_thresh (C12)
+                            if (STATS) ++n_pass;
+                            const float power = nhq[u] * rcp_approx(dd[u]);
+                            const float alpha = fminf(amax, ex2_approx(fmaf(power, 1.4426950408889634f, at.y)));   // C11
+                            const float Tn = T * (1.0f - alpha);
+                            if (Tn < tmin) {                              // C12: stop, no blend
+                                act = false;
+                            } else {
+                                const float w = alpha * T;
+                                C0 = fmaf(at.z, w, C0); C1 = fmaf(at.w, w, C1); C2 = fmaf(s_blue[j], w, C2);
+                                T = Tn;
+                                last = base + j + 1;
+                                if (STATS) ++n_blend;
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (STATS) {
+        atomicAdd(stats + 0, (unsigned long long)n_visit); atomicAdd(stats + 1, (unsigned long long)n_pass);
+        atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)last);
+        return;
+    }
+    if (inside) {
+        image[3 * pid] = fmaf(T, P.bg[0], C0);
+        image[3 * pid + 1] = fmaf(T, P.bg[1], C1);
+        image[3 * pid + 2] = fmaf(T, P.bg[2], C2);
+        final_T[pid] = T;
+        n_contrib[pid] = last;
+    }
+}
+
+// Transposed butterfly (see rasterize.cu): 8 per-lane values -> lane L with (L & 3) == 0 holds the total of value L >> 2.
+__device__ __forceinline__ float warp_reduce8(const float* v, int lane) {
+    float w[4], x[2];
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float send = b4 ? v[i] : v[i + 4], keep = b4 ? v[i + 4] : v[i];
+        w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const float send = b3 ? w[i] : w[i + 2], keep = b3 ? w[i + 2] : w[i];
+        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    const float send = b2 ? x[0] : x[1], keep = b2 ? x[1] : x[0];
+    float y = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    y += __shfl_xor_sync(0xffffffffu, y, 2);
+    y += __shfl_xor_sync(0xffffffffu, y, 1);
+    return y;
+}
+
+// Backward (a9 with the f2 evaluation).  A thread owns PPT consecutive pixels of a row and sums their 16 gradient
+// terms per entry in registers (dL/dM_c 9, dL/do_c 3, dL/do 1, dL/drgb 3); two transposed butterflies leave the
+// warp totals spread over the lanes, which issue two RED instructions each.  With g_p = dL/dpower:
+//   dL/dc = -(g_p/dd) c,  dL/ddd = -g_p power/dd,  dL/dd_c = dL/dc x o_c + 2 dL/ddd d_c,  dL/do_c = d_c x dL/dc,
+//   dL/dM_c = dL/dd_c d^T.
+#ifndef XPR_RAY_BWD_PPT
+#define XPR_RAY_BWD_PPT 2
+#endif
+template <int PPT>
+__global__ void __launch_bounds__(BLOCK / PPT)
+rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, const float4* __restrict__ conic_opac,
+                         const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ rays,
+                         const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
+                         const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
+                         const float* __restrict__ dL, float* __restrict__ g_rec, float* __restrict__ g_opac,
+                         float* __restrict__ g_rgb) {
+    constexpr int THREADS = BLOCK / PPT, BATCH = THREADS;
+    __shared__ float4 s_geo[3 * BATCH];
+    __shared__ float4 s_gate[BATCH];   // thr, o, log2 o, index (bits)
+    __shared__ float4 s_col[BATCH];    // r, g, b, -
+    __shared__ uint32_t s_max[THREADS / 32];
+    const int tile = blockIdx.x;
+    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int lane = threadIdx.x & 31;
+    constexpr int TPR = TILE / PPT;
+    const int px0 = tx * TILE + (threadIdx.x % TPR) * PPT;
+    const int py = ty * TILE + (threadIdx.x / TPR);
+    const uint2 rg = ranges[tile];
+    const float lnr = P.lnr;
+
+    uint32_t n[PPT];
+    float T[PPT], S0[PPT], S1[PPT], S2[PPT], g0[PPT], g1[PPT], g2[PPT], d0[PPT], d1[PPT], d2[PPT];
+    uint32_t wmax = 0;
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+        const int px = px0 + k;
+        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = 0.0f; d0[k] = d1[k] = 0.0f; d2[k] = 1.0f;
+        if (px < P.W && py < P.H) {
+            const int64_t pid = (int64_t)py * P.W + px;
+            n[k] = n_contrib[pid];
+            T[k] = final_T[pid];
+            g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
+            d0[k] = rays[3 * pid]; d1[k] = rays[3 * pid + 1]; d2[k] = rays[3 * pid + 2];
+        }
+        S0[k] = T[k] * P.bg[0]; S1[k] = T[k] * P.bg[1]; S2[k] = T[k] * P.bg[2];
+        wmax = max(wmax, n[k]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+    if (lane == 0) s_max[threadIdx.x >> 5] = wmax;
+    __syncthreads();
+    uint32_t max_n = 0;
+#pragma unroll
+    for (int w = 0; w < THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
+
+    // lane 4 i owns value i of butterfly A (dL/dM_c[0..8)) and value i of butterfly B (dL/dM_c[8], dL/do_c, dL/do, rgb)
+    const int vi = lane >> 2;
+    const bool red_lane = (lane & 3) == 0;
+    float* const baseB = (vi < 4) ? (g_rec + 8 + vi) : (vi == 4) ? g_opac : (g_rgb + (vi - 5));
+    const uint32_t strideB = (vi < 4) ? 12u : (vi == 4) ? 1u : 3u;
+
+    for (uint32_t hi = max_n; hi > 0;) {
+        const uint32_t cnt = min((uint32_t)BATCH, hi);
+        __syncthreads();
+        if (threadIdx.x < cnt) {      // slot j holds list position hi-1-j (descending)
+            const uint32_t g = vals[rg.x + hi - 1 - threadIdx.x];
+            s_geo[3 * threadIdx.x] = ray_rec[3 * (size_t)g];
+            s_geo[3 * threadIdx.x + 1] = ray_rec[3 * (size_t)g + 1];
+            s_geo[3 * threadIdx.x + 2] = ray_rec[3 * (size_t)g + 2];
+            const float o = conic_opac[g].w;
+            s_gate[threadIdx.x] = make_float4(-lnv[g], o, __log2f(o), __uint_as_float(g));
+            s_col[threadIdx.x] = make_float4(rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1], rgb[3 * (size_t)g + 2], 0.0f);
+        }
+        __syncthreads();
+        for (uint32_t j = 0; j < cnt; ++j) {
+            const uint32_t pos = hi - 1 - j;
+            if (pos >= wmax) continue;     // warp-uniform
+            const float4 r0 = s_geo[3 * j], r1 = s_geo[3 * j + 1], r2 = s_geo[3 * j + 2];
+            const float4 ga = s_gate[j];
+            RayEval e[PPT];
+            bool contrib[PPT], any_c = false;
+#pragma unroll
+            for (int k = 0; k < PPT; ++k) {
+                e[k] = eval_ray(r0, r1, r2, d0[k], d1[k], d2[k]);
+                const float tv = __fmul_rn(lnr, e[k].dd), tg = __fmul_rn(ga.x, e[k].dd);
+                contrib[k] = (pos < n[k]) && (e[k].nhq > tv) && !(e[k].nhq < tg);
+                any_c |= contrib[k];
+            }
+            if (!__any_sync(0xffffffffu, any_c)) continue;
+            const float4 c = s_col[j];
+            const float o0 = r2.y, o1 = r2.z, o2 = r2.w;
+            float va[8], vb[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) va[i] = vb[i] = 0.f;
+#pragma unroll
+            for (int k = 0; k < PPT; ++k) {
+                // a pixel that does not contribute enters with 1/dd = 0 and o G = 0: every term vanishes
+                const float rdd = contrib[k] ? rcp_approx(e[k].dd) : 0.0f;
+                const float power = e[k].nhq * rdd;
+                const float og = contrib[k] ? ex2_approx(fmaf(power, 1.4426950408889634f, ga.z)) : 0.0f;   // o G
+                const float alpha = fminf(P.amax, og);
+                const float inv = rcp_approx(1.0f - alpha);
+                T[k] = T[k] * inv;                     // transmittance in front of this entry
+                const float w = alpha * T[k];
+                vb[5] = fmaf(w, g0[k], vb[5]); vb[6] = fmaf(w, g1[k], vb[6]); vb[7] = fmaf(w, g2[k], vb[7]);
+                const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
+                const float gS = fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]));
+                const float dalpha = fmaf(T[k], gc, -(inv * gS));
+                S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
+                const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
+                const float gp = og * live;            // dL/dpower; dL/do = gp / o, divided once per warp below
+                vb[4] += gp;
+                const float k1 = -gp * rdd;            // dL/dc = k1 c
+                const float gc0 = k1 * e[k].c0, gc1 = k1 * e[k].c1, gc2 = k1 * e[k].c2;
+                const float gdd2 = 2.0f * k1 * power;  // 2 dL/ddd
+                const float gd0 = fmaf(gdd2, e[k].dc0, fmaf(gc1, o2, -(gc2 * o1)));
+                const float gd1 = fmaf(gdd2, e[k].dc1, fmaf(gc2, o0, -(gc0 * o2)));
+                const float gd2 = fmaf(gdd2, e[k].dc2, fmaf(gc0, o1, -(gc1 * o0)));
+                vb[1] += fmaf(e[k].dc1, gc2, -(e[k].dc2 * gc1));     // dL/do_c = d_c x dL/dc
+                vb[2] += fmaf(e[k].dc2, gc0, -(e[k].dc0 * gc2));
+                vb[3] += fmaf(e[k].dc0, gc1, -(e[k].dc1 * gc0));
+                va[0] = fmaf(gd0, d0[k], va[0]); va[1] = fmaf(gd0, d1[k], va[1]); va[2] = fmaf(gd0, d2[k], va[2]);
+                va[3] = fmaf(gd1, d0[k], va[3]); va[4] = fmaf(gd1, d1[k], va[4]); va[5] = fmaf(gd1, d2[k], va[5]);
+                va[6] = fmaf(gd2, d0[k], va[6]); va[7] = fmaf(gd2, d1[k], va[7]); vb[0] = fmaf(gd2, d2[k], vb[0]);
+            }
+            const float ta = warp_reduce8(va, lane);
+            float tb = warp_reduce8(vb, lane);
+            if (red_lane) {
+                const uint32_t g = __float_as_uint(ga.w);
+                if (vi == 4) tb *= rcp_approx(ga.y);   // dL/do = (sum g_p) / o
+                atomicAdd(g_rec + 12 * (size_t)g + vi, ta);
+                atomicAdd(baseB + (size_t)strideB * g, tb);
+            }
+        }
+        hi -= cnt;
+    }
+}
+
+int32_t make_params(const xpr_camera* cam, const xpr_config* cfg, RayRasterParams& P) {
+    P.W = cam->width; P.H = cam->height; P.TW = tiles_x(cam);
+    P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
+    P.lnr = (float)log(0.0113);
+    for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
+    return XPR_OK;
+}
+
+int32_t check_ray_cam_cfg(const xpr_camera* cam, const xpr_config* cfg) {
+    if (!cam || !cfg) return XPR_ERR_INVALID_ARG;
+    if (cam->width <= 0 || cam->height <= 0) return XPR_ERR_INVALID_ARG;
+    if (cfg->tile != TILE) return XPR_ERR_UNSUPPORTED;
+    return XPR_OK;
+}
+
+}  // namespace
+}  // namespace xpr
+
+using namespace xpr;
+
+extern "C" int32_t xpr_rasterize_ray_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                         const float* conic_opac, const float* rgb, const float* lnv,
+                                         const float* pixel_rays, const uint32_t* vals_sorted,
+                                         const uint32_t* tile_ranges, float* image, float* final_T,
+                                         uint32_t* n_contrib, void* stream) {
+    if (int32_t s = check_ray_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4) ||
+        !aligned(pixel_rays, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(ray_rec, 16) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+                  !aligned(vals_sorted, 4)))
+        return XPR_ERR_INVALID_ARG;
+    RayRasterParams P;
+    make_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    rasterize_ray_fwd_kernel<false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays,
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_ray_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N,
+                                           const float* ray_rec, const float* conic_opac, const float* rgb,
+                                           const float* lnv, const float* pixel_rays, const uint32_t* vals_sorted,
+                                           const uint32_t* tile_ranges, uint64_t* stats, void* stream) {
+    if (int32_t s = check_ray_cam_cfg(cam, cfg)) return s;
+    if (N < 0 || !aligned(tile_ranges, 8) || !aligned(stats, 8) || !aligned(pixel_rays, 4)) return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(ray_rec, 16) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+                  !aligned(vals_sorted, 4)))
+        return XPR_ERR_INVALID_ARG;
+    RayRasterParams P;
+    make_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
+    rasterize_ray_fwd_kernel<true><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays,
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr, nullptr, nullptr,
+        reinterpret_cast<unsigned long long*>(stats));
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                         const float* conic_opac, const float* rgb, const float* lnv,
+                                         const float* pixel_rays, const uint32_t* vals_sorted,
+                                         const uint32_t* tile_ranges, const float* final_T, const uint32_t* n_contrib,
+                                         const float* dL_dimage, float* g_ray_rec, float* g_opac, float* g_rgb,
+                                         int32_t zero_init, void* stream) {
+    if (int32_t s = check_ray_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4) ||
+        !aligned(pixel_rays, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(ray_rec, 16) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+        !aligned(vals_sorted, 4) || !aligned(g_ray_rec, 4) || !aligned(g_opac, 4) || !aligned(g_rgb, 4))
+        return XPR_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (zero_init) {
+        XPR_CUDA(cudaMemsetAsync(g_ray_rec, 0, sizeof(float) * 12 * (size_t)N, st));
+        XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * (size_t)N, st));
+        XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * (size_t)N, st));
+    }
+    RayRasterParams P;
+    make_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    rasterize_ray_bwd_kernel<XPR_RAY_BWD_PPT><<<T, BLOCK / XPR_RAY_BWD_PPT, 0, st>>>(
+        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays,
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_ray_rec, g_opac,
+        g_rgb);
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}

@@ -3,6 +3,9 @@
 No arithmetic of the method lives here -- each stage is one call into libxpr.so (binding.py).
 Call stack of one step:
     xpr_project -> xpr_bin_sort -> xpr_rasterize_fwd -> [loss outside] -> xpr_rasterize_bwd -> xpr_project_bwd
+With cfg["ray_eval"] = 1 (XPR-3DGUT evaluation):
+    xpr_pixel_info, xpr_project -> xpr_project_ray -> xpr_bin_sort -> xpr_rasterize_ray_fwd -> [loss] ->
+    xpr_rasterize_ray_bwd -> xpr_project_bwd (zero footprint gradients) -> xpr_ray_bwd
 """
 from __future__ import annotations
 
@@ -18,6 +21,7 @@ class SplatPipeline:
         self.N = int(N)
         self.device = torch.device(device)
         self.cam = cam if isinstance(cam, xb.XprCamera) else xb.make_camera(cam)
+        self.ray_eval = bool(cfg.get("ray_eval", 0)) if isinstance(cfg, dict) else False
         self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
         self.K = (int(self.cfg.sh_degree) + 1) ** 2
         self.W, self.H = int(self.cam.width), int(self.cam.height)
@@ -42,6 +46,11 @@ class SplatPipeline:
         self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb = e(N, 2), e(N, 3), e(N), e(N, 3)
         self.g_means, self.g_scales, self.g_quats = e(N, 3), e(N, 3), e(N, 4)
         self.g_opacities, self.g_sh = e(N), e(N, self.K, 3)
+        if self.ray_eval:   # f2: shader record, per-pixel rays, record gradient
+            self.ray_rec, self.g_ray_rec = e(N, 12), e(N, 12)
+            self.pixel_rays = e(self.H, self.W, 3)
+            self.pixel_info()
+            self.g_mean2d.zero_(); self.g_conic.zero_()    # the footprint carries no gradient
 
     def _alloc_pairs(self, cap: int):
         cap = min(int(cap), (1 << 30) - 1)
@@ -57,6 +66,13 @@ class SplatPipeline:
         self._inputs = (means, scales, quats, opacities, sh)
         xb.xpr_project(means, scales, quats, opacities, sh, self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb,
                        self.depth, self.lnv, self.tile_rect, self.tile_count, self.flags)
+
+    def pixel_info(self):
+        xb.xpr_pixel_info(self.cam, self.pixel_rays)
+
+    def project_ray(self):
+        means, scales, quats, _, _ = self._inputs
+        xb.xpr_project_ray(means, scales, quats, self.cam, self.tile_count, self.ray_rec)
 
     def bin_sort(self):
         while True:
@@ -104,10 +120,20 @@ class SplatPipeline:
         return n
 
     def rasterize_fwd(self):
+        if self.ray_eval:
+            xb.xpr_rasterize_ray_fwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv,
+                                     self.pixel_rays, self.vals_sorted, self.tile_ranges, self.image, self.final_T,
+                                     self.n_contrib)
+            return
         xb.xpr_rasterize_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
                              self.tile_ranges, self.image, self.final_T, self.n_contrib)
 
     def rasterize_bwd(self, dL_dimage):
+        if self.ray_eval:
+            xb.xpr_rasterize_ray_bwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv,
+                                     self.pixel_rays, self.vals_sorted, self.tile_ranges, self.final_T, self.n_contrib,
+                                     dL_dimage, self.g_ray_rec, self.g_opac, self.g_rgb, zero_init=True)
+            return
         xb.xpr_rasterize_bwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
                              self.tile_ranges, self.final_T, self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic,
                              self.g_opac, self.g_rgb, zero_init=True)
@@ -117,10 +143,15 @@ class SplatPipeline:
         xb.xpr_project_bwd(means, scales, quats, opacities, sh, self.cam, self.cfg, self.tile_count, self.flags,
                            self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb, self.g_means, self.g_scales,
                            self.g_quats, self.g_opacities, self.g_sh)
+        if self.ray_eval:
+            xb.xpr_ray_bwd(means, scales, quats, self.cam, self.tile_count, self.g_ray_rec, self.g_means,
+                           self.g_scales, self.g_quats)
 
     # ---- whole passes -------------------------------------------------------------------------
     def forward(self, means, scales, quats, opacities, sh):
         self.project(means, scales, quats, opacities, sh)
+        if self.ray_eval:
+            self.project_ray()
         self.bin_sort()
         self.rasterize_fwd()
         return self.image

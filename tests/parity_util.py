@@ -33,6 +33,8 @@ def run_gpu(scene, view=0, cfg_over=None, pair_capacity=None, dL=None):
                        rgb=pipe.rgb.cpu().numpy(), depth=pipe.depth.cpu().numpy(), lnv=pipe.lnv.cpu().numpy(),
                        tile_rect=pipe.tile_rect.cpu().numpy(), tile_count=u32(pipe.tile_count),
                        flags=pipe.flags.cpu().numpy())
+    if pipe.ray_eval:
+        out["proj"].update(ray_rec=pipe.ray_rec.cpu().numpy(), pixel_rays=pipe.pixel_rays.cpu().numpy())
     out["binned"] = dict(keys=pipe.keys_sorted[:I].cpu().numpy().view(np.uint64), vals=u32(pipe.vals_sorted[:I]),
                          ranges=u32(pipe.tile_ranges), num_pairs=I)
     out["fwd"] = dict(image=pipe.image.cpu().numpy(), final_T=pipe.final_T.cpu().numpy(), n_contrib=u32(pipe.n_contrib))
@@ -46,6 +48,8 @@ def run_gpu_backward(g, dL_np):
     pipe.backward(dL)
     torch.cuda.synchronize()
     names = ("g_mean2d", "g_conic", "g_opac", "g_rgb", "g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
+    if pipe.ray_eval:
+        names = names + ("g_ray_rec",)
     return {k: getattr(pipe, k).cpu().numpy() for k in names}
 
 
@@ -59,6 +63,24 @@ def run_oracle(scene, view=0, cfg_over=None, fragile_rel=2e-5):
     r = xo.render(arrays, cam, ocfg, np.float32)
     r.update(cam=cam, cfg=ocfg, arrays=arrays)
     return r
+
+
+def run_oracle_ray(scene, view=0, cfg_over=None, fragile_rel=2e-5, pixel_rays=None):
+    """XPR-3DGUT evaluation (f2).  pixel_rays: use these rays (the GPU's, stage isolation of pixel_info) instead of
+    the oracle's own."""
+    cfg = scenes.default_render_config(scene)
+    if cfg_over:
+        cfg.update(cfg_over)
+    cam = xo.make_camera(scene.cameras[view])
+    ocfg = xo.make_config(cfg, fragile_rel=fragile_rel)
+    s = dict(means=scene.means, scales=scene.scales, quats=scene.quats, opacities=scene.opacities, sh=scene.sh)
+    proj = xo.project(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, ocfg, np.float32)
+    proj["ray_rec"] = xo.project_ray(s["means"], s["scales"], s["quats"], proj["tile_count"], cam, np.float32)
+    proj["pixel_rays_oracle"] = xo.pixel_info(cam, np.float32)
+    proj["pixel_rays"] = proj["pixel_rays_oracle"] if pixel_rays is None else np.ascontiguousarray(pixel_rays, np.float32)
+    binned = xo.bin_sort(proj, cam, ocfg)
+    fwd = xo.rasterize_ray_fwd(proj, binned, cam, ocfg, np.float32)
+    return dict(proj=proj, binned=binned, fwd=fwd, cam=cam, cfg=ocfg, arrays=s)
 
 
 def compare_projection(g, o):

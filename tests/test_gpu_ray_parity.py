@@ -1,0 +1,131 @@
+"""GPU parity of the XPR-3DGUT evaluation: xpr_pixel_info, xpr_project_ray,
+xpr_rasterize_ray_fwd / _bwd and xpr_ray_bwd against the CPU oracle (oracle/xpr_oracle_ray.inc), element by
+element on the same seeded inputs, with the bars of test_gpu_parity.py:
+  pixel rays      <= 1 fp32 ulp of 1 (fp64 sin / cos of two libraries, rounded to fp32; rule R2), then the GPU's rays
+                  are handed to the oracle (stage isolation, as for every other stage)
+  shader record   bit-exact (rule R1)
+  lists           bit-exact;  image <= 1e-4 outside fragile pixels;  n_contrib equal there
+  record / opacity / colour gradients  1e-3 |ref| + 1e-6 + 2e-6 mass, every element
+  parameter gradients, stage-isolated  1e-3 |ref| + 1e-6 (+ the fp32 rounding of the accumulation into
+                  xpr_project_bwd's outputs), end to end reported and bounded group-relative.
+"""
+import numpy as np
+import pytest
+
+import parity_util as pu
+import xpr_oracle as xo
+from paper_2606_11529_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+PARAMS = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
+
+
+def ray_parity(scene, view=0, cfg_over=None):
+    over = dict(cfg_over or {}, ray_eval=1)
+    g = pu.run_gpu(scene, view, over)
+    o = pu.run_oracle_ray(scene, view, over, pixel_rays=g["proj"]["pixel_rays"])
+    vis = pu.compare_projection(g, o)
+    # pixel_info: unit vectors, within one ulp of the oracle's
+    dr = np.abs(g["proj"]["pixel_rays"].astype(np.float64) - o["proj"]["pixel_rays_oracle"].astype(np.float64))
+    assert dr.max() <= 1.2e-7, dr.max()
+    assert (dr > 0).mean() <= 1e-4, (dr > 0).mean()
+    # shader record
+    np.testing.assert_array_equal(g["proj"]["ray_rec"][vis].view(np.uint32), o["proj"]["ray_rec"][vis].view(np.uint32))
+    assert not np.any(g["proj"]["ray_rec"][~vis])
+    pu.compare_binning(g, o)
+    n_frag, _ = pu.compare_forward(g, o)
+    npix = o["fwd"]["image"].shape[0] * o["fwd"]["image"].shape[1]
+    assert n_frag <= max(2, 1e-3 * npix), f"{n_frag} fragile pixels"
+    assert o["fwd"]["pp_pass"] > 0
+    _, dL = scenes.loss_and_grad(scene.loss, o["fwd"]["image"], scene.target(view))
+    frag = (o["fwd"]["fragile"] & (pu.FRAG_EXIT | pu.FRAG_CLAMP)) != 0
+    dL = np.where(frag[..., None], 0.0, dL).astype(np.float32)
+    og = xo.backward_ray(o["arrays"], o, dL, o["cam"], o["cfg"], np.float32)
+    gg = pu.run_gpu_backward(g, dL)
+    mass = xo.rasterize_ray_bwd(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32, mass=True)
+    n_plain = 0
+    for kg, ko in (("g_ray_rec", "g_ray_rec"), ("g_opac", "g_opac_eff"), ("g_rgb", "g_rgb")):   # stage 1
+        bad, err = pu.grad_violations(gg[kg], og[ko], mass[ko])
+        assert bad.sum() == 0, f"{kg}: {bad.sum()} of {bad.size} outside tolerance, max err {err.max()}"
+        n_plain += int(pu.grad_violations(gg[kg], og[ko])[0].sum())
+    assert n_plain <= max(4, 2e-4 * 16 * scene.N), n_plain
+    assert not np.any(gg["g_mean2d"]) and not np.any(gg["g_conic"])      # the footprint carries no gradient
+    # stage 2: the oracle's chain rule fed the GPU's fp32 gradients
+    N = scene.N
+    gz = dict(g_mean2d=np.zeros((N, 2)), g_conic=np.zeros((N, 3)), g_opac_eff=gg["g_opac"], g_rgb=gg["g_rgb"])
+    iso = xo.project_bwd(scene.means, scene.scales, scene.quats, scene.opacities, scene.sh, o["cam"], o["cfg"], gz,
+                         np.float32)
+    part = xo.ray_bwd(scene.means, scene.scales, scene.quats, o["proj"]["tile_count"], gg["g_ray_rec"], o["cam"],
+                      np.float32)
+    total_bad = total = 0
+    for k in PARAMS:
+        ref = iso[k] + part[k] if k in part else iso[k]
+        got, ref = np.asarray(gg[k], np.float64).ravel(), np.asarray(ref, np.float64).ravel()
+        tol = pu.GRAD_RTOL * np.abs(ref) + pu.GRAD_ATOL
+        if k in part:   # fp32 accumulation of the two parts: one rounding of each part
+            tol = tol + 2.4e-7 * (np.abs(iso[k]).ravel() + np.abs(part[k]).ravel())
+        bad = np.abs(got - ref) > tol
+        assert bad.sum() == 0, f"{k} (stage-isolated): {bad.sum()} of {bad.size}, max err {np.abs(got - ref).max()}"
+        bad_e2e, err_e2e = pu.grad_violations(gg[k], og[k])
+        total_bad += int(bad_e2e.sum()); total += bad_e2e.size
+        if bad_e2e.any():
+            r2 = np.asarray(og[k], np.float64).reshape(N, -1)
+            group = np.abs(r2).max(axis=1, keepdims=True) * np.ones_like(r2)
+            assert (err_e2e[bad_e2e] <= 2e-2 * group.ravel()[bad_e2e] + 1e-6).all(), k
+    assert total_bad <= 1e-3 * total, f"end-to-end violators {total_bad}/{total}"
+    culled = o["proj"]["tile_count"] == 0
+    for k in PARAMS + ("g_ray_rec",):
+        assert not np.any(gg[k][culled])
+    return g, o
+
+
+@pytest.mark.parametrize("view", [0, 1])
+def test_ray_config4_ut_fisheye_reduced(view):
+    ray_parity(scenes.make_scene(4, n_override=30000, image_override=(480, 270)), view)
+
+
+def test_ray_config4_with_tile_cull_reduced():
+    ray_parity(scenes.make_scene(4, n_override=30000, image_override=(480, 270)), 0, dict(tile_cull=1))
+
+
+def test_ray_pinhole_ewa_footprint_and_background():
+    # the evaluation does not depend on how the footprint was made: EWA tiling, pinhole rays, non-zero background
+    ray_parity(scenes.make_scene(3, n_override=20000, image_override=(250, 130)), 1, dict(bg=(0.2, 0.4, 0.1)))
+
+
+def test_ray_config1_tiny_and_ragged():
+    ray_parity(scenes.make_scene(1), 0)
+    ray_parity(scenes.make_scene(2, n_override=5000, image_override=(70, 50)), 0)
+
+
+@pytest.mark.parametrize("view", [0, 1])
+def test_ray_config4_full_size(view):
+    ray_parity(scenes.make_scene(4), view, dict(tile_cull=1))
+
+
+def test_ray_stats_match_oracle_counters():
+    import torch
+    from paper_2606_11529_b200 import binding as xb
+    sc = scenes.make_scene(4, n_override=30000, image_override=(480, 270))
+    g = pu.run_gpu(sc, 0, dict(ray_eval=1))
+    o = pu.run_oracle_ray(sc, 0, dict(ray_eval=1), pixel_rays=g["proj"]["pixel_rays"])
+    p = g["pipe"]
+    stats = torch.zeros(4, dtype=torch.int64, device=p.device)
+    xb.xpr_rasterize_ray_stats(p.cam, p.cfg, p.ray_rec, p.conic_opac, p.rgb, p.lnv, p.pixel_rays, p.vals_sorted,
+                               p.tile_ranges, stats)
+    visited, passed, blended, sum_n = stats.tolist()
+    frag = int((o["fwd"]["fragile"] != 0).sum())
+    assert abs(visited - o["fwd"]["pp_visit"]) <= 64 * frag and abs(passed - o["fwd"]["pp_pass"]) <= 64 * frag
+    assert blended <= passed <= visited and sum_n == int(p.n_contrib.sum().item())
+
+
+def test_ray_degenerate_record_is_never_valid():
+    # a zero scale makes M_c infinite: the record is replaced by zeros and the Gaussian contributes nothing (C30)
+    import copy
+    sc = copy.deepcopy(scenes.make_scene(1))
+    sc.scales[:5] = 0.0
+    g, o = ray_parity(sc, 0)
+    vis = o["proj"]["tile_count"] > 0
+    assert vis[:5].any()
+    assert not np.any(g["proj"]["ray_rec"][:5])
