@@ -43,6 +43,9 @@ def parse():
     ap.add_argument("--tile-cull", type=int, default=1, choices=(0, 1),
                     help="1: binning with the paper's tile_cull (XPR-3DGS, PAPER L149/L268-281; same image); "
                          "0: rectangle overlap only")
+    ap.add_argument("--ray-eval", type=int, default=0, choices=(0, 1),
+                    help="1: XPR-3DGUT evaluation along the pixel ray (SURVEY 8(f) f2; meant for --config 4) instead of "
+                         "the 2D conic of north_star")
     ap.add_argument("--stages", action="store_true", help="also print per-stage times to stderr")
     return ap.parse_args()
 
@@ -110,15 +113,16 @@ def aggregate_value(world: int, megapixels: float, ms_per_step: float) -> float:
     return world * megapixels / (ms_per_step / 1e3)
 
 
-def oracle_step(xo, scenes, sc, view, np, tile_cull=0):
+def oracle_step(xo, scenes, sc, view, np, tile_cull=0, ray_eval=0):
     """One fwd+bwd step of the CPU oracle, as it stands (never tuned)."""
     cam = xo.make_camera(sc.cameras[view])
     cfg = xo.make_config(dict(scenes.default_render_config(sc), tile_cull=tile_cull))
     arrays = dict(means=sc.means, scales=sc.scales, quats=sc.quats, opacities=sc.opacities, sh=sc.sh)
+    render, backward = (xo.render_ray, xo.backward_ray) if ray_eval else (xo.render, xo.backward)
     t0 = time.perf_counter()
-    r = xo.render(arrays, cam, cfg, np.float32)
+    r = render(arrays, cam, cfg, np.float32)
     _, dL = scenes.loss_and_grad(sc.loss, r["fwd"]["image"], sc.target(view))
-    xo.backward(arrays, r, dL, cam, cfg, np.float32)
+    backward(arrays, r, dL, cam, cfg, np.float32)
     return time.perf_counter() - t0, r["binned"]["num_pairs"]
 
 
@@ -148,10 +152,10 @@ def run_reference(args):
     from paper_2606_11529_b200 import scenes
     sc, w, h, desc = oracle_sample(args)
     for _ in range(args.warmup):
-        oracle_step(xo, scenes, sc, args.view, np, args.tile_cull)
+        oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval)
     t = 0.0
     for _ in range(args.steps):
-        dt, I = oracle_step(xo, scenes, sc, args.view, np, args.tile_cull)
+        dt, I = oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval)
         t += dt
     ms = 1e3 * t / max(args.steps, 1)
     val = (w * h / 1e6) / (ms / 1e3)
@@ -159,7 +163,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config], "view": args.view, "tile_cull": args.tile_cull, "sample": desc,
+            "config": {"workload": WORKLOADS[args.config], "view": args.view, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "sample": desc,
                        "pairs": int(I)},
             "gaussians_per_s": sc.N / (ms / 1e3),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
@@ -171,6 +175,9 @@ def run_reference(args):
 # algorithmic work per unit: FP32 lane-ops per pixel-pair
 FWD_OPS_VISIT, FWD_OPS_PASS = 8, 9
 BWD_OPS_VISIT, BWD_OPS_PASS = 8, 45
+# f2 (ray evaluation): d_c 9 + cross 6 + two squared norms 6 + 1 + two thresholds and compares 4
+RAY_FWD_OPS_VISIT, RAY_FWD_OPS_PASS = 26, 12
+RAY_BWD_OPS_VISIT, RAY_BWD_OPS_PASS = 26, 57
 SMS, LANES_PER_SM = 148, 128
 
 
@@ -191,7 +198,7 @@ def run_ours(args):
 
     sc = scenes.make_scene(args.config)
     cam = sc.cameras[args.view]
-    cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull)
+    cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval)
     params = pipeline.scene_to_device(sc, dev)
     target = torch.from_numpy(sc.target(args.view)).to(dev)
     pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
@@ -210,6 +217,8 @@ def run_ours(args):
         checked against the capacity after the timed region."""
         ev = (lambda: None) if events is None else (lambda: events.append(_rec()))
         ev(); pipe.project(*params)
+        if args.ray_eval:                   # pixel_info and the shader record belong to the projection stage
+            pipe.pixel_info(); pipe.project_ray()
         ev(); pipe.bin_sort() if sync_count else pipe.bin_sort_async()
         ev(); pipe.rasterize_fwd()
         ev(); dL = loss_grad(pipe.image)
@@ -239,6 +248,8 @@ def run_ours(args):
     # project, bin_sort (compact, 4 depth passes, row scan, rows, pair scan, emit, tile passes, ranges), fwd, bwd,
     # project_bwd
     launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1
+    if args.ray_eval:
+        launches_per_step += 3              # pixel_info, project_ray, ray_bwd
     n_rows = pipe.rows_on_device()
     n_vis = int(torch.count_nonzero(pipe.tile_count).item())
 
@@ -262,8 +273,15 @@ def run_ours(args):
 
     # roofline of the dominant kernel (largest stage): pixel-pair counts from xpr_rasterize_stats
     stats = torch.zeros(4, dtype=torch.int64, device=dev)
-    xb.xpr_rasterize_stats(pipe.cam, pipe.cfg, pipe.mean2d, pipe.conic_opac, pipe.rgb, pipe.lnv, pipe.vals_sorted,
-                           pipe.tile_ranges, stats)
+    if args.ray_eval:
+        xb.xpr_rasterize_ray_stats(pipe.cam, pipe.cfg, pipe.ray_rec, pipe.conic_opac, pipe.rgb, pipe.lnv,
+                                   pipe.pixel_rays, pipe.vals_sorted, pipe.tile_ranges, stats)
+    else:
+        xb.xpr_rasterize_stats(pipe.cam, pipe.cfg, pipe.mean2d, pipe.conic_opac, pipe.rgb, pipe.lnv, pipe.vals_sorted,
+                               pipe.tile_ranges, stats)
+    fwd_ops = (RAY_FWD_OPS_VISIT, RAY_FWD_OPS_PASS) if args.ray_eval else (FWD_OPS_VISIT, FWD_OPS_PASS)
+    bwd_ops = (RAY_BWD_OPS_VISIT, RAY_BWD_OPS_PASS) if args.ray_eval else (BWD_OPS_VISIT, BWD_OPS_PASS)
+    kname = "rasterize_ray_%s_kernel" if args.ray_eval else "rasterize_%s_kernel"
     visit, passed, blended, sum_n = [int(v) for v in stats.cpu().tolist()]
     peaks = {}
     try:
@@ -280,17 +298,17 @@ def run_ours(args):
     sort_bytes = (8 * sc.N + (4 * 16 + 20) * n_vis + 36 * n_rows
                   + n_pairs * (8 + 16 * (tile_passes - 1) + 20))
     rooflines = {
-        "rasterize_fwd": {"kernel": "rasterize_fwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
-                          "achieved": (FWD_OPS_VISIT * visit + FWD_OPS_PASS * passed) / sec("rasterize_fwd") / 1e12},
-        "rasterize_bwd": {"kernel": "rasterize_bwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
-                          "achieved": (BWD_OPS_VISIT * sum_n + BWD_OPS_PASS * blended) / sec("rasterize_bwd") / 1e12},
+        "rasterize_fwd": {"kernel": kname % "fwd", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
+                          "achieved": (fwd_ops[0] * visit + fwd_ops[1] * passed) / sec("rasterize_fwd") / 1e12},
+        "rasterize_bwd": {"kernel": kname % "bwd", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
+                          "achieved": (bwd_ops[0] * sum_n + bwd_ops[1] * blended) / sec("rasterize_bwd") / 1e12},
         "bin_sort": {"kernel": "xpr_bin_sort%s (compact, 4 depth passes on Gaussians, row scan, rows, pair scan, emit, "
                                "%d tile passes on pairs, ranges)" % ("_cull" if args.tile_cull else "", tile_passes), "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
                      "achieved": sort_bytes / sec("bin_sort") / 1e9, "algorithmic_bytes": sort_bytes},
     }
     traffic = {}
     try:   # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu --set full capture
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get("config%d" % args.config, {})
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get("config%d%s" % (args.config, "_ray" if args.ray_eval else ""), {})
     except Exception:
         pass
     for name, r in rooflines.items():
@@ -342,7 +360,10 @@ def run_ours(args):
         def e2e_step():
             for d, h in zip(dev_in, host_in):
                 d.copy_(h, non_blocking=True)
-            pipe.project(*dev_in); pipe.bin_sort_async(); pipe.rasterize_fwd()
+            pipe.project(*dev_in)
+            if args.ray_eval:
+                pipe.pixel_info(); pipe.project_ray()
+            pipe.bin_sort_async(); pipe.rasterize_fwd()
             pipe.rasterize_bwd(loss_grad(pipe.image)); pipe.project_bwd()
             for h, o in zip(host_out, outs):
                 h.copy_(o, non_blocking=True)
@@ -366,7 +387,7 @@ def run_ours(args):
         sys.path.insert(0, os.path.join(ROOT, "oracle"))
         import xpr_oracle as xo
         osc, w, h, desc = oracle_sample(args)
-        dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull)
+        dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull, args.ray_eval)
         cpu = {"value": (w * h / 1e6) / dt, "unit": UNIT, "cores": xo.num_threads(), "kind": "oracle", "sample": desc,
                "seconds": dt}
 
@@ -375,7 +396,7 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "pairs": n_pairs,
+                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "pairs": n_pairs,
                            "candidate_pairs": n_cand, "rows": n_rows, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "tile_digits_on_pairs": tile_passes},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",

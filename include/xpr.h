@@ -197,8 +197,8 @@ int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, cons
  *   nhq = -1/2 |o_c x d_c|^2, dd = |d_c|^2:  nhq > ln(0.0113) dd  and  nhq >= -lnv dd.
  *
  * xpr_pixel_info -- pixel_info of Listing 3: pixel_rays[H,W,3] = unit direction (camera frame) of the ray through
- *   the pixel centre (i+0.5, j+0.5), the inverse of the camera model (fisheye: 12 Newton steps on the radial
- *   polynomial); fp64 inside, rounded to fp32 last (rule R2).  Depends on the intrinsics only.
+ *   the pixel centre (i+0.5, j+0.5), the inverse of the camera model (fisheye: at most 12 Newton steps on the
+ *   radial polynomial); fp64 inside, rounded to fp32 last (rule R2).  Depends on the intrinsics only.
  * xpr_project_ray -- shader record p_sd: ray_rec[N,12] = M_c row-major (9), o_c (3); zeros for a culled Gaussian
  *   (tile_count == 0) and for a record that is not finite (C30).  fp32, rule R1.
  * xpr_rasterize_ray_fwd / _bwd -- xpr_rasterize_fwd / _bwd with this evaluation; opacity o_eff is read from

@@ -50,96 +50,142 @@ __device__ __forceinline__ RayEval eval_ray(const float4 r0, const float4 r1, co
     return e;
 }
 
-// Forward (a8 with the f2 evaluation).  One CTA per tile, one thread per pixel; record of a list entry in shared
-// memory: 5 x float4 = (M_c, o_c | thr = -lnv, log2 o, r, g | b).  STATS as in rasterize.cu.
+// Forward (a8 with the f2 evaluation).  One CTA per tile in the two shapes of rasterize.cu: PPT = 2 (128 threads, a
+// thread owns the pixels (x, y) and (x + 8, y): the shared-memory reads of a list entry are paid once per two
+// pixels) for large images, PPT = 1 (256 threads) where the heaviest tile bounds the kernel.  Record of a list
+// entry in shared memory: 5 x float4 = (M_c, o_c | thr = -lnv, log2 o, r, g | b).  STATS as in rasterize.cu.
+struct RayPix {
+    float d0, d1, d2, T, C0, C1, C2;
+    uint32_t last;
+    bool act;
+};
+
 template <bool STATS>
-__global__ void __launch_bounds__(BLOCK)
+__device__ __forceinline__ void ray_blend(RayPix& p, float nhq, float dd, const float4* __restrict__ rec, uint32_t pos,
+                                          float lnr, float amax, float tmin, uint32_t& n_visit, uint32_t& n_pass,
+                                          uint32_t& n_blend) {
+    if (!p.act) return;
+    if (STATS) ++n_visit;
+    const float4 at = rec[3];
+    const float tv = __fmul_rn(lnr, dd), tg = __fmul_rn(at.x, dd);
+    if ((nhq > tv) && !(nhq < tg)) {                      // valid (L500) and alpha >= alpha_thresh (C12)
+        if (STATS) ++n_pass;
+        const float power = nhq * rcp_approx(dd);
+        const float alpha = fminf(amax, ex2_approx(fmaf(power, 1.4426950408889634f, at.y)));   // C11
+        const float Tn = p.T * (1.0f - alpha);
+        if (Tn < tmin) {                                  // C12: stop, no blend
+            p.act = false;
+        } else {
+            const float w = alpha * p.T;
+            p.C0 = fmaf(at.z, w, p.C0); p.C1 = fmaf(at.w, w, p.C1); p.C2 = fmaf(rec[4].x, w, p.C2);
+            p.T = Tn;
+            p.last = pos;
+            if (STATS) ++n_blend;
+        }
+    }
+}
+
+#ifndef XPR_RAY_FWD_PPT2_MIN_TILES
+#define XPR_RAY_FWD_PPT2_MIN_TILES 4096
+#endif
+
+template <bool STATS, int PPT>
+__global__ void __launch_bounds__(BLOCK / PPT)
 rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, const float4* __restrict__ conic_opac,
                          const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ rays,
                          const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                          float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
                          unsigned long long* __restrict__ stats) {
-    __shared__ float4 s_geo[3 * BLOCK];
-    __shared__ float4 s_att[BLOCK];      // thr, log2 o, r, g
-    __shared__ float s_blue[BLOCK];
+    constexpr int THREADS = BLOCK / PPT, BATCH = THREADS, ROW = TILE / PPT;
+    __shared__ float4 s_rec[5 * BATCH];
     const int tile = blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
-    const int px = tx * TILE + (threadIdx.x % TILE), py = ty * TILE + (threadIdx.x / TILE);
-    const bool inside = (px < P.W) && (py < P.H);
-    const int64_t pid = (int64_t)py * P.W + px;
-    float d0 = 0.f, d1 = 0.f, d2 = 1.f;
-    if (inside) { d0 = rays[3 * pid]; d1 = rays[3 * pid + 1]; d2 = rays[3 * pid + 2]; }
+    const int py = ty * TILE + (threadIdx.x / ROW);
+    int px[PPT];
+    bool inside[PPT];
+    RayPix pix[PPT];
+    bool any_act = false;
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+        px[k] = tx * TILE + (threadIdx.x % ROW) + 8 * k;
+        inside[k] = (px[k] < P.W) && (py < P.H);
+        pix[k].d0 = 0.f; pix[k].d1 = 0.f; pix[k].d2 = 1.f;
+        if (inside[k]) {
+            const int64_t pid = (int64_t)py * P.W + px[k];
+            pix[k].d0 = rays[3 * pid]; pix[k].d1 = rays[3 * pid + 1]; pix[k].d2 = rays[3 * pid + 2];
+        }
+        pix[k].T = 1.0f; pix[k].C0 = pix[k].C1 = pix[k].C2 = 0.0f; pix[k].last = 0; pix[k].act = inside[k];
+        any_act |= inside[k];
+    }
     const uint2 rg = ranges[tile];
     const uint32_t len = rg.y - rg.x;
     const float amax = P.amax, tmin = P.tmin, lnr = P.lnr;
-
-    float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
-    uint32_t last = 0;
-    bool act = inside;
     uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
 
-    for (uint32_t base = 0; base < len; base += BLOCK) {
-        if (__syncthreads_or(act) == 0) break;
-        const uint32_t cnt = min((uint32_t)BLOCK, len - base);
+    for (uint32_t base = 0; base < len; base += BATCH) {
+        if (__syncthreads_or(any_act) == 0) break;
+        const uint32_t cnt = min((uint32_t)BATCH, len - base);
         if (threadIdx.x < cnt) {
             const uint32_t g = vals[rg.x + base + threadIdx.x];
-            s_geo[3 * threadIdx.x] = ray_rec[3 * (size_t)g];
-            s_geo[3 * threadIdx.x + 1] = ray_rec[3 * (size_t)g + 1];
-            s_geo[3 * threadIdx.x + 2] = ray_rec[3 * (size_t)g + 2];
-            s_att[threadIdx.x] = make_float4(-lnv[g], __log2f(conic_opac[g].w), rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1]);
-            s_blue[threadIdx.x] = rgb[3 * (size_t)g + 2];
+            float4* rec = s_rec + 5 * threadIdx.x;
+            rec[0] = ray_rec[3 * (size_t)g]; rec[1] = ray_rec[3 * (size_t)g + 1]; rec[2] = ray_rec[3 * (size_t)g + 2];
+            rec[3] = make_float4(-lnv[g], __log2f(conic_opac[g].w), rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1]);
+            rec[4] = make_float4(rgb[3 * (size_t)g + 2], 0.f, 0.f, 0.f);
         }
         __syncthreads();
-        if (act) {
-            // groups of 4: the evaluations are independent of the transmittance, so their latencies overlap;
-            // the sequential part (gates, alpha, T' = T (1 - alpha), exit test, blend) follows
-            for (uint32_t j0 = 0; j0 < cnt && act; j0 += 4) {
-                float nhq[4], dd[4];
+        if (any_act) {
+            // groups of 4: the evaluations are independent of the transmittance, so their latencies overlap; the
+            // sequential part (gates, alpha, T' = T (1 - alpha), exit test, blend) follows
+            const float4* rq = s_rec;
+            uint32_t j = 0;
+            for (; j + 4 <= cnt && any_act; j += 4, rq += 20) {
+                float nhq[4][PPT], dd[4][PPT];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const uint32_t j = min(j0 + u, cnt - 1);
-                    const RayEval e = eval_ray(s_geo[3 * j], s_geo[3 * j + 1], s_geo[3 * j + 2], d0, d1, d2);
-                    nhq[u] = e.nhq; dd[u] = e.dd;
-                }
+                    const float4 r0 = rq[5 * u], r1 = rq[5 * u + 1], r2 = rq[5 * u + 2];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const uint32_t j = j0 + u;
-                    if (j < cnt && act) {
-                        if (STATS) ++n_visit;
-                        const float4 at = s_att[j];
-                        const float tv = __fmul_rn(lnr, dd[u]), tg = __fmul_rn(at.x, dd[u]);
-                        if ((nhq[u] > tv) && !(nhq[u] < tg)) {            // valid (L500) and alpha >= alpha_thresh (C12)
-                            if (STATS) ++n_pass;
-                            const float power = nhq[u] * rcp_approx(dd[u]);
-                            const float alpha = fminf(amax, ex2_approx(fmaf(power, 1.4426950408889634f, at.y)));   // C11
-                            const float Tn = T * (1.0f - alpha);
-                            if (Tn < tmin) {                              // C12: stop, no blend
-                                act = false;
-                            } else {
-                                const float w = alpha * T;
-                                C0 = fmaf(at.z, w, C0); C1 = fmaf(at.w, w, C1); C2 = fmaf(s_blue[j], w, C2);
-                                T = Tn;
-                                last = base + j + 1;
-                                if (STATS) ++n_blend;
-                            }
-                        }
+                    for (int k = 0; k < PPT; ++k) {
+                        const RayEval e = eval_ray(r0, r1, r2, pix[k].d0, pix[k].d1, pix[k].d2);
+                        nhq[u][k] = e.nhq; dd[u][k] = e.dd;
                     }
                 }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int k = 0; k < PPT; ++k)
+                        ray_blend<STATS>(pix[k], nhq[u][k], dd[u][k], rq + 5 * u, base + j + u + 1, lnr, amax, tmin,
+                                         n_visit, n_pass, n_blend);
+                any_act = pix[0].act || (PPT == 2 && pix[PPT - 1].act);
+            }
+            for (; j < cnt && any_act; ++j, rq += 5) {
+                const float4 r0 = rq[0], r1 = rq[1], r2 = rq[2];
+#pragma unroll
+                for (int k = 0; k < PPT; ++k) {
+                    const RayEval e = eval_ray(r0, r1, r2, pix[k].d0, pix[k].d1, pix[k].d2);
+                    ray_blend<STATS>(pix[k], e.nhq, e.dd, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
+                }
+                any_act = pix[0].act || (PPT == 2 && pix[PPT - 1].act);
             }
         }
     }
     if (STATS) {
+        uint32_t sum_last = 0;
+#pragma unroll
+        for (int k = 0; k < PPT; ++k) sum_last += pix[k].last;
         atomicAdd(stats + 0, (unsigned long long)n_visit); atomicAdd(stats + 1, (unsigned long long)n_pass);
-        atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)last);
+        atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)sum_last);
         return;
     }
-    if (inside) {
-        image[3 * pid] = fmaf(T, P.bg[0], C0);
-        image[3 * pid + 1] = fmaf(T, P.bg[1], C1);
-        image[3 * pid + 2] = fmaf(T, P.bg[2], C2);
-        final_T[pid] = T;
-        n_contrib[pid] = last;
-    }
+#pragma unroll
+    for (int k = 0; k < PPT; ++k)
+        if (inside[k]) {
+            const int64_t pid = (int64_t)py * P.W + px[k];
+            image[3 * pid] = fmaf(pix[k].T, P.bg[0], pix[k].C0);
+            image[3 * pid + 1] = fmaf(pix[k].T, P.bg[1], pix[k].C1);
+            image[3 * pid + 2] = fmaf(pix[k].T, P.bg[2], pix[k].C2);
+            final_T[pid] = pix[k].T;
+            n_contrib[pid] = pix[k].last;
+        }
 }
 
 // Transposed butterfly (see rasterize.cu): 8 per-lane values -> lane L with (L & 3) == 0 holds the total of value L >> 2.
@@ -169,10 +215,13 @@ __device__ __forceinline__ float warp_reduce8(const float* v, int lane) {
 //   dL/dc = -(g_p/dd) c,  dL/ddd = -g_p power/dd,  dL/dd_c = dL/dc x o_c + 2 dL/ddd d_c,  dL/do_c = d_c x dL/dc,
 //   dL/dM_c = dL/dd_c d^T.
 #ifndef XPR_RAY_BWD_PPT
-#define XPR_RAY_BWD_PPT 2
+#define XPR_RAY_BWD_PPT 4
+#endif
+#ifndef XPR_RAY_BWD_MINB
+#define XPR_RAY_BWD_MINB 6
 #endif
 template <int PPT>
-__global__ void __launch_bounds__(BLOCK / PPT)
+__global__ void __launch_bounds__(BLOCK / PPT, XPR_RAY_BWD_MINB * PPT / 4)
 rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, const float4* __restrict__ conic_opac,
                          const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ rays,
                          const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
@@ -337,9 +386,15 @@ extern "C" int32_t xpr_rasterize_ray_fwd(const xpr_camera* cam, const xpr_config
     RayRasterParams P;
     make_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
-    rasterize_ray_fwd_kernel<false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
-        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays,
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    // throughput shape once the image has enough tiles for several waves of every SM
+    if (T >= XPR_RAY_FWD_PPT2_MIN_TILES)
+        rasterize_ray_fwd_kernel<false, 2><<<T, BLOCK / 2, 0, (cudaStream_t)stream>>>(
+            P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+            pixel_rays, vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    else
+        rasterize_ray_fwd_kernel<false, 1><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+            P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
+            pixel_rays, vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }
@@ -357,7 +412,7 @@ extern "C" int32_t xpr_rasterize_ray_stats(const xpr_camera* cam, const xpr_conf
     make_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
     XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
-    rasterize_ray_fwd_kernel<true><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+    rasterize_ray_fwd_kernel<true, 1><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
         P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays,
         vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr, nullptr, nullptr,
         reinterpret_cast<unsigned long long*>(stats));
@@ -389,10 +444,15 @@ extern "C" int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config
     RayRasterParams P;
     make_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
-    rasterize_ray_bwd_kernel<XPR_RAY_BWD_PPT><<<T, BLOCK / XPR_RAY_BWD_PPT, 0, st>>>(
-        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays,
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_ray_rec, g_opac,
-        g_rgb);
+#define XPR_RAY_BWD(PPT_)                                                                                           \
+    rasterize_ray_bwd_kernel<PPT_><<<T, BLOCK / PPT_, 0, st>>>(                                                     \
+        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays, \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_ray_rec, g_opac,  \
+        g_rgb)
+    // more pixels per thread amortise the per-entry reduction (throughput shape); fewer give a heavy tile more warps
+    if (T >= XPR_RAY_FWD_PPT2_MIN_TILES) XPR_RAY_BWD(XPR_RAY_BWD_PPT);
+    else                                 XPR_RAY_BWD(2);
+#undef XPR_RAY_BWD
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }

@@ -42,15 +42,18 @@ __global__ void __launch_bounds__(256) pixel_info_kernel(RayCam C, float* __rest
     } else {
         const double rd = sqrt(xn * xn + yn * yn);
         if (rd > 0.0) {
-            double th = rd;   // theta (1 + k1 th^2 + k2 th^4 + k3 th^6 + k4 th^8) = rd, 12 Newton steps
+            double th = rd;   // theta (1 + k1 th^2 + k2 th^4 + k3 th^6 + k4 th^8) = rd, <= 12 Newton steps
             for (int it = 0; it < 12; ++it) {
                 const double t2 = th * th;
                 const double f = th * (1.0 + t2 * (C.k[0] + t2 * (C.k[1] + t2 * (C.k[2] + t2 * C.k[3])))) - rd;
+                if (!(fabs(f) > 4e-16 * rd)) break;               // converged to fp64 rounding
                 const double fp = 1.0 + t2 * (3.0 * C.k[0] + t2 * (5.0 * C.k[1] + t2 * (7.0 * C.k[2] + t2 * (9.0 * C.k[3]))));
                 th = th - f / fp;
             }
-            const double s = sin(th) / rd;
-            dx = s * xn; dy = s * yn; dz = cos(th);
+            double sn, cs;
+            sincos(th, &sn, &cs);
+            const double s = sn / rd;
+            dx = s * xn; dy = s * yn; dz = cs;
         } else { dx = 0.0; dy = 0.0; dz = 1.0; }
     }
     rays[3 * pid] = (float)dx; rays[3 * pid + 1] = (float)dy; rays[3 * pid + 2] = (float)dz;
