@@ -57,14 +57,13 @@ __device__ __forceinline__ RayEval eval_ray(const float4 r0, const float4 r1, co
 struct RayPix {
     float d0, d1, d2, T, C0, C1, C2;
     uint32_t last;
-    bool act;
 };
 
 template <bool STATS>
-__device__ __forceinline__ void ray_blend(RayPix& p, float nhq, float dd, const float4* __restrict__ rec, uint32_t pos,
+__device__ __forceinline__ void ray_blend(RayPix& p, int& act, float nhq, float dd, const float4* __restrict__ rec, uint32_t pos,
                                           float lnr, float amax, float tmin, uint32_t& n_visit, uint32_t& n_pass,
                                           uint32_t& n_blend) {
-    if (!p.act) return;
+    if (!act) return;
     if (STATS) ++n_visit;
     const float4 at = rec[3];
     const float tv = __fmul_rn(lnr, dd), tg = __fmul_rn(at.x, dd);
@@ -74,7 +73,7 @@ __device__ __forceinline__ void ray_blend(RayPix& p, float nhq, float dd, const 
         const float alpha = fminf(amax, ex2_approx(fmaf(power, 1.4426950408889634f, at.y)));   // C11
         const float Tn = p.T * (1.0f - alpha);
         if (Tn < tmin) {                                  // C12: stop, no blend
-            p.act = false;
+            act = 0;
         } else {
             const float w = alpha * p.T;
             p.C0 = fmaf(at.z, w, p.C0); p.C1 = fmaf(at.w, w, p.C1); p.C2 = fmaf(rec[4].x, w, p.C2);
@@ -102,20 +101,21 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
     const int tx = tile % P.TW, ty = tile / P.TW;
     const int py = ty * TILE + (threadIdx.x / ROW);
     int px[PPT];
-    bool inside[PPT];
+    int inside[PPT];
     RayPix pix[PPT];
+    int act[PPT];
     bool any_act = false;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
         px[k] = tx * TILE + (threadIdx.x % ROW) + 8 * k;
-        inside[k] = (px[k] < P.W) && (py < P.H);
+        inside[k] = ((px[k] < P.W) && (py < P.H)) ? 1 : 0;
         pix[k].d0 = 0.f; pix[k].d1 = 0.f; pix[k].d2 = 1.f;
         if (inside[k]) {
             const int64_t pid = (int64_t)py * P.W + px[k];
             pix[k].d0 = rays[3 * pid]; pix[k].d1 = rays[3 * pid + 1]; pix[k].d2 = rays[3 * pid + 2];
         }
-        pix[k].T = 1.0f; pix[k].C0 = pix[k].C1 = pix[k].C2 = 0.0f; pix[k].last = 0; pix[k].act = inside[k];
-        any_act |= inside[k];
+        pix[k].T = 1.0f; pix[k].C0 = pix[k].C1 = pix[k].C2 = 0.0f; pix[k].last = 0; act[k] = inside[k] ? 1 : 0;
+        any_act |= (inside[k] != 0);
     }
     const uint2 rg = ranges[tile];
     const uint32_t len = rg.y - rg.x;
@@ -153,18 +153,18 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                 for (int u = 0; u < 4; ++u)
 #pragma unroll
                     for (int k = 0; k < PPT; ++k)
-                        ray_blend<STATS>(pix[k], nhq[u][k], dd[u][k], rq + 5 * u, base + j + u + 1, lnr, amax, tmin,
+                        ray_blend<STATS>(pix[k], act[k], nhq[u][k], dd[u][k], rq + 5 * u, base + j + u + 1, lnr, amax, tmin,
                                          n_visit, n_pass, n_blend);
-                any_act = pix[0].act || (PPT == 2 && pix[PPT - 1].act);
+                any_act = (act[0] | act[PPT - 1]) != 0;
             }
             for (; j < cnt && any_act; ++j, rq += 5) {
                 const float4 r0 = rq[0], r1 = rq[1], r2 = rq[2];
 #pragma unroll
                 for (int k = 0; k < PPT; ++k) {
                     const RayEval e = eval_ray(r0, r1, r2, pix[k].d0, pix[k].d1, pix[k].d2);
-                    ray_blend<STATS>(pix[k], e.nhq, e.dd, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
+                    ray_blend<STATS>(pix[k], act[k], e.nhq, e.dd, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
                 }
-                any_act = pix[0].act || (PPT == 2 && pix[PPT - 1].act);
+                any_act = (act[0] | act[PPT - 1]) != 0;
             }
         }
     }

@@ -85,6 +85,28 @@ def test_invalid_arguments_rejected_before_launch(lib):
     assert st == xb.XPR_ERR_INVALID_ARG
 
 
+def test_ray_entry_points_reject_bad_arguments(lib):
+    cam, cfg = _cam_cfg()
+    null = C.c_void_p(0)
+    one = C.c_void_p(16)          # non-NULL, aligned; never dereferenced: the checks come first
+    odd = C.c_void_p(20)          # 4-byte aligned only
+    assert lib.xpr_pixel_info(None, one, null) == 1
+    assert lib.xpr_pixel_info(C.byref(cam), null, null) == 1
+    bad = type(cam)(); C.memmove(C.byref(bad), C.byref(cam), C.sizeof(cam)); bad.model = 7
+    assert lib.xpr_pixel_info(C.byref(bad), one, null) == 1
+    assert lib.xpr_project_ray(C.c_int64(-1), one, one, one, C.byref(cam), one, one, null) == 1
+    assert lib.xpr_project_ray(C.c_int64(0), null, null, null, C.byref(cam), null, null, null) == 0     # N = 0: nothing to do
+    assert lib.xpr_project_ray(C.c_int64(4), one, one, one, C.byref(cam), one, odd, null) == 1          # ray_rec needs 16 B
+    assert lib.xpr_rasterize_ray_fwd(C.byref(cam), C.byref(cfg), C.c_int64(4), null, one, one, one, one, one, one, one,
+                                     one, one, null) == 1
+    assert lib.xpr_rasterize_ray_bwd(C.byref(cam), C.byref(cfg), C.c_int64(4), one, one, one, one, one, one, one, one,
+                                     one, one, null, one, one, C.c_int32(1), null) == 1
+    assert lib.xpr_ray_bwd(C.c_int64(4), one, one, one, C.byref(cam), one, odd, one, one, one, null) == 1
+    cfg8 = type(cfg)(); C.memmove(C.byref(cfg8), C.byref(cfg), C.sizeof(cfg)); cfg8.tile = 8
+    assert lib.xpr_rasterize_ray_fwd(C.byref(cam), C.byref(cfg8), C.c_int64(0), null, null, null, null, one, null, one,
+                                     one, one, one, null) == 4
+
+
 def test_workspace_size_monotone(lib):
     from paper_2606_11529_b200 import binding as xb
     a = xb.xpr_bin_sort_workspace(1000, 10_000, 16)
