@@ -129,3 +129,42 @@ def test_ray_degenerate_record_is_never_valid():
     vis = o["proj"]["tile_count"] > 0
     assert vis[:5].any()
     assert not np.any(g["proj"]["ray_rec"][:5])
+
+
+def test_ray_empty_scene_and_everything_culled():
+    import torch
+    from paper_2606_11529_b200 import pipeline
+    sc = scenes.make_scene(1)
+    for name in ("means", "scales", "quats", "opacities", "sh"):
+        setattr(sc, name, getattr(sc, name)[:0].copy())
+    cfg = dict(scenes.default_render_config(sc), ray_eval=1, bg=(0.1, 0.2, 0.3))
+    pipe = pipeline.SplatPipeline(0, sc.cameras[0], cfg)
+    img = pipe.forward(*pipeline.scene_to_device(sc))
+    pipe.backward(torch.ones(64, 64, 3, device="cuda"))
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(img.cpu().numpy(), np.broadcast_to(np.float32([0.1, 0.2, 0.3]), (64, 64, 3)))
+    assert (pipe.final_T.cpu().numpy() == 1).all() and (pipe.n_contrib.cpu().numpy() == 0).all()
+    sc = scenes.make_scene(1, n_override=500)
+    sc.means[:, 2] -= 10.0          # all behind the camera
+    g = pu.run_gpu(sc, 0, dict(ray_eval=1))
+    assert g["binned"]["num_pairs"] == 0 and not np.any(g["proj"]["ray_rec"]) and (g["fwd"]["image"] == 0).all()
+    gg = pu.run_gpu_backward(g, np.ones((64, 64, 3), np.float32))
+    for k, v in gg.items():
+        assert not np.any(v), k
+
+
+@pytest.mark.parametrize("deg", [0, 2])
+def test_ray_sh_degrees_and_ragged(deg):
+    sc = scenes.make_scene(4, n_override=8000, image_override=(33, 17))
+    sc.sh = sc.sh[:, :(deg + 1) ** 2].copy()
+    sc.sh_degree = deg
+    ray_parity(sc, 0)
+
+
+def test_ray_pixel_rays_depend_on_the_intrinsics_only():
+    # the two poses of config 4 share their intrinsics: identical rays (reading C27)
+    sc = scenes.make_scene(4, n_override=100, image_override=(160, 90))
+    a = pu.run_gpu(sc, 0, dict(ray_eval=1))["proj"]["pixel_rays"]
+    b = pu.run_gpu(sc, 1, dict(ray_eval=1))["proj"]["pixel_rays"]
+    np.testing.assert_array_equal(a, b)
+    np.testing.assert_allclose(np.linalg.norm(a.astype(np.float64), axis=-1), 1.0, atol=2e-7)
