@@ -204,10 +204,12 @@ def run_ours(args):
     pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
+    dL_buf = torch.empty_like(target)
+
     def loss_grad(image):
-        if sc.loss == "l1":
-            return torch.sign(image - target)
-        return 2.0 * (image - target)
+        """dL/dimage of the config's loss (sum |I - target| or sum (I - target)^2), one pass (xpr_loss_grad)."""
+        xb.xpr_loss_grad(sc.loss, image, target, dL_buf)
+        return dL_buf
 
     stage_names = ("project", "bin_sort", "rasterize_fwd", "loss_grad", "rasterize_bwd", "project_bwd")
 
@@ -247,7 +249,7 @@ def run_ours(args):
     passes = 4 + tile_passes              # 8-bit digits: 4 on the depth bits (run on Gaussians) + tile digits (on pairs)
     # project, bin_sort (compact, 4 depth passes, row scan, rows, pair scan, emit, tile passes, ranges), fwd, bwd,
     # project_bwd
-    launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1
+    launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1 + 1      # + loss_grad
     if args.ray_eval:
         launches_per_step += 3              # pixel_info, project_ray, ray_bwd
     n_rows = pipe.rows_on_device()

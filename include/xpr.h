@@ -228,6 +228,15 @@ int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const fl
                     const xpr_camera* cam, const uint32_t* tile_count, const float* g_ray_rec,
                     float* g_means, float* g_scales, float* g_quats, void* stream);
 
+/*
+ * xpr_loss_grad -- convenience for the caller's side of the step (reading C21: the loss lives outside the path):
+ * dL/dimage of the two losses BASELINE.json's configs name, as sums over all n = H*W*3 values, in one pass:
+ *   kind 0: L = sum |I - target|    -> dL = sign(I - target);      kind 1: L = sum (I - target)^2 -> dL = 2 (I - target).
+ * image, target, dL_dimage: DEVICE fp32 [n], 16-byte aligned.
+ */
+int32_t xpr_loss_grad(int32_t kind, int64_t n, const float* image, const float* target, float* dL_dimage,
+                      void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,7 +20,7 @@ FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_R
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
            "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
-           "xpr_ray_bwd")
+           "xpr_ray_bwd", "xpr_loss_grad")
 
 
 class XprCamera(C.Structure):
@@ -235,3 +235,10 @@ def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_rec, g_m
     N = int(means.shape[0])
     _check(lib().xpr_ray_bwd(C.c_int64(N), _p(means), _p(scales), _p(quats), C.byref(cam), _p(tile_count),
                              _p(g_ray_rec), _p(g_means), _p(g_scales), _p(g_quats), _stream(stream)), "xpr_ray_bwd")
+
+
+def xpr_loss_grad(kind: str, image, target, dL_dimage, stream=None):
+    """kind: "l1" (sum of absolute differences) or "l2" (sum of squares); dL/dimage in one pass (xpr.h)."""
+    k = {"l1": 0, "l2": 1}[kind]
+    _check(lib().xpr_loss_grad(C.c_int32(k), C.c_int64(image.numel()), _p(image), _p(target), _p(dL_dimage),
+                               _stream(stream)), "xpr_loss_grad")

@@ -148,3 +148,20 @@ def test_more_than_65536_tiles_three_tile_digit_passes():
         n_frag, _ = pu.compare_forward(g, o)
         assert n_frag <= 1e-3 * 4112 * 4112
         assert int(g["binned"]["keys"].max() >> np.uint64(32)) > 65536
+
+
+@pytest.mark.parametrize("kind", ["l1", "l2"])
+def test_loss_grad_helper_matches_the_definition(kind):
+    import torch
+    from paper_2606_11529_b200 import binding as xb
+    rng = np.random.default_rng(3)
+    for n in (0, 3, 4, 4099, 64 * 64 * 3):
+        img = rng.normal(0.5, 0.3, n).astype(np.float32)
+        tgt = rng.normal(0.5, 0.3, n).astype(np.float32)
+        if n > 2:
+            tgt[1] = img[1]                      # exact zero difference
+        want = scenes.loss_and_grad(kind, img, tgt)[1]
+        out = torch.full((max(n, 1),), 7.0, device="cuda")[:n]
+        xb.xpr_loss_grad(kind, torch.from_numpy(img).cuda(), torch.from_numpy(tgt).cuda(), out)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(out.cpu().numpy().view(np.uint32), want.view(np.uint32))
