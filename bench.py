@@ -43,6 +43,9 @@ def parse():
     ap.add_argument("--tile-cull", type=int, default=1, choices=(0, 1),
                     help="1: binning with the paper's tile_cull (XPR-3DGS, PAPER L149/L268-281; same image); "
                          "0: rectangle overlap only")
+    ap.add_argument("--tile-order", type=int, default=-1, choices=(-1, 0, 1),
+                    help="1: compositing kernels walk the tiles longest list first (xpr_config.tile_order; scheduling "
+                         "only); -1: the pipeline's default (on for 64 <= tiles < 4096)")
     ap.add_argument("--ray-eval", type=int, default=0, choices=(0, 1),
                     help="1: XPR-3DGUT evaluation along the pixel ray (SURVEY 8(f) f2; meant for --config 4) instead of "
                          "the 2D conic of north_star")
@@ -198,7 +201,8 @@ def run_ours(args):
 
     sc = scenes.make_scene(args.config)
     cam = sc.cameras[args.view]
-    cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval)
+    cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval,
+               tile_order=args.tile_order)
     params = pipeline.scene_to_device(sc, dev)
     target = torch.from_numpy(sc.target(args.view)).to(dev)
     pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
@@ -252,6 +256,8 @@ def run_ours(args):
     launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1 + 1      # + loss_grad
     if args.ray_eval:
         launches_per_step += 3              # pixel_info, project_ray, ray_bwd
+    if pipe.tile_order is not None:
+        launches_per_step += 1              # tile_order_kernel at the end of xpr_bin_sort
     n_rows = pipe.rows_on_device()
     n_vis = int(torch.count_nonzero(pipe.tile_count).item())
 
@@ -398,7 +404,7 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "pairs": n_pairs,
+                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
                            "candidate_pairs": n_cand, "rows": n_rows, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "tile_digits_on_pairs": tile_passes},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",

@@ -58,6 +58,10 @@ typedef struct {
     float ut_alpha, ut_beta, ut_kappa;  /* unscented-transform weights: 1, 2, 0 */
     float bg[3];            /* background colour (C13) */
     int32_t tile_cull;      /* 1: xpr_bin_sort_cull drops (Gaussian, tile) pairs that fail tile_cull */
+    uint32_t* tile_order;   /* DEVICE uint32[T] or NULL.  Scheduling only, no effect on any result: when set,
+                               xpr_bin_sort[_cull] also writes the tile indices by decreasing list length (1024
+                               length classes) and the four rasterize calls walk the tiles in that order, so that
+                               the tail of a launch consists of short tiles */
 } xpr_config;
 
 const char* xpr_status_string(int32_t status);

@@ -33,7 +33,7 @@ class XprConfig(C.Structure):
     _fields_ = [("projection", C.c_int32), ("sh_degree", C.c_int32), ("tile", C.c_int32), ("antialias", C.c_int32),
                 ("alpha_thresh", C.c_float), ("alpha_max", C.c_float), ("t_min", C.c_float), ("z_near", C.c_float),
                 ("lowpass", C.c_float), ("ut_alpha", C.c_float), ("ut_beta", C.c_float), ("ut_kappa", C.c_float),
-                ("bg", C.c_float * 3), ("tile_cull", C.c_int32)]
+                ("bg", C.c_float * 3), ("tile_cull", C.c_int32), ("tile_order", C.c_void_p)]
 
 
 class XprError(RuntimeError):
@@ -85,6 +85,7 @@ def make_config(d: dict) -> XprConfig:
     for i in range(3):
         c.bg[i] = float(d["bg"][i])
     c.tile_cull = int(d.get("tile_cull", 0))
+    c.tile_order = None      # the pipeline sets tile_order to a device buffer of T uint32 (scheduling only)
     return c
 
 

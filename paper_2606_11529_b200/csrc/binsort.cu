@@ -903,6 +903,61 @@ ranges_kernel(const unsigned long long* __restrict__ pairs_out, uint32_t T, cons
     if (lane == 0) reinterpret_cast<uint2*>(ranges)[t] = (e > b) ? make_uint2(b, e) : make_uint2(0u, 0u);
 }
 
+// Scheduling aid for the compositing kernels (xpr_config.tile_order): the tile indices by decreasing list length,
+// in 1024 length classes (counting sort, one CTA: T is a few thousand).  Heaviest tiles first means the last wave
+// of a compositing launch is made of short tiles.
+__global__ void __launch_bounds__(1024)
+tile_order_kernel(const uint32_t* __restrict__ ranges, uint32_t T, uint32_t* __restrict__ order) {
+    __shared__ uint32_t s_cnt[1024];
+    __shared__ uint32_t s_warp[32];
+    __shared__ uint32_t s_shift;
+    const uint32_t tid = threadIdx.x;
+    uint32_t mx = 0;
+    for (uint32_t t = tid; t < T; t += 1024) mx = max(mx, ranges[2 * t + 1] - ranges[2 * t]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((tid & 31) == 0) s_warp[tid >> 5] = mx;
+    s_cnt[tid] = 0;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t m = 0;
+        for (int w = 0; w < 32; ++w) m = max(m, s_warp[w]);
+        const int bits = 32 - __clz(m | 1u);
+        s_shift = (uint32_t)max(0, bits - 10);
+    }
+    __syncthreads();
+    const uint32_t shift = s_shift;
+    for (uint32_t t = tid; t < T; t += 1024)      // class 0 = longest
+        atomicAdd(&s_cnt[1023u - min(1023u, (ranges[2 * t + 1] - ranges[2 * t]) >> shift)], 1u);
+    __syncthreads();
+    // exclusive scan of the 1024 class counts
+    const uint32_t c = s_cnt[tid];
+    uint32_t incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((tid & 31) >= (uint32_t)o) incl += v;
+    }
+    if ((tid & 31) == 31) s_warp[tid >> 5] = incl;
+    __syncthreads();
+    if (tid < 32) {
+        uint32_t w = s_warp[tid], wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, wi, o);
+            if (tid >= (uint32_t)o) wi += v;
+        }
+        s_warp[tid] = wi - w;
+    }
+    __syncthreads();
+    s_cnt[tid] = s_warp[tid >> 5] + incl - c;
+    __syncthreads();
+    for (uint32_t t = tid; t < T; t += 1024) {
+        const uint32_t cls = 1023u - min(1023u, (ranges[2 * t + 1] - ranges[2 * t]) >> shift);
+        order[atomicAdd(&s_cnt[cls], 1u)] = t;
+    }
+}
+
 }  // namespace
 }  // namespace xpr
 
@@ -967,6 +1022,10 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     if (N == 0) {
         XPR_CUDA(cudaMemsetAsync(tile_ranges, 0, sizeof(uint32_t) * 2 * (size_t)T, st));
         XPR_CUDA(cudaMemsetAsync(ws + L.header, 0, sizeof(Header), st));       // pair count 0 for an asynchronous caller
+        if (cfg->tile_order) {
+            tile_order_kernel<<<1, 1024, 0, st>>>(tile_ranges, (uint32_t)T, cfg->tile_order);
+            XPR_LAUNCH_CHECK();
+        }
         return XPR_OK;
     }
     XPR_CUDA(cudaMemsetAsync(ws + L.header, 0, L.vkey0 - L.header, st));   // header, scan chains, look-back status words
@@ -1052,6 +1111,10 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     // 6. per-tile ranges ((0, 0) for every tile when there are no pairs or they exceed the capacity)
     ranges_kernel<<<((unsigned)T + 7) / 8, 256, 0, st>>>(&hdr->pairs_out, (uint32_t)T, keys_sorted, tile_ranges);
     XPR_LAUNCH_CHECK();
+    if (cfg->tile_order) {                             // 7. scheduling order of the tiles for the compositing kernels
+        tile_order_kernel<<<1, 1024, 0, st>>>(tile_ranges, (uint32_t)T, cfg->tile_order);
+        XPR_LAUNCH_CHECK();
+    }
     if (!num_pairs_host) return XPR_OK;                // asynchronous mode: the caller reads the count later
     unsigned long long counts[2] = {0, 0};             // candidates I (must fit the capacity), pairs in the output
     XPR_CUDA(cudaMemcpyAsync(counts, &hdr->total_pairs, sizeof(counts), cudaMemcpyDeviceToHost, st));

@@ -16,6 +16,7 @@ struct RasterParams {
     int W, H, TW;
     float amax, tmin;
     float bg[3];
+    const uint32_t* order;   // xpr_config.tile_order: CTA b works on tile order[b] (longest lists first), or NULL
 };
 
 // power = fma(fma(qa, dx, qb*dy), dx, (qc*dy)*dy) with qa = -A/2, qb = -B, qc = -C/2 (R3, C25)
@@ -60,7 +61,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, log2 o, - | r, g, b, -)
     constexpr int FWD_BATCH = BLOCK / PPT;          // one list entry staged per thread
     __shared__ float4 s_rec[3 * FWD_BATCH];
-    const int tile = blockIdx.x;
+    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
     constexpr int FWD_THREADS = BLOCK / PPT, ROW = TILE / PPT;
     const int px0 = tx * TILE + (threadIdx.x % ROW), px1 = px0 + 8, py = ty * TILE + (threadIdx.x / ROW);
@@ -252,7 +253,7 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     __shared__ float4 s_gate[BWD_BATCH];  // C, thr, o, index (bits)
     __shared__ float4 s_col[BWD_BATCH];   // r, g, b, unused
     __shared__ uint32_t s_max[BWD_THREADS / 32];
-    const int tile = blockIdx.x;
+    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
     const int lane = threadIdx.x & 31;
     // a thread owns BWD_PPT consecutive pixels of one row: they share dy and the row terms of `power`
@@ -370,6 +371,7 @@ int32_t make_raster_params(const xpr_camera* cam, const xpr_config* cfg, RasterP
     P.W = cam->width; P.H = cam->height; P.TW = tiles_x(cam);
     P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
     for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
+    P.order = cfg->tile_order;
     return XPR_OK;
 }
 

@@ -19,6 +19,7 @@ struct RayRasterParams {
     int W, H, TW;
     float amax, tmin, lnr;     // lnr = (float) ln(0.0113)
     float bg[3];
+    const uint32_t* order;     // xpr_config.tile_order: CTA b works on tile order[b] (longest lists first), or NULL
 };
 
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -97,7 +98,7 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                          unsigned long long* __restrict__ stats) {
     constexpr int THREADS = BLOCK / PPT, BATCH = THREADS, ROW = TILE / PPT;
     __shared__ float4 s_rec[5 * BATCH];
-    const int tile = blockIdx.x;
+    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
     const int py = ty * TILE + (threadIdx.x / ROW);
     int px[PPT];
@@ -233,7 +234,7 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
     __shared__ float4 s_gate[BATCH];   // thr, o, log2 o, index (bits)
     __shared__ float4 s_col[BATCH];    // r, g, b, -
     __shared__ uint32_t s_max[THREADS / 32];
-    const int tile = blockIdx.x;
+    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
     const int lane = threadIdx.x & 31;
     constexpr int TPR = TILE / PPT;
@@ -355,6 +356,7 @@ int32_t make_params(const xpr_camera* cam, const xpr_config* cfg, RayRasterParam
     P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
     P.lnr = (float)log(0.0113);
     for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
+    P.order = cfg->tile_order;
     return XPR_OK;
 }
 

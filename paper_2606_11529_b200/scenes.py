@@ -193,7 +193,7 @@ def default_render_config(scene: Scene) -> dict:
     """Renderer constants; fp32-rounded values as Python floats."""
     return dict(projection=scene.projection, sh_degree=scene.sh_degree, tile=16, antialias=scene.antialias,
                 alpha_thresh=_f32(1.0 / 255.0), alpha_max=_f32(0.99), t_min=_f32(1e-4), z_near=_f32(0.2),
-                lowpass=_f32(0.3), ut_alpha=1.0, ut_beta=2.0, ut_kappa=0.0, bg=(0.0, 0.0, 0.0), tile_cull=0, ray_eval=0)
+                lowpass=_f32(0.3), ut_alpha=1.0, ut_beta=2.0, ut_kappa=0.0, bg=(0.0, 0.0, 0.0), tile_cull=0, ray_eval=0, tile_order=-1)
 
 
 def loss_and_grad(kind: str, image: np.ndarray, target: np.ndarray):

@@ -35,7 +35,8 @@ def test_header_symbols_all_exported(lib):
 def test_struct_layout_matches_header():
     from paper_2606_11529_b200 import binding
     assert C.sizeof(binding.XprCamera) == 3 * 4 + 4 * 4 + 4 * 4 + 12 * 4
-    assert C.sizeof(binding.XprConfig) == 4 * 4 + 8 * 4 + 3 * 4 + 4
+    assert C.sizeof(binding.XprConfig) == 4 * 4 + 8 * 4 + 3 * 4 + 4 + 8     # + tile_order pointer
+    assert binding.XprConfig.tile_order.offset == 64
 
 
 def test_status_strings_and_version(lib):

@@ -165,3 +165,24 @@ def test_loss_grad_helper_matches_the_definition(kind):
         xb.xpr_loss_grad(kind, torch.from_numpy(img).cuda(), torch.from_numpy(tgt).cuda(), out)
         torch.cuda.synchronize()
         np.testing.assert_array_equal(out.cpu().numpy().view(np.uint32), want.view(np.uint32))
+
+
+def test_tile_order_is_a_permutation_by_decreasing_length_and_changes_no_result():
+    sc = scenes.make_scene(3, n_override=40000, image_override=(480, 270))
+    a = pu.run_gpu(sc, 0, dict(tile_cull=1, tile_order=1))
+    b = pu.run_gpu(sc, 0, dict(tile_cull=1, tile_order=0))
+    assert b["pipe"].tile_order is None
+    order = pu.u32(a["pipe"].tile_order)
+    T = a["pipe"].T
+    np.testing.assert_array_equal(np.sort(order), np.arange(T, dtype=np.uint32))
+    ln = (a["binned"]["ranges"][:, 1] - a["binned"]["ranges"][:, 0]).astype(np.int64)
+    shift = max(0, int(ln.max()).bit_length() - 10)
+    cls = np.minimum(1023, ln[order] >> shift)
+    assert (np.diff(cls) <= 0).all() and ln[order[0]] >> shift == ln.max() >> shift
+    for k in ("image", "final_T", "n_contrib"):
+        np.testing.assert_array_equal(a["fwd"][k], b["fwd"][k])
+    dL = np.random.default_rng(0).standard_normal((270, 480, 3)).astype(np.float32)
+    ga, gb = pu.run_gpu_backward(a, dL), pu.run_gpu_backward(b, dL)
+    for k in ("g_means", "g_sh", "g_opacities"):
+        bad, _ = pu.grad_violations(ga[k], gb[k])
+        assert bad.mean() <= 1e-4, k          # the atomics' order differs, nothing else
