@@ -365,30 +365,83 @@ def run_ours(args):
         h2d = sum(t.numel() * t.element_size() for t in host_in)
         d2h = sum(t.numel() * t.element_size() for t in host_out)
 
-        def e2e_step():
-            for d, h in zip(dev_in, host_in):
-                d.copy_(h, non_blocking=True)
-            pipe.project(*dev_in)
+        def run_step(inputs):
+            pipe.project(*inputs)
             if args.ray_eval:
                 pipe.pixel_info(); pipe.project_ray()
             pipe.bin_sort_async(); pipe.rasterize_fwd()
             pipe.rasterize_bwd(loss_grad(pipe.image)); pipe.project_bwd()
+
+        def e2e_step():       # one stream: copy in, step, copy out (the latency of a single step)
+            for d, h in zip(dev_in, host_in):
+                d.copy_(h, non_blocking=True)
+            run_step(dev_in)
             for h, o in zip(host_out, outs):
                 h.copy_(o, non_blocking=True)
 
         for _ in range(2):
             e2e_step()
         barrier()
-        k = max(3, min(args.steps, 10))
+        k = max(3, args.steps)
         t_ms = 0.0
         for _ in range(k):
             flush.fill_(1)
             a = _rec(); e2e_step(); b = _rec()
             torch.cuda.synchronize()
             t_ms += a.elapsed_time(b)
-        t_ms = max_over_ranks(t_ms, world, dev)
-        e2e = {"value": aggregate_value(world, mp, t_ms / k), "unit": UNIT, "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "ms_per_step": t_ms / k}
+        lat_ms = max_over_ranks(t_ms, world, dev) / k
+
+        # the same K steps as a three-stage software pipeline: the H2D copy of step i+1 and the D2H copy of step i-1
+        # run on their own streams (PCIe is full duplex) under the kernels of step i.  Inputs and the outputs'
+        # staging copies are double-buffered; every step still copies all its inputs in and all its results out.
+        s_c = torch.cuda.current_stream()
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+        dev_in2 = [dev_in, [torch.empty_like(p) for p in params]]
+        stage = [[torch.empty_like(o) for o in outs] for _ in range(2)]
+
+        def pipelined(n):
+            ev_in, ev_c, ev_out = [None] * n, [None] * n, [None] * n
+            start = torch.cuda.Event(enable_timing=True); start.record(s_c)
+            s_in.wait_event(start); s_out.wait_event(start)
+            for i in range(n):
+                bsel = i % 2
+                with torch.cuda.stream(s_in):
+                    if i >= 2:
+                        s_in.wait_event(ev_c[i - 2])            # the kernels that read this input buffer are done
+                    for d, h in zip(dev_in2[bsel], host_in):
+                        d.copy_(h, non_blocking=True)
+                    ev_in[i] = torch.cuda.Event(); ev_in[i].record(s_in)
+                s_c.wait_event(ev_in[i])
+                run_step(dev_in2[bsel])
+                if i >= 2:
+                    s_c.wait_event(ev_out[i - 2])               # this staging buffer has left for the host
+                for st_, o in zip(stage[bsel], outs):
+                    st_.copy_(o, non_blocking=True)
+                ev_c[i] = torch.cuda.Event(); ev_c[i].record(s_c)
+                with torch.cuda.stream(s_out):
+                    s_out.wait_event(ev_c[i])
+                    for h, st_ in zip(host_out, stage[bsel]):
+                        h.copy_(st_, non_blocking=True)
+                    ev_out[i] = torch.cuda.Event(); ev_out[i].record(s_out)
+            end = torch.cuda.Event(enable_timing=True)
+            s_c.wait_stream(s_out); s_c.wait_stream(s_in)
+            end.record(s_c)
+            torch.cuda.synchronize()
+            return start.elapsed_time(end)
+
+        pipelined(3)
+        barrier()
+        t_ms = max_over_ranks(pipelined(k), world, dev)
+        assert pipe.check_capacity() == n_pairs
+        pipe_ms = t_ms / k
+        best = min(pipe_ms, lat_ms)      # tiny configs: the events of the pipeline cost more than the overlap saves
+        e2e = {"value": aggregate_value(world, mp, best), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "ms_per_step": best, "steps": k,
+               "how": ("K steps as a 3-stage pipeline (H2D | kernels | D2H on three streams, double-buffered)"
+                       if pipe_ms <= lat_ms else "K steps on one stream (copy in, kernels, copy out)")
+                      + "; every step copies all inputs from and all results (image + parameter gradients) to pinned "
+                        "host memory",
+               "pipelined_ms_per_step": pipe_ms, "single_stream_ms_per_step": lat_ms}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
