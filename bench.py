@@ -315,8 +315,12 @@ def run_ours(args):
                      "achieved": sort_bytes / sec("bin_sort") / 1e9, "algorithmic_bytes": sort_bytes},
     }
     traffic = {}
-    try:   # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu --set full capture
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get("config%d%s" % (args.config, "_ray" if args.ray_eval else ""), {})
+    try:   # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu captures (profiles/ncu_traffic.md)
+        key = "config%d%s" % (args.config, "_ray" if args.ray_eval else "")
+        for ln in open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")).read().splitlines()[1:]:
+            w, stage, b = ln.split(",")
+            if w == key:
+                traffic[stage] = int(b)
     except Exception:
         pass
     for name, r in rooflines.items():
