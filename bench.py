@@ -335,14 +335,7 @@ def run_ours(args):
     graph_ms = None
     if not args.no_graph:
         try:
-            side = torch.cuda.Stream()
-            side.wait_stream(torch.cuda.current_stream())
-            with torch.cuda.stream(side):
-                step()
-            torch.cuda.current_stream().wait_stream(side)
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                step()
+            g = pipe.capture_step(*params, target, sc.loss, pixel_info=bool(args.ray_eval))
             for _ in range(3):
                 g.replay()
             barrier()

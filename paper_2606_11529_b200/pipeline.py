@@ -22,6 +22,7 @@ class SplatPipeline:
         self.device = torch.device(device)
         self.cam = cam if isinstance(cam, xb.XprCamera) else xb.make_camera(cam)
         self.ray_eval = bool(cfg.get("ray_eval", 0)) if isinstance(cfg, dict) else False
+        self._dL = None
         self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
         self.K = (int(self.cfg.sh_degree) + 1) ** 2
         self.W, self.H = int(self.cam.width), int(self.cam.height)
@@ -169,6 +170,36 @@ class SplatPipeline:
         self.project_bwd()
         return dict(g_means=self.g_means, g_scales=self.g_scales, g_quats=self.g_quats,
                     g_opacities=self.g_opacities, g_sh=self.g_sh)
+
+    def step_async(self, means, scales, quats, opacities, sh, target, loss: str, pixel_info: bool = False):
+        """One training step (forward, dL/dimage of `loss` against `target`, backward) enqueued on the current
+        stream without any host read-back: xpr_bin_sort runs with num_pairs_host = NULL.  The pair buffers must
+        have been sized by an earlier forward(); call check_capacity() once the stream has run."""
+        if self._dL is None:
+            self._dL = torch.empty_like(self.image)
+        self.project(means, scales, quats, opacities, sh)
+        if self.ray_eval:
+            if pixel_info:
+                self.pixel_info()
+            self.project_ray()
+        self.bin_sort_async()
+        self.rasterize_fwd()
+        xb.xpr_loss_grad(loss, self.image, target, self._dL)
+        self.rasterize_bwd(self._dL)
+        self.project_bwd()
+
+    def capture_step(self, means, scales, quats, opacities, sh, target, loss: str, pixel_info: bool = False):
+        """step_async() captured once into a CUDA graph (nothing on the path waits for the host, so the whole step
+        is capturable); graph.replay() then runs a step on the same buffers with no per-launch host work."""
+        side = torch.cuda.Stream(self.device)
+        side.wait_stream(torch.cuda.current_stream(self.device))
+        with torch.cuda.stream(side):                    # warm-up outside the capture (lazy module loading)
+            self.step_async(means, scales, quats, opacities, sh, target, loss, pixel_info)
+        torch.cuda.current_stream(self.device).wait_stream(side)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            self.step_async(means, scales, quats, opacities, sh, target, loss, pixel_info)
+        return graph
 
 
 def scene_to_device(scene, device="cuda:0"):

@@ -186,3 +186,32 @@ def test_tile_order_is_a_permutation_by_decreasing_length_and_changes_no_result(
     for k in ("g_means", "g_sh", "g_opacities"):
         bad, _ = pu.grad_violations(ga[k], gb[k])
         assert bad.mean() <= 1e-4, k          # the atomics' order differs, nothing else
+
+
+@pytest.mark.parametrize("ray", [0, 1])
+def test_captured_step_replays_the_eager_step(ray):
+    """pipeline.capture_step: the whole step in one CUDA graph gives the results of the eager calls."""
+    import torch
+    from paper_2606_11529_b200 import pipeline
+    sc = scenes.make_scene(4 if ray else 3, n_override=20000, image_override=(320, 180))
+    cfg = dict(scenes.default_render_config(sc), tile_cull=1, ray_eval=ray)
+    params = pipeline.scene_to_device(sc)
+    target = torch.from_numpy(sc.target(0)).cuda()
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg)
+    img = pipe.forward(*params).clone()
+    dL = torch.sign(img - target)
+    pipe.backward(dL)
+    torch.cuda.synchronize()
+    want = {k: getattr(pipe, k).clone() for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")}
+    n = pipe.num_pairs
+    graph = pipe.capture_step(*params, target, "l1", pixel_info=bool(ray))
+    for k in want:
+        getattr(pipe, k).fill_(7.0)
+    pipe.image.fill_(7.0)
+    graph.replay(); graph.replay()
+    torch.cuda.synchronize()
+    assert pipe.check_capacity() == n
+    assert torch.equal(pipe.image, img)
+    for k, v in want.items():
+        bad, _ = pu.grad_violations(getattr(pipe, k).cpu().numpy(), v.cpu().numpy())
+        assert bad.mean() <= 1e-4, k            # same kernels, same inputs: only the order of the atomics differs
