@@ -445,10 +445,15 @@ extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cf
         return XPR_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     if (zero_init) {
-        XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 2 * (size_t)N, st));
-        XPR_CUDA(cudaMemsetAsync(g_conic, 0, sizeof(float) * 3 * (size_t)N, st));
-        XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * (size_t)N, st));
-        XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * (size_t)N, st));
+        const size_t n = (size_t)N;
+        if (g_conic == g_mean2d + 2 * n && g_opac == g_conic + 3 * n && g_rgb == g_opac + n) {
+            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 9 * n, st));      // one allocation: one fill
+        } else {
+            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 2 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_conic, 0, sizeof(float) * 3 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
+        }
     }
     RasterParams P;
     make_raster_params(cam, cfg, P);

@@ -439,9 +439,14 @@ extern "C" int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config
         return XPR_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     if (zero_init) {
-        XPR_CUDA(cudaMemsetAsync(g_ray_rec, 0, sizeof(float) * 12 * (size_t)N, st));
-        XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * (size_t)N, st));
-        XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * (size_t)N, st));
+        const size_t n = (size_t)N;
+        if (g_opac == g_ray_rec + 12 * n && g_rgb == g_opac + n) {
+            XPR_CUDA(cudaMemsetAsync(g_ray_rec, 0, sizeof(float) * 16 * n, st));     // one allocation: one fill
+        } else {
+            XPR_CUDA(cudaMemsetAsync(g_ray_rec, 0, sizeof(float) * 12 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
+        }
     }
     RayRasterParams P;
     make_params(cam, cfg, P);

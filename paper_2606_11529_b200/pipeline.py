@@ -52,11 +52,18 @@ class SplatPipeline:
         self.image, self.final_T = e(self.H, self.W, 3), e(self.H, self.W)
         self.n_contrib = e(self.H, self.W, dtype=i32)
         # gradients (a9, a10)
-        self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb = e(N, 2), e(N, 3), e(N), e(N, 3)
+        # the compositing gradients share one allocation, in the order the library checks for, so that
+        # xpr_rasterize_bwd zero-fills them with a single memset
+        g2 = e(9 * N)
+        self.g_mean2d, self.g_conic = g2[:2 * N].view(N, 2), g2[2 * N:5 * N].view(N, 3)
+        self.g_opac, self.g_rgb = g2[5 * N:6 * N], g2[6 * N:].view(N, 3)
         self.g_means, self.g_scales, self.g_quats = e(N, 3), e(N, 3), e(N, 4)
         self.g_opacities, self.g_sh = e(N), e(N, self.K, 3)
         if self.ray_eval:   # f2: shader record, per-pixel rays, record gradient
-            self.ray_rec, self.g_ray_rec = e(N, 12), e(N, 12)
+            self.ray_rec = e(N, 12)
+            g3 = e(16 * N)                                 # g_ray_rec | g_opac | g_rgb: one memset in xpr_rasterize_ray_bwd
+            self.g_ray_rec = g3[:12 * N].view(N, 12)
+            self.g_opac, self.g_rgb = g3[12 * N:13 * N], g3[13 * N:].view(N, 3)
             self.pixel_rays = e(self.H, self.W, 3)
             self.pixel_info()
             self.g_mean2d.zero_(); self.g_conic.zero_()    # the footprint carries no gradient
