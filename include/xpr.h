@@ -171,6 +171,7 @@ int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_
  *   in : forward inputs + final_T, n_contrib, dL_dimage[H,W,3].
  *   out: g_mean2d[N,2], g_conic[N,3] (w.r.t. A,B,C), g_opac[N] (w.r.t. o_eff), g_rgb[N,3];
  *        ACCUMULATED with fp32 atomics; zero-filled first by this call when zero_init != 0.
+ *        (with one fill instead of four when the four arrays are adjacent slices of one allocation, in this order).
  */
 int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
                           const float* conic_opac, const float* rgb, const float* lnv,
