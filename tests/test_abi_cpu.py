@@ -132,3 +132,14 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "xpr_oracle" not in txt and "import oracle" not in txt, f
+
+
+def test_profiles_hold_text_summaries_only():
+    """profiles/ holds ncu summaries as .txt / .csv / .md; every .csv is named by a .md beside it."""
+    d = os.path.join(ROOT, "profiles")
+    names = sorted(os.listdir(d))
+    assert names and all(n.endswith((".txt", ".csv", ".md")) for n in names), names
+    mds = "\n".join(open(os.path.join(d, n)).read() for n in names if n.endswith(".md"))
+    for n in names:
+        if n.endswith(".csv"):
+            assert n in mds, n
