@@ -1038,9 +1038,12 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     for (int p = 0; p < DEPTH_PASSES; ++p) {
         uint32_t* status = status32 + (size_t)p * RADIX * tiles32;
         const int a = p & 1, b = a ^ 1;
-        cudaError_t e = (p < 3)   // mantissa bytes: ~32 distinct digits per warp -> bitmap ranking
-            ? launch_pass<uint32_t, IPT32, true, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr)
-            : launch_pass<uint32_t, IPT32, false, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], vkey[b], vidx[b], hdr, status, nullptr, nullptr);
+        // mantissa bytes: ~32 distinct digits per warp -> bitmap ranking; exponent byte: ballots
+#define XPR_DEPTH_PASS(BITMAP_)                                                                          \
+    launch_pass<uint32_t, IPT32, BITMAP_, 0>(tiles32, st, &hdr->n_vis, nullptr, 8 * p, p, vkey[a], vidx[a], \
+                                             vkey[b], vidx[b], hdr, status, nullptr, nullptr)
+        const cudaError_t e = (p < 3) ? XPR_DEPTH_PASS(true) : XPR_DEPTH_PASS(false);
+#undef XPR_DEPTH_PASS
         XPR_CUDA(e);
     }   // DEPTH_PASSES is even: the sorted list is back in vkey[0] / vidx[0]
     // 3. rows: a row is the run of consecutive tiles one Gaussian covers in one tile row;
@@ -1097,13 +1100,18 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
             uint32_t* status = status64 + (size_t)p * RADIX * tiles64;
             const int row = DEPTH_PASSES + p, shift = 32 + 8 * p;
             const bool last = (p == tpasses - 1);
-            cudaError_t e;
             // bitmap ranking: consecutive pairs of a Gaussian are consecutive tiles (digit 0); after pass 1 a
-            // warp holds many distinct high digits
-            if (!last)       e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 1>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr)
-                                          : launch_pass<uint64_t, IPT64, false, 1>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, nullptr, hdr, status, nullptr, nullptr);
-            else             e = ((p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP)) ? launch_pass<uint64_t, IPT64, true, 2>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0])
-                                          : launch_pass<uint64_t, IPT64, false, 2>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, w1, vals_sorted, hdr, status, vkey[0], vidx[0]);
+            // warp holds many distinct high digits.  MODE 1: words -> words; MODE 2 (last pass): expand to key + value
+#define XPR_TILE_PASS(BITMAP_, MODE_, VOUT_, TK_, TV_)                                                    \
+    launch_pass<uint64_t, IPT64, BITMAP_, MODE_>(tiles64, st, nullptr, &hdr->pairs_out, shift, row, w0, nullptr, \
+                                                 w1, VOUT_, hdr, status, TK_, TV_)
+            const bool bitmap = (p == 0 && XPR_P1_BITMAP) || (p > 0 && XPR_P2_BITMAP);
+            cudaError_t e;
+            if (!last) e = bitmap ? XPR_TILE_PASS(true, 1, nullptr, nullptr, nullptr)
+                                  : XPR_TILE_PASS(false, 1, nullptr, nullptr, nullptr);
+            else       e = bitmap ? XPR_TILE_PASS(true, 2, vals_sorted, vkey[0], vidx[0])
+                                  : XPR_TILE_PASS(false, 2, vals_sorted, vkey[0], vidx[0]);
+#undef XPR_TILE_PASS
             XPR_CUDA(e);
             uint64_t* t = w0; w0 = w1; w1 = t;
         }
