@@ -877,3 +877,6 @@ extern "C" int32_t xpr_oracle_num_threads(void) {
 
 // XPR-3DGUT ray evaluation
 #include "xpr_oracle_ray.inc"
+
+// rendered depth and accumulated opacity
+#include "xpr_oracle_feat.inc"

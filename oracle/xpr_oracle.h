@@ -8,7 +8,7 @@
  *
  * What it computes: the plain definition of tile-based 3DGS rendering and its exact reverse-mode
  * derivative, written from /root/reference/PAPER.md (XPR, arxiv 2606.11529) and the readings
- * C1..C30 / rules R1..R3 in DESIGN.md.  Each function cites the passage it follows
+ * C1..C31 / rules R1..R3 in DESIGN.md.  Each function cites the passage it follows
  * ("PAPER L<line>").  Scalar type: *_f32 = parity mode (every operation individually rounded in
  * fp32, in the order DESIGN.md section 3 fixes; compiled with -ffp-contract=off), *_f64 =
  * self-check mode (closed forms, finite differences).  Gradients are accumulated and returned
@@ -20,7 +20,9 @@
  * P9 fisheye special cases, P10 SH orthonormality/degree-0, P11 linearity, P12 fp32-vs-fp64,
  * P13 tile_cull (dense-sampling maximum, no passing pixel in a dropped pair, image unchanged),
  * P14 3DGUT ray evaluation (brute-force maximum along the ray in the world frame, isotropic closed form,
- * pixel_info as the inverse of the camera model, finite differences).
+ * pixel_info as the inverse of the camera model, finite differences),
+ * P15 rendered depth / accumulated opacity (equal to the pinned colour pass with rgb := (z, 1, .) and bg = 0,
+ * A = 1 - T_final, finite differences).
  * No function here is "parity unpinned".
  */
 #ifndef XPR_ORACLE_H
@@ -167,6 +169,33 @@ int64_t xpr_oracle_bin_sort_cull(int64_t N, const float* depth, const int32_t* t
 
 XO_RAY_DECL(f32, float)
 XO_RAY_DECL(f64, double)
+
+/* ---- Rendered features beyond colour, SURVEY 8(f) f3 (xpr_oracle_feat.inc; Table 2; reading C31):
+ * depth image D = sum_k z_k alpha_k T_k and accumulated opacity A = sum_k alpha_k T_k over the colour pass's own
+ * contributing sequence, no background; depth [N] = camera-space z of the centres (project's output).  The
+ * backward takes dL/dimage, dL/dD, dL/dA and returns rasterize_bwd's outputs plus g_depth [N].  Pin P15. */
+#define XO_FEAT_DECL(S, T)                                                                               \
+    void xpr_oracle_rasterize_fwd_da_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,          \
+                                         const T* mean2d, const T* conic, const T* opac_eff,             \
+                                         const T* rgb, const T* lnv, const T* depth,                     \
+                                         const uint32_t* vals_sorted, const uint32_t* tile_ranges,       \
+                                         T* depth_img, T* alpha_img);                                    \
+    void xpr_oracle_rasterize_bwd_da_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,          \
+                                         const T* mean2d, const T* conic, const T* opac_eff,             \
+                                         const T* rgb, const T* lnv, const T* depth,                     \
+                                         const uint32_t* vals_sorted, const uint32_t* tile_ranges,       \
+                                         const uint32_t* n_contrib, const T* dL_dimage,                  \
+                                         const T* dL_ddepth, const T* dL_dalpha, double* g_mean2d,       \
+                                         double* g_conic, double* g_opac_eff, double* g_rgb,             \
+                                         double* g_depth);
+
+XO_FEAT_DECL(f32, float)
+XO_FEAT_DECL(f64, double)
+
+/* z = (W mu + t)_z: WRITES g_means [N*3] = W[2,:] g_depth (zeros where tile_count == 0); the caller adds it to
+ * project_bwd's g_means. */
+void xpr_oracle_depth_bwd(int64_t N, const xo_camera* cam, const uint32_t* tile_count, const double* g_depth,
+                          double* g_means);
 
 int32_t xpr_oracle_num_threads(void);
 

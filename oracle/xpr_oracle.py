@@ -355,3 +355,59 @@ def backward_ray(scene_arrays: dict, r: dict, dL_dimage, cam: XoCamera, cfg: XoC
     g3.update(g2)
     g3["ray_part"] = gr
     return g3
+
+
+# ---- Rendered depth and accumulated opacity (xpr_oracle_feat.inc, reading C31) ---------------
+
+def rasterize_fwd_da(proj: dict, binned: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """depth image D = sum_k z_k alpha_k T_k and accumulated opacity A = sum_k alpha_k T_k, [H,W] each."""
+    dt = np.dtype(dtype)
+    H, W = int(cam.height), int(cam.width)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv", "depth")]
+    out = dict(depth_img=np.empty((H, W), dt), alpha_img=np.empty((H, W), dt))
+    fn = getattr(lib(), "xpr_oracle_rasterize_fwd_da_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+       _p(out["depth_img"]), _p(out["alpha_img"]))
+    return out
+
+
+def rasterize_bwd_da(proj: dict, binned: dict, fwd: dict, dL_dimage, dL_ddepth, dL_dalpha, cam: XoCamera,
+                     cfg: XoConfig, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv", "depth")]
+    d = [np.ascontiguousarray(x, dt) for x in (dL_dimage, dL_ddepth, dL_dalpha)]
+    out = dict(g_mean2d=np.empty((N, 2), np.float64), g_conic=np.empty((N, 3), np.float64),
+               g_opac_eff=np.empty(N, np.float64), g_rgb=np.empty((N, 3), np.float64), g_depth=np.empty(N, np.float64))
+    fn = getattr(lib(), "xpr_oracle_rasterize_bwd_da_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+       _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), *[_p(x) for x in d],
+       *[_p(out[k]) for k in ("g_mean2d", "g_conic", "g_opac_eff", "g_rgb", "g_depth")])
+    return out
+
+
+def depth_bwd(tile_count, g_depth, cam: XoCamera):
+    N = int(tile_count.shape[0])
+    g = np.ascontiguousarray(g_depth, np.float64)
+    out = np.empty((N, 3), np.float64)
+    lib().xpr_oracle_depth_bwd(C.c_int64(N), C.byref(cam), _p(np.ascontiguousarray(tile_count, np.uint32)), _p(g), _p(out))
+    return out
+
+
+def render_da(scene_arrays: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """render() plus the depth image and the accumulated opacity (fwd["depth_img"], fwd["alpha_img"])."""
+    r = render(scene_arrays, cam, cfg, dtype)
+    r["fwd"].update(rasterize_fwd_da(r["proj"], r["binned"], cam, cfg, dtype))
+    return r
+
+
+def backward_da(scene_arrays: dict, r: dict, dL_dimage, dL_ddepth, dL_dalpha, cam: XoCamera, cfg: XoConfig,
+                dtype=np.float32) -> dict:
+    """Backward of render_da: parameter gradients (fp64) of a loss with dL/dimage, dL/dD, dL/dA."""
+    s = scene_arrays
+    g2 = rasterize_bwd_da(r["proj"], r["binned"], r["fwd"], dL_dimage, dL_ddepth, dL_dalpha, cam, cfg, dtype)
+    g3 = project_bwd(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, g2, dtype)
+    g3["g_means"] = g3["g_means"] + depth_bwd(r["proj"]["tile_count"], g2["g_depth"], cam)
+    g3.update(g2)
+    return g3
