@@ -234,6 +234,36 @@ int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const fl
                     float* g_means, float* g_scales, float* g_quats, void* stream);
 
 /*
+ * ---- Rendered features beyond colour ("rendered features such as depth", Table 2) ----
+ * Reading C31: a rendered feature is blended with the colour's weights over the pixel's contributing
+ * sequence, without a background term:
+ *   depth image D[H,W] = sum_k z_k alpha_k T_k  (z_k = `depth` of xpr_project, the depth of the sort key, L149),
+ *   accumulated opacity A[H,W] = sum_k alpha_k T_k.
+ * xpr_rasterize_feat_fwd -- xpr_rasterize_fwd that also writes depth_img and alpha_img in the same walk (image,
+ *   final_T, n_contrib as xpr_rasterize_fwd: same gates, clamp and exit).  depth: DEVICE fp32 [N].
+ * xpr_rasterize_feat_bwd -- xpr_rasterize_bwd with the two extra incoming gradients dL_ddepth[H,W], dL_dalpha[H,W]
+ *   and the extra output g_depth[N] = dL/dz; ACCUMULATES like xpr_rasterize_bwd, zero-filled first when
+ *   zero_init != 0 (one fill when g_mean2d, g_conic, g_opac, g_rgb, g_depth are adjacent slices, in this order).
+ * xpr_depth_bwd -- z = (W mu + t)_z: ADDS W[2,:] g_depth[i] to g_means[i,:] for every Gaussian with
+ *   tile_count[i] > 0 (call it after xpr_project_bwd, which overwrites g_means).
+ * Errors as the colour calls: null / misaligned pointer, N < 0 -> XPR_ERR_INVALID_ARG before any launch.
+ */
+int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                               const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+                               const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                               float* image, float* final_T, uint32_t* n_contrib, float* depth_img,
+                               float* alpha_img, void* stream);
+int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                               const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+                               const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                               const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
+                               const float* dL_ddepth, const float* dL_dalpha,
+                               float* g_mean2d, float* g_conic, float* g_opac, float* g_rgb, float* g_depth,
+                               int32_t zero_init, void* stream);
+int32_t xpr_depth_bwd(int64_t N, const xpr_camera* cam, const uint32_t* tile_count, const float* g_depth,
+                      float* g_means, void* stream);
+
+/*
  * xpr_loss_grad -- convenience for the caller's side of the step (reading C21: the loss lives outside the path):
  * dL/dimage of the two losses BASELINE.json's configs name, as sums over all n = H*W*3 values, in one pass:
  *   kind 0: L = sum |I - target|    -> dL = sign(I - target);      kind 1: L = sum (I - target)^2 -> dL = 2 (I - target).

@@ -187,6 +187,15 @@ XO_RAY_DECL(f64, double)
                                          const uint32_t* n_contrib, const T* dL_dimage,                  \
                                          const T* dL_ddepth, const T* dL_dalpha, double* g_mean2d,       \
                                          double* g_conic, double* g_opac_eff, double* g_rgb,             \
+                                         double* g_depth);                                               \
+    /* sum of |addend| per element (tolerance aid, like xpr_oracle_rasterize_bwd_mass_*) */             \
+    void xpr_oracle_rasterize_bwd_da_mass_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,     \
+                                         const T* mean2d, const T* conic, const T* opac_eff,             \
+                                         const T* rgb, const T* lnv, const T* depth,                     \
+                                         const uint32_t* vals_sorted, const uint32_t* tile_ranges,       \
+                                         const uint32_t* n_contrib, const T* dL_dimage,                  \
+                                         const T* dL_ddepth, const T* dL_dalpha, double* g_mean2d,       \
+                                         double* g_conic, double* g_opac_eff, double* g_rgb,             \
                                          double* g_depth);
 
 XO_FEAT_DECL(f32, float)

@@ -373,14 +373,14 @@ def rasterize_fwd_da(proj: dict, binned: dict, cam: XoCamera, cfg: XoConfig, dty
 
 
 def rasterize_bwd_da(proj: dict, binned: dict, fwd: dict, dL_dimage, dL_ddepth, dL_dalpha, cam: XoCamera,
-                     cfg: XoConfig, dtype=np.float32) -> dict:
+                     cfg: XoConfig, dtype=np.float32, mass: bool = False) -> dict:
     dt = np.dtype(dtype)
     N = int(proj["tile_count"].shape[0])
     a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv", "depth")]
     d = [np.ascontiguousarray(x, dt) for x in (dL_dimage, dL_ddepth, dL_dalpha)]
     out = dict(g_mean2d=np.empty((N, 2), np.float64), g_conic=np.empty((N, 3), np.float64),
                g_opac_eff=np.empty(N, np.float64), g_rgb=np.empty((N, 3), np.float64), g_depth=np.empty(N, np.float64))
-    fn = getattr(lib(), "xpr_oracle_rasterize_bwd_da_" + _sfx(dt))
+    fn = getattr(lib(), ("xpr_oracle_rasterize_bwd_da_mass_" if mass else "xpr_oracle_rasterize_bwd_da_") + _sfx(dt))
     fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
        _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), *[_p(x) for x in d],
        *[_p(out[k]) for k in ("g_mean2d", "g_conic", "g_opac_eff", "g_rgb", "g_depth")])

@@ -20,7 +20,7 @@ FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_R
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
            "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
-           "xpr_ray_bwd", "xpr_loss_grad")
+           "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_loss_grad")
 
 
 class XprCamera(C.Structure):
@@ -236,6 +236,34 @@ def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_rec, g_m
     N = int(means.shape[0])
     _check(lib().xpr_ray_bwd(C.c_int64(N), _p(means), _p(scales), _p(quats), C.byref(cam), _p(tile_count),
                              _p(g_ray_rec), _p(g_means), _p(g_scales), _p(g_quats), _stream(stream)), "xpr_ray_bwd")
+
+
+# ---- Rendered depth and accumulated opacity (xpr.h) --------------------------------------------
+
+def xpr_rasterize_feat_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, depth, vals_sorted,
+                           tile_ranges, image, final_T, n_contrib, depth_img, alpha_img, stream=None):
+    N = int(mean2d.shape[0])
+    _check(lib().xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
+                                        _p(lnv), _p(depth), _p(vals_sorted), _p(tile_ranges), _p(image), _p(final_T),
+                                        _p(n_contrib), _p(depth_img), _p(alpha_img), _stream(stream)),
+           "xpr_rasterize_feat_fwd")
+
+
+def xpr_rasterize_feat_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, depth, vals_sorted,
+                           tile_ranges, final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_mean2d, g_conic,
+                           g_opac, g_rgb, g_depth, zero_init: bool = True, stream=None):
+    N = int(mean2d.shape[0])
+    _check(lib().xpr_rasterize_feat_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
+                                        _p(lnv), _p(depth), _p(vals_sorted), _p(tile_ranges), _p(final_T),
+                                        _p(n_contrib), _p(dL_dimage), _p(dL_ddepth), _p(dL_dalpha), _p(g_mean2d),
+                                        _p(g_conic), _p(g_opac), _p(g_rgb), _p(g_depth),
+                                        C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_feat_bwd")
+
+
+def xpr_depth_bwd(cam: XprCamera, tile_count, g_depth, g_means, stream=None):
+    N = int(tile_count.shape[0])
+    _check(lib().xpr_depth_bwd(C.c_int64(N), C.byref(cam), _p(tile_count), _p(g_depth), _p(g_means), _stream(stream)),
+           "xpr_depth_bwd")
 
 
 def xpr_loss_grad(kind: str, image, target, dL_dimage, stream=None):

@@ -28,6 +28,7 @@ SOURCES = {
     "rasterize.cu": [],
     "ray.cu": ["-fmad=false"],
     "rasterize_ray.cu": [],
+    "rasterize_feat.cu": [],
 }
 
 

@@ -1,0 +1,397 @@
+// rasterize_feat.cu -- xpr_rasterize_feat_fwd / xpr_rasterize_feat_bwd / xpr_depth_bwd: compositing with the
+// rendered features of SURVEY 8(f) f3 ("rendered features such as depth", Table 2; DESIGN.md
+// reading C31): next to the colour, the same walk blends the depth image D = sum_k z_k alpha_k T_k and the
+// accumulated opacity A = sum_k alpha_k T_k (no background term), and the reverse pass takes dL/dD and dL/dA.
+//
+// Same layout as rasterize.cu: one CTA per 16x16 tile, the tile's list staged through shared memory in
+// batches, decisions taken on `power` in the fixed fp32 order of rule R3.  The record carries z in the slot
+// rasterize.cu leaves unused, so the feature costs no extra shared-memory read.
+#include "common.cuh"
+
+namespace xpr {
+namespace {
+
+constexpr int BLOCK = TILE * TILE;
+
+struct FeatParams {
+    int W, H, TW;
+    float amax, tmin;
+    float bg[3];
+    const uint32_t* order;
+};
+
+#ifndef XPR_FEAT_PPT_MIN_TILES
+#define XPR_FEAT_PPT_MIN_TILES 4096      // same switch as rasterize.cu: throughput shape for large images
+#endif
+
+__device__ __forceinline__ float opac_exp(float power, float l2o) {   // o exp(power) = ex2(power log2 e + log2 o)
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(fmaf(power, 1.4426950408889634f, l2o)));
+    return y;
+}
+
+__device__ __forceinline__ float fast_rcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Transposed butterfly over 8 per-lane values (9 shuffles); lane L with (L & 3) == 0 ends with the total of value L >> 2.
+__device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
+    float w[4], x[2];
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float send = b4 ? v[i] : v[i + 4], keep = b4 ? v[i + 4] : v[i];
+        w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const float send = b3 ? w[i] : w[i + 2], keep = b3 ? w[i + 2] : w[i];
+        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    const float send = b2 ? x[0] : x[1], keep = b2 ? x[1] : x[0];
+    float y = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    y += __shfl_xor_sync(0xffffffffu, y, 2);
+    y += __shfl_xor_sync(0xffffffffu, y, 1);
+    return y;
+}
+
+// Forward: colour, final T, n_contrib, D and A in one walk.  PPT pixels (x, y), (x + 8, y) per thread as in
+// rasterize_fwd_kernel; the blend is the branchy form (a gated pair costs the power evaluation only).
+template <int PPT>
+__global__ void __launch_bounds__(BLOCK / PPT)
+rasterize_feat_fwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
+                          const float* __restrict__ rgb, const float* __restrict__ lnv,
+                          const float* __restrict__ depth, const uint32_t* __restrict__ vals,
+                          const uint2* __restrict__ ranges, float* __restrict__ image, float* __restrict__ final_T,
+                          uint32_t* __restrict__ n_contrib, float* __restrict__ depth_img,
+                          float* __restrict__ alpha_img) {
+    constexpr int THREADS = BLOCK / PPT, BATCH = THREADS, ROW = TILE / PPT;
+    // record: (mx, my, qa, qb | qc, thr = -lnv, log2 o, z | r, g, b, -)
+    __shared__ float4 s_rec[3 * BATCH];
+    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
+    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int py = ty * TILE + (threadIdx.x / ROW);
+    const float pyc = (float)py + 0.5f;
+    const uint2 rg = ranges[tile];
+    const uint32_t len = rg.y - rg.x;
+
+    int px[PPT];
+    float pxc[PPT], T[PPT], C0[PPT], C1[PPT], C2[PPT], D[PPT], A[PPT];
+    uint32_t last[PPT];
+    bool in[PPT], act[PPT], any_act = false;
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+        px[k] = tx * TILE + (threadIdx.x % ROW) + 8 * k;
+        pxc[k] = (float)px[k] + 0.5f;
+        in[k] = (px[k] < P.W) && (py < P.H);
+        act[k] = in[k]; any_act |= act[k];
+        T[k] = 1.0f; C0[k] = C1[k] = C2[k] = D[k] = A[k] = 0.0f; last[k] = 0;
+    }
+    const float amax = P.amax, tmin = P.tmin;
+
+    for (uint32_t base = 0; base < len; base += BATCH) {
+        if (__syncthreads_or(any_act) == 0) break;
+        const uint32_t cnt = min((uint32_t)BATCH, len - base);
+        if (threadIdx.x < cnt) {
+            const uint32_t g = vals[rg.x + base + threadIdx.x];
+            const float2 m = mean2d[g];
+            const float4 co = conic_opac[g];
+            float4* rec = s_rec + 3 * threadIdx.x;
+            rec[0] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
+            rec[1] = make_float4(-0.5f * co.z, -lnv[g], __log2f(co.w), depth[g]);
+            rec[2] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
+        }
+        __syncthreads();
+        if (!any_act) continue;
+        const float4* rq = s_rec;
+        for (uint32_t j = 0; j < cnt && any_act; ++j, rq += 3) {
+            const float4 ge = rq[0], ga = rq[1];
+            const float dy = pyc - ge.y;
+            const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);
+            any_act = false;
+#pragma unroll
+            for (int k = 0; k < PPT; ++k) {
+                if (act[k]) {
+                    const float dx = pxc[k] - ge.x;
+                    const float power = __fmaf_rn(__fmaf_rn(ge.z, dx, t1), dx, t2);     // rule R3
+                    if (!(power > 0.0f) && !(power < ga.y)) {                            // C20, C12
+                        const float alpha = fminf(amax, opac_exp(power, ga.z));          // C11
+                        const float Tn = T[k] * (1.0f - alpha);
+                        if (Tn < tmin) {
+                            act[k] = false;                                              // stop, no blend
+                        } else {
+                            const float4 c = rq[2];
+                            const float w = alpha * T[k];
+                            C0[k] = fmaf(c.x, w, C0[k]); C1[k] = fmaf(c.y, w, C1[k]); C2[k] = fmaf(c.z, w, C2[k]);
+                            D[k] = fmaf(ga.w, w, D[k]);
+                            A[k] += w;
+                            T[k] = Tn;
+                            last[k] = base + j + 1;
+                        }
+                    }
+                }
+                any_act |= act[k];
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+        if (!in[k]) continue;
+        const int64_t pid = (int64_t)py * P.W + px[k];
+        image[3 * pid] = fmaf(T[k], P.bg[0], C0[k]);
+        image[3 * pid + 1] = fmaf(T[k], P.bg[1], C1[k]);
+        image[3 * pid + 2] = fmaf(T[k], P.bg[2], C2[k]);
+        final_T[pid] = T[k];
+        n_contrib[pid] = last[k];
+        depth_img[pid] = D[k];
+        alpha_img[pid] = A[k];
+    }
+}
+
+// Backward: rasterize_bwd_kernel plus the two features.  With gD = dL/dD, gA = dL/dA of the pixel and
+// SD = sum_{j>k} z_j alpha_j T_j, SA = sum_{j>k} alpha_j T_j behind the entry (no background term, C31):
+//   dL/dz_k     = alpha_k T_k gD
+//   dL/dalpha_k = T_k (g . c_k + gD z_k + gA) - (g . S + gD SD + gA SA) / (1 - alpha_k)
+// and from dL/dalpha on as the colour pass.  The per-pixel scalars h = gD z + gA ... are folded so that the
+// feature adds 2 FMAs to each of the two dot products and 2 FMAs for the running sums.
+template <int PPT>
+__global__ void __launch_bounds__(BLOCK / PPT, 2 * PPT)
+rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
+                          const float* __restrict__ rgb, const float* __restrict__ lnv,
+                          const float* __restrict__ depth, const uint32_t* __restrict__ vals,
+                          const uint2* __restrict__ ranges, const float* __restrict__ final_T,
+                          const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL,
+                          const float* __restrict__ dL_dD, const float* __restrict__ dL_dA,
+                          float* __restrict__ g_mean2d, float* __restrict__ g_conic, float* __restrict__ g_opac,
+                          float* __restrict__ g_rgb, float* __restrict__ g_depth) {
+    constexpr int THREADS = BLOCK / PPT, BATCH = THREADS;
+    __shared__ float4 s_geo[BATCH];    // mx, my, A, B
+    __shared__ float4 s_gate[BATCH];   // C, thr, o, index (bits)
+    __shared__ float4 s_col[BATCH];    // r, g, b, log2 o
+    __shared__ float s_z[BATCH];       // z
+    __shared__ uint32_t s_max[THREADS / 32];
+    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
+    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int lane = threadIdx.x & 31;
+    constexpr int TPR = TILE / PPT;
+    const int px0 = tx * TILE + (threadIdx.x % TPR) * PPT;
+    const int py = ty * TILE + (threadIdx.x / TPR);
+    const float pyc = (float)py + 0.5f;
+    const uint2 rg = ranges[tile];
+
+    uint32_t n[PPT];
+    float T[PPT], S0[PPT], S1[PPT], S2[PPT], SD[PPT], SA[PPT], g0[PPT], g1[PPT], g2[PPT], gD[PPT], gA[PPT], pxc[PPT];
+    uint32_t wmax = 0;
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+        const int px = px0 + k;
+        pxc[k] = (float)px + 0.5f;
+        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = gD[k] = gA[k] = 0.0f;
+        if (px < P.W && py < P.H) {
+            const int64_t pid = (int64_t)py * P.W + px;
+            n[k] = n_contrib[pid];
+            T[k] = final_T[pid];
+            g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
+            gD[k] = dL_dD[pid]; gA[k] = dL_dA[pid];
+        }
+        S0[k] = T[k] * P.bg[0]; S1[k] = T[k] * P.bg[1]; S2[k] = T[k] * P.bg[2];
+        SD[k] = 0.0f; SA[k] = 0.0f;
+        wmax = max(wmax, n[k]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+    if (lane == 0) s_max[threadIdx.x >> 5] = wmax;
+    __syncthreads();
+    uint32_t max_n = 0;
+#pragma unroll
+    for (int w = 0; w < THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
+
+    const int vi = lane >> 2;
+    float* const red_base = (vi < 2) ? (g_mean2d + vi) : (vi < 5) ? (g_conic + (vi - 2)) : (g_rgb + (vi - 5));
+    const uint32_t red_stride = (vi < 2) ? 2u : 3u;
+    const bool red_lane = (lane & 3) == 0;
+
+    for (uint32_t hi = max_n; hi > 0;) {
+        const uint32_t cnt = min((uint32_t)BATCH, hi);
+        __syncthreads();
+        if (threadIdx.x < cnt) {      // slot j holds list position hi-1-j (descending)
+            const uint32_t g = vals[rg.x + hi - 1 - threadIdx.x];
+            const float2 m = mean2d[g];
+            const float4 co = conic_opac[g];
+            s_geo[threadIdx.x] = make_float4(m.x, m.y, co.x, co.y);
+            s_gate[threadIdx.x] = make_float4(co.z, -lnv[g], co.w, __uint_as_float(g));
+            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], __log2f(co.w));
+            s_z[threadIdx.x] = depth[g];
+        }
+        __syncthreads();
+        for (uint32_t j = 0; j < cnt; ++j) {
+            const uint32_t pos = hi - 1 - j;
+            if (pos >= wmax) continue;     // warp-uniform
+            const float4 ge = s_geo[j];
+            const float4 ga = s_gate[j];
+            const float Ac = ge.z, Bc = ge.w, Cc = ga.x;
+            const float qa = -0.5f * Ac, qb = -Bc, qc = -0.5f * Cc;
+            const float dy = pyc - ge.y;
+            const float t1 = __fmul_rn(qb, dy), t2 = __fmul_rn(__fmul_rn(qc, dy), dy);
+            float dx[PPT], power[PPT];
+            bool contrib[PPT], any_c = false;
+#pragma unroll
+            for (int k = 0; k < PPT; ++k) {
+                dx[k] = pxc[k] - ge.x;
+                power[k] = __fmaf_rn(__fmaf_rn(qa, dx[k], t1), dx[k], t2);
+                contrib[k] = (pos < n[k]) && !(power[k] > 0.0f) && !(power[k] < ga.y);
+                any_c |= contrib[k];
+            }
+            if (!__any_sync(0xffffffffu, any_c)) continue;
+            const float4 c = s_col[j];
+            const float z = s_z[j];
+            float v[8];                                // mx my A B C r g b
+            v[5] = v[6] = v[7] = 0.f;
+            float sp = 0.f, spx = 0.f, spxx = 0.f, sz = 0.f;
+#pragma unroll
+            for (int k = 0; k < PPT; ++k) {            // branch-free: a pixel that does not contribute has alpha = 0
+                const float og = contrib[k] ? opac_exp(power[k], c.w) : 0.0f;
+                const float alpha = fminf(P.amax, og);
+                const float inv = fast_rcp(1.0f - alpha);
+                T[k] = T[k] * inv;
+                const float w = alpha * T[k];
+                v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
+                sz = fmaf(w, gD[k], sz);               // dL/dz
+                const float gc = fmaf(gD[k], z, fmaf(g2[k], c.z, fmaf(g1[k], c.y, fmaf(g0[k], c.x, gA[k]))));
+                const float gS = fmaf(gA[k], SA[k], fmaf(gD[k], SD[k], fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]))));
+                const float dalpha = fmaf(T[k], gc, -(inv * gS));
+                S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
+                SD[k] = fmaf(z, w, SD[k]); SA[k] += w;
+                const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
+                const float dpow = og * live;
+                const float dxp = dx[k] * dpow;
+                sp += dpow; spx += dxp; spxx = fmaf(dx[k], dxp, spxx);
+            }
+            {
+                const float sy = dy * sp;
+                v[0] = fmaf(Ac, spx, Bc * sy); v[1] = fmaf(Bc, spx, Cc * sy);
+                v[2] = -0.5f * spxx; v[3] = -dy * spx; v[4] = -0.5f * dy * sy;
+            }
+            const float tot = warp_reduce8(v, lane);
+            const float sp_tot = warp_sum(sp);
+            const float sz_tot = warp_sum(sz);
+            const uint32_t g = __float_as_uint(ga.w);
+            if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
+            if (lane == 0) atomicAdd(g_opac + g, sp_tot * fast_rcp(ga.z));
+            if (lane == 1) atomicAdd(g_depth + g, sz_tot);
+        }
+        hi -= cnt;
+    }
+}
+
+// z = (W mu + t)_z  =>  dL/dmu += W[2,:] dL/dz for a Gaussian that was not culled
+__global__ void depth_bwd_kernel(int64_t N, float w0, float w1, float w2, const uint32_t* __restrict__ tile_count,
+                                 const float* __restrict__ g_depth, float* __restrict__ g_means) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N || tile_count[i] == 0) return;
+    const float gz = g_depth[i];
+    g_means[3 * i] += w0 * gz; g_means[3 * i + 1] += w1 * gz; g_means[3 * i + 2] += w2 * gz;
+}
+
+void make_feat_params(const xpr_camera* cam, const xpr_config* cfg, FeatParams& P) {
+    P.W = cam->width; P.H = cam->height; P.TW = tiles_x(cam);
+    P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
+    for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
+    P.order = cfg->tile_order;
+}
+
+}  // namespace
+}  // namespace xpr
+
+using namespace xpr;
+
+extern "C" int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                          const float* conic_opac, const float* rgb, const float* lnv,
+                                          const float* depth, const uint32_t* vals_sorted,
+                                          const uint32_t* tile_ranges, float* image, float* final_T,
+                                          uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4) ||
+        !aligned(depth_img, 4) || !aligned(alpha_img, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+                  !aligned(depth, 4) || !aligned(vals_sorted, 4)))
+        return XPR_ERR_INVALID_ARG;
+    FeatParams P;
+    make_feat_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+#define XPR_FEAT_FWD(PPT_)                                                                                          \
+    rasterize_feat_fwd_kernel<PPT_><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                                    \
+        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, depth,    \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, depth_img, alpha_img)
+    if (T >= XPR_FEAT_PPT_MIN_TILES) XPR_FEAT_FWD(2); else XPR_FEAT_FWD(1);
+#undef XPR_FEAT_FWD
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                          const float* conic_opac, const float* rgb, const float* lnv,
+                                          const float* depth, const uint32_t* vals_sorted,
+                                          const uint32_t* tile_ranges, const float* final_T,
+                                          const uint32_t* n_contrib, const float* dL_dimage, const float* dL_ddepth,
+                                          const float* dL_dalpha, float* g_mean2d, float* g_conic, float* g_opac,
+                                          float* g_rgb, float* g_depth, int32_t zero_init, void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4) ||
+        !aligned(dL_ddepth, 4) || !aligned(dL_dalpha, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) || !aligned(depth, 4) ||
+        !aligned(vals_sorted, 4) || !aligned(g_mean2d, 4) || !aligned(g_conic, 4) || !aligned(g_opac, 4) ||
+        !aligned(g_rgb, 4) || !aligned(g_depth, 4))
+        return XPR_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (zero_init) {
+        const size_t n = (size_t)N;
+        if (g_conic == g_mean2d + 2 * n && g_opac == g_conic + 3 * n && g_rgb == g_opac + n && g_depth == g_rgb + 3 * n) {
+            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 10 * n, st));     // one allocation: one fill
+        } else {
+            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 2 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_conic, 0, sizeof(float) * 3 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_depth, 0, sizeof(float) * n, st));
+        }
+    }
+    FeatParams P;
+    make_feat_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+#define XPR_FEAT_BWD(PPT_)                                                                                          \
+    rasterize_feat_bwd_kernel<PPT_><<<T, BLOCK / PPT_, 0, st>>>(                                                      \
+        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, depth,    \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, dL_ddepth,          \
+        dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth)
+    if (T >= XPR_FEAT_PPT_MIN_TILES) XPR_FEAT_BWD(4); else XPR_FEAT_BWD(2);
+#undef XPR_FEAT_BWD
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_depth_bwd(int64_t N, const xpr_camera* cam, const uint32_t* tile_count, const float* g_depth,
+                                 float* g_means, void* stream) {
+    if (!cam || N < 0) return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(tile_count, 4) || !aligned(g_depth, 4) || !aligned(g_means, 4)) return XPR_ERR_INVALID_ARG;
+    const int threads = 256;
+    const int64_t blocks = (N + threads - 1) / threads;
+    depth_bwd_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(N, cam->w2c[8], cam->w2c[9], cam->w2c[10],
+                                                                              tile_count, g_depth, g_means);
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}

@@ -22,6 +22,10 @@ class SplatPipeline:
         self.device = torch.device(device)
         self.cam = cam if isinstance(cam, xb.XprCamera) else xb.make_camera(cam)
         self.ray_eval = bool(cfg.get("ray_eval", 0)) if isinstance(cfg, dict) else False
+        # f3: the compositing pass also renders the depth image and the accumulated opacity (2D evaluation only)
+        self.features = bool(cfg.get("features", 0)) if isinstance(cfg, dict) else False
+        if self.features and self.ray_eval:
+            raise ValueError("xpr: rendered features (f3) are built for the 2D evaluation, not for ray_eval")
         self._dL = None
         self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
         self.K = (int(self.cfg.sh_degree) + 1) ** 2
@@ -54,9 +58,11 @@ class SplatPipeline:
         # gradients (a9, a10)
         # the compositing gradients share one allocation, in the order the library checks for, so that
         # xpr_rasterize_bwd zero-fills them with a single memset
-        g2 = e(9 * N)
+        g2 = e(10 * N)                                     # ... | g_depth (f3) last
         self.g_mean2d, self.g_conic = g2[:2 * N].view(N, 2), g2[2 * N:5 * N].view(N, 3)
-        self.g_opac, self.g_rgb = g2[5 * N:6 * N], g2[6 * N:].view(N, 3)
+        self.g_opac, self.g_rgb, self.g_depth = g2[5 * N:6 * N], g2[6 * N:9 * N].view(N, 3), g2[9 * N:]
+        if self.features:
+            self.depth_img, self.alpha_img = e(self.H, self.W), e(self.H, self.W)
         self.g_means, self.g_scales, self.g_quats = e(N, 3), e(N, 3), e(N, 4)
         self.g_opacities, self.g_sh = e(N), e(N, self.K, 3)
         if self.ray_eval:   # f2: shader record, per-pixel rays, record gradient
@@ -141,10 +147,24 @@ class SplatPipeline:
                                      self.pixel_rays, self.vals_sorted, self.tile_ranges, self.image, self.final_T,
                                      self.n_contrib)
             return
+        if self.features:
+            xb.xpr_rasterize_feat_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.depth,
+                                      self.vals_sorted, self.tile_ranges, self.image, self.final_T, self.n_contrib,
+                                      self.depth_img, self.alpha_img)
+            return
         xb.xpr_rasterize_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
                              self.tile_ranges, self.image, self.final_T, self.n_contrib)
 
-    def rasterize_bwd(self, dL_dimage):
+    def rasterize_bwd(self, dL_dimage, dL_ddepth=None, dL_dalpha=None):
+        self._feat_bwd = False
+        if self.features and (dL_ddepth is not None or dL_dalpha is not None):
+            z = lambda t: torch.zeros(self.H, self.W, dtype=torch.float32, device=self.device) if t is None else t
+            xb.xpr_rasterize_feat_bwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.depth,
+                                      self.vals_sorted, self.tile_ranges, self.final_T, self.n_contrib, dL_dimage,
+                                      z(dL_ddepth), z(dL_dalpha), self.g_mean2d, self.g_conic, self.g_opac,
+                                      self.g_rgb, self.g_depth, zero_init=True)
+            self._feat_bwd = True
+            return
         if self.ray_eval:
             xb.xpr_rasterize_ray_bwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv,
                                      self.pixel_rays, self.vals_sorted, self.tile_ranges, self.final_T, self.n_contrib,
@@ -162,6 +182,8 @@ class SplatPipeline:
         if self.ray_eval:
             xb.xpr_ray_bwd(means, scales, quats, self.cam, self.tile_count, self.g_ray_rec, self.g_means,
                            self.g_scales, self.g_quats)
+        if getattr(self, "_feat_bwd", False):
+            xb.xpr_depth_bwd(self.cam, self.tile_count, self.g_depth, self.g_means)
 
     # ---- whole passes -------------------------------------------------------------------------
     def forward(self, means, scales, quats, opacities, sh):
@@ -172,8 +194,8 @@ class SplatPipeline:
         self.rasterize_fwd()
         return self.image
 
-    def backward(self, dL_dimage):
-        self.rasterize_bwd(dL_dimage)
+    def backward(self, dL_dimage, dL_ddepth=None, dL_dalpha=None):
+        self.rasterize_bwd(dL_dimage, dL_ddepth, dL_dalpha)
         self.project_bwd()
         return dict(g_means=self.g_means, g_scales=self.g_scales, g_quats=self.g_quats,
                     g_opacities=self.g_opacities, g_sh=self.g_sh)

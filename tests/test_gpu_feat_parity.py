@@ -1,0 +1,146 @@
+"""GPU parity of the rendered features (Table 2; reading C31):
+xpr_rasterize_feat_fwd / xpr_rasterize_feat_bwd / xpr_depth_bwd through the C-ABI binding against the CPU oracle
+(xpr_oracle_feat.inc, pinned by P15) on the same seeded inputs.
+
+Bars: colour image, final_T, n_contrib as the colour pass (1e-4 max abs; n_contrib bit-exact outside fragile
+pixels); accumulated opacity A within 1e-4 max abs; depth image D within 1e-4 * max(1, z_max) -- D is the colour
+blend with c := z, so its error scales with the largest depth on the lists; compositing gradients,
+g_depth included, every element within 1e-3 |ref| + 1e-6 + 2e-6 * mass; parameter gradients strict against the
+oracle's project_bwd + depth_bwd fed the same fp32 2D gradients.
+"""
+import numpy as np
+import pytest
+
+import parity_util as pu
+import xpr_oracle as xo
+from paper_2606_11529_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+PAIRS = (("g_mean2d", "g_mean2d"), ("g_conic", "g_conic"), ("g_opac", "g_opac_eff"), ("g_rgb", "g_rgb"),
+         ("g_depth", "g_depth"))
+PARAMS = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
+
+
+def feat_grads(scene, view, shape):
+    """Seeded dL/dD and dL/dA (a loss 'sum gD * D + sum gA * A'); the colour gradient is the config's own loss."""
+    rng = np.random.default_rng(4000 + 7 * scene.N % 1000 + view)
+    gD = rng.uniform(-1.0, 1.0, shape).astype(np.float32)
+    gA = rng.uniform(-1.0, 1.0, shape).astype(np.float32)
+    return gD, gA
+
+
+def feat_parity(scene, view=0, cfg_over=None):
+    import torch
+    over = dict(features=1)
+    if cfg_over:
+        over.update(cfg_over)
+    g = pu.run_gpu(scene, view, over)
+    pipe = g["pipe"]
+    o = pu.run_oracle(scene, view, cfg_over)
+    pu.compare_projection(g, o)
+    pu.compare_binning(g, o)
+    pu.compare_forward(g, o)                      # colour, final_T, n_contrib of the fused kernel
+    of = xo.rasterize_fwd_da(o["proj"], o["binned"], o["cam"], o["cfg"], np.float32)
+    ok = (o["fwd"]["fragile"] & pu.FRAG_EXIT) == 0
+    A_gpu, D_gpu = pipe.alpha_img.cpu().numpy(), pipe.depth_img.cpu().numpy()
+    errA = np.abs(A_gpu.astype(np.float64) - of["alpha_img"])
+    assert errA[ok].max(initial=0.0) <= pu.IMG_TOL, errA[ok].max()
+    vis = o["proj"]["tile_count"] > 0
+    zmax = max(1.0, float(o["proj"]["depth"][vis].max(initial=1.0)))
+    errD = np.abs(D_gpu.astype(np.float64) - of["depth_img"])
+    assert errD[ok].max(initial=0.0) <= pu.IMG_TOL * zmax, (errD[ok].max(), zmax)
+    # invariant at any size: A = 1 - T_final up to fp32 summation
+    assert np.abs(A_gpu + g["fwd"]["final_T"] - 1.0).max() <= 1e-4
+
+    H, W = ok.shape
+    _, dL = scenes.loss_and_grad(scene.loss, o["fwd"]["image"], scene.target(view))
+    gD, gA = feat_grads(scene, view, (H, W))
+    frag = (o["fwd"]["fragile"] & (pu.FRAG_EXIT | pu.FRAG_CLAMP)) != 0
+    dL = np.where(frag[..., None], 0.0, dL).astype(np.float32)
+    gD = np.where(frag, 0.0, gD).astype(np.float32); gA = np.where(frag, 0.0, gA).astype(np.float32)
+    args = (o["proj"], o["binned"], o["fwd"], dL, gD, gA, o["cam"], o["cfg"], np.float32)
+    og2 = xo.rasterize_bwd_da(*args)
+    mass = xo.rasterize_bwd_da(*args, mass=True)
+    dev = pipe.device
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    pipe.backward(t(dL), t(gD), t(gA))
+    torch.cuda.synchronize()
+    gg = {k: getattr(pipe, k).cpu().numpy() for k in [p[0] for p in PAIRS] + list(PARAMS)}
+    for kg, ko in PAIRS:                                       # compositing, every element
+        bad, err = pu.grad_violations(gg[kg], og2[ko], mass[ko])
+        assert bad.sum() == 0, f"{kg}: {bad.sum()} of {bad.size} outside tolerance, max err {err.max()}"
+    assert np.abs(og2["g_depth"]).max() > 0
+    # parameters: the oracle's project_bwd + depth_bwd fed the GPU's own fp32 2D gradients (stage isolation)
+    g2 = dict(g_mean2d=gg["g_mean2d"], g_conic=gg["g_conic"], g_opac_eff=gg["g_opac"], g_rgb=gg["g_rgb"])
+    iso = xo.project_bwd(scene.means, scene.scales, scene.quats, scene.opacities, scene.sh, o["cam"], o["cfg"], g2,
+                         np.float32)
+    iso["g_means"] = iso["g_means"] + xo.depth_bwd(o["proj"]["tile_count"], gg["g_depth"], o["cam"])
+    for k in PARAMS:
+        bad, err = pu.grad_violations(gg[k], iso[k])
+        assert bad.sum() == 0, f"{k} (stage-isolated): {bad.sum()} of {bad.size}, max err {err.max()}"
+    culled = ~vis
+    for k in PARAMS:
+        assert not np.any(gg[k][culled])
+    return g, o
+
+
+def test_feat_config1_tiny():
+    feat_parity(scenes.make_scene(1))
+
+
+def test_feat_config2_reduced():
+    feat_parity(scenes.make_scene(2, n_override=20000, image_override=(200, 200)))
+
+
+@pytest.mark.parametrize("view", [0, 1])
+def test_feat_config3_reduced(view):
+    feat_parity(scenes.make_scene(3, n_override=50000, image_override=(480, 270)), view)
+
+
+@pytest.mark.parametrize("wh", [(70, 50), (33, 17)])
+def test_feat_ragged(wh):
+    feat_parity(scenes.make_scene(1, image_override=wh))
+
+
+def test_feat_background_and_tile_cull():
+    feat_parity(scenes.make_scene(2, n_override=20000, image_override=(200, 200)), 0,
+                dict(bg=(0.2, 0.5, 0.9), tile_cull=1))
+
+
+def test_feat_config3_full_size_throughput_shape():
+    # 8160 tiles: the 2-pixels-per-thread forward and the 4-pixels-per-thread backward (the launch shape of the bench)
+    feat_parity(scenes.make_scene(3), 0, dict(tile_cull=1))
+
+
+def test_feat_zero_feature_gradients_reduce_to_colour_backward():
+    import torch
+    sc = scenes.make_scene(2, n_override=20000, image_override=(200, 200))
+    g = pu.run_gpu(sc, 0, dict(features=1))
+    pipe = g["pipe"]
+    rng = np.random.default_rng(7)
+    dL = torch.from_numpy(rng.uniform(-1, 1, (200, 200, 3)).astype(np.float32)).to(pipe.device)
+    z = torch.zeros(200, 200, device=pipe.device)
+    pipe.backward(dL, z, z)
+    a = {k: getattr(pipe, k).clone() for k in PARAMS}
+    assert not bool(pipe.g_depth.any())
+    pipe.backward(dL)                       # the colour kernel
+    for k in PARAMS:
+        ref = getattr(pipe, k)
+        # two kernels, two orders of fp32 atomics: a sanity bound (the element-wise bars are in feat_parity)
+        assert bool(((a[k] - ref).abs() <= 2e-3 * ref.abs() + 1e-4 * ref.abs().max()).all()), k
+
+
+def test_feat_everything_culled():
+    import torch
+    sc = scenes.make_scene(1, n_override=500)
+    sc.means[:, 2] -= 10.0          # all behind the camera
+    g = pu.run_gpu(sc, 0, dict(features=1, bg=(0.1, 0.2, 0.3)))
+    pipe = g["pipe"]
+    assert g["binned"]["num_pairs"] == 0
+    assert not bool(pipe.depth_img.any()) and not bool(pipe.alpha_img.any())
+    assert torch.all(pipe.final_T == 1.0)
+    one = torch.ones(64, 64, device=pipe.device)
+    pipe.backward(torch.ones(64, 64, 3, device=pipe.device), one, one)
+    for k in PARAMS + ("g_depth",):
+        assert not bool(getattr(pipe, k).any()), k
