@@ -51,14 +51,17 @@ __device__ __forceinline__ float fast_exp(float x) {   // ex2.approx(x * log2 e)
 #endif
 constexpr int FWD_PPT2_MIN_TILES = XPR_FWD_PPT2_MIN_TILES;
 
-template <bool STATS, int PPT, bool BF>
+// FEAT = true (xpr_rasterize_feat_fwd, reading C31): the same walk also blends the depth image
+// D = sum z alpha T and the accumulated opacity A = sum alpha T; z rides in the record's unused slot.
+template <bool STATS, int PPT, bool BF, bool FEAT = false>
 __global__ void __launch_bounds__(BLOCK / PPT)
 rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                      const float* __restrict__ rgb, const float* __restrict__ lnv,
                      const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                      float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
-                     unsigned long long* __restrict__ stats) {
-    // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, log2 o, - | r, g, b, -)
+                     unsigned long long* __restrict__ stats, const float* __restrict__ depth = nullptr,
+                     float* __restrict__ depth_img = nullptr, float* __restrict__ alpha_img = nullptr) {
+    // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, log2 o, z (FEAT) | r, g, b, -)
     constexpr int FWD_BATCH = BLOCK / PPT;          // one list entry staged per thread
     __shared__ float4 s_rec[3 * FWD_BATCH];
     const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
@@ -72,6 +75,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
 
     float Ta = 1.0f, Ca0 = 0.0f, Ca1 = 0.0f, Ca2 = 0.0f;     // pixel (px0, py)
     float Tb = 1.0f, Cb0 = 0.0f, Cb1 = 0.0f, Cb2 = 0.0f;     // pixel (px1, py)
+    float Da = 0.0f, Aa = 0.0f, Db = 0.0f, Ab = 0.0f;         // FEAT: depth image and accumulated opacity
     uint32_t last_a = 0, last_b = 0;
     bool act_a = in0, act_b = in1;                            // still compositing
     uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
@@ -92,12 +96,13 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             pw_b[u] = __fmaf_rn(__fmaf_rn(ge.z, dxb, t1), dxb, t2);                                  \
         }                                                                                            \
         thr[u] = ga.y; op[u] = ga.z;                                                                 \
+        if (FEAT) zz[u] = ga.w;                                                                      \
         if (BF) c_##u = (rp)[2];                                                                     \
     }
     // valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12)
     // BF (lists produced with tile_cull: > 90 % of the visited pairs pass the gate): branch-free -- a pixel that
     // is done or gated enters with alpha = 0, so T' = T >= t_min and w = 0; otherwise the gated pairs are branched over
-#define XPR_FWD_BLEND(act, power, u, rp, T, C0, C1, C2, last, pos)                                    \
+#define XPR_FWD_BLEND(act, power, u, rp, T, C0, C1, C2, last, pos, Dv, Av)                            \
     if (BF) {                                                                                        \
         if (STATS) {                                                                                 \
             if (act) { ++n_visit; if (!((power) > 0.0f) && !((power) < thr[u])) ++n_pass; }          \
@@ -110,6 +115,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
         act = act && !stop;                                                                          \
         const float w = blend ? alpha * T : 0.0f;                                                    \
         C0 = fmaf(c_##u.x, w, C0); C1 = fmaf(c_##u.y, w, C1); C2 = fmaf(c_##u.z, w, C2);             \
+        if (FEAT) { Dv = fmaf(zz[u], w, Dv); Av += w; }                                              \
         T = blend ? Tn : T;                                                                          \
         last = blend ? (pos) : last;                                                                 \
         if (STATS && blend) ++n_blend;                                                               \
@@ -125,6 +131,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                 const float4 c = (rp)[2];                                                            \
                 const float w = alpha * T;                                                           \
                 C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);                 \
+                if (FEAT) { Dv = fmaf(zz[u], w, Dv); Av += w; }                                      \
                 T = Tn;                                                                              \
                 last = (pos);                                                                        \
                 if (STATS) ++n_blend;                                                                \
@@ -132,11 +139,11 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
         }                                                                                            \
     }
 #define XPR_FWD_STEP(u, rp, pos)                                                                      \
-    XPR_FWD_BLEND(act_a, pw_a[u], u, rp, Ta, Ca0, Ca1, Ca2, last_a, pos)                              \
-    if (PPT == 2) XPR_FWD_BLEND(act_b, pw_b[u], u, rp, Tb, Cb0, Cb1, Cb2, last_b, pos)
+    XPR_FWD_BLEND(act_a, pw_a[u], u, rp, Ta, Ca0, Ca1, Ca2, last_a, pos, Da, Aa)                      \
+    if (PPT == 2) XPR_FWD_BLEND(act_b, pw_b[u], u, rp, Tb, Cb0, Cb1, Cb2, last_b, pos, Db, Ab)
 
     const float amax = P.amax, tmin = P.tmin;
-    float pw_a[4], pw_b[4], thr[4], op[4];
+    float pw_a[4], pw_b[4], thr[4], op[4], zz[4];
     float4 c_0, c_1, c_2, c_3;                         // colours of the group's entries
     for (uint32_t base = 0; base < len; base += FWD_BATCH) {
         if (__syncthreads_or(act_a || act_b) == 0) break;
@@ -147,7 +154,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             const float4 co = conic_opac[g];
             float4* rec = s_rec + 3 * e;
             rec[0] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-            rec[1] = make_float4(-0.5f * co.z, -lnv[g], __log2f(co.w), 0.0f);
+            rec[1] = make_float4(-0.5f * co.z, -lnv[g], __log2f(co.w), FEAT ? depth[g] : 0.0f);
             rec[2] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
         }
         __syncthreads();
@@ -182,6 +189,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
         image[3 * pid + 2] = fmaf(Ta, P.bg[2], Ca2);
         final_T[pid] = Ta;
         n_contrib[pid] = last_a;
+        if (FEAT) { depth_img[pid] = Da; alpha_img[pid] = Aa; }
     }
     if (in1) {
         const int64_t pid = (int64_t)py * P.W + px1;
@@ -190,6 +198,7 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
         image[3 * pid + 2] = fmaf(Tb, P.bg[2], Cb2);
         final_T[pid] = Tb;
         n_contrib[pid] = last_b;
+        if (FEAT) { depth_img[pid] = Db; alpha_img[pid] = Ab; }
     }
 }
 
@@ -403,6 +412,36 @@ extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cf
     const bool bf = cfg->tile_cull != 0;
     if (T >= FWD_PPT2_MIN_TILES) { if (bf) XPR_FWD(2, true); else XPR_FWD(2, false); }
     else                         { XPR_FWD(1, false); }      // latency shape: the branchy blend is shorter
+#undef XPR_FWD
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                          const float* conic_opac, const float* rgb, const float* lnv,
+                                          const float* depth, const uint32_t* vals_sorted,
+                                          const uint32_t* tile_ranges, float* image, float* final_T,
+                                          uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4) ||
+        !aligned(depth_img, 4) || !aligned(alpha_img, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+                  !aligned(depth, 4) || !aligned(vals_sorted, 4)))
+        return XPR_ERR_INVALID_ARG;
+    RasterParams P;
+    make_raster_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    // the launch shapes of xpr_rasterize_fwd
+#define XPR_FWD(PPT_, BF_)                                                                                          \
+    rasterize_fwd_kernel<false, PPT_, BF_, true><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                       \
+        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,           \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr, depth,         \
+        depth_img, alpha_img)
+    const bool bf = cfg->tile_cull != 0;
+    if (T >= FWD_PPT2_MIN_TILES) { if (bf) XPR_FWD(2, true); else XPR_FWD(2, false); }
+    else                         { XPR_FWD(1, false); }
 #undef XPR_FWD
     XPR_LAUNCH_CHECK();
     return XPR_OK;

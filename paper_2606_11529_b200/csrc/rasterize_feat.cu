@@ -1,4 +1,5 @@
-// rasterize_feat.cu -- xpr_rasterize_feat_fwd / xpr_rasterize_feat_bwd / xpr_depth_bwd: compositing with the
+// rasterize_feat.cu -- xpr_rasterize_feat_bwd / xpr_depth_bwd (the forward, xpr_rasterize_feat_fwd, is the FEAT
+// instantiation of rasterize_fwd_kernel in rasterize.cu): compositing with the
 // rendered features of SURVEY 8(f) f3 ("rendered features such as depth", Table 2; DESIGN.md
 // reading C31): next to the colour, the same walk blends the depth image D = sum_k z_k alpha_k T_k and the
 // accumulated opacity A = sum_k alpha_k T_k (no background term), and the reverse pass takes dL/dD and dL/dA.
@@ -36,12 +37,6 @@ __device__ __forceinline__ float fast_rcp(float x) {
     return y;
 }
 
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
 // Transposed butterfly over 8 per-lane values (9 shuffles); lane L with (L & 3) == 0 ends with the total of value L >> 2.
 __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
     float w[4], x[2];
@@ -63,107 +58,23 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
     return y;
 }
 
-// Forward: colour, final T, n_contrib, D and A in one walk.  PPT pixels (x, y), (x + 8, y) per thread as in
-// rasterize_fwd_kernel; the blend is the branchy form (a gated pair costs the power evaluation only).
-template <int PPT>
-__global__ void __launch_bounds__(BLOCK / PPT)
-rasterize_feat_fwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
-                          const float* __restrict__ rgb, const float* __restrict__ lnv,
-                          const float* __restrict__ depth, const uint32_t* __restrict__ vals,
-                          const uint2* __restrict__ ranges, float* __restrict__ image, float* __restrict__ final_T,
-                          uint32_t* __restrict__ n_contrib, float* __restrict__ depth_img,
-                          float* __restrict__ alpha_img) {
-    constexpr int THREADS = BLOCK / PPT, BATCH = THREADS, ROW = TILE / PPT;
-    // record: (mx, my, qa, qb | qc, thr = -lnv, log2 o, z | r, g, b, -)
-    __shared__ float4 s_rec[3 * BATCH];
-    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
-    const int tx = tile % P.TW, ty = tile / P.TW;
-    const int py = ty * TILE + (threadIdx.x / ROW);
-    const float pyc = (float)py + 0.5f;
-    const uint2 rg = ranges[tile];
-    const uint32_t len = rg.y - rg.x;
-
-    int px[PPT];
-    float pxc[PPT], T[PPT], C0[PPT], C1[PPT], C2[PPT], D[PPT], A[PPT];
-    uint32_t last[PPT];
-    bool in[PPT], act[PPT], any_act = false;
-#pragma unroll
-    for (int k = 0; k < PPT; ++k) {
-        px[k] = tx * TILE + (threadIdx.x % ROW) + 8 * k;
-        pxc[k] = (float)px[k] + 0.5f;
-        in[k] = (px[k] < P.W) && (py < P.H);
-        act[k] = in[k]; any_act |= act[k];
-        T[k] = 1.0f; C0[k] = C1[k] = C2[k] = D[k] = A[k] = 0.0f; last[k] = 0;
-    }
-    const float amax = P.amax, tmin = P.tmin;
-
-    for (uint32_t base = 0; base < len; base += BATCH) {
-        if (__syncthreads_or(any_act) == 0) break;
-        const uint32_t cnt = min((uint32_t)BATCH, len - base);
-        if (threadIdx.x < cnt) {
-            const uint32_t g = vals[rg.x + base + threadIdx.x];
-            const float2 m = mean2d[g];
-            const float4 co = conic_opac[g];
-            float4* rec = s_rec + 3 * threadIdx.x;
-            rec[0] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-            rec[1] = make_float4(-0.5f * co.z, -lnv[g], __log2f(co.w), depth[g]);
-            rec[2] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
-        }
-        __syncthreads();
-        if (!any_act) continue;
-        const float4* rq = s_rec;
-        for (uint32_t j = 0; j < cnt && any_act; ++j, rq += 3) {
-            const float4 ge = rq[0], ga = rq[1];
-            const float dy = pyc - ge.y;
-            const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);
-            any_act = false;
-#pragma unroll
-            for (int k = 0; k < PPT; ++k) {
-                if (act[k]) {
-                    const float dx = pxc[k] - ge.x;
-                    const float power = __fmaf_rn(__fmaf_rn(ge.z, dx, t1), dx, t2);     // rule R3
-                    if (!(power > 0.0f) && !(power < ga.y)) {                            // C20, C12
-                        const float alpha = fminf(amax, opac_exp(power, ga.z));          // C11
-                        const float Tn = T[k] * (1.0f - alpha);
-                        if (Tn < tmin) {
-                            act[k] = false;                                              // stop, no blend
-                        } else {
-                            const float4 c = rq[2];
-                            const float w = alpha * T[k];
-                            C0[k] = fmaf(c.x, w, C0[k]); C1[k] = fmaf(c.y, w, C1[k]); C2[k] = fmaf(c.z, w, C2[k]);
-                            D[k] = fmaf(ga.w, w, D[k]);
-                            A[k] += w;
-                            T[k] = Tn;
-                            last[k] = base + j + 1;
-                        }
-                    }
-                }
-                any_act |= act[k];
-            }
-        }
-    }
-#pragma unroll
-    for (int k = 0; k < PPT; ++k) {
-        if (!in[k]) continue;
-        const int64_t pid = (int64_t)py * P.W + px[k];
-        image[3 * pid] = fmaf(T[k], P.bg[0], C0[k]);
-        image[3 * pid + 1] = fmaf(T[k], P.bg[1], C1[k]);
-        image[3 * pid + 2] = fmaf(T[k], P.bg[2], C2[k]);
-        final_T[pid] = T[k];
-        n_contrib[pid] = last[k];
-        depth_img[pid] = D[k];
-        alpha_img[pid] = A[k];
-    }
-}
-
 // Backward: rasterize_bwd_kernel plus the two features.  With gD = dL/dD, gA = dL/dA of the pixel and
 // SD = sum_{j>k} z_j alpha_j T_j, SA = sum_{j>k} alpha_j T_j behind the entry (no background term, C31):
 //   dL/dz_k     = alpha_k T_k gD
 //   dL/dalpha_k = T_k (g . c_k + gD z_k + gA) - (g . S + gD SD + gA SA) / (1 - alpha_k)
-// and from dL/dalpha on as the colour pass.  The per-pixel scalars h = gD z + gA ... are folded so that the
-// feature adds 2 FMAs to each of the two dot products and 2 FMAs for the running sums.
+// and from dL/dalpha on as the colour pass.  SA telescopes (alpha_j T_j = T_j - T_{j+1}):
+//   SA_k = T_k (1 - alpha_k) - T_final   =>   gA (T_k - SA_k / (1 - alpha_k)) = gA T_final / (1 - alpha_k),
+// so the accumulated-opacity term is the per-pixel constant gA T_final entering the "behind" dot product with a
+// minus sign: no running sum, no cancellation.  The depth term adds one FMA to each dot product, one to SD and
+// one to dL/dz.  sum dpow (dL/do) and dL/dz share one butterfly (6 shuffles for the two).
+#ifndef XPR_FEAT_BWD_PPT
+#define XPR_FEAT_BWD_PPT 4          // pixels per thread in the throughput shape
+#endif
+#ifndef XPR_FEAT_BWD_MINB
+#define XPR_FEAT_BWD_MINB 10        // 64-thread CTAs per SM at 4 pixels per thread
+#endif
 template <int PPT>
-__global__ void __launch_bounds__(BLOCK / PPT, 2 * PPT)
+__global__ void __launch_bounds__(BLOCK / PPT, XPR_FEAT_BWD_MINB * PPT / 4)
 rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                           const float* __restrict__ rgb, const float* __restrict__ lnv,
                           const float* __restrict__ depth, const uint32_t* __restrict__ vals,
@@ -188,22 +99,22 @@ rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const
     const uint2 rg = ranges[tile];
 
     uint32_t n[PPT];
-    float T[PPT], S0[PPT], S1[PPT], S2[PPT], SD[PPT], SA[PPT], g0[PPT], g1[PPT], g2[PPT], gD[PPT], gA[PPT], pxc[PPT];
+    float T[PPT], S0[PPT], S1[PPT], S2[PPT], SD[PPT], g0[PPT], g1[PPT], g2[PPT], gD[PPT], gAT[PPT], pxc[PPT];
     uint32_t wmax = 0;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
         const int px = px0 + k;
         pxc[k] = (float)px + 0.5f;
-        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = gD[k] = gA[k] = 0.0f;
+        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = gD[k] = gAT[k] = 0.0f;
         if (px < P.W && py < P.H) {
             const int64_t pid = (int64_t)py * P.W + px;
             n[k] = n_contrib[pid];
             T[k] = final_T[pid];
             g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
-            gD[k] = dL_dD[pid]; gA[k] = dL_dA[pid];
+            gD[k] = dL_dD[pid]; gAT[k] = dL_dA[pid] * T[k];      // gA T_final
         }
         S0[k] = T[k] * P.bg[0]; S1[k] = T[k] * P.bg[1]; S2[k] = T[k] * P.bg[2];
-        SD[k] = 0.0f; SA[k] = 0.0f;
+        SD[k] = 0.0f;
         wmax = max(wmax, n[k]);
     }
 #pragma unroll
@@ -265,11 +176,11 @@ rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const
                 const float w = alpha * T[k];
                 v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
                 sz = fmaf(w, gD[k], sz);               // dL/dz
-                const float gc = fmaf(gD[k], z, fmaf(g2[k], c.z, fmaf(g1[k], c.y, fmaf(g0[k], c.x, gA[k]))));
-                const float gS = fmaf(gA[k], SA[k], fmaf(gD[k], SD[k], fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]))));
+                const float gc = fmaf(gD[k], z, fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x)));
+                const float gS = fmaf(gD[k], SD[k], fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], fmaf(g0[k], S0[k], -gAT[k]))));
                 const float dalpha = fmaf(T[k], gc, -(inv * gS));
                 S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
-                SD[k] = fmaf(z, w, SD[k]); SA[k] += w;
+                SD[k] = fmaf(z, w, SD[k]);
                 const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
                 const float dpow = og * live;
                 const float dxp = dx[k] * dpow;
@@ -281,12 +192,14 @@ rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const
                 v[2] = -0.5f * spxx; v[3] = -dy * spx; v[4] = -0.5f * dy * sy;
             }
             const float tot = warp_reduce8(v, lane);
-            const float sp_tot = warp_sum(sp);
-            const float sz_tot = warp_sum(sz);
+            // lanes 0-15 end with the warp total of sp, lanes 16-31 with that of sz
+            float r2 = ((lane & 16) ? sz : sp) + __shfl_xor_sync(0xffffffffu, (lane & 16) ? sp : sz, 16);
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
             const uint32_t g = __float_as_uint(ga.w);
             if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
-            if (lane == 0) atomicAdd(g_opac + g, sp_tot * fast_rcp(ga.z));
-            if (lane == 1) atomicAdd(g_depth + g, sz_tot);
+            if (lane == 0) atomicAdd(g_opac + g, r2 * fast_rcp(ga.z));
+            if (lane == 16) atomicAdd(g_depth + g, r2);
         }
         hi -= cnt;
     }
@@ -312,32 +225,6 @@ void make_feat_params(const xpr_camera* cam, const xpr_config* cfg, FeatParams& 
 }  // namespace xpr
 
 using namespace xpr;
-
-extern "C" int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                                          const float* conic_opac, const float* rgb, const float* lnv,
-                                          const float* depth, const uint32_t* vals_sorted,
-                                          const uint32_t* tile_ranges, float* image, float* final_T,
-                                          uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
-    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
-    if (N < 0) return XPR_ERR_INVALID_ARG;
-    if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4) ||
-        !aligned(depth_img, 4) || !aligned(alpha_img, 4))
-        return XPR_ERR_INVALID_ARG;
-    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-                  !aligned(depth, 4) || !aligned(vals_sorted, 4)))
-        return XPR_ERR_INVALID_ARG;
-    FeatParams P;
-    make_feat_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
-#define XPR_FEAT_FWD(PPT_)                                                                                          \
-    rasterize_feat_fwd_kernel<PPT_><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                                    \
-        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, depth,    \
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, depth_img, alpha_img)
-    if (T >= XPR_FEAT_PPT_MIN_TILES) XPR_FEAT_FWD(2); else XPR_FEAT_FWD(1);
-#undef XPR_FEAT_FWD
-    XPR_LAUNCH_CHECK();
-    return XPR_OK;
-}
 
 extern "C" int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
                                           const float* conic_opac, const float* rgb, const float* lnv,
@@ -377,7 +264,7 @@ extern "C" int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_confi
         P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, depth,    \
         vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, dL_ddepth,          \
         dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth)
-    if (T >= XPR_FEAT_PPT_MIN_TILES) XPR_FEAT_BWD(4); else XPR_FEAT_BWD(2);
+    if (T >= XPR_FEAT_PPT_MIN_TILES) XPR_FEAT_BWD(XPR_FEAT_BWD_PPT); else XPR_FEAT_BWD(2);
 #undef XPR_FEAT_BWD
     XPR_LAUNCH_CHECK();
     return XPR_OK;
