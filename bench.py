@@ -46,6 +46,9 @@ def parse():
     ap.add_argument("--tile-order", type=int, default=-1, choices=(-1, 0, 1),
                     help="1: compositing kernels walk the tiles longest list first (xpr_config.tile_order; scheduling "
                          "only); -1: the pipeline's default (on for 64 <= tiles < 4096)")
+    ap.add_argument("--features", type=int, default=0, choices=(0, 1),
+                    help="1: also render the depth image and the accumulated opacity and take their gradients "
+                         "(SURVEY 8(f) f3, DESIGN.md 6.8; 2D evaluation only; not part of the headline workload)")
     ap.add_argument("--ray-eval", type=int, default=0, choices=(0, 1),
                     help="1: XPR-3DGUT evaluation along the pixel ray (SURVEY 8(f) f2; meant for --config 4) instead of "
                          "the 2D conic of north_star")
@@ -116,7 +119,7 @@ def aggregate_value(world: int, megapixels: float, ms_per_step: float) -> float:
     return world * megapixels / (ms_per_step / 1e3)
 
 
-def oracle_step(xo, scenes, sc, view, np, tile_cull=0, ray_eval=0):
+def oracle_step(xo, scenes, sc, view, np, tile_cull=0, ray_eval=0, features=0):
     """One fwd+bwd step of the CPU oracle, as it stands (never tuned)."""
     cam = xo.make_camera(sc.cameras[view])
     cfg = xo.make_config(dict(scenes.default_render_config(sc), tile_cull=tile_cull))
@@ -125,7 +128,12 @@ def oracle_step(xo, scenes, sc, view, np, tile_cull=0, ray_eval=0):
     t0 = time.perf_counter()
     r = render(arrays, cam, cfg, np.float32)
     _, dL = scenes.loss_and_grad(sc.loss, r["fwd"]["image"], sc.target(view))
-    backward(arrays, r, dL, cam, cfg, np.float32)
+    if features:     # f3: the depth / accumulated-opacity pass and the backward with their (here constant) gradients
+        r["fwd"].update(xo.rasterize_fwd_da(r["proj"], r["binned"], cam, cfg, np.float32))
+        one = np.ones(r["fwd"]["image"].shape[:2], np.float32)
+        xo.backward_da(arrays, r, dL, one, one, cam, cfg, np.float32)
+    else:
+        backward(arrays, r, dL, cam, cfg, np.float32)
     return time.perf_counter() - t0, r["binned"]["num_pairs"]
 
 
@@ -155,10 +163,10 @@ def run_reference(args):
     from paper_2606_11529_b200 import scenes
     sc, w, h, desc = oracle_sample(args)
     for _ in range(args.warmup):
-        oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval)
+        oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval, args.features)
     t = 0.0
     for _ in range(args.steps):
-        dt, I = oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval)
+        dt, I = oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval, args.features)
         t += dt
     ms = 1e3 * t / max(args.steps, 1)
     val = (w * h / 1e6) / (ms / 1e3)
@@ -166,7 +174,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config], "view": args.view, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "sample": desc,
+            "config": {"workload": WORKLOADS[args.config], "view": args.view, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "sample": desc,
                        "pairs": int(I)},
             "gaussians_per_s": sc.N / (ms / 1e3),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
@@ -181,6 +189,8 @@ BWD_OPS_VISIT, BWD_OPS_PASS = 8, 45
 # f2 (ray evaluation): d_c 9 + cross 6 + two squared norms 6 + 1 + two thresholds and compares 4
 RAY_FWD_OPS_VISIT, RAY_FWD_OPS_PASS = 26, 12
 RAY_BWD_OPS_VISIT, RAY_BWD_OPS_PASS = 26, 57
+# f3 (depth + accumulated opacity): 2 more lane-ops per blended pair forward, 4 more backward
+FEAT_FWD_EXTRA, FEAT_BWD_EXTRA = 2, 4
 SMS, LANES_PER_SM = 148, 128
 
 
@@ -201,14 +211,20 @@ def run_ours(args):
 
     sc = scenes.make_scene(args.config)
     cam = sc.cameras[args.view]
+    if args.features and args.ray_eval:
+        raise SystemExit("bench.py: --features 1 is built for the 2D evaluation (not with --ray-eval 1)")
     cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval,
-               tile_order=args.tile_order)
+               tile_order=args.tile_order, features=args.features)
     params = pipeline.scene_to_device(sc, dev)
     target = torch.from_numpy(sc.target(args.view)).to(dev)
     pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     dL_buf = torch.empty_like(target)
+    if args.features:    # loss + sum gD D + sum gA A with seeded constant gD, gA ~ U[-1, 1] (linear in the features)
+        gen = torch.Generator(device="cpu").manual_seed(4000 + args.config)
+        pipe.feature_grads = tuple((torch.rand(cam.height, cam.width, generator=gen) * 2 - 1).to(dev) for _ in range(2))
+    feat_grads = pipe.feature_grads or (None, None)
 
     def loss_grad(image):
         """dL/dimage of the config's loss (sum |I - target| or sum (I - target)^2), one pass (xpr_loss_grad)."""
@@ -228,7 +244,7 @@ def run_ours(args):
         ev(); pipe.bin_sort() if sync_count else pipe.bin_sort_async()
         ev(); pipe.rasterize_fwd()
         ev(); dL = loss_grad(pipe.image)
-        ev(); pipe.rasterize_bwd(dL)
+        ev(); pipe.rasterize_bwd(dL, *feat_grads)
         ev(); pipe.project_bwd()
         ev()
 
@@ -256,6 +272,8 @@ def run_ours(args):
     launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1 + 1      # + loss_grad
     if args.ray_eval:
         launches_per_step += 3              # pixel_info, project_ray, ray_bwd
+    if args.features:
+        launches_per_step += 1              # depth_bwd
     if pipe.tile_order is not None:
         launches_per_step += 1              # tile_order_kernel at the end of xpr_bin_sort
     n_rows = pipe.rows_on_device()
@@ -291,6 +309,8 @@ def run_ours(args):
     bwd_ops = (RAY_BWD_OPS_VISIT, RAY_BWD_OPS_PASS) if args.ray_eval else (BWD_OPS_VISIT, BWD_OPS_PASS)
     kname = "rasterize_ray_%s_kernel" if args.ray_eval else "rasterize_%s_kernel"
     visit, passed, blended, sum_n = [int(v) for v in stats.cpu().tolist()]
+    feat_fwd_ops = FEAT_FWD_EXTRA * blended if args.features else 0
+    feat_bwd_ops = FEAT_BWD_EXTRA * blended if args.features else 0
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -306,17 +326,19 @@ def run_ours(args):
     sort_bytes = (8 * sc.N + (4 * 16 + 20) * n_vis + 36 * n_rows
                   + n_pairs * (8 + 16 * (tile_passes - 1) + 20))
     rooflines = {
-        "rasterize_fwd": {"kernel": kname % "fwd", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
-                          "achieved": (fwd_ops[0] * visit + fwd_ops[1] * passed) / sec("rasterize_fwd") / 1e12},
-        "rasterize_bwd": {"kernel": kname % "bwd", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak,
-                          "achieved": (bwd_ops[0] * sum_n + bwd_ops[1] * blended) / sec("rasterize_bwd") / 1e12},
+        "rasterize_fwd": {"kernel": (kname % "fwd") + ("<FEAT>" if args.features else ""), "bound": "alu",
+                          "unit": "T lane-op/s", "peak": alu_peak,
+                          "achieved": (fwd_ops[0] * visit + fwd_ops[1] * passed + feat_fwd_ops) / sec("rasterize_fwd") / 1e12},
+        "rasterize_bwd": {"kernel": "rasterize_feat_bwd_kernel" if args.features else kname % "bwd", "bound": "alu",
+                          "unit": "T lane-op/s", "peak": alu_peak,
+                          "achieved": (bwd_ops[0] * sum_n + bwd_ops[1] * blended + feat_bwd_ops) / sec("rasterize_bwd") / 1e12},
         "bin_sort": {"kernel": "xpr_bin_sort%s (compact, 4 depth passes on Gaussians, row scan, rows, pair scan, emit, "
                                "%d tile passes on pairs, ranges)" % ("_cull" if args.tile_cull else "", tile_passes), "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
                      "achieved": sort_bytes / sec("bin_sort") / 1e9, "algorithmic_bytes": sort_bytes},
     }
     traffic = {}
     try:   # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed ncu captures (profiles/ncu_traffic.md)
-        key = "config%d%s" % (args.config, "_ray" if args.ray_eval else "")
+        key = "config%d%s" % (args.config, "_ray" if args.ray_eval else "_feat" if args.features else "")
         for ln in open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")).read().splitlines()[1:]:
             w, stage, b = ln.split(",")
             if w == key:
@@ -358,6 +380,8 @@ def run_ours(args):
         host_in = [torch.from_numpy(a).pin_memory() for a in (sc.means, sc.scales, sc.quats, sc.opacities, sc.sh)]
         dev_in = [torch.empty_like(p) for p in params]
         outs = [pipe.image, pipe.g_means, pipe.g_scales, pipe.g_quats, pipe.g_opacities, pipe.g_sh]
+        if args.features:
+            outs += [pipe.depth_img, pipe.alpha_img]
         host_out = [torch.empty(o.shape, dtype=o.dtype).pin_memory() for o in outs]
         h2d = sum(t.numel() * t.element_size() for t in host_in)
         d2h = sum(t.numel() * t.element_size() for t in host_out)
@@ -367,7 +391,7 @@ def run_ours(args):
             if args.ray_eval:
                 pipe.pixel_info(); pipe.project_ray()
             pipe.bin_sort_async(); pipe.rasterize_fwd()
-            pipe.rasterize_bwd(loss_grad(pipe.image)); pipe.project_bwd()
+            pipe.rasterize_bwd(loss_grad(pipe.image), *feat_grads); pipe.project_bwd()
 
         def e2e_step():       # one stream: copy in, step, copy out (the latency of a single step)
             for d, h in zip(dev_in, host_in):
@@ -445,7 +469,7 @@ def run_ours(args):
         sys.path.insert(0, os.path.join(ROOT, "oracle"))
         import xpr_oracle as xo
         osc, w, h, desc = oracle_sample(args)
-        dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull, args.ray_eval)
+        dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull, args.ray_eval, args.features)
         cpu = {"value": (w * h / 1e6) / dt, "unit": UNIT, "cores": xo.num_threads(), "kind": "oracle", "sample": desc,
                "seconds": dt}
 
@@ -454,7 +478,7 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
+                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
                            "candidate_pairs": n_cand, "rows": n_rows, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "tile_digits_on_pairs": tile_passes},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",

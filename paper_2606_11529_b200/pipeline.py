@@ -27,6 +27,8 @@ class SplatPipeline:
         if self.features and self.ray_eval:
             raise ValueError("xpr: rendered features (f3) are built for the 2D evaluation, not for ray_eval")
         self._dL = None
+        # f3: constant (dL/dD, dL/dA) of a loss that is linear in the features; step_async() feeds them to the backward
+        self.feature_grads = None
         self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
         self.K = (int(self.cfg.sh_degree) + 1) ** 2
         self.W, self.H = int(self.cam.width), int(self.cam.height)
@@ -214,7 +216,7 @@ class SplatPipeline:
         self.bin_sort_async()
         self.rasterize_fwd()
         xb.xpr_loss_grad(loss, self.image, target, self._dL)
-        self.rasterize_bwd(self._dL)
+        self.rasterize_bwd(self._dL, *(self.feature_grads or (None, None)))
         self.project_bwd()
 
     def capture_step(self, means, scales, quats, opacities, sh, target, loss: str, pixel_info: bool = False):

@@ -108,6 +108,34 @@ def test_ray_entry_points_reject_bad_arguments(lib):
                                      one, one, one, null) == 4
 
 
+def test_feature_entry_points_reject_bad_arguments(lib):
+    """f3 (xpr_rasterize_feat_fwd / _bwd, xpr_depth_bwd): the argument checks come before any launch."""
+    cam, cfg = _cam_cfg()
+    null = C.c_void_p(0)
+    one = C.c_void_p(16)
+    odd = C.c_void_p(18)          # not 4-byte aligned
+    N4, N0, Nm = C.c_int64(4), C.c_int64(0), C.c_int64(-1)
+    fwd = lambda n, *a: lib.xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg), n, *a, null)
+    # mean2d conic_opac rgb lnv depth vals ranges image final_T n_contrib depth_img alpha_img
+    assert fwd(Nm, *[one] * 12) == 1
+    assert fwd(N4, one, one, one, one, null, one, one, one, one, one, one, one) == 1        # depth NULL
+    assert fwd(N4, *[one] * 10, null, one) == 1                                              # depth_img NULL
+    assert fwd(N4, *[one] * 11, odd) == 1                                                    # alpha_img misaligned
+    assert lib.xpr_rasterize_feat_fwd(None, C.byref(cfg), N4, *[one] * 12, null) == 1
+    cfg8 = type(cfg)(); C.memmove(C.byref(cfg8), C.byref(cfg), C.sizeof(cfg)); cfg8.tile = 8
+    assert lib.xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg8), N4, *[one] * 12, null) == 4
+    bwd = lambda n, *a: lib.xpr_rasterize_feat_bwd(C.byref(cam), C.byref(cfg), n, *a, C.c_int32(1), null)
+    # mean2d conic_opac rgb lnv depth vals ranges final_T n_contrib dL dL_dD dL_dA g_mean2d g_conic g_opac g_rgb g_depth
+    assert bwd(Nm, *[one] * 17) == 1
+    assert bwd(N4, *[one] * 10, null, *[one] * 6) == 1                                       # dL_ddepth NULL
+    assert bwd(N4, *[one] * 16, null) == 1                                                   # g_depth NULL
+    assert bwd(N0, *[null] * 6, one, one, one, one, one, one, *[null] * 5) == 0              # N = 0: nothing to do
+    assert lib.xpr_depth_bwd(Nm, C.byref(cam), one, one, one, null) == 1
+    assert lib.xpr_depth_bwd(N4, None, one, one, one, null) == 1
+    assert lib.xpr_depth_bwd(N4, C.byref(cam), one, null, one, null) == 1
+    assert lib.xpr_depth_bwd(N0, C.byref(cam), null, null, null, null) == 0
+
+
 def test_workspace_size_monotone(lib):
     from paper_2606_11529_b200 import binding as xb
     a = xb.xpr_bin_sort_workspace(1000, 10_000, 16)

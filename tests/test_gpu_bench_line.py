@@ -46,3 +46,11 @@ def test_bench_line_ray_evaluation():
     assert d["config"]["ray_eval"] == 1 and d["value"] > 0
     assert d["roofline"]["kernel"].startswith("rasterize_ray_")
     assert d["gpu_launches"] == 3 * (17 + 3)    # 1080p: two tile-digit passes; + pixel_info, project_ray, ray_bwd
+
+
+def test_bench_line_rendered_features():
+    d = _run("--config", "3", "--features", "1", "--no-cpu-baseline")
+    assert d["config"]["features"] == 1 and d["value"] > 0
+    assert d["rooflines"]["rasterize_bwd"]["kernel"] == "rasterize_feat_bwd_kernel"
+    assert d["gpu_launches"] == 3 * (17 + 1)    # + depth_bwd
+    assert d["e2e"]["d2h_bytes_per_step"] > 1920 * 1080 * 4 * 5    # image, D and A all come back
