@@ -201,6 +201,27 @@ XO_RAY_DECL(f64, double)
 XO_FEAT_DECL(f32, float)
 XO_FEAT_DECL(f64, double)
 
+/* N-channel features (same section; pin P16): feat [N*C], feat_img [H*W*C] = sum_k feat[g_k,:] alpha_k T_k over the
+ * colour pass's contributing sequence, no background (rgb is only an argument of the shared walk and does not
+ * influence the result).  The backward takes dL/dfeat_img ALONE and returns that part of g_mean2d, g_conic, g_opac_eff
+ * plus g_feat [N*C]; colour / D / A parts of a loss add (every step is linear in the incoming gradient). */
+#define XO_FEATN_DECL(S, T)                                                                              \
+    void xpr_oracle_rasterize_fwd_featn_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,       \
+                                            const T* mean2d, const T* conic, const T* opac_eff,          \
+                                            const T* rgb, const T* lnv, const T* feat, int32_t C,        \
+                                            const uint32_t* vals_sorted, const uint32_t* tile_ranges,    \
+                                            T* feat_img);                                                \
+    void xpr_oracle_rasterize_bwd_featn_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,       \
+                                            const T* mean2d, const T* conic, const T* opac_eff,          \
+                                            const T* rgb, const T* lnv, const T* feat, int32_t C,        \
+                                            const uint32_t* vals_sorted, const uint32_t* tile_ranges,    \
+                                            const uint32_t* n_contrib, const T* dL_dfeat,                \
+                                            double* g_mean2d, double* g_conic, double* g_opac_eff,       \
+                                            double* g_feat);
+
+XO_FEATN_DECL(f32, float)
+XO_FEATN_DECL(f64, double)
+
 /* z = (W mu + t)_z: WRITES g_means [N*3] = W[2,:] g_depth (zeros where tile_count == 0); the caller adds it to
  * project_bwd's g_means. */
 void xpr_oracle_depth_bwd(int64_t N, const xo_camera* cam, const uint32_t* tile_count, const double* g_depth,

@@ -387,6 +387,39 @@ def rasterize_bwd_da(proj: dict, binned: dict, fwd: dict, dL_dimage, dL_ddepth, 
     return out
 
 
+def rasterize_fwd_featn(proj: dict, binned: dict, feat, cam: XoCamera, cfg: XoConfig, dtype=np.float32):
+    """N-channel feature image [H,W,C] = sum_k feat[g_k,:] alpha_k T_k (no background); feat [N,C]."""
+    dt = np.dtype(dtype)
+    H, W = int(cam.height), int(cam.width)
+    N = int(proj["tile_count"].shape[0])
+    f = np.ascontiguousarray(feat, dt).reshape(N, -1)
+    Cn = int(f.shape[1])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv")]
+    out = np.empty((H, W, Cn), dt)
+    fn = getattr(lib(), "xpr_oracle_rasterize_fwd_featn_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(f), C.c_int32(Cn), _p(binned["vals"]),
+       _p(binned["ranges"]), _p(out))
+    return out
+
+
+def rasterize_bwd_featn(proj: dict, binned: dict, fwd: dict, feat, dL_dfeat, cam: XoCamera, cfg: XoConfig,
+                        dtype=np.float32) -> dict:
+    """The feature part of the compositing gradients (fp64) for dL/dfeat_img [H,W,C] alone, plus g_feat [N,C]."""
+    dt = np.dtype(dtype)
+    N = int(proj["tile_count"].shape[0])
+    f = np.ascontiguousarray(feat, dt).reshape(N, -1)
+    Cn = int(f.shape[1])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv")]
+    d = np.ascontiguousarray(dL_dfeat, dt)
+    out = dict(g_mean2d=np.empty((N, 2), np.float64), g_conic=np.empty((N, 3), np.float64),
+               g_opac_eff=np.empty(N, np.float64), g_feat=np.empty((N, Cn), np.float64))
+    fn = getattr(lib(), "xpr_oracle_rasterize_bwd_featn_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(f), C.c_int32(Cn), _p(binned["vals"]),
+       _p(binned["ranges"]), _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), _p(d),
+       *[_p(out[k]) for k in ("g_mean2d", "g_conic", "g_opac_eff", "g_feat")])
+    return out
+
+
 def depth_bwd(tile_count, g_depth, cam: XoCamera):
     N = int(tile_count.shape[0])
     g = np.ascontiguousarray(g_depth, np.float64)

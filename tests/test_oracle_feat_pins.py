@@ -121,3 +121,91 @@ def test_p15_finite_differences(which):
         err = np.abs(fd - an)
         tol = 2e-6 * np.maximum(np.abs(an), np.abs(fd)) + 1e-7 * scale_all + 1e-9
         assert not (err > tol).any(), (k, np.argwhere(err > tol)[:5], fd[err > tol][:5], an[err > tol][:5])
+
+
+# ---- P16: N-channel features (xpr_oracle_rasterize_fwd_featn / _bwd_featn) -------------------------------------------
+
+def test_p16_three_channels_are_the_colour_pass():
+    # C = 3, feat = rgb, bg = 0: forward and backward reproduce the pinned colour pass (P1, P2, P6)
+    arr, co = _scene(21, opac_boost=1.0)
+    cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=1, bg=(0.0, 0.0, 0.0)))
+    for dtype in (np.float32, np.float64):
+        r = xo.render(arr, cam, cfg, dtype)
+        F = xo.rasterize_fwd_featn(r["proj"], r["binned"], r["proj"]["rgb"], cam, cfg, dtype)
+        assert np.array_equal(F, r["fwd"]["image"]) and F.max() > 0.1
+    rng = np.random.default_rng(1)
+    Gw = rng.normal(0, 1, (co.height, co.width, 3))
+    a = xo.rasterize_bwd_featn(r["proj"], r["binned"], r["fwd"], r["proj"]["rgb"], Gw, cam, cfg, np.float64)
+    b = xo.rasterize_bwd(r["proj"], r["binned"], r["fwd"], Gw, cam, cfg, np.float64)
+    for ka, kb in (("g_mean2d", "g_mean2d"), ("g_conic", "g_conic"), ("g_opac_eff", "g_opac_eff"), ("g_feat", "g_rgb")):
+        assert np.allclose(a[ka], b[kb], rtol=1e-13, atol=1e-15), ka
+        assert np.abs(b[kb]).max() > 0
+
+
+def test_p16_depth_and_one_are_the_p15_passes():
+    # C = 2, feat = (z, 1): the P15-pinned depth image and accumulated opacity, forward and backward; the colour
+    # argument of the shared walk (a non-zero background here) does not enter
+    arr, co = _scene(7, opac_boost=1.0)
+    cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=1, bg=(0.3, 0.6, 0.9)))
+    r = xo.render_da(arr, cam, cfg, np.float64)
+    z = r["proj"]["depth"]
+    feat = np.stack([z, np.ones_like(z)], 1)
+    F = xo.rasterize_fwd_featn(r["proj"], r["binned"], feat, cam, cfg, np.float64)
+    assert np.array_equal(F[..., 0], r["fwd"]["depth_img"]) and np.array_equal(F[..., 1], r["fwd"]["alpha_img"])
+    rng = np.random.default_rng(2)
+    Gf = rng.normal(0, 1, (co.height, co.width, 2))
+    a = xo.rasterize_bwd_featn(r["proj"], r["binned"], r["fwd"], feat, Gf, cam, cfg, np.float64)
+    Z3 = np.zeros((co.height, co.width, 3))
+    b = xo.rasterize_bwd_da(r["proj"], r["binned"], r["fwd"], Z3, Gf[..., 0], Gf[..., 1], cam, cfg, np.float64)
+    for k in ("g_mean2d", "g_conic", "g_opac_eff"):
+        assert np.allclose(a[k], b[k], rtol=1e-12, atol=1e-14), k
+    assert np.allclose(a["g_feat"][:, 0], b["g_depth"], rtol=1e-13, atol=1e-15)
+    assert (b["g_rgb"] == 0).all()
+
+
+def test_p16_finite_differences_five_channels():
+    # the hand-derived backward against central differences of the forward, on the compositing inputs themselves
+    # (feat, o_eff, mean2d, conic; lists and lnv fixed: the gates are piecewise constant, C15)
+    found = None
+    for seed in range(40):
+        arr, co = _scene(600 + seed, n=12, opac_boost=1.0)
+        cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=1), fragile_rel=1e-4)
+        r = xo.render(arr, cam, cfg, np.float64)
+        if (r["fwd"]["fragile"] == 0).all() and (r["fwd"]["n_contrib"] > 2).any():
+            found = (arr, co, cam, cfg, r)
+            break
+    assert found is not None
+    arr, co, cam, cfg, r = found
+    rng = np.random.default_rng(3)
+    N, Cn = r["proj"]["depth"].shape[0], 5
+    feat = rng.normal(0, 1, (N, Cn))
+    Gf = rng.normal(0, 1, (co.height, co.width, Cn))
+    g = xo.rasterize_bwd_featn(r["proj"], r["binned"], r["fwd"], feat, Gf, cam, cfg, np.float64)
+
+    def loss(proj, f):
+        return float((xo.rasterize_fwd_featn(proj, r["binned"], f, cam, cfg, np.float64) * Gf).sum())
+
+    vis = np.flatnonzero(r["proj"]["tile_count"] > 0)
+    assert vis.size >= 5
+    checks = 0
+    for key, gk in (("feat", "g_feat"), ("opac_eff", "g_opac_eff"), ("mean2d", "g_mean2d"), ("conic", "g_conic")):
+        base = feat if key == "feat" else r["proj"][key]
+        scale = np.abs(g[gk]).max()
+        assert scale > 0
+        for i in vis[:6]:
+            for j in range(base[i].size if base.ndim > 1 else 1):
+                idx = (i, j) if base.ndim > 1 else (i,)
+                h = 1e-6 * max(1.0, abs(base[idx]))
+                vals = []
+                for sgn in (+1, -1):
+                    p2, f2 = dict(r["proj"]), feat
+                    pert = base.copy(); pert[idx] += sgn * h
+                    if key == "feat":
+                        f2 = pert
+                    else:
+                        p2[key] = pert
+                    vals.append(loss(p2, f2))
+                fd = (vals[0] - vals[1]) / (2 * h)
+                assert abs(fd - g[gk][idx]) <= 2e-6 * scale + 1e-5 * abs(fd), (key, idx, fd, g[gk][idx])
+                checks += 1
+    assert checks > 60
