@@ -264,6 +264,28 @@ int32_t xpr_depth_bwd(int64_t N, const xpr_camera* cam, const uint32_t* tile_cou
                       float* g_means, void* stream);
 
 /*
+ * N-channel features (same reading C31; SURVEY 8(f) f3 "N-channel feature outputs"): feat [N,C] row-major, any C >= 1;
+ *   feat_img[H,W,C] = sum_k feat[g_k,:] alpha_k T_k over the colour pass's contributing sequence, no background.
+ * xpr_rasterize_featn_fwd -- REPLAYS the walk of a finished colour pass (xpr_rasterize_fwd or xpr_rasterize_feat_fwd on
+ *   the same lists): in n_contrib[H,W]; out feat_img (fully overwritten).  One launch, grid = (tiles, ceil(C / 8)).
+ * xpr_rasterize_featn_bwd -- reverse mode for dL_dfeat[H,W,C] ALONE: ADDS that part to g_mean2d[N,2], g_conic[N,3],
+ *   g_opac[N] (so it can follow xpr_rasterize_bwd / _feat_bwd, whose parts it completes: every step is linear in the
+ *   incoming gradient) and to g_feat[N,C].  zero_init bit 0: zero-fill g_mean2d, g_conic, g_opac first; bit 1: zero-fill
+ *   g_feat first.  in: final_T, n_contrib of the colour pass.
+ * Errors: C < 1, N < 0, null / misaligned pointer -> XPR_ERR_INVALID_ARG before any launch.
+ */
+int32_t xpr_rasterize_featn_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                const float* conic_opac, const float* lnv, const float* feat, int32_t C,
+                                const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                                const uint32_t* n_contrib, float* feat_img, void* stream);
+int32_t xpr_rasterize_featn_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
+                                const float* conic_opac, const float* lnv, const float* feat, int32_t C,
+                                const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                                const float* final_T, const uint32_t* n_contrib, const float* dL_dfeat,
+                                float* g_mean2d, float* g_conic, float* g_opac, float* g_feat,
+                                int32_t zero_init, void* stream);
+
+/*
  * xpr_loss_grad -- convenience for the caller's side of the step (reading C21: the loss lives outside the path):
  * dL/dimage of the two losses BASELINE.json's configs name, as sums over all n = H*W*3 values, in one pass:
  *   kind 0: L = sum |I - target|    -> dL = sign(I - target);      kind 1: L = sum (I - target)^2 -> dL = 2 (I - target).

@@ -20,7 +20,7 @@ FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_R
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
            "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
-           "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_loss_grad")
+           "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad")
 
 
 class XprCamera(C.Structure):
@@ -264,6 +264,25 @@ def xpr_depth_bwd(cam: XprCamera, tile_count, g_depth, g_means, stream=None):
     N = int(tile_count.shape[0])
     _check(lib().xpr_depth_bwd(C.c_int64(N), C.byref(cam), _p(tile_count), _p(g_depth), _p(g_means), _stream(stream)),
            "xpr_depth_bwd")
+
+
+def xpr_rasterize_featn_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, lnv, feat, vals_sorted, tile_ranges,
+                            n_contrib, feat_img, stream=None):
+    N, Cn = int(feat.shape[0]), int(feat.shape[1])
+    _check(lib().xpr_rasterize_featn_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(lnv),
+                                         _p(feat), C.c_int32(Cn), _p(vals_sorted), _p(tile_ranges), _p(n_contrib),
+                                         _p(feat_img), _stream(stream)), "xpr_rasterize_featn_fwd")
+
+
+def xpr_rasterize_featn_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, lnv, feat, vals_sorted, tile_ranges,
+                            final_T, n_contrib, dL_dfeat, g_mean2d, g_conic, g_opac, g_feat, zero_init: int = 2,
+                            stream=None):
+    N, Cn = int(feat.shape[0]), int(feat.shape[1])
+    _check(lib().xpr_rasterize_featn_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(lnv),
+                                         _p(feat), C.c_int32(Cn), _p(vals_sorted), _p(tile_ranges), _p(final_T),
+                                         _p(n_contrib), _p(dL_dfeat), _p(g_mean2d), _p(g_conic), _p(g_opac),
+                                         _p(g_feat), C.c_int32(int(zero_init)), _stream(stream)),
+           "xpr_rasterize_featn_bwd")
 
 
 def xpr_loss_grad(kind: str, image, target, dL_dimage, stream=None):

@@ -176,6 +176,30 @@ class SplatPipeline:
                              self.tile_ranges, self.final_T, self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic,
                              self.g_opac, self.g_rgb, zero_init=True)
 
+    # ---- N-channel features (f3): replay of the finished colour pass ---------------------------
+    def rasterize_featn_fwd(self, feat, feat_img=None):
+        """feat [N,C] -> feat_img [H,W,C] = sum_k feat[g_k,:] alpha_k T_k (call after rasterize_fwd)."""
+        if self.ray_eval:
+            raise ValueError("xpr: N-channel features are built for the 2D evaluation")
+        if feat_img is None:
+            feat_img = torch.empty(self.H, self.W, feat.shape[1], dtype=torch.float32, device=self.device)
+        xb.xpr_rasterize_featn_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.lnv, feat, self.vals_sorted,
+                                   self.tile_ranges, self.n_contrib, feat_img)
+        return feat_img
+
+    def rasterize_featn_bwd(self, feat, dL_dfeat, g_feat=None, first: bool = False):
+        """Adds the feature part of the compositing gradients (call between rasterize_bwd and project_bwd; first=True
+        when no colour backward ran: the geometric gradients are then zero-filled here); returns g_feat [N,C]."""
+        if g_feat is None:
+            g_feat = torch.empty_like(feat)
+        xb.xpr_rasterize_featn_bwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.lnv, feat, self.vals_sorted,
+                                   self.tile_ranges, self.final_T, self.n_contrib, dL_dfeat, self.g_mean2d, self.g_conic,
+                                   self.g_opac, g_feat, zero_init=3 if first else 2)
+        if first:
+            self.g_rgb.zero_()
+            self._feat_bwd = False
+        return g_feat
+
     def project_bwd(self):
         means, scales, quats, opacities, sh = self._inputs
         xb.xpr_project_bwd(means, scales, quats, opacities, sh, self.cam, self.cfg, self.tile_count, self.flags,

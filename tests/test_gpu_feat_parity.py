@@ -144,3 +144,96 @@ def test_feat_everything_culled():
     pipe.backward(torch.ones(64, 64, 3, device=pipe.device), one, one)
     for k in PARAMS + ("g_depth",):
         assert not bool(getattr(pipe, k).any()), k
+
+
+# ---- N-channel features (xpr_rasterize_featn_fwd / _bwd) against the oracle (pin P16) ----------------------------
+
+FLOOR_REL = 1e-3      # group-relative fp32 summation floor of the geometric gradients
+
+
+def featn_parity(scene, Cn, view=0, cfg_over=None, with_colour=True):
+    import torch
+    g = pu.run_gpu(scene, view, cfg_over)
+    pipe = g["pipe"]
+    o = pu.run_oracle(scene, view, cfg_over)
+    pu.compare_binning(g, o)
+    pu.compare_forward(g, o)
+    rng = np.random.default_rng(5000 + Cn + view)
+    feat = rng.normal(0.0, 1.0, (scene.N, Cn)).astype(np.float32)
+    H, W = o["fwd"]["n_contrib"].shape
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(pipe.device)
+    F_gpu = pipe.rasterize_featn_fwd(t(feat)).cpu().numpy()
+    F_ref = xo.rasterize_fwd_featn(o["proj"], o["binned"], feat, o["cam"], o["cfg"], np.float32)
+    ok = (o["fwd"]["fragile"] & pu.FRAG_EXIT) == 0
+    fmax = max(1.0, float(np.abs(feat).max()))
+    err = np.abs(F_gpu.astype(np.float64) - F_ref).max(axis=2)
+    assert err[ok].max(initial=0.0) <= pu.IMG_TOL * fmax, (err[ok].max(), fmax)      # |F| <= max|feat| (1 - T)
+    assert np.abs(F_ref).max() > 0.1
+
+    gF = rng.uniform(-1.0, 1.0, (H, W, Cn)).astype(np.float32)
+    frag = (o["fwd"]["fragile"] & (pu.FRAG_EXIT | pu.FRAG_CLAMP)) != 0
+    gF = np.where(frag[..., None], 0.0, gF).astype(np.float32)
+    ref = xo.rasterize_bwd_featn(o["proj"], o["binned"], o["fwd"], feat, gF, o["cam"], o["cfg"], np.float32)
+    # mass of every element = the same backward with |gF| and |feat| ... not available as a variant: bound it by the
+    # oracle run on (|feat|, |gF|) for g_feat (sign-definite terms) and use the group scale for the geometric parts
+    if with_colour:
+        _, dL = scenes.loss_and_grad(scene.loss, o["fwd"]["image"], scene.target(view))
+        dL = np.where(frag[..., None], 0.0, dL).astype(np.float32)
+        col = xo.rasterize_bwd(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32)
+        mass = xo.rasterize_bwd(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32, mass=True)
+        pipe.rasterize_bwd(t(dL))
+        g_feat = pipe.rasterize_featn_bwd(t(feat), t(gF))
+    else:
+        col = {k: 0.0 for k in ("g_mean2d", "g_conic", "g_opac_eff")}
+        mass = {k: 0.0 for k in ("g_mean2d", "g_conic", "g_opac_eff")}
+        g_feat = pipe.rasterize_featn_bwd(t(feat), t(gF), first=True)
+    torch.cuda.synchronize()
+    # g_feat: sums of alpha T gF over pixels; mass = the same sum with |gF|
+    m = xo.rasterize_bwd_featn(o["proj"], o["binned"], o["fwd"], feat, np.abs(gF), o["cam"], o["cfg"], np.float32)
+    bad, e = pu.grad_violations(g_feat.cpu().numpy(), ref["g_feat"], m["g_feat"])
+    assert bad.sum() == 0, f"g_feat: {bad.sum()} of {bad.size}, max err {e.max()}"
+    assert np.abs(ref["g_feat"]).max() > 0
+    # geometric parts: colour part + feature part; the fp32 summation floor is taken relative to the Gaussian's
+    # largest component of that gradient among the two parts (cancellation-aware, DESIGN.md 5 / 6.8)
+    for kg, ko in (("g_mean2d", "g_mean2d"), ("g_conic", "g_conic"), ("g_opac", "g_opac_eff")):
+        total = np.asarray(ref[ko] + col[ko], np.float64).reshape(scene.N, -1)
+        floor = (np.abs(np.asarray(ref[ko]).reshape(scene.N, -1)).max(axis=1, keepdims=True)
+                 + np.abs(np.asarray(col[ko] if with_colour else 0.0 * total).reshape(scene.N, -1)).max(axis=1, keepdims=True))
+        got = getattr(pipe, kg).cpu().numpy().reshape(scene.N, -1).astype(np.float64)
+        tol = pu.GRAD_RTOL * np.abs(total) + pu.GRAD_ATOL + FLOOR_REL * floor
+        if with_colour:
+            tol = tol + pu.GRAD_KAPPA * np.asarray(mass[ko]).reshape(scene.N, -1)
+        worst = np.abs(got - total) - tol
+        assert (worst <= 0).all(), f"{kg}: {(worst > 0).sum()} of {worst.size} outside tolerance, max excess {worst.max()}"
+    return pipe
+
+
+@pytest.mark.parametrize("Cn", [1, 3, 8, 13])
+def test_featn_config1(Cn):
+    featn_parity(scenes.make_scene(1), Cn)
+
+
+def test_featn_config2_reduced_alone():
+    featn_parity(scenes.make_scene(2, n_override=20000, image_override=(200, 200)), 5, with_colour=False)
+
+
+@pytest.mark.parametrize("view", [0, 1])
+def test_featn_config3_reduced(view):
+    featn_parity(scenes.make_scene(3, n_override=50000, image_override=(480, 270)), 16, view, dict(tile_cull=1))
+
+
+def test_featn_ragged():
+    featn_parity(scenes.make_scene(1, image_override=(70, 50)), 4)
+
+
+def test_featn_three_channels_of_rgb_are_the_colour_image():
+    import torch
+    sc = scenes.make_scene(2, n_override=20000, image_override=(200, 200))
+    g = pu.run_gpu(sc, 0, dict(bg=(0.0, 0.0, 0.0)))
+    pipe = g["pipe"]
+    F = pipe.rasterize_featn_fwd(pipe.rgb)
+    assert float((F - pipe.image).abs().max()) <= 1e-6
+
+
+def test_featn_config3_full_size():
+    featn_parity(scenes.make_scene(3), 8, 0, dict(tile_cull=1))
