@@ -273,7 +273,7 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     const uint2 rg = ranges[tile];
 
     uint32_t n[BWD_PPT];
-    float T[BWD_PPT], S0[BWD_PPT], S1[BWD_PPT], S2[BWD_PPT], g0[BWD_PPT], g1[BWD_PPT], g2[BWD_PPT], pxc[BWD_PPT];
+    float T[BWD_PPT], Q[BWD_PPT], g0[BWD_PPT], g1[BWD_PPT], g2[BWD_PPT], pxc[BWD_PPT];
     uint32_t wmax = 0;
 #pragma unroll
     for (int k = 0; k < BWD_PPT; ++k) {
@@ -286,8 +286,9 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             T[k] = final_T[pid];
             g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
         }
-        // colour behind the current entry, S_k = sum_{j>k} c_j alpha_j T_j + T_final bg (C13)
-        S0[k] = T[k] * P.bg[0]; S1[k] = T[k] * P.bg[1]; S2[k] = T[k] * P.bg[2];
+        // colour behind the current entry, S_k = sum_{j>k} c_j alpha_j T_j + T_final bg (C13), enters only through
+        // g . S_k: one running scalar Q_k = g . S_k = sum_{j>k} (g . c_j) alpha_j T_j + T_final (g . bg)
+        Q[k] = T[k] * fmaf(g2[k], P.bg[2], fmaf(g1[k], P.bg[1], g0[k] * P.bg[0]));
         wmax = max(wmax, n[k]);
     }
 #pragma unroll
@@ -341,7 +342,7 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
             // the thread's pixels share dy: accumulate sum dpow, sum dpow dx, sum dpow dx^2 and form the five
             // geometric gradients once per entry (dpow = dL/dpower of a pixel).  Branch-free over the pixels:
             // one that does not contribute enters with o G = 0, hence alpha = 0, 1/(1-alpha) = 1, w = 0 -- its T
-            // and S are unchanged and all its terms vanish.
+            // and Q are unchanged and all its terms vanish.
             float sp = 0.f, spx = 0.f, spxx = 0.f;
 #pragma unroll
             for (int k = 0; k < BWD_PPT; ++k) {
@@ -353,9 +354,8 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
                 v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
                 // dL/dalpha = sum_ch g_ch (c_ch T - S_ch / (1 - alpha)) = T (g . c) - (g . S) / (1 - alpha)
                 const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
-                const float gS = fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]));
-                const float dalpha = fmaf(T[k], gc, -(inv * gS));
-                S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
+                const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
+                Q[k] = fmaf(gc, w, Q[k]);
                 const float live = (og < P.amax) ? dalpha : 0.0f;   // C14: the clamp has zero derivative
                 const float dpow = og * live;          // dL/dpower; dL/do = G live = dpow / o: summed as sp below
                 const float dxp = dx[k] * dpow;

@@ -65,13 +65,15 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
 // and from dL/dalpha on as the colour pass.  SA telescopes (alpha_j T_j = T_j - T_{j+1}):
 //   SA_k = T_k (1 - alpha_k) - T_final   =>   gA (T_k - SA_k / (1 - alpha_k)) = gA T_final / (1 - alpha_k),
 // so the accumulated-opacity term is the per-pixel constant gA T_final entering the "behind" dot product with a
-// minus sign: no running sum, no cancellation.  The depth term adds one FMA to each dot product, one to SD and
-// one to dL/dz.  sum dpow (dL/do) and dL/dz share one butterfly (6 shuffles for the two).
+// minus sign: no running sum, no cancellation.  Everything behind the entry enters through ONE running scalar
+//   Q_k = g . S_k + gD SD_k - gA T_final = sum_{j>k} (g . c_j + gD z_j) alpha_j T_j + T_final (g . bg - gA),
+// so the depth term costs one FMA in the dot product g . c + gD z and one for dL/dz.  sum dpow (dL/do) and dL/dz
+// share one butterfly (6 shuffles for the two).
 #ifndef XPR_FEAT_BWD_PPT
 #define XPR_FEAT_BWD_PPT 4          // pixels per thread in the throughput shape
 #endif
 #ifndef XPR_FEAT_BWD_MINB
-#define XPR_FEAT_BWD_MINB 10        // 64-thread CTAs per SM at 4 pixels per thread
+#define XPR_FEAT_BWD_MINB 12        // 64-thread CTAs per SM at 4 pixels per thread (80 registers)
 #endif
 template <int PPT>
 __global__ void __launch_bounds__(BLOCK / PPT, XPR_FEAT_BWD_MINB * PPT / 4)
@@ -99,22 +101,23 @@ rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const
     const uint2 rg = ranges[tile];
 
     uint32_t n[PPT];
-    float T[PPT], S0[PPT], S1[PPT], S2[PPT], SD[PPT], g0[PPT], g1[PPT], g2[PPT], gD[PPT], gAT[PPT], pxc[PPT];
+    float T[PPT], Q[PPT], g0[PPT], g1[PPT], g2[PPT], gD[PPT], pxc[PPT];
     uint32_t wmax = 0;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
         const int px = px0 + k;
         pxc[k] = (float)px + 0.5f;
-        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = gD[k] = gAT[k] = 0.0f;
+        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = gD[k] = 0.0f;
+        float gA = 0.0f;
         if (px < P.W && py < P.H) {
             const int64_t pid = (int64_t)py * P.W + px;
             n[k] = n_contrib[pid];
             T[k] = final_T[pid];
             g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
-            gD[k] = dL_dD[pid]; gAT[k] = dL_dA[pid] * T[k];      // gA T_final
+            gD[k] = dL_dD[pid]; gA = dL_dA[pid];
         }
-        S0[k] = T[k] * P.bg[0]; S1[k] = T[k] * P.bg[1]; S2[k] = T[k] * P.bg[2];
-        SD[k] = 0.0f;
+        // Q_k = g . S_k + gD SD_k - gA T_final: one running scalar for everything "behind" the entry
+        Q[k] = T[k] * (fmaf(g2[k], P.bg[2], fmaf(g1[k], P.bg[1], g0[k] * P.bg[0])) - gA);
         wmax = max(wmax, n[k]);
     }
 #pragma unroll
@@ -177,10 +180,8 @@ rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const
                 v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
                 sz = fmaf(w, gD[k], sz);               // dL/dz
                 const float gc = fmaf(gD[k], z, fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x)));
-                const float gS = fmaf(gD[k], SD[k], fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], fmaf(g0[k], S0[k], -gAT[k]))));
-                const float dalpha = fmaf(T[k], gc, -(inv * gS));
-                S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
-                SD[k] = fmaf(z, w, SD[k]);
+                const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
+                Q[k] = fmaf(gc, w, Q[k]);
                 const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
                 const float dpow = og * live;
                 const float dxp = dx[k] * dpow;
