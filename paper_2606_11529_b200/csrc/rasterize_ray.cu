@@ -244,7 +244,7 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
     const float lnr = P.lnr;
 
     uint32_t n[PPT];
-    float T[PPT], S0[PPT], S1[PPT], S2[PPT], g0[PPT], g1[PPT], g2[PPT], d0[PPT], d1[PPT], d2[PPT];
+    float T[PPT], Q[PPT], g0[PPT], g1[PPT], g2[PPT], d0[PPT], d1[PPT], d2[PPT];
     uint32_t wmax = 0;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
@@ -257,7 +257,8 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
             d0[k] = rays[3 * pid]; d1[k] = rays[3 * pid + 1]; d2[k] = rays[3 * pid + 2];
         }
-        S0[k] = T[k] * P.bg[0]; S1[k] = T[k] * P.bg[1]; S2[k] = T[k] * P.bg[2];
+        // Q_k = g . S_k, the colour behind the entry as one running scalar (rasterize.cu)
+        Q[k] = T[k] * fmaf(g2[k], P.bg[2], fmaf(g1[k], P.bg[1], g0[k] * P.bg[0]));
         wmax = max(wmax, n[k]);
     }
 #pragma unroll
@@ -319,9 +320,8 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                 const float w = alpha * T[k];
                 vb[5] = fmaf(w, g0[k], vb[5]); vb[6] = fmaf(w, g1[k], vb[6]); vb[7] = fmaf(w, g2[k], vb[7]);
                 const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
-                const float gS = fmaf(g2[k], S2[k], fmaf(g1[k], S1[k], g0[k] * S0[k]));
-                const float dalpha = fmaf(T[k], gc, -(inv * gS));
-                S0[k] = fmaf(c.x, w, S0[k]); S1[k] = fmaf(c.y, w, S1[k]); S2[k] = fmaf(c.z, w, S2[k]);
+                const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
+                Q[k] = fmaf(gc, w, Q[k]);
                 const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
                 const float gp = og * live;            // dL/dpower; dL/do = gp / o, divided once per warp below
                 vb[4] += gp;
