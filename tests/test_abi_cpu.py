@@ -134,6 +134,20 @@ def test_feature_entry_points_reject_bad_arguments(lib):
     assert lib.xpr_depth_bwd(N4, None, one, one, one, null) == 1
     assert lib.xpr_depth_bwd(N4, C.byref(cam), one, null, one, null) == 1
     assert lib.xpr_depth_bwd(N0, C.byref(cam), null, null, null, null) == 0
+    # N-channel features: mean2d conic_opac lnv feat C vals ranges n_contrib feat_img
+    fn = lambda n, c, *a: lib.xpr_rasterize_featn_fwd(C.byref(cam), C.byref(cfg), n, a[0], a[1], a[2], a[3], C.c_int32(c),
+                                                      a[4], a[5], a[6], a[7], null)
+    assert fn(N4, 0, *[one] * 8) == 1                                                         # C < 1
+    assert fn(Nm, 3, *[one] * 8) == 1
+    assert fn(N4, 3, one, one, one, null, one, one, one, one) == 1                            # feat NULL
+    assert fn(N4, 3, *[one] * 7, null) == 1                                                   # feat_img NULL
+    bn = lambda n, c, *a: lib.xpr_rasterize_featn_bwd(C.byref(cam), C.byref(cfg), n, a[0], a[1], a[2], a[3], C.c_int32(c),
+                                                      *a[4:], C.c_int32(3), null)
+    # mean2d conic_opac lnv feat | vals ranges final_T n_contrib dL_dfeat g_mean2d g_conic g_opac g_feat
+    assert bn(N4, 0, *[one] * 13) == 1
+    assert bn(N4, 5, *[one] * 12, null) == 1                                                  # g_feat NULL
+    assert bn(N4, 5, *[one] * 8, odd, *[one] * 4) == 1                                        # dL_dfeat misaligned
+    assert bn(N0, 5, *[null] * 5, one, one, one, one, *[null] * 4) == 0                       # N = 0: nothing to do
 
 
 def test_workspace_size_monotone(lib):
