@@ -49,6 +49,9 @@ def parse():
     ap.add_argument("--features", type=int, default=0, choices=(0, 1),
                     help="1: also render the depth image and the accumulated opacity and take their gradients "
                          "(SURVEY 8(f) f3, DESIGN.md 6.8; 2D evaluation only; not part of the headline workload)")
+    ap.add_argument("--featn", type=int, default=0,
+                    help="C > 0: after the timed steps, also time xpr_rasterize_featn_fwd / _bwd with C seeded feature "
+                         "channels on the lists of the last step (reported as 'featn'; not part of the step)")
     ap.add_argument("--ray-eval", type=int, default=0, choices=(0, 1),
                     help="1: XPR-3DGUT evaluation along the pixel ray (SURVEY 8(f) f2; meant for --config 4) instead of "
                          "the 2D conic of north_star")
@@ -372,6 +375,27 @@ def run_ours(args):
         except Exception as e:      # capture unsupported in this environment: report, do not hide
             graph_ms = "unavailable: %s" % (str(e).splitlines()[0][:120],)
 
+    featn = None
+    if args.featn > 0 and not args.ray_eval:     # N-channel features: the two kernels alone, warm L2
+        gen = torch.Generator(device="cpu").manual_seed(5000 + args.featn)
+        feat = torch.randn(sc.N, args.featn, generator=gen).to(dev)
+        gF = (torch.rand(cam.height, cam.width, args.featn, generator=gen) * 2 - 1).to(dev)
+        F_img, g_feat = torch.empty_like(gF), torch.empty_like(feat)
+
+        def _time(fn, n=20):
+            for _ in range(3):
+                fn()
+            a = _rec()
+            for _ in range(n):
+                fn()
+            b = _rec()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / n
+        featn = {"C": args.featn,
+                 "fwd_ms": _time(lambda: pipe.rasterize_featn_fwd(feat, F_img)),
+                 "bwd_ms": _time(lambda: pipe.rasterize_featn_bwd(feat, gF, g_feat)),
+                 "how": "20 back-to-back launches each, CUDA events, warm L2, after the timed steps"}
+
     clocks = sampler.stop()      # sampled (every 20 ms) over the timed steps and the graph replays
 
     # end to end through the public API with HOST buffers: H2D of the parameters, the step, D2H of results
@@ -486,7 +510,7 @@ def run_ours(args):
                 "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,
                 "pixel_pairs": {"visited": visit, "passed_gate": passed, "blended": blended, "sum_n_contrib": sum_n},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-                "cuda_graph_ms_per_step": graph_ms, "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}
+                "cuda_graph_ms_per_step": graph_ms, "featn": featn, "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
         if args.stages:
             print(json.dumps(stage_ms, indent=1), file=sys.stderr)

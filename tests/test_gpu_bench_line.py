@@ -54,3 +54,9 @@ def test_bench_line_rendered_features():
     assert d["rooflines"]["rasterize_bwd"]["kernel"] == "rasterize_feat_bwd_kernel"
     assert d["gpu_launches"] == 3 * (17 + 1)    # + depth_bwd
     assert d["e2e"]["d2h_bytes_per_step"] > 1920 * 1080 * 4 * 5    # image, D and A all come back
+
+
+def test_bench_line_reports_n_channel_feature_timings():
+    d = _run("--featn", "5", "--no-cpu-baseline", "--no-e2e", "--no-graph")
+    assert d["featn"]["C"] == 5 and d["featn"]["fwd_ms"] > 0 and d["featn"]["bwd_ms"] > 0
+    assert d["gpu_launches"] == 3 * 16          # the step itself is unchanged
