@@ -210,41 +210,53 @@ rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const
 // F[p, c] = sum_k feat[g_k, c] alpha_k T_k over the colour pass's contributing sequence: the walk is REPLAYED from the
 // colour pass's n_contrib (an entry contributes iff pos < n_contrib and it passes the two gates on `power`, the same
 // bit-identical decisions; the exit test is implied by n_contrib).  Channels are processed in chunks of CH = 8:
-// grid = (tiles, chunks), one launch for any C.  One pixel per thread forward, two backward.
+// grid = (tiles, chunks), one launch for any C.  Two pixels per thread, forward and backward.
 constexpr int FEATN_CH = 8;
 
-template <int CH>
-__global__ void __launch_bounds__(BLOCK)
+template <int CH, int PPT>
+__global__ void __launch_bounds__(BLOCK / PPT)
 rasterize_featn_fwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
                            const float* __restrict__ lnv, const float* __restrict__ feat, int C,
                            const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                            const uint32_t* __restrict__ n_contrib, float* __restrict__ feat_img) {
-    __shared__ float4 s_rec[2 * BLOCK];            // (mx, my, qa, qb | qc, thr, log2 o, -)
-    __shared__ float s_f[CH * BLOCK];              // CH channels per entry
-    __shared__ uint32_t s_max[BLOCK / 32];
+    // PPT = 2: a thread owns the pixels (x, y) and (x + 8, y), as rasterize_fwd_kernel: the record, the channel values
+    // and the row terms of `power` are read / formed once per two pixels
+    constexpr int THREADS = BLOCK / PPT, ROW = TILE / PPT;
+    __shared__ float4 s_rec[2 * THREADS];          // (mx, my, qa, qb | qc, thr, log2 o, -)
+    __shared__ float s_f[CH * THREADS];            // CH channels per entry
+    __shared__ uint32_t s_max[THREADS / 32];
     const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
     const int c0 = blockIdx.y * CH;
-    const int px = tx * TILE + (threadIdx.x % TILE), py = ty * TILE + (threadIdx.x / TILE);
-    const bool in = (px < P.W) && (py < P.H);
-    const float pxc = (float)px + 0.5f, pyc = (float)py + 0.5f;
-    const int64_t pid = (int64_t)py * P.W + px;
+    const int py = ty * TILE + (threadIdx.x / ROW);
+    const float pyc = (float)py + 0.5f;
     const uint2 rg = ranges[tile];
-    const uint32_t n = in ? n_contrib[pid] : 0u;
-    uint32_t wmax = n;
+    int64_t pid[PPT];
+    bool in[PPT];
+    uint32_t n[PPT], wmax = 0;
+    float pxc[PPT], T[PPT], F[PPT][CH];
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+        const int px = tx * TILE + (threadIdx.x % ROW) + 8 * k;
+        in[k] = (px < P.W) && (py < P.H);
+        pid[k] = (int64_t)py * P.W + px;
+        pxc[k] = (float)px + 0.5f;
+        n[k] = in[k] ? n_contrib[pid[k]] : 0u;
+        wmax = max(wmax, n[k]);
+        T[k] = 1.0f;
+#pragma unroll
+        for (int c = 0; c < CH; ++c) F[k][c] = 0.0f;
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
     if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = wmax;
     __syncthreads();
     uint32_t max_n = 0;
 #pragma unroll
-    for (int w = 0; w < BLOCK / 32; ++w) max_n = max(max_n, s_max[w]);
+    for (int w = 0; w < THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
 
-    float T = 1.0f, F[CH];
-#pragma unroll
-    for (int c = 0; c < CH; ++c) F[c] = 0.0f;
-    for (uint32_t base = 0; base < max_n; base += BLOCK) {
-        const uint32_t cnt = min((uint32_t)BLOCK, max_n - base);
+    for (uint32_t base = 0; base < max_n; base += THREADS) {
+        const uint32_t cnt = min((uint32_t)THREADS, max_n - base);
         __syncthreads();
         if (threadIdx.x < cnt) {
             const uint32_t g = vals[rg.x + base + threadIdx.x];
@@ -260,27 +272,39 @@ rasterize_featn_fwd_kernel(FeatParams P, const float2* __restrict__ mean2d, cons
         const uint32_t lim = min(cnt, wmax - base);
         for (uint32_t j = 0; j < lim; ++j) {
             const float4 ge = s_rec[2 * j], ga = s_rec[2 * j + 1];
-            const float dy = pyc - ge.y, dx = pxc - ge.x;
+            const float dy = pyc - ge.y;
             const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);
-            const float power = __fmaf_rn(__fmaf_rn(ge.z, dx, t1), dx, t2);          // rule R3
-            if ((base + j < n) && !(power > 0.0f) && !(power < ga.y)) {
-                const float alpha = fminf(P.amax, opac_exp(power, ga.z));
-                const float w = alpha * T;
-                T = T * (1.0f - alpha);
-                const float4* f4 = reinterpret_cast<const float4*>(s_f + CH * j);
+            float w[PPT];
+            bool any = false;
 #pragma unroll
-                for (int q = 0; q < CH / 4; ++q) {
-                    const float4 f = f4[q];
-                    F[4 * q] = fmaf(f.x, w, F[4 * q]); F[4 * q + 1] = fmaf(f.y, w, F[4 * q + 1]);
-                    F[4 * q + 2] = fmaf(f.z, w, F[4 * q + 2]); F[4 * q + 3] = fmaf(f.w, w, F[4 * q + 3]);
+            for (int k = 0; k < PPT; ++k) {
+                const float dx = pxc[k] - ge.x;
+                const float power = __fmaf_rn(__fmaf_rn(ge.z, dx, t1), dx, t2);      // rule R3
+                const bool c = (base + j < n[k]) && !(power > 0.0f) && !(power < ga.y);
+                const float alpha = c ? fminf(P.amax, opac_exp(power, ga.z)) : 0.0f;
+                w[k] = alpha * T[k];
+                T[k] = T[k] * (1.0f - alpha);
+                any |= c;
+            }
+            if (!any) continue;
+            const float4* f4 = reinterpret_cast<const float4*>(s_f + CH * j);
+#pragma unroll
+            for (int q = 0; q < CH / 4; ++q) {
+                const float4 f = f4[q];
+#pragma unroll
+                for (int k = 0; k < PPT; ++k) {
+                    F[k][4 * q] = fmaf(f.x, w[k], F[k][4 * q]); F[k][4 * q + 1] = fmaf(f.y, w[k], F[k][4 * q + 1]);
+                    F[k][4 * q + 2] = fmaf(f.z, w[k], F[k][4 * q + 2]); F[k][4 * q + 3] = fmaf(f.w, w[k], F[k][4 * q + 3]);
                 }
             }
         }
     }
-    if (in) {
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+        if (!in[k]) continue;
 #pragma unroll
         for (int c = 0; c < CH; ++c)
-            if (c0 + c < C) feat_img[pid * C + c0 + c] = F[c];
+            if (c0 + c < C) feat_img[pid[k] * C + c0 + c] = F[k][c];
     }
 }
 
@@ -517,7 +541,7 @@ extern "C" int32_t xpr_rasterize_featn_fwd(const xpr_camera* cam, const xpr_conf
     FeatParams P;
     make_feat_params(cam, cfg, P);
     const dim3 grid(tiles_x(cam) * tiles_y(cam), (C + FEATN_CH - 1) / FEATN_CH);
-    rasterize_featn_fwd_kernel<FEATN_CH><<<grid, BLOCK, 0, (cudaStream_t)stream>>>(
+    rasterize_featn_fwd_kernel<FEATN_CH, 2><<<grid, BLOCK / 2, 0, (cudaStream_t)stream>>>(
         P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), lnv, feat, C,
         vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), n_contrib, feat_img);
     XPR_LAUNCH_CHECK();
