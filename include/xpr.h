@@ -92,7 +92,9 @@ int32_t xpr_project(int64_t N, const float* means, const float* scales, const fl
  * key = (uint64)t << 32 | float_bits(depth) (BASELINE.json:north_star, C10), value = Gaussian
  * index; stable LSD radix sort by key (hand-written onesweep); per-tile bounds.
  *   in : depth[N], tile_rect[N,4], tile_count[N] from xpr_project; pair_capacity = length of the
- *        output arrays (must be < 2^30).
+ *        output arrays (must be < 2^30; 0 is allowed and makes the call a size probe: with any visible
+ *        Gaussian it reports XPR_ERR_CAPACITY and the capacity that suffices, in both modes below).
+ *        N must be < 2^30 (XPR_ERR_UNSUPPORTED otherwise: the sort's look-back words carry 30-bit counts).
  *   out: keys_sorted[I] u64, vals_sorted[I] u32, tile_ranges[T,2] = (start,end) per tile, (0,0)
  *        for an empty tile; *num_pairs_host (HOST int64) = I.
  *   Capacity: pair_capacity must hold I = sum of tile_count (the candidate pairs) and must exceed

@@ -94,14 +94,20 @@ def num_tiles(cam: XprCamera, cfg: XprConfig):
     return (int(cam.width) + ts - 1) // ts, (int(cam.height) + ts - 1) // ts
 
 
-def _p(t):
-    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+_F32, _I32, _U8, _I64 = (torch.float32,), (torch.int32, torch.uint32), (torch.uint8,), (torch.int64, torch.uint64)
+
+
+def _p(t, dtypes=None):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL).  `dtypes`: the element types the C signature
+    accepts for this argument (a tensor of another type would be reinterpreted silently by the library)."""
     if t is None:
         return C.c_void_p(0)
     if not t.is_cuda:
         raise TypeError("xpr: expected a CUDA tensor (the library takes device pointers; no CPU fallback)")
     if not t.is_contiguous():
         raise ValueError("xpr: tensor must be contiguous")
+    if dtypes is not None and t.dtype not in dtypes:
+        raise TypeError(f"xpr: expected a tensor of {' / '.join(str(d) for d in dtypes)}, got {t.dtype}")
     return C.c_void_p(t.data_ptr())
 
 
@@ -122,9 +128,9 @@ def xpr_version() -> int:
 def xpr_project(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, depth,
                 lnv, tile_rect, tile_count, flags, stream=None):
     N = int(means.shape[0])
-    _check(lib().xpr_project(C.c_int64(N), _p(means), _p(scales), _p(quats), _p(opacities), _p(sh), C.byref(cam),
-                             C.byref(cfg), _p(mean2d), _p(conic_opac), _p(rgb), _p(depth), _p(lnv), _p(tile_rect),
-                             _p(tile_count), _p(flags), _stream(stream)), "xpr_project")
+    _check(lib().xpr_project(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), _p(opacities, _F32), _p(sh, _F32), C.byref(cam),
+                             C.byref(cfg), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32), _p(depth, _F32), _p(lnv, _F32), _p(tile_rect, _I32),
+                             _p(tile_count, _I32), _p(flags, _U8), _stream(stream)), "xpr_project")
 
 
 def xpr_bin_sort_workspace(N: int, pair_capacity: int, n_tiles: int) -> int:
@@ -143,14 +149,14 @@ def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, p
     first 8 bytes of `workspace` (xpr.h); the caller checks it against pair_capacity later."""
     N = int(tile_count.shape[0])
     n_pairs = C.c_int64(0)
-    tail = (C.byref(cam), C.byref(cfg), C.c_int64(pair_capacity), _p(keys_sorted), _p(vals_sorted), _p(tile_ranges),
-            C.byref(n_pairs) if sync else None, _p(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+    tail = (C.byref(cam), C.byref(cfg), C.c_int64(pair_capacity), _p(keys_sorted, _I64), _p(vals_sorted, _I32), _p(tile_ranges, _I32),
+            C.byref(n_pairs) if sync else None, _p(workspace, _U8), C.c_size_t(workspace.numel() * workspace.element_size()),
             _stream(stream))
     if cull_data is None:
-        st = lib().xpr_bin_sort(C.c_int64(N), _p(depth), _p(tile_rect), _p(tile_count), *tail)
+        st = lib().xpr_bin_sort(C.c_int64(N), _p(depth, _F32), _p(tile_rect, _I32), _p(tile_count, _I32), *tail)
     else:
-        st = lib().xpr_bin_sort_cull(C.c_int64(N), _p(depth), _p(tile_rect), _p(tile_count), _p(cull_data[0]),
-                                     _p(cull_data[1]), _p(cull_data[2]), *tail)
+        st = lib().xpr_bin_sort_cull(C.c_int64(N), _p(depth, _F32), _p(tile_rect, _I32), _p(tile_count, _I32), _p(cull_data[0], _F32),
+                                     _p(cull_data[1], _F32), _p(cull_data[2], _F32), *tail)
     if not sync:
         _check(st, "xpr_bin_sort")
         return st, None
@@ -163,79 +169,79 @@ def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, p
 def xpr_rasterize_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, image,
                       final_T, n_contrib, stream=None):
     N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
-                                   _p(lnv), _p(vals_sorted), _p(tile_ranges), _p(image), _p(final_T), _p(n_contrib),
+    _check(lib().xpr_rasterize_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
+                                   _p(lnv, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32), _p(n_contrib, _I32),
                                    _stream(stream)), "xpr_rasterize_fwd")
 
 
 def xpr_rasterize_stats(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, stats,
                         stream=None):
     N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
-                                     _p(lnv), _p(vals_sorted), _p(tile_ranges), _p(stats), _stream(stream)),
+    _check(lib().xpr_rasterize_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
+                                     _p(lnv, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(stats, _I64), _stream(stream)),
            "xpr_rasterize_stats")
 
 
 def xpr_rasterize_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, final_T,
                       n_contrib, dL_dimage, g_mean2d, g_conic, g_opac, g_rgb, zero_init: bool = True, stream=None):
     N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
-                                   _p(lnv), _p(vals_sorted), _p(tile_ranges), _p(final_T), _p(n_contrib),
-                                   _p(dL_dimage), _p(g_mean2d), _p(g_conic), _p(g_opac), _p(g_rgb),
+    _check(lib().xpr_rasterize_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
+                                   _p(lnv, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32), _p(n_contrib, _I32),
+                                   _p(dL_dimage, _F32), _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
                                    C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_bwd")
 
 
 def xpr_project_bwd(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, tile_count, flags, g_mean2d,
                     g_conic, g_opac, g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None):
     N = int(means.shape[0])
-    _check(lib().xpr_project_bwd(C.c_int64(N), _p(means), _p(scales), _p(quats), _p(opacities), _p(sh), C.byref(cam),
-                                 C.byref(cfg), _p(tile_count), _p(flags), _p(g_mean2d), _p(g_conic), _p(g_opac),
-                                 _p(g_rgb), _p(g_means), _p(g_scales), _p(g_quats), _p(g_opacities), _p(g_sh),
+    _check(lib().xpr_project_bwd(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), _p(opacities, _F32), _p(sh, _F32), C.byref(cam),
+                                 C.byref(cfg), _p(tile_count, _I32), _p(flags, _U8), _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32),
+                                 _p(g_rgb, _F32), _p(g_means, _F32), _p(g_scales, _F32), _p(g_quats, _F32), _p(g_opacities, _F32), _p(g_sh, _F32),
                                  _stream(stream)), "xpr_project_bwd")
 
 
 # ---- XPR-3DGUT ray evaluation (xpr.h) ----------------------------------------------------------
 
 def xpr_pixel_info(cam: XprCamera, pixel_rays, stream=None):
-    _check(lib().xpr_pixel_info(C.byref(cam), _p(pixel_rays), _stream(stream)), "xpr_pixel_info")
+    _check(lib().xpr_pixel_info(C.byref(cam), _p(pixel_rays, _F32), _stream(stream)), "xpr_pixel_info")
 
 
 def xpr_project_ray(means, scales, quats, cam: XprCamera, tile_count, ray_rec, stream=None):
     N = int(means.shape[0])
-    _check(lib().xpr_project_ray(C.c_int64(N), _p(means), _p(scales), _p(quats), C.byref(cam), _p(tile_count),
-                                 _p(ray_rec), _stream(stream)), "xpr_project_ray")
+    _check(lib().xpr_project_ray(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), C.byref(cam), _p(tile_count, _I32),
+                                 _p(ray_rec, _F32), _stream(stream)), "xpr_project_ray")
 
 
 def xpr_rasterize_ray_fwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, pixel_rays, vals_sorted,
                           tile_ranges, image, final_T, n_contrib, stream=None):
     N = int(ray_rec.shape[0])
-    _check(lib().xpr_rasterize_ray_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec), _p(conic_opac), _p(rgb),
-                                       _p(lnv), _p(pixel_rays), _p(vals_sorted), _p(tile_ranges), _p(image),
-                                       _p(final_T), _p(n_contrib), _stream(stream)), "xpr_rasterize_ray_fwd")
+    _check(lib().xpr_rasterize_ray_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
+                                       _p(lnv, _F32), _p(pixel_rays, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(image, _F32),
+                                       _p(final_T, _F32), _p(n_contrib, _I32), _stream(stream)), "xpr_rasterize_ray_fwd")
 
 
 def xpr_rasterize_ray_stats(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, pixel_rays, vals_sorted,
                             tile_ranges, stats, stream=None):
     N = int(ray_rec.shape[0])
-    _check(lib().xpr_rasterize_ray_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec), _p(conic_opac),
-                                         _p(rgb), _p(lnv), _p(pixel_rays), _p(vals_sorted), _p(tile_ranges),
-                                         _p(stats), _stream(stream)), "xpr_rasterize_ray_stats")
+    _check(lib().xpr_rasterize_ray_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec, _F32), _p(conic_opac, _F32),
+                                         _p(rgb, _F32), _p(lnv, _F32), _p(pixel_rays, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32),
+                                         _p(stats, _I64), _stream(stream)), "xpr_rasterize_ray_stats")
 
 
 def xpr_rasterize_ray_bwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, pixel_rays, vals_sorted,
                           tile_ranges, final_T, n_contrib, dL_dimage, g_ray_rec, g_opac, g_rgb, zero_init: bool = True,
                           stream=None):
     N = int(ray_rec.shape[0])
-    _check(lib().xpr_rasterize_ray_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec), _p(conic_opac), _p(rgb),
-                                       _p(lnv), _p(pixel_rays), _p(vals_sorted), _p(tile_ranges), _p(final_T),
-                                       _p(n_contrib), _p(dL_dimage), _p(g_ray_rec), _p(g_opac), _p(g_rgb),
+    _check(lib().xpr_rasterize_ray_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
+                                       _p(lnv, _F32), _p(pixel_rays, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32),
+                                       _p(n_contrib, _I32), _p(dL_dimage, _F32), _p(g_ray_rec, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
                                        C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_ray_bwd")
 
 
 def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_rec, g_means, g_scales, g_quats, stream=None):
     N = int(means.shape[0])
-    _check(lib().xpr_ray_bwd(C.c_int64(N), _p(means), _p(scales), _p(quats), C.byref(cam), _p(tile_count),
-                             _p(g_ray_rec), _p(g_means), _p(g_scales), _p(g_quats), _stream(stream)), "xpr_ray_bwd")
+    _check(lib().xpr_ray_bwd(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), C.byref(cam), _p(tile_count, _I32),
+                             _p(g_ray_rec, _F32), _p(g_means, _F32), _p(g_scales, _F32), _p(g_quats, _F32), _stream(stream)), "xpr_ray_bwd")
 
 
 # ---- Rendered depth and accumulated opacity (xpr.h) --------------------------------------------
@@ -243,9 +249,9 @@ def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_rec, g_m
 def xpr_rasterize_feat_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, depth, vals_sorted,
                            tile_ranges, image, final_T, n_contrib, depth_img, alpha_img, stream=None):
     N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
-                                        _p(lnv), _p(depth), _p(vals_sorted), _p(tile_ranges), _p(image), _p(final_T),
-                                        _p(n_contrib), _p(depth_img), _p(alpha_img), _stream(stream)),
+    _check(lib().xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
+                                        _p(lnv, _F32), _p(depth, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32),
+                                        _p(n_contrib, _I32), _p(depth_img, _F32), _p(alpha_img, _F32), _stream(stream)),
            "xpr_rasterize_feat_fwd")
 
 
@@ -253,40 +259,40 @@ def xpr_rasterize_feat_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, r
                            tile_ranges, final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_mean2d, g_conic,
                            g_opac, g_rgb, g_depth, zero_init: bool = True, stream=None):
     N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_feat_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(rgb),
-                                        _p(lnv), _p(depth), _p(vals_sorted), _p(tile_ranges), _p(final_T),
-                                        _p(n_contrib), _p(dL_dimage), _p(dL_ddepth), _p(dL_dalpha), _p(g_mean2d),
-                                        _p(g_conic), _p(g_opac), _p(g_rgb), _p(g_depth),
+    _check(lib().xpr_rasterize_feat_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
+                                        _p(lnv, _F32), _p(depth, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32),
+                                        _p(n_contrib, _I32), _p(dL_dimage, _F32), _p(dL_ddepth, _F32), _p(dL_dalpha, _F32), _p(g_mean2d, _F32),
+                                        _p(g_conic, _F32), _p(g_opac, _F32), _p(g_rgb, _F32), _p(g_depth, _F32),
                                         C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_feat_bwd")
 
 
 def xpr_depth_bwd(cam: XprCamera, tile_count, g_depth, g_means, stream=None):
     N = int(tile_count.shape[0])
-    _check(lib().xpr_depth_bwd(C.c_int64(N), C.byref(cam), _p(tile_count), _p(g_depth), _p(g_means), _stream(stream)),
+    _check(lib().xpr_depth_bwd(C.c_int64(N), C.byref(cam), _p(tile_count, _I32), _p(g_depth, _F32), _p(g_means, _F32), _stream(stream)),
            "xpr_depth_bwd")
 
 
 def xpr_rasterize_featn_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, lnv, feat, vals_sorted, tile_ranges,
                             n_contrib, feat_img, stream=None):
     N, Cn = int(feat.shape[0]), int(feat.shape[1])
-    _check(lib().xpr_rasterize_featn_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(lnv),
-                                         _p(feat), C.c_int32(Cn), _p(vals_sorted), _p(tile_ranges), _p(n_contrib),
-                                         _p(feat_img), _stream(stream)), "xpr_rasterize_featn_fwd")
+    _check(lib().xpr_rasterize_featn_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(lnv, _F32),
+                                         _p(feat, _F32), C.c_int32(Cn), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(n_contrib, _I32),
+                                         _p(feat_img, _F32), _stream(stream)), "xpr_rasterize_featn_fwd")
 
 
 def xpr_rasterize_featn_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, lnv, feat, vals_sorted, tile_ranges,
                             final_T, n_contrib, dL_dfeat, g_mean2d, g_conic, g_opac, g_feat, zero_init: int = 2,
                             stream=None):
     N, Cn = int(feat.shape[0]), int(feat.shape[1])
-    _check(lib().xpr_rasterize_featn_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d), _p(conic_opac), _p(lnv),
-                                         _p(feat), C.c_int32(Cn), _p(vals_sorted), _p(tile_ranges), _p(final_T),
-                                         _p(n_contrib), _p(dL_dfeat), _p(g_mean2d), _p(g_conic), _p(g_opac),
-                                         _p(g_feat), C.c_int32(int(zero_init)), _stream(stream)),
+    _check(lib().xpr_rasterize_featn_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(lnv, _F32),
+                                         _p(feat, _F32), C.c_int32(Cn), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32),
+                                         _p(n_contrib, _I32), _p(dL_dfeat, _F32), _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32),
+                                         _p(g_feat, _F32), C.c_int32(int(zero_init)), _stream(stream)),
            "xpr_rasterize_featn_bwd")
 
 
 def xpr_loss_grad(kind: str, image, target, dL_dimage, stream=None):
     """kind: "l1" (sum of absolute differences) or "l2" (sum of squares); dL/dimage in one pass (xpr.h)."""
     k = {"l1": 0, "l2": 1}[kind]
-    _check(lib().xpr_loss_grad(C.c_int32(k), C.c_int64(image.numel()), _p(image), _p(target), _p(dL_dimage),
+    _check(lib().xpr_loss_grad(C.c_int32(k), C.c_int64(image.numel()), _p(image, _F32), _p(target, _F32), _p(dL_dimage, _F32),
                                _stream(stream)), "xpr_loss_grad")

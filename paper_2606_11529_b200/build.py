@@ -54,7 +54,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if p.wait() != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
     if force or procs or not _newer(OUT, objs):
-        cmd = [NVCC, "-shared", "-o", OUT, *objs, "-cudart", "static"]
+        # the CUDA runtime is linked dynamically (libcudart.so.12: the one PyTorch has already loaded, else the
+        # toolkit's through the rpath), so the library carries no runtime entry points it never calls
+        cmd = [NVCC, "-shared", "-o", OUT, *objs, "-cudart", "shared", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
         subprocess.run(cmd, check=True)
     return OUT
 

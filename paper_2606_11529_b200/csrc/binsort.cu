@@ -903,6 +903,15 @@ ranges_kernel(const unsigned long long* __restrict__ pairs_out, uint32_t T, cons
     if (lane == 0) reinterpret_cast<uint2*>(ranges)[t] = (e > b) ? make_uint2(b, e) : make_uint2(0u, 0u);
 }
 
+// pair_capacity == 0 (a caller probing for the size): the row / pair kernels do not run, so the capacity the call
+// needs -- the candidate pairs, and one more than the rows -- is put where scan_kernel<1> would have put it.
+__global__ void capacity_probe_kernel(Header* __restrict__ hdr) {
+    const unsigned long long rows = hdr->rows_total, cand = hdr->cand_total;
+    hdr->total_pairs = (cand > rows + 1) ? cand : ((rows > 0 || cand > 0) ? rows + 1 : 0ull);
+    hdr->pairs_out = 0ull;
+    hdr->pairs_eff = 0ull;
+}
+
 // Scheduling aid for the compositing kernels (xpr_config.tile_order): the tile indices by decreasing list length,
 // in 1024 length classes (counting sort, one CTA: T is a few thousand).  Heaviest tiles first means the last wave
 // of a compositing launch is made of short tiles.
@@ -964,8 +973,9 @@ tile_order_kernel(const uint32_t* __restrict__ ranges, uint32_t T, uint32_t* __r
 using namespace xpr;
 
 extern "C" int32_t xpr_bin_sort_workspace(int64_t N, int64_t pair_capacity, int32_t num_tiles, size_t* bytes) {
-    if (!bytes || N < 0 || N > 0x7fffffffLL || pair_capacity < 0 || pair_capacity >= (1LL << 30) || num_tiles <= 0)
+    if (!bytes || N < 0 || pair_capacity < 0 || pair_capacity >= (1LL << 30) || num_tiles <= 0)
         return XPR_ERR_INVALID_ARG;
+    if (N >= (1LL << 30)) return XPR_ERR_UNSUPPORTED;      // the look-back status words carry 30-bit counts
     *bytes = make_layout(N, pair_capacity, num_tiles).total;
     return XPR_OK;
 }
@@ -993,8 +1003,8 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
                              uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
                              int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
-    if (N < 0 || N > 0x7fffffffLL || pair_capacity < 0 || pair_capacity >= (1LL << 30))
-        return XPR_ERR_INVALID_ARG;
+    if (N < 0 || pair_capacity < 0 || pair_capacity >= (1LL << 30)) return XPR_ERR_INVALID_ARG;
+    if (N >= (1LL << 30)) return XPR_ERR_UNSUPPORTED;      // the look-back status words carry 30-bit counts
     const int TW = tiles_x(cam), TH = tiles_y(cam);
     const int64_t T64 = (int64_t)TW * TH;
     if (T64 > 0x7fffffffLL) return XPR_ERR_UNSUPPORTED;
@@ -1115,6 +1125,9 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
             XPR_CUDA(e);
             uint64_t* t = w0; w0 = w1; w1 = t;
         }
+    } else {
+        capacity_probe_kernel<<<1, 1, 0, st>>>(hdr);       // visible Gaussians but no room at all: XPR_ERR_CAPACITY below
+        XPR_LAUNCH_CHECK();
     }
     // 6. per-tile ranges ((0, 0) for every tile when there are no pairs or they exceed the capacity)
     ranges_kernel<<<((unsigned)T + 7) / 8, 256, 0, st>>>(&hdr->pairs_out, (uint32_t)T, keys_sorted, tile_ranges);

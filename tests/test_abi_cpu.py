@@ -158,6 +158,11 @@ def test_workspace_size_monotone(lib):
     assert b >= 8 * 1_000_000        # the second buffer of 8-byte packed words (tile << 32 | rank)
     with pytest.raises(xb.XprError):
         xb.xpr_bin_sort_workspace(1000, 1 << 30, 16)
+    # N >= 2^30 would overflow the 30-bit counts of the sort's look-back words: refused, not corrupted
+    with pytest.raises(xb.XprError) as e:
+        xb.xpr_bin_sort_workspace(1 << 30, 1000, 16)
+    assert e.value.status == xb.XPR_ERR_UNSUPPORTED
+    assert xb.xpr_bin_sort_workspace((1 << 30) - 1, 0, 16) > 0
 
 
 def test_binding_refuses_cpu_tensors():

@@ -65,6 +65,47 @@ def test_capacity_error_reports_required_pairs_then_regrows():
     np.testing.assert_array_equal(pu.u32(pipe.vals_sorted[:I]), o["binned"]["vals"])
 
 
+def test_capacity_zero_is_a_size_probe_in_both_modes():
+    """pair_capacity = 0 with visible Gaussians: xpr.h promises XPR_ERR_CAPACITY and the capacity that suffices --
+    synchronously through *num_pairs_host, asynchronously in workspace[0:8] -- never a clean OK with empty lists."""
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline
+    sc = scenes.make_scene(1)
+    I = pu.run_oracle(sc)["binned"]["num_pairs"]
+    cfg = scenes.default_render_config(sc)
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg, pair_capacity=64)
+    pipe.project(*pipeline.scene_to_device(sc))
+    ws = torch.empty(xb.xpr_bin_sort_workspace(sc.N, 0, pipe.T), dtype=torch.uint8, device="cuda")
+    guard_k = torch.full((64,), -7, dtype=torch.int64, device="cuda")
+    guard_v = torch.full((64,), -7, dtype=torch.int32, device="cuda")
+    st, need = xb.xpr_bin_sort(pipe.depth, pipe.tile_rect, pipe.tile_count, pipe.cam, pipe.cfg, 0, guard_k, guard_v,
+                               pipe.tile_ranges, ws, raise_on_capacity=False)
+    assert st == xb.XPR_ERR_CAPACITY and need == I
+    ws.zero_(); pipe.tile_ranges.fill_(-1)
+    xb.xpr_bin_sort(pipe.depth, pipe.tile_rect, pipe.tile_count, pipe.cam, pipe.cfg, 0, guard_k, guard_v,
+                    pipe.tile_ranges, ws, sync=False)
+    torch.cuda.synchronize()
+    counts = ws[:16].view(torch.int64).tolist()
+    assert counts == [I, 0]
+    assert (guard_k == -7).all() and (guard_v == -7).all() and not pipe.tile_ranges.any()
+    # a retry with the reported capacity succeeds
+    pipe._alloc_pairs(need + 1)
+    assert pipe.bin_sort() == I
+
+
+def test_binding_rejects_a_tensor_of_the_wrong_element_type():
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline
+    sc = scenes.make_scene(1, n_override=50)
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], scenes.default_render_config(sc))
+    m, s, q, o, sh = pipeline.scene_to_device(sc)
+    with pytest.raises(TypeError):
+        pipe.project(m.double(), s, q, o, sh)
+    with pytest.raises(TypeError):
+        xb.xpr_bin_sort(pipe.depth, pipe.tile_rect.long(), pipe.tile_count, pipe.cam, pipe.cfg, pipe.pair_capacity,
+                        pipe.keys_sorted, pipe.vals_sorted, pipe.tile_ranges, pipe.workspace)
+
+
 def test_fullscreen_gaussian_and_depth_ties():
     """One Gaussian covering every tile plus exact duplicates (equal keys): the stable order of equal
     keys is ascending Gaussian index (C10), so sorted values must match bit-exactly."""
