@@ -306,8 +306,7 @@ def run_ours(args):
         xb.xpr_rasterize_ray_stats(pipe.cam, pipe.cfg, pipe.ray_rec, pipe.conic_opac, pipe.rgb, pipe.lnv,
                                    pipe.pixel_rays, pipe.vals_sorted, pipe.tile_ranges, stats)
     else:
-        xb.xpr_rasterize_stats(pipe.cam, pipe.cfg, pipe.mean2d, pipe.conic_opac, pipe.rgb, pipe.lnv, pipe.vals_sorted,
-                               pipe.tile_ranges, stats)
+        xb.xpr_rasterize_stats(pipe.cam, pipe.cfg, pipe.shade_rec, pipe.vals_sorted, pipe.tile_ranges, stats)
     fwd_ops = (RAY_FWD_OPS_VISIT, RAY_FWD_OPS_PASS) if args.ray_eval else (FWD_OPS_VISIT, FWD_OPS_PASS)
     bwd_ops = (RAY_BWD_OPS_VISIT, RAY_BWD_OPS_PASS) if args.ray_eval else (BWD_OPS_VISIT, BWD_OPS_PASS)
     kname = "rasterize_ray_%s_kernel" if args.ray_eval else "rasterize_%s_kernel"

@@ -75,7 +75,11 @@ int32_t xpr_version(void);           /* 10000*major + 100*minor + patch */
  *   out: mean2d[N,2], conic_opac[N,4] = (A,B,C,o_eff) with (A,B,C) the inverse of the low-passed
  *        2D covariance, rgb[N,3], depth[N] (camera z of the mean), lnv[N] = ln(o_eff/alpha_thresh),
  *        tile_rect[N,4] = (x_min,y_min,x_max,y_max) half-open in tile units,
- *        tile_count[N] = rectangle area if visible else 0, flags[N].
+ *        tile_count[N] = rectangle area if visible else 0, flags[N];
+ *        shade_rec[N,12] (may be NULL) = the shader data p_sd of the primitive packed as the
+ *        compositing calls read it, 3 x float4, 16-byte aligned:
+ *          (mx, my, -A/2, -B | -C/2, -lnv, log2 o_eff, depth | r, g, b, o_eff)
+ *        -- the pre-scaled conic of reading C25 (exact in fp32); log2 by lg2.approx (it only feeds exp()).
  *   For a culled Gaussian only tile_count (=0) and flags (=0) are written; its other outputs are
  *   left untouched (they are never read downstream).
  *   Arithmetic follows rule R1: fp32, every operation individually rounded, no FMA contraction,
@@ -84,7 +88,15 @@ int32_t xpr_version(void);           /* 10000*major + 100*minor + patch */
 int32_t xpr_project(int64_t N, const float* means, const float* scales, const float* quats,
                     const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
                     float* mean2d, float* conic_opac, float* rgb, float* depth, float* lnv,
-                    int32_t* tile_rect, uint32_t* tile_count, uint8_t* flags, void* stream);
+                    int32_t* tile_rect, uint32_t* tile_count, uint8_t* flags, float* shade_rec, void* stream);
+
+/*
+ * xpr_shade_record -- builds shade_rec[N,12] (layout above) from the separate projection outputs, for a caller
+ * whose projection did not come from xpr_project; depth may be NULL (slot 7 is then 0; it is only read by the
+ * rendered-depth feature).  Records of culled Gaussians (tile_count == 0) are not written.
+ */
+int32_t xpr_shade_record(int64_t N, const float* mean2d, const float* conic_opac, const float* rgb, const float* lnv,
+                         const float* depth, const uint32_t* tile_count, float* shade_rec, void* stream);
 
 /*
  * xpr_bin_sort -- Rasterizer stage: prefix-sum of tile counts, replication,
@@ -150,10 +162,11 @@ int32_t xpr_bin_sort_cull(int64_t N, const float* depth, const int32_t* tile_rec
  *   skip if power > 0 (L289) or power < -lnv (alpha < alpha_thresh, L679, C12);
  *   alpha = min(alpha_max, o_eff exp(power));  T' = T (1 - alpha);  stop WITHOUT blending if
  *   T' < t_min;  C += rgb alpha T;  T = T'.   Finally C += T bg.
+ *   in : shade_rec[N,12] of xpr_project (or xpr_shade_record), the lists of xpr_bin_sort[_cull].
  *   out: image[H,W,3], final_T[H,W], n_contrib[H,W] = 1 + list position of the last blended entry.
+ *   The records of a tile's list are gathered into shared memory by cp.async (three-stage ring).
  */
-int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                          const float* conic_opac, const float* rgb, const float* lnv,
+int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
                           const uint32_t* vals_sorted, const uint32_t* tile_ranges,
                           float* image, float* final_T, uint32_t* n_contrib, void* stream);
 
@@ -162,8 +175,7 @@ int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t 
  * xpr_rasterize_fwd without writing an image; stats[0..3] (DEVICE uint64[4], overwritten) =
  * {pixel-pairs visited, pixel-pairs passing both gates, pixel-pairs blended, sum of n_contrib}.
  */
-int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                            const float* conic_opac, const float* rgb, const float* lnv,
+int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
                             const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats,
                             void* stream);
 
@@ -175,8 +187,7 @@ int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_
  *        ACCUMULATED with fp32 atomics; zero-filled first by this call when zero_init != 0.
  *        (with one fill instead of four when the four arrays are adjacent slices of one allocation, in this order).
  */
-int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                          const float* conic_opac, const float* rgb, const float* lnv,
+int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
                           const uint32_t* vals_sorted, const uint32_t* tile_ranges,
                           const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
                           float* g_mean2d, float* g_conic, float* g_opac, float* g_rgb,
@@ -242,7 +253,7 @@ int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const fl
  *   depth image D[H,W] = sum_k z_k alpha_k T_k  (z_k = `depth` of xpr_project, the depth of the sort key, L149),
  *   accumulated opacity A[H,W] = sum_k alpha_k T_k.
  * xpr_rasterize_feat_fwd -- xpr_rasterize_fwd that also writes depth_img and alpha_img in the same walk (image,
- *   final_T, n_contrib as xpr_rasterize_fwd: same gates, clamp and exit).  depth: DEVICE fp32 [N].
+ *   final_T, n_contrib as xpr_rasterize_fwd: same gates, clamp and exit).  z_k is slot 7 of shade_rec.
  * xpr_rasterize_feat_bwd -- xpr_rasterize_bwd with the two extra incoming gradients dL_ddepth[H,W], dL_dalpha[H,W]
  *   and the extra output g_depth[N] = dL/dz; ACCUMULATES like xpr_rasterize_bwd, zero-filled first when
  *   zero_init != 0 (one fill when g_mean2d, g_conic, g_opac, g_rgb, g_depth are adjacent slices, in this order).
@@ -250,13 +261,11 @@ int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const fl
  *   tile_count[i] > 0 (call it after xpr_project_bwd, which overwrites g_means).
  * Errors as the colour calls: null / misaligned pointer, N < 0 -> XPR_ERR_INVALID_ARG before any launch.
  */
-int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                               const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
                                const uint32_t* vals_sorted, const uint32_t* tile_ranges,
                                float* image, float* final_T, uint32_t* n_contrib, float* depth_img,
                                float* alpha_img, void* stream);
-int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                               const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
                                const uint32_t* vals_sorted, const uint32_t* tile_ranges,
                                const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
                                const float* dL_ddepth, const float* dL_dalpha,

@@ -18,7 +18,7 @@ XPR_OK, XPR_ERR_INVALID_ARG, XPR_ERR_CAPACITY, XPR_ERR_CUDA, XPR_ERR_UNSUPPORTED
 FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_RGB_POS_B = 1, 2, 4, 8, 16, 32
 
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
-           "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
+           "xpr_shade_record", "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
            "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad")
 
@@ -126,11 +126,18 @@ def xpr_version() -> int:
 
 
 def xpr_project(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, depth,
-                lnv, tile_rect, tile_count, flags, stream=None):
+                lnv, tile_rect, tile_count, flags, shade_rec=None, stream=None):
     N = int(means.shape[0])
     _check(lib().xpr_project(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), _p(opacities, _F32), _p(sh, _F32), C.byref(cam),
                              C.byref(cfg), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32), _p(depth, _F32), _p(lnv, _F32), _p(tile_rect, _I32),
-                             _p(tile_count, _I32), _p(flags, _U8), _stream(stream)), "xpr_project")
+                             _p(tile_count, _I32), _p(flags, _U8), _p(shade_rec, _F32), _stream(stream)), "xpr_project")
+
+
+def xpr_shade_record(mean2d, conic_opac, rgb, lnv, depth, tile_count, shade_rec, stream=None):
+    N = int(mean2d.shape[0])
+    _check(lib().xpr_shade_record(C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32), _p(lnv, _F32),
+                                  _p(depth, _F32), _p(tile_count, _I32), _p(shade_rec, _F32), _stream(stream)),
+           "xpr_shade_record")
 
 
 def xpr_bin_sort_workspace(N: int, pair_capacity: int, n_tiles: int) -> int:
@@ -166,28 +173,27 @@ def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, p
     return st, int(n_pairs.value)
 
 
-def xpr_rasterize_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, image,
-                      final_T, n_contrib, stream=None):
-    N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
-                                   _p(lnv, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32), _p(n_contrib, _I32),
+def xpr_rasterize_fwd(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, tile_ranges, image, final_T, n_contrib,
+                      stream=None):
+    N = int(shade_rec.shape[0])
+    _check(lib().xpr_rasterize_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(shade_rec, _F32), _p(vals_sorted, _I32),
+                                   _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32), _p(n_contrib, _I32),
                                    _stream(stream)), "xpr_rasterize_fwd")
 
 
-def xpr_rasterize_stats(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, stats,
-                        stream=None):
-    N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
-                                     _p(lnv, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(stats, _I64), _stream(stream)),
+def xpr_rasterize_stats(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, tile_ranges, stats, stream=None):
+    N = int(shade_rec.shape[0])
+    _check(lib().xpr_rasterize_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(shade_rec, _F32),
+                                     _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(stats, _I64), _stream(stream)),
            "xpr_rasterize_stats")
 
 
-def xpr_rasterize_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, vals_sorted, tile_ranges, final_T,
-                      n_contrib, dL_dimage, g_mean2d, g_conic, g_opac, g_rgb, zero_init: bool = True, stream=None):
-    N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
-                                   _p(lnv, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32), _p(n_contrib, _I32),
-                                   _p(dL_dimage, _F32), _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
+def xpr_rasterize_bwd(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, tile_ranges, final_T, n_contrib,
+                      dL_dimage, g_mean2d, g_conic, g_opac, g_rgb, zero_init: bool = True, stream=None):
+    N = int(shade_rec.shape[0])
+    _check(lib().xpr_rasterize_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(shade_rec, _F32), _p(vals_sorted, _I32),
+                                   _p(tile_ranges, _I32), _p(final_T, _F32), _p(n_contrib, _I32), _p(dL_dimage, _F32),
+                                   _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
                                    C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_bwd")
 
 
@@ -246,24 +252,25 @@ def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_rec, g_m
 
 # ---- Rendered depth and accumulated opacity (xpr.h) --------------------------------------------
 
-def xpr_rasterize_feat_fwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, depth, vals_sorted,
-                           tile_ranges, image, final_T, n_contrib, depth_img, alpha_img, stream=None):
-    N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
-                                        _p(lnv, _F32), _p(depth, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32),
-                                        _p(n_contrib, _I32), _p(depth_img, _F32), _p(alpha_img, _F32), _stream(stream)),
-           "xpr_rasterize_feat_fwd")
+def xpr_rasterize_feat_fwd(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, tile_ranges, image, final_T,
+                           n_contrib, depth_img, alpha_img, stream=None):
+    N = int(shade_rec.shape[0])
+    _check(lib().xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(shade_rec, _F32),
+                                        _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(image, _F32),
+                                        _p(final_T, _F32), _p(n_contrib, _I32), _p(depth_img, _F32),
+                                        _p(alpha_img, _F32), _stream(stream)), "xpr_rasterize_feat_fwd")
 
 
-def xpr_rasterize_feat_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, rgb, lnv, depth, vals_sorted,
-                           tile_ranges, final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_mean2d, g_conic,
-                           g_opac, g_rgb, g_depth, zero_init: bool = True, stream=None):
-    N = int(mean2d.shape[0])
-    _check(lib().xpr_rasterize_feat_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(mean2d, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
-                                        _p(lnv, _F32), _p(depth, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32),
-                                        _p(n_contrib, _I32), _p(dL_dimage, _F32), _p(dL_ddepth, _F32), _p(dL_dalpha, _F32), _p(g_mean2d, _F32),
-                                        _p(g_conic, _F32), _p(g_opac, _F32), _p(g_rgb, _F32), _p(g_depth, _F32),
-                                        C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_feat_bwd")
+def xpr_rasterize_feat_bwd(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, tile_ranges, final_T, n_contrib,
+                           dL_dimage, dL_ddepth, dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth,
+                           zero_init: bool = True, stream=None):
+    N = int(shade_rec.shape[0])
+    _check(lib().xpr_rasterize_feat_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(shade_rec, _F32),
+                                        _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32),
+                                        _p(n_contrib, _I32), _p(dL_dimage, _F32), _p(dL_ddepth, _F32),
+                                        _p(dL_dalpha, _F32), _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32),
+                                        _p(g_rgb, _F32), _p(g_depth, _F32), C.c_int32(1 if zero_init else 0),
+                                        _stream(stream)), "xpr_rasterize_feat_bwd")
 
 
 def xpr_depth_bwd(cam: XprCamera, tile_count, g_depth, g_means, stream=None):

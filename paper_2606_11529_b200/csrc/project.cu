@@ -241,7 +241,7 @@ project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const f
                const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
                float* __restrict__ mean2d, float* __restrict__ conic_opac, float* __restrict__ rgb,
                float* __restrict__ depth, float* __restrict__ lnv, int32_t* __restrict__ rect,
-               uint32_t* __restrict__ tcount, uint8_t* __restrict__ flags) {
+               uint32_t* __restrict__ tcount, uint8_t* __restrict__ flags, float4* __restrict__ shade_rec) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
@@ -281,12 +281,17 @@ project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const f
     reinterpret_cast<int4*>(rect)[i] = make_int4(F.rect[0], F.rect[1], F.rect[2], F.rect[3]);
     tcount[i] = F.tc;
     flags[i] = fl;
+    if (shade_rec) {   // shader data p_sd as the compositing kernels read it: pre-scaled conic (C25, exact)
+        shade_rec[3 * i] = make_float4(F.m[0], F.m[1], -0.5f * F.A, -F.B);
+        shade_rec[3 * i + 1] = make_float4(-0.5f * F.C, -F.lnv, __log2f(F.o_eff), F.p[2]);
+        shade_rec[3 * i + 2] = make_float4(col[0], col[1], col[2], F.o_eff);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
 // Backward.  The forward intermediates are recomputed in fp32 exactly as above (so the clamp and
-// culling decisions are the forward's); the chain rule itself runs in fp64 (B200 has a full-rate
-// FP64 pipe and the kernel is HBM-bound), which keeps the ill-conditioned conic -> covariance
+// culling decisions are the forward's); the chain rule itself runs in fp64 (the kernel is HBM- and
+// latency-bound, not bound by the FP64 pipe, which runs at half the fp32 rate on B200), which keeps the ill-conditioned conic -> covariance
 // step (G2 = -K G_K K) inside the 1e-3 relative gradient tolerance.
 // ---------------------------------------------------------------------------------------------
 typedef double B;
@@ -668,13 +673,15 @@ using namespace xpr;
 extern "C" int32_t xpr_project(int64_t N, const float* means, const float* scales, const float* quats,
                                const float* opacities, const float* sh, const xpr_camera* cam,
                                const xpr_config* cfg, float* mean2d, float* conic_opac, float* rgb, float* depth,
-                               float* lnv, int32_t* tile_rect, uint32_t* tile_count, uint8_t* flags, void* stream) {
+                               float* lnv, int32_t* tile_rect, uint32_t* tile_count, uint8_t* flags,
+                               float* shade_rec, void* stream) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0 || N > 0x7fffffffLL) return XPR_ERR_INVALID_ARG;
     if (N == 0) return XPR_OK;
     if (!aligned(means, 4) || !aligned(scales, 4) || !aligned(quats, 16) || !aligned(opacities, 4) ||
         !aligned(sh, 16) || !aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) ||
-        !aligned(depth, 4) || !aligned(lnv, 4) || !aligned(tile_rect, 16) || !aligned(tile_count, 4) || !flags)
+        !aligned(depth, 4) || !aligned(lnv, 4) || !aligned(tile_rect, 16) || !aligned(tile_count, 4) || !flags ||
+        (shade_rec && !aligned(shade_rec, 16)))
         return XPR_ERR_INVALID_ARG;
     ProjParams P;
     if (int32_t s = make_params(cam, cfg, P)) return s;
@@ -683,7 +690,8 @@ extern "C" int32_t xpr_project(int64_t N, const float* means, const float* scale
     const unsigned blocks = (unsigned)((N + threads - 1) / threads);
 #define XPR_GO(KK)                                                                                              \
     project_kernel<KK><<<blocks, threads, 0, st>>>(N, P, means, scales, quats, opacities, sh, mean2d, conic_opac, \
-                                                   rgb, depth, lnv, tile_rect, tile_count, flags)
+                                                   rgb, depth, lnv, tile_rect, tile_count, flags,                \
+                                                   reinterpret_cast<float4*>(shade_rec))
     switch (cfg->sh_degree) {
         case 0: XPR_GO(1); break;
         case 1: XPR_GO(4); break;

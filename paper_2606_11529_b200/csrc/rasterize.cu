@@ -1,16 +1,26 @@
-// rasterize.cu -- xpr_rasterize_fwd / xpr_rasterize_bwd: per-tile front-to-back alpha compositing
-// (Algorithm 1, Listing 1) and its reverse-mode pass.
+// rasterize.cu -- xpr_rasterize_fwd / xpr_rasterize_bwd (+ the depth / accumulated-opacity variants
+// xpr_rasterize_feat_fwd / _bwd): per-tile front-to-back alpha compositing (Algorithm 1,
+// Listing 1) and its reverse-mode pass.
 //
-// One CTA per 16x16 tile, one thread per pixel.  The tile's list vals_sorted[start..end) is
-// staged through shared memory in batches; every thread walks the batch with warp-broadcast
-// LDS.128 reads.  Decisions (the power > 0 guard and the alpha gate) are taken on `power`,
-// computed in the fixed fp32 order of rule R3 with explicit _rn intrinsics, never on exp().
+// One CTA per 16x16 tile.  The tile's list vals_sorted[start..end) is a list of Gaussian indices; the shader
+// data p_sd of a Gaussian is one 48-byte record shade_rec[g] = 3 x float4
+//     (mx, my, qa, qb | qc, thr, log2 o, z | r, g, b, o),   qa = -A/2, qb = -B, qc = -C/2, thr = -lnv   (C25),
+// written by xpr_project.  Batches of records are gathered into shared memory with cp.async (16-byte LDGSTS, no
+// register staging) through a three-stage ring: while batch b is walked, the copies of batches b+1 and b+2 are
+// in flight and the list indices of batch b+3 are being loaded, so a CTA waits for memory only at its start and
+// there is one barrier per batch.  Every thread walks the batch with warp-broadcast LDS.128 reads.
+// Decisions (the power > 0 guard and the alpha gate) are taken on `power`, computed in the fixed fp32 order of
+// rule R3, never on exp().  A thread owns 2 (forward) or 4 (backward) pixels of one tile row and works on them
+// as PAIRS with the packed fp32 instructions of sm_100 (fma.rn.f32x2 -> FFMA2 ...: two individually rounded
+// results per issue slot -- the kernels are issue-bound), packed.cuh.
 #include "common.cuh"
+#include "packed.cuh"
 
 namespace xpr {
 namespace {
 
-constexpr int BLOCK = TILE * TILE;   // 256 threads = 256 pixels
+constexpr int BLOCK = TILE * TILE;   // 256 pixels
+constexpr int STAGES = 3;            // cp.async ring depth
 
 struct RasterParams {
     int W, H, TW;
@@ -19,164 +29,201 @@ struct RasterParams {
     const uint32_t* order;   // xpr_config.tile_order: CTA b works on tile order[b] (longest lists first), or NULL
 };
 
-// power = fma(fma(qa, dx, qb*dy), dx, (qc*dy)*dy) with qa = -A/2, qb = -B, qc = -C/2 (R3, C25)
-__device__ __forceinline__ float eval_power(float qa, float qb, float qc, float dx, float dy) {
-    return __fmaf_rn(__fmaf_rn(qa, dx, __fmul_rn(qb, dy)), dx, __fmul_rn(__fmul_rn(qc, dy), dy));
-}
-
-// o * exp(power) = ex2(power * log2 e + log2 o): one FFMA + one MUFU; l2o = log2 o is staged with the record
-__device__ __forceinline__ float opac_exp(float power, float l2o) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(fmaf(power, 1.4426950408889634f, l2o)));
-    return y;
-}
-
-__device__ __forceinline__ float fast_exp(float x) {   // ex2.approx(x * log2 e); x in [-lnv, 0]
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x * 1.4426950408889634f));
-    return y;
+// gather one record (3 x 16 bytes) into a ring slot
+__device__ __forceinline__ void stage_record(float4* slot, const float4* __restrict__ rec, uint32_t g) {
+    const float4* src = rec + 3 * (size_t)g;
+    cp_async16(slot, src);
+    cp_async16(slot + 1, src + 1);
+    cp_async16(slot + 2, src + 2);
 }
 
 // Forward compositing (a8).  One CTA per 16x16 tile, in two shapes:
 //   PPT = 2: 128 threads, a thread owns the two pixels (x, y) and (x + 8, y) of one row, so the row terms
 //            of `power` (dy, qb*dy, (qc*dy)*dy) and the shared-memory reads of a list entry are paid once
-//            per two pixels -- fewer instructions per pixel-pair (throughput shape, large images);
+//            per two pixels, and the pixel pair shares packed instructions (throughput shape, large images);
 //   PPT = 1: 256 threads, one pixel each -- twice the warps on a tile, i.e. half the critical path of a
 //            heavy tile (latency shape, images with few tiles where the longest list bounds the kernel).
-// The arithmetic per pixel is exactly eval_power's (rule R3) in both.
+// The arithmetic per pixel is exactly power = fma(fma(qa, dx, qb*dy), dx, (qc*dy)*dy) (rule R3) in both.
+// BF (lists produced with tile_cull: > 90 % of the visited pairs pass the gate): branch-free blend -- a pixel
+//   that is done or gated enters with alpha = 0, so T' = T >= t_min and w = 0; otherwise gated pairs are branched over.
 // STATS = true: the same walk, additionally counting pixel-pair events into stats[0..3] =
-// {visited, passed both gates, blended, sum of n_contrib} (xpr_rasterize_stats; roofline accounting).
+//   {visited, passed both gates, blended, sum of n_contrib} (xpr_rasterize_stats; roofline accounting).
+// FEAT = true (xpr_rasterize_feat_fwd, SURVEY 8(f) f3, reading C31): the same walk also blends the depth image
+//   D = sum z alpha T and the accumulated opacity A = sum alpha T; z rides in the record.
 #ifndef XPR_FWD_PPT2_MIN_TILES
 #define XPR_FWD_PPT2_MIN_TILES 4096
 #endif
 constexpr int FWD_PPT2_MIN_TILES = XPR_FWD_PPT2_MIN_TILES;
 
-// FEAT = true (xpr_rasterize_feat_fwd, SURVEY 8(f) f3, reading C31): the same walk also blends the depth image
-// D = sum z alpha T and the accumulated opacity A = sum alpha T; z rides in the record's unused slot.
-template <bool STATS, int PPT, bool BF, bool FEAT = false>
+template <bool STATS, int PPT, bool BF, bool FEAT>
 __global__ void __launch_bounds__(BLOCK / PPT)
-rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
-                     const float* __restrict__ rgb, const float* __restrict__ lnv,
-                     const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
-                     float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
-                     unsigned long long* __restrict__ stats, const float* __restrict__ depth = nullptr,
-                     float* __restrict__ depth_img = nullptr, float* __restrict__ alpha_img = nullptr) {
-    // record of one list entry: 3 x float4 = (mx, my, qa, qb | qc, thr = -lnv, log2 o, z (FEAT) | r, g, b, -)
-    constexpr int FWD_BATCH = BLOCK / PPT;          // one list entry staged per thread
-    __shared__ float4 s_rec[3 * FWD_BATCH];
+rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint32_t* __restrict__ vals,
+                     const uint2* __restrict__ ranges, float* __restrict__ image, float* __restrict__ final_T,
+                     uint32_t* __restrict__ n_contrib, unsigned long long* __restrict__ stats,
+                     float* __restrict__ depth_img, float* __restrict__ alpha_img) {
+    constexpr int THREADS = BLOCK / PPT, B = THREADS, ROW = TILE / PPT;
+    constexpr bool PACKED = BF && (PPT == 2);
+    __shared__ float4 s_rec[STAGES][3 * B];
+    const int tid = threadIdx.x;
     const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
-    constexpr int FWD_THREADS = BLOCK / PPT, ROW = TILE / PPT;
-    const int px0 = tx * TILE + (threadIdx.x % ROW), px1 = px0 + 8, py = ty * TILE + (threadIdx.x / ROW);
+    const int px0 = tx * TILE + (tid % ROW), px1 = px0 + 8, py = ty * TILE + (tid / ROW);
     const bool in0 = (px0 < P.W) && (py < P.H), in1 = (PPT == 2) && (px1 < P.W) && (py < P.H);
     const float pxc0 = (float)px0 + 0.5f, pxc1 = (float)px1 + 0.5f, pyc = (float)py + 0.5f;
+    const f32x2 px2 = pack2(pxc0, pxc1);
     const uint2 rg = ranges[tile];
     const uint32_t len = rg.y - rg.x;
+    const uint32_t* const list = vals + rg.x;
 
-    float Ta = 1.0f, Ca0 = 0.0f, Ca1 = 0.0f, Ca2 = 0.0f;     // pixel (px0, py)
-    float Tb = 1.0f, Cb0 = 0.0f, Cb1 = 0.0f, Cb2 = 0.0f;     // pixel (px1, py)
-    float Da = 0.0f, Aa = 0.0f, Db = 0.0f, Ab = 0.0f;         // FEAT: depth image and accumulated opacity
+    // pixel state: scalar (branchy shapes) or packed pairs (lane 0 = pixel a, lane 1 = pixel b)
+    float Ta = 1.0f, Ca0 = 0.0f, Ca1 = 0.0f, Ca2 = 0.0f, Tb = 1.0f, Cb0 = 0.0f, Cb1 = 0.0f, Cb2 = 0.0f;
+    float Da = 0.0f, Aa = 0.0f, Db = 0.0f, Ab = 0.0f;
+    f32x2 T2 = pack2(1.0f, 1.0f), C0_2 = 0ull, C1_2 = 0ull, C2_2 = 0ull, D2 = 0ull, A2 = 0ull;
     uint32_t last_a = 0, last_b = 0;
     bool act_a = in0, act_b = in1;                            // still compositing
     uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
+    float amax = P.amax, tmin = P.tmin;
+    asm volatile("" : "+f"(amax), "+f"(tmin));     // keep both in registers (else re-read from the constant bank per entry)
 
-    // The list is walked in groups of 4 entries.  Phase 1 of a group computes the 4 (x PPT) values of
-    // `power` -- independent of each other and of the transmittance, so their latencies overlap -- and
-    // phase 2 runs the sequential part (gate, alpha, T' = T (1 - alpha), exit test, blend).
-#define XPR_FWD_POWER(u, rp)                                                                          \
-    {                                                                                                \
-        const float4 ge = (rp)[0];                                                                   \
-        const float4 ga = (rp)[1];                                                                   \
-        const float dy = pyc - ge.y;                                                                 \
-        const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);               \
-        const float dxa = pxc0 - ge.x;                                                               \
-        pw_a[u] = __fmaf_rn(__fmaf_rn(ge.z, dxa, t1), dxa, t2);                                      \
-        if (PPT == 2) {                                                                              \
-            const float dxb = pxc1 - ge.x;                                                           \
-            pw_b[u] = __fmaf_rn(__fmaf_rn(ge.z, dxb, t1), dxb, t2);                                  \
-        }                                                                                            \
-        thr[u] = ga.y; op[u] = ga.z;                                                                 \
-        if (FEAT) zz[u] = ga.w;                                                                      \
-        if (BF) c_##u = (rp)[2];                                                                     \
+    // ---- staging ring: batches 0 and 1 on their way, indices of batch 2 loading -------------------------------
+    {
+        uint32_t g0 = 0, g1 = 0;
+        if ((uint32_t)tid < len) g0 = list[tid];
+        if ((uint32_t)(B + tid) < len) g1 = list[B + tid];
+        if ((uint32_t)tid < len) stage_record(&s_rec[0][3 * tid], rec, g0);
+        cp_async_commit();
+        if ((uint32_t)(B + tid) < len) stage_record(&s_rec[1][3 * tid], rec, g1);
+        cp_async_commit();
     }
-    // valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12)
-    // BF (lists produced with tile_cull: > 90 % of the visited pairs pass the gate): branch-free -- a pixel that
-    // is done or gated enters with alpha = 0, so T' = T >= t_min and w = 0; otherwise the gated pairs are branched over
-#define XPR_FWD_BLEND(act, power, u, rp, T, C0, C1, C2, last, pos, Dv, Av)                            \
-    if (BF) {                                                                                        \
-        if (STATS) {                                                                                 \
-            if (act) { ++n_visit; if (!((power) > 0.0f) && !((power) < thr[u])) ++n_pass; }          \
-        }                                                                                            \
-        const bool pass = act && !((power) > 0.0f) && !((power) < thr[u]);                           \
-        const float alpha = pass ? fminf(amax, opac_exp(power, op[u])) : 0.0f;      /* C11 */        \
-        const float Tn = T * (1.0f - alpha);                                                         \
-        const bool stop = Tn < tmin;                                        /* C12: stop, no blend */\
-        const bool blend = pass && !stop;                                                            \
-        act = act && !stop;                                                                          \
-        const float w = blend ? alpha * T : 0.0f;                                                    \
-        C0 = fmaf(c_##u.x, w, C0); C1 = fmaf(c_##u.y, w, C1); C2 = fmaf(c_##u.z, w, C2);             \
-        if (FEAT) { Dv = fmaf(zz[u], w, Dv); Av += w; }                                              \
-        T = blend ? Tn : T;                                                                          \
-        last = blend ? (pos) : last;                                                                 \
-        if (STATS && blend) ++n_blend;                                                               \
-    } else if (act) {                                                                                \
-        if (STATS) ++n_visit;                                                                        \
-        if (!((power) > 0.0f) && !((power) < thr[u])) {                                              \
-            if (STATS) ++n_pass;                                                                     \
-            const float alpha = fminf(amax, opac_exp(power, op[u]));        /* C11 */                \
-            const float Tn = T * (1.0f - alpha);                                                     \
-            if (Tn < tmin) {                                                /* C12: stop, no blend */\
-                act = false;                                                                         \
-            } else {                                                                                 \
-                const float4 c = (rp)[2];                                                            \
-                const float w = alpha * T;                                                           \
-                C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);                 \
-                if (FEAT) { Dv = fmaf(zz[u], w, Dv); Av += w; }                                      \
-                T = Tn;                                                                              \
-                last = (pos);                                                                        \
-                if (STATS) ++n_blend;                                                                \
-            }                                                                                        \
-        }                                                                                            \
-    }
-#define XPR_FWD_STEP(u, rp, pos)                                                                      \
-    XPR_FWD_BLEND(act_a, pw_a[u], u, rp, Ta, Ca0, Ca1, Ca2, last_a, pos, Da, Aa)                      \
-    if (PPT == 2) XPR_FWD_BLEND(act_b, pw_b[u], u, rp, Tb, Cb0, Cb1, Cb2, last_b, pos, Db, Ab)
+    uint32_t g_next = ((uint32_t)(2 * B + tid) < len) ? list[2 * B + tid] : 0u;   // index of this thread's entry of batch b + 2
 
-    const float amax = P.amax, tmin = P.tmin;
-    float pw_a[4], pw_b[4], thr[4], op[4], zz[4];
-    float4 c_0, c_1, c_2, c_3;                         // colours of the group's entries
-    for (uint32_t base = 0; base < len; base += FWD_BATCH) {
-        if (__syncthreads_or(act_a || act_b) == 0) break;
-        const uint32_t cnt = min((uint32_t)FWD_BATCH, len - base);
-        for (uint32_t e = threadIdx.x; e < cnt; e += FWD_THREADS) {
-            const uint32_t g = vals[rg.x + base + e];
-            const float2 m = mean2d[g];
-            const float4 co = conic_opac[g];
-            float4* rec = s_rec + 3 * e;
-            rec[0] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-            rec[1] = make_float4(-0.5f * co.z, -lnv[g], __log2f(co.w), FEAT ? depth[g] : 0.0f);
-            rec[2] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], 0.0f);
+    float pw_a[4], pw_b[4], thr[4], l2o[4], zz[4];
+    f32x2 pw2[4];
+    float4 col[4];                                             // colours of the group's entries (BF)
+    uint32_t stage = 0;
+    for (uint32_t base = 0; base < len; base += B) {
+        cp_async_wait<1>();                                    // this thread's copies of batch b have landed
+        if (__syncthreads_or(act_a || act_b) == 0) break;      // ... everyone's; and everyone is done with batch b - 1
+        {   // batch b + 2 goes into the slot batch b - 1 just left; then the indices of batch b + 3 start loading
+            const uint32_t s2 = (stage + 2 >= STAGES) ? stage + 2 - STAGES : stage + 2;
+            if (base + 2 * B + tid < len) stage_record(&s_rec[s2][3 * tid], rec, g_next);
+            cp_async_commit();
+            g_next = (base + 3 * B + tid < len) ? list[base + 3 * B + tid] : 0u;
         }
-        __syncthreads();
+        const uint32_t cnt = min((uint32_t)B, len - base);
+        // The list is walked in groups of 4 entries.  Phase 1 of a group computes the 4 (x PPT) values of
+        // `power` -- independent of each other and of the transmittance, so their latencies overlap -- and
+        // phase 2 runs the sequential part (gate, alpha, T' = T (1 - alpha), exit test, blend).
+        auto power = [&](int u, const float4* rq) {
+            const float4 ge = rq[0];
+            const float4 ga = rq[1];
+            const float dy = pyc - ge.y;
+            const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);
+            if (PPT == 2) {
+                const f32x2 dx2 = sub2(px2, bcast2(ge.x));
+                pw2[u] = fma2(fma2(bcast2(ge.z), dx2, bcast2(t1)), dx2, bcast2(t2));
+                if (!PACKED) unpack2(pw2[u], pw_a[u], pw_b[u]);
+            } else {
+                const float dxa = pxc0 - ge.x;
+                pw_a[u] = __fmaf_rn(__fmaf_rn(ge.z, dxa, t1), dxa, t2);
+            }
+            thr[u] = ga.y; l2o[u] = ga.z;
+            if (FEAT) zz[u] = ga.w;
+            if (BF) col[u] = rq[2];
+        };
+        // valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12)
+        auto blend_packed = [&](int u, uint32_t pos) {
+            float pa, pb;
+            unpack2(pw2[u], pa, pb);
+            const bool pass_a = act_a && !(pa > 0.0f) && !(pa < thr[u]);
+            const bool pass_b = act_b && !(pb > 0.0f) && !(pb < thr[u]);
+            float ea, eb;                                       // o exp(power) = ex2(power log2 e + log2 o)
+            unpack2(fma2(pw2[u], bcast2(LOG2E), bcast2(l2o[u])), ea, eb);
+            // a gated or finished pixel gets ex2(-inf) = 0: alpha = 0 without a select after the MUFU
+            const float al_a = fminf(amax, ex2_approx(pass_a ? ea : -INFINITY));      // C11
+            const float al_b = fminf(amax, ex2_approx(pass_b ? eb : -INFINITY));
+            const f32x2 al2 = pack2(al_a, al_b);
+            float tn_a, tn_b, w_a, w_b, t_a, t_b;
+            unpack2(mul2(T2, sub2(bcast2(1.0f), al2)), tn_a, tn_b);             // T' = T (1 - alpha)
+            unpack2(mul2(al2, T2), w_a, w_b);
+            unpack2(T2, t_a, t_b);
+            act_a = act_a && !(tn_a < tmin);                    // C12: stop without blending
+            act_b = act_b && !(tn_b < tmin);
+            // a pixel that was done or gated has alpha = 0: w = 0 and T' = T already; only the stopping entry needs the select
+            const f32x2 w2 = pack2(act_a ? w_a : 0.0f, act_b ? w_b : 0.0f);
+            T2 = pack2(act_a ? tn_a : t_a, act_b ? tn_b : t_b);
+            C0_2 = fma2(bcast2(col[u].x), w2, C0_2);
+            C1_2 = fma2(bcast2(col[u].y), w2, C1_2);
+            C2_2 = fma2(bcast2(col[u].z), w2, C2_2);
+            if (FEAT) { D2 = fma2(bcast2(zz[u]), w2, D2); A2 = add2(A2, w2); }
+            last_a = (pass_a && act_a) ? pos : last_a;
+            last_b = (pass_b && act_b) ? pos : last_b;
+        };
+        auto blend_scalar = [&](bool& act, float pw, int u, const float4* rq, float& T, float& C0, float& C1, float& C2,
+                                uint32_t& last, uint32_t pos, float& Dv, float& Av) {
+            if (BF) {
+                const bool pass = act && !(pw > 0.0f) && !(pw < thr[u]);
+                const float alpha = pass ? fminf(amax, ex2_approx(fmaf(pw, LOG2E, l2o[u]))) : 0.0f;
+                const float Tn = T * (1.0f - alpha);
+                const bool stop = Tn < tmin;
+                const bool bl = pass && !stop;
+                act = act && !stop;
+                const float w = bl ? alpha * T : 0.0f;
+                C0 = fmaf(col[u].x, w, C0); C1 = fmaf(col[u].y, w, C1); C2 = fmaf(col[u].z, w, C2);
+                if (FEAT) { Dv = fmaf(zz[u], w, Dv); Av += w; }
+                T = bl ? Tn : T;
+                last = bl ? pos : last;
+            } else if (act) {
+                if (STATS) ++n_visit;
+                if (!(pw > 0.0f) && !(pw < thr[u])) {
+                    if (STATS) ++n_pass;
+                    const float alpha = fminf(amax, ex2_approx(fmaf(pw, LOG2E, l2o[u])));
+                    const float Tn = T * (1.0f - alpha);
+                    if (Tn < tmin) {
+                        act = false;
+                    } else {
+                        const float4 c = rq[2];
+                        const float w = alpha * T;
+                        C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+                        if (FEAT) { Dv = fmaf(zz[u], w, Dv); Av += w; }
+                        T = Tn;
+                        last = pos;
+                        if (STATS) ++n_blend;
+                    }
+                }
+            }
+        };
+        auto step = [&](int u, const float4* rq, uint32_t pos) {
+            if (PACKED) {
+                blend_packed(u, pos);
+            } else {
+                blend_scalar(act_a, pw_a[u], u, rq, Ta, Ca0, Ca1, Ca2, last_a, pos, Da, Aa);
+                if (PPT == 2) blend_scalar(act_b, pw_b[u], u, rq, Tb, Cb0, Cb1, Cb2, last_b, pos, Db, Ab);
+            }
+        };
         if (act_a || act_b) {
-            const float4* rq = s_rec;
+            const float4* rq = s_rec[stage];
             uint32_t j = 0;
             for (; j + 4 <= cnt && (act_a || act_b); j += 4, rq += 12) {
-                XPR_FWD_POWER(0, rq) XPR_FWD_POWER(1, rq + 3) XPR_FWD_POWER(2, rq + 6) XPR_FWD_POWER(3, rq + 9)
-                XPR_FWD_STEP(0, rq, base + j + 1)
-                XPR_FWD_STEP(1, rq + 3, base + j + 2)
-                XPR_FWD_STEP(2, rq + 6, base + j + 3)
-                XPR_FWD_STEP(3, rq + 9, base + j + 4)
+                power(0, rq); power(1, rq + 3); power(2, rq + 6); power(3, rq + 9);
+                step(0, rq, base + j + 1);
+                step(1, rq + 3, base + j + 2);
+                step(2, rq + 6, base + j + 3);
+                step(3, rq + 9, base + j + 4);
             }
             for (; j < cnt && (act_a || act_b); ++j, rq += 3) {
-                XPR_FWD_POWER(0, rq)
-                XPR_FWD_STEP(0, rq, base + j + 1)
+                power(0, rq);
+                step(0, rq, base + j + 1);
             }
         }
+        stage = (stage + 1 == STAGES) ? 0 : stage + 1;
     }
-#undef XPR_FWD_POWER
-#undef XPR_FWD_BLEND
-#undef XPR_FWD_STEP
+    cp_async_wait<0>();
+    if (PACKED) {
+        unpack2(T2, Ta, Tb);
+        unpack2(C0_2, Ca0, Cb0); unpack2(C1_2, Ca1, Cb1); unpack2(C2_2, Ca2, Cb2);
+        if (FEAT) { unpack2(D2, Da, Db); unpack2(A2, Aa, Ab); }
+    }
     if (STATS) {
         atomicAdd(stats + 0, (unsigned long long)n_visit); atomicAdd(stats + 1, (unsigned long long)n_pass);
         atomicAdd(stats + 2, (unsigned long long)n_blend); atomicAdd(stats + 3, (unsigned long long)(last_a + last_b));
@@ -202,102 +249,84 @@ rasterize_fwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     }
 }
 
-__device__ __forceinline__ float fast_rcp(float x) {   // rcp.approx (1 ulp); x = 1 - alpha in [0.01, 1]
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// Transposed butterfly: reduces 8 per-lane values across the warp with 9 shuffles (4+2+1+1+1)
-// instead of 40.  On return lane L with (L & 3) == 0 holds the warp total of value (L >> 2).
-__device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
-    float w[4], x[2];
-    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float send = b4 ? v[i] : v[i + 4], keep = b4 ? v[i + 4] : v[i];
-        w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-    }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const float send = b3 ? w[i] : w[i + 2], keep = b3 ? w[i + 2] : w[i];
-        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-    }
-    const float send = b2 ? x[0] : x[1], keep = b2 ? x[1] : x[0];
-    float y = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-    y += __shfl_xor_sync(0xffffffffu, y, 2);
-    y += __shfl_xor_sync(0xffffffffu, y, 1);
-    return y;
-}
-
-// Backward compositing (a9).  One CTA per 16x16 tile; a thread owns BWD_PPT consecutive pixels of one row
-// (4 -> 64 threads, the throughput shape; 2 -> 128 threads for images with few tiles), so that a Gaussian's
-// record is read from shared memory once per BWD_PPT pixel-pairs, the row terms of `power` are shared, and
-// the per-Gaussian reduction runs once per 32 * BWD_PPT pixel-pairs: each lane first sums its own pixels in
-// registers, then one transposed butterfly (14 shuffles for the 9 gradients) leaves the totals spread over
-// lanes, which issue two RED instructions (8 lanes + 1 lane).
+// Backward compositing (a9).  One CTA per 16x16 tile; a thread owns PPT consecutive pixels of one row
+// (4 -> 64 threads, the throughput shape; 2 -> 128 threads for images with few tiles), handled as PPT/2 packed
+// pairs, so that a Gaussian's record is read from shared memory once per PPT pixel-pairs, the row terms of
+// `power` are shared, and the per-Gaussian reduction runs once per 32 * PPT pixel-pairs: each lane first sums
+// its own pixels in registers, then one transposed butterfly (14 shuffles for the 9 gradients) leaves the totals
+// spread over lanes, which issue two RED instructions (8 lanes + 1 lane).
+//
+// Per pixel, branch-free (a gated pixel enters with o G = 0, hence alpha = 0, 1/(1-alpha) = 1, w = 0): restore
+// T_k = T_{k+1} / (1 - alpha_k); dL/dc_k = w g; dL/dalpha_k = T_k (g . c_k) - Q_k / (1 - alpha_k) with the ONE running
+// scalar Q_k = g . S_k (S_k = colour behind k, C13), kept negated (R = -Q) so that both uses are FMAs.
+// FEAT (xpr_rasterize_feat_bwd; reading C31): with gD = dL/dD, gA = dL/dA of the pixel,
+//   dL/dz_k = alpha_k T_k gD,  dL/dalpha_k = T_k (g . c_k + gD z_k + gA) - (g . S + gD SD + gA SA) / (1 - alpha_k);
+// SA telescopes (alpha_j T_j = T_j - T_{j+1}): gA (T_k - SA_k / (1 - alpha_k)) = gA T_final / (1 - alpha_k), so the
+// accumulated-opacity term is the per-pixel constant -gA T_final inside Q: Q_k = sum_{j>k} (g . c_j + gD z_j) alpha_j T_j
+// + T_final (g . bg - gA).
 #ifndef XPR_BWD_PPT_SMALL
 #define XPR_BWD_PPT_SMALL 2
 #endif
-
 #ifndef XPR_BWD_MINB
-#define XPR_BWD_MINB 14      // 64-thread CTAs per SM in the throughput shape (72 registers, no spills; 12: +2.5 % time)
+#define XPR_BWD_MINB 12      // 64-thread CTAs per SM in the throughput shape
 #endif
-template <int BWD_PPT>
-__global__ void __launch_bounds__(BLOCK / BWD_PPT, XPR_BWD_MINB * BWD_PPT / 4)
-rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
-                     const float* __restrict__ rgb, const float* __restrict__ lnv,
-                     const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
-                     const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
-                     const float* __restrict__ dL, float* __restrict__ g_mean2d, float* __restrict__ g_conic,
-                     float* __restrict__ g_opac, float* __restrict__ g_rgb) {
-    constexpr int BWD_THREADS = BLOCK / BWD_PPT, BWD_BATCH = BWD_THREADS;
-    __shared__ float4 s_geo[BWD_BATCH];   // mx, my, A, B
-    __shared__ float4 s_gate[BWD_BATCH];  // C, thr, o, index (bits)
-    __shared__ float4 s_col[BWD_BATCH];   // r, g, b, unused
-    __shared__ uint32_t s_max[BWD_THREADS / 32];
+template <int PPT, bool FEAT>
+__global__ void __launch_bounds__(BLOCK / PPT, XPR_BWD_MINB * PPT / 4)
+rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint32_t* __restrict__ vals,
+                     const uint2* __restrict__ ranges, const float* __restrict__ final_T,
+                     const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL,
+                     const float* __restrict__ dL_dD, const float* __restrict__ dL_dA, float* __restrict__ g_mean2d,
+                     float* __restrict__ g_conic, float* __restrict__ g_opac, float* __restrict__ g_rgb,
+                     float* __restrict__ g_depth) {
+    constexpr int THREADS = BLOCK / PPT, B = THREADS, NP = PPT / 2;
+    __shared__ float4 s_rec[STAGES][3 * B];
+    __shared__ uint32_t s_idx[STAGES][B];
+    __shared__ uint32_t s_max[THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31;
     const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % P.TW, ty = tile / P.TW;
-    const int lane = threadIdx.x & 31;
-    // a thread owns BWD_PPT consecutive pixels of one row: they share dy and the row terms of `power`
-    constexpr int TPR = TILE / BWD_PPT;                 // threads per tile row
-    const int px0 = tx * TILE + (threadIdx.x % TPR) * BWD_PPT;
-    const int py = ty * TILE + (threadIdx.x / TPR);
+    // a thread owns PPT consecutive pixels of one row: they share dy and the row terms of `power`
+    constexpr int TPR = TILE / PPT;                 // threads per tile row
+    const int px0 = tx * TILE + (tid % TPR) * PPT;
+    const int py = ty * TILE + (tid / TPR);
     const float pyc = (float)py + 0.5f;
     const uint2 rg = ranges[tile];
+    const uint32_t* const list = vals + rg.x;
 
-    uint32_t n[BWD_PPT];
-    float T[BWD_PPT], Q[BWD_PPT], g0[BWD_PPT], g1[BWD_PPT], g2[BWD_PPT], pxc[BWD_PPT];
+    uint32_t n[PPT];
+    f32x2 px2[NP], T2[NP], R2[NP], g0_2[NP], g1_2[NP], g2_2[NP], gD_2[NP];
     uint32_t wmax = 0;
 #pragma unroll
-    for (int k = 0; k < BWD_PPT; ++k) {
-        const int px = px0 + k;
-        pxc[k] = (float)px + 0.5f;
-        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = 0.0f;
-        if (px < P.W && py < P.H) {
-            const int64_t pid = (int64_t)py * P.W + px;
-            n[k] = n_contrib[pid];
-            T[k] = final_T[pid];
-            g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
+    for (int p = 0; p < NP; ++p) {
+        float t[2], q[2], a0[2], a1[2], a2[2], aD[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int k = 2 * p + h, px = px0 + k;
+            n[k] = 0; t[h] = 0.0f; a0[h] = a1[h] = a2[h] = aD[h] = 0.0f;
+            float gA = 0.0f;
+            if (px < P.W && py < P.H) {
+                const int64_t pid = (int64_t)py * P.W + px;
+                n[k] = n_contrib[pid];
+                t[h] = final_T[pid];
+                a0[h] = dL[3 * pid]; a1[h] = dL[3 * pid + 1]; a2[h] = dL[3 * pid + 2];
+                if (FEAT) { aD[h] = dL_dD[pid]; gA = dL_dA[pid]; }
+            }
+            // Q = g . S behind the last entry = T_final (g . bg) (C13) (FEAT: - gA T_final)
+            q[h] = t[h] * (fmaf(a2[h], P.bg[2], fmaf(a1[h], P.bg[1], a0[h] * P.bg[0])) - gA);
+            wmax = max(wmax, n[k]);
         }
-        // colour behind the current entry, S_k = sum_{j>k} c_j alpha_j T_j + T_final bg (C13), enters only through
-        // g . S_k: one running scalar Q_k = g . S_k = sum_{j>k} (g . c_j) alpha_j T_j + T_final (g . bg)
-        Q[k] = T[k] * fmaf(g2[k], P.bg[2], fmaf(g1[k], P.bg[1], g0[k] * P.bg[0]));
-        wmax = max(wmax, n[k]);
+        px2[p] = pack2((float)(px0 + 2 * p) + 0.5f, (float)(px0 + 2 * p + 1) + 0.5f);
+        T2[p] = pack2(t[0], t[1]); R2[p] = pack2(-q[0], -q[1]);
+        g0_2[p] = pack2(a0[0], a0[1]); g1_2[p] = pack2(a1[0], a1[1]); g2_2[p] = pack2(a2[0], a2[1]);
+        gD_2[p] = pack2(aD[0], aD[1]);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
-    if (lane == 0) s_max[threadIdx.x >> 5] = wmax;
+    if (lane == 0) s_max[tid >> 5] = wmax;
     __syncthreads();
     uint32_t max_n = 0;
 #pragma unroll
-    for (int w = 0; w < BWD_THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
+    for (int w = 0; w < THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
 
     // lane (4 i) owns gradient i of the 8-value butterfly: its base pointer and per-Gaussian stride
     const int vi = lane >> 2;
@@ -305,110 +334,162 @@ rasterize_bwd_kernel(RasterParams P, const float2* __restrict__ mean2d, const fl
     const uint32_t red_stride = (vi < 2) ? 2u : 3u;
     const bool red_lane = (lane & 3) == 0;
 
-    for (uint32_t hi = max_n; hi > 0;) {
-        const uint32_t cnt = min((uint32_t)BWD_BATCH, hi);
-        __syncthreads();
-        if (threadIdx.x < cnt) {      // slot j holds list position hi-1-j (descending)
-            const uint32_t g = vals[rg.x + hi - 1 - threadIdx.x];
-            const float2 m = mean2d[g];
-            const float4 co = conic_opac[g];
-            s_geo[threadIdx.x] = make_float4(m.x, m.y, co.x, co.y);
-            s_gate[threadIdx.x] = make_float4(co.z, -lnv[g], co.w, __uint_as_float(g));
-            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], __log2f(co.w));
+    // staging ring over the list positions max_n-1 ... 0 (descending): entry e = b B + j is position max_n-1-e
+    auto stage_entry = [&](uint32_t s, uint32_t g) {
+        s_idx[s][tid] = g;
+        stage_record(&s_rec[s][3 * tid], rec, g);
+    };
+    {
+        uint32_t g0 = 0, g1 = 0;
+        if ((uint32_t)tid < max_n) g0 = list[max_n - 1u - (uint32_t)tid];
+        if ((uint32_t)(B + tid) < max_n) g1 = list[max_n - 1u - (uint32_t)(B + tid)];
+        if ((uint32_t)tid < max_n) stage_entry(0, g0);
+        cp_async_commit();
+        if ((uint32_t)(B + tid) < max_n) stage_entry(1, g1);
+        cp_async_commit();
+    }
+    // index of this thread's entry of batch b + 2, loaded one batch ahead of the copy that needs it
+    uint32_t g_next = ((uint32_t)(2 * B + tid) < max_n) ? list[max_n - 1u - (uint32_t)(2 * B + tid)] : 0u;
+
+    const float amax = P.amax;
+    uint32_t stage = 0;
+    for (uint32_t base = 0; base < max_n; base += B) {
+        cp_async_wait<1>();
+        __syncthreads();               // batch b visible to all; everyone is done with batch b - 1
+        {
+            const uint32_t s2 = (stage + 2 >= STAGES) ? stage + 2 - STAGES : stage + 2;
+            if (base + 2 * B + tid < max_n) stage_entry(s2, g_next);
+            cp_async_commit();
+            g_next = (base + 3 * B + tid < max_n) ? list[max_n - 1u - (base + 3 * B + tid)] : 0u;
         }
-        __syncthreads();
-        for (uint32_t j = 0; j < cnt; ++j) {
-            const uint32_t pos = hi - 1 - j;
+        const uint32_t cnt = min((uint32_t)B, max_n - base);
+        const float4* rq = s_rec[stage];
+        for (uint32_t j = 0; j < cnt; ++j, rq += 3) {
+            const uint32_t pos = max_n - 1u - (base + j);
             if (pos >= wmax) continue;     // warp-uniform: nobody in this warp got this far
-            const float4 ge = s_geo[j];
-            const float4 ga = s_gate[j];
-            const float A = ge.z, Bc = ge.w, Cc = ga.x;
-            const float qa = -0.5f * A, qb = -Bc, qc = -0.5f * Cc;
+            const float4 ge = rq[0];       // mx my qa qb
+            const float4 ga = rq[1];       // qc thr log2o z
             const float dy = pyc - ge.y;
-            const float t1 = __fmul_rn(qb, dy), t2 = __fmul_rn(__fmul_rn(qc, dy), dy);   // row terms of eval_power
-            float dx[BWD_PPT], power[BWD_PPT];
-            bool contrib[BWD_PPT], any_c = false;
+            const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);   // row terms of `power`
+            f32x2 dx2[NP], pw2[NP];
+            bool contrib[PPT], any_c = false;
 #pragma unroll
-            for (int k = 0; k < BWD_PPT; ++k) {
-                dx[k] = pxc[k] - ge.x;
-                power[k] = __fmaf_rn(__fmaf_rn(qa, dx[k], t1), dx[k], t2);               // = eval_power(qa, qb, qc, dx, dy)
-                contrib[k] = (pos < n[k]) && !(power[k] > 0.0f) && !(power[k] < ga.y);
-                any_c |= contrib[k];
+            for (int p = 0; p < NP; ++p) {
+                dx2[p] = sub2(px2[p], bcast2(ge.x));
+                pw2[p] = fma2(fma2(bcast2(ge.z), dx2[p], bcast2(t1)), dx2[p], bcast2(t2));   // rule R3, per lane
+                float pa, pb;
+                unpack2(pw2[p], pa, pb);
+                contrib[2 * p] = (pos < n[2 * p]) && !(pa > 0.0f) && !(pa < ga.y);
+                contrib[2 * p + 1] = (pos < n[2 * p + 1]) && !(pb > 0.0f) && !(pb < ga.y);
+                any_c |= contrib[2 * p] || contrib[2 * p + 1];
             }
             if (!__any_sync(0xffffffffu, any_c)) continue;
-            const float4 c = s_col[j];
-            float v[8];                                // mx my A B C r g b
-            v[5] = v[6] = v[7] = 0.f;
+            const float4 c = rq[2];        // r g b o
             // the thread's pixels share dy: accumulate sum dpow, sum dpow dx, sum dpow dx^2 and form the five
-            // geometric gradients once per entry (dpow = dL/dpower of a pixel).  Branch-free over the pixels:
-            // one that does not contribute enters with o G = 0, hence alpha = 0, 1/(1-alpha) = 1, w = 0 -- its T
-            // and Q are unchanged and all its terms vanish.
-            float sp = 0.f, spx = 0.f, spxx = 0.f;
+            // geometric gradients once per entry (dpow = dL/dpower of a pixel)
+            f32x2 sp2, spx2, spxx2, vr2, vg2, vb2, sz2;
 #pragma unroll
-            for (int k = 0; k < BWD_PPT; ++k) {
-                const float og = contrib[k] ? opac_exp(power[k], c.w) : 0.0f;          // o G
-                const float alpha = fminf(P.amax, og);
-                const float inv = fast_rcp(1.0f - alpha);
-                T[k] = T[k] * inv;                     // transmittance in front of this entry
-                const float w = alpha * T[k];
-                v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
-                // dL/dalpha = sum_ch g_ch (c_ch T - S_ch / (1 - alpha)) = T (g . c) - (g . S) / (1 - alpha)
-                const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
-                const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
-                Q[k] = fmaf(gc, w, Q[k]);
-                const float live = (og < P.amax) ? dalpha : 0.0f;   // C14: the clamp has zero derivative
-                const float dpow = og * live;          // dL/dpower; dL/do = G live = dpow / o: summed as sp below
-                const float dxp = dx[k] * dpow;
-                sp += dpow; spx += dxp; spxx = fmaf(dx[k], dxp, spxx);
+            for (int p = 0; p < NP; ++p) {
+                float ea, eb;
+                unpack2(fma2(pw2[p], bcast2(LOG2E), bcast2(ga.z)), ea, eb);
+                const float og_a = contrib[2 * p] ? ex2_approx(ea) : 0.0f;          // o G
+                const float og_b = contrib[2 * p + 1] ? ex2_approx(eb) : 0.0f;
+                const f32x2 al2 = pack2(fminf(amax, og_a), fminf(amax, og_b));       // C11
+                float oma_a, oma_b;
+                unpack2(sub2(bcast2(1.0f), al2), oma_a, oma_b);
+                const f32x2 inv2 = pack2(rcp_approx(oma_a), rcp_approx(oma_b));
+                T2[p] = mul2(T2[p], inv2);                                           // transmittance in front of this entry
+                const f32x2 w2 = mul2(al2, T2[p]);
+                if (p == 0) { vr2 = mul2(w2, g0_2[p]); vg2 = mul2(w2, g1_2[p]); vb2 = mul2(w2, g2_2[p]); }
+                else { vr2 = fma2(w2, g0_2[p], vr2); vg2 = fma2(w2, g1_2[p], vg2); vb2 = fma2(w2, g2_2[p], vb2); }
+                // g . c (FEAT: + gD z)
+                f32x2 gc2 = fma2(g2_2[p], bcast2(c.z), fma2(g1_2[p], bcast2(c.y), mul2(g0_2[p], bcast2(c.x))));
+                if (FEAT) {
+                    gc2 = fma2(gD_2[p], bcast2(ga.w), gc2);
+                    sz2 = (p == 0) ? mul2(w2, gD_2[p]) : fma2(w2, gD_2[p], sz2);     // dL/dz
+                }
+                // dL/dalpha = T (g . c) - Q / (1 - alpha) = T gc + inv R;   R <- R - gc w
+                float da_a, da_b;
+                unpack2(fma2(inv2, R2[p], mul2(T2[p], gc2)), da_a, da_b);
+                R2[p] = fma2(neg2(gc2), w2, R2[p]);
+                // C14: the clamp has zero derivative; dL/dpower = o G dL/dalpha (dL/do = G dL/dalpha = dpow / o: summed as sp)
+                const f32x2 dpow2 = mul2(pack2(og_a, og_b), pack2((og_a < amax) ? da_a : 0.0f, (og_b < amax) ? da_b : 0.0f));
+                const f32x2 dxp2 = mul2(dx2[p], dpow2);
+                if (p == 0) { sp2 = dpow2; spx2 = dxp2; spxx2 = mul2(dx2[p], dxp2); }
+                else { sp2 = add2(sp2, dpow2); spx2 = add2(spx2, dxp2); spxx2 = fma2(dx2[p], dxp2, spxx2); }
             }
+            float v[8];                                // mx my A B C r g b
+            const float sp = sum2(sp2), spx = sum2(spx2), spxx = sum2(spxx2);
+            v[5] = sum2(vr2); v[6] = sum2(vg2); v[7] = sum2(vb2);
             {
+                // dpower/dm = (A dx + B dy, B dx + C dy) = -(2 qa dx + qb dy, qb dx + 2 qc dy); dpower/d(A, B, C) = (-dx^2/2, -dx dy, -dy^2/2)
                 const float sy = dy * sp;              // sum dpow dy
-                v[0] = fmaf(A, spx, Bc * sy); v[1] = fmaf(Bc, spx, Cc * sy);
+                v[0] = -fmaf(2.0f * ge.z, spx, ge.w * sy); v[1] = -fmaf(ge.w, spx, 2.0f * ga.x * sy);
                 v[2] = -0.5f * spxx; v[3] = -dy * spx; v[4] = -0.5f * dy * sy;
             }
             const float tot = warp_reduce8(v, lane);
-            const float sp_tot = warp_sum(sp);         // dL/do = (sum dpow) / o, divided by the one lane that adds it
-            const uint32_t g = __float_as_uint(ga.w);
-            if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
-            if (lane == 0) atomicAdd(g_opac + g, sp_tot * fast_rcp(ga.z));
+            const uint32_t g = s_idx[stage][j];
+            if (FEAT) {
+                // lanes 0-15 end with the warp total of sp, lanes 16-31 with that of sz
+                const float sz = sum2(sz2);
+                float r2 = ((lane & 16) ? sz : sp) + __shfl_xor_sync(0xffffffffu, (lane & 16) ? sp : sz, 16);
+#pragma unroll
+                for (int o = 8; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+                if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
+                if (lane == 0) atomicAdd(g_opac + g, r2 * rcp_approx(c.w));
+                if (lane == 16) atomicAdd(g_depth + g, r2);
+            } else {
+                const float sp_tot = warp_sum(sp);     // dL/do = (sum dpow) / o, divided by the one lane that adds it
+                if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
+                if (lane == 0) atomicAdd(g_opac + g, sp_tot * rcp_approx(c.w));
+            }
         }
-        hi -= cnt;
+        stage = (stage + 1 == STAGES) ? 0 : stage + 1;
     }
+    cp_async_wait<0>();
 }
 
-int32_t make_raster_params(const xpr_camera* cam, const xpr_config* cfg, RasterParams& P) {
+// xpr_shade_record: the 48-byte shader record from the separate projection outputs (for callers that did not
+// get it from xpr_project).  One thread per Gaussian; culled Gaussians are skipped (their record is never read).
+__global__ void __launch_bounds__(256)
+shade_record_kernel(int64_t N, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
+                    const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ depth,
+                    const uint32_t* __restrict__ tcount, float4* __restrict__ rec) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N || tcount[i] == 0u) return;
+    const float2 m = mean2d[i];
+    const float4 co = conic_opac[i];
+    rec[3 * i] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
+    rec[3 * i + 1] = make_float4(-0.5f * co.z, -lnv[i], __log2f(co.w), depth ? depth[i] : 0.0f);
+    rec[3 * i + 2] = make_float4(rgb[3 * i], rgb[3 * i + 1], rgb[3 * i + 2], co.w);
+}
+
+void make_raster_params(const xpr_camera* cam, const xpr_config* cfg, RasterParams& P) {
     P.W = cam->width; P.H = cam->height; P.TW = tiles_x(cam);
     P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
     for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
     P.order = cfg->tile_order;
-    return XPR_OK;
 }
 
-}  // namespace
-}  // namespace xpr
-
-using namespace xpr;
-
-extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                                     const float* conic_opac, const float* rgb, const float* lnv,
-                                     const uint32_t* vals_sorted, const uint32_t* tile_ranges, float* image,
-                                     float* final_T, uint32_t* n_contrib, void* stream) {
+template <bool FEAT>
+int32_t launch_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
+                   const uint32_t* vals_sorted, const uint32_t* tile_ranges, float* image, float* final_T,
+                   uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0) return XPR_ERR_INVALID_ARG;
     if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4))
         return XPR_ERR_INVALID_ARG;
-    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-                  !aligned(vals_sorted, 4)))
-        return XPR_ERR_INVALID_ARG;
+    if (FEAT && (!aligned(depth_img, 4) || !aligned(alpha_img, 4))) return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(shade_rec, 16) || !aligned(vals_sorted, 4))) return XPR_ERR_INVALID_ARG;
     RasterParams P;
     make_raster_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
     // throughput shape once the image has enough tiles for several waves of every SM; branch-free blend when
     // the lists were culled
 #define XPR_FWD(PPT_, BF_)                                                                                          \
-    rasterize_fwd_kernel<false, PPT_, BF_><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                             \
-        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,           \
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr)
+    rasterize_fwd_kernel<false, PPT_, BF_, FEAT><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                       \
+        P, reinterpret_cast<const float4*>(shade_rec), vals_sorted, reinterpret_cast<const uint2*>(tile_ranges),     \
+        image, final_T, n_contrib, nullptr, depth_img, alpha_img)
     const bool bf = cfg->tile_cull != 0;
     if (T >= FWD_PPT2_MIN_TILES) { if (bf) XPR_FWD(2, true); else XPR_FWD(2, false); }
     else                         { XPR_FWD(1, false); }      // latency shape: the branchy blend is shorter
@@ -417,81 +498,33 @@ extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cf
     return XPR_OK;
 }
 
-extern "C" int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                                          const float* conic_opac, const float* rgb, const float* lnv,
-                                          const float* depth, const uint32_t* vals_sorted,
-                                          const uint32_t* tile_ranges, float* image, float* final_T,
-                                          uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
-    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
-    if (N < 0) return XPR_ERR_INVALID_ARG;
-    if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4) ||
-        !aligned(depth_img, 4) || !aligned(alpha_img, 4))
-        return XPR_ERR_INVALID_ARG;
-    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-                  !aligned(depth, 4) || !aligned(vals_sorted, 4)))
-        return XPR_ERR_INVALID_ARG;
-    RasterParams P;
-    make_raster_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
-    // the launch shapes of xpr_rasterize_fwd
-#define XPR_FWD(PPT_, BF_)                                                                                          \
-    rasterize_fwd_kernel<false, PPT_, BF_, true><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                       \
-        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,           \
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr, depth,         \
-        depth_img, alpha_img)
-    const bool bf = cfg->tile_cull != 0;
-    if (T >= FWD_PPT2_MIN_TILES) { if (bf) XPR_FWD(2, true); else XPR_FWD(2, false); }
-    else                         { XPR_FWD(1, false); }
-#undef XPR_FWD
-    XPR_LAUNCH_CHECK();
-    return XPR_OK;
-}
-
-extern "C" int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                                       const float* conic_opac, const float* rgb, const float* lnv,
-                                       const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats,
-                                       void* stream) {
-    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
-    if (N < 0 || !aligned(tile_ranges, 8) || !aligned(stats, 8)) return XPR_ERR_INVALID_ARG;
-    if (N > 0 && (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-                  !aligned(vals_sorted, 4)))
-        return XPR_ERR_INVALID_ARG;
-    RasterParams P;
-    make_raster_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
-    XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
-    rasterize_fwd_kernel<true, 1, false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
-        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr, nullptr, nullptr,
-        reinterpret_cast<unsigned long long*>(stats));
-    XPR_LAUNCH_CHECK();
-    return XPR_OK;
-}
-
-extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                                     const float* conic_opac, const float* rgb, const float* lnv,
-                                     const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* final_T,
-                                     const uint32_t* n_contrib, const float* dL_dimage, float* g_mean2d,
-                                     float* g_conic, float* g_opac, float* g_rgb, int32_t zero_init, void* stream) {
+template <bool FEAT>
+int32_t launch_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
+                   const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* final_T,
+                   const uint32_t* n_contrib, const float* dL_dimage, const float* dL_ddepth, const float* dL_dalpha,
+                   float* g_mean2d, float* g_conic, float* g_opac, float* g_rgb, float* g_depth, int32_t zero_init,
+                   void* stream) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0) return XPR_ERR_INVALID_ARG;
     if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4))
         return XPR_ERR_INVALID_ARG;
+    if (FEAT && (!aligned(dL_ddepth, 4) || !aligned(dL_dalpha, 4))) return XPR_ERR_INVALID_ARG;
     if (N == 0) return XPR_OK;
-    if (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-        !aligned(vals_sorted, 4) || !aligned(g_mean2d, 4) || !aligned(g_conic, 4) || !aligned(g_opac, 4) ||
-        !aligned(g_rgb, 4))
+    if (!aligned(shade_rec, 16) || !aligned(vals_sorted, 4) || !aligned(g_mean2d, 4) || !aligned(g_conic, 4) ||
+        !aligned(g_opac, 4) || !aligned(g_rgb, 4) || (FEAT && !aligned(g_depth, 4)))
         return XPR_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     if (zero_init) {
         const size_t n = (size_t)N;
-        if (g_conic == g_mean2d + 2 * n && g_opac == g_conic + 3 * n && g_rgb == g_opac + n) {
-            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 9 * n, st));      // one allocation: one fill
+        const bool adjacent = g_conic == g_mean2d + 2 * n && g_opac == g_conic + 3 * n && g_rgb == g_opac + n;
+        if (adjacent && (!FEAT || g_depth == g_rgb + 3 * n)) {
+            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * (FEAT ? 10 : 9) * n, st));   // one allocation: one fill
         } else {
             XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 2 * n, st));
             XPR_CUDA(cudaMemsetAsync(g_conic, 0, sizeof(float) * 3 * n, st));
             XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
             XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
+            if (FEAT) XPR_CUDA(cudaMemsetAsync(g_depth, 0, sizeof(float) * n, st));
         }
     }
     RasterParams P;
@@ -499,16 +532,83 @@ extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cf
     const int T = tiles_x(cam) * tiles_y(cam);
     // 4 pixels per thread (64 threads) is the throughput shape; images with few tiles are bounded by their
     // heaviest tile, where more warps per tile (2 pixels per thread) shorten the critical path
-    if (T >= FWD_PPT2_MIN_TILES)
-        rasterize_bwd_kernel<4><<<T, BLOCK / 4, 0, st>>>(
-            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_mean2d, g_conic,
-            g_opac, g_rgb);
-    else
-        rasterize_bwd_kernel<XPR_BWD_PPT_SMALL><<<T, BLOCK / XPR_BWD_PPT_SMALL, 0, st>>>(
-            P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-            vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_mean2d, g_conic,
-            g_opac, g_rgb);
+#define XPR_BWD(PPT_)                                                                                               \
+    rasterize_bwd_kernel<PPT_, FEAT><<<T, BLOCK / PPT_, 0, st>>>(                                                     \
+        P, reinterpret_cast<const float4*>(shade_rec), vals_sorted, reinterpret_cast<const uint2*>(tile_ranges),     \
+        final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth)
+    if (T >= FWD_PPT2_MIN_TILES) XPR_BWD(4);
+    else                         XPR_BWD(XPR_BWD_PPT_SMALL);
+#undef XPR_BWD
     XPR_LAUNCH_CHECK();
     return XPR_OK;
+}
+
+}  // namespace
+}  // namespace xpr
+
+using namespace xpr;
+
+extern "C" int32_t xpr_shade_record(int64_t N, const float* mean2d, const float* conic_opac, const float* rgb,
+                                    const float* lnv, const float* depth, const uint32_t* tile_count,
+                                    float* shade_rec, void* stream) {
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+        (depth && !aligned(depth, 4)) || !aligned(tile_count, 4) || !aligned(shade_rec, 16))
+        return XPR_ERR_INVALID_ARG;
+    shade_record_kernel<<<(unsigned)((N + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        N, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, depth,
+        tile_count, reinterpret_cast<float4*>(shade_rec));
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
+                                     const uint32_t* vals_sorted, const uint32_t* tile_ranges, float* image,
+                                     float* final_T, uint32_t* n_contrib, void* stream) {
+    return launch_fwd<false>(cam, cfg, N, shade_rec, vals_sorted, tile_ranges, image, final_T, n_contrib, nullptr,
+                             nullptr, stream);
+}
+
+extern "C" int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N,
+                                          const float* shade_rec, const uint32_t* vals_sorted,
+                                          const uint32_t* tile_ranges, float* image, float* final_T,
+                                          uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
+    return launch_fwd<true>(cam, cfg, N, shade_rec, vals_sorted, tile_ranges, image, final_T, n_contrib, depth_img,
+                            alpha_img, stream);
+}
+
+extern "C" int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
+                                       const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats,
+                                       void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0 || !aligned(tile_ranges, 8) || !aligned(stats, 8)) return XPR_ERR_INVALID_ARG;
+    if (N > 0 && (!aligned(shade_rec, 16) || !aligned(vals_sorted, 4))) return XPR_ERR_INVALID_ARG;
+    RasterParams P;
+    make_raster_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+    XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
+    rasterize_fwd_kernel<true, 1, false, false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
+        P, reinterpret_cast<const float4*>(shade_rec), vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr,
+        nullptr, nullptr, reinterpret_cast<unsigned long long*>(stats), nullptr, nullptr);
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
+                                     const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* final_T,
+                                     const uint32_t* n_contrib, const float* dL_dimage, float* g_mean2d,
+                                     float* g_conic, float* g_opac, float* g_rgb, int32_t zero_init, void* stream) {
+    return launch_bwd<false>(cam, cfg, N, shade_rec, vals_sorted, tile_ranges, final_T, n_contrib, dL_dimage, nullptr,
+                             nullptr, g_mean2d, g_conic, g_opac, g_rgb, nullptr, zero_init, stream);
+}
+
+extern "C" int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N,
+                                          const float* shade_rec, const uint32_t* vals_sorted,
+                                          const uint32_t* tile_ranges, const float* final_T,
+                                          const uint32_t* n_contrib, const float* dL_dimage, const float* dL_ddepth,
+                                          const float* dL_dalpha, float* g_mean2d, float* g_conic, float* g_opac,
+                                          float* g_rgb, float* g_depth, int32_t zero_init, void* stream) {
+    return launch_bwd<true>(cam, cfg, N, shade_rec, vals_sorted, tile_ranges, final_T, n_contrib, dL_dimage, dL_ddepth,
+                            dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth, zero_init, stream);
 }

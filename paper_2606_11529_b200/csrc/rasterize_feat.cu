@@ -1,5 +1,5 @@
-// rasterize_feat.cu -- xpr_rasterize_feat_bwd / xpr_depth_bwd (the forward, xpr_rasterize_feat_fwd, is the FEAT
-// instantiation of rasterize_fwd_kernel in rasterize.cu): compositing with the
+// rasterize_feat.cu -- xpr_rasterize_featn_fwd / _bwd and xpr_depth_bwd (xpr_rasterize_feat_fwd / _bwd are the FEAT
+// instantiations of rasterize_fwd_kernel / rasterize_bwd_kernel in rasterize.cu): compositing with the
 // rendered features of SURVEY 8(f) f3 ("rendered features such as depth", Table 2; DESIGN.md
 // reading C31): next to the colour, the same walk blends the depth image D = sum_k z_k alpha_k T_k and the
 // accumulated opacity A = sum_k alpha_k T_k (no background term), and the reverse pass takes dL/dD and dL/dA.
@@ -56,154 +56,6 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
     y += __shfl_xor_sync(0xffffffffu, y, 2);
     y += __shfl_xor_sync(0xffffffffu, y, 1);
     return y;
-}
-
-// Backward: rasterize_bwd_kernel plus the two features.  With gD = dL/dD, gA = dL/dA of the pixel and
-// SD = sum_{j>k} z_j alpha_j T_j, SA = sum_{j>k} alpha_j T_j behind the entry (no background term, C31):
-//   dL/dz_k     = alpha_k T_k gD
-//   dL/dalpha_k = T_k (g . c_k + gD z_k + gA) - (g . S + gD SD + gA SA) / (1 - alpha_k)
-// and from dL/dalpha on as the colour pass.  SA telescopes (alpha_j T_j = T_j - T_{j+1}):
-//   SA_k = T_k (1 - alpha_k) - T_final   =>   gA (T_k - SA_k / (1 - alpha_k)) = gA T_final / (1 - alpha_k),
-// so the accumulated-opacity term is the per-pixel constant gA T_final entering the "behind" dot product with a
-// minus sign: no running sum, no cancellation.  Everything behind the entry enters through ONE running scalar
-//   Q_k = g . S_k + gD SD_k - gA T_final = sum_{j>k} (g . c_j + gD z_j) alpha_j T_j + T_final (g . bg - gA),
-// so the depth term costs one FMA in the dot product g . c + gD z and one for dL/dz.  sum dpow (dL/do) and dL/dz
-// share one butterfly (6 shuffles for the two).
-#ifndef XPR_FEAT_BWD_PPT
-#define XPR_FEAT_BWD_PPT 4          // pixels per thread in the throughput shape
-#endif
-#ifndef XPR_FEAT_BWD_MINB
-#define XPR_FEAT_BWD_MINB 12        // 64-thread CTAs per SM at 4 pixels per thread (80 registers)
-#endif
-template <int PPT>
-__global__ void __launch_bounds__(BLOCK / PPT, XPR_FEAT_BWD_MINB * PPT / 4)
-rasterize_feat_bwd_kernel(FeatParams P, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
-                          const float* __restrict__ rgb, const float* __restrict__ lnv,
-                          const float* __restrict__ depth, const uint32_t* __restrict__ vals,
-                          const uint2* __restrict__ ranges, const float* __restrict__ final_T,
-                          const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL,
-                          const float* __restrict__ dL_dD, const float* __restrict__ dL_dA,
-                          float* __restrict__ g_mean2d, float* __restrict__ g_conic, float* __restrict__ g_opac,
-                          float* __restrict__ g_rgb, float* __restrict__ g_depth) {
-    constexpr int THREADS = BLOCK / PPT, BATCH = THREADS;
-    __shared__ float4 s_geo[BATCH];    // mx, my, A, B
-    __shared__ float4 s_gate[BATCH];   // C, thr, o, index (bits)
-    __shared__ float4 s_col[BATCH];    // r, g, b, log2 o
-    __shared__ float s_z[BATCH];       // z
-    __shared__ uint32_t s_max[THREADS / 32];
-    const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
-    const int tx = tile % P.TW, ty = tile / P.TW;
-    const int lane = threadIdx.x & 31;
-    constexpr int TPR = TILE / PPT;
-    const int px0 = tx * TILE + (threadIdx.x % TPR) * PPT;
-    const int py = ty * TILE + (threadIdx.x / TPR);
-    const float pyc = (float)py + 0.5f;
-    const uint2 rg = ranges[tile];
-
-    uint32_t n[PPT];
-    float T[PPT], Q[PPT], g0[PPT], g1[PPT], g2[PPT], gD[PPT], pxc[PPT];
-    uint32_t wmax = 0;
-#pragma unroll
-    for (int k = 0; k < PPT; ++k) {
-        const int px = px0 + k;
-        pxc[k] = (float)px + 0.5f;
-        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = gD[k] = 0.0f;
-        float gA = 0.0f;
-        if (px < P.W && py < P.H) {
-            const int64_t pid = (int64_t)py * P.W + px;
-            n[k] = n_contrib[pid];
-            T[k] = final_T[pid];
-            g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
-            gD[k] = dL_dD[pid]; gA = dL_dA[pid];
-        }
-        // Q_k = g . S_k + gD SD_k - gA T_final: one running scalar for everything "behind" the entry
-        Q[k] = T[k] * (fmaf(g2[k], P.bg[2], fmaf(g1[k], P.bg[1], g0[k] * P.bg[0])) - gA);
-        wmax = max(wmax, n[k]);
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
-    if (lane == 0) s_max[threadIdx.x >> 5] = wmax;
-    __syncthreads();
-    uint32_t max_n = 0;
-#pragma unroll
-    for (int w = 0; w < THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
-
-    const int vi = lane >> 2;
-    float* const red_base = (vi < 2) ? (g_mean2d + vi) : (vi < 5) ? (g_conic + (vi - 2)) : (g_rgb + (vi - 5));
-    const uint32_t red_stride = (vi < 2) ? 2u : 3u;
-    const bool red_lane = (lane & 3) == 0;
-
-    for (uint32_t hi = max_n; hi > 0;) {
-        const uint32_t cnt = min((uint32_t)BATCH, hi);
-        __syncthreads();
-        if (threadIdx.x < cnt) {      // slot j holds list position hi-1-j (descending)
-            const uint32_t g = vals[rg.x + hi - 1 - threadIdx.x];
-            const float2 m = mean2d[g];
-            const float4 co = conic_opac[g];
-            s_geo[threadIdx.x] = make_float4(m.x, m.y, co.x, co.y);
-            s_gate[threadIdx.x] = make_float4(co.z, -lnv[g], co.w, __uint_as_float(g));
-            s_col[threadIdx.x] = make_float4(rgb[3 * g], rgb[3 * g + 1], rgb[3 * g + 2], __log2f(co.w));
-            s_z[threadIdx.x] = depth[g];
-        }
-        __syncthreads();
-        for (uint32_t j = 0; j < cnt; ++j) {
-            const uint32_t pos = hi - 1 - j;
-            if (pos >= wmax) continue;     // warp-uniform
-            const float4 ge = s_geo[j];
-            const float4 ga = s_gate[j];
-            const float Ac = ge.z, Bc = ge.w, Cc = ga.x;
-            const float qa = -0.5f * Ac, qb = -Bc, qc = -0.5f * Cc;
-            const float dy = pyc - ge.y;
-            const float t1 = __fmul_rn(qb, dy), t2 = __fmul_rn(__fmul_rn(qc, dy), dy);
-            float dx[PPT], power[PPT];
-            bool contrib[PPT], any_c = false;
-#pragma unroll
-            for (int k = 0; k < PPT; ++k) {
-                dx[k] = pxc[k] - ge.x;
-                power[k] = __fmaf_rn(__fmaf_rn(qa, dx[k], t1), dx[k], t2);
-                contrib[k] = (pos < n[k]) && !(power[k] > 0.0f) && !(power[k] < ga.y);
-                any_c |= contrib[k];
-            }
-            if (!__any_sync(0xffffffffu, any_c)) continue;
-            const float4 c = s_col[j];
-            const float z = s_z[j];
-            float v[8];                                // mx my A B C r g b
-            v[5] = v[6] = v[7] = 0.f;
-            float sp = 0.f, spx = 0.f, spxx = 0.f, sz = 0.f;
-#pragma unroll
-            for (int k = 0; k < PPT; ++k) {            // branch-free: a pixel that does not contribute has alpha = 0
-                const float og = contrib[k] ? opac_exp(power[k], c.w) : 0.0f;
-                const float alpha = fminf(P.amax, og);
-                const float inv = fast_rcp(1.0f - alpha);
-                T[k] = T[k] * inv;
-                const float w = alpha * T[k];
-                v[5] = fmaf(w, g0[k], v[5]); v[6] = fmaf(w, g1[k], v[6]); v[7] = fmaf(w, g2[k], v[7]);
-                sz = fmaf(w, gD[k], sz);               // dL/dz
-                const float gc = fmaf(gD[k], z, fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x)));
-                const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
-                Q[k] = fmaf(gc, w, Q[k]);
-                const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
-                const float dpow = og * live;
-                const float dxp = dx[k] * dpow;
-                sp += dpow; spx += dxp; spxx = fmaf(dx[k], dxp, spxx);
-            }
-            {
-                const float sy = dy * sp;
-                v[0] = fmaf(Ac, spx, Bc * sy); v[1] = fmaf(Bc, spx, Cc * sy);
-                v[2] = -0.5f * spxx; v[3] = -dy * spx; v[4] = -0.5f * dy * sy;
-            }
-            const float tot = warp_reduce8(v, lane);
-            // lanes 0-15 end with the warp total of sp, lanes 16-31 with that of sz
-            float r2 = ((lane & 16) ? sz : sp) + __shfl_xor_sync(0xffffffffu, (lane & 16) ? sp : sz, 16);
-#pragma unroll
-            for (int o = 8; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
-            const uint32_t g = __float_as_uint(ga.w);
-            if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
-            if (lane == 0) atomicAdd(g_opac + g, r2 * fast_rcp(ga.z));
-            if (lane == 16) atomicAdd(g_depth + g, r2);
-        }
-        hi -= cnt;
-    }
 }
 
 // ---- N-channel features (xpr_rasterize_featn_fwd / _bwd, reading C31) --------------------------------
@@ -483,50 +335,6 @@ void make_feat_params(const xpr_camera* cam, const xpr_config* cfg, FeatParams& 
 }  // namespace xpr
 
 using namespace xpr;
-
-extern "C" int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
-                                          const float* conic_opac, const float* rgb, const float* lnv,
-                                          const float* depth, const uint32_t* vals_sorted,
-                                          const uint32_t* tile_ranges, const float* final_T,
-                                          const uint32_t* n_contrib, const float* dL_dimage, const float* dL_ddepth,
-                                          const float* dL_dalpha, float* g_mean2d, float* g_conic, float* g_opac,
-                                          float* g_rgb, float* g_depth, int32_t zero_init, void* stream) {
-    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
-    if (N < 0) return XPR_ERR_INVALID_ARG;
-    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4) ||
-        !aligned(dL_ddepth, 4) || !aligned(dL_dalpha, 4))
-        return XPR_ERR_INVALID_ARG;
-    if (N == 0) return XPR_OK;
-    if (!aligned(mean2d, 8) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) || !aligned(depth, 4) ||
-        !aligned(vals_sorted, 4) || !aligned(g_mean2d, 4) || !aligned(g_conic, 4) || !aligned(g_opac, 4) ||
-        !aligned(g_rgb, 4) || !aligned(g_depth, 4))
-        return XPR_ERR_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)stream;
-    if (zero_init) {
-        const size_t n = (size_t)N;
-        if (g_conic == g_mean2d + 2 * n && g_opac == g_conic + 3 * n && g_rgb == g_opac + n && g_depth == g_rgb + 3 * n) {
-            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 10 * n, st));     // one allocation: one fill
-        } else {
-            XPR_CUDA(cudaMemsetAsync(g_mean2d, 0, sizeof(float) * 2 * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_conic, 0, sizeof(float) * 3 * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_depth, 0, sizeof(float) * n, st));
-        }
-    }
-    FeatParams P;
-    make_feat_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
-#define XPR_FEAT_BWD(PPT_)                                                                                          \
-    rasterize_feat_bwd_kernel<PPT_><<<T, BLOCK / PPT_, 0, st>>>(                                                      \
-        P, reinterpret_cast<const float2*>(mean2d), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, depth,    \
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, dL_ddepth,          \
-        dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth)
-    if (T >= XPR_FEAT_PPT_MIN_TILES) XPR_FEAT_BWD(XPR_FEAT_BWD_PPT); else XPR_FEAT_BWD(2);
-#undef XPR_FEAT_BWD
-    XPR_LAUNCH_CHECK();
-    return XPR_OK;
-}
 
 extern "C" int32_t xpr_rasterize_featn_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* mean2d,
                                            const float* conic_opac, const float* lnv, const float* feat, int32_t C,

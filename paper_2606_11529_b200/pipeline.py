@@ -42,6 +42,7 @@ class SplatPipeline:
         self.depth, self.lnv = e(N), e(N)
         self.tile_rect, self.tile_count = e(N, 4, dtype=i32), e(N, dtype=i32)
         self.flags = e(N, dtype=torch.uint8)
+        self.shade_rec = e(N, 12)                            # shader data p_sd, 48 bytes per Gaussian (xpr.h)
         # binning / sort outputs (a4-a7)
         self.tile_ranges = e(self.T, 2, dtype=i32)
         # scheduling order of the tiles for the compositing kernels (xpr_config.tile_order; no effect on results)
@@ -89,7 +90,7 @@ class SplatPipeline:
     def project(self, means, scales, quats, opacities, sh):
         self._inputs = (means, scales, quats, opacities, sh)
         xb.xpr_project(means, scales, quats, opacities, sh, self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb,
-                       self.depth, self.lnv, self.tile_rect, self.tile_count, self.flags)
+                       self.depth, self.lnv, self.tile_rect, self.tile_count, self.flags, self.shade_rec)
 
     def pixel_info(self):
         xb.xpr_pixel_info(self.cam, self.pixel_rays)
@@ -150,19 +151,18 @@ class SplatPipeline:
                                      self.n_contrib)
             return
         if self.features:
-            xb.xpr_rasterize_feat_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.depth,
-                                      self.vals_sorted, self.tile_ranges, self.image, self.final_T, self.n_contrib,
-                                      self.depth_img, self.alpha_img)
+            xb.xpr_rasterize_feat_fwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.image,
+                                      self.final_T, self.n_contrib, self.depth_img, self.alpha_img)
             return
-        xb.xpr_rasterize_fwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
-                             self.tile_ranges, self.image, self.final_T, self.n_contrib)
+        xb.xpr_rasterize_fwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.image,
+                             self.final_T, self.n_contrib)
 
     def rasterize_bwd(self, dL_dimage, dL_ddepth=None, dL_dalpha=None):
         self._feat_bwd = False
         if self.features and (dL_ddepth is not None or dL_dalpha is not None):
             z = lambda t: torch.zeros(self.H, self.W, dtype=torch.float32, device=self.device) if t is None else t
-            xb.xpr_rasterize_feat_bwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.depth,
-                                      self.vals_sorted, self.tile_ranges, self.final_T, self.n_contrib, dL_dimage,
+            xb.xpr_rasterize_feat_bwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges,
+                                      self.final_T, self.n_contrib, dL_dimage,
                                       z(dL_ddepth), z(dL_dalpha), self.g_mean2d, self.g_conic, self.g_opac,
                                       self.g_rgb, self.g_depth, zero_init=True)
             self._feat_bwd = True
@@ -172,9 +172,9 @@ class SplatPipeline:
                                      self.pixel_rays, self.vals_sorted, self.tile_ranges, self.final_T, self.n_contrib,
                                      dL_dimage, self.g_ray_rec, self.g_opac, self.g_rgb, zero_init=True)
             return
-        xb.xpr_rasterize_bwd(self.cam, self.cfg, self.mean2d, self.conic_opac, self.rgb, self.lnv, self.vals_sorted,
-                             self.tile_ranges, self.final_T, self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic,
-                             self.g_opac, self.g_rgb, zero_init=True)
+        xb.xpr_rasterize_bwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.final_T,
+                             self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb,
+                             zero_init=True)
 
     # ---- N-channel features (f3): replay of the finished colour pass ---------------------------
     def rasterize_featn_fwd(self, feat, feat_img=None):

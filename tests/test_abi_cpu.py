@@ -59,20 +59,19 @@ def test_invalid_arguments_rejected_before_launch(lib):
     null = C.c_void_p(0)
     # NULL pointers with N > 0
     st = lib.xpr_project(C.c_int64(4), null, null, null, null, null, C.byref(cam), C.byref(cfg), null, null, null,
-                         null, null, null, null, null, null)
+                         null, null, null, null, null, null, null)
     assert st == xb.XPR_ERR_INVALID_ARG
     # negative N
     st = lib.xpr_project(C.c_int64(-1), null, null, null, null, null, C.byref(cam), C.byref(cfg), null, null, null,
-                         null, null, null, null, null, null)
+                         null, null, null, null, null, null, null)
     assert st == xb.XPR_ERR_INVALID_ARG
     # tile != 16 and sh_degree > 3 are unsupported
     cam2, cfg2 = _cam_cfg(tile=8)
     st = lib.xpr_project(C.c_int64(0), null, null, null, null, null, C.byref(cam2), C.byref(cfg2), null, null, null,
-                         null, null, null, null, null, null)
+                         null, null, null, null, null, null, null)
     assert st == xb.XPR_ERR_UNSUPPORTED
     cam3, cfg3 = _cam_cfg(sh_degree=4)
-    st = lib.xpr_rasterize_fwd(C.byref(cam3), C.byref(cfg3), C.c_int64(0), null, null, null, null, null, null, null,
-                               null, null, null)
+    st = lib.xpr_rasterize_fwd(C.byref(cam3), C.byref(cfg3), C.c_int64(0), null, null, null, null, null, null, null)
     assert st == xb.XPR_ERR_UNSUPPORTED
     # bad enum
     cam4, cfg4 = _cam_cfg(projection=7)
@@ -116,20 +115,26 @@ def test_feature_entry_points_reject_bad_arguments(lib):
     odd = C.c_void_p(18)          # not 4-byte aligned
     N4, N0, Nm = C.c_int64(4), C.c_int64(0), C.c_int64(-1)
     fwd = lambda n, *a: lib.xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg), n, *a, null)
-    # mean2d conic_opac rgb lnv depth vals ranges image final_T n_contrib depth_img alpha_img
-    assert fwd(Nm, *[one] * 12) == 1
-    assert fwd(N4, one, one, one, one, null, one, one, one, one, one, one, one) == 1        # depth NULL
-    assert fwd(N4, *[one] * 10, null, one) == 1                                              # depth_img NULL
-    assert fwd(N4, *[one] * 11, odd) == 1                                                    # alpha_img misaligned
-    assert lib.xpr_rasterize_feat_fwd(None, C.byref(cfg), N4, *[one] * 12, null) == 1
+    # shade_rec vals ranges image final_T n_contrib depth_img alpha_img
+    assert fwd(Nm, *[one] * 8) == 1
+    assert fwd(N4, null, *[one] * 7) == 1                                                    # shade_rec NULL
+    assert fwd(N4, C.c_void_p(24), *[one] * 7) == 1                                          # shade_rec needs 16 B
+    assert fwd(N4, *[one] * 6, null, one) == 1                                               # depth_img NULL
+    assert fwd(N4, *[one] * 7, odd) == 1                                                     # alpha_img misaligned
+    assert lib.xpr_rasterize_feat_fwd(None, C.byref(cfg), N4, *[one] * 8, null) == 1
     cfg8 = type(cfg)(); C.memmove(C.byref(cfg8), C.byref(cfg), C.sizeof(cfg)); cfg8.tile = 8
-    assert lib.xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg8), N4, *[one] * 12, null) == 4
+    assert lib.xpr_rasterize_feat_fwd(C.byref(cam), C.byref(cfg8), N4, *[one] * 8, null) == 4
+    # xpr_shade_record: mean2d conic_opac rgb lnv depth tile_count shade_rec
+    assert lib.xpr_shade_record(Nm, *[one] * 7, null) == 1
+    assert lib.xpr_shade_record(N4, *[one] * 6, null, null) == 1                             # shade_rec NULL
+    assert lib.xpr_shade_record(N4, one, C.c_void_p(24), *[one] * 5, null) == 1              # conic_opac needs 16 B
+    assert lib.xpr_shade_record(N0, *[null] * 7, null) == 0
     bwd = lambda n, *a: lib.xpr_rasterize_feat_bwd(C.byref(cam), C.byref(cfg), n, *a, C.c_int32(1), null)
-    # mean2d conic_opac rgb lnv depth vals ranges final_T n_contrib dL dL_dD dL_dA g_mean2d g_conic g_opac g_rgb g_depth
-    assert bwd(Nm, *[one] * 17) == 1
-    assert bwd(N4, *[one] * 10, null, *[one] * 6) == 1                                       # dL_ddepth NULL
-    assert bwd(N4, *[one] * 16, null) == 1                                                   # g_depth NULL
-    assert bwd(N0, *[null] * 6, one, one, one, one, one, one, *[null] * 5) == 0              # N = 0: nothing to do
+    # shade_rec vals ranges final_T n_contrib dL dL_dD dL_dA g_mean2d g_conic g_opac g_rgb g_depth
+    assert bwd(Nm, *[one] * 13) == 1
+    assert bwd(N4, *[one] * 6, null, *[one] * 6) == 1                                        # dL_ddepth NULL
+    assert bwd(N4, *[one] * 12, null) == 1                                                   # g_depth NULL
+    assert bwd(N0, *[null] * 2, one, one, one, one, one, one, *[null] * 5) == 0              # N = 0: nothing to do
     assert lib.xpr_depth_bwd(Nm, C.byref(cam), one, one, one, null) == 1
     assert lib.xpr_depth_bwd(N4, None, one, one, one, null) == 1
     assert lib.xpr_depth_bwd(N4, C.byref(cam), one, null, one, null) == 1
