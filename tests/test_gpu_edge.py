@@ -167,7 +167,13 @@ def test_async_bin_sort_matches_sync_and_overflow_renders_background():
     xb.xpr_bin_sort(small.depth, small.tile_rect, small.tile_count, small.cam, small.cfg, 4096, guard,
                     small.vals_sorted, small.tile_ranges, small.workspace, sync=False)
     torch.cuda.synchronize()
-    assert small.pairs_on_device() == (I, 0)      # candidates, nothing in the output
+    need, written = small.pairs_on_device()       # the capacity that suffices (xpr.h: max(I, rows + 1, 2 x supertile
+    assert written == 0 and need >= I and need > 4096      # words)), nothing in the output
+    exact = pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg, pair_capacity=need)
+    exact.project(*params)
+    st, n = xb.xpr_bin_sort(exact.depth, exact.tile_rect, exact.tile_count, exact.cam, exact.cfg, need, exact.keys_sorted,
+                            exact.vals_sorted, exact.tile_ranges, exact.workspace, raise_on_capacity=False)
+    assert st == xb.XPR_OK and n == I and torch.equal(exact.keys_sorted[:I], keys)     # ... and it does suffice
     assert (guard[4096:] == -7).all()
     assert not small.tile_ranges.any()
     with pytest.raises(xb.XprError):
