@@ -267,12 +267,11 @@ def run_ours(args):
     n_pairs = pipe.num_pairs
     n_cand = pipe.candidates_on_device()
     # our kernels per step: project, emit, passes x onesweep, ranges, rasterize_fwd, rasterize_bwd, project_bwd
-    bits = max(1, (pipe.T - 1).bit_length()) if pipe.T > 1 else 0
-    tile_passes = max(1, (bits + 7) // 8)
-    passes = 4 + tile_passes              # 8-bit digits: 4 on the depth bits (run on Gaussians) + tile digits (on pairs)
-    # project, bin_sort (compact, 4 depth passes, row scan, rows, pair scan, emit, tile passes, ranges), fwd, bwd,
-    # project_bwd
-    launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1 + 1      # + loss_grad
+    ST = ((pipe.TW + 7) // 8) * ((pipe.TH + 7) // 8)
+    tile_passes = max(1, ((max(ST, 1) - 1).bit_length() + 7) // 8)      # 8-bit digits of the supertile id
+    # project, bin_sort (compact, 4 depth passes, rank scan, rows, supertile words, tile scan, supertile passes, final),
+    # fwd, loss_grad, bwd, project_bwd
+    launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1 + 1
     if args.ray_eval:
         launches_per_step += 3              # pixel_info, project_ray, ray_bwd
     if args.features:
@@ -322,20 +321,22 @@ def run_ours(args):
     alu_peak = SMS * LANES_PER_SM * sm_max * 1e6 / 1e12          # T lane-ops/s (FMA = 1 lane-op)
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     sec = lambda n: stage_ms[n] / 1e3
-    # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + 20 B per visible
-    # Gaussian (row scan) + 36 B per row (table written, counts scanned in place, read by emit) + per sorted pair:
-    # 8 B emitted, 16 B per intermediate tile pass, 8 B read + 12 B written by the last one
-    sort_bytes = (8 * sc.N + (4 * 16 + 20) * n_vis + 36 * n_rows
-                  + n_pairs * (8 + 16 * (tile_passes - 1) + 20))
+    # 8 B per Gaussian (compact) + 16 B per visible Gaussian per depth pass + 36 B per visible Gaussian
+    # (rank scan: index, rectangle, tile count read; two offsets written) + 8 B per row (4 written by rows, 4 read by
+    # final) + per supertile word 8 B emitted, 16 B sorted per supertile digit, 8 + 28 B read by final (word; index,
+    # depth bits, rectangle, row base of its Gaussian) + 12 B per pair (key + value written once)
+    n_words = pipe.words_on_device()
+    st_passes = max(1, ((max(1, ((pipe.TW + 7) // 8) * ((pipe.TH + 7) // 8)) - 1).bit_length() + 7) // 8)
+    sort_bytes = (8 * sc.N + (4 * 16 + 36) * n_vis + 8 * n_rows + (8 + 16 * st_passes + 36) * n_words + 12 * n_pairs)
     rooflines = {
         "rasterize_fwd": {"kernel": (kname % "fwd") + ("<FEAT>" if args.features else ""), "bound": "alu",
                           "unit": "T lane-op/s", "peak": alu_peak,
                           "achieved": (fwd_ops[0] * visit + fwd_ops[1] * passed + feat_fwd_ops) / sec("rasterize_fwd") / 1e12},
-        "rasterize_bwd": {"kernel": "rasterize_feat_bwd_kernel" if args.features else kname % "bwd", "bound": "alu",
+        "rasterize_bwd": {"kernel": (kname % "bwd") + ("<FEAT>" if args.features else ""), "bound": "alu",
                           "unit": "T lane-op/s", "peak": alu_peak,
                           "achieved": (bwd_ops[0] * sum_n + bwd_ops[1] * blended + feat_bwd_ops) / sec("rasterize_bwd") / 1e12},
-        "bin_sort": {"kernel": "xpr_bin_sort%s (compact, 4 depth passes on Gaussians, row scan, rows, pair scan, emit, "
-                               "%d tile passes on pairs, ranges)" % ("_cull" if args.tile_cull else "", tile_passes), "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
+        "bin_sort": {"kernel": "xpr_bin_sort%s (compact, 4 depth passes on Gaussians, rank scan, rows, supertile words, "
+                               "tile scan, %d supertile pass(es) on words, final)" % ("_cull" if args.tile_cull else "", tile_passes), "bound": "hbm", "unit": "GB/s", "peak": hbm_peak,
                      "achieved": sort_bytes / sec("bin_sort") / 1e9, "algorithmic_bytes": sort_bytes},
     }
     traffic = {}
@@ -502,8 +503,9 @@ def run_ours(args):
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
                            "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
-                           "candidate_pairs": n_cand, "rows": n_rows, "visible_gaussians": n_vis,
-                           "sort_passes": {"depth_digits_on_gaussians": 4, "tile_digits_on_pairs": tile_passes},
+                           "candidate_pairs": n_cand, "rows": n_rows, "supertile_words": n_words, "visible_gaussians": n_vis,
+                           "sort_passes": {"depth_digits_on_gaussians": 4, "supertile_digits_on_words": tile_passes,
+                                           "on_pairs": 0},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},
                 "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,

@@ -102,19 +102,23 @@ int32_t xpr_shade_record(int64_t N, const float* mean2d, const float* conic_opac
  * xpr_bin_sort -- Rasterizer stage: prefix-sum of tile counts, replication,
  * tile-id assignment  x = x_min + (r mod w), y = y_min + floor(r / w), t = y*tiles_x + x,
  * key = (uint64)t << 32 | float_bits(depth) (BASELINE.json:north_star, C10), value = Gaussian
- * index; stable LSD radix sort by key (hand-written onesweep); per-tile bounds.
+ * index; the result of the stable LSD radix sort by key, produced by hand-written kernels (onesweep passes on the
+ * depth bits of the Gaussians and on the supertile ids, then one pass that writes every pair at its final position,
+ * DESIGN.md 6.2); per-tile bounds.
  *   in : depth[N], tile_rect[N,4], tile_count[N] from xpr_project; pair_capacity = length of the
  *        output arrays (must be < 2^30; 0 is allowed and makes the call a size probe: with any visible
  *        Gaussian it reports XPR_ERR_CAPACITY and the capacity that suffices, in both modes below).
  *        N must be < 2^30 (XPR_ERR_UNSUPPORTED otherwise: the sort's look-back words carry 30-bit counts).
  *   out: keys_sorted[I] u64, vals_sorted[I] u32, tile_ranges[T,2] = (start,end) per tile, (0,0)
  *        for an empty tile; *num_pairs_host (HOST int64) = I.
- *   Capacity: pair_capacity must hold I = sum of tile_count (the candidate pairs) and must exceed
- *   the number of (Gaussian, tile-row) rows, which is <= I; practically: pair_capacity > I.
+ *   Capacity: besides the I output pairs, the output arrays serve as scratch for the (Gaussian, tile row) rows
+ *   (4 bytes each) and for the (Gaussian, 8 x 8-tile supertile) words the call sorts first (8 bytes each, two
+ *   buffers): pair_capacity >= max(I, rows + 1, 2 x words).  rows and words are at most sum of tile_count; for
+ *   Gaussians that cover a few tiles each 2 x words can exceed I.
  *   Nothing inside the call waits for the host: every count stays on the device and every kernel
  *   reads it there.  With num_pairs_host != NULL the call ends with a 16-byte read-back of the counts
  *   and a stream synchronisation; if the capacity does not suffice -> XPR_ERR_CAPACITY with
- *   *num_pairs_host = the capacity that suffices (max(I, rows + 1)).
+ *   *num_pairs_host = the capacity that suffices (max(I, rows + 1, 2 x words)).
  *   With num_pairs_host == NULL the call is fully asynchronous (capturable in a CUDA graph): it
  *   returns XPR_OK after enqueueing; once the stream has run, workspace bytes [0,8) hold (uint64) the
  *   number of sorted pairs, or the capacity that suffices when it exceeds pair_capacity -- the caller
@@ -145,8 +149,9 @@ int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* tile_rect, co
  * survivors are compacted in emission order and only they are sorted.
  *   in : as xpr_bin_sort + the tile-cull data p_tcd of xpr_project: mean2d[N,2], conic_opac[N,4], lnv[N].
  *   out: as xpr_bin_sort; *num_pairs_host = number of SURVIVING pairs (= length of the sorted arrays).
- *   pair_capacity as for xpr_bin_sort: it must hold the CANDIDATE count (sum of tile_count), not only
- *   the survivors; otherwise XPR_ERR_CAPACITY with *num_pairs_host = the capacity that suffices.
+ *   pair_capacity as for xpr_bin_sort, with I the SURVIVING pairs (rejected pairs are never generated, so the
+ *   candidate count sum of tile_count need not fit); otherwise XPR_ERR_CAPACITY with *num_pairs_host = the capacity
+ *   that suffices.
  *   With cfg->tile_cull == 0 the call is xpr_bin_sort; xpr_bin_sort itself rejects cfg->tile_cull != 0.
  */
 int32_t xpr_bin_sort_cull(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,

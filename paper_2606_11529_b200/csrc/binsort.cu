@@ -579,9 +579,10 @@ __device__ __forceinline__ float approx_sqrt(float x) {   // the interval estima
     return y;
 }
 
+constexpr int ROW_SMEM = 2048;     // tile rows whose first-tile counter is kept in shared memory
 template <bool CULL>
 __global__ void __launch_bounds__(128)
-rows_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ row_base,
+rows_kernel(int TW, int TH, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ row_base,
             const int4* __restrict__ rect, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
             const float* __restrict__ lnv, const Header* __restrict__ hdr, uint32_t* __restrict__ row_tab,
             int* __restrict__ tile_diff) {
@@ -595,6 +596,9 @@ rows_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
     const unsigned long long rows_total = hdr->rows_total;
     const uint32_t n_rows = (rows_total >= FIELD_MAX) ? 0u : (uint32_t)rows_total, n_vis = hdr->n_vis;
     const bool store = hdr->rows_eff != 0ull;
+    __shared__ int s_rowstart[ROW_SMEM];
+    for (int y = threadIdx.x; y <= TH && y < ROW_SMEM; y += 128) s_rowstart[y] = 0;
+    __syncthreads();
     const int lane = threadIdx.x & 31;
     for (uint32_t wrow = (blockIdx.x * 128u + threadIdx.x) & ~31u; wrow < n_rows; wrow += gridDim.x * 128u) {
         uint32_t lo = 0, hi = n_vis;                 // first index whose base is > wrow lies in [lo, hi]
@@ -686,10 +690,17 @@ rows_kernel(int TW, const uint32_t* __restrict__ vidx, const uint32_t* __restric
         // -1 behind its end -- the running sum of the array is the number of pairs of every tile
         if (store) row_tab[row] = (uint32_t)xa | ((uint32_t)(xb - xa) << 16);
         if (xb > xa) {
+            // the first tile of a tile row is the hot address (every Gaussian clipped by the left image edge starts
+            // there, every one clipped by the right edge ends at the next row's first tile): those go to shared memory
             const int t0 = ty * TW;
-            atomicAdd(tile_diff + t0 + xa, 1);
-            atomicAdd(tile_diff + t0 + xb, -1);
+            if (xa == 0 && ty < ROW_SMEM) atomicAdd(&s_rowstart[ty], 1); else atomicAdd(tile_diff + t0 + xa, 1);
+            if (xb == TW && ty + 1 < ROW_SMEM) atomicAdd(&s_rowstart[ty + 1], -1); else atomicAdd(tile_diff + t0 + xb, -1);
         }
+    }
+    __syncthreads();
+    for (int y = threadIdx.x; y <= TH && y < ROW_SMEM; y += 128) {
+        const int v = s_rowstart[y];
+        if (v) atomicAdd(tile_diff + y * TW, v);
     }
 }
 
@@ -735,15 +746,19 @@ __device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, 
 // sort by supertile leaves every segment in rank order.  Also the digit histograms of the supertile ids (for
 // the onesweep passes) and the number of words of every supertile (the segments).
 // ---------------------------------------------------------------------------------------------
+constexpr int SEG_SMEM = 4096;              // supertile counters kept in shared memory (larger images: global atomics)
 template <int PASSES>
 __global__ void __launch_bounds__(256)
-l1_emit_kernel(int STW, const uint32_t* __restrict__ vidx, const int4* __restrict__ rect,
+l1_emit_kernel(int STW, uint32_t ST, const uint32_t* __restrict__ vidx, const int4* __restrict__ rect,
                const uint32_t* __restrict__ l1_off, Header* __restrict__ hdr, uint64_t* __restrict__ words,
                uint32_t* __restrict__ seg_cnt) {
     __shared__ uint32_t s_hist[PASSES * RADIX];
+    __shared__ uint32_t s_seg[SEG_SMEM];
     if (hdr->l1_eff == 0ull) return;                    // nothing visible, or the tables do not fit
     const uint32_t n_vis = hdr->n_vis;
+    const bool seg_shared = ST <= (uint32_t)SEG_SMEM;   // a few hundred addresses: global atomics would serialise on them
     for (int b = threadIdx.x; b < PASSES * RADIX; b += 256) s_hist[b] = 0u;
+    if (seg_shared) for (uint32_t b = threadIdx.x; b < ST; b += 256) s_seg[b] = 0u;
     __syncthreads();
     for (uint32_t r = blockIdx.x * 256u + threadIdx.x; r < n_vis; r += gridDim.x * 256u) {
         const int4 q = __ldg(rect + __ldg(vidx + r));
@@ -754,7 +769,7 @@ l1_emit_kernel(int STW, const uint32_t* __restrict__ vidx, const int4* __restric
             for (int sx = sx0; sx < sx1; ++sx) {
                 const uint32_t sid = (uint32_t)(sy * STW + sx);
                 words[off++] = ((uint64_t)sid << 32) | (uint64_t)r;
-                atomicAdd(seg_cnt + sid, 1u);
+                if (seg_shared) atomicAdd(&s_seg[sid], 1u); else atomicAdd(seg_cnt + sid, 1u);
 #pragma unroll
                 for (int d = 0; d < PASSES; ++d) atomicAdd(&s_hist[d * RADIX + ((sid >> (8 * d)) & 255u)], 1u);
             }
@@ -764,6 +779,11 @@ l1_emit_kernel(int STW, const uint32_t* __restrict__ vidx, const int4* __restric
         const uint32_t v = s_hist[b];
         if (v) atomicAdd(&hdr->hist[DEPTH_PASSES * RADIX + b], v);
     }
+    if (seg_shared)
+        for (uint32_t b = threadIdx.x; b < ST; b += 256) {
+            const uint32_t v = s_seg[b];
+            if (v) atomicAdd(seg_cnt + b, v);
+        }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -803,23 +823,48 @@ tile_scan_kernel(uint32_t T, uint32_t ST, unsigned long long pair_capacity, cons
                  uint32_t* __restrict__ chunk_start, Header* __restrict__ hdr) {
     __shared__ uint32_t s_warp[TS_THREADS / 32];
     const uint32_t tid = threadIdx.x;
-    // per-tile counts (running sum of the differences) and bases (exclusive prefix of the counts)
-    uint32_t carry_cnt = 0;                      // running sum of the differences before this block of tiles
-    unsigned long long carry_base = 0;           // pairs of all earlier tiles
-    for (uint32_t t0 = 0; t0 < T; t0 += TS_THREADS) {
-        const uint32_t t = t0 + tid;
-        const uint32_t d = (t < T) ? (uint32_t)tile_diff[t] : 0u;      // two's complement: the sums are exact mod 2^32
-        uint32_t tot_d, tot_c;
-        const uint32_t cnt = carry_cnt + block_scan_incl(d, s_warp, tot_d);
-        const uint32_t c = (t < T) ? cnt : 0u;
-        const uint32_t incl = block_scan_incl(c, s_warp, tot_c);
-        if (t < T) {
-            const unsigned long long start = carry_base + (incl - c);
-            // positions beyond 2^32 cannot occur for a count that fits the capacity; they are zeroed below otherwise
-            ranges[t] = c ? make_uint2((uint32_t)start, (uint32_t)(start + c)) : make_uint2(0u, 0u);
+    // per-tile counts (running sum of the differences) and bases (exclusive prefix of the counts): a thread owns
+    // `per` consecutive tiles, so each of the two prefix sums is a local loop, one block scan and a local loop
+    __shared__ unsigned long long s_wtot[TS_THREADS / 32];
+    __shared__ unsigned long long s_total;
+    const int lane = tid & 31, warp = tid >> 5;
+    const uint32_t per = (T + TS_THREADS - 1) / TS_THREADS;
+    const uint32_t t_lo = min(tid * per, T), t_hi = min(t_lo + per, T);
+    uint32_t dsum = 0;
+    for (uint32_t t = t_lo; t < t_hi; ++t) dsum += (uint32_t)tile_diff[t];          // two's complement: exact mod 2^32
+    uint32_t tot_d;
+    const uint32_t cnt0 = block_scan_incl(dsum, s_warp, tot_d) - dsum;             // running sum before my first tile
+    uint32_t cnt = cnt0;
+    unsigned long long csum = 0;                                                    // pairs of my tiles
+    for (uint32_t t = t_lo; t < t_hi; ++t) { cnt += (uint32_t)tile_diff[t]; csum += cnt; }
+    unsigned long long base;                                                        // pairs of all earlier tiles (64-bit scan)
+    {
+        unsigned long long incl = csum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long a = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += a;
         }
-        carry_cnt += tot_d;
-        carry_base += tot_c;
+        if (lane == 31) s_wtot[warp] = incl;
+        __syncthreads();
+        unsigned long long pre = 0, tot = 0;
+#pragma unroll
+        for (int w = 0; w < TS_THREADS / 32; ++w) {
+            const unsigned long long a = s_wtot[w];
+            if (w < warp) pre += a;
+            tot += a;
+        }
+        base = pre + incl - csum;
+        if (tid == 0) s_total = tot;
+        __syncthreads();
+    }
+    const unsigned long long carry_base = s_total;
+    cnt = cnt0;
+    for (uint32_t t = t_lo; t < t_hi; ++t) {
+        cnt += (uint32_t)tile_diff[t];
+        // positions beyond 2^32 cannot occur for a count that fits the capacity; the ranges are zeroed below otherwise
+        ranges[t] = cnt ? make_uint2((uint32_t)base, (uint32_t)(base + cnt)) : make_uint2(0u, 0u);
+        base += cnt;
     }
     const unsigned long long I = carry_base;
     const unsigned long long rows = hdr->rows_total, l1 = hdr->l1_total;
@@ -860,15 +905,20 @@ tile_scan_kernel(uint32_t T, uint32_t ST, unsigned long long pair_capacity, cons
 
 // ---------------------------------------------------------------------------------------------
 // final: replicate + assign tile id + (the tile digits of the) sort in one pass.  A chunk is up to
-// CHUNK consecutive words of ONE supertile's segment (words in rank order); thread i owns word i:
+// CHUNK consecutive words of ONE supertile's segment (words in rank order); thread i first owns word i:
 //   1. its Gaussian's rows inside the supertile (row table) -> 64-bit mask of the tiles it covers there;
-//   2. per warp and per tile bit: ballot -> number of covering lanes (counts) and of covering lanes before me;
+//   2. per warp and per tile bit present in the warp: ballot -> the column of the bit (which lanes cover the
+//      tile) and its population count;
 //   3. per (chunk, bit): exclusive prefix over the warps, total published, decoupled look-back over the earlier
 //      chunks of the segment (the chunk index is a ticket: every predecessor is running or done);
-//   4. pair (tile of bit b, my Gaussian) goes to tile start + pairs of earlier chunks + pairs of earlier warps +
-//      covering lanes before me: key = tile << 32 | depth bits, value = Gaussian index.  For a fixed bit the
-//      covering lanes of a warp write consecutive positions.
-// Within a tile the pairs are therefore in rank = (depth, index) order: the stable sort by (tile, depth).
+//   4. the warp walks the bits present in it once more: for a fixed bit the covering lanes write consecutive
+//      positions, tile start + pairs of earlier chunks + pairs of earlier warps + covering lanes before me (popcount
+//      of the saved column below the lane): key = tile << 32 | depth bits, value = Gaussian index.
+//      (Measured alternatives, config 5 / config 3, this variant 380 / 48 us: every lane walking its own bits, fewest
+//      instructions but scattered stores, 627 / 50 us; one pair per thread in output order, fully coalesced, with a
+//      select of the k-th set bit per pair 410 / 43 us, with a byte table of word numbers in shared memory 464 / 56 us;
+//      staging key and value of the pairs in shared memory in rounds 655 / 74 us.)
+// Within a tile the pairs are in rank = (depth, index) order: the stable sort by (tile, depth).
 // ---------------------------------------------------------------------------------------------
 #ifndef XPR_FINAL_LB
 #define XPR_FINAL_LB 4
@@ -881,11 +931,12 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
              const uint2* __restrict__ ranges, Header* __restrict__ hdr, uint32_t* __restrict__ status,
              uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out) {
     __shared__ uint32_t s_cnt[CHUNK_WARPS][ST_BINS];    // per warp: covering lanes, then exclusive prefix over warps
+    __shared__ uint32_t s_col[CHUNK_WARPS][ST_BINS];    // per warp: the lanes whose Gaussian covers the bit's tile
     __shared__ uint32_t s_base[ST_BINS];                // global position of the chunk's first pair of every bit
+    __shared__ uint32_t s_tile[ST_BINS];                // tile id of every bit
     __shared__ uint32_t s_chunk, s_seg, s_seg_c0;       // ticket; supertile of the chunk; first chunk of that supertile
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n_chunks = hdr->n_chunks;
-    const uint32_t lt = (1u << lane) - 1u;
     uint32_t seg = 0;                                   // tickets grow: the search resumes where the last one ended
     while (true) {
         __syncthreads();                                // previous chunk done with the shared arrays
@@ -937,17 +988,17 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
                 if (k < 4) m_lo |= bits << (8 * k); else m_hi |= bits << (8 * (k - 4));
             }
         }
-        // 2. per warp: bits present, counts per bit
+        // 2. per warp: the column and the count of every bit present
         const uint32_t u_lo = __reduce_or_sync(0xffffffffu, m_lo), u_hi = __reduce_or_sync(0xffffffffu, m_hi);
         for (uint32_t u = u_lo; u; u &= u - 1u) {
             const int b = __ffs(u) - 1;
             const uint32_t bal = __ballot_sync(0xffffffffu, (m_lo >> b) & 1u);
-            if (lane == 0) s_cnt[warp][b] = (uint32_t)__popc(bal);
+            if (lane == 0) { s_col[warp][b] = bal; s_cnt[warp][b] = (uint32_t)__popc(bal); }
         }
         for (uint32_t u = u_hi; u; u &= u - 1u) {
             const int b = __ffs(u) - 1;
             const uint32_t bal = __ballot_sync(0xffffffffu, (m_hi >> b) & 1u);
-            if (lane == 0) s_cnt[warp][32 + b] = (uint32_t)__popc(bal);
+            if (lane == 0) { s_col[warp][32 + b] = bal; s_cnt[warp][32 + b] = (uint32_t)__popc(bal); }
         }
         __syncthreads();
         // 3. per bit: prefix over the warps, look-back over the earlier chunks of this segment
@@ -985,31 +1036,35 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
                 st_relaxed(my, FLAG_INCLUSIVE | (excl_prev + count));
             }
             const int tx = tx0 + (tid & (ST_EDGE - 1)), ty = ty0 + (tid >> ST_SHIFT);
-            const uint32_t start = (tx < TW && ty < TH) ? ranges[ty * TW + tx].x : 0u;
-            s_base[tid] = start + excl_prev;
+            const bool inside = tx < TW && ty < TH;
+            s_tile[tid] = (uint32_t)(ty * TW + tx);
+            s_base[tid] = (inside ? ranges[ty * TW + tx].x : 0u) + excl_prev;
         }
         __syncthreads();
-        // 4. scatter: for a fixed bit the covering lanes of a warp write consecutive positions
-        for (uint32_t u = u_lo; u; u &= u - 1u) {
-            const int b = __ffs(u) - 1;
-            const bool mine = (m_lo >> b) & 1u;
-            const uint32_t bal = __ballot_sync(0xffffffffu, mine);
-            if (mine) {
-                const uint32_t pos = s_base[b] + s_cnt[warp][b] + (uint32_t)__popc(bal & lt);
-                const uint32_t tile = (uint32_t)((ty0 + (b >> ST_SHIFT)) * TW + tx0 + (b & (ST_EDGE - 1)));
-                keys_out[pos] = ((uint64_t)tile << 32) | (uint64_t)dbits;
-                vals_out[pos] = g;
+        // 4. scatter: the warp walks the bits present in it once more (warp-uniform loop); for a fixed bit the covering
+        //    lanes (the column saved in step 2) write consecutive positions: tile start + pairs of earlier chunks + pairs
+        //    of earlier warps + covering lanes before me
+        {
+            s_cnt[warp][lane] += s_base[lane];          // per warp: first position of the warp's pairs of every bit
+            s_cnt[warp][lane + 32] += s_base[lane + 32];
+            __syncwarp();
+            const uint32_t lt = (1u << lane) - 1u;
+            const uint64_t dkey = (uint64_t)dbits;
+            for (uint32_t u = u_lo; u; u &= u - 1u) {
+                const int b = __ffs(u) - 1;
+                if ((m_lo >> b) & 1u) {
+                    const uint32_t pos = s_cnt[warp][b] + (uint32_t)__popc(s_col[warp][b] & lt);
+                    keys_out[pos] = ((uint64_t)s_tile[b] << 32) | dkey;
+                    vals_out[pos] = g;
+                }
             }
-        }
-        for (uint32_t u = u_hi; u; u &= u - 1u) {
-            const int b = __ffs(u) - 1;
-            const bool mine = (m_hi >> b) & 1u;
-            const uint32_t bal = __ballot_sync(0xffffffffu, mine);
-            if (mine) {
-                const uint32_t pos = s_base[32 + b] + s_cnt[warp][32 + b] + (uint32_t)__popc(bal & lt);
-                const uint32_t tile = (uint32_t)((ty0 + 4 + (b >> ST_SHIFT)) * TW + tx0 + (b & (ST_EDGE - 1)));
-                keys_out[pos] = ((uint64_t)tile << 32) | (uint64_t)dbits;
-                vals_out[pos] = g;
+            for (uint32_t u = u_hi; u; u &= u - 1u) {
+                const int b = __ffs(u) - 1;
+                if ((m_hi >> b) & 1u) {
+                    const uint32_t pos = s_cnt[warp][32 + b] + (uint32_t)__popc(s_col[warp][32 + b] & lt);
+                    keys_out[pos] = ((uint64_t)s_tile[32 + b] << 32) | dkey;
+                    vals_out[pos] = g;
+                }
             }
         }
     }
@@ -1183,19 +1238,18 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     // 4. rows: surviving interval per (Gaussian, tile row) -> row table + difference array over the tile ids
     const unsigned rgrid = 148u * 16u;                               // grid-stride over the rows (count on the device)
     if (cull)
-        rows_kernel<true><<<rgrid, 128, 0, st>>>(TW, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
+        rows_kernel<true><<<rgrid, 128, 0, st>>>(TW, TH, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
                                                  reinterpret_cast<const float4*>(conic_opac), lnv, hdr, row_tab, tile_diff);
     else
-        rows_kernel<false><<<rgrid, 128, 0, st>>>(TW, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, hdr, row_tab,
+        rows_kernel<false><<<rgrid, 128, 0, st>>>(TW, TH, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, hdr, row_tab,
                                                   tile_diff);
     XPR_LAUNCH_CHECK();
     // 5. supertile words in rank order; pass p of the supertile sort reads buffer p and writes buffer p + 1, the
     //    last one writes the half buffer (keys_sorted is free until the final pass)
     uint64_t* w0 = (l1_passes % 2 == 1) ? keys_sorted : words_half;
     uint64_t* w1 = (l1_passes % 2 == 1) ? words_half : keys_sorted;
-    const unsigned egrid = (unsigned)(((size_t)N + 255) / 256) < (unsigned)PERSIST_CTAS ? (unsigned)(((size_t)N + 255) / 256)
-                                                                                       : (unsigned)PERSIST_CTAS;
-#define XPR_EMIT(P_) l1_emit_kernel<P_><<<egrid, 256, 0, st>>>(STW, vidx[0], rect4, l1_off, hdr, w0, seg_cnt)
+    const unsigned egrid = (unsigned)(((size_t)N + 255) / 256) < 2u * 148u ? (unsigned)(((size_t)N + 255) / 256) : 2u * 148u;
+#define XPR_EMIT(P_) l1_emit_kernel<P_><<<egrid, 256, 0, st>>>(STW, (uint32_t)ST, vidx[0], rect4, l1_off, hdr, w0, seg_cnt)
     switch (l1_passes) {
         case 1: XPR_EMIT(1); break;
         case 2: XPR_EMIT(2); break;

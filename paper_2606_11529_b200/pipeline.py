@@ -124,14 +124,18 @@ class SplatPipeline:
         return (self.mean2d, self.conic_opac, self.lnv) if int(self.cfg.tile_cull) else None
 
     def pairs_on_device(self):
-        """(candidate pairs, pairs in the sorted output) of the last bin_sort call, from the first 16 bytes of
-        the workspace (synchronises).  They differ only with tile_cull."""
+        """(I or, when it does not fit, the capacity that suffices; pairs in the sorted output) of the last bin_sort
+        call, from the first 16 bytes of the workspace (synchronises)."""
         c = self.workspace[:16].view(torch.int64).tolist()
         return int(c[0]), int(c[1])
 
     def rows_on_device(self) -> int:
         """Number of (Gaussian, tile row) segments of the last bin_sort call (workspace bytes [24, 32))."""
         return int(self.workspace[24:32].view(torch.int64).item())
+
+    def words_on_device(self) -> int:
+        """Number of (Gaussian, supertile) words of the last bin_sort call (workspace bytes [16, 24))."""
+        return int(self.workspace[16:24].view(torch.int64).item())
 
     def candidates_on_device(self) -> int:
         """Candidate pairs (sum of tile_count over the visible Gaussians) of the last call (workspace bytes [40, 48))."""

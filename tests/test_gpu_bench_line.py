@@ -26,7 +26,7 @@ def test_bench_line_ours():
         assert k in d, k
     assert d["n_gpus"] == 1 and d["steps"] == 3 and d["value"] > 0 and d["vs_baseline"] is None
     assert "workload" in d["config"] and "model" not in d["config"]
-    assert d["gpu_launches"] == 3 * 16          # 64x64 image: 16 tiles, one tile-digit pass; + xpr_loss_grad
+    assert d["gpu_launches"] == 3 * 16          # 11 launches of xpr_bin_sort (one supertile-digit pass); + xpr_loss_grad
     r = d["roofline"]
     assert r["bound"] in ("hbm", "alu", "tensor") and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
     assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0 and d["e2e"]["value"] > 0
@@ -45,14 +45,14 @@ def test_bench_line_ray_evaluation():
     d = _run("--config", "4", "--ray-eval", "1", "--no-cpu-baseline", "--no-e2e")
     assert d["config"]["ray_eval"] == 1 and d["value"] > 0
     assert d["roofline"]["kernel"].startswith("rasterize_ray_")
-    assert d["gpu_launches"] == 3 * (17 + 3)    # 1080p: two tile-digit passes; + pixel_info, project_ray, ray_bwd
+    assert d["gpu_launches"] == 3 * (16 + 3)    # 1080p: 135 supertiles, one digit pass; + pixel_info, project_ray, ray_bwd
 
 
 def test_bench_line_rendered_features():
     d = _run("--config", "3", "--features", "1", "--no-cpu-baseline")
     assert d["config"]["features"] == 1 and d["value"] > 0
-    assert d["rooflines"]["rasterize_bwd"]["kernel"] == "rasterize_feat_bwd_kernel"
-    assert d["gpu_launches"] == 3 * (17 + 1)    # + depth_bwd
+    assert d["rooflines"]["rasterize_bwd"]["kernel"] == "rasterize_bwd_kernel<FEAT>"
+    assert d["gpu_launches"] == 3 * (16 + 1)    # + depth_bwd
     assert d["e2e"]["d2h_bytes_per_step"] > 1920 * 1080 * 4 * 5    # image, D and A all come back
 
 
