@@ -55,6 +55,10 @@ def parse():
     ap.add_argument("--ray-eval", type=int, default=0, choices=(0, 1),
                     help="1: XPR-3DGUT evaluation along the pixel ray (SURVEY 8(f) f2; meant for --config 4) instead of "
                          "the 2D conic of north_star")
+    ap.add_argument("--sort-compare", action="store_true",
+                    help="after the timed steps, also time cub::DeviceRadixSort::SortPairs (libxpr_cubcmp.so, built on demand; "
+                         "never on the path) on the same (key, value) pairs in emission order, beside xpr_bin_sort "
+                         "(reported as 'cub_compare'; BASELINE.json:north_star)")
     ap.add_argument("--stages", action="store_true", help="also print per-stage times to stderr")
     return ap.parse_args()
 
@@ -396,6 +400,44 @@ def run_ours(args):
                  "bwd_ms": _time(lambda: pipe.rasterize_featn_bwd(feat, gF, g_feat)),
                  "how": "20 back-to-back launches each, CUDA events, warm L2, after the timed steps"}
 
+    cub_compare = None
+    if args.sort_compare:
+        import ctypes as C
+        from paper_2606_11529_b200 import build as xbuild
+        cl = C.CDLL(xbuild.build_cub_compare())
+        cl.xpr_cubcmp_sort_pairs.restype = C.c_int32
+        I = n_pairs
+        ks, vs = pipe.keys_sorted[:I].clone(), pipe.vals_sorted[:I].clone()
+        # the pairs in EMISSION order (Gaussian by Gaussian, row-major inside its rectangle = ascending tile id):
+        # a stable sort of the sorted pairs by Gaussian index restores it
+        order = torch.argsort(vs.to(torch.int64), stable=True)
+        kin, vin = ks[order].contiguous(), vs[order].contiguous()
+        kout, vout = torch.empty_like(kin), torch.empty_like(vin)
+        end_bit = 32 + max(1, (pipe.T - 1).bit_length())
+        nbytes = C.c_size_t(0)
+        stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+        p = lambda t: C.c_void_p(t.data_ptr())
+        assert cl.xpr_cubcmp_sort_pairs(C.c_int64(I), p(kin), p(vin), p(kout), p(vout), None, C.byref(nbytes), 0, end_bit, stream) == 0
+        temp = torch.empty(max(int(nbytes.value), 1), dtype=torch.uint8, device=dev)
+        run = lambda: cl.xpr_cubcmp_sort_pairs(C.c_int64(I), p(kin), p(vin), p(kout), p(vout), p(temp), C.byref(nbytes), 0, end_bit, stream)
+        for _ in range(3):
+            assert run() == 0
+        torch.cuda.synchronize()
+        same = bool(torch.equal(kout, ks) and torch.equal(vout, vs))     # both are THE stable sort by key
+        ts = []
+        for _ in range(max(args.steps, 5)):
+            flush.fill_(1)
+            a = _rec(); run(); b = _rec()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ts.sort()
+        cub_compare = {"pairs": I, "key_bits_sorted": end_bit, "cub_sort_pairs_ms": {"median": ts[len(ts) // 2], "min": ts[0]},
+                       "cub_temp_bytes": int(nbytes.value), "output_equals_xpr_bin_sort": same,
+                       "xpr_bin_sort_ms": stage_ms["bin_sort"],
+                       "note": "CUB sorts (u64 key, u32 value) pairs that already exist in memory; xpr_bin_sort starts from the "
+                               "projection outputs: it also compacts, scans, culls, generates the pairs and writes tile_ranges"}
+        del ks, vs, kin, vin, kout, vout, temp, order
+
     clocks = sampler.stop()      # sampled (every 20 ms) over the timed steps and the graph replays
 
     # end to end through the public API with HOST buffers: H2D of the parameters, the step, D2H of results
@@ -511,7 +553,7 @@ def run_ours(args):
                 "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,
                 "pixel_pairs": {"visited": visit, "passed_gate": passed, "blended": blended, "sum_n_contrib": sum_n},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-                "cuda_graph_ms_per_step": graph_ms, "featn": featn, "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}
+                "cuda_graph_ms_per_step": graph_ms, "featn": featn, "cub_compare": cub_compare, "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
         if args.stages:
             print(json.dumps(stage_ms, indent=1), file=sys.stderr)

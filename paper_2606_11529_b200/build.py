@@ -61,5 +61,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return OUT
 
 
+CUBCMP_OUT = os.path.join(HERE, "libxpr_cubcmp.so")
+
+
+def build_cub_compare(force: bool = False) -> str:
+    """libxpr_cubcmp.so: cub::DeviceRadixSort::SortPairs behind one C function, for `bench.py --sort-compare` only
+    (BASELINE.json:north_star: "CUB is timed only as a comparison").  Never linked into or loaded by libxpr.so."""
+    src = os.path.join(CSRC, "cub_compare.cu")
+    if force or not _newer(CUBCMP_OUT, [src, os.path.abspath(__file__)]):
+        cmd = [NVCC, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
+               "-shared", "-o", CUBCMP_OUT, src, "-cudart", "shared", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
+        subprocess.run(cmd, check=True)
+    return CUBCMP_OUT
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--cub-compare" in sys.argv:
+        print(build_cub_compare(force="--force" in sys.argv))
