@@ -162,6 +162,19 @@ int64_t xpr_oracle_bin_sort_cull(int64_t N, const float* depth, const int32_t* t
                                           const T* dL_dimage, double* g_ray_rec, double* g_opac_eff,     \
                                           double* g_rgb);                                                \
     /* chain rule record -> (mu, s, q); WRITES its outputs (the caller adds them to project_bwd's) */    \
+    /* the same sums in the form the GPU accumulates: g_ray_acc [N*16] = S_c = sum k c c^T (6), D = sum 2 dL/ddd  \
+       d d^T (6), sum dL/do_c (3), unused (1); mass != 0: sums of |addend|.  xpr_oracle_ray_bwd_acc applies the     \
+       chain rule to them; the two routes are equal (pin P14f) */                                                   \
+    void xpr_oracle_rasterize_ray_bwd_acc_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,     \
+                                          const T* ray_rec, const T* opac_eff, const T* rgb,             \
+                                          const T* lnv, const T* pixel_rays, const uint32_t* vals_sorted,\
+                                          const uint32_t* tile_ranges, const uint32_t* n_contrib,        \
+                                          const T* dL_dimage, int32_t mass, double* g_ray_acc,           \
+                                          double* g_opac_eff, double* g_rgb);                            \
+    void xpr_oracle_ray_bwd_acc_##S(int64_t N, const T* means, const T* scales, const T* quats,          \
+                                const xo_camera* cam, const uint32_t* tile_count,                        \
+                                const double* g_ray_acc, double* g_means, double* g_scales,              \
+                                double* g_quats);                                                        \
     void xpr_oracle_ray_bwd_##S(int64_t N, const T* means, const T* scales, const T* quats,              \
                                 const xo_camera* cam, const uint32_t* tile_count,                        \
                                 const double* g_ray_rec, double* g_means, double* g_scales,              \

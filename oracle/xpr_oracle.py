@@ -329,6 +329,36 @@ def ray_bwd(means, scales, quats, tile_count, g_ray_rec, cam: XoCamera, dtype=np
     return out
 
 
+def rasterize_ray_bwd_acc(proj: dict, binned: dict, fwd: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32,
+                          mass: bool = False) -> dict:
+    """rasterize_ray_bwd with the record gradient in the accumulator form the GPU sums (g_ray_acc [N,16]: S_c 6, D 6,
+    sum dL/do_c 3, unused 1; xpr_oracle_ray.inc)."""
+    dt = np.dtype(dtype)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("ray_rec", "opac_eff", "rgb", "lnv", "pixel_rays")]
+    dL = np.ascontiguousarray(dL_dimage, dt)
+    out = dict(g_ray_acc=np.empty((N, 16), np.float64), g_opac_eff=np.empty(N, np.float64),
+               g_rgb=np.empty((N, 3), np.float64))
+    fn = getattr(lib(), "xpr_oracle_rasterize_ray_bwd_acc_" + _sfx(dt))
+    fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+       _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), _p(dL), C.c_int32(1 if mass else 0),
+       _p(out["g_ray_acc"]), _p(out["g_opac_eff"]), _p(out["g_rgb"]))
+    return out
+
+
+def ray_bwd_acc(means, scales, quats, tile_count, g_ray_acc, cam: XoCamera, dtype=np.float32) -> dict:
+    """Chain rule from the accumulators of rasterize_ray_bwd_acc to (mu, s, q)."""
+    dt = np.dtype(dtype)
+    N = int(means.shape[0])
+    a = [np.ascontiguousarray(x, dt) for x in (means, scales, quats)]
+    out = dict(g_means=np.empty((N, 3), np.float64), g_scales=np.empty((N, 3), np.float64),
+               g_quats=np.empty((N, 4), np.float64))
+    getattr(lib(), "xpr_oracle_ray_bwd_acc_" + _sfx(dt))(
+        C.c_int64(N), *[_p(x) for x in a], C.byref(cam), _p(np.ascontiguousarray(tile_count, np.uint32)),
+        _p(np.ascontiguousarray(g_ray_acc, np.float64)), *[_p(out[k]) for k in ("g_means", "g_scales", "g_quats")])
+    return out
+
+
 def render_ray(scene_arrays: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
     """XPR-3DGUT forward (PAPER A.1.2): project (2D footprint for tiling / culling) -> shader record -> bin_sort ->
     pixel_info -> compositing with the ray evaluation."""

@@ -230,3 +230,59 @@ def test_p14e_agrees_with_the_2d_path_for_small_distant_gaussians():
     b = xo.render_ray(arr, cam, cfg, np.float64)["fwd"]["image"]
     assert np.abs(a - np.array([0.1, 0.2, 0.3])).max() > 0.2          # something is drawn
     assert np.abs(a - b).max() < 2e-2 and np.abs(a - b).mean() < 5e-4
+
+
+# ------------------------------------------------------------------------------------------------
+# P14f: the accumulator form of the record gradient (what the GPU sums: S_c = sum k c c^T, D = sum 2 dL/ddd d d^T,
+# sum dL/do_c) determines the same parameter gradients as the plain form (dL/dM_c, dL/do_c) of the definition:
+#   dL/dM_c - dL/do_c p^T = -(S_c - tr(S_c) I) M_c^-T + M_c D      (o_c = -M_c p, d_c = M_c d, c = o_c x d_c).
+# The plain route is pinned by finite differences (P14d); here the two routes must agree in fp64 on general scenes
+# (EWA / UT footprints, pinhole and fisheye), and the mass of the accumulators equals the brute-force sum over
+# one-pixel gradients, as for the other mass outputs (tests/test_oracle_mass_pins.py).
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,kw", [(1, dict(n_override=400)), (4, dict(n_override=6000, image_override=(96, 64))),
+                                       (2, dict(n_override=3000, image_override=(80, 80)))])
+def test_p14f_accumulator_route_equals_plain_route(config, kw):
+    sc = scenes.make_scene(config, **kw)
+    arr = {k: getattr(sc, k).astype(np.float64) for k in PARAMS}
+    cam = xo.make_camera(sc.cameras[0]); cfg = xo.make_config(scenes.default_render_config(sc))
+    r = xo.render_ray(arr, cam, cfg, np.float64)
+    assert r["fwd"]["pp_pass"] > 500
+    H, W = int(cam.height), int(cam.width)
+    G = np.random.default_rng(3).normal(0, 1, (H, W, 3))
+    plain = xo.rasterize_ray_bwd(r["proj"], r["binned"], r["fwd"], G, cam, cfg, np.float64)
+    acc = xo.rasterize_ray_bwd_acc(r["proj"], r["binned"], r["fwd"], G, cam, cfg, np.float64)
+    # (equal up to the order in which the tiles' contributions are added)
+    np.testing.assert_allclose(acc["g_opac_eff"], plain["g_opac_eff"], rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(acc["g_rgb"], plain["g_rgb"], rtol=1e-12, atol=1e-14)
+    s3 = np.abs(plain["g_ray_rec"][:, 9:12]).max()
+    np.testing.assert_allclose(acc["g_ray_acc"][:, 12:15], plain["g_ray_rec"][:, 9:12], rtol=1e-12, atol=1e-13 * s3)
+    tc = r["proj"]["tile_count"]
+    a = xo.ray_bwd(arr["means"], arr["scales"], arr["quats"], tc, plain["g_ray_rec"], cam, np.float64)
+    b = xo.ray_bwd_acc(arr["means"], arr["scales"], arr["quats"], tc, acc["g_ray_acc"], cam, np.float64)
+    for k in ("g_means", "g_scales", "g_quats"):
+        scale = np.abs(a[k]).max(axis=1, keepdims=True) + 1e-300
+        assert np.abs(a[k]).max() > 0
+        # per Gaussian: agreement to rounding of the LARGER of the two cancelling parts of the plain route
+        big = (np.abs(plain["g_ray_rec"]).max(axis=1, keepdims=True) * (1 + np.abs(arr["means"]).max()) + scale)
+        assert (np.abs(a[k] - b[k]) <= 1e-9 * big / np.minimum(arr["scales"].min(axis=1, keepdims=True), 1.0)).all(), k
+        # and to 1e-7 relative of the Gaussian's largest component for all but a handful (plain-route cancellation in fp64)
+        rel = np.abs(a[k] - b[k]) / scale
+        assert np.quantile(rel, 0.99) < 1e-8, (k, np.quantile(rel, 0.99))
+
+
+def test_p14f_accumulator_mass_equals_brute_force():
+    from test_oracle_mass_pins import _tiny, _one_pixel
+    arr, co = _tiny(24, opac_boost=1.5, ls=(-1.4, 0.4))
+    cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=0))
+    r = xo.render_ray(arr, cam, cfg, np.float64)
+    H, W = co.height, co.width
+    dL = np.random.default_rng(6).standard_normal((H, W, 3))
+    bwd = lambda d: xo.rasterize_ray_bwd_acc(r["proj"], r["binned"], r["fwd"], d, cam, cfg, np.float64)
+    m = xo.rasterize_ray_bwd_acc(r["proj"], r["binned"], r["fwd"], dL, cam, cfg, np.float64, mass=True)
+    brute = 0.0
+    for y in range(H):
+        for x in range(W):
+            brute = brute + np.abs(bwd(_one_pixel(dL, y, x))["g_ray_acc"])
+    assert np.abs(brute).max() > 0
+    np.testing.assert_allclose(m["g_ray_acc"], brute, rtol=1e-10, atol=1e-10 * np.abs(brute).max())
