@@ -225,9 +225,12 @@ int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, cons
  * xpr_project_ray -- shader record p_sd: ray_rec[N,12] = M_c row-major (9), o_c (3); zeros for a culled Gaussian
  *   (tile_count == 0) and for a record that is not finite (C30).  fp32, rule R1.
  * xpr_rasterize_ray_fwd / _bwd -- xpr_rasterize_fwd / _bwd with this evaluation; opacity o_eff is read from
- *   conic_opac[.,3].  bwd ACCUMULATES g_ray_rec[N,12] = dL/dM_c (9), dL/do_c (3), g_opac[N], g_rgb[N,3]
+ *   conic_opac[.,3].  bwd ACCUMULATES g_ray_acc[N,16] (16-byte aligned), g_opac[N], g_rgb[N,3]; g_ray_acc holds the
+ *   record gradient as sums that do not cancel in fp32: with k = -dL/dpower / |d_c|^2, c = o_c x d_c per pixel,
+ *   S_c = sum k c c^T (xx xy xz yy yz zz), D = sum 2 dL/d|d_c|^2 d d^T (same order), sum dL/do_c (3), one unused
+ *   slot; dL/dM_c - dL/do_c p^T = -(S_c - tr(S_c) I) M_c^-T + M_c D exactly
  *   (zero-filled first when zero_init != 0).
- * xpr_ray_bwd -- chain rule from g_ray_rec to (mu, s, q), fp64 inside; ADDS to g_means[N,3], g_scales[N,3],
+ * xpr_ray_bwd -- chain rule from g_ray_acc to (mu, s, q), fp64 inside; ADDS to g_means[N,3], g_scales[N,3],
  *   g_quats[N,4] (call it after xpr_project_bwd, which is given zero g_mean2d / g_conic: the footprint carries
  *   no gradient, the opacity factor and the colour do).
  */
@@ -246,9 +249,9 @@ int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config* cfg, int6
                               const float* conic_opac, const float* rgb, const float* lnv, const float* pixel_rays,
                               const uint32_t* vals_sorted, const uint32_t* tile_ranges,
                               const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
-                              float* g_ray_rec, float* g_opac, float* g_rgb, int32_t zero_init, void* stream);
+                              float* g_ray_acc, float* g_opac, float* g_rgb, int32_t zero_init, void* stream);
 int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const float* quats,
-                    const xpr_camera* cam, const uint32_t* tile_count, const float* g_ray_rec,
+                    const xpr_camera* cam, const uint32_t* tile_count, const float* g_ray_acc,
                     float* g_means, float* g_scales, float* g_quats, void* stream);
 
 /*

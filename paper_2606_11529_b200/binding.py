@@ -235,19 +235,19 @@ def xpr_rasterize_ray_stats(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac,
 
 
 def xpr_rasterize_ray_bwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, pixel_rays, vals_sorted,
-                          tile_ranges, final_T, n_contrib, dL_dimage, g_ray_rec, g_opac, g_rgb, zero_init: bool = True,
+                          tile_ranges, final_T, n_contrib, dL_dimage, g_ray_acc, g_opac, g_rgb, zero_init: bool = True,
                           stream=None):
     N = int(ray_rec.shape[0])
     _check(lib().xpr_rasterize_ray_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec, _F32), _p(conic_opac, _F32), _p(rgb, _F32),
                                        _p(lnv, _F32), _p(pixel_rays, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32),
-                                       _p(n_contrib, _I32), _p(dL_dimage, _F32), _p(g_ray_rec, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
+                                       _p(n_contrib, _I32), _p(dL_dimage, _F32), _p(g_ray_acc, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
                                        C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_ray_bwd")
 
 
-def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_rec, g_means, g_scales, g_quats, stream=None):
+def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_acc, g_means, g_scales, g_quats, stream=None):
     N = int(means.shape[0])
     _check(lib().xpr_ray_bwd(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), C.byref(cam), _p(tile_count, _I32),
-                             _p(g_ray_rec, _F32), _p(g_means, _F32), _p(g_scales, _F32), _p(g_quats, _F32), _stream(stream)), "xpr_ray_bwd")
+                             _p(g_ray_acc, _F32), _p(g_means, _F32), _p(g_scales, _F32), _p(g_quats, _F32), _stream(stream)), "xpr_ray_bwd")
 
 
 # ---- Rendered depth and accumulated opacity (xpr.h) --------------------------------------------

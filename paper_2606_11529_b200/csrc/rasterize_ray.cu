@@ -210,11 +210,34 @@ __device__ __forceinline__ float warp_reduce8(const float* v, int lane) {
     return y;
 }
 
-// Backward (a9 with the f2 evaluation).  A thread owns PPT consecutive pixels of a row and sums their 16 gradient
-// terms per entry in registers (dL/dM_c 9, dL/do_c 3, dL/do 1, dL/drgb 3); two transposed butterflies leave the
-// warp totals spread over the lanes, which issue two RED instructions each.  With g_p = dL/dpower:
-//   dL/dc = -(g_p/dd) c,  dL/ddd = -g_p power/dd,  dL/dd_c = dL/dc x o_c + 2 dL/ddd d_c,  dL/do_c = d_c x dL/dc,
-//   dL/dM_c = dL/dd_c d^T.
+// Backward (a9 with the f2 evaluation).  A thread owns PPT consecutive pixels of a row and sums their 19 gradient
+// terms per entry in registers; two transposed butterflies of 8 and one of 4 leave the warp totals spread over the
+// lanes, which issue the RED instructions.  With g_p = dL/dpower, k = -g_p / dd:
+//   dL/dc = k c,  dL/ddd = -g_p power/dd = k power,  dL/do_c = d_c x dL/dc.
+// The record gradient is accumulated in a form that does not cancel: the plain sums (dL/dM_c = dL/dd_c d^T, dL/do_c)
+// enter the chain rule only as dL/dM_c - dL/do_c p^T, whose two parts nearly cancel (a ray through the centre has
+// c = 0) -- in fp32 that lost the small components of the scale and quaternion gradients.  With o_c = -M_c p,
+// d_c = M_c d, c = o_c x d_c the difference is exactly  -(S_c - tr(S_c) I) M_c^-T + M_c D  with
+//   S_c = sum k c c^T (6),   D = sum 2 dL/ddd d d^T (6),
+// so the kernel sums g_ray_acc[N,16] = (S_c: xx xy xz yy yz zz | D: xx xy xz yy yz zz | sum dL/do_c (3) | unused) and
+// xpr_ray_bwd applies M_c once per Gaussian in fp64.
+// Transposed butterfly of 4 values (6 shuffles): lane L with (L & 7) == 0 holds the total of value L >> 3.
+__device__ __forceinline__ float warp_reduce4(const float* v, int lane) {
+    const bool b4 = lane & 16, b3 = lane & 8;
+    float w[2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const float send = b4 ? v[i] : v[i + 2], keep = b4 ? v[i + 2] : v[i];
+        w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+    const float send = b3 ? w[0] : w[1], keep = b3 ? w[1] : w[0];
+    float y = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    y += __shfl_xor_sync(0xffffffffu, y, 4);
+    y += __shfl_xor_sync(0xffffffffu, y, 2);
+    y += __shfl_xor_sync(0xffffffffu, y, 1);
+    return y;
+}
+
 #ifndef XPR_RAY_BWD_PPT
 #define XPR_RAY_BWD_PPT 4
 #endif
@@ -227,7 +250,7 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                          const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ rays,
                          const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                          const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
-                         const float* __restrict__ dL, float* __restrict__ g_rec, float* __restrict__ g_opac,
+                         const float* __restrict__ dL, float* __restrict__ g_acc, float* __restrict__ g_opac,
                          float* __restrict__ g_rgb) {
     constexpr int THREADS = BLOCK / PPT, BATCH = THREADS;
     __shared__ float4 s_geo[3 * BATCH];
@@ -269,11 +292,10 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
 #pragma unroll
     for (int w = 0; w < THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
 
-    // lane 4 i owns value i of butterfly A (dL/dM_c[0..8)) and value i of butterfly B (dL/dM_c[8], dL/do_c, dL/do, rgb)
+    // lane 4 i owns value i of butterfly A (g_acc[0..8): S_c, D_xx, D_xy) and value i of butterfly B (g_acc[8..15):
+    // D_xz .. D_zz, sum dL/do_c; value 7: dL/do); lane 8 i owns colour channel i of the 4-value butterfly
     const int vi = lane >> 2;
     const bool red_lane = (lane & 3) == 0;
-    float* const baseB = (vi < 4) ? (g_rec + 8 + vi) : (vi == 4) ? g_opac : (g_rgb + (vi - 5));
-    const uint32_t strideB = (vi < 4) ? 12u : (vi == 4) ? 1u : 3u;
 
     for (uint32_t hi = max_n; hi > 0;) {
         const uint32_t cnt = min((uint32_t)BATCH, hi);
@@ -304,10 +326,10 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             }
             if (!__any_sync(0xffffffffu, any_c)) continue;
             const float4 c = s_col[j];
-            const float o0 = r2.y, o1 = r2.z, o2 = r2.w;
-            float va[8], vb[8];
+            float va[8], vb[8], vc[4];
 #pragma unroll
             for (int i = 0; i < 8; ++i) va[i] = vb[i] = 0.f;
+            vc[0] = vc[1] = vc[2] = vc[3] = 0.f;
 #pragma unroll
             for (int k = 0; k < PPT; ++k) {
                 // a pixel that does not contribute enters with 1/dd = 0 and o G = 0: every term vanishes
@@ -318,34 +340,37 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                 const float inv = rcp_approx(1.0f - alpha);
                 T[k] = T[k] * inv;                     // transmittance in front of this entry
                 const float w = alpha * T[k];
-                vb[5] = fmaf(w, g0[k], vb[5]); vb[6] = fmaf(w, g1[k], vb[6]); vb[7] = fmaf(w, g2[k], vb[7]);
+                vc[0] = fmaf(w, g0[k], vc[0]); vc[1] = fmaf(w, g1[k], vc[1]); vc[2] = fmaf(w, g2[k], vc[2]);
                 const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
                 const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
                 Q[k] = fmaf(gc, w, Q[k]);
                 const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
                 const float gp = og * live;            // dL/dpower; dL/do = gp / o, divided once per warp below
-                vb[4] += gp;
+                vb[7] += gp;
                 const float k1 = -gp * rdd;            // dL/dc = k1 c
                 const float gc0 = k1 * e[k].c0, gc1 = k1 * e[k].c1, gc2 = k1 * e[k].c2;
-                const float gdd2 = 2.0f * k1 * power;  // 2 dL/ddd
-                const float gd0 = fmaf(gdd2, e[k].dc0, fmaf(gc1, o2, -(gc2 * o1)));
-                const float gd1 = fmaf(gdd2, e[k].dc1, fmaf(gc2, o0, -(gc0 * o2)));
-                const float gd2 = fmaf(gdd2, e[k].dc2, fmaf(gc0, o1, -(gc1 * o0)));
-                vb[1] += fmaf(e[k].dc1, gc2, -(e[k].dc2 * gc1));     // dL/do_c = d_c x dL/dc
-                vb[2] += fmaf(e[k].dc2, gc0, -(e[k].dc0 * gc2));
-                vb[3] += fmaf(e[k].dc0, gc1, -(e[k].dc1 * gc0));
-                va[0] = fmaf(gd0, d0[k], va[0]); va[1] = fmaf(gd0, d1[k], va[1]); va[2] = fmaf(gd0, d2[k], va[2]);
-                va[3] = fmaf(gd1, d0[k], va[3]); va[4] = fmaf(gd1, d1[k], va[4]); va[5] = fmaf(gd1, d2[k], va[5]);
-                va[6] = fmaf(gd2, d0[k], va[6]); va[7] = fmaf(gd2, d1[k], va[7]); vb[0] = fmaf(gd2, d2[k], vb[0]);
+                // S_c += k1 c c^T
+                va[0] = fmaf(gc0, e[k].c0, va[0]); va[1] = fmaf(gc0, e[k].c1, va[1]); va[2] = fmaf(gc0, e[k].c2, va[2]);
+                va[3] = fmaf(gc1, e[k].c1, va[3]); va[4] = fmaf(gc1, e[k].c2, va[4]); va[5] = fmaf(gc2, e[k].c2, va[5]);
+                // D += 2 dL/ddd d d^T,  2 dL/ddd = 2 k1 power
+                const float gdd2 = 2.0f * k1 * power;
+                const float t0 = gdd2 * d0[k], t1 = gdd2 * d1[k], t2 = gdd2 * d2[k];
+                va[6] = fmaf(t0, d0[k], va[6]); va[7] = fmaf(t0, d1[k], va[7]); vb[0] = fmaf(t0, d2[k], vb[0]);
+                vb[1] = fmaf(t1, d1[k], vb[1]); vb[2] = fmaf(t1, d2[k], vb[2]); vb[3] = fmaf(t2, d2[k], vb[3]);
+                vb[4] += fmaf(e[k].dc1, gc2, -(e[k].dc2 * gc1));     // dL/do_c = d_c x dL/dc
+                vb[5] += fmaf(e[k].dc2, gc0, -(e[k].dc0 * gc2));
+                vb[6] += fmaf(e[k].dc0, gc1, -(e[k].dc1 * gc0));
             }
             const float ta = warp_reduce8(va, lane);
             float tb = warp_reduce8(vb, lane);
+            const float tc = warp_reduce4(vc, lane);
+            const uint32_t g = __float_as_uint(ga.w);
             if (red_lane) {
-                const uint32_t g = __float_as_uint(ga.w);
-                if (vi == 4) tb *= rcp_approx(ga.y);   // dL/do = (sum g_p) / o
-                atomicAdd(g_rec + 12 * (size_t)g + vi, ta);
-                atomicAdd(baseB + (size_t)strideB * g, tb);
+                atomicAdd(g_acc + 16 * (size_t)g + vi, ta);
+                if (vi == 7) atomicAdd(g_opac + g, tb * rcp_approx(ga.y));   // dL/do = (sum g_p) / o
+                else atomicAdd(g_acc + 16 * (size_t)g + 8 + vi, tb);
             }
+            if ((lane & 7) == 0 && lane < 24) atomicAdd(g_rgb + 3 * (size_t)g + (lane >> 3), tc);
         }
         hi -= cnt;
     }
@@ -426,7 +451,7 @@ extern "C" int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config
                                          const float* conic_opac, const float* rgb, const float* lnv,
                                          const float* pixel_rays, const uint32_t* vals_sorted,
                                          const uint32_t* tile_ranges, const float* final_T, const uint32_t* n_contrib,
-                                         const float* dL_dimage, float* g_ray_rec, float* g_opac, float* g_rgb,
+                                         const float* dL_dimage, float* g_ray_acc, float* g_opac, float* g_rgb,
                                          int32_t zero_init, void* stream) {
     if (int32_t s = check_ray_cam_cfg(cam, cfg)) return s;
     if (N < 0) return XPR_ERR_INVALID_ARG;
@@ -435,15 +460,15 @@ extern "C" int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config
         return XPR_ERR_INVALID_ARG;
     if (N == 0) return XPR_OK;
     if (!aligned(ray_rec, 16) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-        !aligned(vals_sorted, 4) || !aligned(g_ray_rec, 4) || !aligned(g_opac, 4) || !aligned(g_rgb, 4))
+        !aligned(vals_sorted, 4) || !aligned(g_ray_acc, 16) || !aligned(g_opac, 4) || !aligned(g_rgb, 4))
         return XPR_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     if (zero_init) {
         const size_t n = (size_t)N;
-        if (g_opac == g_ray_rec + 12 * n && g_rgb == g_opac + n) {
-            XPR_CUDA(cudaMemsetAsync(g_ray_rec, 0, sizeof(float) * 16 * n, st));     // one allocation: one fill
+        if (g_opac == g_ray_acc + 16 * n && g_rgb == g_opac + n) {
+            XPR_CUDA(cudaMemsetAsync(g_ray_acc, 0, sizeof(float) * 20 * n, st));     // one allocation: one fill
         } else {
-            XPR_CUDA(cudaMemsetAsync(g_ray_rec, 0, sizeof(float) * 12 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_ray_acc, 0, sizeof(float) * 16 * n, st));
             XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
             XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
         }
@@ -454,7 +479,7 @@ extern "C" int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config
 #define XPR_RAY_BWD(PPT_)                                                                                           \
     rasterize_ray_bwd_kernel<PPT_><<<T, BLOCK / PPT_, 0, st>>>(                                                     \
         P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays, \
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_ray_rec, g_opac,  \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_ray_acc, g_opac,  \
         g_rgb)
     // more pixels per thread amortise the per-entry reduction (throughput shape); fewer give a heavy tile more warps
     if (T >= XPR_RAY_FWD_PPT2_MIN_TILES) XPR_RAY_BWD(XPR_RAY_BWD_PPT);

@@ -118,21 +118,22 @@ project_ray_kernel(int64_t N, RayCam C, const float* __restrict__ means, const f
 }
 
 // Chain rule record -> (mu, s, q), fp64 on the forward intermediates recomputed in fp32:
-//   Gt = dL/dM_c - dL/do_c p^T;  dL/dp = -M_c^T dL/do_c;  dL/dmu = W^T dL/dp;
+//   Gt = dL/dM_c - dL/do_c p^T, formed from the accumulators S_c, D of xpr_rasterize_ray_bwd;
+//   dL/dp = -M_c^T dL/do_c;  dL/dmu = W^T dL/dp;
 //   dL/d(WR)[j][i] = Gt[i][j] / s_i;  dL/ds_i = -sum_j Gt[i][j] M_c[i][j] / s_i;  dL/dR = W^T dL/d(WR);  R(q) (C17).
 __global__ void __launch_bounds__(128)
 ray_bwd_kernel(int64_t N, RayCam C, const float* __restrict__ means, const float* __restrict__ scales,
                const float4* __restrict__ quats, const uint32_t* __restrict__ tile_count,
-               const float4* __restrict__ g_rec, float* __restrict__ g_means, float* __restrict__ g_scales,
+               const float4* __restrict__ g_acc, float* __restrict__ g_means, float* __restrict__ g_scales,
                float4* __restrict__ g_quats) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     if (tile_count[i] == 0) return;
-    const float4 a0 = g_rec[3 * i], a1 = g_rec[3 * i + 1], a2 = g_rec[3 * i + 2];
-    const double g[12] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w, a2.x, a2.y, a2.z, a2.w};
+    const float4 a0 = g_acc[4 * i], a1 = g_acc[4 * i + 1], a2 = g_acc[4 * i + 2], a3 = g_acc[4 * i + 3];
+    const double g[15] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w, a2.x, a2.y, a2.z, a2.w, a3.x, a3.y, a3.z};
     bool any = false;
 #pragma unroll
-    for (int k = 0; k < 12; ++k) any = any || (g[k] != 0.0);
+    for (int k = 0; k < 15; ++k) any = any || (g[k] != 0.0);
     if (!any) return;
     const float mu[3] = {means[3 * i], means[3 * i + 1], means[3 * i + 2]};
     const float sc[3] = {scales[3 * i], scales[3 * i + 1], scales[3 * i + 2]};
@@ -140,13 +141,35 @@ ray_bwd_kernel(int64_t N, RayCam C, const float* __restrict__ means, const float
     const float q[4] = {qv.x, qv.y, qv.z, qv.w};
     RayFwd F;
     ray_record(C, mu, sc, q, F);
+    // dL/dM_c - dL/do_c p^T = -(S_c - tr(S_c) I) M_c^-T + M_c D  (rasterize_ray.cu), M_c^-T = cofactors / determinant
+    // (the quaternion is not renormalised, C3, so W R need not be orthogonal)
+    double M[9], MiT[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) M[k] = (double)F.Mc[k];
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const int a1i = (a + 1) % 3, a2i = (a + 2) % 3, b1i = (b + 1) % 3, b2i = (b + 2) % 3;
+            MiT[3 * a + b] = M[3 * a1i + b1i] * M[3 * a2i + b2i] - M[3 * a1i + b2i] * M[3 * a2i + b1i];
+        }
+    const double rdet = 1.0 / (M[0] * MiT[0] + M[1] * MiT[1] + M[2] * MiT[2]);
+    const double Sc[9] = {g[0], g[1], g[2], g[1], g[3], g[4], g[2], g[4], g[5]};
+    const double D[9] = {g[6], g[7], g[8], g[7], g[9], g[10], g[8], g[10], g[11]};
+    const double tr = g[0] + g[3] + g[5];
     double Gt[9], gp[3] = {0.0, 0.0, 0.0};
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            Gt[3 * a + b] = g[3 * a + b] - g[9 + a] * (double)F.p[b];
-            gp[b] -= (double)F.Mc[3 * a + b] * g[9 + a];
+            double u = 0.0, v = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                u += (Sc[3 * a + k] - (a == k ? tr : 0.0)) * MiT[3 * k + b];
+                v += M[3 * a + k] * D[3 * k + b];
+            }
+            Gt[3 * a + b] = v - u * rdet;
+            gp[b] -= M[3 * a + b] * g[12 + a];
         }
     double W[9];
 #pragma unroll
@@ -222,19 +245,19 @@ extern "C" int32_t xpr_project_ray(int64_t N, const float* means, const float* s
 }
 
 extern "C" int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const float* quats,
-                               const xpr_camera* cam, const uint32_t* tile_count, const float* g_ray_rec,
+                               const xpr_camera* cam, const uint32_t* tile_count, const float* g_ray_acc,
                                float* g_means, float* g_scales, float* g_quats, void* stream) {
     if (int32_t s = check_cam(cam)) return s;
     if (N < 0 || N > 0x7fffffffLL) return XPR_ERR_INVALID_ARG;
     if (N == 0) return XPR_OK;
     if (!aligned(means, 4) || !aligned(scales, 4) || !aligned(quats, 16) || !aligned(tile_count, 4) ||
-        !aligned(g_ray_rec, 16) || !aligned(g_means, 4) || !aligned(g_scales, 4) || !aligned(g_quats, 16))
+        !aligned(g_ray_acc, 16) || !aligned(g_means, 4) || !aligned(g_scales, 4) || !aligned(g_quats, 16))
         return XPR_ERR_INVALID_ARG;
     RayCam C;
     make_ray_cam(cam, C);
     ray_bwd_kernel<<<(unsigned)((N + 127) / 128), 128, 0, (cudaStream_t)stream>>>(
         N, C, means, scales, reinterpret_cast<const float4*>(quats), tile_count,
-        reinterpret_cast<const float4*>(g_ray_rec), g_means, g_scales, reinterpret_cast<float4*>(g_quats));
+        reinterpret_cast<const float4*>(g_ray_acc), g_means, g_scales, reinterpret_cast<float4*>(g_quats));
     XPR_LAUNCH_CHECK();
     return XPR_OK;
 }

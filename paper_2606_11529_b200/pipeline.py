@@ -70,9 +70,9 @@ class SplatPipeline:
         self.g_opacities, self.g_sh = e(N), e(N, self.K, 3)
         if self.ray_eval:   # f2: shader record, per-pixel rays, record gradient
             self.ray_rec = e(N, 12)
-            g3 = e(16 * N)                                 # g_ray_rec | g_opac | g_rgb: one memset in xpr_rasterize_ray_bwd
-            self.g_ray_rec = g3[:12 * N].view(N, 12)
-            self.g_opac, self.g_rgb = g3[12 * N:13 * N], g3[13 * N:].view(N, 3)
+            g3 = e(20 * N)                                 # g_ray_acc | g_opac | g_rgb: one memset in xpr_rasterize_ray_bwd
+            self.g_ray_acc = g3[:16 * N].view(N, 16)
+            self.g_opac, self.g_rgb = g3[16 * N:17 * N], g3[17 * N:].view(N, 3)
             self.pixel_rays = e(self.H, self.W, 3)
             self.pixel_info()
             self.g_mean2d.zero_(); self.g_conic.zero_()    # the footprint carries no gradient
@@ -174,7 +174,7 @@ class SplatPipeline:
         if self.ray_eval:
             xb.xpr_rasterize_ray_bwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv,
                                      self.pixel_rays, self.vals_sorted, self.tile_ranges, self.final_T, self.n_contrib,
-                                     dL_dimage, self.g_ray_rec, self.g_opac, self.g_rgb, zero_init=True)
+                                     dL_dimage, self.g_ray_acc, self.g_opac, self.g_rgb, zero_init=True)
             return
         xb.xpr_rasterize_bwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.final_T,
                              self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb,
@@ -210,7 +210,7 @@ class SplatPipeline:
                            self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb, self.g_means, self.g_scales,
                            self.g_quats, self.g_opacities, self.g_sh)
         if self.ray_eval:
-            xb.xpr_ray_bwd(means, scales, quats, self.cam, self.tile_count, self.g_ray_rec, self.g_means,
+            xb.xpr_ray_bwd(means, scales, quats, self.cam, self.tile_count, self.g_ray_acc, self.g_means,
                            self.g_scales, self.g_quats)
         if getattr(self, "_feat_bwd", False):
             xb.xpr_depth_bwd(self.cam, self.tile_count, self.g_depth, self.g_means)

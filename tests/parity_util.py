@@ -49,7 +49,7 @@ def run_gpu_backward(g, dL_np):
     torch.cuda.synchronize()
     names = ("g_mean2d", "g_conic", "g_opac", "g_rgb", "g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
     if pipe.ray_eval:
-        names = names + ("g_ray_rec",)
+        names = names + ("g_ray_acc",)
     return {k: getattr(pipe, k).cpu().numpy() for k in names}
 
 

@@ -22,6 +22,9 @@ pytestmark = pytest.mark.gpu
 PARAMS = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
 
 
+E2E_STATS = []      # (scene, N, end-to-end violators, elements) of every case run, printed by the last test
+
+
 def ray_parity(scene, view=0, cfg_over=None):
     over = dict(cfg_over or {}, ray_eval=1)
     g = pu.run_gpu(scene, view, over)
@@ -44,21 +47,24 @@ def ray_parity(scene, view=0, cfg_over=None):
     dL = np.where(frag[..., None], 0.0, dL).astype(np.float32)
     og = xo.backward_ray(o["arrays"], o, dL, o["cam"], o["cfg"], np.float32)
     gg = pu.run_gpu_backward(g, dL)
-    mass = xo.rasterize_ray_bwd(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32, mass=True)
+    # stage 1: the record gradient in the accumulator form the kernel sums (S_c, D, sum dL/do_c: xpr.h; the oracle's
+    # accumulator route is pinned equal to its plain route, P14f), opacity and colour -- every element
+    oa = xo.rasterize_ray_bwd_acc(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32)
+    mass = xo.rasterize_ray_bwd_acc(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32, mass=True)
     n_plain = 0
-    for kg, ko in (("g_ray_rec", "g_ray_rec"), ("g_opac", "g_opac_eff"), ("g_rgb", "g_rgb")):   # stage 1
-        bad, err = pu.grad_violations(gg[kg], og[ko], mass[ko])
+    for kg, ko in (("g_ray_acc", "g_ray_acc"), ("g_opac", "g_opac_eff"), ("g_rgb", "g_rgb")):
+        bad, err = pu.grad_violations(gg[kg], oa[ko], mass[ko])
         assert bad.sum() == 0, f"{kg}: {bad.sum()} of {bad.size} outside tolerance, max err {err.max()}"
-        n_plain += int(pu.grad_violations(gg[kg], og[ko])[0].sum())
-    assert n_plain <= max(4, 2e-4 * 16 * scene.N), n_plain
+        n_plain += int(pu.grad_violations(gg[kg], oa[ko])[0].sum())
+    assert n_plain <= max(4, 2e-4 * 19 * scene.N), n_plain
     assert not np.any(gg["g_mean2d"]) and not np.any(gg["g_conic"])      # the footprint carries no gradient
     # stage 2: the oracle's chain rule fed the GPU's fp32 gradients
     N = scene.N
     gz = dict(g_mean2d=np.zeros((N, 2)), g_conic=np.zeros((N, 3)), g_opac_eff=gg["g_opac"], g_rgb=gg["g_rgb"])
     iso = xo.project_bwd(scene.means, scene.scales, scene.quats, scene.opacities, scene.sh, o["cam"], o["cfg"], gz,
                          np.float32)
-    part = xo.ray_bwd(scene.means, scene.scales, scene.quats, o["proj"]["tile_count"], gg["g_ray_rec"], o["cam"],
-                      np.float32)
+    part = xo.ray_bwd_acc(scene.means, scene.scales, scene.quats, o["proj"]["tile_count"], gg["g_ray_acc"], o["cam"],
+                          np.float32)
     total_bad = total = 0
     for k in PARAMS:
         ref = iso[k] + part[k] if k in part else iso[k]
@@ -73,13 +79,13 @@ def ray_parity(scene, view=0, cfg_over=None):
         if bad_e2e.any():
             r2 = np.asarray(og[k], np.float64).reshape(N, -1)
             group = np.abs(r2).max(axis=1, keepdims=True) * np.ones_like(r2)
-            assert (err_e2e[bad_e2e] <= 2e-2 * group.ravel()[bad_e2e] + 1e-6).all(), k
-    # reported bound: the chain rule forms Gt = dL/dM_c - dL/do_c p^T from two fp32 sums that nearly cancel (a ray
-    # through the centre has c = 0), so scale / quaternion components far below their Gaussian's largest one inherit
-    # the summation floor of stage 1; measured up to 1.0e-3 of all elements on object-like scenes (2D path: 1e-5)
-    assert total_bad <= 5e-3 * total, f"end-to-end violators {total_bad}/{total}"
+            assert (err_e2e[bad_e2e] <= 1e-2 * group.ravel()[bad_e2e] + 1e-6).all(), k
+    # end to end against the oracle's PLAIN route (the definition): the accumulators no longer cancel, so what is left
+    # is the fp32 summation floor of stage 1 on elements far below their Gaussian's largest component (as on the 2D path)
+    E2E_STATS.append((scene.name, scene.N, total_bad, total))
+    assert total_bad <= 1e-3 * total, f"end-to-end violators {total_bad}/{total}"
     culled = o["proj"]["tile_count"] == 0
-    for k in PARAMS + ("g_ray_rec",):
+    for k in PARAMS + ("g_ray_acc",):
         assert not np.any(gg[k][culled])
     return g, o
 
@@ -172,3 +178,9 @@ def test_ray_pixel_rays_depend_on_the_intrinsics_only():
     b = pu.run_gpu(sc, 1, dict(ray_eval=1))["proj"]["pixel_rays"]
     np.testing.assert_array_equal(a, b)
     np.testing.assert_allclose(np.linalg.norm(a.astype(np.float64), axis=-1), 1.0, atol=2e-7)
+
+
+def test_zz_report_end_to_end_violators(capsys):
+    with capsys.disabled():
+        for name, n, bad, tot in E2E_STATS:
+            print(f"\n[f2 end to end] {name} N={n}: {bad} of {tot} elements outside 1e-3 rel + 1e-6 abs ({bad / max(tot, 1):.2e})", end="")
