@@ -455,7 +455,10 @@ void rasterize_fwd_strict(const xo_camera* cam, const xo_config* cfg, int64_t N,
 // MASS = true accumulates |addend| instead of the addend: the "mass" sum_pixels |term| of every
 // gradient element, i.e. the scale an fp32 sum of those terms is conditioned on (used only to
 // derive the cancellation-aware part of the gradient tolerance).
-template <class S, bool MASS = false>
+// ACC = float: every sum of this function (per list position over the tile's pixels, then over the tiles) is kept in
+// fp32 instead of fp64, in this function's fixed order -- what a careful fp32 CPU implementation would return.  Used
+// only to put the GPU's fp32 summation error beside that of a CPU fp32 sum (tests/test_gpu_parity.py).
+template <class S, bool MASS = false, class ACC = double>
 void rasterize_bwd(const xo_camera* cam, const xo_config* cfg, int64_t N, const S* mean2d, const S* conic, const S* opac,
                    const S* rgb, const S* lnv, const uint32_t* vals, const uint32_t* ranges, const uint32_t* n_contrib,
                    const S* dL, double* g_mean2d, double* g_conic, double* g_opac, double* g_rgb) {
@@ -468,7 +471,7 @@ void rasterize_bwd(const xo_camera* cam, const xo_config* cfg, int64_t N, const 
         const int tx = t % TW, ty = t / TW;
         const uint32_t b = ranges[2 * t], e = ranges[2 * t + 1];
         if (e <= b) continue;
-        std::vector<double> acc((size_t)(e - b) * 9, 0.0);   // per list position: m(2) conic(3) o(1) rgb(3)
+        std::vector<ACC> acc((size_t)(e - b) * 9, ACC(0));   // per list position: m(2) conic(3) o(1) rgb(3)
         std::vector<Contrib<S>> rec;
         for (int py = ty * ts; py < std::min(H, (ty + 1) * ts); ++py)
             for (int px = tx * ts; px < std::min(W, (tx + 1) * ts); ++px) {
@@ -482,11 +485,11 @@ void rasterize_bwd(const xo_camera* cam, const xo_config* cfg, int64_t N, const 
                 for (size_t r = rec.size(); r-- > 0;) {
                     const Contrib<S>& q = rec[r];
                     const double al = (double)q.alpha, Tk = (double)q.T;
-                    double* a9 = &acc[(size_t)q.pos * 9];
+                    ACC* a9 = &acc[(size_t)q.pos * 9];
                     double dalpha = 0.0;
                     for (int ch = 0; ch < 3; ++ch) {
                         const double ck = (double)rgb[3 * q.g + ch];
-                        a9[6 + ch] += MASS ? std::fabs(al * Tk * g[ch]) : al * Tk * g[ch];
+                        a9[6 + ch] += ACC(MASS ? std::fabs(al * Tk * g[ch]) : al * Tk * g[ch]);
                         dalpha += g[ch] * (ck * Tk - Sb[ch] / (1.0 - al));
                     }
                     for (int ch = 0; ch < 3; ++ch) Sb[ch] += (double)rgb[3 * q.g + ch] * al * Tk;
@@ -497,15 +500,26 @@ void rasterize_bwd(const xo_camera* cam, const xo_config* cfg, int64_t N, const 
                     const double dx = (double)q.dx, dy = (double)q.dy;
                     const double add[6] = {(A * dx + B * dy) * dpow, (B * dx + C * dy) * dpow,   // d power / d m = A dx + B dy, ..
                                            -0.5 * dx * dx * dpow, -dx * dy * dpow, -0.5 * dy * dy * dpow, G * dalpha};
-                    for (int j = 0; j < 6; ++j) a9[j] += MASS ? std::fabs(add[j]) : add[j];
+                    for (int j = 0; j < 6; ++j) a9[j] += ACC(MASS ? std::fabs(add[j]) : add[j]);
                 }
             }
         for (uint32_t k = 0; k < e - b; ++k) {
             const uint32_t gi = vals[b + k];
-            const double* a9 = &acc[(size_t)k * 9];
+            const ACC* a9 = &acc[(size_t)k * 9];
             bool any = false;
-            for (int j = 0; j < 9; ++j) any |= (a9[j] != 0.0);
+            for (int j = 0; j < 9; ++j) any |= (a9[j] != ACC(0));
             if (!any) continue;
+            if (sizeof(ACC) == 4) {   // fp32 sum over the tiles too, serialised (order = whichever tile arrives first)
+#pragma omp critical(xo_acc32)
+                {
+                    g_mean2d[2 * gi] = (double)((float)g_mean2d[2 * gi] + (float)a9[0]);
+                    g_mean2d[2 * gi + 1] = (double)((float)g_mean2d[2 * gi + 1] + (float)a9[1]);
+                    for (int j = 0; j < 3; ++j) g_conic[3 * gi + j] = (double)((float)g_conic[3 * gi + j] + (float)a9[2 + j]);
+                    g_opac[gi] = (double)((float)g_opac[gi] + (float)a9[5]);
+                    for (int j = 0; j < 3; ++j) g_rgb[3 * gi + j] = (double)((float)g_rgb[3 * gi + j] + (float)a9[6 + j]);
+                }
+                continue;
+            }
 #pragma omp atomic
             g_mean2d[2 * gi] += a9[0];
 #pragma omp atomic
@@ -701,6 +715,14 @@ inline uint32_t float_bits(float f) { uint32_t u; std::memcpy(&u, &f, 4); return
         double* g_rgb) {                                                                                            \
         rasterize_bwd<T, true>(cam, cfg, N, mean2d, conic, opac_eff, rgb, lnv, vals_sorted, tile_ranges, n_contrib, \
                                dL_dimage, g_mean2d, g_conic, g_opac_eff, g_rgb);                                    \
+    }                                                                                                               \
+    extern "C" void xpr_oracle_rasterize_bwd_acc32_##SFX(                                                           \
+        const xo_camera* cam, const xo_config* cfg, int64_t N, const T* mean2d, const T* conic, const T* opac_eff,  \
+        const T* rgb, const T* lnv, const uint32_t* vals_sorted, const uint32_t* tile_ranges,                       \
+        const uint32_t* n_contrib, const T* dL_dimage, double* g_mean2d, double* g_conic, double* g_opac_eff,       \
+        double* g_rgb) {                                                                                            \
+        rasterize_bwd<T, false, float>(cam, cfg, N, mean2d, conic, opac_eff, rgb, lnv, vals_sorted, tile_ranges,    \
+                                       n_contrib, dL_dimage, g_mean2d, g_conic, g_opac_eff, g_rgb);                 \
     }                                                                                                               \
     extern "C" void xpr_oracle_project_bwd_##SFX(                                                                   \
         int64_t N, const T* means, const T* scales, const T* quats, const T* opacities, const T* sh,                \

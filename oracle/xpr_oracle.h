@@ -83,6 +83,13 @@ enum { XO_FRAG_EXIT = 1, XO_FRAG_CLAMP = 2, XO_FRAG_GATE = 4 };
                                       const uint32_t* tile_ranges, const uint32_t* n_contrib,           \
                                       const T* dL_dimage, double* g_mean2d, double* g_conic,            \
                                       double* g_opac_eff, double* g_rgb);                               \
+    /* Same loop with every sum kept in fp32 (a CPU fp32 implementation; reported beside the GPU) */ \
+    void xpr_oracle_rasterize_bwd_acc32_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,      \
+                                      const T* mean2d, const T* conic, const T* opac_eff, const T* rgb, \
+                                      const T* lnv, const uint32_t* vals_sorted,                        \
+                                      const uint32_t* tile_ranges, const uint32_t* n_contrib,           \
+                                      const T* dL_dimage, double* g_mean2d, double* g_conic,            \
+                                      double* g_opac_eff, double* g_rgb);                               \
     /* Same loop with |addend| accumulated: per-element mass sum_pixels |term| (tolerance scale only). */ \
     void xpr_oracle_rasterize_bwd_mass_##S(const xo_camera* cam, const xo_config* cfg, int64_t N,       \
                                       const T* mean2d, const T* conic, const T* opac_eff, const T* rgb, \

@@ -188,14 +188,17 @@ def rasterize_fwd_strict(proj: dict, cam: XoCamera, cfg: XoConfig, dtype=np.floa
 
 
 def rasterize_bwd(proj: dict, binned: dict, fwd: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32,
-                  mass: bool = False) -> dict:
+                  mass: bool = False, acc32: bool = False) -> dict:
+    """acc32: every sum kept in fp32 (what a CPU fp32 implementation returns; only to put the GPU's summation error
+    beside it)."""
     dt = np.dtype(dtype)
     N = int(proj["tile_count"].shape[0])
     a = [np.ascontiguousarray(proj[k], dt) for k in ("mean2d", "conic", "opac_eff", "rgb", "lnv")]
     dL = np.ascontiguousarray(dL_dimage, dt)
     out = dict(g_mean2d=np.empty((N, 2), np.float64), g_conic=np.empty((N, 3), np.float64),
                g_opac_eff=np.empty(N, np.float64), g_rgb=np.empty((N, 3), np.float64))
-    fn = getattr(lib(), ("xpr_oracle_rasterize_bwd_mass_" if mass else "xpr_oracle_rasterize_bwd_") + _sfx(dt))
+    name = "xpr_oracle_rasterize_bwd_mass_" if mass else "xpr_oracle_rasterize_bwd_acc32_" if acc32 else "xpr_oracle_rasterize_bwd_"
+    fn = getattr(lib(), name + _sfx(dt))
     fn(C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
        _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), _p(dL),
        _p(out["g_mean2d"]), _p(out["g_conic"]), _p(out["g_opac_eff"]), _p(out["g_rgb"]))

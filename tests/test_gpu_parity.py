@@ -7,7 +7,7 @@ Gradient parity is asserted per kernel on identical inputs
            1e-3 |ref| + 1e-6 + 2e-6 * mass (mass = sum_pixels |term|, from the oracle)
   stage 2  xpr_project_bwd    vs oracle project_bwd fed the SAME fp32 2D gradients -> strict
 and the end-to-end composition is reported (its few violators are elements whose value is
-cancelled by the covariance chain rule; they are bounded group-relative: within 2 % of the Gaussian's
+cancelled by the covariance chain rule; they are bounded group-relative: within 1 % of the Gaussian's
 largest component of that gradient -- the chain rule G2 = -K G_K K amplifies the fp32 summation floor of
 stage 1 by the conditioning of K, and which elements are hit depends on the order of the atomics).
 """
@@ -22,6 +22,9 @@ pytestmark = pytest.mark.gpu
 
 PAIRS_2D = (("g_mean2d", "g_mean2d"), ("g_conic", "g_conic"), ("g_opac", "g_opac_eff"), ("g_rgb", "g_rgb"))
 PARAMS = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
+
+
+E2E_STATS = []      # per case: elements outside 1e-3 |ref| + 1e-6 -- 2D stage (GPU, CPU fp32), end to end (GPU, CPU fp32)
 
 
 def full_parity(scene, view=0, cfg_over=None, expect_pairs=True):
@@ -48,7 +51,7 @@ def full_parity(scene, view=0, cfg_over=None, expect_pairs=True):
         n_plain += int(pu.grad_violations(gg[kg], og[ko])[0].sum())
     # without the mass term only cancellation-dominated elements may fail (the oracle's own fp32 and
     # fp64 modes disagree there too): a handful per million
-    assert n_plain <= max(4, 5e-5 * 9 * scene.N), n_plain
+    assert n_plain <= max(4, 2e-6 * 9 * scene.N), n_plain         # measured: 0-2 of 9 M (config 3), 0 of 27 M (config 5)
     g2 = dict(g_mean2d=gg["g_mean2d"], g_conic=gg["g_conic"], g_opac_eff=gg["g_opac"], g_rgb=gg["g_rgb"])
     iso = xo.project_bwd(scene.means, scene.scales, scene.quats, scene.opacities, scene.sh, o["cam"], o["cfg"], g2,
                          np.float32)
@@ -61,8 +64,18 @@ def full_parity(scene, view=0, cfg_over=None, expect_pairs=True):
         if bad_e2e.any():
             ref = np.asarray(og[k], np.float64).reshape(scene.N, -1)
             group = np.abs(ref).max(axis=1, keepdims=True) * np.ones_like(ref)
-            assert (err_e2e[bad_e2e] <= 2e-2 * group.ravel()[bad_e2e] + 1e-6).all(), k
-    assert total_bad <= 1e-3 * total, f"end-to-end violators {total_bad}/{total}"
+            assert (err_e2e[bad_e2e] <= 1e-2 * group.ravel()[bad_e2e] + 1e-6).all(), k
+    assert total_bad <= max(4, 2e-5 * total), f"end-to-end violators {total_bad}/{total}"     # measured <= 4e-6
+    # The same count for a CPU that keeps its sums in fp32 (the oracle's loops with float accumulators, then the same
+    # fp64 chain rule): north_star's bar is met end to end by neither on cancellation-dominated elements, and the GPU
+    # (fp32 registers, shuffles, atomics in arbitrary order) must not be worse than that by more than a small factor
+    c32 = xo.rasterize_bwd(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32, acc32=True)
+    cpu32 = xo.project_bwd(scene.means, scene.scales, scene.quats, scene.opacities, scene.sh, o["cam"], o["cfg"], c32,
+                           np.float32)
+    cpu_bad = sum(int(pu.grad_violations(cpu32[k], og[k])[0].sum()) for k in PARAMS)
+    cpu_plain = sum(int(pu.grad_violations(c32[ko], og[ko])[0].sum()) for _, ko in PAIRS_2D)
+    E2E_STATS.append((scene.name, scene.N, n_plain, cpu_plain, total_bad, cpu_bad, total))
+    assert total_bad <= 3 * cpu_bad + max(4, 2e-5 * total), (total_bad, cpu_bad)
     culled = o["proj"]["tile_count"] == 0
     for k in PARAMS:                                              # P11: a culled Gaussian gets exactly zero
         assert not np.any(gg[k][culled])
@@ -188,3 +201,12 @@ def test_tile_cull_config3_full_size_bench_configuration():
 def test_tile_cull_config5_full_size():
     g, o = full_parity(scenes.make_scene(5), 0, CULL)
     assert o["binned"]["num_pairs"] > 50_000_000
+
+
+def test_zz_report_gradient_violators(capsys):
+    """Prints, for every case of this file, how many gradient elements miss north_star's plain bar 1e-3 |ref| + 1e-6 on
+    the GPU and for a CPU fp32 sum of the same terms (DESIGN.md 5 quotes these numbers)."""
+    with capsys.disabled():
+        for name, n, g1, c1, g2, c2, tot in E2E_STATS:
+            print(f"\n[2D gradients] {name} N={n}: compositing stage GPU {g1} / CPU-fp32 {c1} of {9 * n}; "
+                  f"end to end GPU {g2} / CPU-fp32 {c2} of {tot}", end="")
