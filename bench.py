@@ -40,6 +40,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--no-plain", action="store_true", help="skip the extra timing of the plain path (tile_cull 0)")
     ap.add_argument("--tile-cull", type=int, default=1, choices=(0, 1),
                     help="1: binning with the paper's tile_cull (XPR-3DGS, PAPER L149/L268-281; same image); "
                          "0: rectangle overlap only")
@@ -300,6 +301,9 @@ def run_ours(args):
     total_ms = max_over_ranks(float(sum(step_ms)), world, dev)
     ms = total_ms / args.steps
     stage_ms = {n: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in all_events])) for i, n in enumerate(stage_names)}
+    stage_ms_median = {n: float(np.median([e[i].elapsed_time(e[i + 1]) for e in all_events])) for i, n in enumerate(stage_names)}
+    step_stats = {"mean": float(np.mean(step_ms)), "median": float(np.median(step_ms)), "min": float(np.min(step_ms)),
+                  "max": float(np.max(step_ms)), "note": "this rank's K timed steps, CUDA events; ms_per_step is the mean, max over ranks"}
     mp = cam.width * cam.height / 1e6
     value = aggregate_value(world, mp, ms)
 
@@ -354,11 +358,48 @@ def run_ours(args):
         pass
     for name, r in rooflines.items():
         r["frac"] = r["achieved"] / r["peak"]
+        if r["bound"] == "hbm":
+            r["frac_of_nominal_8TBs"] = r["achieved"] / 8000.0
         r["traffic"] = traffic.get(name)
+        r["traffic_source"] = ("profiles/ncu_traffic.csv (dram__bytes_read.sum + dram__bytes_write.sum of a committed ncu --set full "
+                               "capture of this workload, see profiles/ncu_traffic.md; not measured by this run)"
+                               if traffic.get(name) is not None else None)
         r["peak_source"] = "MEASURED_PEAKS.json" if peaks else "fallback (B200_PROFILING.md)"
         r["ms_per_launch"] = stage_ms[name]
     dom = max(rooflines, key=lambda n: stage_ms[n])
     roof = rooflines[dom]
+
+    # the plain north_star path (rectangle-overlap binning, no tile_cull) on the same workload, same protocol, when the
+    # headline run used tile_cull: its own pipeline and buffers, K timed steps with the L2 flushed in between
+    plain_path = None
+    if args.tile_cull and not args.no_plain:
+        cfg0 = dict(cfg, tile_cull=0)
+        pipe0 = pipeline.SplatPipeline(sc.N, cam, cfg0, device=dev)
+        pipe0.feature_grads = pipe.feature_grads
+
+        def step0(sync):
+            pipe0.project(*params)
+            if args.ray_eval:
+                pipe0.pixel_info(); pipe0.project_ray()
+            pipe0.bin_sort() if sync else pipe0.bin_sort_async()
+            pipe0.rasterize_fwd()
+            xb.xpr_loss_grad(sc.loss, pipe0.image, target, dL_buf)
+            pipe0.rasterize_bwd(dL_buf, *feat_grads)
+            pipe0.project_bwd()
+        for _ in range(3):
+            step0(True)
+        barrier()
+        t0 = []
+        for _ in range(args.steps):
+            flush.fill_(1)
+            a = _rec(); step0(False); b = _rec()
+            torch.cuda.synchronize()
+            t0.append(a.elapsed_time(b))
+        n0 = pipe0.check_capacity()
+        ms0 = max_over_ranks(float(np.mean(t0)), world, dev)
+        plain_path = {"tile_cull": 0, "pairs": n0, "ms_per_step": ms0, "ms_per_step_median": float(np.median(t0)),
+                      "ms_per_step_min": float(np.min(t0)), "value": aggregate_value(world, mp, ms0), "unit": UNIT}
+        del pipe0
 
     # the same step captured once in a CUDA graph and replayed (no host work between the 15 launches)
     graph_ms = None
@@ -538,19 +579,32 @@ def run_ours(args):
         dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull, args.ray_eval, args.features)
         cpu = {"value": (w * h / 1e6) / dt, "unit": UNIT, "cores": xo.num_threads(), "kind": "oracle", "sample": desc,
                "seconds": dt}
+        if args.config <= 2:     # also one thread for the two small configs (a fresh process: OMP_NUM_THREADS=1)
+            code = ("import sys, time, numpy as np; sys.path[:0] = [%r, %r]; import bench, xpr_oracle as xo; "
+                    "from paper_2606_11529_b200 import scenes; sc = scenes.make_scene(%d); "
+                    "dt, _ = bench.oracle_step(xo, scenes, sc, %d, np, %d, %d, %d); print(dt, xo.num_threads())"
+                    % (ROOT, os.path.join(ROOT, "oracle"), args.config, args.view, args.tile_cull, args.ray_eval, args.features))
+            try:
+                out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600,
+                                     env=dict(os.environ, OMP_NUM_THREADS="1"))
+                dt1, th1 = out.stdout.split()[-2:]
+                cpu["one_thread"] = {"value": (w * h / 1e6) / float(dt1), "unit": UNIT, "cores": int(th1), "seconds": float(dt1)}
+            except Exception as e:
+                cpu["one_thread"] = "unavailable: %s" % (str(e)[:100],)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
+                           "image": [cam.width, cam.height], "views": 1, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
                            "candidate_pairs": n_cand, "rows": n_rows, "supertile_words": n_words, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "supertile_digits_on_words": tile_passes,
                                            "on_pairs": 0},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},
-                "gaussians_per_s": world * sc.N / (ms / 1e3), "stage_ms": stage_ms,
+                "gaussians_per_s": world * sc.N / (ms / 1e3), "ms_per_step_stats": step_stats, "stage_ms": stage_ms,
+                "stage_ms_median": stage_ms_median, "plain_path": plain_path,
                 "pixel_pairs": {"visited": visit, "passed_gate": passed, "blended": blended, "sum_n_contrib": sum_n},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
                 "cuda_graph_ms_per_step": graph_ms, "featn": featn, "cub_compare": cub_compare, "roofline": roof, "rooflines": rooflines, "cpu_baseline": cpu}

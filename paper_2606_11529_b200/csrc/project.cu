@@ -235,56 +235,130 @@ __device__ __forceinline__ void load_sh(const float* __restrict__ sh, int64_t i,
     }
 }
 
+// Forward kernel.  Most Gaussians are culled (90 % in config 3: half of them lie behind the camera, most of the rest
+// project outside the image), and the survivors are scattered, so one thread per Gaussian from start to end runs the
+// long geometry and the 48-coefficient colour evaluation with a dozen active lanes per warp (measured: 12 of 32, the
+// kernel was issue-bound on divergent code).  A CTA therefore owns PROJ_THREADS * PROJ_IPT consecutive Gaussians and
+// works in three phases, each over a dense list in shared memory:
+//   A  every Gaussian: camera-space depth of the mean, the z_near test (the first test of project_geometry);
+//      survivors are compacted, the others get tile_count = flags = 0;
+//   B  every survivor of A: the full geometry (EWA or UT), rectangle, visibility; visible ones are compacted and their
+//      geometric outputs written, the others get tile_count = flags = 0;
+//   C  every visible Gaussian: view direction, SH basis, colour (the only reader of the 192-byte SH row), flags and
+//      the packed shader record.
+// Every Gaussian runs exactly the arithmetic of the one-thread version (same functions, same inputs): the outputs
+// are bit-identical.
+// measured on config 3 (us): 128 threads x 2: 49.2; 128 x 4: 50.2; 256 x 8: 51.3; 256 x 2: 52.1; 256 x 4 (72 registers):
+// 57.5; one thread per Gaussian without compaction: 48.5 -- the kernel is bound by the latency of its gathers, not by issue
+#ifndef XPR_PROJ_THREADS
+#define XPR_PROJ_THREADS 128
+#endif
+#ifndef XPR_PROJ_IPT
+#define XPR_PROJ_IPT 2
+#endif
+#ifndef XPR_PROJ_MINB
+#define XPR_PROJ_MINB 6
+#endif
+constexpr int PROJ_THREADS = XPR_PROJ_THREADS, PROJ_IPT = XPR_PROJ_IPT, PROJ_CHUNK = PROJ_THREADS * PROJ_IPT;
+
 template <int K>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(PROJ_THREADS, XPR_PROJ_MINB)
 project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const float* __restrict__ scales,
                const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
                float* __restrict__ mean2d, float* __restrict__ conic_opac, float* __restrict__ rgb,
                float* __restrict__ depth, float* __restrict__ lnv, int32_t* __restrict__ rect,
                uint32_t* __restrict__ tcount, uint8_t* __restrict__ flags, float4* __restrict__ shade_rec) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
-    const float sc[3] = {__ldg(scales + 3 * i), __ldg(scales + 3 * i + 1), __ldg(scales + 3 * i + 2)};
-    const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
-    const float q[4] = {q4.x, q4.y, q4.z, q4.w};
-    const float o = __ldg(opac + i);
-    Fwd F;
-    if (!project_geometry(P, mu, sc, q, o, F)) {
-        tcount[i] = 0u;
-        flags[i] = 0;
-        return;
-    }
-    float dir[3], dnorm, Y[16];
-    view_dir(P, mu, dir, dnorm);
-    sh_basis(dir[0], dir[1], dir[2], Y);
-    float c[3 * K];
-    load_sh<K>(sh, i, c);
-    uint8_t fl = XPR_FLAG_VISIBLE;
-    if (F.clamp_u) fl |= XPR_FLAG_CLAMP_U;
-    if (F.clamp_v) fl |= XPR_FLAG_CLAMP_V;
-    float col[3];
+    __shared__ uint16_t s_a[PROJ_CHUNK], s_b[PROJ_CHUNK];     // survivors of phase A / of phase B (offsets in the chunk)
+    __shared__ uint8_t s_clamp[PROJ_CHUNK];                   // clamp bits of the visible ones (by position in s_b)
+    __shared__ uint32_t s_na, s_nb;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int64_t base = (int64_t)blockIdx.x * PROJ_CHUNK;
+    const int n_here = (int)min((int64_t)PROJ_CHUNK, N - base);
+    if (tid == 0) { s_na = 0u; s_nb = 0u; }
+    __syncthreads();
+    const uint32_t lt = (1u << lane) - 1u;
+    // ---- phase A ---------------------------------------------------------------------------------------------
 #pragma unroll
-    for (int ch = 0; ch < 3; ++ch) {
-        float acc = Y[0] * c[ch];
-#pragma unroll
-        for (int k = 1; k < K; ++k) acc = acc + Y[k] * c[3 * k + ch];
-        const float raw = acc + 0.5f;
-        col[ch] = (0.0f < raw) ? raw : 0.0f;
-        if (raw > 0.0f) fl |= (uint8_t)(XPR_FLAG_RGB_POS_R << ch);
+    for (int k = 0; k < PROJ_IPT; ++k) {
+        const int j = k * PROJ_THREADS + tid;
+        bool keep = false;
+        if (j < n_here) {
+            const int64_t i = base + j;
+            const float m0 = __ldg(means + 3 * i), m1 = __ldg(means + 3 * i + 1), m2 = __ldg(means + 3 * i + 2);
+            const float pz = ((P.W[6] * m0 + P.W[7] * m1) + P.W[8] * m2) + P.t[2];     // = F.p[2] of project_geometry
+            keep = pz > P.z_near;
+            if (!keep) { tcount[i] = 0u; flags[i] = 0; }
+        }
+        const uint32_t m = __ballot_sync(0xffffffffu, keep);
+        uint32_t pos = 0;
+        if (lane == 0 && m) pos = atomicAdd(&s_na, (uint32_t)__popc(m));
+        pos = __shfl_sync(0xffffffffu, pos, 0);
+        if (keep) s_a[pos + __popc(m & lt)] = (uint16_t)j;
     }
-    reinterpret_cast<float2*>(mean2d)[i] = make_float2(F.m[0], F.m[1]);
-    reinterpret_cast<float4*>(conic_opac)[i] = make_float4(F.A, F.B, F.C, F.o_eff);
-    rgb[3 * i] = col[0]; rgb[3 * i + 1] = col[1]; rgb[3 * i + 2] = col[2];
-    depth[i] = F.p[2];
-    lnv[i] = F.lnv;
-    reinterpret_cast<int4*>(rect)[i] = make_int4(F.rect[0], F.rect[1], F.rect[2], F.rect[3]);
-    tcount[i] = F.tc;
-    flags[i] = fl;
-    if (shade_rec) {   // shader data p_sd as the compositing kernels read it: pre-scaled conic (C25, exact)
-        shade_rec[3 * i] = make_float4(F.m[0], F.m[1], -0.5f * F.A, -F.B);
-        shade_rec[3 * i + 1] = make_float4(-0.5f * F.C, -F.lnv, __log2f(F.o_eff), F.p[2]);
-        shade_rec[3 * i + 2] = make_float4(col[0], col[1], col[2], F.o_eff);
+    __syncthreads();
+    // ---- phase B ---------------------------------------------------------------------------------------------
+    const int na = (int)s_na;
+    for (int idx0 = 0; idx0 < na; idx0 += PROJ_THREADS) {
+        const int idx = idx0 + tid;
+        bool vis = false;
+        Fwd F;
+        int64_t i = 0;
+        if (idx < na) {
+            i = base + s_a[idx];
+            const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
+            const float sc[3] = {__ldg(scales + 3 * i), __ldg(scales + 3 * i + 1), __ldg(scales + 3 * i + 2)};
+            const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
+            const float q[4] = {q4.x, q4.y, q4.z, q4.w};
+            vis = project_geometry(P, mu, sc, q, __ldg(opac + i), F);
+            if (!vis) { tcount[i] = 0u; flags[i] = 0; }
+        }
+        const uint32_t m = __ballot_sync(0xffffffffu, vis);
+        uint32_t pos = 0;
+        if (lane == 0 && m) pos = atomicAdd(&s_nb, (uint32_t)__popc(m));
+        pos = __shfl_sync(0xffffffffu, pos, 0);
+        if (vis) {
+            const uint32_t slot = pos + (uint32_t)__popc(m & lt);
+            s_b[slot] = (uint16_t)(i - base);
+            s_clamp[slot] = (uint8_t)((F.clamp_u ? XPR_FLAG_CLAMP_U : 0) | (F.clamp_v ? XPR_FLAG_CLAMP_V : 0));
+            reinterpret_cast<float2*>(mean2d)[i] = make_float2(F.m[0], F.m[1]);
+            reinterpret_cast<float4*>(conic_opac)[i] = make_float4(F.A, F.B, F.C, F.o_eff);
+            depth[i] = F.p[2];
+            lnv[i] = F.lnv;
+            reinterpret_cast<int4*>(rect)[i] = make_int4(F.rect[0], F.rect[1], F.rect[2], F.rect[3]);
+            tcount[i] = F.tc;
+        }
+    }
+    __syncthreads();           // also makes this CTA's geometric outputs visible to phase C
+    // ---- phase C ---------------------------------------------------------------------------------------------
+    const int nb = (int)s_nb;
+    for (int idx = tid; idx < nb; idx += PROJ_THREADS) {
+        const int64_t i = base + s_b[idx];
+        const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
+        float dir[3], dnorm, Y[16];
+        view_dir(P, mu, dir, dnorm);
+        sh_basis(dir[0], dir[1], dir[2], Y);
+        float c[3 * K];
+        load_sh<K>(sh, i, c);
+        uint8_t fl = (uint8_t)(XPR_FLAG_VISIBLE | s_clamp[idx]);
+        float col[3];
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) {
+            float acc = Y[0] * c[ch];
+#pragma unroll
+            for (int k = 1; k < K; ++k) acc = acc + Y[k] * c[3 * k + ch];
+            const float raw = acc + 0.5f;
+            col[ch] = (0.0f < raw) ? raw : 0.0f;
+            if (raw > 0.0f) fl |= (uint8_t)(XPR_FLAG_RGB_POS_R << ch);
+        }
+        rgb[3 * i] = col[0]; rgb[3 * i + 1] = col[1]; rgb[3 * i + 2] = col[2];
+        flags[i] = fl;
+        if (shade_rec) {   // shader data p_sd as the compositing kernels read it: pre-scaled conic (C25, exact)
+            const float2 m = reinterpret_cast<const float2*>(mean2d)[i];        // written in phase B by this CTA
+            const float4 co = reinterpret_cast<const float4*>(conic_opac)[i];
+            shade_rec[3 * i] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
+            shade_rec[3 * i + 1] = make_float4(-0.5f * co.z, -lnv[i], __log2f(co.w), depth[i]);
+            shade_rec[3 * i + 2] = make_float4(col[0], col[1], col[2], co.w);
+        }
     }
 }
 
@@ -546,12 +620,12 @@ __device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, 
     g_opacities[i] = (float)g_o;
 }
 
-// Backward kernel.  Only a fraction of the Gaussians is visible (26 % in config 3) and they are
+// Backward kernel.  Only a fraction of the Gaussians is visible (10 % in config 3, view 0) and they are
 // scattered, so one thread per Gaussian would run the heavy chain rule with a handful of active lanes
-// per warp.  Each CTA therefore owns PBWD_THREADS * ipt consecutive Gaussians and works in three
-// phases: (1) read tile_count / flags coalesced and compact the visible indices into shared memory,
-// (2) run the chain rule over the dense list, (3) write zeros for the culled ones, coalesced, skipping
-// the visible ones (every output element is written exactly once).
+// per warp.  Each CTA therefore owns PBWD_THREADS * ipt consecutive Gaussians: (1) it reads tile_count
+// coalesced and compacts the visible indices into shared memory, (2) it runs the chain rule over the dense
+// list.  The zeros of the culled Gaussians come from a cudaMemsetAsync issued by xpr_project_bwd before the
+// launch (236 B per Gaussian at K = 16: most of the call's bytes, moved at fill bandwidth).
 constexpr int PBWD_THREADS = 128, PBWD_MAX_IPT = 16;
 
 #ifndef XPR_PBWD_MINB
@@ -567,9 +641,8 @@ project_bwd_kernel(int64_t N, ProjParams P, int ipt, const float* __restrict__ m
                    float* __restrict__ g_scales, float* __restrict__ g_quats, float* __restrict__ g_opacities,
                    float* __restrict__ g_sh) {
     __shared__ uint16_t s_list[PBWD_THREADS * PBWD_MAX_IPT];
-    __shared__ uint32_t s_vis[PBWD_THREADS * PBWD_MAX_IPT / 32];   // bit j: Gaussian base + j is visible
     __shared__ uint32_t s_cnt;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
     const int chunk = PBWD_THREADS * ipt;
     const int64_t base = (int64_t)blockIdx.x * chunk;
     const int n_here = (int)min((int64_t)chunk, N - base);
@@ -589,39 +662,15 @@ project_bwd_kernel(int64_t N, ProjParams P, int ipt, const float* __restrict__ m
         const bool vis = (vbits >> k) & 1u;
         const uint32_t m = __ballot_sync(0xffffffffu, vis);
         uint32_t pos = 0;
-        if (lane == 0) {
-            s_vis[k * (PBWD_THREADS / 32) + warp] = m;
-            if (m) pos = atomicAdd(&s_cnt, (uint32_t)__popc(m));
-        }
+        if (lane == 0 && m) pos = atomicAdd(&s_cnt, (uint32_t)__popc(m));
         pos = __shfl_sync(0xffffffffu, pos, 0);
         if (vis) s_list[pos + __popc(m & ((1u << lane) - 1u))] = (uint16_t)j;
     }
     __syncthreads();
     const int cnt = (int)s_cnt;
-    // zeros for the culled Gaussians first: the stores drain while the dense phase waits on its gathers
-    auto culled = [&](int j) { return !((s_vis[j >> 5] >> (j & 31)) & 1u); };
-#pragma unroll 4
-    for (int e = tid; e < 3 * n_here; e += PBWD_THREADS) {
-        if (culled(e / 3)) { g_means[3 * base + e] = 0.0f; g_scales[3 * base + e] = 0.0f; }
-    }
-#pragma unroll 4
-    for (int j = tid; j < n_here; j += PBWD_THREADS) {
-        if (culled(j)) {
-            reinterpret_cast<float4*>(g_quats)[base + j] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-            g_opacities[base + j] = 0.0f;
-        }
-    }
-    if constexpr ((3 * K) % 4 == 0) {
-        constexpr int V = (3 * K) / 4;                 // float4 per Gaussian
-        float4* p4 = reinterpret_cast<float4*>(g_sh) + base * V;
-#pragma unroll 8
-        for (int e = tid; e < V * n_here; e += PBWD_THREADS)
-            if (culled(e / V)) p4[e] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-    } else {
-        float* p = g_sh + base * (3 * K);
-        for (int e = tid; e < 3 * K * n_here; e += PBWD_THREADS)
-            if (culled(e / (3 * K))) p[e] = 0.0f;
-    }
+    // (the outputs were zero-filled by the host side of the call with cudaMemsetAsync -- a full-bandwidth fill instead of
+    // zero stores issued from this 168-register, low-occupancy kernel: 236 B per culled Gaussian are 70 % of the bytes
+    // of the call at 10 % visibility)
     for (int idx = tid; idx < cnt; idx += PBWD_THREADS)
         project_bwd_one<K>(base + s_list[idx], P, means, scales, quats, opac, sh, flags, g_mean2d, g_conic, g_opac,
                            g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh);
@@ -686,8 +735,8 @@ extern "C" int32_t xpr_project(int64_t N, const float* means, const float* scale
     ProjParams P;
     if (int32_t s = make_params(cam, cfg, P)) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    const int threads = 128;
-    const unsigned blocks = (unsigned)((N + threads - 1) / threads);
+    const int threads = PROJ_THREADS;
+    const unsigned blocks = (unsigned)((N + PROJ_CHUNK - 1) / PROJ_CHUNK);
 #define XPR_GO(KK)                                                                                              \
     project_kernel<KK><<<blocks, threads, 0, st>>>(N, P, means, scales, quats, opacities, sh, mean2d, conic_opac, \
                                                    rgb, depth, lnv, tile_rect, tile_count, flags,                \
@@ -728,6 +777,19 @@ extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* s
     ipt = ipt < 1 ? 1 : (ipt > PBWD_MAX_IPT ? PBWD_MAX_IPT : ipt);
     const int64_t chunk = (int64_t)PBWD_THREADS * ipt;
     const unsigned blocks = (unsigned)((N + chunk - 1) / chunk);
+    {   // zero-fill: one memset when the five outputs are adjacent slices of one allocation, in this order
+        const size_t n = (size_t)N, K3 = 3 * (size_t)((cfg->sh_degree + 1) * (cfg->sh_degree + 1));
+        if (g_scales == g_means + 3 * n && g_quats == g_scales + 3 * n && g_opacities == g_quats + 4 * n &&
+            g_sh == g_opacities + n) {
+            XPR_CUDA(cudaMemsetAsync(g_means, 0, sizeof(float) * (11 + K3) * n, st));
+        } else {
+            XPR_CUDA(cudaMemsetAsync(g_means, 0, sizeof(float) * 3 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_scales, 0, sizeof(float) * 3 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_quats, 0, sizeof(float) * 4 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_opacities, 0, sizeof(float) * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_sh, 0, sizeof(float) * K3 * n, st));
+        }
+    }
 #define XPR_GO(KK)                                                                                                  \
     project_bwd_kernel<KK><<<blocks, PBWD_THREADS, 0, st>>>(N, P, ipt, means, scales, quats, opacities, sh, tile_count, \
                                                             flags, g_mean2d, g_conic, g_opac, g_rgb, g_means, g_scales, \

@@ -66,8 +66,12 @@ class SplatPipeline:
         self.g_opac, self.g_rgb, self.g_depth = g2[5 * N:6 * N], g2[6 * N:9 * N].view(N, 3), g2[9 * N:]
         if self.features:
             self.depth_img, self.alpha_img = e(self.H, self.W), e(self.H, self.W)
-        self.g_means, self.g_scales, self.g_quats = e(N, 3), e(N, 3), e(N, 4)
-        self.g_opacities, self.g_sh = e(N), e(N, self.K, 3)
+        # the parameter gradients share one allocation, in the order the library checks for (one zero-fill in xpr_project_bwd)
+        K3 = 3 * self.K
+        g4 = e((11 + K3) * N)
+        self.g_means, self.g_scales = g4[:3 * N].view(N, 3), g4[3 * N:6 * N].view(N, 3)
+        self.g_quats, self.g_opacities = g4[6 * N:10 * N].view(N, 4), g4[10 * N:11 * N]
+        self.g_sh = g4[11 * N:].view(N, self.K, 3)
         if self.ray_eval:   # f2: shader record, per-pixel rays, record gradient
             self.ray_rec = e(N, 12)
             g3 = e(20 * N)                                 # g_ray_acc | g_opac | g_rgb: one memset in xpr_rasterize_ray_bwd

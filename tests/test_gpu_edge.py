@@ -262,3 +262,36 @@ def test_captured_step_replays_the_eager_step(ray):
     for k, v in want.items():
         bad, _ = pu.grad_violations(getattr(pipe, k).cpu().numpy(), v.cpu().numpy())
         assert bad.mean() <= 1e-4, k            # same kernels, same inputs: only the order of the atomics differs
+
+
+@pytest.mark.parametrize("seed", [0, 1])
+def test_tile_cull_needle_gaussians_bit_exact(seed):
+    """f1 adversarial case: rows_kernel keeps, per (Gaussian, tile row), ONE interval of tiles and settles its ends with
+    the exact per-tile predicate; that equals the oracle's tile-by-tile test only if the kept tiles of a row are
+    contiguous.  Needles -- scale ratios 1e3 .. 1e4 (screen-space sigma up to ~900 px against the 0.55 px low-pass
+    floor), rotated in the image plane by any angle incl. 45 degrees, opaque and faint, centres inside and far
+    outside the image -- are where the conservative 2^-18 margin of reading C8 could open a gap.  Lists, keys and
+    ranges must be bit-exact, and the image must equal the one without tile_cull."""
+    import torch
+    rng = np.random.default_rng(700 + seed)
+    sc = scenes.make_scene(3, n_override=4000, image_override=(960, 540))
+    n = sc.N
+    z = rng.uniform(2.0, 9.0, n)
+    sc.means = np.stack([rng.uniform(-1.6, 1.6, n) * z, rng.uniform(-1.0, 1.0, n) * z, z], 1).astype(np.float32)
+    long_ = np.exp(rng.uniform(np.log(0.3), np.log(4.0), n))
+    ratio = np.exp(rng.uniform(np.log(1e3), np.log(1e4), n))
+    sc.scales = np.stack([long_, long_ / ratio, long_ / ratio], 1).astype(np.float32)
+    ang = np.where(rng.random(n) < 0.3, np.pi / 4, rng.uniform(0, np.pi, n))      # in-plane rotation about the view axis
+    tilt = rng.normal(0, 0.05, n)                                                  # slightly out of the image plane
+    q = np.stack([np.cos(ang / 2), tilt * 0.5, tilt * 0.5, np.sin(ang / 2)], 1)
+    sc.quats = (q / np.linalg.norm(q, axis=1, keepdims=True)).astype(np.float32)
+    sc.opacities = np.where(rng.random(n) < 0.5, rng.uniform(0.9, 0.999, n), rng.uniform(0.004, 0.05, n)).astype(np.float32)
+    g = pu.run_gpu(sc, 0, dict(tile_cull=1))
+    o = pu.run_oracle(sc, 0, dict(tile_cull=1))
+    pu.compare_projection(g, o)
+    assert o["binned"]["num_pairs"] > 20000 and o["binned"]["num_pairs"] < 0.5 * o["binned"]["num_candidates"]
+    pu.compare_binning(g, o)                      # bit-exact keys, values, ranges
+    pu.compare_forward(g, o)
+    g0 = pu.run_gpu(sc, 0, dict(tile_cull=0))
+    ok = (o["fwd"]["fragile"] & pu.FRAG_EXIT) == 0
+    assert np.array_equal(g0["fwd"]["image"][ok], g["fwd"]["image"][ok])          # culling changes no pixel (PAPER L683)
