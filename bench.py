@@ -37,6 +37,10 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--view", type=int, default=0)
+    ap.add_argument("--views", type=int, default=1,
+                    help="V > 1: a step renders the batch of views view .. view+V-1 of the scene with ONE call per stage "
+                         "(xpr_config.views; SURVEY 8(f) f3; meant for --config 5, whose scene has four views); the metric "
+                         "counts the pixels of all V images")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-graph", action="store_true")
@@ -127,8 +131,16 @@ def aggregate_value(world: int, megapixels: float, ms_per_step: float) -> float:
     return world * megapixels / (ms_per_step / 1e3)
 
 
-def oracle_step(xo, scenes, sc, view, np, tile_cull=0, ray_eval=0, features=0):
-    """One fwd+bwd step of the CPU oracle, as it stands (never tuned)."""
+def oracle_step(xo, scenes, sc, view, np, tile_cull=0, ray_eval=0, features=0, views=1):
+    """One fwd+bwd step of the CPU oracle, as it stands (never tuned); a batch of views is a loop over the views."""
+    t_all, pairs = 0.0, 0
+    for v in range(view, view + max(1, views)):
+        dt, n = _oracle_view(xo, scenes, sc, v, np, tile_cull, ray_eval, features)
+        t_all += dt; pairs += n
+    return t_all, pairs
+
+
+def _oracle_view(xo, scenes, sc, view, np, tile_cull, ray_eval, features):
     cam = xo.make_camera(sc.cameras[view])
     cfg = xo.make_config(dict(scenes.default_render_config(sc), tile_cull=tile_cull))
     arrays = dict(means=sc.means, scales=sc.scales, quats=sc.quats, opacities=sc.opacities, sh=sc.sh)
@@ -171,18 +183,18 @@ def run_reference(args):
     from paper_2606_11529_b200 import scenes
     sc, w, h, desc = oracle_sample(args)
     for _ in range(args.warmup):
-        oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval, args.features)
+        oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval, args.features, args.views)
     t = 0.0
     for _ in range(args.steps):
-        dt, I = oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval, args.features)
+        dt, I = oracle_step(xo, scenes, sc, args.view, np, args.tile_cull, args.ray_eval, args.features, args.views)
         t += dt
     ms = 1e3 * t / max(args.steps, 1)
-    val = (w * h / 1e6) / (ms / 1e3)
+    val = (max(1, args.views) * w * h / 1e6) / (ms / 1e3)
     cores = xo.num_threads()
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config], "view": args.view, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "sample": desc,
+            "config": {"workload": WORKLOADS[args.config], "view": args.view, "views": max(1, args.views), "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "sample": desc,
                        "pairs": int(I)},
             "gaussians_per_s": sc.N / (ms / 1e3),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
@@ -219,13 +231,21 @@ def run_ours(args):
 
     sc = scenes.make_scene(args.config)
     cam = sc.cameras[args.view]
+    V = max(1, args.views)
+    if V > 1 and (args.features or args.ray_eval or args.view + V > len(sc.cameras)):
+        raise SystemExit("bench.py: --views V needs V cameras in the scene (config 5 has four) and the 2D colour pass")
     if args.features and args.ray_eval:
         raise SystemExit("bench.py: --features 1 is built for the 2D evaluation (not with --ray-eval 1)")
     cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval,
                tile_order=args.tile_order, features=args.features)
     params = pipeline.scene_to_device(sc, dev)
-    target = torch.from_numpy(sc.target(args.view)).to(dev)
-    pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
+    if V > 1:
+        target = torch.from_numpy(np.stack([sc.target(args.view + v) for v in range(V)])).to(dev)
+        pipe = pipeline.SplatPipeline(sc.N, [sc.cameras[args.view + v] for v in range(V)], cfg, device=dev)
+        args.no_plain = True      # the extra plain-path timing is a single-view leg
+    else:
+        target = torch.from_numpy(sc.target(args.view)).to(dev)
+        pipe = pipeline.SplatPipeline(sc.N, cam, cfg, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     dL_buf = torch.empty_like(target)
@@ -304,7 +324,7 @@ def run_ours(args):
     stage_ms_median = {n: float(np.median([e[i].elapsed_time(e[i + 1]) for e in all_events])) for i, n in enumerate(stage_names)}
     step_stats = {"mean": float(np.mean(step_ms)), "median": float(np.median(step_ms)), "min": float(np.min(step_ms)),
                   "max": float(np.max(step_ms)), "note": "this rank's K timed steps, CUDA events; ms_per_step is the mean, max over ranks"}
-    mp = cam.width * cam.height / 1e6
+    mp = V * cam.width * cam.height / 1e6
     value = aggregate_value(world, mp, ms)
 
     # roofline of the dominant kernel (largest stage): pixel-pair counts from xpr_rasterize_stats
@@ -576,8 +596,8 @@ def run_ours(args):
         sys.path.insert(0, os.path.join(ROOT, "oracle"))
         import xpr_oracle as xo
         osc, w, h, desc = oracle_sample(args)
-        dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull, args.ray_eval, args.features)
-        cpu = {"value": (w * h / 1e6) / dt, "unit": UNIT, "cores": xo.num_threads(), "kind": "oracle", "sample": desc,
+        dt, _ = oracle_step(xo, scenes, osc, args.view, np, args.tile_cull, args.ray_eval, args.features, args.views)
+        cpu = {"value": (V * w * h / 1e6) / dt, "unit": UNIT, "cores": xo.num_threads(), "kind": "oracle", "sample": desc,
                "seconds": dt}
         if args.config <= 2:     # also one thread for the two small configs (a fresh process: OMP_NUM_THREADS=1)
             code = ("import sys, time, numpy as np; sys.path[:0] = [%r, %r]; import bench, xpr_oracle as xo; "
@@ -597,13 +617,13 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "views": 1, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
+                           "image": [cam.width, cam.height], "views": V, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
                            "candidate_pairs": n_cand, "rows": n_rows, "supertile_words": n_words, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "supertile_digits_on_words": tile_passes,
                                            "on_pairs": 0},
                            "l2": "flushed between timed steps (256 MiB write); inputs (236 MB) also exceed L2",
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},
-                "gaussians_per_s": world * sc.N / (ms / 1e3), "ms_per_step_stats": step_stats, "stage_ms": stage_ms,
+                "gaussians_per_s": world * V * sc.N / (ms / 1e3), "ms_per_step_stats": step_stats, "stage_ms": stage_ms,
                 "stage_ms_median": stage_ms_median, "plain_path": plain_path,
                 "pixel_pairs": {"visited": visit, "passed_gate": passed, "blended": blended, "sum_n_contrib": sum_n},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,

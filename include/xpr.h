@@ -62,7 +62,16 @@ typedef struct {
                                xpr_bin_sort[_cull] also writes the tile indices by decreasing list length (1024
                                length classes) and the four rasterize calls walk the tiles in that order, so that
                                the tail of a launch consists of short tiles */
+    int32_t views;          /* 0 or 1: one view.  V in 2..8: ONE call renders a batch of V views of the same Gaussians (PAPER
+                               L19, Table 2 "batched views"; BASELINE.json configs[4]): `cam` then points to V cameras of
+                               equal model, width and height; per-Gaussian outputs of xpr_project (and the inputs of the later
+                               calls) are [V*N, ...] view-major, index v*N + i; tile_rect rows are offset by v*tiles_y, so that
+                               the tile id of a pair is v*T + t and one xpr_bin_sort[_cull] call (its N = V*N) sorts all views
+                               (keys = (v*T + t) << 32 | depth bits; tile_ranges [V*T, 2]); images are [V, H, W, .], the
+                               compositing calls launch V*T tiles; xpr_project_bwd SUMS the parameter gradients over the views.
+                               xpr_pixel_info, xpr_project_ray, xpr_ray_bwd, xpr_depth_bwd and the featn calls take one view */
 } xpr_config;
+enum { XPR_MAX_VIEWS = 8 };
 
 const char* xpr_status_string(int32_t status);
 int32_t xpr_last_cuda_error(void);   /* cudaError_t of the last XPR_ERR_CUDA on this thread */

@@ -254,6 +254,23 @@ def backward(scene_arrays: dict, r: dict, dL_dimage, cam: XoCamera, cfg: XoConfi
     return g3
 
 
+# ---- batch of views (Table 2): the definition is a loop over the views ------------
+
+def render_views(scene_arrays: dict, cams: list, cfg: XoConfig, dtype=np.float32) -> list:
+    """One render() per camera: a batch of views is V independent renders of the same primitives."""
+    return [render(scene_arrays, cam, cfg, dtype) for cam in cams]
+
+
+def backward_views(scene_arrays: dict, rs: list, dLs: list, cams: list, cfg: XoConfig, dtype=np.float32) -> dict:
+    """Parameter gradients of L = sum over the views of L_v: the sum of the single-view gradients (fp64)."""
+    out = None
+    for r, dL, cam in zip(rs, dLs, cams):
+        g = backward(scene_arrays, r, dL, cam, cfg, dtype)
+        g = {k: g[k] for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")}
+        out = g if out is None else {k: out[k] + g[k] for k in out}
+    return out
+
+
 # ---- XPR-3DGUT ray evaluation (SURVEY 8(f) f2; xpr_oracle_ray.inc) -------------------------------------------
 
 def pixel_info(cam: XoCamera, dtype=np.float32):

@@ -33,7 +33,7 @@ class XprConfig(C.Structure):
     _fields_ = [("projection", C.c_int32), ("sh_degree", C.c_int32), ("tile", C.c_int32), ("antialias", C.c_int32),
                 ("alpha_thresh", C.c_float), ("alpha_max", C.c_float), ("t_min", C.c_float), ("z_near", C.c_float),
                 ("lowpass", C.c_float), ("ut_alpha", C.c_float), ("ut_beta", C.c_float), ("ut_kappa", C.c_float),
-                ("bg", C.c_float * 3), ("tile_cull", C.c_int32), ("tile_order", C.c_void_p)]
+                ("bg", C.c_float * 3), ("tile_cull", C.c_int32), ("tile_order", C.c_void_p), ("views", C.c_int32)]
 
 
 class XprError(RuntimeError):
@@ -86,7 +86,16 @@ def make_config(d: dict) -> XprConfig:
         c.bg[i] = float(d["bg"][i])
     c.tile_cull = int(d.get("tile_cull", 0))
     c.tile_order = None      # the pipeline sets tile_order to a device buffer of T uint32 (scheduling only)
+    c.views = int(d.get("views", 1))
     return c
+
+
+def make_cameras(cams):
+    """A contiguous array of xpr_camera for a batch of views (xpr_config.views)."""
+    arr = (XprCamera * len(cams))()
+    for i, cam in enumerate(cams):
+        C.memmove(C.byref(arr[i]), C.byref(make_camera(cam)), C.sizeof(XprCamera))
+    return arr
 
 
 def num_tiles(cam: XprCamera, cfg: XprConfig):

@@ -582,7 +582,7 @@ __device__ __forceinline__ float approx_sqrt(float x) {   // the interval estima
 constexpr int ROW_SMEM = 2048;     // tile rows whose first-tile counter is kept in shared memory
 template <bool CULL>
 __global__ void __launch_bounds__(128)
-rows_kernel(int TW, int TH, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ row_base,
+rows_kernel(int TW, int TH, int TH_view, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ row_base,
             const int4* __restrict__ rect, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
             const float* __restrict__ lnv, const Header* __restrict__ hdr, uint32_t* __restrict__ row_tab,
             int* __restrict__ tile_diff) {
@@ -634,9 +634,10 @@ rows_kernel(int TW, int TH, const uint32_t* __restrict__ vidx, const uint32_t* _
         }
         int xa = r.x, xb = r.z;                                 // kept tiles of this row: [xa, xb)
         if (CULL) {
-            const auto keep = [&](int tx) { return tile_keep(mx, my, A, B, C, L, (uint32_t)tx, (uint32_t)ty); };
+            const int tyv = ty % TH_view;              // batch of views: the tile rows of view v are offset by v * TH_view
+            const auto keep = [&](int tx) { return tile_keep(mx, my, A, B, C, L, (uint32_t)tx, (uint32_t)tyv); };
             // estimate: x extent of {q <= L} over dy in [lo, hi] (pixel-centre hull of the row)
-            const float lo = (float)(TILE * ty) + 0.5f - my, hi = (float)(TILE * ty + TILE) - 0.5f - my;
+            const float lo = (float)(TILE * tyv) + 0.5f - my, hi = (float)(TILE * tyv + TILE) - 0.5f - my;
             float left = 1e30f, right = -1e30f;
             const float rA = __fdividef(1.0f, A);
             const float dy_ext = __fdividef(B * ext, C);        // dy at the ellipse's extreme x: -B dx / C, dx = -+ext
@@ -1164,7 +1165,8 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0 || pair_capacity < 0 || pair_capacity >= (1LL << 30)) return XPR_ERR_INVALID_ARG;
     if (N >= (1LL << 30)) return XPR_ERR_UNSUPPORTED;      // the look-back status words carry 30-bit counts
-    const int TW = tiles_x(cam), TH = tiles_y(cam);
+    // a batch of V views (xpr_config.views) is one image of V * tiles_y tile rows: view v owns rows [v tiles_y, (v+1) tiles_y)
+    const int TW = tiles_x(cam), TH_view = tiles_y(cam), TH = TH_view * num_views(cfg);
     const int64_t T64 = (int64_t)TW * TH;
     if (T64 > (1 << 24) || TW > 0xffff) return XPR_ERR_UNSUPPORTED;   // row table: 16-bit columns
     const int32_t T = (int32_t)T64;
@@ -1238,10 +1240,10 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     // 4. rows: surviving interval per (Gaussian, tile row) -> row table + difference array over the tile ids
     const unsigned rgrid = 148u * 16u;                               // grid-stride over the rows (count on the device)
     if (cull)
-        rows_kernel<true><<<rgrid, 128, 0, st>>>(TW, TH, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
+        rows_kernel<true><<<rgrid, 128, 0, st>>>(TW, TH, TH_view, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
                                                  reinterpret_cast<const float4*>(conic_opac), lnv, hdr, row_tab, tile_diff);
     else
-        rows_kernel<false><<<rgrid, 128, 0, st>>>(TW, TH, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, hdr, row_tab,
+        rows_kernel<false><<<rgrid, 128, 0, st>>>(TW, TH, TH_view, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, hdr, row_tab,
                                                   tile_diff);
     XPR_LAUNCH_CHECK();
     // 5. supertile words in rank order; pass p of the supertile sort reads buffer p and writes buffer p + 1, the

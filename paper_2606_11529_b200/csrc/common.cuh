@@ -36,8 +36,14 @@ inline int32_t check_cam_cfg(const xpr_camera* cam, const xpr_config* cfg) {
     if (cfg->sh_degree > 3) return XPR_ERR_UNSUPPORTED;
     if (cfg->tile != TILE) return XPR_ERR_UNSUPPORTED;
     if (cfg->projection == 0 && cam->model != 0) return XPR_ERR_UNSUPPORTED;  // EWA Jacobian is the pinhole's
+    if (cfg->views < 0) return XPR_ERR_INVALID_ARG;
+    if (cfg->views > XPR_MAX_VIEWS) return XPR_ERR_UNSUPPORTED;
+    for (int v = 1; v < cfg->views; ++v)      // a batch of views shares the image geometry (xpr.h)
+        if (cam[v].model != cam->model || cam[v].width != cam->width || cam[v].height != cam->height) return XPR_ERR_INVALID_ARG;
     return XPR_OK;
 }
+
+inline int num_views(const xpr_config* cfg) { return cfg->views > 1 ? cfg->views : 1; }
 
 inline int tiles_x(const xpr_camera* cam) { return (cam->width + TILE - 1) / TILE; }
 inline int tiles_y(const xpr_camera* cam) { return (cam->height + TILE - 1) / TILE; }

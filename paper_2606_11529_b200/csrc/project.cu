@@ -27,6 +27,7 @@ struct ProjParams {
     float cpos[3];                 // camera position -W^T t
     int TW, TH;
 };
+struct ProjBatch { ProjParams p[XPR_MAX_VIEWS]; };   // one entry per view of a batch (xpr_config.views), kernel parameter
 
 // Real SH basis, degree <= 3, index k = l^2 + l + m, Condon-Shortley sign (reading C5).
 #define XPR_SH_C0 ((float)0.28209479177387814)   // 1/(2 sqrt(pi))
@@ -263,7 +264,7 @@ constexpr int PROJ_THREADS = XPR_PROJ_THREADS, PROJ_IPT = XPR_PROJ_IPT, PROJ_CHU
 
 template <int K>
 __global__ void __launch_bounds__(PROJ_THREADS, XPR_PROJ_MINB)
-project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const float* __restrict__ scales,
+project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __restrict__ means, const float* __restrict__ scales,
                const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
                float* __restrict__ mean2d, float* __restrict__ conic_opac, float* __restrict__ rgb,
                float* __restrict__ depth, float* __restrict__ lnv, int32_t* __restrict__ rect,
@@ -271,6 +272,10 @@ project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const f
     __shared__ uint16_t s_a[PROJ_CHUNK], s_b[PROJ_CHUNK];     // survivors of phase A / of phase B (offsets in the chunk)
     __shared__ uint8_t s_clamp[PROJ_CHUNK];                   // clamp bits of the visible ones (by position in s_b)
     __shared__ uint32_t s_na, s_nb;
+    // batch of views (xpr_config.views): blockIdx.y is the view; its outputs live at index v N + i, its tile rows at v TH
+    const ProjParams& P = PB.p[blockIdx.y];
+    const int64_t vo = (int64_t)blockIdx.y * N;
+    const int yoff = (int)blockIdx.y * P.TH;
     const int tid = threadIdx.x, lane = tid & 31;
     const int64_t base = (int64_t)blockIdx.x * PROJ_CHUNK;
     const int n_here = (int)min((int64_t)PROJ_CHUNK, N - base);
@@ -287,7 +292,7 @@ project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const f
             const float m0 = __ldg(means + 3 * i), m1 = __ldg(means + 3 * i + 1), m2 = __ldg(means + 3 * i + 2);
             const float pz = ((P.W[6] * m0 + P.W[7] * m1) + P.W[8] * m2) + P.t[2];     // = F.p[2] of project_geometry
             keep = pz > P.z_near;
-            if (!keep) { tcount[i] = 0u; flags[i] = 0; }
+            if (!keep) { tcount[vo + i] = 0u; flags[vo + i] = 0; }
         }
         const uint32_t m = __ballot_sync(0xffffffffu, keep);
         uint32_t pos = 0;
@@ -310,7 +315,7 @@ project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const f
             const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
             const float q[4] = {q4.x, q4.y, q4.z, q4.w};
             vis = project_geometry(P, mu, sc, q, __ldg(opac + i), F);
-            if (!vis) { tcount[i] = 0u; flags[i] = 0; }
+            if (!vis) { tcount[vo + i] = 0u; flags[vo + i] = 0; }
         }
         const uint32_t m = __ballot_sync(0xffffffffu, vis);
         uint32_t pos = 0;
@@ -320,12 +325,13 @@ project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const f
             const uint32_t slot = pos + (uint32_t)__popc(m & lt);
             s_b[slot] = (uint16_t)(i - base);
             s_clamp[slot] = (uint8_t)((F.clamp_u ? XPR_FLAG_CLAMP_U : 0) | (F.clamp_v ? XPR_FLAG_CLAMP_V : 0));
-            reinterpret_cast<float2*>(mean2d)[i] = make_float2(F.m[0], F.m[1]);
-            reinterpret_cast<float4*>(conic_opac)[i] = make_float4(F.A, F.B, F.C, F.o_eff);
-            depth[i] = F.p[2];
-            lnv[i] = F.lnv;
-            reinterpret_cast<int4*>(rect)[i] = make_int4(F.rect[0], F.rect[1], F.rect[2], F.rect[3]);
-            tcount[i] = F.tc;
+            const int64_t o = vo + i;
+            reinterpret_cast<float2*>(mean2d)[o] = make_float2(F.m[0], F.m[1]);
+            reinterpret_cast<float4*>(conic_opac)[o] = make_float4(F.A, F.B, F.C, F.o_eff);
+            depth[o] = F.p[2];
+            lnv[o] = F.lnv;
+            reinterpret_cast<int4*>(rect)[o] = make_int4(F.rect[0], F.rect[1] + yoff, F.rect[2], F.rect[3] + yoff);
+            tcount[o] = F.tc;
         }
     }
     __syncthreads();           // also makes this CTA's geometric outputs visible to phase C
@@ -350,14 +356,15 @@ project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const f
             col[ch] = (0.0f < raw) ? raw : 0.0f;
             if (raw > 0.0f) fl |= (uint8_t)(XPR_FLAG_RGB_POS_R << ch);
         }
-        rgb[3 * i] = col[0]; rgb[3 * i + 1] = col[1]; rgb[3 * i + 2] = col[2];
-        flags[i] = fl;
+        const int64_t o = vo + i;
+        rgb[3 * o] = col[0]; rgb[3 * o + 1] = col[1]; rgb[3 * o + 2] = col[2];
+        flags[o] = fl;
         if (shade_rec) {   // shader data p_sd as the compositing kernels read it: pre-scaled conic (C25, exact)
-            const float2 m = reinterpret_cast<const float2*>(mean2d)[i];        // written in phase B by this CTA
-            const float4 co = reinterpret_cast<const float4*>(conic_opac)[i];
-            shade_rec[3 * i] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-            shade_rec[3 * i + 1] = make_float4(-0.5f * co.z, -lnv[i], __log2f(co.w), depth[i]);
-            shade_rec[3 * i + 2] = make_float4(col[0], col[1], col[2], co.w);
+            const float2 m = reinterpret_cast<const float2*>(mean2d)[o];        // written in phase B by this CTA
+            const float4 co = reinterpret_cast<const float4*>(conic_opac)[o];
+            shade_rec[3 * o] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
+            shade_rec[3 * o + 1] = make_float4(-0.5f * co.z, -lnv[o], __log2f(co.w), depth[o]);
+            shade_rec[3 * o + 2] = make_float4(col[0], col[1], col[2], co.w);
         }
     }
 }
@@ -421,8 +428,14 @@ __device__ __forceinline__ void camera_jac(const ProjParams& P, const B p[3], B 
 }
 
 template <int K>
-__device__ __forceinline__ void store_sh_grad(float* __restrict__ g_sh, int64_t i, const float* g) {
+__device__ __forceinline__ void store_sh_grad(float* __restrict__ g_sh, int64_t i, const float* g, bool accum = false) {
     float* p = g_sh + (int64_t)3 * K * i;
+    if (accum) {       // batch of views: the views' contributions are summed (fp32 atomics; at most XPR_MAX_VIEWS terms)
+#pragma unroll
+        for (int j = 0; j < 3 * K; ++j)
+            if (g[j] != 0.0f) atomicAdd(p + j, g[j]);
+        return;
+    }
     if constexpr ((3 * K) % 4 == 0) {
         float4* p4 = reinterpret_cast<float4*>(p);
 #pragma unroll
@@ -435,7 +448,7 @@ __device__ __forceinline__ void store_sh_grad(float* __restrict__ g_sh, int64_t 
 
 // One visible Gaussian: recompute the forward, chain rule in fp64, store its 59 gradient floats.
 template <int K>
-__device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, const float* __restrict__ means,
+__device__ __forceinline__ void project_bwd_one(int64_t i, int64_t vo, bool accum, const ProjParams& P, const float* __restrict__ means,
                                                 const float* __restrict__ scales, const float* __restrict__ quats,
                                                 const float* __restrict__ opac, const float* __restrict__ sh,
                                                 const uint8_t* __restrict__ flags, const float* __restrict__ g_mean2d,
@@ -445,7 +458,7 @@ __device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, 
                                                 float* __restrict__ g_opacities, float* __restrict__ g_sh) {
     B g_mu[3] = {0, 0, 0}, g_s[3] = {0, 0, 0}, g_q[4] = {0, 0, 0, 0}, g_o = 0;
     // every load of this Gaussian is issued up front (the kernel is latency-bound: DESIGN.md 6.1)
-    const uint8_t fl = flags[i];
+    const uint8_t fl = flags[vo + i];        // per-view quantities live at v N + i (xpr_config.views)
     Fwd F;
     float mu[3], sc[3], q[4], o;
     mu[0] = __ldg(means + 3 * i); mu[1] = __ldg(means + 3 * i + 1); mu[2] = __ldg(means + 3 * i + 2);
@@ -453,10 +466,11 @@ __device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, 
     const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
     q[0] = q4.x; q[1] = q4.y; q[2] = q4.z; q[3] = q4.w;
     o = __ldg(opac + i);
-    const float2 gm_f = __ldg(reinterpret_cast<const float2*>(g_mean2d) + i);
-    const float gK_f[3] = {__ldg(g_conic + 3 * i), __ldg(g_conic + 3 * i + 1), __ldg(g_conic + 3 * i + 2)};
-    const float go_f = __ldg(g_opac + i);
-    const float grgb_f[3] = {__ldg(g_rgb + 3 * i), __ldg(g_rgb + 3 * i + 1), __ldg(g_rgb + 3 * i + 2)};
+    const int64_t vi = vo + i;
+    const float2 gm_f = __ldg(reinterpret_cast<const float2*>(g_mean2d) + vi);
+    const float gK_f[3] = {__ldg(g_conic + 3 * vi), __ldg(g_conic + 3 * vi + 1), __ldg(g_conic + 3 * vi + 2)};
+    const float go_f = __ldg(g_opac + vi);
+    const float grgb_f[3] = {__ldg(g_rgb + 3 * vi), __ldg(g_rgb + 3 * vi + 1), __ldg(g_rgb + 3 * vi + 2)};
     {   // colour first: rgb = max(0, 1/2 + sum_k Y_k(d) sh_k), d = (mu - cam_pos)/|mu - cam_pos|.  Its 3K
         // coefficient gradients are stored at once, so they do not occupy registers during the chain rule.
         float c[3 * K];
@@ -479,7 +493,7 @@ __device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, 
 #pragma unroll
             for (int j = 0; j < 3; ++j) gd[j] += dY[k][j] * w;
         }
-        store_sh_grad<K>(g_sh, i, gsh);
+        store_sh_grad<K>(g_sh, i, gsh, accum);
         const B dot = (B)dir[0] * gd[0] + (B)dir[1] * gd[1] + (B)dir[2] * gd[2];
 #pragma unroll
         for (int j = 0; j < 3; ++j) g_mu[j] = (gd[j] - (B)dir[j] * dot) / (B)dnorm;
@@ -611,8 +625,16 @@ __device__ __forceinline__ void project_bwd_one(int64_t i, const ProjParams& P, 
         float z[3 * K];
 #pragma unroll
         for (int j = 0; j < 3 * K; ++j) z[j] = 0.0f;
-        store_sh_grad<K>(g_sh, i, z);
+        if (!accum) store_sh_grad<K>(g_sh, i, z);
         g_mu[0] = g_mu[1] = g_mu[2] = 0;
+    }
+    if (accum) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) { atomicAdd(g_means + 3 * i + j, (float)g_mu[j]); atomicAdd(g_scales + 3 * i + j, (float)g_s[j]); }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) atomicAdd(g_quats + 4 * i + j, (float)g_q[j]);
+        atomicAdd(g_opacities + i, (float)g_o);
+        return;
     }
     g_means[3 * i] = (float)g_mu[0]; g_means[3 * i + 1] = (float)g_mu[1]; g_means[3 * i + 2] = (float)g_mu[2];
     g_scales[3 * i] = (float)g_s[0]; g_scales[3 * i + 1] = (float)g_s[1]; g_scales[3 * i + 2] = (float)g_s[2];
@@ -633,7 +655,7 @@ constexpr int PBWD_THREADS = 128, PBWD_MAX_IPT = 16;
 #endif
 template <int K>
 __global__ void __launch_bounds__(PBWD_THREADS, XPR_PBWD_MINB)
-project_bwd_kernel(int64_t N, ProjParams P, int ipt, const float* __restrict__ means, const float* __restrict__ scales,
+project_bwd_kernel(int64_t N, const __grid_constant__ ProjBatch PB, int ipt, const float* __restrict__ means, const float* __restrict__ scales,
                    const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
                    const uint32_t* __restrict__ tcount, const uint8_t* __restrict__ flags,
                    const float* __restrict__ g_mean2d, const float* __restrict__ g_conic,
@@ -642,6 +664,9 @@ project_bwd_kernel(int64_t N, ProjParams P, int ipt, const float* __restrict__ m
                    float* __restrict__ g_sh) {
     __shared__ uint16_t s_list[PBWD_THREADS * PBWD_MAX_IPT];
     __shared__ uint32_t s_cnt;
+    const ProjParams& P = PB.p[blockIdx.y];            // batch of views: blockIdx.y is the view
+    const int64_t vo = (int64_t)blockIdx.y * N;
+    const bool accum = gridDim.y > 1;
     const int tid = threadIdx.x, lane = tid & 31;
     const int chunk = PBWD_THREADS * ipt;
     const int64_t base = (int64_t)blockIdx.x * chunk;
@@ -652,7 +677,7 @@ project_bwd_kernel(int64_t N, ProjParams P, int ipt, const float* __restrict__ m
 #pragma unroll
     for (int k = 0; k < PBWD_MAX_IPT; ++k) {
         const int j = k * PBWD_THREADS + tid;
-        tc[k] = (k < ipt && j < n_here) ? __ldg(tcount + base + j) : 0u;
+        tc[k] = (k < ipt && j < n_here) ? __ldg(tcount + vo + base + j) : 0u;
     }
     uint32_t vbits = 0;
 #pragma unroll
@@ -672,7 +697,7 @@ project_bwd_kernel(int64_t N, ProjParams P, int ipt, const float* __restrict__ m
     // zero stores issued from this 168-register, low-occupancy kernel: 236 B per culled Gaussian are 70 % of the bytes
     // of the call at 10 % visibility)
     for (int idx = tid; idx < cnt; idx += PBWD_THREADS)
-        project_bwd_one<K>(base + s_list[idx], P, means, scales, quats, opac, sh, flags, g_mean2d, g_conic, g_opac,
+        project_bwd_one<K>(base + s_list[idx], vo, accum, P, means, scales, quats, opac, sh, flags, g_mean2d, g_conic, g_opac,
                            g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh);
 }
 
@@ -732,11 +757,13 @@ extern "C" int32_t xpr_project(int64_t N, const float* means, const float* scale
         !aligned(depth, 4) || !aligned(lnv, 4) || !aligned(tile_rect, 16) || !aligned(tile_count, 4) || !flags ||
         (shade_rec && !aligned(shade_rec, 16)))
         return XPR_ERR_INVALID_ARG;
-    ProjParams P;
-    if (int32_t s = make_params(cam, cfg, P)) return s;
+    ProjBatch P;
+    const int V = num_views(cfg);
+    for (int v = 0; v < V; ++v)
+        if (int32_t s = make_params(cam + v, cfg, P.p[v])) return s;
     cudaStream_t st = (cudaStream_t)stream;
     const int threads = PROJ_THREADS;
-    const unsigned blocks = (unsigned)((N + PROJ_CHUNK - 1) / PROJ_CHUNK);
+    const dim3 blocks((unsigned)((N + PROJ_CHUNK - 1) / PROJ_CHUNK), (unsigned)V);
 #define XPR_GO(KK)                                                                                              \
     project_kernel<KK><<<blocks, threads, 0, st>>>(N, P, means, scales, quats, opacities, sh, mean2d, conic_opac, \
                                                    rgb, depth, lnv, tile_rect, tile_count, flags,                \
@@ -766,8 +793,10 @@ extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* s
         !aligned(g_opac, 4) || !aligned(g_rgb, 4) || !aligned(g_means, 4) || !aligned(g_scales, 4) ||
         !aligned(g_quats, 16) || !aligned(g_opacities, 4) || !aligned(g_sh, 16))
         return XPR_ERR_INVALID_ARG;
-    ProjParams P;
-    if (int32_t s = make_params(cam, cfg, P)) return s;
+    ProjBatch P;
+    const int V = num_views(cfg);
+    for (int v = 0; v < V; ++v)
+        if (int32_t s = make_params(cam + v, cfg, P.p[v])) return s;
     cudaStream_t st = (cudaStream_t)stream;
     // Gaussians per CTA: enough CTAs for one full wave (148 SMs x 4 CTAs) before growing the chunk
 #ifndef XPR_PBWD_WAVES
@@ -776,7 +805,7 @@ extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* s
     int ipt = (int)(N / ((int64_t)148 * 4 * PBWD_THREADS * XPR_PBWD_WAVES));
     ipt = ipt < 1 ? 1 : (ipt > PBWD_MAX_IPT ? PBWD_MAX_IPT : ipt);
     const int64_t chunk = (int64_t)PBWD_THREADS * ipt;
-    const unsigned blocks = (unsigned)((N + chunk - 1) / chunk);
+    const dim3 blocks((unsigned)((N + chunk - 1) / chunk), (unsigned)V);
     {   // zero-fill: one memset when the five outputs are adjacent slices of one allocation, in this order
         const size_t n = (size_t)N, K3 = 3 * (size_t)((cfg->sh_degree + 1) * (cfg->sh_degree + 1));
         if (g_scales == g_means + 3 * n && g_quats == g_scales + 3 * n && g_opacities == g_quats + 4 * n &&

@@ -24,6 +24,7 @@ constexpr int STAGES = 3;            // cp.async ring depth
 
 struct RasterParams {
     int W, H, TW;
+    int T;                   // tiles per view: tile index b of a batch of views is view b / T, tile b % T of that view
     float amax, tmin;
     float bg[3];
     const uint32_t* order;   // xpr_config.tile_order: CTA b works on tile order[b] (longest lists first), or NULL
@@ -66,7 +67,9 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
     __shared__ float4 s_rec[STAGES][3 * B];
     const int tid = threadIdx.x;
     const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
-    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int view = tile / P.T, vt = tile - view * P.T;       // batch of views: the images are stacked, [V, H, W, .]
+    const int64_t vbase = (int64_t)view * P.H * P.W;
+    const int tx = vt % P.TW, ty = vt / P.TW;
     const int px0 = tx * TILE + (tid % ROW), px1 = px0 + 8, py = ty * TILE + (tid / ROW);
     const bool in0 = (px0 < P.W) && (py < P.H), in1 = (PPT == 2) && (px1 < P.W) && (py < P.H);
     const float pxc0 = (float)px0 + 0.5f, pxc1 = (float)px1 + 0.5f, pyc = (float)py + 0.5f;
@@ -231,7 +234,7 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
         return;
     }
     if (in0) {
-        const int64_t pid = (int64_t)py * P.W + px0;
+        const int64_t pid = vbase + (int64_t)py * P.W + px0;
         image[3 * pid] = fmaf(Ta, P.bg[0], Ca0);
         image[3 * pid + 1] = fmaf(Ta, P.bg[1], Ca1);
         image[3 * pid + 2] = fmaf(Ta, P.bg[2], Ca2);
@@ -240,7 +243,7 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
         if (FEAT) { depth_img[pid] = Da; alpha_img[pid] = Aa; }
     }
     if (in1) {
-        const int64_t pid = (int64_t)py * P.W + px1;
+        const int64_t pid = vbase + (int64_t)py * P.W + px1;
         image[3 * pid] = fmaf(Tb, P.bg[0], Cb0);
         image[3 * pid + 1] = fmaf(Tb, P.bg[1], Cb1);
         image[3 * pid + 2] = fmaf(Tb, P.bg[2], Cb2);
@@ -291,7 +294,9 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
     __shared__ uint32_t s_max[THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31;
     const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
-    const int tx = tile % P.TW, ty = tile / P.TW;
+    const int view = tile / P.T, vt = tile - view * P.T;
+    const int64_t vbase = (int64_t)view * P.H * P.W;
+    const int tx = vt % P.TW, ty = vt / P.TW;
     // a thread owns PPT consecutive pixels of one row: they share dy and the row terms of `power`
     constexpr int TPR = TILE / PPT;                 // threads per tile row
     const int px0 = tx * TILE + (tid % TPR) * PPT;
@@ -312,7 +317,7 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
             n[k] = 0; t[h] = 0.0f; a0[h] = a1[h] = a2[h] = aD[h] = 0.0f;
             float gA = 0.0f;
             if (px < P.W && py < P.H) {
-                const int64_t pid = (int64_t)py * P.W + px;
+                const int64_t pid = vbase + (int64_t)py * P.W + px;
                 n[k] = n_contrib[pid];
                 t[h] = final_T[pid];
                 a0[h] = dL[3 * pid]; a1[h] = dL[3 * pid + 1]; a2[h] = dL[3 * pid + 2];
@@ -472,7 +477,7 @@ shade_record_kernel(int64_t N, const float2* __restrict__ mean2d, const float4* 
 }
 
 void make_raster_params(const xpr_camera* cam, const xpr_config* cfg, RasterParams& P) {
-    P.W = cam->width; P.H = cam->height; P.TW = tiles_x(cam);
+    P.W = cam->width; P.H = cam->height; P.TW = tiles_x(cam); P.T = tiles_x(cam) * tiles_y(cam);
     P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
     for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
     P.order = cfg->tile_order;
@@ -490,7 +495,7 @@ int32_t launch_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, cons
     if (N > 0 && (!aligned(shade_rec, 16) || !aligned(vals_sorted, 4))) return XPR_ERR_INVALID_ARG;
     RasterParams P;
     make_raster_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
+    const int T = tiles_x(cam) * tiles_y(cam) * num_views(cfg);
     // throughput shape once the image has enough tiles for several waves of every SM; branch-free blend when
     // the lists were culled
 #define XPR_FWD(PPT_, BF_)                                                                                          \
@@ -536,7 +541,7 @@ int32_t launch_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, cons
     }
     RasterParams P;
     make_raster_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
+    const int T = tiles_x(cam) * tiles_y(cam) * num_views(cfg);
     // 4 pixels per thread (64 threads) is the throughput shape; images with few tiles are bounded by their
     // heaviest tile, where more warps per tile (2 pixels per thread) shorten the critical path
 #define XPR_BWD(PPT_)                                                                                               \
@@ -593,7 +598,7 @@ extern "C" int32_t xpr_rasterize_stats(const xpr_camera* cam, const xpr_config* 
     if (N > 0 && (!aligned(shade_rec, 16) || !aligned(vals_sorted, 4))) return XPR_ERR_INVALID_ARG;
     RasterParams P;
     make_raster_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
+    const int T = tiles_x(cam) * tiles_y(cam) * num_views(cfg);
     XPR_CUDA(cudaMemsetAsync(stats, 0, 4 * sizeof(uint64_t), (cudaStream_t)stream));
     rasterize_fwd_kernel<true, 1, false, false><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
         P, reinterpret_cast<const float4*>(shade_rec), vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), nullptr,

@@ -20,22 +20,33 @@ class SplatPipeline:
     def __init__(self, N: int, cam, cfg: dict, pair_capacity: int | None = None, device="cuda:0"):
         self.N = int(N)
         self.device = torch.device(device)
-        self.cam = cam if isinstance(cam, xb.XprCamera) else xb.make_camera(cam)
+        # a list of cameras = a batch of views rendered by ONE call per stage (xpr_config.views; Table 2)
+        self.V = len(cam) if isinstance(cam, (list, tuple)) else 1
+        if self.V > 1:
+            self.cam = xb.make_cameras(cam)
+            cam0 = self.cam[0]
+            cfg = dict(cfg, views=self.V)
+        else:
+            cam = cam[0] if isinstance(cam, (list, tuple)) else cam
+            self.cam = cam if isinstance(cam, xb.XprCamera) else xb.make_camera(cam)
+            cam0 = self.cam
         self.ray_eval = bool(cfg.get("ray_eval", 0)) if isinstance(cfg, dict) else False
         # f3: the compositing pass also renders the depth image and the accumulated opacity (2D evaluation only)
         self.features = bool(cfg.get("features", 0)) if isinstance(cfg, dict) else False
         if self.features and self.ray_eval:
             raise ValueError("xpr: rendered features (f3) are built for the 2D evaluation, not for ray_eval")
+        if self.V > 1 and (self.features or self.ray_eval):
+            raise ValueError("xpr: a batch of views is built for the colour pass of the 2D evaluation")
         self._dL = None
         # f3: constant (dL/dD, dL/dA) of a loss that is linear in the features; step_async() feeds them to the backward
         self.feature_grads = None
         self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
         self.K = (int(self.cfg.sh_degree) + 1) ** 2
-        self.W, self.H = int(self.cam.width), int(self.cam.height)
-        self.TW, self.TH = xb.num_tiles(self.cam, self.cfg)
-        self.T = self.TW * self.TH
+        self.W, self.H = int(cam0.width), int(cam0.height)
+        self.TW, self.TH = xb.num_tiles(cam0, self.cfg)
+        self.T = self.TW * self.TH * self.V           # tiles of all views (tile id of view v: v T_view + t)
         d, f32, i32 = self.device, torch.float32, torch.int32
-        N = self.N
+        N = self.N * self.V                           # per-(view, Gaussian) arrays, view-major
         e = lambda *s, dtype=f32: torch.empty(*s, dtype=dtype, device=d)
         # projection outputs (a1-a3)
         self.mean2d, self.conic_opac, self.rgb = e(N, 2), e(N, 4), e(N, 3)
@@ -56,8 +67,9 @@ class SplatPipeline:
         self.num_pairs = 0
         self._alloc_pairs(int(pair_capacity) if pair_capacity else max(1 << 16, 8 * N))
         # compositing outputs (a8)
-        self.image, self.final_T = e(self.H, self.W, 3), e(self.H, self.W)
-        self.n_contrib = e(self.H, self.W, dtype=i32)
+        vshape = (self.V,) if self.V > 1 else ()
+        self.image, self.final_T = e(*vshape, self.H, self.W, 3), e(*vshape, self.H, self.W)
+        self.n_contrib = e(*vshape, self.H, self.W, dtype=i32)
         # gradients (a9, a10)
         # the compositing gradients share one allocation, in the order the library checks for, so that
         # xpr_rasterize_bwd zero-fills them with a single memset
@@ -67,6 +79,7 @@ class SplatPipeline:
         if self.features:
             self.depth_img, self.alpha_img = e(self.H, self.W), e(self.H, self.W)
         # the parameter gradients share one allocation, in the order the library checks for (one zero-fill in xpr_project_bwd)
+        N = self.N                                     # (summed over the views of a batch)
         K3 = 3 * self.K
         g4 = e((11 + K3) * N)
         self.g_means, self.g_scales = g4[:3 * N].view(N, 3), g4[3 * N:6 * N].view(N, 3)
@@ -87,7 +100,7 @@ class SplatPipeline:
         d = self.device
         self.keys_sorted = torch.empty(max(cap, 1), dtype=torch.int64, device=d)
         self.vals_sorted = torch.empty(max(cap, 1), dtype=torch.int32, device=d)
-        ws = xb.xpr_bin_sort_workspace(self.N, cap, self.T)
+        ws = xb.xpr_bin_sort_workspace(self.N * self.V, cap, self.T)
         self.workspace = torch.empty(ws, dtype=torch.uint8, device=d)
 
     # ---- stages ------------------------------------------------------------------------------

@@ -35,7 +35,7 @@ def test_header_symbols_all_exported(lib):
 def test_struct_layout_matches_header():
     from paper_2606_11529_b200 import binding
     assert C.sizeof(binding.XprCamera) == 3 * 4 + 4 * 4 + 4 * 4 + 12 * 4
-    assert C.sizeof(binding.XprConfig) == 4 * 4 + 8 * 4 + 3 * 4 + 4 + 8     # + tile_order pointer
+    assert C.sizeof(binding.XprConfig) == 4 * 4 + 8 * 4 + 3 * 4 + 4 + 8 + 8     # + tile_order pointer, views (+ padding)
     assert binding.XprConfig.tile_order.offset == 64
 
 
@@ -78,6 +78,11 @@ def test_invalid_arguments_rejected_before_launch(lib):
     st = lib.xpr_project_bwd(C.c_int64(0), null, null, null, null, null, C.byref(cam4), C.byref(cfg4), null, null,
                              null, null, null, null, null, null, null, null, null, null)
     assert st == xb.XPR_ERR_INVALID_ARG
+    # a batch of views: at most XPR_MAX_VIEWS = 8, negative counts are invalid
+    cam5, cfg5 = _cam_cfg(views=9)
+    assert lib.xpr_rasterize_fwd(C.byref(cam5), C.byref(cfg5), C.c_int64(0), null, null, null, null, null, null, null) == xb.XPR_ERR_UNSUPPORTED
+    cam6, cfg6 = _cam_cfg(views=-1)
+    assert lib.xpr_rasterize_fwd(C.byref(cam6), C.byref(cfg6), C.c_int64(0), null, null, null, null, null, null, null) == xb.XPR_ERR_INVALID_ARG
     # misaligned workspace
     n = C.c_int64(0)
     st = lib.xpr_bin_sort(C.c_int64(0), null, null, null, C.byref(cam), C.byref(cfg), C.c_int64(0), null, null,

@@ -60,3 +60,9 @@ def test_bench_line_reports_n_channel_feature_timings():
     d = _run("--featn", "5", "--no-cpu-baseline", "--no-e2e", "--no-graph")
     assert d["featn"]["C"] == 5 and d["featn"]["fwd_ms"] > 0 and d["featn"]["bwd_ms"] > 0
     assert d["gpu_launches"] == 3 * 16          # the step itself is unchanged
+
+
+def test_bench_line_batch_of_views():
+    d = _run("--config", "5", "--views", "2", "--no-cpu-baseline", "--no-e2e", "--no-graph")
+    assert d["config"]["views"] == 2 and d["value"] > 0
+    assert d["gpu_launches"] == 3 * 16          # a batch of views costs the launches of one view

@@ -211,3 +211,37 @@ def test_gradient_mass_bounds_gradient_and_equals_it_for_sign_definite_terms():
     mp = xo.rasterize_bwd(r["proj"], r["binned"], r["fwd"], np.abs(dL), cam, cfg, np.float64, mass=True)
     np.testing.assert_allclose(mp["g_rgb"], gp["g_rgb"], rtol=1e-13, atol=0)
     np.testing.assert_allclose(m["g_rgb"], gp["g_rgb"], rtol=1e-13, atol=0)   # mass depends on |dL| only
+
+
+def test_p6_fd_batch_of_views_is_the_gradient_of_the_summed_loss():
+    """Batch of views (Table 2): the loss of a batch is the sum of the views' losses, so its gradient is
+    pinned by central finite differences of that SUM through two forwards with different cameras (never by adding up
+    backward formulas)."""
+    def make(seed):
+        cams = [xo.make_camera(cam_obj(w2c=scenes.look_at(e, (0.0, 0.1, 3.0)).astype(np.float64), cx=19.0, cy=13.5))
+                for e in ((0.3, -0.2, -1.0), (-0.6, 0.3, -0.4))]
+        arr = draw_scene(2100 + seed, 5, 4, z=(1.5, 4.5))
+        Gws = [np.random.default_rng(10 * seed + v).normal(0, 1, (24, 40, 3)) for v in range(2)]
+        return arr, cams, xo.make_config(cfg_dict(sh_degree=1), fragile_rel=1e-4), Gws
+
+    for seed in range(40):
+        arr, cams, cfg, Gws = make(seed)
+        rs = xo.render_views(arr, cams, cfg, np.float64)
+        if all((r["fwd"]["fragile"] == 0).all() and (r["proj"]["tile_count"] > 0).sum() >= 4 for r in rs):
+            break
+    else:
+        raise AssertionError("no suitable seed")
+    loss = lambda a: sum(float((r["fwd"]["image"] * G).sum()) for r, G in zip(xo.render_views(a, cams, cfg, np.float64), Gws))
+    g = xo.backward_views(arr, rs, Gws, cams, cfg, np.float64)
+    names = dict(means="g_means", scales="g_scales", quats="g_quats", opacities="g_opacities", sh="g_sh")
+    scale_all = max(np.abs(g[n]).max() for n in names.values())
+    for k, n in names.items():
+        base, an = arr[k], g[n]
+        it = np.nditer(base, flags=["multi_index"])
+        for _ in it:
+            idx = it.multi_index
+            h = 1e-6 * max(1.0, abs(base[idx])) if k != "scales" else 1e-5 * abs(base[idx])
+            ap = {kk: v.copy() for kk, v in arr.items()}; ap[k][idx] += h
+            am = {kk: v.copy() for kk, v in arr.items()}; am[k][idx] -= h
+            fd = (loss(ap) - loss(am)) / (2 * h)
+            assert abs(fd - an[idx]) <= 2e-6 * max(abs(fd), abs(an[idx])) + 1e-7 * scale_all + 1e-9, (k, idx, fd, an[idx])
