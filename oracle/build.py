@@ -17,7 +17,7 @@ FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
 
 
 def build(force: bool = False) -> str:
-    deps = [SRC, os.path.join(HERE, "xpr_oracle_ray.inc"), os.path.join(HERE, "xpr_oracle_feat.inc"), os.path.join(HERE, "xpr_oracle.h"), os.path.abspath(__file__)]
+    deps = [SRC, os.path.join(HERE, "xpr_oracle_ray.inc"), os.path.join(HERE, "xpr_oracle_feat.inc"), os.path.join(HERE, "xpr_oracle_lin.inc"), os.path.join(HERE, "xpr_oracle.h"), os.path.abspath(__file__)]
     if not force and os.path.exists(OUT) and all(os.path.getmtime(OUT) >= os.path.getmtime(d) for d in deps):
         return OUT
     cmd = ["g++", *FLAGS, "-o", OUT, SRC]

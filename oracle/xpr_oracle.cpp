@@ -13,6 +13,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <limits>
 #include <numeric>
 #include <vector>
 #ifdef _OPENMP
@@ -902,3 +903,6 @@ extern "C" int32_t xpr_oracle_num_threads(void) {
 
 // rendered depth and accumulated opacity
 #include "xpr_oracle_feat.inc"
+
+// XPR-LinPrim
+#include "xpr_oracle_lin.inc"

@@ -494,3 +494,77 @@ def backward_da(scene_arrays: dict, r: dict, dL_dimage, dL_ddepth, dL_dalpha, ca
     g3["g_means"] = g3["g_means"] + depth_bwd(r["proj"]["tile_count"], g2["g_depth"], cam)
     g3.update(g2)
     return g3
+
+
+# ---- XPR-LinPrim (xpr_oracle_lin.inc; PAPER A.1.3 L506-697) ----------------------------------------
+
+def lin_project(means, scales, quats, opacities, sh, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """lin_rec [N,20] = (mu2D 2, sigma, depth | (kx, ky, h) of the four slab pairs | rgb, 0); depth = |p|."""
+    dt = np.dtype(dtype)
+    N = int(means.shape[0])
+    a = [np.ascontiguousarray(x, dt) for x in (means, scales, quats, opacities, sh)]
+    out = dict(lin_rec=np.empty((N, 20), dt), depth=np.empty(N, dt), tile_rect=np.empty((N, 4), np.int32),
+               tile_count=np.empty(N, np.uint32))
+    getattr(lib(), "xpr_oracle_lin_project_" + _sfx(dt))(
+        C.c_int64(N), *[_p(x) for x in a], C.byref(cam), C.byref(cfg), _p(out["lin_rec"]), _p(out["depth"]),
+        _p(out["tile_rect"]), _p(out["tile_count"]))
+    return out
+
+
+def lin_chord(rec20, pix_xy, dtype=np.float64):
+    """sigma * (tau_exit - tau_enter) of one primitive at pixel-centre positions pix_xy [n,2] (0 where the ray misses)."""
+    dt = np.dtype(dtype)
+    r = np.ascontiguousarray(rec20, dt)
+    p = np.ascontiguousarray(pix_xy, dt).reshape(-1, 2)
+    out = np.empty(len(p), dt)
+    getattr(lib(), "xpr_oracle_lin_chord_" + _sfx(dt))(_p(r), C.c_int64(len(p)), _p(p), _p(out))
+    return out
+
+
+def lin_tile_keep(rec20, tile_xy, cfg: XoConfig, dtype=np.float32):
+    dt = np.dtype(dtype)
+    r = np.ascontiguousarray(rec20, dt)
+    t = np.ascontiguousarray(tile_xy, np.int32).reshape(-1, 2)
+    keep = np.zeros(len(t), np.uint8)
+    getattr(lib(), "xpr_oracle_lin_tile_keep_" + _sfx(dt))(_p(r), C.c_int64(len(t)), _p(t), C.c_int32(cfg.tile), C.byref(cfg), _p(keep))
+    return keep.astype(bool)
+
+
+def lin_bin_sort(proj: dict, cam: XoCamera, cfg: XoConfig) -> dict:
+    lib().xpr_oracle_lin_bin_sort.restype = C.c_int64
+    tx, ty = tiles(cam, cfg)
+    N = int(proj["tile_count"].shape[0])
+    depth = np.ascontiguousarray(proj["depth"], np.float32)
+    rec = np.ascontiguousarray(proj["lin_rec"], np.float32)
+    I = int(proj["tile_count"].astype(np.int64).sum())
+    keys, vals = np.empty(I, np.uint64), np.empty(I, np.uint32)
+    ranges = np.zeros((tx * ty, 2), np.uint32)
+    n = lib().xpr_oracle_lin_bin_sort(C.c_int64(N), _p(depth), _p(proj["tile_rect"]), _p(proj["tile_count"]), _p(rec),
+                                      C.byref(cfg), C.c_int32(tx), C.c_int32(ty), C.c_int32(int(cfg.tile_cull)),
+                                      C.c_int64(I), _p(keys), _p(vals), _p(ranges))
+    assert n <= I
+    return dict(keys=keys[:n].copy(), vals=vals[:n].copy(), ranges=ranges, num_pairs=int(n), num_candidates=I)
+
+
+def lin_rasterize_fwd(proj: dict, binned: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    H, W = int(cam.height), int(cam.width)
+    N = int(proj["tile_count"].shape[0])
+    rec = np.ascontiguousarray(proj["lin_rec"], dt)
+    out = dict(image=np.empty((H, W, 3), dt), final_T=np.empty((H, W), dt), n_contrib=np.empty((H, W), np.uint32),
+               fragile=np.empty((H, W), np.uint8))
+    counters = np.zeros(2, np.int64)
+    getattr(lib(), "xpr_oracle_lin_rasterize_fwd_" + _sfx(dt))(
+        C.byref(cam), C.byref(cfg), C.c_int64(N), _p(rec), _p(binned["vals"]), _p(binned["ranges"]), _p(out["image"]),
+        _p(out["final_T"]), _p(out["n_contrib"]), _p(out["fragile"]), _p(counters))
+    out["pp_visit"], out["pp_pass"] = int(counters[0]), int(counters[1])
+    return out
+
+
+def render_lin(scene_arrays: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """XPR-LinPrim forward: project -> bin_sort (Eq. 2 cull when cfg.tile_cull) -> compositing with Beer-Lambert alpha."""
+    s = scene_arrays
+    proj = lin_project(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, dtype)
+    binned = lin_bin_sort(proj, cam, cfg)
+    fwd = lin_rasterize_fwd(proj, binned, cam, cfg, dtype)
+    return dict(proj=proj, binned=binned, fwd=fwd)
