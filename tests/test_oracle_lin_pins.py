@@ -163,7 +163,7 @@ def test_p18c_image_unchanged_by_tile_cull_and_invariants():
     np.testing.assert_array_equal(r0["fwd"]["image"], r1["fwd"]["image"])
     np.testing.assert_array_equal(r0["fwd"]["final_T"], r1["fwd"]["final_T"])
     # P2 analogue: rgb = 1, bg = 0 => image = 1 - final_T (sum alpha_k T_k telescopes)
-    arr1 = dict(arr, sh=np.zeros_like(sc.sh)); arr1["sh"][:, 0, :] = 0.5 / C0
+    arr1 = dict(arr, sh=np.full((sc.N, 1, 3), 0.5 / C0, np.float32))
     r = xo.render_lin(arr1, cam, xo.make_config(dict(d, tile_cull=1, sh_degree=0)), np.float64)
     np.testing.assert_allclose(r["fwd"]["image"][..., 0], 1 - r["fwd"]["final_T"], atol=1e-12)
     assert (r["fwd"]["final_T"] < 0.9).any()
