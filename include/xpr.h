@@ -314,6 +314,56 @@ int32_t xpr_rasterize_featn_bwd(const xpr_camera* cam, const xpr_config* cfg, in
                                 int32_t zero_init, void* stream);
 
 /*
+ * ---- XPR-LinPrim (PAPER A.1.3 L506-697, Listings 4-5, Eq. 2): forward path ----
+ * Primitive: the octahedron {x : |S^-1 R^T (x - mu)|_1 <= 1} with homogeneous density
+ * sigma = -log(1 - 0.99 o) / (2 min(s)) (L506-524); alpha = 1 - exp(-sigma (tau_exit - tau_enter)) (L528).
+ * The body of the paper's `project` listing is lost in the extraction (L545-560); DESIGN.md section 3 readings L1-L6
+ * fill it and both sides (oracle/xpr_oracle_lin.inc, these kernels) follow them.
+ *
+ * xpr_lin_project -- Vertex-shader stage: p = W mu + t, dist = |p| (the sort depth, "Euclidean depth" L532, L2),
+ *   A = J W R diag(s) with J = (d pixel / dp of the pinhole; p^T / |p|) (L534-536, L1), the projected octahedron
+ *   {|A^-1 (p2D - mu2D, tau)|_1 <= 1} written as four slab pairs with normals n = c0 +- c1 +- c2, c_k the rows of
+ *   A^-1 (L538-542): tau in [m_i - h_i, m_i + h_i], m_i = -(kx_i dx + ky_i dy), kx = n_x / n_z, ky = n_y / n_z,
+ *   h = 1 / |n_z| (h = +inf when |n_z| < 1e-12: the slab does not bound tau, L566, L4); footprint = the exact
+ *   axis-aligned box of the shadow, half extents max_j |A[0][j]|, max_j |A[1][j]| (L3); colour as xpr_project (C5).
+ *   in : means[N,3], scales[N,3] (activated, > 0), quats[N,4] (w,x,y,z; normalised inside), opacities[N] in [0,1),
+ *        sh[N,K,3]; cam: ONE pinhole camera (fisheye, cfg->views > 1 -> XPR_ERR_UNSUPPORTED).
+ *   out: lin_rec[N,20] fp32, 16-byte aligned = (mu2D.x, mu2D.y, sigma, dist | (kx_i, ky_i, h_i) i = 0..3 | r, g, b, 0),
+ *        all 0 for a culled primitive; depth[N] = dist; tile_rect[N,4], tile_count[N] as xpr_project.
+ *   Culled: p_z <= z_near, non-finite record, empty rectangle.
+ *
+ * xpr_bin_sort_lin -- xpr_bin_sort for LinPrim pairs; with cfg->tile_cull != 0 a candidate (primitive, tile) is kept
+ *   iff Eq. 2's upper bound of the chord over the tile (corners x0 = 16 tx + 1/2, x1 = 16 (tx + 1) + 1/2 as the listing
+ *   prints them, L6; bound = max(0, min_{i,j} max_corners (m_i - m_j) + h_i + h_j)) gives sigma dtau >= -log(1 -
+ *   alpha_thresh) (L589-612, L633-676).  The bound is a minimum of functions convex in the tile position, so along one
+ *   tile row the kept tiles form ONE interval: the call shrinks each row of the rectangle from both ends.
+ *   Arguments, capacity contract and error behaviour as xpr_bin_sort_cull, with lin_rec in place of the tile-cull data.
+ *
+ * xpr_lin_rasterize_fwd -- Shader stage (Alg. 1; evaluate L618-629): per pixel, front to back over the tile's
+ *   list: x = sigma (min_i (m_i + h_i) - max_i (m_i - h_i)) or 0 when that is not positive; skip when
+ *   x < -log(1 - alpha_thresh) (decided on x, rule R3); alpha = min(alpha_max, 1 - exp(-x)); T' = T (1 - alpha); stop
+ *   WITHOUT blending if T' < t_min; C += rgb alpha T; T = T'; finally C += T bg (L5: the common rules C11-C13).
+ *   out: image[H,W,3], final_T[H,W], n_contrib[H,W] (1-based list position of the last blended primitive).
+ * xpr_lin_rasterize_stats -- the same walk, no image: stats[4] (DEVICE uint64) = {(pixel, primitive) evaluations,
+ *   those that pass the gate, those blended, sum of n_contrib}.
+ * Errors (all four): null cam / cfg, N < 0, misaligned pointer -> XPR_ERR_INVALID_ARG; cfg->tile != 16, a fisheye
+ *   camera or cfg->views > 1 -> XPR_ERR_UNSUPPORTED; nothing is launched in either case.
+ * The backward pass of LinPrim is not part of this library.
+ */
+int32_t xpr_lin_project(int64_t N, const float* means, const float* scales, const float* quats, const float* opacities,
+                        const float* sh, const xpr_camera* cam, const xpr_config* cfg, float* lin_rec, float* depth,
+                        int32_t* tile_rect, uint32_t* tile_count, void* stream);
+int32_t xpr_bin_sort_lin(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
+                         const float* lin_rec, const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
+                         uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges, int64_t* num_pairs_host,
+                         void* workspace, size_t workspace_bytes, void* stream);
+int32_t xpr_lin_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* lin_rec,
+                              const uint32_t* vals_sorted, const uint32_t* tile_ranges, float* image, float* final_T,
+                              uint32_t* n_contrib, void* stream);
+int32_t xpr_lin_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* lin_rec,
+                                const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats, void* stream);
+
+/*
  * xpr_loss_grad -- convenience for the caller's side of the step (reading C21: the loss lives outside the path):
  * dL/dimage of the two losses BASELINE.json's configs name, as sums over all n = H*W*3 values, in one pass:
  *   kind 0: L = sum |I - target|    -> dL = sign(I - target);      kind 1: L = sum (I - target)^2 -> dL = 2 (I - target).

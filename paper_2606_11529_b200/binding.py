@@ -20,7 +20,8 @@ FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_R
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
            "xpr_shade_record", "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
-           "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad")
+           "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad",
+           "xpr_lin_project", "xpr_bin_sort_lin", "xpr_lin_rasterize_fwd", "xpr_lin_rasterize_stats")
 
 
 class XprCamera(C.Structure):
@@ -158,9 +159,10 @@ def xpr_bin_sort_workspace(N: int, pair_capacity: int, n_tiles: int) -> int:
 
 def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, pair_capacity: int, keys_sorted,
                  vals_sorted, tile_ranges, workspace, stream=None, raise_on_capacity: bool = True, sync: bool = True,
-                 cull_data=None):
+                 cull_data=None, lin_rec=None):
     """Returns (status, I).  On XPR_ERR_CAPACITY I is the required capacity.
     cull_data = (mean2d, conic_opac, lnv): call xpr_bin_sort_cull (tile_cull applied when cfg.tile_cull != 0).
+    lin_rec: call xpr_bin_sort_lin (LinPrim pairs; Eq. 2 bound when cfg.tile_cull != 0).
     sync=False: num_pairs_host = NULL -- nothing waits for the host, I is returned as None and stays in the
     first 8 bytes of `workspace` (xpr.h); the caller checks it against pair_capacity later."""
     N = int(tile_count.shape[0])
@@ -168,7 +170,9 @@ def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, p
     tail = (C.byref(cam), C.byref(cfg), C.c_int64(pair_capacity), _p(keys_sorted, _I64), _p(vals_sorted, _I32), _p(tile_ranges, _I32),
             C.byref(n_pairs) if sync else None, _p(workspace, _U8), C.c_size_t(workspace.numel() * workspace.element_size()),
             _stream(stream))
-    if cull_data is None:
+    if lin_rec is not None:
+        st = lib().xpr_bin_sort_lin(C.c_int64(N), _p(depth, _F32), _p(tile_rect, _I32), _p(tile_count, _I32), _p(lin_rec, _F32), *tail)
+    elif cull_data is None:
         st = lib().xpr_bin_sort(C.c_int64(N), _p(depth, _F32), _p(tile_rect, _I32), _p(tile_count, _I32), *tail)
     else:
         st = lib().xpr_bin_sort_cull(C.c_int64(N), _p(depth, _F32), _p(tile_rect, _I32), _p(tile_count, _I32), _p(cull_data[0], _F32),
@@ -305,6 +309,29 @@ def xpr_rasterize_featn_bwd(cam: XprCamera, cfg: XprConfig, mean2d, conic_opac, 
                                          _p(n_contrib, _I32), _p(dL_dfeat, _F32), _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32),
                                          _p(g_feat, _F32), C.c_int32(int(zero_init)), _stream(stream)),
            "xpr_rasterize_featn_bwd")
+
+
+def xpr_lin_project(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, lin_rec, depth, tile_rect,
+                    tile_count, stream=None):
+    N = int(means.shape[0])
+    _check(lib().xpr_lin_project(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), _p(opacities, _F32),
+                                 _p(sh, _F32), C.byref(cam), C.byref(cfg), _p(lin_rec, _F32), _p(depth, _F32),
+                                 _p(tile_rect, _I32), _p(tile_count, _I32), _stream(stream)), "xpr_lin_project")
+
+
+def xpr_lin_rasterize_fwd(cam: XprCamera, cfg: XprConfig, lin_rec, vals_sorted, tile_ranges, image, final_T, n_contrib,
+                          stream=None):
+    N = int(lin_rec.shape[0])
+    _check(lib().xpr_lin_rasterize_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(lin_rec, _F32), _p(vals_sorted, _I32),
+                                       _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32), _p(n_contrib, _I32),
+                                       _stream(stream)), "xpr_lin_rasterize_fwd")
+
+
+def xpr_lin_rasterize_stats(cam: XprCamera, cfg: XprConfig, lin_rec, vals_sorted, tile_ranges, stats, stream=None):
+    N = int(lin_rec.shape[0])
+    _check(lib().xpr_lin_rasterize_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(lin_rec, _F32),
+                                         _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(stats, _I64), _stream(stream)),
+           "xpr_lin_rasterize_stats")
 
 
 def xpr_loss_grad(kind: str, image, target, dL_dimage, stream=None):

@@ -29,6 +29,7 @@ SOURCES = {
     "ray.cu": ["-fmad=false"],
     "rasterize_ray.cu": [],
     "rasterize_feat.cu": [],
+    "rasterize_lin.cu": [],
 }
 
 

@@ -580,12 +580,42 @@ __device__ __forceinline__ float approx_sqrt(float x) {   // the interval estima
 }
 
 constexpr int ROW_SMEM = 2048;     // tile rows whose first-tile counter is kept in shared memory
-template <bool CULL>
+// XPR-LinPrim's tile_cull (Eq. 2; reading L6): the bound on the chord over the tile,
+//   dt_upper = max(0, min over the 16 ordered slab pairs of h_i + h_j + max over the 4 corners of (m_i - m_j)),
+// keeps the pair iff sigma dt_upper >= -log(1 - alpha_thresh).  rec = lin_rec of the primitive (20 floats).  Every
+// operation individually rounded, order as the oracle's.  m_i - m_j is affine in the tile position, so the kept tiles
+// are the intersection of half-planes: convex, one interval per tile row.
+__device__ __forceinline__ bool lin_tile_keep(const float* __restrict__ rec, int tx, int ty, float req) {
+    const float ts = (float)TILE, mx = rec[0], my = rec[1];
+    const float x0 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)tx), 0.5f), mx), x1 = __fsub_rn(__fadd_rn(__fadd_rn(__fmul_rn(ts, (float)tx), ts), 0.5f), mx);
+    const float y0 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)ty), 0.5f), my), y1 = __fsub_rn(__fadd_rn(__fadd_rn(__fmul_rn(ts, (float)ty), ts), 0.5f), my);
+    float mc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float kx = rec[4 + 3 * i], ky = rec[5 + 3 * i];
+        mc[i][0] = -__fmaf_rn(kx, x0, __fmul_rn(ky, y0)); mc[i][1] = -__fmaf_rn(kx, x1, __fmul_rn(ky, y0));
+        mc[i][2] = -__fmaf_rn(kx, x0, __fmul_rn(ky, y1)); mc[i][3] = -__fmaf_rn(kx, x1, __fmul_rn(ky, y1));
+    }
+    float best = INFINITY;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            float d = __fsub_rn(mc[i][0], mc[j][0]);
+#pragma unroll
+            for (int c = 1; c < 4; ++c) d = fmaxf(d, __fsub_rn(mc[i][c], mc[j][c]));
+            best = fminf(best, __fadd_rn(__fadd_rn(d, rec[6 + 3 * i]), rec[6 + 3 * j]));
+        }
+    const float dt_upper = fmaxf(0.0f, best);
+    return !(__fmul_rn(rec[2], dt_upper) < req);
+}
+
+template <int CULL>
 __global__ void __launch_bounds__(128)
 rows_kernel(int TW, int TH, int TH_view, const uint32_t* __restrict__ vidx, const uint32_t* __restrict__ row_base,
             const int4* __restrict__ rect, const float2* __restrict__ mean2d, const float4* __restrict__ conic_opac,
-            const float* __restrict__ lnv, const Header* __restrict__ hdr, uint32_t* __restrict__ row_tab,
-            int* __restrict__ tile_diff) {
+            const float* __restrict__ lnv, const float* __restrict__ lin_rec, float lin_req,
+            const Header* __restrict__ hdr, uint32_t* __restrict__ row_tab, int* __restrict__ tile_diff) {
     // one thread per row (grid-stride, a warp takes 32 consecutive rows).  The Gaussian of a row is the last one
     // whose first row is <= row: the warp finds it for its first row with a cooperative 32-ary search in the
     // strictly increasing row_base (4 dependent loads for 10^6 Gaussians instead of 20), loads the next 32 bases
@@ -626,14 +656,20 @@ rows_kernel(int TW, int TH, int TH_view, const uint32_t* __restrict__ vidx, cons
         const int4 r = rect[g];
         const int ty = r.y + (int)(row - row_base[s]);
         float mx = 0.f, my = 0.f, A = 0.f, B = 0.f, C = 0.f, L = 0.f, ext = 0.f, det = 0.f;
-        if (CULL) {
+        if (CULL == 1) {
             const float2 m = mean2d[g]; const float4 co = conic_opac[g];
             mx = m.x; my = m.y; A = co.x; B = co.y; C = co.z; L = lnv[g];
             det = A * C - B * B;
             ext = approx_sqrt(fmaxf(__fdividef(2.0f * L * C, det), 0.0f));   // half-width of the ellipse {q = L} in x
         }
         int xa = r.x, xb = r.z;                                 // kept tiles of this row: [xa, xb)
-        if (CULL) {
+        if (CULL == 2) {
+            // LinPrim: the kept tiles of the row are an interval (convexity above): its first and last tile by the exact predicate
+            const float* rec = lin_rec + 20 * (size_t)g;
+            while (xa < xb && !lin_tile_keep(rec, xa, ty, lin_req)) ++xa;
+            while (xb > xa && !lin_tile_keep(rec, xb - 1, ty, lin_req)) --xb;
+        }
+        if (CULL == 1) {
             const int tyv = ty % TH_view;              // batch of views: the tile rows of view v are offset by v * TH_view
             const auto keep = [&](int tx) { return tile_keep(mx, my, A, B, C, L, (uint32_t)tx, (uint32_t)tyv); };
             // estimate: x extent of {q <= L} over dy in [lo, hi] (pixel-centre hull of the row)
@@ -1159,6 +1195,7 @@ static cudaError_t launch_pass(unsigned tiles, cudaStream_t st, const uint32_t* 
 // Common body of xpr_bin_sort (cull == false; the cull-data pointers are unused) and xpr_bin_sort_cull.
 static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int32_t* tile_rect,
                              const uint32_t* tile_count, const float* mean2d, const float* conic_opac, const float* lnv,
+                             const float* lin_rec,
                              const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
                              uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
                              int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream) {
@@ -1240,11 +1277,14 @@ static int32_t bin_sort_impl(bool cull, int64_t N, const float* depth, const int
     // 4. rows: surviving interval per (Gaussian, tile row) -> row table + difference array over the tile ids
     const unsigned rgrid = 148u * 16u;                               // grid-stride over the rows (count on the device)
     if (cull)
-        rows_kernel<true><<<rgrid, 128, 0, st>>>(TW, TH, TH_view, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
-                                                 reinterpret_cast<const float4*>(conic_opac), lnv, hdr, row_tab, tile_diff);
+        rows_kernel<1><<<rgrid, 128, 0, st>>>(TW, TH, TH_view, vidx[0], row_base, rect4, reinterpret_cast<const float2*>(mean2d),
+                                              reinterpret_cast<const float4*>(conic_opac), lnv, nullptr, 0.0f, hdr, row_tab, tile_diff);
+    else if (lin_rec && cfg->tile_cull != 0)
+        rows_kernel<2><<<rgrid, 128, 0, st>>>(TW, TH, TH_view, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, lin_rec,
+                                              (float)(-log(1.0 - (double)cfg->alpha_thresh)), hdr, row_tab, tile_diff);
     else
-        rows_kernel<false><<<rgrid, 128, 0, st>>>(TW, TH, TH_view, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, hdr, row_tab,
-                                                  tile_diff);
+        rows_kernel<0><<<rgrid, 128, 0, st>>>(TW, TH, TH_view, vidx[0], row_base, rect4, nullptr, nullptr, nullptr, nullptr, 0.0f,
+                                              hdr, row_tab, tile_diff);
     XPR_LAUNCH_CHECK();
     // 5. supertile words in rank order; pass p of the supertile sort reads buffer p and writes buffer p + 1, the
     //    last one writes the half buffer (keys_sorted is free until the final pass)
@@ -1305,7 +1345,7 @@ extern "C" int32_t xpr_bin_sort(int64_t N, const float* depth, const int32_t* ti
                                 uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
                                 int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (cfg && cfg->tile_cull != 0) return XPR_ERR_INVALID_ARG;     // tile_cull needs the cull data: xpr_bin_sort_cull
-    return bin_sort_impl(false, N, depth, tile_rect, tile_count, nullptr, nullptr, nullptr, cam, cfg, pair_capacity,
+    return bin_sort_impl(false, N, depth, tile_rect, tile_count, nullptr, nullptr, nullptr, nullptr, cam, cfg, pair_capacity,
                          keys_sorted, vals_sorted, tile_ranges, num_pairs_host, workspace, workspace_bytes, stream);
 }
 
@@ -1316,6 +1356,19 @@ extern "C" int32_t xpr_bin_sort_cull(int64_t N, const float* depth, const int32_
                                      uint32_t* tile_ranges, int64_t* num_pairs_host, void* workspace,
                                      size_t workspace_bytes, void* stream) {
     const bool cull = cfg && cfg->tile_cull != 0;
-    return bin_sort_impl(cull, N, depth, tile_rect, tile_count, mean2d, conic_opac, lnv, cam, cfg, pair_capacity,
+    return bin_sort_impl(cull, N, depth, tile_rect, tile_count, mean2d, conic_opac, lnv, nullptr, cam, cfg, pair_capacity,
+                         keys_sorted, vals_sorted, tile_ranges, num_pairs_host, workspace, workspace_bytes, stream);
+}
+
+// xpr_bin_sort for XPR-LinPrim: the same binning and sort; with cfg->tile_cull != 0 the pairs are culled
+// with the per-tile chord bound of Eq. 2 read from lin_rec[N,20] of xpr_lin_project.
+extern "C" int32_t xpr_bin_sort_lin(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
+                                    const float* lin_rec, const xpr_camera* cam, const xpr_config* cfg,
+                                    int64_t pair_capacity, uint64_t* keys_sorted, uint32_t* vals_sorted,
+                                    uint32_t* tile_ranges, int64_t* num_pairs_host, void* workspace,
+                                    size_t workspace_bytes, void* stream) {
+    if (N > 0 && !aligned(lin_rec, 16)) return XPR_ERR_INVALID_ARG;
+    if (cfg && num_views(cfg) != 1) return XPR_ERR_UNSUPPORTED;
+    return bin_sort_impl(false, N, depth, tile_rect, tile_count, nullptr, nullptr, nullptr, lin_rec, cam, cfg, pair_capacity,
                          keys_sorted, vals_sorted, tile_ranges, num_pairs_host, workspace, workspace_bytes, stream);
 }

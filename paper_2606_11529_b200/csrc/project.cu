@@ -370,6 +370,133 @@ project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __r
 }
 
 // ---------------------------------------------------------------------------------------------
+// XPR-LinPrim projection (PAPER A.1.3 L506-560, readings L1-L4 of DESIGN.md): octahedron
+// {x : |S^-1 R^T (x - mu)|_1 <= 1} with homogeneous density sigma = -log(1 - 0.99 o) / (2 min s).  The linear map from
+// the local frame to (pixel x, pixel y, Euclidean depth) is A = J W R diag(s), J = [d pixel / d p ; p^T / |p|]; the rows
+// c0, c1, c2 of A^-1 give the four slab pairs n_i = c0 +- c1 +- c2 of the projected octahedron.  The record holds, per
+// slab, kx = n_x / n_z, ky = n_y / n_z, h = 1 / |n_z|: tau in [m - h, m + h], m = -(kx dx + ky dy).  One thread per
+// primitive; fp32, every operation individually rounded (this file is compiled with -fmad=false), order as the oracle's.
+// lin_rec[N,20] = (mu2D 2, sigma, depth | (kx, ky, h) x 4 | r, g, b, 0).
+// ---------------------------------------------------------------------------------------------
+template <int K>
+__global__ void __launch_bounds__(128)
+lin_project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const float* __restrict__ scales,
+                   const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
+                   float4* __restrict__ lin_rec, float* __restrict__ depth, int32_t* __restrict__ rect,
+                   uint32_t* __restrict__ tcount) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
+    const float* W = P.W;
+    float p[3];
+    for (int a = 0; a < 3; ++a) p[a] = ((W[3 * a] * mu[0] + W[3 * a + 1] * mu[1]) + W[3 * a + 2] * mu[2]) + P.t[a];
+    bool vis = p[2] > P.z_near;
+    float rec[20];
+    int4 rc = make_int4(0, 0, 0, 0);
+    uint32_t tc = 0;
+    float dist = 0.0f;
+    if (vis) {
+        const float sc[3] = {__ldg(scales + 3 * i), __ldg(scales + 3 * i + 1), __ldg(scales + 3 * i + 2)};
+        const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
+        const float o = __ldg(opac + i);
+        const float x = p[0], y = p[1], z = p[2];
+        dist = sqrtf((x * x + y * y) + z * z);
+        const float u = x / z, v = y / z;
+        const float m0 = P.fx * u + P.cx, m1 = P.fy * v + P.cy;
+        float R[9];
+        {
+            const float w = q4.x, qx = q4.y, qy = q4.z, qz = q4.w;
+            const float xx = qx * qx, yy = qy * qy, zz = qz * qz, xy = qx * qy, xz = qx * qz, yz = qy * qz;
+            const float wx = w * qx, wy = w * qy, wz = w * qz;
+            R[0] = 1.0f - 2.0f * (yy + zz); R[1] = 2.0f * (xy - wz); R[2] = 2.0f * (xz + wy);
+            R[3] = 2.0f * (xy + wz); R[4] = 1.0f - 2.0f * (xx + zz); R[5] = 2.0f * (yz - wx);
+            R[6] = 2.0f * (xz - wy); R[7] = 2.0f * (yz + wx); R[8] = 1.0f - 2.0f * (xx + yy);
+        }
+        float Bm[9], A[9];
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                const float r0 = R[b] * sc[b], r1 = R[3 + b] * sc[b], r2 = R[6 + b] * sc[b];
+                Bm[3 * a + b] = (W[3 * a] * r0 + W[3 * a + 1] * r1) + W[3 * a + 2] * r2;
+            }
+        const float j00 = P.fx / z, j11 = P.fy / z;
+        const float J[9] = {j00, 0.0f, -(j00 * u), 0.0f, j11, -(j11 * v), x / dist, y / dist, z / dist};
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b)
+                A[3 * a + b] = (J[3 * a] * Bm[b] + J[3 * a + 1] * Bm[3 + b]) + J[3 * a + 2] * Bm[6 + b];
+        float cof[9];
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                const int a1 = (a + 1) % 3, a2 = (a + 2) % 3, b1 = (b + 1) % 3, b2 = (b + 2) % 3;
+                cof[3 * a + b] = A[3 * a1 + b1] * A[3 * a2 + b2] - A[3 * a1 + b2] * A[3 * a2 + b1];
+            }
+        const float det = (A[0] * cof[0] + A[1] * cof[1]) + A[2] * cof[2];
+        vis = (fabsf(det) > 0.0f) && isfinite(det);
+        float Ai[9];
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) Ai[3 * a + b] = cof[3 * b + a] / det;
+        const float smin = fminf(sc[0], fminf(sc[1], sc[2]));
+        const float sigma = (float)(-log(1.0 - 0.99 * (double)o) / (2.0 * (double)smin));     // R2
+        vis = vis && (sigma > 0.0f) && isfinite(sigma);
+        const float ex = fmaxf(fabsf(A[0]), fmaxf(fabsf(A[1]), fabsf(A[2])));
+        const float ey = fmaxf(fabsf(A[3]), fmaxf(fabsf(A[4]), fabsf(A[5])));
+        vis = vis && (fmaxf(ex, ey) > 0.0f);
+        if (vis) {
+            const float ts = (float)TILE;
+            rc.x = (int)fminf(fmaxf(floorf((m0 - ex) / ts), 0.0f), (float)P.TW);
+            rc.y = (int)fminf(fmaxf(floorf((m1 - ey) / ts), 0.0f), (float)P.TH);
+            rc.z = (int)fminf(fmaxf(ceilf((m0 + ex) / ts), 0.0f), (float)P.TW);
+            rc.w = (int)fminf(fmaxf(ceilf((m1 + ey) / ts), 0.0f), (float)P.TH);
+            const long long t2 = (long long)(rc.z - rc.x) * (long long)(rc.w - rc.y);
+            vis = t2 > 0;
+            tc = (uint32_t)t2;
+        }
+        if (vis) {
+            rec[0] = m0; rec[1] = m1; rec[2] = sigma; rec[3] = dist;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const bool p1 = s < 2, p2 = (s & 1) == 0;
+                float n[3];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) n[k] = (Ai[k] + (p1 ? Ai[3 + k] : -Ai[3 + k])) + (p2 ? Ai[6 + k] : -Ai[6 + k]);
+                float kx = 0.0f, ky = 0.0f, h = INFINITY;                                  // L4
+                if (fabs((double)n[2]) >= 1e-12) { const float inv = 1.0f / n[2]; kx = n[0] * inv; ky = n[1] * inv; h = fabsf(inv); }
+                rec[4 + 3 * s] = kx; rec[5 + 3 * s] = ky; rec[6 + 3 * s] = h;
+            }
+#pragma unroll
+            for (int k = 0; k < 16; ++k)
+                if (!isfinite(rec[k]) && !(k >= 4 && (k - 4) % 3 == 2)) vis = false;
+        }
+    }
+    if (!vis) {          // culled: an all-zero record (xpr.h)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) lin_rec[5 * i + k] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        depth[i] = 0.0f;
+        reinterpret_cast<int4*>(rect)[i] = make_int4(0, 0, 0, 0);
+        tcount[i] = 0u;
+        return;
+    }
+    float dir[3], dnorm, Y[16];
+    view_dir(P, mu, dir, dnorm);
+    sh_basis(dir[0], dir[1], dir[2], Y);
+    float c[3 * K];
+    load_sh<K>(sh, i, c);
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {
+        float acc = Y[0] * c[ch];
+#pragma unroll
+        for (int k = 1; k < K; ++k) acc = acc + Y[k] * c[3 * k + ch];
+        const float raw = acc + 0.5f;
+        rec[16 + ch] = (0.0f < raw) ? raw : 0.0f;
+    }
+    rec[19] = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) lin_rec[5 * i + k] = make_float4(rec[4 * k], rec[4 * k + 1], rec[4 * k + 2], rec[4 * k + 3]);
+    depth[i] = dist;
+    reinterpret_cast<int4*>(rect)[i] = rc;
+    tcount[i] = tc;
+}
+
+// ---------------------------------------------------------------------------------------------
 // Backward.  The forward intermediates are recomputed in fp32 exactly as above (so the clamp and
 // culling decisions are the forward's); the chain rule itself runs in fp64 (the kernel is HBM- and
 // latency-bound, not bound by the FP64 pipe, which runs at half the fp32 rate on B200), which keeps the ill-conditioned conic -> covariance
@@ -823,6 +950,34 @@ extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* s
     project_bwd_kernel<KK><<<blocks, PBWD_THREADS, 0, st>>>(N, P, ipt, means, scales, quats, opacities, sh, tile_count, \
                                                             flags, g_mean2d, g_conic, g_opac, g_rgb, g_means, g_scales, \
                                                             g_quats, g_opacities, g_sh)
+    switch (cfg->sh_degree) {
+        case 0: XPR_GO(1); break;
+        case 1: XPR_GO(4); break;
+        case 2: XPR_GO(9); break;
+        default: XPR_GO(16); break;
+    }
+#undef XPR_GO
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_lin_project(int64_t N, const float* means, const float* scales, const float* quats,
+                                   const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
+                                   float* lin_rec, float* depth, int32_t* tile_rect, uint32_t* tile_count, void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (cam->model != 0 || num_views(cfg) != 1) return XPR_ERR_UNSUPPORTED;      // LinPrim: pinhole, one view
+    if (N < 0 || N > 0x7fffffffLL) return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(means, 4) || !aligned(scales, 4) || !aligned(quats, 16) || !aligned(opacities, 4) || !aligned(sh, 16) ||
+        !aligned(lin_rec, 16) || !aligned(depth, 4) || !aligned(tile_rect, 16) || !aligned(tile_count, 4))
+        return XPR_ERR_INVALID_ARG;
+    ProjParams P;
+    if (int32_t s = make_params(cam, cfg, P)) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned blocks = (unsigned)((N + 127) / 128);
+#define XPR_GO(KK)                                                                                              \
+    lin_project_kernel<KK><<<blocks, 128, 0, st>>>(N, P, means, scales, quats, opacities, sh,                    \
+                                                   reinterpret_cast<float4*>(lin_rec), depth, tile_rect, tile_count)
     switch (cfg->sh_degree) {
         case 0: XPR_GO(1); break;
         case 1: XPR_GO(4); break;

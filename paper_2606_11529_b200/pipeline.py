@@ -282,3 +282,55 @@ def scene_to_device(scene, device="cuda:0"):
     """Upload a scenes.Scene's parameter arrays; returns (means, scales, quats, opacities, sh)."""
     t = lambda a: torch.from_numpy(a).to(device).contiguous()
     return t(scene.means), t(scene.scales), t(scene.quats), t(scene.opacities), t(scene.sh)
+
+
+class LinPrimPipeline:
+    """Forward path of XPR-LinPrim (PAPER A.1.3): xpr_lin_project -> xpr_bin_sort_lin ->
+    xpr_lin_rasterize_fwd.  Buffers and call order only, like SplatPipeline; one pinhole view."""
+
+    def __init__(self, N: int, cam, cfg: dict, pair_capacity: int | None = None, device="cuda:0"):
+        self.N = int(N)
+        self.device = torch.device(device)
+        self.cam = cam if isinstance(cam, xb.XprCamera) else xb.make_camera(cam)
+        self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
+        self.W, self.H = int(self.cam.width), int(self.cam.height)
+        self.TW, self.TH = xb.num_tiles(self.cam, self.cfg)
+        self.T = self.TW * self.TH
+        d, f32, i32 = self.device, torch.float32, torch.int32
+        e = lambda *s, dtype=f32: torch.empty(*s, dtype=dtype, device=d)
+        self.lin_rec, self.depth = e(self.N, 20), e(self.N)
+        self.tile_rect, self.tile_count = e(self.N, 4, dtype=i32), e(self.N, dtype=i32)
+        self.tile_ranges = e(self.T, 2, dtype=i32)
+        self.image, self.final_T = e(self.H, self.W, 3), e(self.H, self.W)
+        self.n_contrib = e(self.H, self.W, dtype=i32)
+        self.num_pairs = 0
+        self._alloc_pairs(int(pair_capacity) if pair_capacity else max(1 << 16, 8 * self.N))
+
+    _alloc_pairs = SplatPipeline._alloc_pairs
+    V = 1
+
+    def project(self, means, scales, quats, opacities, sh):
+        xb.xpr_lin_project(means, scales, quats, opacities, sh, self.cam, self.cfg, self.lin_rec, self.depth,
+                           self.tile_rect, self.tile_count)
+
+    def bin_sort(self):
+        while True:
+            st, n = xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg,
+                                    self.pair_capacity, self.keys_sorted, self.vals_sorted, self.tile_ranges,
+                                    self.workspace, raise_on_capacity=False, lin_rec=self.lin_rec)
+            if st == xb.XPR_OK:
+                self.num_pairs = n
+                return n
+            if n >= (1 << 30):
+                raise xb.XprError(st, "xpr_bin_sort_lin (pair count exceeds 2^30)")
+            self._alloc_pairs(int(n * 1.25) + 1024)
+
+    def rasterize_fwd(self):
+        xb.xpr_lin_rasterize_fwd(self.cam, self.cfg, self.lin_rec, self.vals_sorted, self.tile_ranges, self.image,
+                                 self.final_T, self.n_contrib)
+
+    def forward(self, means, scales, quats, opacities, sh):
+        self.project(means, scales, quats, opacities, sh)
+        self.bin_sort()
+        self.rasterize_fwd()
+        return self.image

@@ -200,3 +200,35 @@ def test_profiles_hold_text_summaries_only():
     for n in names:
         if n.endswith(".csv"):
             assert n in mds, n
+
+
+def test_linprim_entry_points_reject_bad_arguments(lib):
+    """f4 (xpr_lin_project, xpr_bin_sort_lin, xpr_lin_rasterize_fwd / _stats): the argument checks come before any launch."""
+    cam, cfg = _cam_cfg()
+    null, one, odd = C.c_void_p(0), C.c_void_p(16), C.c_void_p(20)
+    N4, N0, Nm = C.c_int64(4), C.c_int64(0), C.c_int64(-1)
+    # means scales quats opacities sh | cam cfg | lin_rec depth tile_rect tile_count
+    prj = lambda n, cm, cf, *a: lib.xpr_lin_project(n, *a[:5], cm, cf, *a[5:], null)
+    assert prj(Nm, C.byref(cam), C.byref(cfg), *[one] * 9) == 1
+    assert prj(N4, None, C.byref(cfg), *[one] * 9) == 1
+    assert prj(N4, C.byref(cam), C.byref(cfg), *[one] * 5, odd, one, one, one) == 1           # lin_rec needs 16 B
+    assert prj(N4, C.byref(cam), C.byref(cfg), null, *[one] * 8) == 1                         # means NULL
+    assert prj(N0, C.byref(cam), C.byref(cfg), *[null] * 9) == 0                              # N = 0: nothing to do
+    fish = type(cam)(); C.memmove(C.byref(fish), C.byref(cam), C.sizeof(cam)); fish.model = 1
+    assert prj(N4, C.byref(fish), C.byref(cfg), *[one] * 9) == 4                              # LinPrim: pinhole only
+    cfg8 = type(cfg)(); C.memmove(C.byref(cfg8), C.byref(cfg), C.sizeof(cfg)); cfg8.tile = 8
+    ras = lambda n, cm, cf, *a: lib.xpr_lin_rasterize_fwd(cm, cf, n, *a, null)
+    # lin_rec vals ranges image final_T n_contrib
+    assert ras(Nm, C.byref(cam), C.byref(cfg), *[one] * 6) == 1
+    assert ras(N4, C.byref(cam), None, *[one] * 6) == 1
+    assert ras(N4, C.byref(cam), C.byref(cfg), odd, *[one] * 5) == 1
+    assert ras(N4, C.byref(cam), C.byref(cfg), one, one, one, null, one, one) == 1            # image NULL
+    assert ras(N4, C.byref(cam), C.byref(cfg8), *[one] * 6) == 4
+    assert ras(N4, C.byref(fish), C.byref(cfg), *[one] * 6) == 4
+    assert lib.xpr_lin_rasterize_stats(C.byref(cam), C.byref(cfg), N4, one, one, one, null, null) == 1
+    # xpr_bin_sort_lin: as xpr_bin_sort, + lin_rec
+    bs = lambda n, rec, cap, *a: lib.xpr_bin_sort_lin(n, one, one, one, rec, C.byref(cam), C.byref(cfg), C.c_int64(cap), *a)
+    assert bs(N4, odd, 1024, one, one, one, None, C.c_void_p(256), C.c_size_t(1 << 20), null) == 1   # lin_rec needs 16 B
+    assert bs(Nm, one, 1024, one, one, one, None, C.c_void_p(256), C.c_size_t(1 << 20), null) == 1
+    assert bs(N4, one, 1024, one, one, one, None, C.c_void_p(256), C.c_size_t(64), null) == 1        # workspace too small
+    assert bs(C.c_int64(1 << 30), one, 1024, one, one, one, None, C.c_void_p(256), C.c_size_t(1 << 20), null) == 4
