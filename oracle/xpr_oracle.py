@@ -568,3 +568,40 @@ def render_lin(scene_arrays: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float3
     binned = lin_bin_sort(proj, cam, cfg)
     fwd = lin_rasterize_fwd(proj, binned, cam, cfg, dtype)
     return dict(proj=proj, binned=binned, fwd=fwd)
+
+
+def lin_rasterize_bwd(proj: dict, binned: dict, fwd: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32,
+                      mass: bool = False) -> np.ndarray:
+    """dL/d(lin_rec) [N,20] (fp64) in the layout of the record; mass=True: sum of |addend| per element."""
+    dt = np.dtype(dtype)
+    N = int(proj["tile_count"].shape[0])
+    rec = np.ascontiguousarray(proj["lin_rec"], dt)
+    dL = np.ascontiguousarray(dL_dimage, dt)
+    g = np.empty((N, 20), np.float64)
+    getattr(lib(), "xpr_oracle_lin_rasterize_bwd_" + _sfx(dt))(
+        C.byref(cam), C.byref(cfg), C.c_int64(N), _p(rec), _p(binned["vals"]), _p(binned["ranges"]),
+        _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), _p(dL), C.c_int32(1 if mass else 0), _p(g))
+    return g
+
+
+def lin_project_bwd(means, scales, quats, opacities, sh, cam: XoCamera, cfg: XoConfig, g_lin_rec, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    N = int(means.shape[0])
+    K = (int(cfg.sh_degree) + 1) ** 2
+    a = [np.ascontiguousarray(x, dt) for x in (means, scales, quats, opacities, sh)]
+    out = dict(g_means=np.empty((N, 3), np.float64), g_scales=np.empty((N, 3), np.float64),
+               g_quats=np.empty((N, 4), np.float64), g_opacities=np.empty(N, np.float64),
+               g_sh=np.empty((N, K, 3), np.float64))
+    getattr(lib(), "xpr_oracle_lin_project_bwd_" + _sfx(dt))(
+        C.c_int64(N), *[_p(x) for x in a], C.byref(cam), C.byref(cfg), _p(np.ascontiguousarray(g_lin_rec, np.float64)),
+        *[_p(out[k]) for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")])
+    return out
+
+
+def backward_lin(scene_arrays: dict, r: dict, dL_dimage, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    """Full LinPrim backward given render_lin() output and dL/dimage; parameter gradients (fp64) + g_lin_rec."""
+    s = scene_arrays
+    g2 = lin_rasterize_bwd(r["proj"], r["binned"], r["fwd"], dL_dimage, cam, cfg, dtype)
+    g3 = lin_project_bwd(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, g2, dtype)
+    g3["g_lin_rec"] = g2
+    return g3
