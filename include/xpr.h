@@ -314,7 +314,7 @@ int32_t xpr_rasterize_featn_bwd(const xpr_camera* cam, const xpr_config* cfg, in
                                 int32_t zero_init, void* stream);
 
 /*
- * ---- XPR-LinPrim (PAPER A.1.3 L506-697, Listings 4-5, Eq. 2): forward path ----
+ * ---- XPR-LinPrim (PAPER A.1.3 L506-697, Listings 4-5, Eq. 2): forward and backward path ----
  * Primitive: the octahedron {x : |S^-1 R^T (x - mu)|_1 <= 1} with homogeneous density
  * sigma = -log(1 - 0.99 o) / (2 min(s)) (L506-524); alpha = 1 - exp(-sigma (tau_exit - tau_enter)) (L528).
  * The body of the paper's `project` listing is lost in the extraction (L545-560); DESIGN.md section 3 readings L1-L6
@@ -326,8 +326,8 @@ int32_t xpr_rasterize_featn_bwd(const xpr_camera* cam, const xpr_config* cfg, in
  *   A^-1 (L538-542): tau in [m_i - h_i, m_i + h_i], m_i = -(kx_i dx + ky_i dy), kx = n_x / n_z, ky = n_y / n_z,
  *   h = 1 / |n_z| (h = +inf when |n_z| < 1e-12: the slab does not bound tau, L566, L4); footprint = the exact
  *   axis-aligned box of the shadow, half extents max_j |A[0][j]|, max_j |A[1][j]| (L3); colour as xpr_project (C5).
- *   in : means[N,3], scales[N,3] (activated, > 0), quats[N,4] (w,x,y,z; normalised inside), opacities[N] in [0,1),
- *        sh[N,K,3]; cam: ONE pinhole camera (fisheye, cfg->views > 1 -> XPR_ERR_UNSUPPORTED).
+ *   in : means[N,3], scales[N,3] (activated, > 0), quats[N,4] (w,x,y,z), opacities[N] in [0,1),
+ *        sh[N,K,3] as xpr_project (quaternions are not renormalised, C3); cam: ONE pinhole camera (fisheye, cfg->views > 1 -> XPR_ERR_UNSUPPORTED).
  *   out: lin_rec[N,20] fp32, 16-byte aligned = (mu2D.x, mu2D.y, sigma, dist | (kx_i, ky_i, h_i) i = 0..3 | r, g, b, 0),
  *        all 0 for a culled primitive; depth[N] = dist; tile_rect[N,4], tile_count[N] as xpr_project.
  *   Culled: p_z <= z_near, non-finite record, empty rectangle.
@@ -348,7 +348,23 @@ int32_t xpr_rasterize_featn_bwd(const xpr_camera* cam, const xpr_config* cfg, in
  *   those that pass the gate, those blended, sum of n_contrib}.
  * Errors (all four): null cam / cfg, N < 0, misaligned pointer -> XPR_ERR_INVALID_ARG; cfg->tile != 16, a fisheye
  *   camera or cfg->views > 1 -> XPR_ERR_UNSUPPORTED; nothing is launched in either case.
- * The backward pass of LinPrim is not part of this library.
+ *
+ * xpr_lin_rasterize_bwd -- reverse mode through the loop above (the paper relies on AD): back to front from
+ *   n_contrib, T_k = T_{k+1} / (1 - alpha_k); dL/dalpha_k as xpr_rasterize_bwd; alpha = min(alpha_max, 1 - exp(-x)): no
+ *   gradient where the clamp is active (C14), else G = dL/dx = exp(-x) dL/dalpha; with en / ex the slab pairs the ray
+ *   enters / leaves through (the first one on ties): dL/dsigma += dtau G, and with gm = sigma G: dL/dh_ex += gm,
+ *   dL/dh_en += gm, dL/dkx_ex -= dx gm, dL/dkx_en += dx gm (ky with dy), dL/dmu2D += gm ((kx, ky)_ex - (kx, ky)_en);
+ *   gates, exit and the choice of en / ex are piecewise constant (C15).
+ *   in : lin_rec, vals_sorted, tile_ranges as the forward; final_T[H,W], n_contrib[H,W] of the forward; dL_dimage[H,W,3].
+ *   out: g_lin_rec[N,20] fp32, 16-byte aligned, in the layout of lin_rec (slots 3 and 19 stay 0): zero-filled by the
+ *        call, then accumulated with fp32 atomics (summation order not fixed: DESIGN.md section 5).
+ * xpr_lin_project_bwd -- reverse mode through xpr_lin_project: slabs -> A^-1 (dL/dA = -A^-T dL/dA^-1 A^-T) -> A = J W R
+ *   diag(s) -> (mu, s, q); sigma(o, min s) (the first shortest half-axis on ties); J(p) and mu2D -> mu; colour as
+ *   xpr_project_bwd (clamped channels carry none, C16).  The forward is recomputed in fp32, the chain rule runs in fp64.
+ *   in : the parameters, tile_count[N] and lin_rec[N,20] of the forward, g_lin_rec[N,20].
+ *   out: g_means[N,3], g_scales[N,3], g_quats[N,4] (16-byte aligned), g_opacities[N], g_sh[N,K,3] (16-byte aligned):
+ *        every element written, zeros for culled primitives.  depth (sort only) and the footprint carry no gradient.
+ * Errors as above.
  */
 int32_t xpr_lin_project(int64_t N, const float* means, const float* scales, const float* quats, const float* opacities,
                         const float* sh, const xpr_camera* cam, const xpr_config* cfg, float* lin_rec, float* depth,
@@ -362,6 +378,13 @@ int32_t xpr_lin_rasterize_fwd(const xpr_camera* cam, const xpr_config* cfg, int6
                               uint32_t* n_contrib, void* stream);
 int32_t xpr_lin_rasterize_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* lin_rec,
                                 const uint32_t* vals_sorted, const uint32_t* tile_ranges, uint64_t* stats, void* stream);
+int32_t xpr_lin_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* lin_rec,
+                              const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* final_T,
+                              const uint32_t* n_contrib, const float* dL_dimage, float* g_lin_rec, void* stream);
+int32_t xpr_lin_project_bwd(int64_t N, const float* means, const float* scales, const float* quats, const float* opacities,
+                            const float* sh, const xpr_camera* cam, const xpr_config* cfg, const uint32_t* tile_count,
+                            const float* lin_rec, const float* g_lin_rec, float* g_means, float* g_scales, float* g_quats,
+                            float* g_opacities, float* g_sh, void* stream);
 
 /*
  * xpr_loss_grad -- convenience for the caller's side of the step (reading C21: the loss lives outside the path):

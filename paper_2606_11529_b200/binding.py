@@ -21,7 +21,8 @@ SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_proje
            "xpr_shade_record", "xpr_bin_sort", "xpr_bin_sort_cull", "xpr_rasterize_fwd", "xpr_rasterize_stats", "xpr_rasterize_bwd", "xpr_project_bwd",
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
            "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad",
-           "xpr_lin_project", "xpr_bin_sort_lin", "xpr_lin_rasterize_fwd", "xpr_lin_rasterize_stats")
+           "xpr_lin_project", "xpr_bin_sort_lin", "xpr_lin_rasterize_fwd", "xpr_lin_rasterize_stats",
+           "xpr_lin_rasterize_bwd", "xpr_lin_project_bwd")
 
 
 class XprCamera(C.Structure):
@@ -332,6 +333,23 @@ def xpr_lin_rasterize_stats(cam: XprCamera, cfg: XprConfig, lin_rec, vals_sorted
     _check(lib().xpr_lin_rasterize_stats(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(lin_rec, _F32),
                                          _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(stats, _I64), _stream(stream)),
            "xpr_lin_rasterize_stats")
+
+
+def xpr_lin_rasterize_bwd(cam: XprCamera, cfg: XprConfig, lin_rec, vals_sorted, tile_ranges, final_T, n_contrib,
+                          dL_dimage, g_lin_rec, stream=None):
+    N = int(lin_rec.shape[0])
+    _check(lib().xpr_lin_rasterize_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(lin_rec, _F32), _p(vals_sorted, _I32),
+                                       _p(tile_ranges, _I32), _p(final_T, _F32), _p(n_contrib, _I32), _p(dL_dimage, _F32),
+                                       _p(g_lin_rec, _F32), _stream(stream)), "xpr_lin_rasterize_bwd")
+
+
+def xpr_lin_project_bwd(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, tile_count, lin_rec,
+                        g_lin_rec, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None):
+    N = int(means.shape[0])
+    _check(lib().xpr_lin_project_bwd(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), _p(opacities, _F32),
+                                     _p(sh, _F32), C.byref(cam), C.byref(cfg), _p(tile_count, _I32), _p(lin_rec, _F32),
+                                     _p(g_lin_rec, _F32), _p(g_means, _F32), _p(g_scales, _F32), _p(g_quats, _F32),
+                                     _p(g_opacities, _F32), _p(g_sh, _F32), _stream(stream)), "xpr_lin_project_bwd")
 
 
 def xpr_loss_grad(kind: str, image, target, dL_dimage, stream=None):

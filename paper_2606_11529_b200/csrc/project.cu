@@ -378,6 +378,104 @@ project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __r
 // primitive; fp32, every operation individually rounded (this file is compiled with -fmad=false), order as the oracle's.
 // lin_rec[N,20] = (mu2D 2, sigma, depth | (kx, ky, h) x 4 | r, g, b, 0).
 // ---------------------------------------------------------------------------------------------
+struct LinGeom {
+    float p[3], dist, R[9], Bm[9], J[9], Ai[9], sigma, smin;
+    int jmin;
+};
+
+// Geometry of one primitive, shared by the forward and the backward kernel (which recomputes it so that every culling
+// decision is the forward's).  Returns visibility; rec[0..15], rc, tc are set when visible.
+__device__ __forceinline__ bool lin_geometry(const ProjParams& P, const float mu[3], const float* __restrict__ scales,
+                                             const float* __restrict__ quats, const float* __restrict__ opac, int64_t i,
+                                             LinGeom& G, float rec[20], int4& rc, uint32_t& tc) {
+    const float* W = P.W;
+    float* p = G.p;
+    for (int a = 0; a < 3; ++a) p[a] = ((W[3 * a] * mu[0] + W[3 * a + 1] * mu[1]) + W[3 * a + 2] * mu[2]) + P.t[a];
+    bool vis = p[2] > P.z_near;
+    rc = make_int4(0, 0, 0, 0);
+    tc = 0;
+    G.dist = 0.0f;
+    if (!vis) return false;
+    const float sc[3] = {__ldg(scales + 3 * i), __ldg(scales + 3 * i + 1), __ldg(scales + 3 * i + 2)};
+    const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
+    const float o = __ldg(opac + i);
+    const float x = p[0], y = p[1], z = p[2];
+    const float dist = sqrtf((x * x + y * y) + z * z);
+    G.dist = dist;
+    const float u = x / z, v = y / z;
+    const float m0 = P.fx * u + P.cx, m1 = P.fy * v + P.cy;
+    float* R = G.R;
+    {
+        const float w = q4.x, qx = q4.y, qy = q4.z, qz = q4.w;
+        const float xx = qx * qx, yy = qy * qy, zz = qz * qz, xy = qx * qy, xz = qx * qz, yz = qy * qz;
+        const float wx = w * qx, wy = w * qy, wz = w * qz;
+        R[0] = 1.0f - 2.0f * (yy + zz); R[1] = 2.0f * (xy - wz); R[2] = 2.0f * (xz + wy);
+        R[3] = 2.0f * (xy + wz); R[4] = 1.0f - 2.0f * (xx + zz); R[5] = 2.0f * (yz - wx);
+        R[6] = 2.0f * (xz - wy); R[7] = 2.0f * (yz + wx); R[8] = 1.0f - 2.0f * (xx + yy);
+    }
+    float* Bm = G.Bm;
+    float A[9];
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+            const float r0 = R[b] * sc[b], r1 = R[3 + b] * sc[b], r2 = R[6 + b] * sc[b];
+            Bm[3 * a + b] = (W[3 * a] * r0 + W[3 * a + 1] * r1) + W[3 * a + 2] * r2;
+        }
+    const float j00 = P.fx / z, j11 = P.fy / z;
+    float* J = G.J;
+    J[0] = j00; J[1] = 0.0f; J[2] = -(j00 * u); J[3] = 0.0f; J[4] = j11; J[5] = -(j11 * v);
+    J[6] = x / dist; J[7] = y / dist; J[8] = z / dist;
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b)
+            A[3 * a + b] = (J[3 * a] * Bm[b] + J[3 * a + 1] * Bm[3 + b]) + J[3 * a + 2] * Bm[6 + b];
+    float cof[9];
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+            const int a1 = (a + 1) % 3, a2 = (a + 2) % 3, b1 = (b + 1) % 3, b2 = (b + 2) % 3;
+            cof[3 * a + b] = A[3 * a1 + b1] * A[3 * a2 + b2] - A[3 * a1 + b2] * A[3 * a2 + b1];
+        }
+    const float det = (A[0] * cof[0] + A[1] * cof[1]) + A[2] * cof[2];
+    vis = (fabsf(det) > 0.0f) && isfinite(det);
+    float* Ai = G.Ai;
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) Ai[3 * a + b] = cof[3 * b + a] / det;
+    const float smin = fminf(sc[0], fminf(sc[1], sc[2]));
+    G.smin = smin;
+    G.jmin = (sc[0] == smin) ? 0 : (sc[1] == smin) ? 1 : 2;
+    const float sigma = (float)(-log(1.0 - 0.99 * (double)o) / (2.0 * (double)smin));     // R2
+    G.sigma = sigma;
+    vis = vis && (sigma > 0.0f) && isfinite(sigma);
+    const float ex = fmaxf(fabsf(A[0]), fmaxf(fabsf(A[1]), fabsf(A[2])));
+    const float ey = fmaxf(fabsf(A[3]), fmaxf(fabsf(A[4]), fabsf(A[5])));
+    vis = vis && (fmaxf(ex, ey) > 0.0f);
+    if (vis) {
+        const float ts = (float)TILE;
+        rc.x = (int)fminf(fmaxf(floorf((m0 - ex) / ts), 0.0f), (float)P.TW);
+        rc.y = (int)fminf(fmaxf(floorf((m1 - ey) / ts), 0.0f), (float)P.TH);
+        rc.z = (int)fminf(fmaxf(ceilf((m0 + ex) / ts), 0.0f), (float)P.TW);
+        rc.w = (int)fminf(fmaxf(ceilf((m1 + ey) / ts), 0.0f), (float)P.TH);
+        const long long t2 = (long long)(rc.z - rc.x) * (long long)(rc.w - rc.y);
+        vis = t2 > 0;
+        tc = (uint32_t)t2;
+    }
+    if (vis) {
+        rec[0] = m0; rec[1] = m1; rec[2] = sigma; rec[3] = dist;
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            const bool p1 = s < 2, p2 = (s & 1) == 0;
+            float n[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) n[k] = (Ai[k] + (p1 ? Ai[3 + k] : -Ai[3 + k])) + (p2 ? Ai[6 + k] : -Ai[6 + k]);
+            float kx = 0.0f, ky = 0.0f, h = INFINITY;                                  // L4
+            if (fabs((double)n[2]) >= 1e-12) { const float inv = 1.0f / n[2]; kx = n[0] * inv; ky = n[1] * inv; h = fabsf(inv); }
+            rec[4 + 3 * s] = kx; rec[5 + 3 * s] = ky; rec[6 + 3 * s] = h;
+        }
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+            if (!isfinite(rec[k]) && !(k >= 4 && (k - 4) % 3 == 2)) vis = false;
+    }
+    return vis;
+}
+
 template <int K>
 __global__ void __launch_bounds__(128)
 lin_project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const float* __restrict__ scales,
@@ -387,86 +485,12 @@ lin_project_kernel(int64_t N, ProjParams P, const float* __restrict__ means, con
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
-    const float* W = P.W;
-    float p[3];
-    for (int a = 0; a < 3; ++a) p[a] = ((W[3 * a] * mu[0] + W[3 * a + 1] * mu[1]) + W[3 * a + 2] * mu[2]) + P.t[a];
-    bool vis = p[2] > P.z_near;
     float rec[20];
-    int4 rc = make_int4(0, 0, 0, 0);
-    uint32_t tc = 0;
-    float dist = 0.0f;
-    if (vis) {
-        const float sc[3] = {__ldg(scales + 3 * i), __ldg(scales + 3 * i + 1), __ldg(scales + 3 * i + 2)};
-        const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
-        const float o = __ldg(opac + i);
-        const float x = p[0], y = p[1], z = p[2];
-        dist = sqrtf((x * x + y * y) + z * z);
-        const float u = x / z, v = y / z;
-        const float m0 = P.fx * u + P.cx, m1 = P.fy * v + P.cy;
-        float R[9];
-        {
-            const float w = q4.x, qx = q4.y, qy = q4.z, qz = q4.w;
-            const float xx = qx * qx, yy = qy * qy, zz = qz * qz, xy = qx * qy, xz = qx * qz, yz = qy * qz;
-            const float wx = w * qx, wy = w * qy, wz = w * qz;
-            R[0] = 1.0f - 2.0f * (yy + zz); R[1] = 2.0f * (xy - wz); R[2] = 2.0f * (xz + wy);
-            R[3] = 2.0f * (xy + wz); R[4] = 1.0f - 2.0f * (xx + zz); R[5] = 2.0f * (yz - wx);
-            R[6] = 2.0f * (xz - wy); R[7] = 2.0f * (yz + wx); R[8] = 1.0f - 2.0f * (xx + yy);
-        }
-        float Bm[9], A[9];
-        for (int a = 0; a < 3; ++a)
-            for (int b = 0; b < 3; ++b) {
-                const float r0 = R[b] * sc[b], r1 = R[3 + b] * sc[b], r2 = R[6 + b] * sc[b];
-                Bm[3 * a + b] = (W[3 * a] * r0 + W[3 * a + 1] * r1) + W[3 * a + 2] * r2;
-            }
-        const float j00 = P.fx / z, j11 = P.fy / z;
-        const float J[9] = {j00, 0.0f, -(j00 * u), 0.0f, j11, -(j11 * v), x / dist, y / dist, z / dist};
-        for (int a = 0; a < 3; ++a)
-            for (int b = 0; b < 3; ++b)
-                A[3 * a + b] = (J[3 * a] * Bm[b] + J[3 * a + 1] * Bm[3 + b]) + J[3 * a + 2] * Bm[6 + b];
-        float cof[9];
-        for (int a = 0; a < 3; ++a)
-            for (int b = 0; b < 3; ++b) {
-                const int a1 = (a + 1) % 3, a2 = (a + 2) % 3, b1 = (b + 1) % 3, b2 = (b + 2) % 3;
-                cof[3 * a + b] = A[3 * a1 + b1] * A[3 * a2 + b2] - A[3 * a1 + b2] * A[3 * a2 + b1];
-            }
-        const float det = (A[0] * cof[0] + A[1] * cof[1]) + A[2] * cof[2];
-        vis = (fabsf(det) > 0.0f) && isfinite(det);
-        float Ai[9];
-        for (int a = 0; a < 3; ++a)
-            for (int b = 0; b < 3; ++b) Ai[3 * a + b] = cof[3 * b + a] / det;
-        const float smin = fminf(sc[0], fminf(sc[1], sc[2]));
-        const float sigma = (float)(-log(1.0 - 0.99 * (double)o) / (2.0 * (double)smin));     // R2
-        vis = vis && (sigma > 0.0f) && isfinite(sigma);
-        const float ex = fmaxf(fabsf(A[0]), fmaxf(fabsf(A[1]), fabsf(A[2])));
-        const float ey = fmaxf(fabsf(A[3]), fmaxf(fabsf(A[4]), fabsf(A[5])));
-        vis = vis && (fmaxf(ex, ey) > 0.0f);
-        if (vis) {
-            const float ts = (float)TILE;
-            rc.x = (int)fminf(fmaxf(floorf((m0 - ex) / ts), 0.0f), (float)P.TW);
-            rc.y = (int)fminf(fmaxf(floorf((m1 - ey) / ts), 0.0f), (float)P.TH);
-            rc.z = (int)fminf(fmaxf(ceilf((m0 + ex) / ts), 0.0f), (float)P.TW);
-            rc.w = (int)fminf(fmaxf(ceilf((m1 + ey) / ts), 0.0f), (float)P.TH);
-            const long long t2 = (long long)(rc.z - rc.x) * (long long)(rc.w - rc.y);
-            vis = t2 > 0;
-            tc = (uint32_t)t2;
-        }
-        if (vis) {
-            rec[0] = m0; rec[1] = m1; rec[2] = sigma; rec[3] = dist;
-#pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                const bool p1 = s < 2, p2 = (s & 1) == 0;
-                float n[3];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) n[k] = (Ai[k] + (p1 ? Ai[3 + k] : -Ai[3 + k])) + (p2 ? Ai[6 + k] : -Ai[6 + k]);
-                float kx = 0.0f, ky = 0.0f, h = INFINITY;                                  // L4
-                if (fabs((double)n[2]) >= 1e-12) { const float inv = 1.0f / n[2]; kx = n[0] * inv; ky = n[1] * inv; h = fabsf(inv); }
-                rec[4 + 3 * s] = kx; rec[5 + 3 * s] = ky; rec[6 + 3 * s] = h;
-            }
-#pragma unroll
-            for (int k = 0; k < 16; ++k)
-                if (!isfinite(rec[k]) && !(k >= 4 && (k - 4) % 3 == 2)) vis = false;
-        }
-    }
+    int4 rc;
+    uint32_t tc;
+    LinGeom G;
+    const bool vis = lin_geometry(P, mu, scales, quats, opac, i, G, rec, rc, tc);
+    const float dist = G.dist;
     if (!vis) {          // culled: an all-zero record (xpr.h)
 #pragma unroll
         for (int k = 0; k < 5; ++k) lin_rec[5 * i + k] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
@@ -828,6 +852,145 @@ project_bwd_kernel(int64_t N, const __grid_constant__ ProjBatch PB, int ipt, con
                            g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh);
 }
 
+// XPR-LinPrim projection backward (f4): dL/d(lin_rec) [N,20] -> parameter gradients.  One thread per primitive; the forward
+// geometry is recomputed in fp32 exactly as lin_project_kernel does (same culling, same slabs), the chain rule runs in
+// fp64:
+//   slabs (kx, ky, h) -> n = c0 + e1 c1 + e2 c2 -> A^-1;  dL/dA = -A^-T (dL/dA^-1) A^-T;  A = J B: dL/dJ = dL/dA B^T,
+//   dL/dB = J^T dL/dA;  B = W R diag(s);  sigma(o, min s);  J(p) and mu2D -> p = W mu + t;  colour as project_bwd.
+// Every primitive's outputs are written (zeros when culled): no zero-fill, no atomics.
+template <int K>
+__global__ void __launch_bounds__(128)
+lin_project_bwd_kernel(int64_t N, ProjParams P, const float* __restrict__ means, const float* __restrict__ scales,
+                       const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
+                       const uint32_t* __restrict__ tcount, const float4* __restrict__ lin_rec,
+                       const float4* __restrict__ g_rec, float* __restrict__ g_means, float* __restrict__ g_scales,
+                       float* __restrict__ g_quats, float* __restrict__ g_opacities, float* __restrict__ g_sh) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    B g_mu[3] = {0, 0, 0}, g_s[3] = {0, 0, 0}, g_q[4] = {0, 0, 0, 0}, g_o = 0;
+    const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
+    float rec[20];
+    int4 rc;
+    uint32_t tc;
+    LinGeom G;
+    const bool vis = (tcount[i] != 0u) && lin_geometry(P, mu, scales, quats, opac, i, G, rec, rc, tc);
+    if (!vis) {
+        float z[3 * K];
+#pragma unroll
+        for (int j = 0; j < 3 * K; ++j) z[j] = 0.0f;
+        store_sh_grad<K>(g_sh, i, z);
+    } else {
+        float gr[20];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const float4 v = __ldg(g_rec + 5 * i + k);
+            gr[4 * k] = v.x; gr[4 * k + 1] = v.y; gr[4 * k + 2] = v.z; gr[4 * k + 3] = v.w;
+        }
+        {   // colour (C5, C16): the forward's clamp decision is the stored colour itself
+            const float4 col = __ldg(lin_rec + 5 * i + 4);
+            float c[3 * K];
+            load_sh<K>(sh, i, c);
+            float dir[3], dnorm, Y[16];
+            view_dir(P, mu, dir, dnorm);
+            sh_basis(dir[0], dir[1], dir[2], Y);
+            B dY[16][3];
+            sh_basis_grad((B)dir[0], (B)dir[1], (B)dir[2], dY);
+            B gd[3] = {0, 0, 0};
+            float gsh[3 * K];
+            const float g0 = (col.x > 0.0f) ? gr[16] : 0.0f, g1 = (col.y > 0.0f) ? gr[17] : 0.0f, g2 = (col.z > 0.0f) ? gr[18] : 0.0f;
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                gsh[3 * k] = Y[k] * g0; gsh[3 * k + 1] = Y[k] * g1; gsh[3 * k + 2] = Y[k] * g2;
+                const B w = (B)fmaf(c[3 * k], g0, fmaf(c[3 * k + 1], g1, c[3 * k + 2] * g2));
+#pragma unroll
+                for (int j = 0; j < 3; ++j) gd[j] += dY[k][j] * w;
+            }
+            store_sh_grad<K>(g_sh, i, gsh);
+            const B dot = (B)dir[0] * gd[0] + (B)dir[1] * gd[1] + (B)dir[2] * gd[2];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) g_mu[j] = (gd[j] - (B)dir[j] * dot) / (B)dnorm;
+        }
+        B Ai[3][3], gAi[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) { Ai[a][b] = (B)G.Ai[3 * a + b]; gAi[a][b] = 0; }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            const B e1 = (s < 2) ? 1.0 : -1.0, e2 = ((s & 1) == 0) ? 1.0 : -1.0;
+            B n[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) n[k] = Ai[0][k] + e1 * Ai[1][k] + e2 * Ai[2][k];
+            if (!(fabs(n[2]) >= 1e-12)) continue;                                 // L4: constants
+            const B inv = 1.0 / n[2], gkx = (B)gr[4 + 3 * s], gky = (B)gr[5 + 3 * s], gh = (B)gr[6 + 3 * s];
+            const B gn[3] = {gkx * inv, gky * inv, -(gkx * n[0] + gky * n[1]) * inv * inv - gh * (n[2] > 0 ? 1.0 : -1.0) * inv * inv};
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { gAi[0][k] += gn[k]; gAi[1][k] += e1 * gn[k]; gAi[2][k] += e2 * gn[k]; }
+        }
+        B tmp[3][3], gA[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) tmp[a][b] = Ai[0][a] * gAi[0][b] + Ai[1][a] * gAi[1][b] + Ai[2][a] * gAi[2][b];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) gA[a][b] = -(tmp[a][0] * Ai[b][0] + tmp[a][1] * Ai[b][1] + tmp[a][2] * Ai[b][2]);
+        B gJ[3][3], gB[3][3], gM[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                gJ[a][b] = gA[a][0] * (B)G.Bm[3 * b] + gA[a][1] * (B)G.Bm[3 * b + 1] + gA[a][2] * (B)G.Bm[3 * b + 2];
+                gB[a][b] = (B)G.J[a] * gA[0][b] + (B)G.J[3 + a] * gA[1][b] + (B)G.J[6 + a] * gA[2][b];
+            }
+        const float* W = P.W;
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) gM[a][b] = (B)W[a] * gB[0][b] + (B)W[3 + a] * gB[1][b] + (B)W[6 + a] * gB[2][b];
+        const float sc[3] = {__ldg(scales + 3 * i), __ldg(scales + 3 * i + 1), __ldg(scales + 3 * i + 2)};
+        B gR[3][3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) { g_s[j] += (B)G.R[3 * a + j] * gM[a][j]; gR[a][j] = (B)sc[j] * gM[a][j]; }
+        {
+            const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
+            const B w = q4.x, x = q4.y, y = q4.z, z = q4.w;
+            g_q[0] = 2.0 * (-z * gR[0][1] + y * gR[0][2] + z * gR[1][0] - x * gR[1][2] - y * gR[2][0] + x * gR[2][1]);
+            g_q[1] = 2.0 * (y * gR[0][1] + z * gR[0][2] + y * gR[1][0] - 2.0 * x * gR[1][1] - w * gR[1][2] + z * gR[2][0] + w * gR[2][1] - 2.0 * x * gR[2][2]);
+            g_q[2] = 2.0 * (-2.0 * y * gR[0][0] + x * gR[0][1] + w * gR[0][2] + x * gR[1][0] + z * gR[1][2] - w * gR[2][0] + z * gR[2][1] - 2.0 * y * gR[2][2]);
+            g_q[3] = 2.0 * (-2.0 * z * gR[0][0] - w * gR[0][1] + x * gR[0][2] + w * gR[1][0] - 2.0 * z * gR[1][1] + y * gR[1][2] + x * gR[2][0] + y * gR[2][1]);
+        }
+        // density sigma = -log(1 - 0.99 o) / (2 min s)
+        const B gsig = (B)gr[2], smin = (B)G.smin, od = (B)__ldg(opac + i);
+        g_o = gsig * 0.99 / ((1.0 - 0.99 * od) * 2.0 * smin);
+        {
+            const B gsm = -gsig * (B)G.sigma / smin;
+            if (G.jmin == 0) g_s[0] += gsm; else if (G.jmin == 1) g_s[1] += gsm; else g_s[2] += gsm;
+        }
+        // J(p) and mu2D
+        const B x = G.p[0], y = G.p[1], z = G.p[2], d = (B)G.dist, fx = P.fx, fy = P.fy;
+        B g_p[3] = {0, 0, 0};
+        g_p[2] += gJ[0][0] * (-fx / (z * z)) + gJ[1][1] * (-fy / (z * z));
+        g_p[0] += gJ[0][2] * (-fx / (z * z)); g_p[2] += gJ[0][2] * (2.0 * fx * x / (z * z * z));
+        g_p[1] += gJ[1][2] * (-fy / (z * z)); g_p[2] += gJ[1][2] * (2.0 * fy * y / (z * z * z));
+        const B r[3] = {x / d, y / d, z / d};
+        const B rg = r[0] * gJ[2][0] + r[1] * gJ[2][1] + r[2] * gJ[2][2];
+#pragma unroll
+        for (int b = 0; b < 3; ++b) g_p[b] += (gJ[2][b] - r[b] * rg) / d;
+        g_p[0] += (B)gr[0] * fx / z; g_p[1] += (B)gr[1] * fy / z;
+        g_p[2] += -(B)gr[0] * fx * x / (z * z) - (B)gr[1] * fy * y / (z * z);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) g_mu[j] += (B)W[j] * g_p[0] + (B)W[3 + j] * g_p[1] + (B)W[6 + j] * g_p[2];
+    }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { g_means[3 * i + j] = (float)g_mu[j]; g_scales[3 * i + j] = (float)g_s[j]; }
+    reinterpret_cast<float4*>(g_quats)[i] = make_float4((float)g_q[0], (float)g_q[1], (float)g_q[2], (float)g_q[3]);
+    g_opacities[i] = (float)g_o;
+}
+
 int32_t make_params(const xpr_camera* cam, const xpr_config* cfg, ProjParams& P) {
     for (int i = 0; i < 3; ++i) {
         for (int j = 0; j < 3; ++j) P.W[3 * i + j] = cam->w2c[4 * i + j];
@@ -978,6 +1141,39 @@ extern "C" int32_t xpr_lin_project(int64_t N, const float* means, const float* s
 #define XPR_GO(KK)                                                                                              \
     lin_project_kernel<KK><<<blocks, 128, 0, st>>>(N, P, means, scales, quats, opacities, sh,                    \
                                                    reinterpret_cast<float4*>(lin_rec), depth, tile_rect, tile_count)
+    switch (cfg->sh_degree) {
+        case 0: XPR_GO(1); break;
+        case 1: XPR_GO(4); break;
+        case 2: XPR_GO(9); break;
+        default: XPR_GO(16); break;
+    }
+#undef XPR_GO
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_lin_project_bwd(int64_t N, const float* means, const float* scales, const float* quats,
+                                       const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
+                                       const uint32_t* tile_count, const float* lin_rec, const float* g_lin_rec,
+                                       float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh,
+                                       void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (cam->model != 0 || num_views(cfg) != 1) return XPR_ERR_UNSUPPORTED;
+    if (N < 0 || N > 0x7fffffffLL) return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(means, 4) || !aligned(scales, 4) || !aligned(quats, 16) || !aligned(opacities, 4) || !aligned(sh, 16) ||
+        !aligned(tile_count, 4) || !aligned(lin_rec, 16) || !aligned(g_lin_rec, 16) || !aligned(g_means, 4) ||
+        !aligned(g_scales, 4) || !aligned(g_quats, 16) || !aligned(g_opacities, 4) || !aligned(g_sh, 16))
+        return XPR_ERR_INVALID_ARG;
+    ProjParams P;
+    if (int32_t s = make_params(cam, cfg, P)) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned blocks = (unsigned)((N + 127) / 128);
+#define XPR_GO(KK)                                                                                                    \
+    lin_project_bwd_kernel<KK><<<blocks, 128, 0, st>>>(N, P, means, scales, quats, opacities, sh, tile_count,          \
+                                                       reinterpret_cast<const float4*>(lin_rec),                       \
+                                                       reinterpret_cast<const float4*>(g_lin_rec), g_means, g_scales,  \
+                                                       g_quats, g_opacities, g_sh)
     switch (cfg->sh_degree) {
         case 0: XPR_GO(1); break;
         case 1: XPR_GO(4); break;

@@ -285,8 +285,9 @@ def scene_to_device(scene, device="cuda:0"):
 
 
 class LinPrimPipeline:
-    """Forward path of XPR-LinPrim (PAPER A.1.3): xpr_lin_project -> xpr_bin_sort_lin ->
-    xpr_lin_rasterize_fwd.  Buffers and call order only, like SplatPipeline; one pinhole view."""
+    """XPR-LinPrim (PAPER A.1.3): xpr_lin_project -> xpr_bin_sort_lin -> xpr_lin_rasterize_fwd ->
+    [loss outside] -> xpr_lin_rasterize_bwd -> xpr_lin_project_bwd.  Buffers and call order only, like SplatPipeline;
+    one pinhole view."""
 
     def __init__(self, N: int, cam, cfg: dict, pair_capacity: int | None = None, device="cuda:0"):
         self.N = int(N)
@@ -303,6 +304,10 @@ class LinPrimPipeline:
         self.tile_ranges = e(self.T, 2, dtype=i32)
         self.image, self.final_T = e(self.H, self.W, 3), e(self.H, self.W)
         self.n_contrib = e(self.H, self.W, dtype=i32)
+        self.K = (int(self.cfg.sh_degree) + 1) ** 2
+        self.g_lin_rec = e(self.N, 20)
+        self.g_means, self.g_scales, self.g_quats = e(self.N, 3), e(self.N, 3), e(self.N, 4)
+        self.g_opacities, self.g_sh = e(self.N), e(self.N, self.K, 3)
         self.num_pairs = 0
         self._alloc_pairs(int(pair_capacity) if pair_capacity else max(1 << 16, 8 * self.N))
 
@@ -310,6 +315,7 @@ class LinPrimPipeline:
     V = 1
 
     def project(self, means, scales, quats, opacities, sh):
+        self._inputs = (means, scales, quats, opacities, sh)
         xb.xpr_lin_project(means, scales, quats, opacities, sh, self.cam, self.cfg, self.lin_rec, self.depth,
                            self.tile_rect, self.tile_count)
 
@@ -334,3 +340,9 @@ class LinPrimPipeline:
         self.bin_sort()
         self.rasterize_fwd()
         return self.image
+
+    def backward(self, dL_dimage):
+        xb.xpr_lin_rasterize_bwd(self.cam, self.cfg, self.lin_rec, self.vals_sorted, self.tile_ranges, self.final_T,
+                                 self.n_contrib, dL_dimage, self.g_lin_rec)
+        xb.xpr_lin_project_bwd(*self._inputs, self.cam, self.cfg, self.tile_count, self.lin_rec, self.g_lin_rec,
+                               self.g_means, self.g_scales, self.g_quats, self.g_opacities, self.g_sh)

@@ -232,3 +232,18 @@ def test_linprim_entry_points_reject_bad_arguments(lib):
     assert bs(Nm, one, 1024, one, one, one, None, C.c_void_p(256), C.c_size_t(1 << 20), null) == 1
     assert bs(N4, one, 1024, one, one, one, None, C.c_void_p(256), C.c_size_t(64), null) == 1        # workspace too small
     assert bs(C.c_int64(1 << 30), one, 1024, one, one, one, None, C.c_void_p(256), C.c_size_t(1 << 20), null) == 4
+    # backward: lin_rec vals ranges final_T n_contrib dL g_lin_rec
+    rb = lambda n, cm, cf, *a: lib.xpr_lin_rasterize_bwd(cm, cf, n, *a, null)
+    assert rb(Nm, C.byref(cam), C.byref(cfg), *[one] * 7) == 1
+    assert rb(N4, C.byref(cam), C.byref(cfg), *[one] * 6, odd) == 1                           # g_lin_rec needs 16 B
+    assert rb(N4, C.byref(cam), C.byref(cfg), *[one] * 5, null, one) == 1                     # dL NULL
+    assert rb(N4, C.byref(fish), C.byref(cfg), *[one] * 7) == 4
+    assert rb(N0, C.byref(cam), C.byref(cfg), null, null, one, one, one, one, null) == 0      # N = 0: nothing to do
+    # means scales quats opacities sh | cam cfg | tile_count lin_rec g_lin_rec g_means g_scales g_quats g_opacities g_sh
+    pb = lambda n, cm, cf, *a: lib.xpr_lin_project_bwd(n, *a[:5], cm, cf, *a[5:], null)
+    assert pb(Nm, C.byref(cam), C.byref(cfg), *[one] * 13) == 1
+    assert pb(N4, C.byref(cam), C.byref(cfg), *[one] * 7, odd, *[one] * 5) == 1               # g_lin_rec needs 16 B
+    assert pb(N4, C.byref(cam), C.byref(cfg), *[one] * 10, odd, one, one) == 1                # g_quats needs 16 B
+    assert pb(N4, C.byref(cam), C.byref(cfg), *[one] * 12, null) == 1                         # g_sh NULL
+    assert pb(N4, C.byref(fish), C.byref(cfg), *[one] * 13) == 4
+    assert pb(N0, C.byref(cam), C.byref(cfg), *[null] * 13) == 0
