@@ -605,3 +605,58 @@ def backward_lin(scene_arrays: dict, r: dict, dL_dimage, cam: XoCamera, cfg: XoC
     g3 = lin_project_bwd(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, g2, dtype)
     g3["g_lin_rec"] = g2
     return g3
+
+
+# ---- rendered depth / accumulated opacity with the ray evaluation (f3 x f2; reading C31) ---------------------------
+
+def rasterize_ray_fwd_da(proj: dict, binned: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    dt = np.dtype(dtype)
+    H, W = int(cam.height), int(cam.width)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("ray_rec", "opac_eff", "rgb", "lnv", "depth", "pixel_rays")]
+    out = dict(depth_img=np.empty((H, W), dt), alpha_img=np.empty((H, W), dt))
+    getattr(lib(), "xpr_oracle_rasterize_ray_fwd_da_" + _sfx(dt))(
+        C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+        _p(out["depth_img"]), _p(out["alpha_img"]))
+    return out
+
+
+def rasterize_ray_bwd_da(proj: dict, binned: dict, fwd: dict, dL_dimage, dL_ddepth, dL_dalpha, cam: XoCamera,
+                         cfg: XoConfig, dtype=np.float32, acc: bool = False, mass: bool = False) -> dict:
+    """rasterize_ray_bwd for a loss that also depends on the depth image and the accumulated opacity; acc=True returns the
+    record gradient in the accumulator form (g_ray_acc [N,16]) instead of g_ray_rec [N,12]."""
+    dt = np.dtype(dtype)
+    N = int(proj["tile_count"].shape[0])
+    a = [np.ascontiguousarray(proj[k], dt) for k in ("ray_rec", "opac_eff", "rgb", "lnv", "depth", "pixel_rays")]
+    g = [np.ascontiguousarray(x, dt) for x in (dL_dimage, dL_ddepth, dL_dalpha)]
+    key = "g_ray_acc" if acc else "g_ray_rec"
+    out = {key: np.empty((N, 16 if acc else 12), np.float64), "g_opac_eff": np.empty(N, np.float64),
+           "g_rgb": np.empty((N, 3), np.float64), "g_depth": np.empty(N, np.float64)}
+    getattr(lib(), "xpr_oracle_rasterize_ray_bwd_da_" + _sfx(dt))(
+        C.byref(cam), C.byref(cfg), C.c_int64(N), *[_p(x) for x in a], _p(binned["vals"]), _p(binned["ranges"]),
+        _p(np.ascontiguousarray(fwd["n_contrib"], np.uint32)), *[_p(x) for x in g],
+        C.c_int32((1 if acc else 0) | (2 if mass else 0)), _p(out[key]), _p(out["g_opac_eff"]), _p(out["g_rgb"]),
+        _p(out["g_depth"]))
+    return out
+
+
+def render_ray_da(scene_arrays: dict, cam: XoCamera, cfg: XoConfig, dtype=np.float32) -> dict:
+    r = render_ray(scene_arrays, cam, cfg, dtype)
+    r["fwd"].update(rasterize_ray_fwd_da(r["proj"], r["binned"], cam, cfg, dtype))
+    return r
+
+
+def backward_ray_da(scene_arrays: dict, r: dict, dL_dimage, dL_ddepth, dL_dalpha, cam: XoCamera, cfg: XoConfig,
+                    dtype=np.float32) -> dict:
+    """Backward of render_ray_da (backward_ray + the depth's own path z = (W mu + t)_z)."""
+    s = scene_arrays
+    g2 = rasterize_ray_bwd_da(r["proj"], r["binned"], r["fwd"], dL_dimage, dL_ddepth, dL_dalpha, cam, cfg, dtype)
+    N = int(s["means"].shape[0])
+    gz = dict(g_mean2d=np.zeros((N, 2)), g_conic=np.zeros((N, 3)), g_opac_eff=g2["g_opac_eff"], g_rgb=g2["g_rgb"])
+    g3 = project_bwd(s["means"], s["scales"], s["quats"], s["opacities"], s["sh"], cam, cfg, gz, dtype)
+    gr = ray_bwd(s["means"], s["scales"], s["quats"], r["proj"]["tile_count"], g2["g_ray_rec"], cam, dtype)
+    for k in ("g_means", "g_scales", "g_quats"):
+        g3[k] = g3[k] + gr[k]
+    g3["g_means"] = g3["g_means"] + depth_bwd(r["proj"]["tile_count"], g2["g_depth"], cam)
+    g3.update(g2)
+    return g3

@@ -209,3 +209,88 @@ def test_p16_finite_differences_five_channels():
                 assert abs(fd - g[gk][idx]) <= 2e-6 * scale + 1e-5 * abs(fd), (key, idx, fd, g[gk][idx])
                 checks += 1
     assert checks > 60
+
+
+# ---- P15r: depth / accumulated opacity with the ray evaluation (f3 x f2) ------------------------------------------------
+
+def test_p15r_ray_depth_and_alpha_are_colour_channels():
+    # with rgb := (z, 1, 2 z), bg = 0 the pinned ray colour pass (P14) renders D and A bit for bit
+    arr, co = _scene(7, opac_boost=1.0)
+    for dtype in (np.float32, np.float64):
+        cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=1, bg=(0.3, 0.6, 0.9)))
+        r = xo.render_ray_da(arr, cam, cfg, dtype)
+        assert (r["fwd"]["n_contrib"] > 3).any()
+        p2 = dict(r["proj"])
+        z = r["proj"]["depth"]
+        p2["rgb"] = np.stack([z, np.ones_like(z), 2 * z], 1).astype(dtype)
+        f2 = xo.rasterize_ray_fwd(p2, r["binned"], cam, xo.make_config(cfg_dict(sh_degree=1, bg=(0.0, 0.0, 0.0))), dtype)
+        assert np.array_equal(f2["n_contrib"], r["fwd"]["n_contrib"])
+        assert np.array_equal(f2["image"][..., 0], r["fwd"]["depth_img"])
+        assert np.array_equal(f2["image"][..., 1], r["fwd"]["alpha_img"])
+    f = r["fwd"]
+    assert np.abs(f["alpha_img"] - (1.0 - f["final_T"])).max() < 1e-13 and f["depth_img"].max() > 1.0
+
+
+def test_p15r_ray_backward_reduces_and_routes_agree():
+    arr, co = _scene(3, opac_boost=1.0)
+    cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=1))
+    r = xo.render_ray_da(arr, cam, cfg, np.float64)
+    rng = np.random.default_rng(0)
+    Gw, Gd, Ga = rng.normal(0, 1, (co.height, co.width, 3)), rng.normal(0, 1, (co.height, co.width)), rng.normal(0, 1, (co.height, co.width))
+    Z = np.zeros((co.height, co.width))
+    a = xo.rasterize_ray_bwd_da(r["proj"], r["binned"], r["fwd"], Gw, Z, Z, cam, cfg, np.float64)
+    b = xo.rasterize_ray_bwd(r["proj"], r["binned"], r["fwd"], Gw, cam, cfg, np.float64)
+    for k in b:                                                     # gD = gA = 0: exactly rasterize_ray_bwd
+        assert np.allclose(a[k], b[k], rtol=1e-13, atol=1e-15), k
+    assert (a["g_depth"] == 0).all()
+    # the accumulator form and the plain record gradient give the same parameter gradients (as P14f), features included
+    g1 = xo.rasterize_ray_bwd_da(r["proj"], r["binned"], r["fwd"], Gw, Gd, Ga, cam, cfg, np.float64)
+    g2 = xo.rasterize_ray_bwd_da(r["proj"], r["binned"], r["fwd"], Gw, Gd, Ga, cam, cfg, np.float64, acc=True)
+    tc = r["proj"]["tile_count"]
+    p1 = xo.ray_bwd(arr["means"], arr["scales"], arr["quats"], tc, g1["g_ray_rec"], cam, np.float64)
+    p2 = xo.ray_bwd_acc(arr["means"], arr["scales"], arr["quats"], tc, g2["g_ray_acc"], cam, np.float64)
+    for k in p1:
+        s = np.abs(p1[k]).max()
+        assert s > 0 and np.abs(p1[k] - p2[k]).max() <= 1e-9 * s, k
+    assert np.allclose(g1["g_depth"], g2["g_depth"], rtol=1e-12, atol=1e-15) and np.abs(g1["g_depth"]).max() > 0
+    m = xo.rasterize_ray_bwd_da(r["proj"], r["binned"], r["fwd"], Gw, Gd, Ga, cam, cfg, np.float64, mass=True)
+    assert (m["g_depth"] >= np.abs(g1["g_depth"]) * (1 - 1e-12)).all()
+
+
+def _loss_ray(arr, cam, cfg, Gw, Gd, Ga):
+    r = xo.render_ray_da(arr, cam, cfg, np.float64)
+    f = r["fwd"]
+    return float((f["image"] * Gw).sum() + (f["depth_img"] * Gd).sum() + (f["alpha_img"] * Ga).sum()), r
+
+
+def test_p15r_ray_finite_differences():
+    found = None
+    for seed in range(60):
+        w2c = scenes.look_at((0.3, -0.2, -1.0), (0.0, 0.1, 3.0)).astype(np.float64)
+        co = cam_obj(w2c=w2c, cx=19.0, cy=13.5, fy=66.0)
+        arr = draw_scene(800 + seed, 6, 4, z=(1.5, 4.5), opac_boost=1.0)
+        cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=1), fragile_rel=1e-4)
+        rng = np.random.default_rng(seed)
+        Gw, Gd, Ga = rng.normal(0, 1, (co.height, co.width, 3)), rng.normal(0, 1, (co.height, co.width)), rng.normal(0, 1, (co.height, co.width))
+        L0, r = _loss_ray(arr, cam, cfg, Gw, Gd, Ga)
+        if (r["fwd"]["fragile"] == 0).all() and (r["proj"]["tile_count"] > 0).sum() >= 5 and (r["fwd"]["n_contrib"] > 2).any():
+            found = (arr, cam, cfg, Gw, Gd, Ga, r)
+            break
+    assert found is not None
+    arr, cam, cfg, Gw, Gd, Ga, r = found
+    g = xo.backward_ray_da(arr, r, Gw, Gd, Ga, cam, cfg, np.float64)
+    scale_all = max(np.abs(g[NAMES[k]]).max() for k in PARAMS)
+    h_rel = 1e-6
+    for k in PARAMS:
+        base, an = arr[k], g[NAMES[k]]
+        fd = np.zeros_like(base)
+        it = np.nditer(base, flags=["multi_index"])
+        for _ in it:
+            idx = it.multi_index
+            h = h_rel * max(1.0, abs(base[idx])) if k != "scales" else h_rel * abs(base[idx]) * 10
+            ap = {kk: v.copy() for kk, v in arr.items()}; ap[k][idx] += h
+            am = {kk: v.copy() for kk, v in arr.items()}; am[k][idx] -= h
+            fd[idx] = (_loss_ray(ap, cam, cfg, Gw, Gd, Ga)[0] - _loss_ray(am, cam, cfg, Gw, Gd, Ga)[0]) / (2 * h)
+        err = np.abs(fd - an)
+        tol = 2e-6 * np.maximum(np.abs(an), np.abs(fd)) + 1e-7 * scale_all + 1e-9
+        assert not (err > tol).any(), (k, np.argwhere(err > tol)[:5], fd[err > tol][:5], an[err > tol][:5])
