@@ -276,8 +276,23 @@ int32_t xpr_ray_bwd(int64_t N, const float* means, const float* scales, const fl
  *   zero_init != 0 (one fill when g_mean2d, g_conic, g_opac, g_rgb, g_depth are adjacent slices, in this order).
  * xpr_depth_bwd -- z = (W mu + t)_z: ADDS W[2,:] g_depth[i] to g_means[i,:] for every Gaussian with
  *   tile_count[i] > 0 (call it after xpr_project_bwd, which overwrites g_means).
+ * xpr_rasterize_ray_feat_fwd / _bwd -- the same two features with the XPR-3DGUT ray evaluation (f2 x f3): C31 blends a
+ *   feature with the weights alpha_k T_k of the colour pass whichever evaluation produced alpha_k (Eq. 1 L439-444 here).
+ *   Arguments of xpr_rasterize_ray_fwd / _bwd plus depth[N] (of xpr_project), depth_img / alpha_img, dL_ddepth /
+ *   dL_dalpha and g_depth[N]; zero_init: one fill when g_ray_acc, g_opac, g_rgb, g_depth are adjacent slices in this order.
  * Errors as the colour calls: null / misaligned pointer, N < 0 -> XPR_ERR_INVALID_ARG before any launch.
  */
+int32_t xpr_rasterize_ray_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                   const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+                                   const float* pixel_rays, const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                                   float* image, float* final_T, uint32_t* n_contrib, float* depth_img, float* alpha_img,
+                                   void* stream);
+int32_t xpr_rasterize_ray_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                   const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+                                   const float* pixel_rays, const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                                   const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
+                                   const float* dL_ddepth, const float* dL_dalpha, float* g_ray_acc, float* g_opac,
+                                   float* g_rgb, float* g_depth, int32_t zero_init, void* stream);
 int32_t xpr_rasterize_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
                                const uint32_t* vals_sorted, const uint32_t* tile_ranges,
                                float* image, float* final_T, uint32_t* n_contrib, float* depth_img,

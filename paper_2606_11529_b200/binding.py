@@ -22,7 +22,7 @@ SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_proje
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
            "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad",
            "xpr_lin_project", "xpr_bin_sort_lin", "xpr_lin_rasterize_fwd", "xpr_lin_rasterize_stats",
-           "xpr_lin_rasterize_bwd", "xpr_lin_project_bwd")
+           "xpr_lin_rasterize_bwd", "xpr_lin_project_bwd", "xpr_rasterize_ray_feat_fwd", "xpr_rasterize_ray_feat_bwd")
 
 
 class XprCamera(C.Structure):
@@ -256,6 +256,28 @@ def xpr_rasterize_ray_bwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, r
                                        _p(lnv, _F32), _p(pixel_rays, _F32), _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32),
                                        _p(n_contrib, _I32), _p(dL_dimage, _F32), _p(g_ray_acc, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
                                        C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_ray_bwd")
+
+
+def xpr_rasterize_ray_feat_fwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, depth, pixel_rays, vals_sorted,
+                               tile_ranges, image, final_T, n_contrib, depth_img, alpha_img, stream=None):
+    N = int(ray_rec.shape[0])
+    _check(lib().xpr_rasterize_ray_feat_fwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec, _F32), _p(conic_opac, _F32),
+                                            _p(rgb, _F32), _p(lnv, _F32), _p(depth, _F32), _p(pixel_rays, _F32),
+                                            _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32),
+                                            _p(n_contrib, _I32), _p(depth_img, _F32), _p(alpha_img, _F32), _stream(stream)),
+           "xpr_rasterize_ray_feat_fwd")
+
+
+def xpr_rasterize_ray_feat_bwd(cam: XprCamera, cfg: XprConfig, ray_rec, conic_opac, rgb, lnv, depth, pixel_rays, vals_sorted,
+                               tile_ranges, final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_ray_acc, g_opac, g_rgb,
+                               g_depth, zero_init: bool = True, stream=None):
+    N = int(ray_rec.shape[0])
+    _check(lib().xpr_rasterize_ray_feat_bwd(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(ray_rec, _F32), _p(conic_opac, _F32),
+                                            _p(rgb, _F32), _p(lnv, _F32), _p(depth, _F32), _p(pixel_rays, _F32),
+                                            _p(vals_sorted, _I32), _p(tile_ranges, _I32), _p(final_T, _F32), _p(n_contrib, _I32),
+                                            _p(dL_dimage, _F32), _p(dL_ddepth, _F32), _p(dL_dalpha, _F32), _p(g_ray_acc, _F32),
+                                            _p(g_opac, _F32), _p(g_rgb, _F32), _p(g_depth, _F32),
+                                            C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_ray_feat_bwd")
 
 
 def xpr_ray_bwd(means, scales, quats, cam: XprCamera, tile_count, g_ray_acc, g_means, g_scales, g_quats, stream=None):

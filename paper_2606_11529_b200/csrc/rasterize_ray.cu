@@ -57,10 +57,11 @@ __device__ __forceinline__ RayEval eval_ray(const float4 r0, const float4 r1, co
 // entry in shared memory: 5 x float4 = (M_c, o_c | thr = -lnv, log2 o, r, g | b).  STATS as in rasterize.cu.
 struct RayPix {
     float d0, d1, d2, T, C0, C1, C2;
+    float D, A;            // FEAT: rendered depth and accumulated opacity (reading C31)
     uint32_t last;
 };
 
-template <bool STATS>
+template <bool STATS, bool FEAT = false>
 __device__ __forceinline__ void ray_blend(RayPix& p, int& act, float nhq, float dd, const float4* __restrict__ rec, uint32_t pos,
                                           float lnr, float amax, float tmin, uint32_t& n_visit, uint32_t& n_pass,
                                           uint32_t& n_blend) {
@@ -78,6 +79,7 @@ __device__ __forceinline__ void ray_blend(RayPix& p, int& act, float nhq, float 
         } else {
             const float w = alpha * p.T;
             p.C0 = fmaf(at.z, w, p.C0); p.C1 = fmaf(at.w, w, p.C1); p.C2 = fmaf(rec[4].x, w, p.C2);
+            if (FEAT) { p.D = fmaf(rec[4].y, w, p.D); p.A += w; }
             p.T = Tn;
             p.last = pos;
             if (STATS) ++n_blend;
@@ -89,13 +91,14 @@ __device__ __forceinline__ void ray_blend(RayPix& p, int& act, float nhq, float 
 #define XPR_RAY_FWD_PPT2_MIN_TILES 4096
 #endif
 
-template <bool STATS, int PPT>
+template <bool STATS, int PPT, bool FEAT = false>
 __global__ void __launch_bounds__(BLOCK / PPT)
 rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, const float4* __restrict__ conic_opac,
                          const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ rays,
                          const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                          float* __restrict__ image, float* __restrict__ final_T, uint32_t* __restrict__ n_contrib,
-                         unsigned long long* __restrict__ stats) {
+                         unsigned long long* __restrict__ stats, const float* __restrict__ depth = nullptr,
+                         float* __restrict__ depth_img = nullptr, float* __restrict__ alpha_img = nullptr) {
     constexpr int THREADS = BLOCK / PPT, BATCH = THREADS, ROW = TILE / PPT;
     __shared__ float4 s_rec[5 * BATCH];
     const int tile = P.order ? (int)P.order[blockIdx.x] : (int)blockIdx.x;
@@ -115,7 +118,7 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             const int64_t pid = (int64_t)py * P.W + px[k];
             pix[k].d0 = rays[3 * pid]; pix[k].d1 = rays[3 * pid + 1]; pix[k].d2 = rays[3 * pid + 2];
         }
-        pix[k].T = 1.0f; pix[k].C0 = pix[k].C1 = pix[k].C2 = 0.0f; pix[k].last = 0; act[k] = inside[k] ? 1 : 0;
+        pix[k].T = 1.0f; pix[k].C0 = pix[k].C1 = pix[k].C2 = 0.0f; pix[k].D = pix[k].A = 0.0f; pix[k].last = 0; act[k] = inside[k] ? 1 : 0;
         any_act |= (inside[k] != 0);
     }
     const uint2 rg = ranges[tile];
@@ -131,7 +134,7 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             float4* rec = s_rec + 5 * threadIdx.x;
             rec[0] = ray_rec[3 * (size_t)g]; rec[1] = ray_rec[3 * (size_t)g + 1]; rec[2] = ray_rec[3 * (size_t)g + 2];
             rec[3] = make_float4(-lnv[g], __log2f(conic_opac[g].w), rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1]);
-            rec[4] = make_float4(rgb[3 * (size_t)g + 2], 0.f, 0.f, 0.f);
+            rec[4] = make_float4(rgb[3 * (size_t)g + 2], FEAT ? depth[g] : 0.f, 0.f, 0.f);
         }
         __syncthreads();
         if (any_act) {
@@ -154,7 +157,7 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                 for (int u = 0; u < 4; ++u)
 #pragma unroll
                     for (int k = 0; k < PPT; ++k)
-                        ray_blend<STATS>(pix[k], act[k], nhq[u][k], dd[u][k], rq + 5 * u, base + j + u + 1, lnr, amax, tmin,
+                        ray_blend<STATS, FEAT>(pix[k], act[k], nhq[u][k], dd[u][k], rq + 5 * u, base + j + u + 1, lnr, amax, tmin,
                                          n_visit, n_pass, n_blend);
                 any_act = (act[0] | act[PPT - 1]) != 0;
             }
@@ -163,7 +166,7 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
 #pragma unroll
                 for (int k = 0; k < PPT; ++k) {
                     const RayEval e = eval_ray(r0, r1, r2, pix[k].d0, pix[k].d1, pix[k].d2);
-                    ray_blend<STATS>(pix[k], act[k], e.nhq, e.dd, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
+                    ray_blend<STATS, FEAT>(pix[k], act[k], e.nhq, e.dd, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
                 }
                 any_act = (act[0] | act[PPT - 1]) != 0;
             }
@@ -186,6 +189,7 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             image[3 * pid + 2] = fmaf(pix[k].T, P.bg[2], pix[k].C2);
             final_T[pid] = pix[k].T;
             n_contrib[pid] = pix[k].last;
+            if (FEAT) { depth_img[pid] = pix[k].D; alpha_img[pid] = pix[k].A; }
         }
 }
 
@@ -244,14 +248,18 @@ __device__ __forceinline__ float warp_reduce4(const float* v, int lane) {
 #ifndef XPR_RAY_BWD_MINB
 #define XPR_RAY_BWD_MINB 6
 #endif
-template <int PPT>
+// FEAT (xpr_rasterize_ray_feat_bwd; reading C31, as rasterize.cu): with gD = dL/dD, gA = dL/dA of the pixel,
+//   dL/dz_k = alpha_k T_k gD;  g . c_k becomes g . c_k + gD z_k;  the accumulated-opacity term is the constant -gA T_final in Q.
+template <int PPT, bool FEAT = false>
 __global__ void __launch_bounds__(BLOCK / PPT, XPR_RAY_BWD_MINB * PPT / 4)
 rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, const float4* __restrict__ conic_opac,
                          const float* __restrict__ rgb, const float* __restrict__ lnv, const float* __restrict__ rays,
                          const uint32_t* __restrict__ vals, const uint2* __restrict__ ranges,
                          const float* __restrict__ final_T, const uint32_t* __restrict__ n_contrib,
                          const float* __restrict__ dL, float* __restrict__ g_acc, float* __restrict__ g_opac,
-                         float* __restrict__ g_rgb) {
+                         float* __restrict__ g_rgb, const float* __restrict__ depth = nullptr,
+                         const float* __restrict__ dL_dD = nullptr, const float* __restrict__ dL_dA = nullptr,
+                         float* __restrict__ g_depth = nullptr) {
     constexpr int THREADS = BLOCK / PPT, BATCH = THREADS;
     __shared__ float4 s_geo[3 * BATCH];
     __shared__ float4 s_gate[BATCH];   // thr, o, log2 o, index (bits)
@@ -267,21 +275,23 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
     const float lnr = P.lnr;
 
     uint32_t n[PPT];
-    float T[PPT], Q[PPT], g0[PPT], g1[PPT], g2[PPT], d0[PPT], d1[PPT], d2[PPT];
+    float T[PPT], Q[PPT], g0[PPT], g1[PPT], g2[PPT], d0[PPT], d1[PPT], d2[PPT], gD[PPT];
     uint32_t wmax = 0;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
         const int px = px0 + k;
-        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = 0.0f; d0[k] = d1[k] = 0.0f; d2[k] = 1.0f;
+        n[k] = 0; T[k] = 0.0f; g0[k] = g1[k] = g2[k] = 0.0f; d0[k] = d1[k] = 0.0f; d2[k] = 1.0f; gD[k] = 0.0f;
+        float gA = 0.0f;
         if (px < P.W && py < P.H) {
             const int64_t pid = (int64_t)py * P.W + px;
             n[k] = n_contrib[pid];
             T[k] = final_T[pid];
             g0[k] = dL[3 * pid]; g1[k] = dL[3 * pid + 1]; g2[k] = dL[3 * pid + 2];
             d0[k] = rays[3 * pid]; d1[k] = rays[3 * pid + 1]; d2[k] = rays[3 * pid + 2];
+            if (FEAT) { gD[k] = dL_dD[pid]; gA = dL_dA[pid]; }
         }
-        // Q_k = g . S_k, the colour behind the entry as one running scalar (rasterize.cu)
-        Q[k] = T[k] * fmaf(g2[k], P.bg[2], fmaf(g1[k], P.bg[1], g0[k] * P.bg[0]));
+        // Q_k = g . S_k, the colour behind the entry as one running scalar (rasterize.cu) (FEAT: - gA T_final)
+        Q[k] = T[k] * (fmaf(g2[k], P.bg[2], fmaf(g1[k], P.bg[1], g0[k] * P.bg[0])) - gA);
         wmax = max(wmax, n[k]);
     }
 #pragma unroll
@@ -307,7 +317,8 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             s_geo[3 * threadIdx.x + 2] = ray_rec[3 * (size_t)g + 2];
             const float o = conic_opac[g].w;
             s_gate[threadIdx.x] = make_float4(-lnv[g], o, __log2f(o), __uint_as_float(g));
-            s_col[threadIdx.x] = make_float4(rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1], rgb[3 * (size_t)g + 2], 0.0f);
+            s_col[threadIdx.x] = make_float4(rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1], rgb[3 * (size_t)g + 2],
+                                             FEAT ? depth[g] : 0.0f);
         }
         __syncthreads();
         for (uint32_t j = 0; j < cnt; ++j) {
@@ -341,7 +352,8 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                 T[k] = T[k] * inv;                     // transmittance in front of this entry
                 const float w = alpha * T[k];
                 vc[0] = fmaf(w, g0[k], vc[0]); vc[1] = fmaf(w, g1[k], vc[1]); vc[2] = fmaf(w, g2[k], vc[2]);
-                const float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
+                float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
+                if (FEAT) { vc[3] = fmaf(w, gD[k], vc[3]); gc = fmaf(gD[k], c.w, gc); }       // dL/dz; g . c + gD z
                 const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
                 Q[k] = fmaf(gc, w, Q[k]);
                 const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
@@ -371,6 +383,7 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
                 else atomicAdd(g_acc + 16 * (size_t)g + 8 + vi, tb);
             }
             if ((lane & 7) == 0 && lane < 24) atomicAdd(g_rgb + 3 * (size_t)g + (lane >> 3), tc);
+            if (FEAT && lane == 24) atomicAdd(g_depth + g, tc);
         }
         hi -= cnt;
     }
@@ -397,33 +410,52 @@ int32_t check_ray_cam_cfg(const xpr_camera* cam, const xpr_config* cfg) {
 
 using namespace xpr;
 
-extern "C" int32_t xpr_rasterize_ray_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
-                                         const float* conic_opac, const float* rgb, const float* lnv,
-                                         const float* pixel_rays, const uint32_t* vals_sorted,
-                                         const uint32_t* tile_ranges, float* image, float* final_T,
-                                         uint32_t* n_contrib, void* stream) {
+static int32_t ray_fwd_impl(bool feat, const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                            const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+                            const float* pixel_rays, const uint32_t* vals_sorted, const uint32_t* tile_ranges, float* image,
+                            float* final_T, uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
     if (int32_t s = check_ray_cam_cfg(cam, cfg)) return s;
     if (N < 0) return XPR_ERR_INVALID_ARG;
     if (!aligned(tile_ranges, 8) || !aligned(image, 4) || !aligned(final_T, 4) || !aligned(n_contrib, 4) ||
         !aligned(pixel_rays, 4))
         return XPR_ERR_INVALID_ARG;
+    if (feat && (!aligned(depth_img, 4) || !aligned(alpha_img, 4))) return XPR_ERR_INVALID_ARG;
     if (N > 0 && (!aligned(ray_rec, 16) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-                  !aligned(vals_sorted, 4)))
+                  !aligned(vals_sorted, 4) || (feat && !aligned(depth, 4))))
         return XPR_ERR_INVALID_ARG;
     RayRasterParams P;
     make_params(cam, cfg, P);
     const int T = tiles_x(cam) * tiles_y(cam);
+#define XPR_RAY_FWD(PPT_, FEAT_)                                                                                      \
+    rasterize_ray_fwd_kernel<false, PPT_, FEAT_><<<T, BLOCK / PPT_, 0, (cudaStream_t)stream>>>(                       \
+        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays, \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr, depth, depth_img, \
+        alpha_img)
     // throughput shape once the image has enough tiles for several waves of every SM
-    if (T >= XPR_RAY_FWD_PPT2_MIN_TILES)
-        rasterize_ray_fwd_kernel<false, 2><<<T, BLOCK / 2, 0, (cudaStream_t)stream>>>(
-            P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-            pixel_rays, vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
-    else
-        rasterize_ray_fwd_kernel<false, 1><<<T, BLOCK, 0, (cudaStream_t)stream>>>(
-            P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv,
-            pixel_rays, vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), image, final_T, n_contrib, nullptr);
+    const bool big = T >= XPR_RAY_FWD_PPT2_MIN_TILES;
+    if (feat) { if (big) XPR_RAY_FWD(2, true); else XPR_RAY_FWD(1, true); }
+    else      { if (big) XPR_RAY_FWD(2, false); else XPR_RAY_FWD(1, false); }
+#undef XPR_RAY_FWD
     XPR_LAUNCH_CHECK();
     return XPR_OK;
+}
+
+extern "C" int32_t xpr_rasterize_ray_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                         const float* conic_opac, const float* rgb, const float* lnv,
+                                         const float* pixel_rays, const uint32_t* vals_sorted,
+                                         const uint32_t* tile_ranges, float* image, float* final_T,
+                                         uint32_t* n_contrib, void* stream) {
+    return ray_fwd_impl(false, cam, cfg, N, ray_rec, conic_opac, rgb, lnv, nullptr, pixel_rays, vals_sorted, tile_ranges,
+                        image, final_T, n_contrib, nullptr, nullptr, stream);
+}
+
+extern "C" int32_t xpr_rasterize_ray_feat_fwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                              const float* conic_opac, const float* rgb, const float* lnv,
+                                              const float* depth, const float* pixel_rays, const uint32_t* vals_sorted,
+                                              const uint32_t* tile_ranges, float* image, float* final_T,
+                                              uint32_t* n_contrib, float* depth_img, float* alpha_img, void* stream) {
+    return ray_fwd_impl(true, cam, cfg, N, ray_rec, conic_opac, rgb, lnv, depth, pixel_rays, vals_sorted, tile_ranges,
+                        image, final_T, n_contrib, depth_img, alpha_img, stream);
 }
 
 extern "C" int32_t xpr_rasterize_ray_stats(const xpr_camera* cam, const xpr_config* cfg, int64_t N,
@@ -447,44 +479,72 @@ extern "C" int32_t xpr_rasterize_ray_stats(const xpr_camera* cam, const xpr_conf
     return XPR_OK;
 }
 
+static int32_t ray_bwd_impl(bool feat, const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                            const float* conic_opac, const float* rgb, const float* lnv, const float* depth,
+                            const float* pixel_rays, const uint32_t* vals_sorted, const uint32_t* tile_ranges,
+                            const float* final_T, const uint32_t* n_contrib, const float* dL_dimage, const float* dL_ddepth,
+                            const float* dL_dalpha, float* g_ray_acc, float* g_opac, float* g_rgb, float* g_depth,
+                            int32_t zero_init, void* stream) {
+    if (int32_t s = check_ray_cam_cfg(cam, cfg)) return s;
+    if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4) ||
+        !aligned(pixel_rays, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (feat && (!aligned(dL_ddepth, 4) || !aligned(dL_dalpha, 4))) return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(ray_rec, 16) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
+        !aligned(vals_sorted, 4) || !aligned(g_ray_acc, 16) || !aligned(g_opac, 4) || !aligned(g_rgb, 4))
+        return XPR_ERR_INVALID_ARG;
+    if (feat && (!aligned(depth, 4) || !aligned(g_depth, 4))) return XPR_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (zero_init) {
+        const size_t n = (size_t)N;
+        if (g_opac == g_ray_acc + 16 * n && g_rgb == g_opac + n) {
+            const bool with_depth = feat && g_depth == g_rgb + 3 * n;
+            XPR_CUDA(cudaMemsetAsync(g_ray_acc, 0, sizeof(float) * (with_depth ? 21 : 20) * n, st));   // one allocation: one fill
+            if (feat && !with_depth) XPR_CUDA(cudaMemsetAsync(g_depth, 0, sizeof(float) * n, st));
+        } else {
+            XPR_CUDA(cudaMemsetAsync(g_ray_acc, 0, sizeof(float) * 16 * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
+            XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
+            if (feat) XPR_CUDA(cudaMemsetAsync(g_depth, 0, sizeof(float) * n, st));
+        }
+    }
+    RayRasterParams P;
+    make_params(cam, cfg, P);
+    const int T = tiles_x(cam) * tiles_y(cam);
+#define XPR_RAY_BWD(PPT_, FEAT_)                                                                                    \
+    rasterize_ray_bwd_kernel<PPT_, FEAT_><<<T, BLOCK / PPT_, 0, st>>>(                                              \
+        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays, \
+        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_ray_acc, g_opac,  \
+        g_rgb, depth, dL_ddepth, dL_dalpha, g_depth)
+    // more pixels per thread amortise the per-entry reduction (throughput shape); fewer give a heavy tile more warps
+    const bool big = T >= XPR_RAY_FWD_PPT2_MIN_TILES;
+    if (feat) { if (big) XPR_RAY_BWD(XPR_RAY_BWD_PPT, true); else XPR_RAY_BWD(2, true); }
+    else      { if (big) XPR_RAY_BWD(XPR_RAY_BWD_PPT, false); else XPR_RAY_BWD(2, false); }
+#undef XPR_RAY_BWD
+    XPR_LAUNCH_CHECK();
+    return XPR_OK;
+}
+
 extern "C" int32_t xpr_rasterize_ray_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
                                          const float* conic_opac, const float* rgb, const float* lnv,
                                          const float* pixel_rays, const uint32_t* vals_sorted,
                                          const uint32_t* tile_ranges, const float* final_T, const uint32_t* n_contrib,
                                          const float* dL_dimage, float* g_ray_acc, float* g_opac, float* g_rgb,
                                          int32_t zero_init, void* stream) {
-    if (int32_t s = check_ray_cam_cfg(cam, cfg)) return s;
-    if (N < 0) return XPR_ERR_INVALID_ARG;
-    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4) ||
-        !aligned(pixel_rays, 4))
-        return XPR_ERR_INVALID_ARG;
-    if (N == 0) return XPR_OK;
-    if (!aligned(ray_rec, 16) || !aligned(conic_opac, 16) || !aligned(rgb, 4) || !aligned(lnv, 4) ||
-        !aligned(vals_sorted, 4) || !aligned(g_ray_acc, 16) || !aligned(g_opac, 4) || !aligned(g_rgb, 4))
-        return XPR_ERR_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)stream;
-    if (zero_init) {
-        const size_t n = (size_t)N;
-        if (g_opac == g_ray_acc + 16 * n && g_rgb == g_opac + n) {
-            XPR_CUDA(cudaMemsetAsync(g_ray_acc, 0, sizeof(float) * 20 * n, st));     // one allocation: one fill
-        } else {
-            XPR_CUDA(cudaMemsetAsync(g_ray_acc, 0, sizeof(float) * 16 * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_opac, 0, sizeof(float) * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_rgb, 0, sizeof(float) * 3 * n, st));
-        }
-    }
-    RayRasterParams P;
-    make_params(cam, cfg, P);
-    const int T = tiles_x(cam) * tiles_y(cam);
-#define XPR_RAY_BWD(PPT_)                                                                                           \
-    rasterize_ray_bwd_kernel<PPT_><<<T, BLOCK / PPT_, 0, st>>>(                                                     \
-        P, reinterpret_cast<const float4*>(ray_rec), reinterpret_cast<const float4*>(conic_opac), rgb, lnv, pixel_rays, \
-        vals_sorted, reinterpret_cast<const uint2*>(tile_ranges), final_T, n_contrib, dL_dimage, g_ray_acc, g_opac,  \
-        g_rgb)
-    // more pixels per thread amortise the per-entry reduction (throughput shape); fewer give a heavy tile more warps
-    if (T >= XPR_RAY_FWD_PPT2_MIN_TILES) XPR_RAY_BWD(XPR_RAY_BWD_PPT);
-    else                                 XPR_RAY_BWD(2);
-#undef XPR_RAY_BWD
-    XPR_LAUNCH_CHECK();
-    return XPR_OK;
+    return ray_bwd_impl(false, cam, cfg, N, ray_rec, conic_opac, rgb, lnv, nullptr, pixel_rays, vals_sorted, tile_ranges,
+                        final_T, n_contrib, dL_dimage, nullptr, nullptr, g_ray_acc, g_opac, g_rgb, nullptr, zero_init, stream);
+}
+
+extern "C" int32_t xpr_rasterize_ray_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* ray_rec,
+                                              const float* conic_opac, const float* rgb, const float* lnv,
+                                              const float* depth, const float* pixel_rays, const uint32_t* vals_sorted,
+                                              const uint32_t* tile_ranges, const float* final_T,
+                                              const uint32_t* n_contrib, const float* dL_dimage, const float* dL_ddepth,
+                                              const float* dL_dalpha, float* g_ray_acc, float* g_opac, float* g_rgb,
+                                              float* g_depth, int32_t zero_init, void* stream) {
+    return ray_bwd_impl(true, cam, cfg, N, ray_rec, conic_opac, rgb, lnv, depth, pixel_rays, vals_sorted, tile_ranges,
+                        final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_ray_acc, g_opac, g_rgb, g_depth, zero_init,
+                        stream);
 }

@@ -33,8 +33,6 @@ class SplatPipeline:
         self.ray_eval = bool(cfg.get("ray_eval", 0)) if isinstance(cfg, dict) else False
         # f3: the compositing pass also renders the depth image and the accumulated opacity (2D evaluation only)
         self.features = bool(cfg.get("features", 0)) if isinstance(cfg, dict) else False
-        if self.features and self.ray_eval:
-            raise ValueError("xpr: rendered features (f3) are built for the 2D evaluation, not for ray_eval")
         if self.V > 1 and (self.features or self.ray_eval):
             raise ValueError("xpr: a batch of views is built for the colour pass of the 2D evaluation")
         self._dL = None
@@ -87,9 +85,9 @@ class SplatPipeline:
         self.g_sh = g4[11 * N:].view(N, self.K, 3)
         if self.ray_eval:   # f2: shader record, per-pixel rays, record gradient
             self.ray_rec = e(N, 12)
-            g3 = e(20 * N)                                 # g_ray_acc | g_opac | g_rgb: one memset in xpr_rasterize_ray_bwd
+            g3 = e(21 * N)                                 # g_ray_acc | g_opac | g_rgb | g_depth: one memset in the ray backward
             self.g_ray_acc = g3[:16 * N].view(N, 16)
-            self.g_opac, self.g_rgb = g3[16 * N:17 * N], g3[17 * N:].view(N, 3)
+            self.g_opac, self.g_rgb, self.g_depth = g3[16 * N:17 * N], g3[17 * N:20 * N].view(N, 3), g3[20 * N:]
             self.pixel_rays = e(self.H, self.W, 3)
             self.pixel_info()
             self.g_mean2d.zero_(); self.g_conic.zero_()    # the footprint carries no gradient
@@ -166,6 +164,11 @@ class SplatPipeline:
         return n
 
     def rasterize_fwd(self):
+        if self.ray_eval and self.features:
+            xb.xpr_rasterize_ray_feat_fwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv, self.depth,
+                                          self.pixel_rays, self.vals_sorted, self.tile_ranges, self.image, self.final_T,
+                                          self.n_contrib, self.depth_img, self.alpha_img)
+            return
         if self.ray_eval:
             xb.xpr_rasterize_ray_fwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv,
                                      self.pixel_rays, self.vals_sorted, self.tile_ranges, self.image, self.final_T,
@@ -182,6 +185,13 @@ class SplatPipeline:
         self._feat_bwd = False
         if self.features and (dL_ddepth is not None or dL_dalpha is not None):
             z = lambda t: torch.zeros(self.H, self.W, dtype=torch.float32, device=self.device) if t is None else t
+            if self.ray_eval:
+                xb.xpr_rasterize_ray_feat_bwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv,
+                                              self.depth, self.pixel_rays, self.vals_sorted, self.tile_ranges, self.final_T,
+                                              self.n_contrib, dL_dimage, z(dL_ddepth), z(dL_dalpha), self.g_ray_acc,
+                                              self.g_opac, self.g_rgb, self.g_depth, zero_init=True)
+                self._feat_bwd = True
+                return
             xb.xpr_rasterize_feat_bwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges,
                                       self.final_T, self.n_contrib, dL_dimage,
                                       z(dL_ddepth), z(dL_dalpha), self.g_mean2d, self.g_conic, self.g_opac,

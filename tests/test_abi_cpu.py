@@ -247,3 +247,22 @@ def test_linprim_entry_points_reject_bad_arguments(lib):
     assert pb(N4, C.byref(cam), C.byref(cfg), *[one] * 12, null) == 1                         # g_sh NULL
     assert pb(N4, C.byref(fish), C.byref(cfg), *[one] * 13) == 4
     assert pb(N0, C.byref(cam), C.byref(cfg), *[null] * 13) == 0
+
+
+def test_ray_feature_entry_points_reject_bad_arguments(lib):
+    """f2 x f3 (xpr_rasterize_ray_feat_fwd / _bwd): the argument checks come before any launch."""
+    cam, cfg = _cam_cfg()
+    null, one, odd = C.c_void_p(0), C.c_void_p(16), C.c_void_p(18)
+    N4, N0, Nm = C.c_int64(4), C.c_int64(0), C.c_int64(-1)
+    # ray_rec conic_opac rgb lnv depth rays vals ranges image final_T n_contrib depth_img alpha_img
+    fwd = lambda n, *a: lib.xpr_rasterize_ray_feat_fwd(C.byref(cam), C.byref(cfg), n, *a, null)
+    assert fwd(Nm, *[one] * 13) == 1
+    assert fwd(N4, *[one] * 4, null, *[one] * 8) == 1                                        # depth NULL
+    assert fwd(N4, *[one] * 11, null, one) == 1                                              # depth_img NULL
+    assert fwd(N4, *[one] * 12, odd) == 1                                                    # alpha_img misaligned
+    # ... final_T n_contrib dL dL_dD dL_dA g_ray_acc g_opac g_rgb g_depth
+    bwd = lambda n, *a: lib.xpr_rasterize_ray_feat_bwd(C.byref(cam), C.byref(cfg), n, *a, C.c_int32(1), null)
+    assert bwd(Nm, *[one] * 17) == 1
+    assert bwd(N4, *[one] * 11, null, *[one] * 5) == 1                                       # dL_ddepth NULL
+    assert bwd(N4, *[one] * 16, null) == 1                                                   # g_depth NULL
+    assert bwd(N0, *[null] * 5, one, null, one, one, one, one, one, one, *[null] * 4) == 0   # N = 0: nothing to do

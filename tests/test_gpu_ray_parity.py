@@ -180,6 +180,73 @@ def test_ray_pixel_rays_depend_on_the_intrinsics_only():
     np.testing.assert_allclose(np.linalg.norm(a.astype(np.float64), axis=-1), 1.0, atol=2e-7)
 
 
+def ray_feat_parity(scene, view=0, cfg_over=None):
+    """f2 x f3: depth image and accumulated opacity rendered by the ray evaluation (xpr_rasterize_ray_feat_fwd / _bwd).
+    Bars as tests/test_gpu_feat_parity.py: A within 1e-4, D within 1e-4 max(1, z_max), compositing gradients (accumulators,
+    opacity, colour, g_depth) every element within 1e-3 |ref| + 1e-6 + 2e-6 mass, parameters stage-isolated."""
+    import torch
+    over = dict(cfg_over or {}, ray_eval=1)
+    g = pu.run_gpu(scene, view, dict(over, features=1))
+    pipe = g["pipe"]
+    o = pu.run_oracle_ray(scene, view, over, pixel_rays=g["proj"]["pixel_rays"])
+    pu.compare_binning(g, o)
+    pu.compare_forward(g, o)
+    of = xo.rasterize_ray_fwd_da(o["proj"], o["binned"], o["cam"], o["cfg"], np.float32)
+    ok = (o["fwd"]["fragile"] & pu.FRAG_EXIT) == 0
+    A_gpu, D_gpu = pipe.alpha_img.cpu().numpy(), pipe.depth_img.cpu().numpy()
+    vis = o["proj"]["tile_count"] > 0
+    zmax = max(1.0, float(o["proj"]["depth"][vis].max(initial=1.0)))
+    assert np.abs(A_gpu.astype(np.float64) - of["alpha_img"])[ok].max(initial=0.0) <= pu.IMG_TOL
+    assert np.abs(D_gpu.astype(np.float64) - of["depth_img"])[ok].max(initial=0.0) <= pu.IMG_TOL * zmax
+    assert np.abs(A_gpu + g["fwd"]["final_T"] - 1.0).max() <= 1e-4 and D_gpu.max() > 0
+    H, W = ok.shape
+    _, dL = scenes.loss_and_grad(scene.loss, o["fwd"]["image"], scene.target(view))
+    rng = np.random.default_rng(4100 + view)
+    gD, gA = rng.uniform(-1, 1, (H, W)).astype(np.float32), rng.uniform(-1, 1, (H, W)).astype(np.float32)
+    frag = (o["fwd"]["fragile"] & (pu.FRAG_EXIT | pu.FRAG_CLAMP)) != 0
+    dL = np.where(frag[..., None], 0.0, dL).astype(np.float32)
+    gD = np.where(frag, 0.0, gD).astype(np.float32); gA = np.where(frag, 0.0, gA).astype(np.float32)
+    args = (o["proj"], o["binned"], o["fwd"], dL, gD, gA, o["cam"], o["cfg"], np.float32)
+    oa = xo.rasterize_ray_bwd_da(*args, acc=True)
+    mass = xo.rasterize_ray_bwd_da(*args, acc=True, mass=True)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(pipe.device)
+    pipe.backward(t(dL), t(gD), t(gA))
+    torch.cuda.synchronize()
+    gg = {k: getattr(pipe, k).cpu().numpy() for k in ("g_ray_acc", "g_opac", "g_rgb", "g_depth") + PARAMS}
+    for kg, ko in (("g_ray_acc", "g_ray_acc"), ("g_opac", "g_opac_eff"), ("g_rgb", "g_rgb"), ("g_depth", "g_depth")):
+        bad, err = pu.grad_violations(gg[kg], oa[ko], mass[ko])
+        assert bad.sum() == 0, f"{kg}: {bad.sum()} of {bad.size} outside tolerance, max err {err.max()}"
+    assert np.abs(oa["g_depth"]).max() > 0
+    N = scene.N
+    gz = dict(g_mean2d=np.zeros((N, 2)), g_conic=np.zeros((N, 3)), g_opac_eff=gg["g_opac"], g_rgb=gg["g_rgb"])
+    iso = xo.project_bwd(scene.means, scene.scales, scene.quats, scene.opacities, scene.sh, o["cam"], o["cfg"], gz, np.float32)
+    part = xo.ray_bwd_acc(scene.means, scene.scales, scene.quats, o["proj"]["tile_count"], gg["g_ray_acc"], o["cam"], np.float32)
+    dpart = xo.depth_bwd(o["proj"]["tile_count"], gg["g_depth"], o["cam"])
+    og = xo.backward_ray_da(o["arrays"], o, dL, gD, gA, o["cam"], o["cfg"], np.float32)
+    total_bad = total = 0
+    for k in PARAMS:
+        parts = [iso[k]] + ([part[k]] if k in part else []) + ([dpart] if k == "g_means" else [])
+        ref = sum(parts)
+        got, ref = np.asarray(gg[k], np.float64).ravel(), np.asarray(ref, np.float64).ravel()
+        tol = pu.GRAD_RTOL * np.abs(ref) + pu.GRAD_ATOL + 2.4e-7 * sum(np.abs(x).ravel() for x in parts) * (len(parts) > 1)
+        bad = np.abs(got - ref) > tol
+        assert bad.sum() == 0, f"{k} (stage-isolated): {bad.sum()} of {bad.size}, max err {np.abs(got - ref).max()}"
+        b2, _ = pu.grad_violations(gg[k], og[k])
+        total_bad += int(b2.sum()); total += b2.size
+    assert total_bad <= 1e-3 * total, f"end-to-end violators {total_bad}/{total}"
+    return total_bad, total
+
+
+def test_ray_feat_config4_reduced_and_tiny():
+    print("RAY_FEAT e2e", ray_feat_parity(scenes.make_scene(4, n_override=30000, image_override=(480, 270)), 0))
+    ray_feat_parity(scenes.make_scene(1), 0)
+    ray_feat_parity(scenes.make_scene(3, n_override=20000, image_override=(250, 130)), 1, dict(bg=(0.2, 0.4, 0.1), tile_cull=1))
+
+
+def test_ray_feat_config4_full_size():
+    print("RAY_FEAT full e2e", ray_feat_parity(scenes.make_scene(4), 0))
+
+
 def test_zz_report_end_to_end_violators(capsys):
     with capsys.disabled():
         for name, n, bad, tot in E2E_STATS:
