@@ -53,7 +53,7 @@ def parse():
                          "only); -1: the pipeline's default (on for 64 <= tiles < 4096)")
     ap.add_argument("--features", type=int, default=0, choices=(0, 1),
                     help="1: also render the depth image and the accumulated opacity and take their gradients "
-                         "(SURVEY 8(f) f3, DESIGN.md 6.8; 2D evaluation only; not part of the headline workload)")
+                         "(SURVEY 8(f) f3, DESIGN.md 6.8; with --ray-eval 1 through the ray kernels; not part of the headline workload)")
     ap.add_argument("--featn", type=int, default=0,
                     help="C > 0: after the timed steps, also time xpr_rasterize_featn_fwd / _bwd with C seeded feature "
                          "channels on the lists of the last step (reported as 'featn'; not part of the step)")
@@ -149,9 +149,10 @@ def _oracle_view(xo, scenes, sc, view, np, tile_cull, ray_eval, features):
     r = render(arrays, cam, cfg, np.float32)
     _, dL = scenes.loss_and_grad(sc.loss, r["fwd"]["image"], sc.target(view))
     if features:     # f3: the depth / accumulated-opacity pass and the backward with their (here constant) gradients
-        r["fwd"].update(xo.rasterize_fwd_da(r["proj"], r["binned"], cam, cfg, np.float32))
+        fwd_da, bwd_da = (xo.rasterize_ray_fwd_da, xo.backward_ray_da) if ray_eval else (xo.rasterize_fwd_da, xo.backward_da)
+        r["fwd"].update(fwd_da(r["proj"], r["binned"], cam, cfg, np.float32))
         one = np.ones(r["fwd"]["image"].shape[:2], np.float32)
-        xo.backward_da(arrays, r, dL, one, one, cam, cfg, np.float32)
+        bwd_da(arrays, r, dL, one, one, cam, cfg, np.float32)
     else:
         backward(arrays, r, dL, cam, cfg, np.float32)
     return time.perf_counter() - t0, r["binned"]["num_pairs"]
@@ -234,8 +235,6 @@ def run_ours(args):
     V = max(1, args.views)
     if V > 1 and (args.features or args.ray_eval or args.view + V > len(sc.cameras)):
         raise SystemExit("bench.py: --views V needs V cameras in the scene (config 5 has four) and the 2D colour pass")
-    if args.features and args.ray_eval:
-        raise SystemExit("bench.py: --features 1 is built for the 2D evaluation (not with --ray-eval 1)")
     cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval,
                tile_order=args.tile_order, features=args.features)
     params = pipeline.scene_to_device(sc, dev)

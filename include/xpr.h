@@ -211,6 +211,11 @@ int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t 
  * xpr_project_bwd -- reverse mode through projection (EWA or UT) and SH (DESIGN.md section 3,
  * readings C16-C19).  One thread per Gaussian; a culled Gaussian (tile_count == 0) gets zeros.
  *   out (fully overwritten): g_means[N,3] g_scales[N,3] g_quats[N,4] g_opacities[N] g_sh[N,K,3].
+ *   The call is a zero-fill of the five outputs (one cudaMemsetAsync when they are adjacent slices of one allocation,
+ *   in this order) followed by a kernel over the visible Gaussians only.  The fill (59 floats per Gaussian at degree 3)
+ *   is pure HBM traffic with no input: xpr_project_bwd_fill issues it alone -- e.g. on a second stream, under the
+ *   ALU-bound xpr_rasterize_bwd -- and xpr_project_bwd_filled is xpr_project_bwd without it (the caller orders the two:
+ *   the fill must have completed, and nothing may have written the arrays since).
  */
 int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, const float* quats,
                         const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
@@ -218,6 +223,14 @@ int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, cons
                         const float* g_mean2d, const float* g_conic, const float* g_opac, const float* g_rgb,
                         float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh,
                         void* stream);
+int32_t xpr_project_bwd_fill(int64_t N, const xpr_config* cfg, float* g_means, float* g_scales, float* g_quats,
+                             float* g_opacities, float* g_sh, void* stream);
+int32_t xpr_project_bwd_filled(int64_t N, const float* means, const float* scales, const float* quats,
+                               const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
+                               const uint32_t* tile_count, const uint8_t* flags,
+                               const float* g_mean2d, const float* g_conic, const float* g_opac, const float* g_rgb,
+                               float* g_means, float* g_scales, float* g_quats, float* g_opacities, float* g_sh,
+                               void* stream);
 
 /*
  * ---- XPR-3DGUT evaluation (PAPER A.1.2 L437-444 Eq. 1, Listing 3) -----------------

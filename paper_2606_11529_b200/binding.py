@@ -22,7 +22,8 @@ SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_proje
            "xpr_pixel_info", "xpr_project_ray", "xpr_rasterize_ray_fwd", "xpr_rasterize_ray_stats", "xpr_rasterize_ray_bwd",
            "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad",
            "xpr_lin_project", "xpr_bin_sort_lin", "xpr_lin_rasterize_fwd", "xpr_lin_rasterize_stats",
-           "xpr_lin_rasterize_bwd", "xpr_lin_project_bwd", "xpr_rasterize_ray_feat_fwd", "xpr_rasterize_ray_feat_bwd")
+           "xpr_lin_rasterize_bwd", "xpr_lin_project_bwd", "xpr_rasterize_ray_feat_fwd", "xpr_rasterize_ray_feat_bwd",
+           "xpr_project_bwd_fill", "xpr_project_bwd_filled")
 
 
 class XprCamera(C.Structure):
@@ -211,10 +212,18 @@ def xpr_rasterize_bwd(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, ti
                                    C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_bwd")
 
 
+def xpr_project_bwd_fill(cfg: XprConfig, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None):
+    N = int(g_means.shape[0])
+    _check(lib().xpr_project_bwd_fill(C.c_int64(N), C.byref(cfg), _p(g_means, _F32), _p(g_scales, _F32), _p(g_quats, _F32),
+                                      _p(g_opacities, _F32), _p(g_sh, _F32), _stream(stream)), "xpr_project_bwd_fill")
+
+
 def xpr_project_bwd(means, scales, quats, opacities, sh, cam: XprCamera, cfg: XprConfig, tile_count, flags, g_mean2d,
-                    g_conic, g_opac, g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None):
+                    g_conic, g_opac, g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None, filled: bool = False):
+    """filled=True: xpr_project_bwd_filled (the outputs were zero-filled by xpr_project_bwd_fill, ordered by the caller)."""
     N = int(means.shape[0])
-    _check(lib().xpr_project_bwd(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), _p(opacities, _F32), _p(sh, _F32), C.byref(cam),
+    fn = lib().xpr_project_bwd_filled if filled else lib().xpr_project_bwd
+    _check(fn(C.c_int64(N), _p(means, _F32), _p(scales, _F32), _p(quats, _F32), _p(opacities, _F32), _p(sh, _F32), C.byref(cam),
                                  C.byref(cfg), _p(tile_count, _I32), _p(flags, _U8), _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32),
                                  _p(g_rgb, _F32), _p(g_means, _F32), _p(g_scales, _F32), _p(g_quats, _F32), _p(g_opacities, _F32), _p(g_sh, _F32),
                                  _stream(stream)), "xpr_project_bwd")

@@ -1069,12 +1069,38 @@ extern "C" int32_t xpr_project(int64_t N, const float* means, const float* scale
     return XPR_OK;
 }
 
-extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, const float* quats,
-                                   const float* opacities, const float* sh, const xpr_camera* cam,
-                                   const xpr_config* cfg, const uint32_t* tile_count, const uint8_t* flags,
-                                   const float* g_mean2d, const float* g_conic, const float* g_opac,
-                                   const float* g_rgb, float* g_means, float* g_scales, float* g_quats,
-                                   float* g_opacities, float* g_sh, void* stream) {
+// zero-fill of the five parameter-gradient arrays: one memset when they are adjacent slices of one allocation, in this order
+static int32_t fill_param_grads(int64_t N, const xpr_config* cfg, float* g_means, float* g_scales, float* g_quats,
+                                float* g_opacities, float* g_sh, cudaStream_t st) {
+    const size_t n = (size_t)N, K3 = 3 * (size_t)((cfg->sh_degree + 1) * (cfg->sh_degree + 1));
+    if (g_scales == g_means + 3 * n && g_quats == g_scales + 3 * n && g_opacities == g_quats + 4 * n &&
+        g_sh == g_opacities + n) {
+        XPR_CUDA(cudaMemsetAsync(g_means, 0, sizeof(float) * (11 + K3) * n, st));
+    } else {
+        XPR_CUDA(cudaMemsetAsync(g_means, 0, sizeof(float) * 3 * n, st));
+        XPR_CUDA(cudaMemsetAsync(g_scales, 0, sizeof(float) * 3 * n, st));
+        XPR_CUDA(cudaMemsetAsync(g_quats, 0, sizeof(float) * 4 * n, st));
+        XPR_CUDA(cudaMemsetAsync(g_opacities, 0, sizeof(float) * n, st));
+        XPR_CUDA(cudaMemsetAsync(g_sh, 0, sizeof(float) * K3 * n, st));
+    }
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_project_bwd_fill(int64_t N, const xpr_config* cfg, float* g_means, float* g_scales, float* g_quats,
+                                        float* g_opacities, float* g_sh, void* stream) {
+    if (!cfg || cfg->sh_degree < 0 || cfg->sh_degree > 3 || N < 0 || N > 0x7fffffffLL) return XPR_ERR_INVALID_ARG;
+    if (N == 0) return XPR_OK;
+    if (!aligned(g_means, 4) || !aligned(g_scales, 4) || !aligned(g_quats, 16) || !aligned(g_opacities, 4) || !aligned(g_sh, 16))
+        return XPR_ERR_INVALID_ARG;
+    return fill_param_grads(N, cfg, g_means, g_scales, g_quats, g_opacities, g_sh, (cudaStream_t)stream);
+}
+
+static int32_t project_bwd_impl(bool fill, int64_t N, const float* means, const float* scales, const float* quats,
+                                const float* opacities, const float* sh, const xpr_camera* cam,
+                                const xpr_config* cfg, const uint32_t* tile_count, const uint8_t* flags,
+                                const float* g_mean2d, const float* g_conic, const float* g_opac,
+                                const float* g_rgb, float* g_means, float* g_scales, float* g_quats,
+                                float* g_opacities, float* g_sh, void* stream) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0 || N > 0x7fffffffLL) return XPR_ERR_INVALID_ARG;
     if (N == 0) return XPR_OK;
@@ -1096,19 +1122,8 @@ extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* s
     ipt = ipt < 1 ? 1 : (ipt > PBWD_MAX_IPT ? PBWD_MAX_IPT : ipt);
     const int64_t chunk = (int64_t)PBWD_THREADS * ipt;
     const dim3 blocks((unsigned)((N + chunk - 1) / chunk), (unsigned)V);
-    {   // zero-fill: one memset when the five outputs are adjacent slices of one allocation, in this order
-        const size_t n = (size_t)N, K3 = 3 * (size_t)((cfg->sh_degree + 1) * (cfg->sh_degree + 1));
-        if (g_scales == g_means + 3 * n && g_quats == g_scales + 3 * n && g_opacities == g_quats + 4 * n &&
-            g_sh == g_opacities + n) {
-            XPR_CUDA(cudaMemsetAsync(g_means, 0, sizeof(float) * (11 + K3) * n, st));
-        } else {
-            XPR_CUDA(cudaMemsetAsync(g_means, 0, sizeof(float) * 3 * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_scales, 0, sizeof(float) * 3 * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_quats, 0, sizeof(float) * 4 * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_opacities, 0, sizeof(float) * n, st));
-            XPR_CUDA(cudaMemsetAsync(g_sh, 0, sizeof(float) * K3 * n, st));
-        }
-    }
+    if (fill)
+        if (int32_t s = fill_param_grads(N, cfg, g_means, g_scales, g_quats, g_opacities, g_sh, st)) return s;
 #define XPR_GO(KK)                                                                                                  \
     project_bwd_kernel<KK><<<blocks, PBWD_THREADS, 0, st>>>(N, P, ipt, means, scales, quats, opacities, sh, tile_count, \
                                                             flags, g_mean2d, g_conic, g_opac, g_rgb, g_means, g_scales, \
@@ -1122,6 +1137,26 @@ extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* s
 #undef XPR_GO
     XPR_LAUNCH_CHECK();
     return XPR_OK;
+}
+
+extern "C" int32_t xpr_project_bwd(int64_t N, const float* means, const float* scales, const float* quats,
+                                   const float* opacities, const float* sh, const xpr_camera* cam,
+                                   const xpr_config* cfg, const uint32_t* tile_count, const uint8_t* flags,
+                                   const float* g_mean2d, const float* g_conic, const float* g_opac,
+                                   const float* g_rgb, float* g_means, float* g_scales, float* g_quats,
+                                   float* g_opacities, float* g_sh, void* stream) {
+    return project_bwd_impl(true, N, means, scales, quats, opacities, sh, cam, cfg, tile_count, flags, g_mean2d, g_conic,
+                            g_opac, g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh, stream);
+}
+
+extern "C" int32_t xpr_project_bwd_filled(int64_t N, const float* means, const float* scales, const float* quats,
+                                          const float* opacities, const float* sh, const xpr_camera* cam,
+                                          const xpr_config* cfg, const uint32_t* tile_count, const uint8_t* flags,
+                                          const float* g_mean2d, const float* g_conic, const float* g_opac,
+                                          const float* g_rgb, float* g_means, float* g_scales, float* g_quats,
+                                          float* g_opacities, float* g_sh, void* stream) {
+    return project_bwd_impl(false, N, means, scales, quats, opacities, sh, cam, cfg, tile_count, flags, g_mean2d, g_conic,
+                            g_opac, g_rgb, g_means, g_scales, g_quats, g_opacities, g_sh, stream);
 }
 
 extern "C" int32_t xpr_lin_project(int64_t N, const float* means, const float* scales, const float* quats,

@@ -36,6 +36,11 @@ class SplatPipeline:
         if self.V > 1 and (self.features or self.ray_eval):
             raise ValueError("xpr: a batch of views is built for the colour pass of the 2D evaluation")
         self._dL = None
+        # overlap_fill = 1: the zero-fill of the parameter gradients (xpr_project_bwd_fill: HBM traffic without inputs) runs on
+        # a second stream under the compositing backward.  Off by default: measured on config 3 / 5 the compositing kernel
+        # slows down by what the fill saves (0.326 -> 0.351 ms, project_bwd 0.083 -> 0.045 ms: step -1 %), DESIGN.md 6.5
+        self.overlap_fill = bool(cfg.get("overlap_fill", 0)) if isinstance(cfg, dict) else False
+        self._filled = False
         # f3: constant (dL/dD, dL/dA) of a loss that is linear in the features; step_async() feeds them to the backward
         self.feature_grads = None
         self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
@@ -181,8 +186,22 @@ class SplatPipeline:
         xb.xpr_rasterize_fwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.image,
                              self.final_T, self.n_contrib)
 
+    def _fork_fill(self):
+        if not self.overlap_fill:
+            return
+        if not hasattr(self, "_side"):
+            self._side = torch.cuda.Stream(device=self.device)
+            self._ev_fork, self._ev_join = torch.cuda.Event(), torch.cuda.Event()
+        self._ev_fork.record(torch.cuda.current_stream())      # after every earlier reader / writer of the gradient arrays
+        self._side.wait_event(self._ev_fork)
+        xb.xpr_project_bwd_fill(self.cfg, self.g_means, self.g_scales, self.g_quats, self.g_opacities, self.g_sh,
+                                stream=self._side)
+        self._ev_join.record(self._side)
+        self._filled = True
+
     def rasterize_bwd(self, dL_dimage, dL_ddepth=None, dL_dalpha=None):
         self._feat_bwd = False
+        self._fork_fill()
         if self.features and (dL_ddepth is not None or dL_dalpha is not None):
             z = lambda t: torch.zeros(self.H, self.W, dtype=torch.float32, device=self.device) if t is None else t
             if self.ray_eval:
@@ -233,9 +252,12 @@ class SplatPipeline:
 
     def project_bwd(self):
         means, scales, quats, opacities, sh = self._inputs
+        filled, self._filled = self._filled, False
+        if filled:
+            torch.cuda.current_stream().wait_event(self._ev_join)
         xb.xpr_project_bwd(means, scales, quats, opacities, sh, self.cam, self.cfg, self.tile_count, self.flags,
                            self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb, self.g_means, self.g_scales,
-                           self.g_quats, self.g_opacities, self.g_sh)
+                           self.g_quats, self.g_opacities, self.g_sh, filled=filled)
         if self.ray_eval:
             xb.xpr_ray_bwd(means, scales, quats, self.cam, self.tile_count, self.g_ray_acc, self.g_means,
                            self.g_scales, self.g_quats)

@@ -295,3 +295,40 @@ def test_tile_cull_needle_gaussians_bit_exact(seed):
     g0 = pu.run_gpu(sc, 0, dict(tile_cull=0))
     ok = (o["fwd"]["fragile"] & pu.FRAG_EXIT) == 0
     assert np.array_equal(g0["fwd"]["image"][ok], g["fwd"]["image"][ok])          # culling changes no pixel
+
+
+@pytest.mark.gpu
+def test_overlapped_zero_fill_gives_the_same_gradients():
+    """xpr_project_bwd_fill on a second stream + xpr_project_bwd_filled (pipeline option overlap_fill) against the plain
+    xpr_project_bwd: same parameter gradients bit for bit (no atomics at one view), also when captured in a CUDA graph."""
+    import numpy as np
+    import torch
+    from paper_2606_11529_b200 import pipeline, scenes
+    sc = scenes.make_scene(2, n_override=20000, image_override=(320, 240))
+    cfg = scenes.default_render_config(sc)
+    params = pipeline.scene_to_device(sc)
+    target = torch.from_numpy(sc.target(0)).cuda()
+    names = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], dict(cfg, overlap_fill=1))
+    pipe.forward(*params)
+    for k in names:
+        getattr(pipe, k).fill_(float("nan"))                # the fill must really happen
+    pipe.step_async(*params, target, sc.loss)               # fill on the side stream, xpr_project_bwd_filled
+    torch.cuda.synchronize()
+    a = {k: getattr(pipe, k).cpu().numpy().copy() for k in names}
+    for k in names:
+        getattr(pipe, k).fill_(float("nan"))
+    pipe.project_bwd()                                      # no fork before it: the plain xpr_project_bwd on the same 2D gradients
+    torch.cuda.synchronize()
+    for k in names:
+        b = getattr(pipe, k).cpu().numpy()
+        assert np.isfinite(b).all() and np.array_equal(a[k], b), k
+    assert np.abs(a["g_means"]).max() > 0
+    graph = pipe.capture_step(*params, target, sc.loss)     # the fork / join is captured with the step
+    for k in names:
+        getattr(pipe, k).fill_(float("nan"))
+    graph.replay()
+    torch.cuda.synchronize()
+    for k in names:
+        c = getattr(pipe, k).cpu().numpy()                  # (the compositing atomics may sum in another order)
+        assert np.isfinite(c).all() and np.allclose(c, a[k], rtol=1e-2, atol=1e-3 * np.abs(a[k]).max()), k
