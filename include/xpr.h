@@ -93,6 +93,9 @@ int32_t xpr_version(void);           /* 10000*major + 100*minor + patch */
  *   left untouched (they are never read downstream).
  *   Arithmetic follows rule R1: fp32, every operation individually rounded, no FMA contraction,
  *   so that depth bits, rectangles and tile counts are bit-reproducible.
+ *   Two readings the paper does not fix and nothing can pin: the EWA Jacobian is evaluated at
+ *   x/z clamped to [-(cx + 0.15 W)/fx, ((W - cx) + 0.15 W)/fx] (likewise y; C6), and with the UT a Gaussian is culled
+ *   when any of its 7 sigma points has z <= 0 (C18).
  */
 int32_t xpr_project(int64_t N, const float* means, const float* scales, const float* quats,
                     const float* opacities, const float* sh, const xpr_camera* cam, const xpr_config* cfg,
