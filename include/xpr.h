@@ -2,7 +2,7 @@
  * xpr.h -- C-ABI boundary of libxpr.so: the tile-based splatting forward + backward hot path of
  * "XPR: An Extensible Cross-Platform Point-Based Differentiable Renderer" (arxiv 2606.11529),
  * hand-written CUDA for NVIDIA B200 (sm_100a).  Citations are PAPER.md line numbers ("PAPER L..")
- * plus the readings C1..C30 and arithmetic rules R1..R3 listed in DESIGN.md section 3.
+ * plus the readings C1..C32, L1..L6 and arithmetic rules R1..R3 listed in DESIGN.md section 3.
  *
  * Conventions
  *  - Every function returns an int32_t status (XPR_OK == 0).  No exceptions, no global state other
