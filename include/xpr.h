@@ -31,7 +31,8 @@
 extern "C" {
 #endif
 
-enum { XPR_OK = 0, XPR_ERR_INVALID_ARG = 1, XPR_ERR_CAPACITY = 2, XPR_ERR_CUDA = 3, XPR_ERR_UNSUPPORTED = 4 };
+enum { XPR_OK = 0, XPR_ERR_INVALID_ARG = 1, XPR_ERR_CAPACITY = 2, XPR_ERR_CUDA = 3, XPR_ERR_UNSUPPORTED = 4,
+       XPR_ERR_SCRATCH_LIMIT = 5 /* xpr_bin_sort_static: the sizes need more than XPR_STATIC_SCRATCH_BYTES of workspace */ };
 
 /* flags byte written per Gaussian by xpr_project */
 enum { XPR_FLAG_VISIBLE = 1, XPR_FLAG_CLAMP_U = 2, XPR_FLAG_CLAMP_V = 4,
@@ -171,6 +172,33 @@ int32_t xpr_bin_sort_cull(int64_t N, const float* depth, const int32_t* tile_rec
                           const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
                           uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
                           int64_t* num_pairs_host, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * xpr_bin_sort_static -- xpr_bin_sort / xpr_bin_sort_cull WITHOUT a caller workspace and without any allocation, for
+ * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ * The scratch is a static device array of XPR_STATIC_SCRATCH_BYTES (16 MiB) inside the library: every GPU that loads
+ * libxpr.so holds it until the process exits.  The call itself issues no cudaMalloc, cudaFree or allocating library
+ * routine; its first call on a device looks the array's address up (cudaGetSymbolAddress, with the current device) --
+ * make that first call at set-up, outside any stream capture.
+ *   Arguments and results exactly as xpr_bin_sort_cull (mean2d, conic_opac, lnv are read only when cfg->tile_cull != 0
+ *   and may be NULL otherwise: the call is then xpr_bin_sort), minus workspace / workspace_bytes.
+ *   Limit: the sizes must satisfy xpr_bin_sort_workspace(N, pair_capacity, tiles) <= XPR_STATIC_SCRATCH_BYTES, about
+ *   20 N + 9 pair_capacity + 272 tiles bytes -- e.g. N = 200 000 (view x Gaussian entries) with pair_capacity
+ *   = 1 048 576, or N = 262 144 with pair_capacity = 786 432, at 1920 x 1080 (8160 tiles); beyond it ->
+ *   XPR_ERR_SCRATCH_LIMIT before anything is launched (use xpr_bin_sort with a workspace of your own).
+ *   Sharing: all calls on a device use the SAME array, which keeps the previous call's contents.  Every call zero-fills
+ *   the part that must start at zero and writes every other part before reading it, so calls in stream order are
+ *   independent of each other; calls that OVERLAP on the GPU (two streams with no ordering between them, or this call
+ *   in two graphs replayed concurrently) race on the array and give undefined results.  In the asynchronous mode
+ *   (num_pairs_host == NULL) the counts xpr_bin_sort leaves in workspace bytes [0,16) stay inside the library: size
+ *   pair_capacity from an earlier synchronous call.
+ */
+enum { XPR_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024 };
+int32_t xpr_bin_sort_static(int64_t N, const float* depth, const int32_t* tile_rect, const uint32_t* tile_count,
+                            const float* mean2d, const float* conic_opac, const float* lnv,
+                            const xpr_camera* cam, const xpr_config* cfg, int64_t pair_capacity,
+                            uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* tile_ranges,
+                            int64_t* num_pairs_host, void* stream);
 
 /*
  * xpr_rasterize_fwd -- Shader stage (Algorithm 1, Listing 1).

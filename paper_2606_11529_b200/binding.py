@@ -15,6 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libxpr.so")
 
 XPR_OK, XPR_ERR_INVALID_ARG, XPR_ERR_CAPACITY, XPR_ERR_CUDA, XPR_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
+XPR_ERR_SCRATCH_LIMIT = 5
+XPR_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024
 FLAG_VISIBLE, FLAG_CLAMP_U, FLAG_CLAMP_V, FLAG_RGB_POS_R, FLAG_RGB_POS_G, FLAG_RGB_POS_B = 1, 2, 4, 8, 16, 32
 
 SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_project", "xpr_bin_sort_workspace",
@@ -23,7 +25,7 @@ SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_proje
            "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad",
            "xpr_lin_project", "xpr_bin_sort_lin", "xpr_lin_rasterize_fwd", "xpr_lin_rasterize_stats",
            "xpr_lin_rasterize_bwd", "xpr_lin_project_bwd", "xpr_rasterize_ray_feat_fwd", "xpr_rasterize_ray_feat_bwd",
-           "xpr_project_bwd_fill", "xpr_project_bwd_filled")
+           "xpr_project_bwd_fill", "xpr_project_bwd_filled", "xpr_bin_sort_static")
 
 
 class XprCamera(C.Structure):
@@ -186,6 +188,21 @@ def xpr_bin_sort(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, p
         return st, int(n_pairs.value)
     _check(st, "xpr_bin_sort")
     return st, int(n_pairs.value)
+
+
+def xpr_bin_sort_static(depth, tile_rect, tile_count, cam: XprCamera, cfg: XprConfig, pair_capacity: int, keys_sorted,
+                        vals_sorted, tile_ranges, cull_data=None, stream=None, sync: bool = True):
+    """xpr_bin_sort[_cull] on the library's static scratch (no workspace, no allocation; xpr.h).  Returns (status, I);
+    raises XprError (XPR_ERR_SCRATCH_LIMIT) when the sizes need more than XPR_STATIC_SCRATCH_BYTES."""
+    N = int(tile_count.shape[0])
+    n_pairs = C.c_int64(0)
+    cd = cull_data if cull_data is not None else (None, None, None)
+    st = lib().xpr_bin_sort_static(C.c_int64(N), _p(depth, _F32), _p(tile_rect, _I32), _p(tile_count, _I32),
+                                   _p(cd[0], _F32), _p(cd[1], _F32), _p(cd[2], _F32), C.byref(cam), C.byref(cfg),
+                                   C.c_int64(pair_capacity), _p(keys_sorted, _I64), _p(vals_sorted, _I32),
+                                   _p(tile_ranges, _I32), C.byref(n_pairs) if sync else None, _stream(stream))
+    _check(st, "xpr_bin_sort_static")
+    return st, (int(n_pairs.value) if sync else None)
 
 
 def xpr_rasterize_fwd(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, tile_ranges, image, final_T, n_contrib,

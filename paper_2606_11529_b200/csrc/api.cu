@@ -12,6 +12,9 @@ extern "C" const char* xpr_status_string(int32_t status) {
         case XPR_ERR_CAPACITY: return "XPR_ERR_CAPACITY: more tile-Gaussian pairs than pair_capacity";
         case XPR_ERR_CUDA: return "XPR_ERR_CUDA: CUDA runtime failure (see xpr_last_cuda_error)";
         case XPR_ERR_UNSUPPORTED: return "XPR_ERR_UNSUPPORTED: configuration outside the implemented path";
+        case XPR_ERR_SCRATCH_LIMIT:
+            return "XPR_ERR_SCRATCH_LIMIT: these sizes need more workspace than the static scratch of xpr_bin_sort_static "
+                   "(XPR_STATIC_SCRATCH_BYTES); use xpr_bin_sort with a caller-provided workspace";
         default: return "XPR: unknown status";
     }
 }

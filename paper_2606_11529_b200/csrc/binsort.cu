@@ -49,6 +49,7 @@
 //                     segment and chunk tables of the supertiles.
 //   final_kernel      per chunk of a supertile segment: masks, ballot ranking, look-back, scatter.
 #include "common.cuh"
+#include <mutex>
 
 namespace xpr {
 namespace {
@@ -1406,4 +1407,55 @@ extern "C" int32_t xpr_bin_sort_lin(int64_t N, const float* depth, const int32_t
     if (cfg && num_views(cfg) != 1) return XPR_ERR_UNSUPPORTED;
     return bin_sort_impl(false, N, depth, tile_rect, tile_count, nullptr, nullptr, nullptr, lin_rec, cam, cfg, pair_capacity,
                          keys_sorted, vals_sorted, tile_ranges, num_pairs_host, workspace, workspace_bytes, stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// xpr_bin_sort_static -- xpr_bin_sort / xpr_bin_sort_cull for callers that cannot allocate (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc): the workspace is a file-scope device array of
+// XPR_STATIC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.  The entry point calls no
+// cudaMalloc / cudaFree / allocating library routine; inputs and outputs are still the caller's.
+// In host code the array's NAME is a host-side stand-in, not a device address: its device address is taken once per
+// device, with that device current, by cudaGetSymbolAddress (below) and that pointer is what the kernels get.
+// All calls on a device share the array, which keeps the last call's contents: bin_sort_impl zero-fills everything
+// that must start at zero (header, chains, look-back words, counters: bytes [header, zero_end)) at the start of EVERY
+// call, and every other region is written before it is read.  Two calls that overlap on the GPU (different streams
+// without an ordering between them) race on the array.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_xpr_static_scratch[XPR_STATIC_SCRATCH_BYTES];
+
+static int32_t static_scratch_address(void** out) {
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static void* ptrs[MAX_DEV] = {};
+    int dev = -1;
+    XPR_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) return XPR_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptrs[dev]) {                      // set-up, once per device, with that device current
+        void* p = nullptr;
+        XPR_CUDA(cudaGetSymbolAddress(&p, g_xpr_static_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return XPR_ERR_UNSUPPORTED;
+        ptrs[dev] = p;
+    }
+    *out = ptrs[dev];
+    return XPR_OK;
+}
+
+extern "C" int32_t xpr_bin_sort_static(int64_t N, const float* depth, const int32_t* tile_rect,
+                                       const uint32_t* tile_count, const float* mean2d, const float* conic_opac,
+                                       const float* lnv, const xpr_camera* cam, const xpr_config* cfg,
+                                       int64_t pair_capacity, uint64_t* keys_sorted, uint32_t* vals_sorted,
+                                       uint32_t* tile_ranges, int64_t* num_pairs_host, void* stream) {
+    if (int32_t s = check_cam_cfg(cam, cfg)) return s;
+    if (N < 0 || pair_capacity < 0 || pair_capacity >= (1LL << 30)) return XPR_ERR_INVALID_ARG;
+    if (N >= (1LL << 30)) return XPR_ERR_UNSUPPORTED;
+    const int64_t T64 = (int64_t)tiles_x(cam) * tiles_y(cam) * num_views(cfg);
+    if (T64 > (1 << 24)) return XPR_ERR_UNSUPPORTED;
+    // the sizes this entry point serves: those whose workspace fits the static array
+    if (make_layout(N, pair_capacity, (int32_t)T64).total > (size_t)XPR_STATIC_SCRATCH_BYTES) return XPR_ERR_SCRATCH_LIMIT;
+    void* ws = nullptr;
+    if (int32_t s = static_scratch_address(&ws)) return s;
+    const bool cull = cfg->tile_cull != 0;
+    return bin_sort_impl(cull, N, depth, tile_rect, tile_count, mean2d, conic_opac, lnv, nullptr, cam, cfg, pair_capacity,
+                         keys_sorted, vals_sorted, tile_ranges, num_pairs_host, ws, (size_t)XPR_STATIC_SCRATCH_BYTES, stream);
 }

@@ -266,3 +266,21 @@ def test_ray_feature_entry_points_reject_bad_arguments(lib):
     assert bwd(N4, *[one] * 11, null, *[one] * 5) == 1                                       # dL_ddepth NULL
     assert bwd(N4, *[one] * 16, null) == 1                                                   # g_depth NULL
     assert bwd(N0, *[null] * 5, one, null, one, one, one, one, one, one, *[null] * 4) == 0   # N = 0: nothing to do
+
+
+def test_bin_sort_static_rejects_before_launch(lib):
+    """xpr_bin_sort_static (no-allocation entry point): argument errors and the size limit are reported before any CUDA call."""
+    cam, cfg = _cam_cfg()
+    null, one = C.c_void_p(0), C.c_void_p(256)
+    call = lambda n, cap, cm=cam, cf=cfg: lib.xpr_bin_sort_static(C.c_int64(n), one, one, one, null, null, null, C.byref(cm),
+                                                                 C.byref(cf), C.c_int64(cap), one, one, one, None, null)
+    assert call(-1, 1024) == 1
+    assert call(4, -1) == 1
+    assert call(1 << 30, 1024) == 4
+    assert lib.xpr_bin_sort_static(C.c_int64(4), one, one, one, null, null, null, None, C.byref(cfg), C.c_int64(16), one, one,
+                                   one, None, null) == 1
+    assert call(4, 1 << 22) == 5 and call(2_000_000, 1024) == 5            # beyond XPR_STATIC_SCRATCH_BYTES
+    assert lib.xpr_status_string(C.c_int32(5)).decode().startswith("XPR_ERR_SCRATCH_LIMIT")
+    from paper_2606_11529_b200 import binding
+    src = open(os.path.join(ROOT, "include", "xpr.h")).read()
+    assert "XPR_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024" in src and binding.XPR_STATIC_SCRATCH_BYTES == 16 * 1024 * 1024
