@@ -698,9 +698,30 @@ rows_kernel(int TW, int TH, int TH_view, const uint32_t* __restrict__ vidx, cons
         int xa = r.x, xb = r.z;                                 // kept tiles of this row: [xa, xb)
         if (CULL == 2) {
             // LinPrim: the kept tiles of the row are an interval (convexity above): its first and last tile by the exact predicate
+            // (one interval [a, b) inside [xa, xb)).  The tile under the projected centre is kept whenever the row has a
+            // kept tile near the centre column: from such a seed both ends are found by bisection (the predicate is
+            // monotone on either side of a kept tile), O(log w) evaluations of the 64-term bound instead of one per
+            // dropped tile; without a kept seed (rows far from the centre of a slanted primitive) the row is shrunk
+            // from both ends tile by tile.  Either way the predicate alone decides: the result is the oracle's.
             const float* rec = lin_rec + 20 * (size_t)g;
-            while (xa < xb && !lin_tile_keep(rec, xa, ty, lin_req)) ++xa;
-            while (xb > xa && !lin_tile_keep(rec, xb - 1, ty, lin_req)) --xb;
+            const int seed = min(max((int)floorf(rec[0] * (1.0f / (float)TILE)), xa), xb - 1);
+            if (lin_tile_keep(rec, seed, ty, lin_req)) {
+                int lo = xa, hi = seed;                    // first kept tile in [xa, seed]: keep(hi) holds
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (lin_tile_keep(rec, mid, ty, lin_req)) hi = mid; else lo = mid + 1;
+                }
+                xa = hi;
+                lo = seed; hi = xb - 1;                    // last kept tile in [seed, xb - 1]: keep(lo) holds
+                while (lo < hi) {
+                    const int mid = (lo + hi + 1) >> 1;
+                    if (lin_tile_keep(rec, mid, ty, lin_req)) lo = mid; else hi = mid - 1;
+                }
+                xb = lo + 1;
+            } else {
+                while (xa < xb && !lin_tile_keep(rec, xa, ty, lin_req)) ++xa;
+                while (xb > xa && !lin_tile_keep(rec, xb - 1, ty, lin_req)) --xb;
+            }
         }
         if (CULL == 1) {
             const int tyv = ty % TH_view;              // batch of views: the tile rows of view v are offset by v * TH_view
