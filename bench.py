@@ -51,6 +51,12 @@ def parse():
     ap.add_argument("--tile-order", type=int, default=-1, choices=(-1, 0, 1),
                     help="1: compositing kernels walk the tiles longest list first (xpr_config.tile_order; scheduling "
                          "only); -1: the pipeline's default (on for 64 <= tiles < 4096)")
+    ap.add_argument("--fuse-loss", type=int, default=1, choices=(0, 1),
+                    help="1: the loss gradient is formed inside the compositing backward (xpr_rasterize_bwd_loss) instead of a "
+                         "separate xpr_loss_grad pass (colour pass of the 2D evaluation only; same results)")
+    ap.add_argument("--overlap-fill", type=int, default=-1, choices=(-1, 0, 1, 2),
+                    help="pipeline option overlap_fill: the zero-fill of the parameter gradients on a second stream, forked at the "
+                         "compositing backward (1) or at the binning stage (2); 0 off; -1 the pipeline's default")
     ap.add_argument("--features", type=int, default=0, choices=(0, 1),
                     help="1: also render the depth image and the accumulated opacity and take their gradients "
                          "(SURVEY 8(f) f3, DESIGN.md 6.8; with --ray-eval 1 through the ray kernels; not part of the headline workload)")
@@ -237,6 +243,9 @@ def run_ours(args):
         raise SystemExit("bench.py: --views V needs V cameras in the scene (config 5 has four) and the 2D colour pass")
     cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval,
                tile_order=args.tile_order, features=args.features)
+    if args.overlap_fill >= 0:
+        cfg["overlap_fill"] = args.overlap_fill
+    cfg["fuse_loss"] = args.fuse_loss
     params = pipeline.scene_to_device(sc, dev)
     if V > 1:
         target = torch.from_numpy(np.stack([sc.target(args.view + v) for v in range(V)])).to(dev)
@@ -258,6 +267,17 @@ def run_ours(args):
         xb.xpr_loss_grad(sc.loss, image, target, dL_buf)
         return dL_buf
 
+    fused = pipe.can_fuse_loss()         # loss gradient inside the compositing backward: the loss_grad stage is then empty
+
+    def loss_stage(p):
+        return None if fused else loss_grad(p.image)
+
+    def bwd_stage(p, dL):
+        if fused:
+            p.rasterize_bwd_loss(target, sc.loss)
+        else:
+            p.rasterize_bwd(dL, *feat_grads)
+
     stage_names = ("project", "bin_sort", "rasterize_fwd", "loss_grad", "rasterize_bwd", "project_bwd")
 
     def step(events=None, sync_count=False):
@@ -270,8 +290,8 @@ def run_ours(args):
             pipe.pixel_info(); pipe.project_ray()
         ev(); pipe.bin_sort() if sync_count else pipe.bin_sort_async()
         ev(); pipe.rasterize_fwd()
-        ev(); dL = loss_grad(pipe.image)
-        ev(); pipe.rasterize_bwd(dL, *feat_grads)
+        ev(); dL = loss_stage(pipe)
+        ev(); bwd_stage(pipe, dL)
         ev(); pipe.project_bwd()
         ev()
 
@@ -296,6 +316,8 @@ def run_ours(args):
     # project, bin_sort (compact, 4 depth passes, rank scan, rows, supertile words, tile scan, supertile passes, final),
     # fwd, loss_grad, bwd, project_bwd
     launches_per_step = 1 + (1 + 4 + 1 + 1 + 1 + 1 + tile_passes + 1) + 1 + 1 + 1 + 1
+    if fused:
+        launches_per_step -= 1              # no loss_grad kernel
     if args.ray_eval:
         launches_per_step += 3              # pixel_info, project_ray, ray_bwd
     if args.features:
@@ -402,8 +424,7 @@ def run_ours(args):
                 pipe0.pixel_info(); pipe0.project_ray()
             pipe0.bin_sort() if sync else pipe0.bin_sort_async()
             pipe0.rasterize_fwd()
-            xb.xpr_loss_grad(sc.loss, pipe0.image, target, dL_buf)
-            pipe0.rasterize_bwd(dL_buf, *feat_grads)
+            bwd_stage(pipe0, loss_stage(pipe0))
             pipe0.project_bwd()
         for _ in range(3):
             step0(True)
@@ -517,7 +538,7 @@ def run_ours(args):
             if args.ray_eval:
                 pipe.pixel_info(); pipe.project_ray()
             pipe.bin_sort_async(); pipe.rasterize_fwd()
-            pipe.rasterize_bwd(loss_grad(pipe.image), *feat_grads); pipe.project_bwd()
+            bwd_stage(pipe, loss_stage(pipe)); pipe.project_bwd()
 
         def e2e_step():       # one stream: copy in, step, copy out (the latency of a single step)
             for d, h in zip(dev_in, host_in):
@@ -616,7 +637,7 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "views": V, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "pairs": n_pairs,
+                           "image": [cam.width, cam.height], "views": V, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "fuse_loss": int(fused), "pairs": n_pairs,
                            "candidate_pairs": n_cand, "rows": n_rows, "supertile_words": n_words, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "supertile_digits_on_words": tile_passes,
                                            "on_pairs": 0},

@@ -237,6 +237,19 @@ int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t 
                           const float* final_T, const uint32_t* n_contrib, const float* dL_dimage,
                           float* g_mean2d, float* g_conic, float* g_opac, float* g_rgb,
                           int32_t zero_init, void* stream);
+/*
+ * xpr_rasterize_bwd_loss -- xpr_rasterize_bwd for the two losses BASELINE.json's configs name, with the loss gradient
+ * formed inside the kernel: dL/dimage = sign(I - target) (loss_kind 0, L = sum |I - target|) or 2 (I - target)
+ * (loss_kind 1, L = sum (I - target)^2) from `image` (the output of xpr_rasterize_fwd) and `target`, both [H,W,3]
+ * ([V,H,W,3] for a batch of views) -- the values xpr_loss_grad would write, so every result is that of xpr_loss_grad
+ * followed by xpr_rasterize_bwd, one pass over the image and one launch less.  Other arguments and errors as
+ * xpr_rasterize_bwd; loss_kind outside {0, 1} -> XPR_ERR_INVALID_ARG.
+ */
+int32_t xpr_rasterize_bwd_loss(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
+                               const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* image,
+                               const float* final_T, const uint32_t* n_contrib, int32_t loss_kind, const float* target,
+                               float* g_mean2d, float* g_conic, float* g_opac, float* g_rgb, int32_t zero_init,
+                               void* stream);
 
 /*
  * xpr_project_bwd -- reverse mode through projection (EWA or UT) and SH (DESIGN.md section 3,

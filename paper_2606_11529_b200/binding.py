@@ -25,7 +25,7 @@ SYMBOLS = ("xpr_status_string", "xpr_last_cuda_error", "xpr_version", "xpr_proje
            "xpr_ray_bwd", "xpr_rasterize_feat_fwd", "xpr_rasterize_feat_bwd", "xpr_depth_bwd", "xpr_rasterize_featn_fwd", "xpr_rasterize_featn_bwd", "xpr_loss_grad",
            "xpr_lin_project", "xpr_bin_sort_lin", "xpr_lin_rasterize_fwd", "xpr_lin_rasterize_stats",
            "xpr_lin_rasterize_bwd", "xpr_lin_project_bwd", "xpr_rasterize_ray_feat_fwd", "xpr_rasterize_ray_feat_bwd",
-           "xpr_project_bwd_fill", "xpr_project_bwd_filled", "xpr_bin_sort_static")
+           "xpr_project_bwd_fill", "xpr_project_bwd_filled", "xpr_bin_sort_static", "xpr_rasterize_bwd_loss")
 
 
 class XprCamera(C.Structure):
@@ -227,6 +227,17 @@ def xpr_rasterize_bwd(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, ti
                                    _p(tile_ranges, _I32), _p(final_T, _F32), _p(n_contrib, _I32), _p(dL_dimage, _F32),
                                    _p(g_mean2d, _F32), _p(g_conic, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
                                    C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_bwd")
+
+
+def xpr_rasterize_bwd_loss(cam: XprCamera, cfg: XprConfig, shade_rec, vals_sorted, tile_ranges, image, final_T, n_contrib,
+                           kind: str, target, g_mean2d, g_conic, g_opac, g_rgb, zero_init: bool = True, stream=None):
+    """xpr_loss_grad + xpr_rasterize_bwd in one launch: kind "l1" (sum |I - target|) or "l2" (sum (I - target)^2)."""
+    N = int(shade_rec.shape[0])
+    _check(lib().xpr_rasterize_bwd_loss(C.byref(cam), C.byref(cfg), C.c_int64(N), _p(shade_rec, _F32), _p(vals_sorted, _I32),
+                                        _p(tile_ranges, _I32), _p(image, _F32), _p(final_T, _F32), _p(n_contrib, _I32),
+                                        C.c_int32({"l1": 0, "l2": 1}[kind]), _p(target, _F32), _p(g_mean2d, _F32),
+                                        _p(g_conic, _F32), _p(g_opac, _F32), _p(g_rgb, _F32),
+                                        C.c_int32(1 if zero_init else 0), _stream(stream)), "xpr_rasterize_bwd_loss")
 
 
 def xpr_project_bwd_fill(cfg: XprConfig, g_means, g_scales, g_quats, g_opacities, g_sh, stream=None):

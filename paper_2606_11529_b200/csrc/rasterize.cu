@@ -287,7 +287,11 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
                      const uint32_t* __restrict__ n_contrib, const float* __restrict__ dL,
                      const float* __restrict__ dL_dD, const float* __restrict__ dL_dA, float* __restrict__ g_mean2d,
                      float* __restrict__ g_conic, float* __restrict__ g_opac, float* __restrict__ g_rgb,
-                     float* __restrict__ g_depth) {
+                     float* __restrict__ g_depth, int loss_kind, const float* __restrict__ image,
+                     const float* __restrict__ target) {
+    // loss_kind < 0: dL is the incoming gradient.  loss_kind 0 / 1 (xpr_rasterize_bwd_loss): the gradient of the loss
+    // sum |I - target| / sum (I - target)^2 is formed here from the rendered image and the target, the values
+    // xpr_loss_grad would have written (one pass over the image and one launch less per step).
     constexpr int THREADS = BLOCK / PPT, B = THREADS, NP = PPT / 2;
     __shared__ float4 s_rec[STAGES][3 * B];
     __shared__ uint32_t s_idx[STAGES][B];
@@ -320,7 +324,16 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
                 const int64_t pid = vbase + (int64_t)py * P.W + px;
                 n[k] = n_contrib[pid];
                 t[h] = final_T[pid];
-                a0[h] = dL[3 * pid]; a1[h] = dL[3 * pid + 1]; a2[h] = dL[3 * pid + 2];
+                if (loss_kind < 0) {
+                    a0[h] = dL[3 * pid]; a1[h] = dL[3 * pid + 1]; a2[h] = dL[3 * pid + 2];
+                } else {
+                    const float d0 = image[3 * pid] - target[3 * pid], d1 = image[3 * pid + 1] - target[3 * pid + 1],
+                                d2 = image[3 * pid + 2] - target[3 * pid + 2];
+                    auto sgn = [](float d) { return d > 0.0f ? 1.0f : (d < 0.0f ? -1.0f : d); };
+                    a0[h] = loss_kind == 0 ? sgn(d0) : 2.0f * d0;
+                    a1[h] = loss_kind == 0 ? sgn(d1) : 2.0f * d1;
+                    a2[h] = loss_kind == 0 ? sgn(d2) : 2.0f * d2;
+                }
                 if (FEAT) { aD[h] = dL_dD[pid]; gA = dL_dA[pid]; }
             }
             // Q = g . S behind the last entry = T_final (g . bg) (C13) (FEAT: - gA T_final)
@@ -515,10 +528,11 @@ int32_t launch_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, cons
                    const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* final_T,
                    const uint32_t* n_contrib, const float* dL_dimage, const float* dL_ddepth, const float* dL_dalpha,
                    float* g_mean2d, float* g_conic, float* g_opac, float* g_rgb, float* g_depth, int32_t zero_init,
-                   void* stream) {
+                   void* stream, int loss_kind = -1, const float* image = nullptr, const float* target = nullptr) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0) return XPR_ERR_INVALID_ARG;
-    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4) || !aligned(dL_dimage, 4))
+    if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4)) return XPR_ERR_INVALID_ARG;
+    if (loss_kind < 0 ? !aligned(dL_dimage, 4) : (loss_kind > 1 || !aligned(image, 4) || !aligned(target, 4)))
         return XPR_ERR_INVALID_ARG;
     if (FEAT && (!aligned(dL_ddepth, 4) || !aligned(dL_dalpha, 4))) return XPR_ERR_INVALID_ARG;
     if (N == 0) return XPR_OK;
@@ -547,7 +561,8 @@ int32_t launch_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, cons
 #define XPR_BWD(PPT_)                                                                                               \
     rasterize_bwd_kernel<PPT_, FEAT><<<T, BLOCK / PPT_, 0, st>>>(                                                     \
         P, reinterpret_cast<const float4*>(shade_rec), vals_sorted, reinterpret_cast<const uint2*>(tile_ranges),     \
-        final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth)
+        final_T, n_contrib, dL_dimage, dL_ddepth, dL_dalpha, g_mean2d, g_conic, g_opac, g_rgb, g_depth, loss_kind,   \
+        image, target)
     if (T >= FWD_PPT2_MIN_TILES) XPR_BWD(XPR_BWD_PPT_LARGE);
     else                         XPR_BWD(XPR_BWD_PPT_SMALL);
 #undef XPR_BWD
@@ -613,6 +628,16 @@ extern "C" int32_t xpr_rasterize_bwd(const xpr_camera* cam, const xpr_config* cf
                                      float* g_conic, float* g_opac, float* g_rgb, int32_t zero_init, void* stream) {
     return launch_bwd<false>(cam, cfg, N, shade_rec, vals_sorted, tile_ranges, final_T, n_contrib, dL_dimage, nullptr,
                              nullptr, g_mean2d, g_conic, g_opac, g_rgb, nullptr, zero_init, stream);
+}
+
+extern "C" int32_t xpr_rasterize_bwd_loss(const xpr_camera* cam, const xpr_config* cfg, int64_t N, const float* shade_rec,
+                                          const uint32_t* vals_sorted, const uint32_t* tile_ranges, const float* image,
+                                          const float* final_T, const uint32_t* n_contrib, int32_t loss_kind,
+                                          const float* target, float* g_mean2d, float* g_conic, float* g_opac,
+                                          float* g_rgb, int32_t zero_init, void* stream) {
+    if (loss_kind != 0 && loss_kind != 1) return XPR_ERR_INVALID_ARG;
+    return launch_bwd<false>(cam, cfg, N, shade_rec, vals_sorted, tile_ranges, final_T, n_contrib, nullptr, nullptr, nullptr,
+                             g_mean2d, g_conic, g_opac, g_rgb, nullptr, zero_init, stream, loss_kind, image, target);
 }
 
 extern "C" int32_t xpr_rasterize_feat_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N,

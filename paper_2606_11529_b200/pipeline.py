@@ -39,8 +39,11 @@ class SplatPipeline:
         # overlap_fill = 1: the zero-fill of the parameter gradients (xpr_project_bwd_fill: HBM traffic without inputs) runs on
         # a second stream under the compositing backward.  Off by default: measured on config 3 / 5 the compositing kernel
         # slows down by what the fill saves (0.326 -> 0.351 ms, project_bwd 0.083 -> 0.045 ms: step -1 %), DESIGN.md 6.5
-        self.overlap_fill = bool(cfg.get("overlap_fill", 0)) if isinstance(cfg, dict) else False
+        self.overlap_fill = int(cfg.get("overlap_fill", 0)) if isinstance(cfg, dict) else 0
         self._filled = False
+        # fuse_loss: step_async() forms dL/dimage of the two configured losses inside the compositing backward
+        # (xpr_rasterize_bwd_loss) instead of a separate xpr_loss_grad pass; colour pass of the 2D evaluation only
+        self.fuse_loss = bool(cfg.get("fuse_loss", 1)) if isinstance(cfg, dict) else True
         # f3: constant (dL/dD, dL/dA) of a loss that is linear in the features; step_async() feeds them to the backward
         self.feature_grads = None
         self.cfg = cfg if isinstance(cfg, xb.XprConfig) else xb.make_config(cfg)
@@ -120,6 +123,7 @@ class SplatPipeline:
         xb.xpr_project_ray(means, scales, quats, self.cam, self.tile_count, self.ray_rec)
 
     def bin_sort(self):
+        self._fork_fill(2)
         while True:
             st, n = xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg,
                                     self.pair_capacity, self.keys_sorted, self.vals_sorted, self.tile_ranges,
@@ -135,6 +139,7 @@ class SplatPipeline:
         """xpr_bin_sort without the host read-back of I (num_pairs_host = NULL): nothing in the step waits for
         the host, so the whole step can be enqueued ahead or captured in a CUDA graph.  The buffers must have
         been sized by an earlier bin_sort(); pairs_on_device() / check_capacity() read the count afterwards."""
+        self._fork_fill(2)
         xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg, self.pair_capacity,
                         self.keys_sorted, self.vals_sorted, self.tile_ranges, self.workspace, sync=False,
                         cull_data=self._cull_data())
@@ -186,8 +191,8 @@ class SplatPipeline:
         xb.xpr_rasterize_fwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.image,
                              self.final_T, self.n_contrib)
 
-    def _fork_fill(self):
-        if not self.overlap_fill:
+    def _fork_fill(self, where: int):
+        if self.overlap_fill != where or self._filled:
             return
         if not hasattr(self, "_side"):
             self._side = torch.cuda.Stream(device=self.device)
@@ -201,7 +206,7 @@ class SplatPipeline:
 
     def rasterize_bwd(self, dL_dimage, dL_ddepth=None, dL_dalpha=None):
         self._feat_bwd = False
-        self._fork_fill()
+        self._fork_fill(1)
         if self.features and (dL_ddepth is not None or dL_dalpha is not None):
             z = lambda t: torch.zeros(self.H, self.W, dtype=torch.float32, device=self.device) if t is None else t
             if self.ray_eval:
@@ -225,6 +230,17 @@ class SplatPipeline:
         xb.xpr_rasterize_bwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.final_T,
                              self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb,
                              zero_init=True)
+
+    def can_fuse_loss(self) -> bool:
+        return self.fuse_loss and not self.ray_eval and not self.features
+
+    def rasterize_bwd_loss(self, target, loss: str):
+        """xpr_loss_grad + xpr_rasterize_bwd in one launch (the loss gradient is formed in the kernel's prologue)."""
+        self._feat_bwd = False
+        self._fork_fill(1)
+        xb.xpr_rasterize_bwd_loss(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.image,
+                                  self.final_T, self.n_contrib, loss, target, self.g_mean2d, self.g_conic, self.g_opac,
+                                  self.g_rgb, zero_init=True)
 
     # ---- N-channel features (f3): replay of the finished colour pass ---------------------------
     def rasterize_featn_fwd(self, feat, feat_img=None):
@@ -292,8 +308,11 @@ class SplatPipeline:
             self.project_ray()
         self.bin_sort_async()
         self.rasterize_fwd()
-        xb.xpr_loss_grad(loss, self.image, target, self._dL)
-        self.rasterize_bwd(self._dL, *(self.feature_grads or (None, None)))
+        if self.can_fuse_loss():
+            self.rasterize_bwd_loss(target, loss)
+        else:
+            xb.xpr_loss_grad(loss, self.image, target, self._dL)
+            self.rasterize_bwd(self._dL, *(self.feature_grads or (None, None)))
         self.project_bwd()
 
     def capture_step(self, means, scales, quats, opacities, sh, target, loss: str, pixel_info: bool = False):

@@ -284,3 +284,16 @@ def test_bin_sort_static_rejects_before_launch(lib):
     from paper_2606_11529_b200 import binding
     src = open(os.path.join(ROOT, "include", "xpr.h")).read()
     assert "XPR_STATIC_SCRATCH_BYTES = 16 * 1024 * 1024" in src and binding.XPR_STATIC_SCRATCH_BYTES == 16 * 1024 * 1024
+
+
+def test_rasterize_bwd_loss_rejects_bad_arguments(lib):
+    cam, cfg = _cam_cfg()
+    null, one, odd = C.c_void_p(0), C.c_void_p(16), C.c_void_p(18)
+    # shade_rec vals ranges image final_T n_contrib | kind target | g_mean2d g_conic g_opac g_rgb
+    f = lambda n, kind, *a: lib.xpr_rasterize_bwd_loss(C.byref(cam), C.byref(cfg), C.c_int64(n), *a[:6], C.c_int32(kind), *a[6:],
+                                                       C.c_int32(1), null)
+    assert f(4, 2, *[one] * 11) == 1 and f(4, -1, *[one] * 11) == 1          # loss_kind outside {0, 1}
+    assert f(-1, 0, *[one] * 11) == 1
+    assert f(4, 0, one, one, one, null, *[one] * 7) == 1                      # image NULL
+    assert f(4, 1, *[one] * 6, odd, *[one] * 4) == 1                          # target misaligned
+    assert f(0, 0, null, null, one, one, one, one, one, *[null] * 4) == 0     # N = 0: nothing to do

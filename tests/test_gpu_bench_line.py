@@ -26,7 +26,8 @@ def test_bench_line_ours():
         assert k in d, k
     assert d["n_gpus"] == 1 and d["steps"] == 3 and d["value"] > 0 and d["vs_baseline"] is None
     assert "workload" in d["config"] and "model" not in d["config"]
-    assert d["gpu_launches"] == 3 * 16          # 11 launches of xpr_bin_sort (one supertile-digit pass); + xpr_loss_grad
+    assert d["gpu_launches"] == 3 * 15          # 11 launches of xpr_bin_sort (one supertile-digit pass); loss gradient fused
+    assert d["config"]["fuse_loss"] == 1 and d["stage_ms"]["loss_grad"] < 0.005
     r = d["roofline"]
     assert r["bound"] in ("hbm", "alu", "tensor") and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
     assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0 and d["e2e"]["value"] > 0
@@ -59,10 +60,15 @@ def test_bench_line_rendered_features():
 def test_bench_line_reports_n_channel_feature_timings():
     d = _run("--featn", "5", "--no-cpu-baseline", "--no-e2e", "--no-graph")
     assert d["featn"]["C"] == 5 and d["featn"]["fwd_ms"] > 0 and d["featn"]["bwd_ms"] > 0
-    assert d["gpu_launches"] == 3 * 16          # the step itself is unchanged
+    assert d["gpu_launches"] == 3 * 15          # the step itself is unchanged
 
 
 def test_bench_line_batch_of_views():
     d = _run("--config", "5", "--views", "2", "--no-cpu-baseline", "--no-e2e", "--no-graph")
     assert d["config"]["views"] == 2 and d["value"] > 0
-    assert d["gpu_launches"] == 3 * 16          # a batch of views costs the launches of one view
+    assert d["gpu_launches"] == 3 * 15          # a batch of views costs the launches of one view
+
+
+def test_bench_line_separate_loss_kernel():
+    d = _run("--fuse-loss", "0", "--no-cpu-baseline", "--no-e2e", "--no-graph", "--no-plain")
+    assert d["config"]["fuse_loss"] == 0 and d["gpu_launches"] == 3 * 16 and d["stage_ms"]["loss_grad"] > 0.005

@@ -332,3 +332,38 @@ def test_overlapped_zero_fill_gives_the_same_gradients():
     for k in names:
         c = getattr(pipe, k).cpu().numpy()                  # (the compositing atomics may sum in another order)
         assert np.isfinite(c).all() and np.allclose(c, a[k], rtol=1e-2, atol=1e-3 * np.abs(a[k]).max()), k
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("config,n,wh", [(1, None, None), (2, 20000, (320, 240))])
+def test_fused_loss_backward_matches_separate_loss_grad(config, n, wh):
+    """xpr_rasterize_bwd_loss (loss gradient formed in the kernel's prologue) against xpr_loss_grad followed by
+    xpr_rasterize_bwd: the same per-pixel dL values enter the same arithmetic, so the 2D gradients agree up to the order
+    of the fp32 atomics (the bar of the GPU-vs-GPU comparisons: a handful of elements outside 1e-3 |ref| + 1e-6); both
+    losses (config 1: sum of squares, config 2: sum of absolute differences)."""
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline
+    sc = scenes.make_scene(config, n_override=n, image_override=wh)
+    cfg = scenes.default_render_config(sc)
+    params = pipeline.scene_to_device(sc)
+    target = torch.from_numpy(sc.target(0)).cuda()
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg)
+    pipe.forward(*params)
+    dL = torch.empty_like(pipe.image)
+    xb.xpr_loss_grad(sc.loss, pipe.image, target, dL)
+    pipe.rasterize_bwd(dL)
+    torch.cuda.synchronize()
+    names = ("g_mean2d", "g_conic", "g_opac", "g_rgb")
+    ref = {k: getattr(pipe, k).cpu().numpy().copy() for k in names}
+    for k in names:
+        getattr(pipe, k).fill_(float("nan"))
+    assert pipe.can_fuse_loss()
+    pipe.rasterize_bwd_loss(target, sc.loss)
+    torch.cuda.synchronize()
+    total = bad = 0
+    for k in names:
+        got = getattr(pipe, k).cpu().numpy()
+        assert np.isfinite(got).all() and np.abs(ref[k]).max() > 0
+        b, _ = pu.grad_violations(got, ref[k])
+        bad += int(b.sum()); total += b.size
+    assert bad <= max(4, 2e-5 * total), (bad, total)
