@@ -12,6 +12,7 @@
 #include <math.h>
 
 #include "common.cuh"
+#include "packed.cuh"
 
 namespace xpr {
 namespace {
@@ -249,7 +250,7 @@ __device__ __forceinline__ void load_sh(const float* __restrict__ sh, int64_t i,
 //      the packed shader record.
 // Every Gaussian runs exactly the arithmetic of the one-thread version (same functions, same inputs): the outputs
 // are bit-identical.
-// measured on config 3 (us): 128 threads x 2: 49.2; 128 x 4: 50.2; 256 x 8: 51.3; 256 x 2: 52.1; 256 x 4 (72 registers):
+// measured on config 3 (us), before the inputs were staged through shared memory: 128 threads x 2: 49.2; 128 x 4: 50.2; 256 x 8: 51.3; 256 x 2: 52.1; 256 x 4 (72 registers):
 // 57.5; one thread per Gaussian without compaction: 48.5 -- the kernel is bound by the latency of its gathers, not by issue
 #ifndef XPR_PROJ_THREADS
 #define XPR_PROJ_THREADS 128
@@ -280,6 +281,28 @@ project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __r
     const int64_t base = (int64_t)blockIdx.x * PROJ_CHUNK;
     const int n_here = (int)min((int64_t)PROJ_CHUNK, N - base);
     if (tid == 0) { s_na = 0u; s_nb = 0u; }
+    // ---- staging: the CTA's 44 input bytes per Gaussian (means, scales, quats, opacities: four contiguous runs) go to
+    // shared memory with 16-byte cp.async, all in flight at once and without registers -- the per-thread loads of the
+    // phases kept ~18 KB in flight per SM where latency x bandwidth asks for ~35 KB (the kernel was bound by the
+    // latency of its loads at 1/3 of the DRAM peak).  Phases A and B then read shared memory only.
+    __shared__ __align__(16) float s_mu[3 * PROJ_CHUNK], s_sc[3 * PROJ_CHUNK], s_q[4 * PROJ_CHUNK], s_o[PROJ_CHUNK];
+    {
+        const float* gm = means + 3 * base; const float* gs = scales + 3 * base;
+        const float* gq = quats + 4 * base; const float* go = opac + base;
+        const bool bulk = n_here == PROJ_CHUNK && ((reinterpret_cast<uintptr_t>(gm) | reinterpret_cast<uintptr_t>(gs) |
+                                                    reinterpret_cast<uintptr_t>(gq) | reinterpret_cast<uintptr_t>(go)) & 15u) == 0;
+        if (bulk) {
+            for (int v = tid; v < 3 * PROJ_CHUNK / 4; v += PROJ_THREADS) { cp_async16(s_mu + 4 * v, gm + 4 * v); cp_async16(s_sc + 4 * v, gs + 4 * v); }
+            for (int v = tid; v < PROJ_CHUNK; v += PROJ_THREADS) cp_async16(s_q + 4 * v, gq + 4 * v);
+            for (int v = tid; v < PROJ_CHUNK / 4; v += PROJ_THREADS) cp_async16(s_o + 4 * v, go + 4 * v);
+            cp_async_commit();
+            cp_async_wait<0>();
+        } else {        // last chunk or unaligned arrays: element by element
+            for (int v = tid; v < 3 * n_here; v += PROJ_THREADS) { s_mu[v] = __ldg(gm + v); s_sc[v] = __ldg(gs + v); }
+            for (int v = tid; v < 4 * n_here; v += PROJ_THREADS) s_q[v] = __ldg(gq + v);
+            for (int v = tid; v < n_here; v += PROJ_THREADS) s_o[v] = __ldg(go + v);
+        }
+    }
     __syncthreads();
     const uint32_t lt = (1u << lane) - 1u;
     // ---- phase A ---------------------------------------------------------------------------------------------
@@ -289,7 +312,7 @@ project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __r
         bool keep = false;
         if (j < n_here) {
             const int64_t i = base + j;
-            const float m0 = __ldg(means + 3 * i), m1 = __ldg(means + 3 * i + 1), m2 = __ldg(means + 3 * i + 2);
+            const float m0 = s_mu[3 * j], m1 = s_mu[3 * j + 1], m2 = s_mu[3 * j + 2];
             const float pz = ((P.W[6] * m0 + P.W[7] * m1) + P.W[8] * m2) + P.t[2];     // = F.p[2] of project_geometry
             keep = pz > P.z_near;
             if (!keep) { tcount[vo + i] = 0u; flags[vo + i] = 0; }
@@ -309,12 +332,13 @@ project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __r
         Fwd F;
         int64_t i = 0;
         if (idx < na) {
-            i = base + s_a[idx];
-            const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
-            const float sc[3] = {__ldg(scales + 3 * i), __ldg(scales + 3 * i + 1), __ldg(scales + 3 * i + 2)};
-            const float4 q4 = __ldg(reinterpret_cast<const float4*>(quats) + i);
+            const int j = s_a[idx];
+            i = base + j;
+            const float mu[3] = {s_mu[3 * j], s_mu[3 * j + 1], s_mu[3 * j + 2]};
+            const float sc[3] = {s_sc[3 * j], s_sc[3 * j + 1], s_sc[3 * j + 2]};
+            const float4 q4 = reinterpret_cast<const float4*>(s_q)[j];
             const float q[4] = {q4.x, q4.y, q4.z, q4.w};
-            vis = project_geometry(P, mu, sc, q, __ldg(opac + i), F);
+            vis = project_geometry(P, mu, sc, q, s_o[j], F);
             if (!vis) { tcount[vo + i] = 0u; flags[vo + i] = 0; }
         }
         const uint32_t m = __ballot_sync(0xffffffffu, vis);
@@ -338,13 +362,14 @@ project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __r
     // ---- phase C ---------------------------------------------------------------------------------------------
     const int nb = (int)s_nb;
     for (int idx = tid; idx < nb; idx += PROJ_THREADS) {
-        const int64_t i = base + s_b[idx];
-        const float mu[3] = {__ldg(means + 3 * i), __ldg(means + 3 * i + 1), __ldg(means + 3 * i + 2)};
+        const int jb = s_b[idx];
+        const int64_t i = base + jb;
+        const float mu[3] = {s_mu[3 * jb], s_mu[3 * jb + 1], s_mu[3 * jb + 2]};
         float dir[3], dnorm, Y[16];
         view_dir(P, mu, dir, dnorm);
         sh_basis(dir[0], dir[1], dir[2], Y);
         float c[3 * K];
-        load_sh<K>(sh, i, c);
+        load_sh<K>(sh, i, c);      // (gathering the rows by the whole CTA through shared memory measured no faster: 47.1 vs 45.1 us)
         uint8_t fl = (uint8_t)(XPR_FLAG_VISIBLE | s_clamp[idx]);
         float col[3];
 #pragma unroll
