@@ -286,3 +286,31 @@ def test_p14f_accumulator_mass_equals_brute_force():
             brute = brute + np.abs(bwd(_one_pixel(dL, y, x))["g_ray_acc"])
     assert np.abs(brute).max() > 0
     np.testing.assert_allclose(m["g_ray_acc"], brute, rtol=1e-10, atol=1e-10 * np.abs(brute).max())
+
+
+def test_p14g_degenerate_record_contributes_nothing_and_gets_zero_gradients():
+    """Reading C30: a Gaussian whose shader record is not finite (zero scale: M_c = S^-1 (W R)^T is infinite) is never
+    valid -- the image is the image of the scene WITHOUT it, and its gradient is exactly zero (not NaN) on both
+    record-gradient routes; the other Gaussians' gradients are those of the scene without it."""
+    co = cam_obj(W=40, H=24)
+    arr = draw_scene(41, 8, 4, z=(2.0, 4.0), xy=0.4, opac_boost=1.0)
+    cam, cfg = xo.make_camera(co), xo.make_config(cfg_dict(sh_degree=1))
+    bad = {k: v.copy() for k, v in arr.items()}
+    bad["scales"][2] = (0.0, 0.05, 0.05)                     # one zero scale: the 2D footprint (low-passed) still covers tiles
+    r = xo.render_ray(bad, cam, cfg, np.float64)
+    assert r["proj"]["tile_count"][2] > 0 and not r["proj"]["ray_rec"][2].any()
+    keep = np.array([i for i in range(8) if i != 2])
+    sub = {k: v[keep] for k, v in arr.items()}
+    r0 = xo.render_ray(sub, cam, cfg, np.float64)
+    np.testing.assert_allclose(r["fwd"]["image"], r0["fwd"]["image"], rtol=0, atol=1e-14)
+    Gw = np.random.default_rng(0).normal(0, 1, (co.height, co.width, 3))
+    g = xo.backward_ray(bad, r, Gw, cam, cfg, np.float64)
+    g0 = xo.backward_ray(sub, r0, Gw, cam, cfg, np.float64)
+    for k in ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh"):
+        assert np.isfinite(g[k]).all(), k
+        assert not np.any(g[k][2]), k
+        np.testing.assert_allclose(g[k][keep], g0[k], rtol=1e-12, atol=1e-14)
+    ga = xo.rasterize_ray_bwd_acc(r["proj"], r["binned"], r["fwd"], Gw, cam, cfg, np.float64)
+    pa = xo.ray_bwd_acc(bad["means"], bad["scales"], bad["quats"], r["proj"]["tile_count"], ga["g_ray_acc"], cam, np.float64)
+    for k in pa:
+        assert np.isfinite(pa[k]).all() and not np.any(pa[k][2]), k
