@@ -29,7 +29,7 @@ def batch_parity(sc, views, cfg_over=None):
     keys = bp.keys_sorted[:I_total].cpu().numpy().view(np.uint64)
     vals = pu.u32(bp.vals_sorted[:I_total])
     ranges = pu.u32(bp.tile_ranges).reshape(V, T, 2)
-    dLs, og_sum, singles = [], None, []
+    dLs, og_sum, singles, tol_sum = [], None, [], None
     for k, v in enumerate(views):
         g = pu.run_gpu(sc, v, cfg_over)                       # the single-view GPU run
         o = pu.run_oracle(sc, v, cfg_over)
@@ -62,6 +62,9 @@ def batch_parity(sc, views, cfg_over=None):
         dLs.append(dL)
         og = xo.backward(o["arrays"], o, dL, o["cam"], o["cfg"], np.float32)
         og_sum = {p: og[p].copy() for p in PARAMS} if og_sum is None else {p: og_sum[p] + og[p] for p in PARAMS}
+        mass = xo.rasterize_bwd(o["proj"], o["binned"], o["fwd"], dL, o["cam"], o["cfg"], np.float32, mass=True)
+        tp = pu.propagated_param_tol(o["arrays"], o["cam"], o["cfg"], og, mass)     # the view's stage-1 bar at the parameters
+        tol_sum = tp if tol_sum is None else {p: tol_sum[p] + tp[p] for p in PARAMS}
         singles.append((g, dL))
     assert off == I_total
     bp.backward(torch.from_numpy(np.stack(dLs) if V > 1 else dLs[0]).to(bp.device))
@@ -71,10 +74,10 @@ def batch_parity(sc, views, cfg_over=None):
         got = getattr(bp, p).cpu().numpy()
         bad, err = pu.grad_violations(got, og_sum[p])
         total_bad += int(bad.sum()); total += bad.size
-        if bad.any():
-            ref = np.asarray(og_sum[p], np.float64).reshape(N, -1)
-            group = np.abs(ref).max(axis=1, keepdims=True) * np.ones_like(ref)
-            assert (err[bad] <= 1e-2 * group.ravel()[bad] + 1e-6).all(), p
+        # every element within the bar DERIVED from the stage bars (parity_util.propagated_param_tol; the sum over the
+        # views carries one fp32 rounding per added view: 2.4e-7 of the magnitudes)
+        ok = pu.e2e_within_propagated(got, og_sum[p], tol_sum[p] + 2.4e-7 * V * np.abs(og_sum[p]))
+        assert ok.all(), (p, int((~ok).sum()))
     assert total_bad <= max(4, 2e-5 * total), (total_bad, total)
     # and against the sum of the single-view GPU gradients: the same kernels, but the fp32 atomics of the compositing
     # backward land in another order, so agreement is at the bar of the oracle comparison, not bit for bit
