@@ -339,7 +339,7 @@ def test_overlapped_zero_fill_gives_the_same_gradients():
 def test_fused_loss_backward_matches_separate_loss_grad(config, n, wh):
     """xpr_rasterize_bwd_loss (loss gradient formed in the kernel's prologue) against xpr_loss_grad followed by
     xpr_rasterize_bwd: the same per-pixel dL values enter the same arithmetic, so the 2D gradients agree up to the order
-    of the fp32 atomics (the bar of the GPU-vs-GPU comparisons: a handful of elements outside 1e-3 |ref| + 1e-6); both
+    of the fp32 atomics; both
     losses (config 1: sum of squares, config 2: sum of absolute differences)."""
     import torch
     from paper_2606_11529_b200 import binding as xb, pipeline
@@ -360,10 +360,13 @@ def test_fused_loss_backward_matches_separate_loss_grad(config, n, wh):
     assert pipe.can_fuse_loss()
     pipe.rasterize_bwd_loss(target, sc.loss)
     torch.cuda.synchronize()
-    total = bad = 0
-    for k in names:
-        got = getattr(pipe, k).cpu().numpy()
+    # both runs sum the same terms with fp32 atomics in an arbitrary order: each is within the stage-1 bar of the exact sum
+    # (1e-3 |ref| + 1e-6 + 2e-6 mass), so their difference is within 1e-3 |ref| + 2e-6 + 4e-6 mass -- every
+    # element, with the oracle's mass for the very dL the GPU used
+    o = pu.run_oracle(sc, 0)
+    mass = xo.rasterize_bwd(o["proj"], o["binned"], o["fwd"], dL.cpu().numpy(), o["cam"], o["cfg"], np.float32, mass=True)
+    for k, ko in zip(names, ("g_mean2d", "g_conic", "g_opac_eff", "g_rgb")):
+        got = getattr(pipe, k).cpu().numpy().astype(np.float64)
         assert np.isfinite(got).all() and np.abs(ref[k]).max() > 0
-        b, _ = pu.grad_violations(got, ref[k])
-        bad += int(b.sum()); total += b.size
-    assert bad <= max(4, 2e-5 * total), (bad, total)
+        tol = 1e-3 * np.abs(ref[k]) + 2e-6 + 4e-6 * mass[ko].reshape(got.shape)
+        assert (np.abs(got - ref[k]) <= tol).all(), (k, int((np.abs(got - ref[k]) > tol).sum()))
