@@ -66,6 +66,10 @@ def parse():
     ap.add_argument("--ray-eval", type=int, default=0, choices=(0, 1),
                     help="1: XPR-3DGUT evaluation along the pixel ray (SURVEY 8(f) f2; meant for --config 4) instead of "
                          "the 2D conic of north_star")
+    ap.add_argument("--linprim", type=float, default=0.0,
+                    help="M > 0: time XPR-LinPrim instead (SURVEY 8(f) f4, DESIGN.md 11): one forward + backward step on the "
+                         "config's scene read as octahedra with half-axes = M x the Gaussian scales (DESIGN.md uses 3); "
+                         "one GPU, pinhole configs (1, 2, 3, 5)")
     ap.add_argument("--sort-compare", action="store_true",
                     help="after the timed steps, also time cub::DeviceRadixSort::SortPairs (libxpr_cubcmp.so, built on demand; "
                          "never on the path) on the same (key, value) pairs in emission order, beside xpr_bin_sort "
@@ -219,6 +223,111 @@ RAY_BWD_OPS_VISIT, RAY_BWD_OPS_PASS = 26, 57
 # f3 (depth + accumulated opacity): 2 more lane-ops per blended pair forward, 4 more backward
 FEAT_FWD_EXTRA, FEAT_BWD_EXTRA = 2, 4
 SMS, LANES_PER_SM = 148, 128
+
+
+LIN_FWD_OPS_VISIT, LIN_FWD_OPS_PASS = 34, 9   # chord: dx, dy, 4 x (mul, fma, neg), 8 add/sub, 6 min/max, compare, mul; blend: as the Gaussians
+
+
+def run_linprim(args):
+    """f4: the LinPrim step (xpr_lin_project -> xpr_bin_sort_lin -> xpr_lin_rasterize_fwd -> loss gradient ->
+    xpr_lin_rasterize_bwd -> xpr_lin_project_bwd), same protocol as the Gaussian step: W warm-up steps, K timed steps
+    with the L2 flushed in between, CUDA events per stage, clocks sampled during the timed region."""
+    import numpy as np
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline, scenes
+    world, _, local = rank_env()
+    if world > 1:
+        raise SystemExit("bench.py --linprim: one GPU")
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    xb.lib()
+    sc = scenes.make_scene(args.config)
+    cam = sc.cameras[args.view]
+    if int(cam.model) != 0:
+        raise SystemExit("bench.py --linprim: pinhole configs only")
+    cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull)
+    scales = np.ascontiguousarray(sc.scales * np.float32(args.linprim), np.float32)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    params = (t(sc.means), t(scales), t(sc.quats), t(sc.opacities), t(sc.sh))
+    target = t(sc.target(args.view))
+    dL = torch.empty_like(target)
+    pipe = pipeline.LinPrimPipeline(sc.N, cam, cfg, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    names = ("project", "bin_sort", "rasterize_fwd", "loss_grad", "rasterize_bwd", "project_bwd")
+
+    def rec():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
+
+    def step(events, sync):
+        ev = events.append
+        ev(rec()); pipe.project(*params)
+        ev(rec()); pipe.bin_sort() if sync else pipe.bin_sort_async()
+        ev(rec()); pipe.rasterize_fwd()
+        ev(rec()); xb.xpr_loss_grad(sc.loss, pipe.image, target, dL)
+        ev(rec()); pipe.rasterize_bwd(dL)
+        ev(rec()); pipe.project_bwd()
+        ev(rec())
+
+    for _ in range(max(args.warmup, 3)):
+        step([], True)
+    torch.cuda.synchronize()
+    n_pairs = pipe.num_pairs
+    sampler = ClockSampler(local)
+    sampler.start()
+    runs = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        evs = []
+        step(evs, False)
+        torch.cuda.synchronize()
+        runs.append(evs)
+    clocks = sampler.stop()
+    per_step = np.array([e[0].elapsed_time(e[-1]) for e in runs])
+    stage_ms = {n: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in runs])) for i, n in enumerate(names)}
+    ms = float(per_step.mean())
+    stats = torch.zeros(4, dtype=torch.int64, device=dev)
+    xb.xpr_lin_rasterize_stats(pipe.cam, pipe.cfg, pipe.lin_rec, pipe.vals_sorted, pipe.tile_ranges, stats)
+    visit, passed, blended, sum_n = [int(v) for v in stats.tolist()]
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    alu_peak = SMS * LANES_PER_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    ach = (LIN_FWD_OPS_VISIT * visit + LIN_FWD_OPS_PASS * passed) / (stage_ms["rasterize_fwd"] / 1e3) / 1e12
+    roofline = {"kernel": "lin_rasterize_fwd_kernel", "bound": "alu", "unit": "T lane-op/s", "peak": alu_peak, "achieved": ach,
+                "frac": ach / alu_peak, "traffic": None,
+                "algorithmic": "%d x visited + %d x passed lane-ops per (pixel, primitive)" % (LIN_FWD_OPS_VISIT, LIN_FWD_OPS_PASS)}
+    mp = cam.width * cam.height / 1e6
+    cpu = None
+    if not args.no_cpu_baseline:
+        sys.path.insert(0, os.path.join(ROOT, "oracle"))
+        import xpr_oracle as xo
+        arr = dict(means=sc.means, scales=scales, quats=sc.quats, opacities=sc.opacities, sh=sc.sh)
+        ocam, ocfg = xo.make_camera(cam), xo.make_config(cfg)
+        t0 = time.perf_counter()
+        r = xo.render_lin(arr, ocam, ocfg, np.float32)
+        _, g = scenes.loss_and_grad(sc.loss, r["fwd"]["image"], sc.target(args.view))
+        xo.backward_lin(arr, r, g.astype(np.float32), ocam, ocfg, np.float32)
+        dt = time.perf_counter() - t0
+        cpu = {"value": mp / dt, "unit": "MP/s", "cores": os.cpu_count(), "kind": "oracle", "seconds": dt,
+               "sample": "full workload, %d primitives, %dx%d, 1 step" % (sc.N, cam.width, cam.height)}
+    print(json.dumps({
+        "metric": "fwd_bwd_megapixels_per_s", "value": mp / (ms / 1e3), "unit": "MP/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config] + " read as octahedra (XPR-LinPrim)", "method": "linprim",
+                   "half_axes": "%g x the Gaussian scales" % args.linprim, "view": args.view, "tile_cull": args.tile_cull,
+                   "primitives": sc.N, "image": [cam.width, cam.height], "pairs": n_pairs,
+                   "l2": "flushed between timed steps (256 MiB write)", "parallelism": "1 GPU"},
+        "ms_per_step_stats": {"mean": ms, "median": float(np.median(per_step)), "min": float(per_step.min())},
+        "stage_ms": stage_ms, "counts": {"visited": visit, "passed": passed, "blended": blended, "sum_n_contrib": sum_n},
+        "roofline": roofline, "clocks": clocks, "e2e": None, "gpu_launches": args.steps * (1 + 11 + 1 + 1 + 1 + 1),
+        "cpu_baseline": cpu}))
 
 
 def run_ours(args):
@@ -659,5 +768,7 @@ if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.linprim > 0:
+        run_linprim(a)
     else:
         run_ours(a)

@@ -392,8 +392,20 @@ class LinPrimPipeline:
         self.rasterize_fwd()
         return self.image
 
-    def backward(self, dL_dimage):
+    def bin_sort_async(self):
+        """xpr_bin_sort_lin without the host read-back (buffers sized by an earlier bin_sort())."""
+        xb.xpr_bin_sort(self.depth, self.tile_rect, self.tile_count, self.cam, self.cfg, self.pair_capacity,
+                        self.keys_sorted, self.vals_sorted, self.tile_ranges, self.workspace, sync=False,
+                        lin_rec=self.lin_rec)
+
+    def rasterize_bwd(self, dL_dimage):
         xb.xpr_lin_rasterize_bwd(self.cam, self.cfg, self.lin_rec, self.vals_sorted, self.tile_ranges, self.final_T,
                                  self.n_contrib, dL_dimage, self.g_lin_rec)
+
+    def project_bwd(self):
         xb.xpr_lin_project_bwd(*self._inputs, self.cam, self.cfg, self.tile_count, self.lin_rec, self.g_lin_rec,
                                self.g_means, self.g_scales, self.g_quats, self.g_opacities, self.g_sh)
+
+    def backward(self, dL_dimage):
+        self.rasterize_bwd(dL_dimage)
+        self.project_bwd()

@@ -72,3 +72,12 @@ def test_bench_line_batch_of_views():
 def test_bench_line_separate_loss_kernel():
     d = _run("--fuse-loss", "0", "--no-cpu-baseline", "--no-e2e", "--no-graph", "--no-plain")
     assert d["config"]["fuse_loss"] == 0 and d["gpu_launches"] == 3 * 16 and d["stage_ms"]["loss_grad"] > 0.005
+
+
+def test_bench_line_linprim():
+    d = _run("--linprim", "3", "--config", "2")
+    assert d["config"]["method"] == "linprim" and d["value"] > 0 and d["config"]["pairs"] > 1000
+    assert set(d["stage_ms"]) == {"project", "bin_sort", "rasterize_fwd", "loss_grad", "rasterize_bwd", "project_bwd"}
+    assert d["roofline"]["kernel"] == "lin_rasterize_fwd_kernel" and 0 < d["roofline"]["frac"] < 1
+    assert d["counts"]["visited"] >= d["counts"]["passed"] >= d["counts"]["blended"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
