@@ -335,6 +335,40 @@ def test_overlapped_zero_fill_gives_the_same_gradients():
 
 
 @pytest.mark.gpu
+def test_fused_loss_backward_on_a_batch_of_views():
+    """xpr_rasterize_bwd_loss with xpr_config.views = 2: image and target are [V,H,W,3]; same comparison as the single-view
+    test below (the mass of a batch is per (view, Gaussian): the oracle's, view by view)."""
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline
+    sc = scenes.make_scene(3, n_override=20000, image_override=(250, 130))
+    cfg = scenes.default_render_config(sc)
+    params = pipeline.scene_to_device(sc)
+    views = [0, 1]
+    target = torch.from_numpy(np.stack([sc.target(v) for v in views])).cuda()
+    pipe = pipeline.SplatPipeline(sc.N, [sc.cameras[v] for v in views], cfg)
+    pipe.forward(*params)
+    dL = torch.empty_like(pipe.image)
+    xb.xpr_loss_grad(sc.loss, pipe.image, target, dL)
+    pipe.rasterize_bwd(dL)
+    torch.cuda.synchronize()
+    names = ("g_mean2d", "g_conic", "g_opac", "g_rgb")
+    ref = {k: getattr(pipe, k).cpu().numpy().astype(np.float64) for k in names}
+    for k in names:
+        getattr(pipe, k).fill_(float("nan"))
+    pipe.rasterize_bwd_loss(target, sc.loss)
+    torch.cuda.synchronize()
+    N = sc.N
+    for vi, v in enumerate(views):
+        o = pu.run_oracle(sc, v)
+        mass = xo.rasterize_bwd(o["proj"], o["binned"], o["fwd"], dL[vi].cpu().numpy(), o["cam"], o["cfg"], np.float32, mass=True)
+        for k, ko in zip(names, ("g_mean2d", "g_conic", "g_opac_eff", "g_rgb")):
+            got = getattr(pipe, k).cpu().numpy().astype(np.float64)[vi * N:(vi + 1) * N]
+            r = ref[k][vi * N:(vi + 1) * N]
+            assert np.isfinite(got).all() and np.abs(r).max() > 0
+            tol = 1e-3 * np.abs(r) + 2e-6 + 4e-6 * mass[ko].reshape(got.shape)
+            assert (np.abs(got - r) <= tol).all(), (v, k, int((np.abs(got - r) > tol).sum()))
+
+
 @pytest.mark.parametrize("config,n,wh", [(1, None, None), (2, 20000, (320, 240))])
 def test_fused_loss_backward_matches_separate_loss_grad(config, n, wh):
     """xpr_rasterize_bwd_loss (loss gradient formed in the kernel's prologue) against xpr_loss_grad followed by
