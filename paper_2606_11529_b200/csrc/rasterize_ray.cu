@@ -9,6 +9,7 @@
 #include <math.h>
 
 #include "common.cuh"
+#include "packed.cuh"
 
 namespace xpr {
 namespace {
@@ -21,17 +22,6 @@ struct RayRasterParams {
     float bg[3];
     const uint32_t* order;     // xpr_config.tile_order: CTA b works on tile order[b] (longest lists first), or NULL
 };
-
-__device__ __forceinline__ float ex2_approx(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-__device__ __forceinline__ float rcp_approx(float x) {
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 
 // evaluate (Listing 3) in the fixed fp32 order of DESIGN.md 3 (rule R3)
 struct RayEval { float dc0, dc1, dc2, c0, c1, c2, nhq, dd; };
@@ -49,6 +39,29 @@ __device__ __forceinline__ RayEval eval_ray(const float4 r0, const float4 r1, co
     e.dd = __fmaf_rn(e.dc2, e.dc2, __fmaf_rn(e.dc1, e.dc1, __fmul_rn(e.dc0, e.dc0)));
     e.nhq = __fmul_rn(-0.5f, q);
     return e;
+}
+
+// The same evaluation for a PAIR of pixels with the packed fp32 instructions of sm_100 (packed.cuh): the record operands are
+// broadcast, the two rays sit in the two lanes; every lane is rounded exactly as the scalar code above (rule R3 holds).
+struct RayEval2 { f32x2 dc0, dc1, dc2, c0, c1, c2, nhq, dd; };
+__device__ __forceinline__ RayEval2 eval_ray2(const float4 r0, const float4 r1, const float4 r2, f32x2 d0, f32x2 d1, f32x2 d2) {
+    RayEval2 e;
+    e.dc0 = fma2(bcast2(r0.z), d2, fma2(bcast2(r0.y), d1, mul2(bcast2(r0.x), d0)));
+    e.dc1 = fma2(bcast2(r1.y), d2, fma2(bcast2(r1.x), d1, mul2(bcast2(r0.w), d0)));
+    e.dc2 = fma2(bcast2(r2.x), d2, fma2(bcast2(r1.w), d1, mul2(bcast2(r1.z), d0)));
+    const f32x2 o0 = bcast2(r2.y), o1 = bcast2(r2.z), o2 = bcast2(r2.w);
+    e.c0 = fma2(o1, e.dc2, neg2(mul2(o2, e.dc1)));
+    e.c1 = fma2(o2, e.dc0, neg2(mul2(o0, e.dc2)));
+    e.c2 = fma2(o0, e.dc1, neg2(mul2(o1, e.dc0)));
+    const f32x2 q = fma2(e.c2, e.c2, fma2(e.c1, e.c1, mul2(e.c0, e.c0)));
+    e.dd = fma2(e.dc2, e.dc2, fma2(e.dc1, e.dc1, mul2(e.dc0, e.dc0)));
+    e.nhq = mul2(bcast2(-0.5f), q);
+    return e;
+}
+__device__ __forceinline__ void unpack_eval(const RayEval2& p, RayEval& a, RayEval& b) {
+    unpack2(p.dc0, a.dc0, b.dc0); unpack2(p.dc1, a.dc1, b.dc1); unpack2(p.dc2, a.dc2, b.dc2);
+    unpack2(p.c0, a.c0, b.c0); unpack2(p.c1, a.c1, b.c1); unpack2(p.c2, a.c2, b.c2);
+    unpack2(p.nhq, a.nhq, b.nhq); unpack2(p.dd, a.dd, b.dd);
 }
 
 // Forward (a8 with the f2 evaluation).  One CTA per tile in the two shapes of rasterize.cu: PPT = 2 (128 threads, a
@@ -125,6 +138,8 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
     const uint32_t len = rg.y - rg.x;
     const float amax = P.amax, tmin = P.tmin, lnr = P.lnr;
     uint32_t n_visit = 0, n_pass = 0, n_blend = 0;
+    // the pixel pair's ray components, lane 0 = pixel 0, lane 1 = pixel 1 (PPT == 2)
+    const f32x2 D0 = pack2(pix[0].d0, pix[PPT - 1].d0), D1 = pack2(pix[0].d1, pix[PPT - 1].d1), D2 = pack2(pix[0].d2, pix[PPT - 1].d2);
 
     for (uint32_t base = 0; base < len; base += BATCH) {
         if (__syncthreads_or(any_act) == 0) break;
@@ -147,10 +162,12 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const float4 r0 = rq[5 * u], r1 = rq[5 * u + 1], r2 = rq[5 * u + 2];
-#pragma unroll
-                    for (int k = 0; k < PPT; ++k) {
-                        const RayEval e = eval_ray(r0, r1, r2, pix[k].d0, pix[k].d1, pix[k].d2);
-                        nhq[u][k] = e.nhq; dd[u][k] = e.dd;
+                    if (PPT == 2) {
+                        const RayEval2 e = eval_ray2(r0, r1, r2, D0, D1, D2);
+                        unpack2(e.nhq, nhq[u][0], nhq[u][PPT - 1]); unpack2(e.dd, dd[u][0], dd[u][PPT - 1]);
+                    } else {
+                        const RayEval e = eval_ray(r0, r1, r2, pix[0].d0, pix[0].d1, pix[0].d2);
+                        nhq[u][0] = e.nhq; dd[u][0] = e.dd;
                     }
                 }
 #pragma unroll
@@ -163,10 +180,15 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             }
             for (; j < cnt && any_act; ++j, rq += 5) {
                 const float4 r0 = rq[0], r1 = rq[1], r2 = rq[2];
-#pragma unroll
-                for (int k = 0; k < PPT; ++k) {
-                    const RayEval e = eval_ray(r0, r1, r2, pix[k].d0, pix[k].d1, pix[k].d2);
-                    ray_blend<STATS, FEAT>(pix[k], act[k], e.nhq, e.dd, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
+                if (PPT == 2) {
+                    const RayEval2 e2 = eval_ray2(r0, r1, r2, D0, D1, D2);
+                    float na, nb, da, db;
+                    unpack2(e2.nhq, na, nb); unpack2(e2.dd, da, db);
+                    ray_blend<STATS, FEAT>(pix[0], act[0], na, da, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
+                    ray_blend<STATS, FEAT>(pix[PPT - 1], act[PPT - 1], nb, db, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
+                } else {
+                    const RayEval e = eval_ray(r0, r1, r2, pix[0].d0, pix[0].d1, pix[0].d2);
+                    ray_blend<STATS, FEAT>(pix[0], act[0], e.nhq, e.dd, rq, base + j + 1, lnr, amax, tmin, n_visit, n_pass, n_blend);
                 }
                 any_act = (act[0] | act[PPT - 1]) != 0;
             }
@@ -191,27 +213,6 @@ rasterize_ray_fwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             n_contrib[pid] = pix[k].last;
             if (FEAT) { depth_img[pid] = pix[k].D; alpha_img[pid] = pix[k].A; }
         }
-}
-
-// Transposed butterfly (see rasterize.cu): 8 per-lane values -> lane L with (L & 3) == 0 holds the total of value L >> 2.
-__device__ __forceinline__ float warp_reduce8(const float* v, int lane) {
-    float w[4], x[2];
-    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float send = b4 ? v[i] : v[i + 4], keep = b4 ? v[i + 4] : v[i];
-        w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-    }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const float send = b3 ? w[i] : w[i + 2], keep = b3 ? w[i + 2] : w[i];
-        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-    }
-    const float send = b2 ? x[0] : x[1], keep = b2 ? x[1] : x[0];
-    float y = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-    y += __shfl_xor_sync(0xffffffffu, y, 2);
-    y += __shfl_xor_sync(0xffffffffu, y, 1);
-    return y;
 }
 
 // Backward (a9 with the f2 evaluation).  A thread owns PPT consecutive pixels of a row and sums their 19 gradient
@@ -301,6 +302,19 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
     uint32_t max_n = 0;
 #pragma unroll
     for (int w = 0; w < THREADS / 32; ++w) max_n = max(max_n, s_max[w]);
+    // the thread's pixels as PAIRS of neighbours (lane 0 = pixel 2p, lane 1 = pixel 2p + 1) for the packed fp32
+    // instructions of sm_100 (packed.cuh): the evaluation, the blend weights and the accumulator terms run two pixels per
+    // issue slot; the two lanes of an accumulator are added once per entry, before the warp reduction
+    constexpr int NP = PPT / 2;
+    f32x2 T2[NP], Q2[NP], g0_2[NP], g1_2[NP], g2_2[NP], gD_2[NP], d0_2[NP], d1_2[NP], d2_2[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        T2[p] = pack2(T[2 * p], T[2 * p + 1]); Q2[p] = pack2(Q[2 * p], Q[2 * p + 1]);
+        g0_2[p] = pack2(g0[2 * p], g0[2 * p + 1]); g1_2[p] = pack2(g1[2 * p], g1[2 * p + 1]); g2_2[p] = pack2(g2[2 * p], g2[2 * p + 1]);
+        gD_2[p] = pack2(gD[2 * p], gD[2 * p + 1]);
+        d0_2[p] = pack2(d0[2 * p], d0[2 * p + 1]); d1_2[p] = pack2(d1[2 * p], d1[2 * p + 1]); d2_2[p] = pack2(d2[2 * p], d2[2 * p + 1]);
+    }
+    const float amax = P.amax;
 
     // lane 4 i owns value i of butterfly A (g_acc[0..8): S_c, D_xx, D_xy) and value i of butterfly B (g_acc[8..15):
     // D_xz .. D_zz, sum dL/do_c; value 7: dL/do); lane 8 i owns colour channel i of the 4-value butterfly
@@ -326,53 +340,70 @@ rasterize_ray_bwd_kernel(RayRasterParams P, const float4* __restrict__ ray_rec, 
             if (pos >= wmax) continue;     // warp-uniform
             const float4 r0 = s_geo[3 * j], r1 = s_geo[3 * j + 1], r2 = s_geo[3 * j + 2];
             const float4 ga = s_gate[j];
-            RayEval e[PPT];
+            RayEval2 e2[NP];
+            float nhq[PPT], dd[PPT];
             bool contrib[PPT], any_c = false;
 #pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                e2[p] = eval_ray2(r0, r1, r2, d0_2[p], d1_2[p], d2_2[p]);
+                unpack2(e2[p].nhq, nhq[2 * p], nhq[2 * p + 1]); unpack2(e2[p].dd, dd[2 * p], dd[2 * p + 1]);
+            }
+#pragma unroll
             for (int k = 0; k < PPT; ++k) {
-                e[k] = eval_ray(r0, r1, r2, d0[k], d1[k], d2[k]);
-                const float tv = __fmul_rn(lnr, e[k].dd), tg = __fmul_rn(ga.x, e[k].dd);
-                contrib[k] = (pos < n[k]) && (e[k].nhq > tv) && !(e[k].nhq < tg);
+                const float tv = __fmul_rn(lnr, dd[k]), tg = __fmul_rn(ga.x, dd[k]);
+                contrib[k] = (pos < n[k]) && (nhq[k] > tv) && !(nhq[k] < tg);
                 any_c |= contrib[k];
             }
             if (!__any_sync(0xffffffffu, any_c)) continue;
             const float4 c = s_col[j];
+            f32x2 va2[8], vb2[8], vc2[4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) va2[i] = vb2[i] = 0ull;
+            vc2[0] = vc2[1] = vc2[2] = vc2[3] = 0ull;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                const int k = 2 * p;
+                // a pixel that does not contribute enters with 1/dd = 0 and o G = 0: every term vanishes
+                const f32x2 rdd2 = pack2(contrib[k] ? rcp_approx(dd[k]) : 0.0f, contrib[k + 1] ? rcp_approx(dd[k + 1]) : 0.0f);
+                const f32x2 power2 = mul2(e2[p].nhq, rdd2);
+                float ea, eb;
+                unpack2(fma2(power2, bcast2(LOG2E), bcast2(ga.z)), ea, eb);
+                const float og_a = contrib[k] ? ex2_approx(ea) : 0.0f, og_b = contrib[k + 1] ? ex2_approx(eb) : 0.0f;   // o G
+                const f32x2 al2 = pack2(fminf(amax, og_a), fminf(amax, og_b));
+                float oma_a, oma_b;
+                unpack2(sub2(bcast2(1.0f), al2), oma_a, oma_b);
+                const f32x2 inv2 = pack2(rcp_approx(oma_a), rcp_approx(oma_b));
+                T2[p] = mul2(T2[p], inv2);             // transmittance in front of this entry
+                const f32x2 w2 = mul2(al2, T2[p]);
+                vc2[0] = fma2(w2, g0_2[p], vc2[0]); vc2[1] = fma2(w2, g1_2[p], vc2[1]); vc2[2] = fma2(w2, g2_2[p], vc2[2]);
+                f32x2 gc2 = fma2(g2_2[p], bcast2(c.z), fma2(g1_2[p], bcast2(c.y), mul2(g0_2[p], bcast2(c.x))));
+                if (FEAT) { vc2[3] = fma2(w2, gD_2[p], vc2[3]); gc2 = fma2(gD_2[p], bcast2(c.w), gc2); }   // dL/dz; g . c + gD z
+                float da_a, da_b;
+                unpack2(fma2(T2[p], gc2, neg2(mul2(inv2, Q2[p]))), da_a, da_b);
+                Q2[p] = fma2(gc2, w2, Q2[p]);
+                // C14: no gradient where the clamp is active; dL/dpower = o G dL/dalpha (dL/do = that / o, divided once per warp)
+                const f32x2 gp2 = mul2(pack2(og_a, og_b), pack2((og_a < amax) ? da_a : 0.0f, (og_b < amax) ? da_b : 0.0f));
+                vb2[7] = add2(vb2[7], gp2);
+                const f32x2 k1 = mul2(neg2(gp2), rdd2);                  // dL/dc = k1 c
+                const f32x2 gc0 = mul2(k1, e2[p].c0), gc1 = mul2(k1, e2[p].c1), gcz = mul2(k1, e2[p].c2);
+                // S_c += k1 c c^T
+                va2[0] = fma2(gc0, e2[p].c0, va2[0]); va2[1] = fma2(gc0, e2[p].c1, va2[1]); va2[2] = fma2(gc0, e2[p].c2, va2[2]);
+                va2[3] = fma2(gc1, e2[p].c1, va2[3]); va2[4] = fma2(gc1, e2[p].c2, va2[4]); va2[5] = fma2(gcz, e2[p].c2, va2[5]);
+                // D += 2 dL/ddd d d^T,  2 dL/ddd = 2 k1 power
+                const f32x2 gdd2 = mul2(mul2(bcast2(2.0f), k1), power2);
+                const f32x2 t0 = mul2(gdd2, d0_2[p]), t1 = mul2(gdd2, d1_2[p]), t2 = mul2(gdd2, d2_2[p]);
+                va2[6] = fma2(t0, d0_2[p], va2[6]); va2[7] = fma2(t0, d1_2[p], va2[7]); vb2[0] = fma2(t0, d2_2[p], vb2[0]);
+                vb2[1] = fma2(t1, d1_2[p], vb2[1]); vb2[2] = fma2(t1, d2_2[p], vb2[2]); vb2[3] = fma2(t2, d2_2[p], vb2[3]);
+                // dL/do_c = d_c x dL/dc
+                vb2[4] = add2(vb2[4], fma2(e2[p].dc1, gcz, neg2(mul2(e2[p].dc2, gc1))));
+                vb2[5] = add2(vb2[5], fma2(e2[p].dc2, gc0, neg2(mul2(e2[p].dc0, gcz))));
+                vb2[6] = add2(vb2[6], fma2(e2[p].dc0, gc1, neg2(mul2(e2[p].dc1, gc0))));
+            }
             float va[8], vb[8], vc[4];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) va[i] = vb[i] = 0.f;
-            vc[0] = vc[1] = vc[2] = vc[3] = 0.f;
+            for (int i = 0; i < 8; ++i) { va[i] = sum2(va2[i]); vb[i] = sum2(vb2[i]); }
 #pragma unroll
-            for (int k = 0; k < PPT; ++k) {
-                // a pixel that does not contribute enters with 1/dd = 0 and o G = 0: every term vanishes
-                const float rdd = contrib[k] ? rcp_approx(e[k].dd) : 0.0f;
-                const float power = e[k].nhq * rdd;
-                const float og = contrib[k] ? ex2_approx(fmaf(power, 1.4426950408889634f, ga.z)) : 0.0f;   // o G
-                const float alpha = fminf(P.amax, og);
-                const float inv = rcp_approx(1.0f - alpha);
-                T[k] = T[k] * inv;                     // transmittance in front of this entry
-                const float w = alpha * T[k];
-                vc[0] = fmaf(w, g0[k], vc[0]); vc[1] = fmaf(w, g1[k], vc[1]); vc[2] = fmaf(w, g2[k], vc[2]);
-                float gc = fmaf(g2[k], c.z, fmaf(g1[k], c.y, g0[k] * c.x));
-                if (FEAT) { vc[3] = fmaf(w, gD[k], vc[3]); gc = fmaf(gD[k], c.w, gc); }       // dL/dz; g . c + gD z
-                const float dalpha = fmaf(T[k], gc, -(inv * Q[k]));
-                Q[k] = fmaf(gc, w, Q[k]);
-                const float live = (og < P.amax) ? dalpha : 0.0f;   // C14
-                const float gp = og * live;            // dL/dpower; dL/do = gp / o, divided once per warp below
-                vb[7] += gp;
-                const float k1 = -gp * rdd;            // dL/dc = k1 c
-                const float gc0 = k1 * e[k].c0, gc1 = k1 * e[k].c1, gc2 = k1 * e[k].c2;
-                // S_c += k1 c c^T
-                va[0] = fmaf(gc0, e[k].c0, va[0]); va[1] = fmaf(gc0, e[k].c1, va[1]); va[2] = fmaf(gc0, e[k].c2, va[2]);
-                va[3] = fmaf(gc1, e[k].c1, va[3]); va[4] = fmaf(gc1, e[k].c2, va[4]); va[5] = fmaf(gc2, e[k].c2, va[5]);
-                // D += 2 dL/ddd d d^T,  2 dL/ddd = 2 k1 power
-                const float gdd2 = 2.0f * k1 * power;
-                const float t0 = gdd2 * d0[k], t1 = gdd2 * d1[k], t2 = gdd2 * d2[k];
-                va[6] = fmaf(t0, d0[k], va[6]); va[7] = fmaf(t0, d1[k], va[7]); vb[0] = fmaf(t0, d2[k], vb[0]);
-                vb[1] = fmaf(t1, d1[k], vb[1]); vb[2] = fmaf(t1, d2[k], vb[2]); vb[3] = fmaf(t2, d2[k], vb[3]);
-                vb[4] += fmaf(e[k].dc1, gc2, -(e[k].dc2 * gc1));     // dL/do_c = d_c x dL/dc
-                vb[5] += fmaf(e[k].dc2, gc0, -(e[k].dc0 * gc2));
-                vb[6] += fmaf(e[k].dc0, gc1, -(e[k].dc1 * gc0));
-            }
+            for (int i = 0; i < 4; ++i) vc[i] = sum2(vc2[i]);
             const float ta = warp_reduce8(va, lane);
             float tb = warp_reduce8(vb, lane);
             const float tc = warp_reduce4(vc, lane);
