@@ -348,8 +348,8 @@ def run_ours(args):
     sc = scenes.make_scene(args.config)
     cam = sc.cameras[args.view]
     V = max(1, args.views)
-    if V > 1 and (args.features or args.ray_eval or args.view + V > len(sc.cameras)):
-        raise SystemExit("bench.py: --views V needs V cameras in the scene (config 5 has four) and the 2D colour pass")
+    if V > 1 and (args.ray_eval or args.view + V > len(sc.cameras)):
+        raise SystemExit("bench.py: --views V needs V cameras in the scene (config 5 has four) and the 2D evaluation")
     cfg = dict(scenes.default_render_config(sc), tile_cull=args.tile_cull, ray_eval=args.ray_eval,
                tile_order=args.tile_order, features=args.features)
     if args.overlap_fill >= 0:
@@ -368,7 +368,8 @@ def run_ours(args):
     dL_buf = torch.empty_like(target)
     if args.features:    # loss + sum gD D + sum gA A with seeded constant gD, gA ~ U[-1, 1] (linear in the features)
         gen = torch.Generator(device="cpu").manual_seed(4000 + args.config)
-        pipe.feature_grads = tuple((torch.rand(cam.height, cam.width, generator=gen) * 2 - 1).to(dev) for _ in range(2))
+        vs = (V,) if V > 1 else ()
+        pipe.feature_grads = tuple((torch.rand(*vs, cam.height, cam.width, generator=gen) * 2 - 1).to(dev) for _ in range(2))
     feat_grads = pipe.feature_grads or (None, None)
 
     def loss_grad(image):

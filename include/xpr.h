@@ -70,7 +70,9 @@ typedef struct {
                                the tile id of a pair is v*T + t and one xpr_bin_sort[_cull] call (its N = V*N) sorts all views
                                (keys = (v*T + t) << 32 | depth bits; tile_ranges [V*T, 2]); images are [V, H, W, .], the
                                compositing calls launch V*T tiles; xpr_project_bwd SUMS the parameter gradients over the views.
-                               xpr_pixel_info, xpr_project_ray, xpr_ray_bwd, xpr_depth_bwd and the featn calls take one view */
+                               xpr_rasterize_feat_fwd / _bwd take the batch too (depth_img, alpha_img, dL_ddepth, dL_dalpha are
+                               [V, H, W]; g_depth [V*N]).  xpr_pixel_info, xpr_project_ray, xpr_ray_bwd, the featn calls and
+                               xpr_depth_bwd take one view (call xpr_depth_bwd once per view on that view's slices: it adds) */
 } xpr_config;
 enum { XPR_MAX_VIEWS = 8 };
 

@@ -33,8 +33,8 @@ class SplatPipeline:
         self.ray_eval = bool(cfg.get("ray_eval", 0)) if isinstance(cfg, dict) else False
         # f3: the compositing pass also renders the depth image and the accumulated opacity (2D evaluation only)
         self.features = bool(cfg.get("features", 0)) if isinstance(cfg, dict) else False
-        if self.V > 1 and (self.features or self.ray_eval):
-            raise ValueError("xpr: a batch of views is built for the colour pass of the 2D evaluation")
+        if self.V > 1 and self.ray_eval:
+            raise ValueError("xpr: a batch of views is built for the 2D evaluation (colour, depth and accumulated opacity)")
         self._dL = None
         # overlap_fill = 1: the zero-fill of the parameter gradients (xpr_project_bwd_fill: HBM traffic without inputs) runs on
         # a second stream under the compositing backward.  Off by default: measured on config 3 / 5 the compositing kernel
@@ -83,7 +83,7 @@ class SplatPipeline:
         self.g_mean2d, self.g_conic = g2[:2 * N].view(N, 2), g2[2 * N:5 * N].view(N, 3)
         self.g_opac, self.g_rgb, self.g_depth = g2[5 * N:6 * N], g2[6 * N:9 * N].view(N, 3), g2[9 * N:]
         if self.features:
-            self.depth_img, self.alpha_img = e(self.H, self.W), e(self.H, self.W)
+            self.depth_img, self.alpha_img = e(*vshape, self.H, self.W), e(*vshape, self.H, self.W)
         # the parameter gradients share one allocation, in the order the library checks for (one zero-fill in xpr_project_bwd)
         N = self.N                                     # (summed over the views of a batch)
         K3 = 3 * self.K
@@ -208,7 +208,7 @@ class SplatPipeline:
         self._feat_bwd = False
         self._fork_fill(1)
         if self.features and (dL_ddepth is not None or dL_dalpha is not None):
-            z = lambda t: torch.zeros(self.H, self.W, dtype=torch.float32, device=self.device) if t is None else t
+            z = lambda t: torch.zeros_like(self.final_T) if t is None else t
             if self.ray_eval:
                 xb.xpr_rasterize_ray_feat_bwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv,
                                               self.depth, self.pixel_rays, self.vals_sorted, self.tile_ranges, self.final_T,
@@ -278,7 +278,13 @@ class SplatPipeline:
             xb.xpr_ray_bwd(means, scales, quats, self.cam, self.tile_count, self.g_ray_acc, self.g_means,
                            self.g_scales, self.g_quats)
         if getattr(self, "_feat_bwd", False):
-            xb.xpr_depth_bwd(self.cam, self.tile_count, self.g_depth, self.g_means)
+            if self.V > 1:      # z of view v is (W_v mu + t_v)_z: the call ADDS, so the views accumulate one after the other
+                N = self.N
+                for v in range(self.V):
+                    xb.xpr_depth_bwd(self.cam[v], self.tile_count[v * N:(v + 1) * N], self.g_depth[v * N:(v + 1) * N],
+                                     self.g_means)
+            else:
+                xb.xpr_depth_bwd(self.cam, self.tile_count, self.g_depth, self.g_means)
 
     # ---- whole passes -------------------------------------------------------------------------
     def forward(self, means, scales, quats, opacities, sh):

@@ -150,3 +150,48 @@ def test_batch_of_four_views_config5_full_size_equals_single_views():
         bad, _ = pu.grad_violations(getattr(bp, p).cpu().numpy(), acc[p].cpu().numpy())
         nb += int(bad.sum()); total += bad.size
     assert nb <= 4e-5 * total, (nb, total)
+
+
+def test_batch_of_two_views_with_rendered_features():
+    """f3 x f3: depth image and accumulated opacity for a batch of views (FEAT kernels over V T tiles, xpr_depth_bwd once
+    per view).  Per view the forward equals the single-view GPU run bit for bit; the parameter gradients of the loss
+    sum_v (L_v + sum gD_v D_v + sum gA_v A_v) equal the oracle's sum over the views of backward_da (reading C31, C32)."""
+    import torch
+    from paper_2606_11529_b200 import pipeline
+    sc = scenes.make_scene(3, n_override=20000, image_override=(250, 130))
+    views, N = [0, 1], sc.N
+    cfg = dict(scenes.default_render_config(sc), tile_cull=1, features=1)
+    params = pipeline.scene_to_device(sc)
+    bp = pipeline.SplatPipeline(N, [sc.cameras[v] for v in views], cfg)
+    bp.forward(*params)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(77)
+    dLs, gDs, gAs, og_sum = [], [], [], None
+    for k, v in enumerate(views):
+        g = pu.run_gpu(sc, v, dict(tile_cull=1, features=1))
+        p1 = g["pipe"]
+        assert torch.equal(bp.image[k], p1.image) and torch.equal(bp.final_T[k], p1.final_T)
+        assert torch.equal(bp.depth_img[k], p1.depth_img) and torch.equal(bp.alpha_img[k], p1.alpha_img)
+        assert float(bp.depth_img[k].max()) > 0
+        o = pu.run_oracle(sc, v, dict(tile_cull=1))
+        o["fwd"].update(xo.rasterize_fwd_da(o["proj"], o["binned"], o["cam"], o["cfg"], np.float32))
+        _, dL = scenes.loss_and_grad(sc.loss, o["fwd"]["image"], sc.target(v))
+        H, W = dL.shape[:2]
+        gD, gA = rng.uniform(-1, 1, (H, W)).astype(np.float32), rng.uniform(-1, 1, (H, W)).astype(np.float32)
+        frag = (o["fwd"]["fragile"] & (pu.FRAG_EXIT | pu.FRAG_CLAMP)) != 0
+        dL = np.where(frag[..., None], 0.0, dL).astype(np.float32)
+        gD = np.where(frag, 0.0, gD).astype(np.float32); gA = np.where(frag, 0.0, gA).astype(np.float32)
+        dLs.append(dL); gDs.append(gD); gAs.append(gA)
+        og = xo.backward_da(o["arrays"], o, dL, gD, gA, o["cam"], o["cfg"], np.float32)
+        og_sum = {p: og[p].copy() for p in PARAMS} if og_sum is None else {p: og_sum[p] + og[p] for p in PARAMS}
+    t = lambda a: torch.from_numpy(np.stack(a)).to(bp.device)
+    bp.backward(t(dLs), t(gDs), t(gAs))
+    torch.cuda.synchronize()
+    total = bad = 0
+    for p in PARAMS:
+        got = getattr(bp, p).cpu().numpy()
+        assert np.isfinite(got).all()
+        b, _ = pu.grad_violations(got, og_sum[p])
+        bad += int(b.sum()); total += b.size
+    assert np.abs(og_sum["g_means"]).max() > 0
+    assert bad <= max(4, 2e-5 * total), (bad, total)
