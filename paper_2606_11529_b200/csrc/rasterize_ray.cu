@@ -58,12 +58,6 @@ __device__ __forceinline__ RayEval2 eval_ray2(const float4 r0, const float4 r1, 
     e.nhq = mul2(bcast2(-0.5f), q);
     return e;
 }
-__device__ __forceinline__ void unpack_eval(const RayEval2& p, RayEval& a, RayEval& b) {
-    unpack2(p.dc0, a.dc0, b.dc0); unpack2(p.dc1, a.dc1, b.dc1); unpack2(p.dc2, a.dc2, b.dc2);
-    unpack2(p.c0, a.c0, b.c0); unpack2(p.c1, a.c1, b.c1); unpack2(p.c2, a.c2, b.c2);
-    unpack2(p.nhq, a.nhq, b.nhq); unpack2(p.dd, a.dd, b.dd);
-}
-
 // Forward (a8 with the f2 evaluation).  One CTA per tile in the two shapes of rasterize.cu: PPT = 2 (128 threads, a
 // thread owns the pixels (x, y) and (x + 8, y): the shared-memory reads of a list entry are paid once per two
 // pixels) for large images, PPT = 1 (256 threads) where the heaviest tile bounds the kernel.  Record of a list
