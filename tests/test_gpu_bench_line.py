@@ -28,6 +28,9 @@ def test_bench_line_ours():
     assert "workload" in d["config"] and "model" not in d["config"]
     assert d["gpu_launches"] == 3 * 15          # 11 launches of xpr_bin_sort (one supertile-digit pass); loss gradient fused
     assert d["config"]["fuse_loss"] == 1 and d["stage_ms"]["loss_grad"] < 0.005
+    st = d["ms_per_step_stats"]
+    # the stages are timed in a second, instrumented pass and sum to ITS step time
+    assert abs(sum(d["stage_ms"].values()) - st["instrumented_ms_per_step"]) < 0.02 * st["instrumented_ms_per_step"]
     r = d["roofline"]
     assert r["bound"] in ("hbm", "alu", "tensor") and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
     assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0 and d["e2e"]["value"] > 0
