@@ -166,7 +166,7 @@ def backward_pair(sc, mul, cfg_over):
     return pipe, o, og, mass, arr, ocam, ocfg
 
 
-@pytest.mark.parametrize("case", ["small", "ragged", "sh3"])
+@pytest.mark.parametrize("case", ["small", "ragged", "sh3", "config3_full_size"])
 def test_lin_backward_parity(case):
     """Stage 1: the record gradient against the oracle's, element by element, within 1e-3 |ref| + 1e-6 + 2e-6 mass (the fp32
     summation floor of DESIGN.md section 5).  Stage 2 (stage-isolated, strict 1e-3 |ref| + 1e-6): xpr_lin_project_bwd fed
@@ -176,8 +176,10 @@ def test_lin_backward_parity(case):
         sc, mul = scenes.make_scene(2, n_override=4000, image_override=(160, 160)), 3.0
     elif case == "ragged":
         sc, mul = scenes.make_scene(1, n_override=20000, image_override=(333, 207)), 2.0
-    else:
+    elif case == "sh3":
         sc, mul = scenes.make_scene(3, n_override=30000, image_override=(320, 256)), 5.0
+    else:       # the workload `bench.py --linprim 3 --config 3` times: 1 M octahedra, 1920x1080, Eq. 2's cull on
+        sc, mul = scenes.make_scene(3), 3.0
     pipe, o, og, mass, arr, ocam, ocfg = backward_pair(sc, mul, dict(tile_cull=1))
     g_rec = pipe.g_lin_rec.cpu().numpy()
     assert np.isfinite(g_rec).all()
