@@ -30,6 +30,11 @@ struct RasterParams {
     const uint32_t* order;   // xpr_config.tile_order: CTA b works on tile order[b] (longest lists first), or NULL
 };
 
+// Both gates of a list entry on m = -power: valid (power <= 0, L289) and alpha >= alpha_thresh (power >= -lnv, L679)
+// <=> 0 <= m <= lnv <=> bits(m) <= bits(lnv) as unsigned integers, for lnv > 0 (xpr_project culls a Gaussian with
+// lnv <= 0: its extent is empty).  m < 0 has the sign bit set and compares above every positive float.
+__device__ __forceinline__ bool gate(float m, uint32_t lnv_bits) { return __float_as_uint(m) <= lnv_bits; }
+
 // gather one record (3 x 16 bytes) into a ring slot
 __device__ __forceinline__ void stage_record(float4* slot, const float4* __restrict__ rec, uint32_t g) {
     const float4* src = rec + 3 * (size_t)g;
@@ -100,7 +105,8 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
     }
     uint32_t g_next = ((uint32_t)(2 * B + tid) < len) ? list[2 * B + tid] : 0u;   // index of this thread's entry of batch b + 2
 
-    float pw_a[4], pw_b[4], thr[4], l2o[4], zz[4];
+    float pw_a[4], pw_b[4], l2o[4], zz[4];          // pw: MINUS power (see `power` below)
+    uint32_t lim[4];                                // bits of lnv: the gate's upper limit
     f32x2 pw2[4];
     float4 col[4];                                             // colours of the group's entries (BF)
     uint32_t stage = 0;
@@ -121,27 +127,31 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
             const float4 ge = rq[0];
             const float4 ga = rq[1];
             const float dy = pyc - ge.y;
-            const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);
+            // the kernel carries -power: every operand negated, every rounding symmetric, so the bits are those of
+            // rule R3's power with the sign flipped -- and both gates become ONE unsigned compare (below)
+            const float t1 = __fmul_rn(-ge.w, dy), t2 = __fmul_rn(__fmul_rn(-ga.x, dy), dy);
             if (PPT == 2) {
                 const f32x2 dx2 = sub2(px2, bcast2(ge.x));
-                pw2[u] = fma2(fma2(bcast2(ge.z), dx2, bcast2(t1)), dx2, bcast2(t2));
+                pw2[u] = fma2(fma2(bcast2(-ge.z), dx2, bcast2(t1)), dx2, bcast2(t2));
                 if (!PACKED) unpack2(pw2[u], pw_a[u], pw_b[u]);
             } else {
                 const float dxa = pxc0 - ge.x;
-                pw_a[u] = __fmaf_rn(__fmaf_rn(ge.z, dxa, t1), dxa, t2);
+                pw_a[u] = __fmaf_rn(__fmaf_rn(-ge.z, dxa, t1), dxa, t2);
             }
-            thr[u] = ga.y; l2o[u] = ga.z;
+            lim[u] = __float_as_uint(-ga.y); l2o[u] = ga.z;
             if (FEAT) zz[u] = ga.w;
             if (BF) col[u] = rq[2];
         };
-        // valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12)
+        // valid = power <= 0 (L289, C20); alpha >= alpha_thresh <=> power >= -lnv (L679, C12): with m = -power both
+        // read 0 <= m <= lnv, and for lnv > 0 (every visible Gaussian) that is bits(m) <= bits(lnv) as unsigned integers
+        // (a negative m has the sign bit set and compares above any positive float; m = +0 when power = -0)
         auto blend_packed = [&](int u, uint32_t pos) {
             float pa, pb;
             unpack2(pw2[u], pa, pb);
-            const bool pass_a = act_a && !(pa > 0.0f) && !(pa < thr[u]);
-            const bool pass_b = act_b && !(pb > 0.0f) && !(pb < thr[u]);
+            const bool pass_a = act_a && gate(pa, lim[u]);
+            const bool pass_b = act_b && gate(pb, lim[u]);
             float ea, eb;                                       // o exp(power) = ex2(power log2 e + log2 o)
-            unpack2(fma2(pw2[u], bcast2(LOG2E), bcast2(l2o[u])), ea, eb);
+            unpack2(fma2(pw2[u], bcast2(-LOG2E), bcast2(l2o[u])), ea, eb);
             // a gated or finished pixel gets ex2(-inf) = 0: alpha = 0 without a select after the MUFU
             const float al_a = fminf(amax, ex2_approx(pass_a ? ea : -INFINITY));      // C11
             const float al_b = fminf(amax, ex2_approx(pass_b ? eb : -INFINITY));
@@ -166,8 +176,8 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
         auto blend_scalar = [&](bool& act, float pw, int u, const float4* rq, float& T, float& C0, float& C1, float& C2,
                                 uint32_t& last, uint32_t pos, float& Dv, float& Av) {
             if (BF) {
-                const bool pass = act && !(pw > 0.0f) && !(pw < thr[u]);
-                const float alpha = pass ? fminf(amax, ex2_approx(fmaf(pw, LOG2E, l2o[u]))) : 0.0f;
+                const bool pass = act && gate(pw, lim[u]);
+                const float alpha = pass ? fminf(amax, ex2_approx(fmaf(pw, -LOG2E, l2o[u]))) : 0.0f;
                 const float Tn = T * (1.0f - alpha);
                 const bool stop = Tn < tmin;
                 const bool bl = pass && !stop;
@@ -179,9 +189,9 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
                 last = bl ? pos : last;
             } else if (act) {
                 if (STATS) ++n_visit;
-                if (!(pw > 0.0f) && !(pw < thr[u])) {
+                if (gate(pw, lim[u])) {
                     if (STATS) ++n_pass;
-                    const float alpha = fminf(amax, ex2_approx(fmaf(pw, LOG2E, l2o[u])));
+                    const float alpha = fminf(amax, ex2_approx(fmaf(pw, -LOG2E, l2o[u])));
                     const float Tn = T * (1.0f - alpha);
                     if (Tn < tmin) {
                         act = false;
@@ -272,13 +282,13 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
 #define XPR_BWD_PPT_SMALL 2
 #endif
 #ifndef XPR_BWD_PPT_LARGE
-#define XPR_BWD_PPT_LARGE 4  // pixels per thread in the throughput shape (4: two warps per tile; 8: one)
+#define XPR_BWD_PPT_LARGE 8  // pixels per thread in the throughput shape (8: one warp per tile; 4: two)
 #endif
 #ifndef XPR_BWD_MINB
 #define XPR_BWD_MINB 14      // 64-thread CTAs per SM in the throughput shape (72 registers; 12: +1.5 % time, 10: +3 %)
 #endif
 #ifndef XPR_BWD_MINB8
-#define XPR_BWD_MINB8 20     // 32-thread CTAs per SM at 8 pixels per thread
+#define XPR_BWD_MINB8 16     // 32-thread CTAs per SM at 8 pixels per thread (124 registers; 20 spills, 12: +8 % time)
 #endif
 template <int PPT, bool FEAT>
 __global__ void __launch_bounds__(BLOCK / PPT, PPT == 8 ? XPR_BWD_MINB8 : XPR_BWD_MINB * PPT / 4)
@@ -395,17 +405,18 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
             const float4 ge = rq[0];       // mx my qa qb
             const float4 ga = rq[1];       // qc thr log2o z
             const float dy = pyc - ge.y;
-            const float t1 = __fmul_rn(ge.w, dy), t2 = __fmul_rn(__fmul_rn(ga.x, dy), dy);   // row terms of `power`
-            f32x2 dx2[NP], pw2[NP];
+            const float t1 = __fmul_rn(-ge.w, dy), t2 = __fmul_rn(__fmul_rn(-ga.x, dy), dy);   // row terms of -power
+            const uint32_t lim = __float_as_uint(-ga.y);                                         // bits of lnv
+            f32x2 dx2[NP], pw2[NP];                                                              // pw2 = -power (forward kernel)
             bool contrib[PPT], any_c = false;
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 dx2[p] = sub2(px2[p], bcast2(ge.x));
-                pw2[p] = fma2(fma2(bcast2(ge.z), dx2[p], bcast2(t1)), dx2[p], bcast2(t2));   // rule R3, per lane
+                pw2[p] = fma2(fma2(bcast2(-ge.z), dx2[p], bcast2(t1)), dx2[p], bcast2(t2));  // rule R3, per lane, negated
                 float pa, pb;
                 unpack2(pw2[p], pa, pb);
-                contrib[2 * p] = (pos < n[2 * p]) && !(pa > 0.0f) && !(pa < ga.y);
-                contrib[2 * p + 1] = (pos < n[2 * p + 1]) && !(pb > 0.0f) && !(pb < ga.y);
+                contrib[2 * p] = (pos < n[2 * p]) && gate(pa, lim);
+                contrib[2 * p + 1] = (pos < n[2 * p + 1]) && gate(pb, lim);
                 any_c |= contrib[2 * p] || contrib[2 * p + 1];
             }
             if (!__any_sync(0xffffffffu, any_c)) continue;
@@ -416,7 +427,7 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 float ea, eb;
-                unpack2(fma2(pw2[p], bcast2(LOG2E), bcast2(ga.z)), ea, eb);
+                unpack2(fma2(pw2[p], bcast2(-LOG2E), bcast2(ga.z)), ea, eb);
                 const float og_a = contrib[2 * p] ? ex2_approx(ea) : 0.0f;          // o G
                 const float og_b = contrib[2 * p + 1] ? ex2_approx(eb) : 0.0f;
                 const f32x2 al2 = pack2(fminf(amax, og_a), fminf(amax, og_b));       // C11
