@@ -152,9 +152,10 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
             const bool pass_b = act_b && gate(pb, lim[u]);
             float ea, eb;                                       // o exp(power) = ex2(power log2 e + log2 o)
             unpack2(fma2(pw2[u], bcast2(-LOG2E), bcast2(l2o[u])), ea, eb);
-            // a gated or finished pixel gets ex2(-inf) = 0: alpha = 0 without a select after the MUFU
-            const float al_a = fminf(amax, ex2_approx(pass_a ? ea : -INFINITY));      // C11
-            const float al_b = fminf(amax, ex2_approx(pass_b ? eb : -INFINITY));
+            // a gated or finished pixel gets alpha = 0 (SASS: a predicated MUFU.EX2 over a zeroed register pair; selecting
+            // the exponent, ex2(-inf) = 0, measured 1.2 % slower)
+            const float al_a = fminf(amax, pass_a ? ex2_approx(ea) : 0.0f);           // C11
+            const float al_b = fminf(amax, pass_b ? ex2_approx(eb) : 0.0f);
             const f32x2 al2 = pack2(al_a, al_b);
             float tn_a, tn_b, w_a, w_b, t_a, t_b;
             unpack2(mul2(T2, sub2(bcast2(1.0f), al2)), tn_a, tn_b);             // T' = T (1 - alpha)
@@ -445,11 +446,12 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
                     sz2 = (p == 0) ? mul2(w2, gD_2[p]) : fma2(w2, gD_2[p], sz2);     // dL/dz
                 }
                 // dL/dalpha = T (g . c) - Q / (1 - alpha) = T gc + inv R;   R <- R - gc w
-                float da_a, da_b;
-                unpack2(fma2(inv2, R2[p], mul2(T2[p], gc2)), da_a, da_b);
+                const f32x2 da2 = fma2(inv2, R2[p], mul2(T2[p], gc2));
                 R2[p] = fma2(neg2(gc2), w2, R2[p]);
-                // C14: the clamp has zero derivative; dL/dpower = o G dL/dalpha (dL/do = G dL/dalpha = dpow / o: summed as sp)
-                const f32x2 dpow2 = mul2(pack2(og_a, og_b), pack2((og_a < amax) ? da_a : 0.0f, (og_b < amax) ? da_b : 0.0f));
+                // C14: the clamp has zero derivative; dL/dpower = o G dL/dalpha (dL/do = G dL/dalpha = dpow / o: summed as sp).
+                // The mask as a 1 / 0 factor (one FSET per pixel and one packed product instead of compare + select per pixel)
+                const f32x2 m2 = pack2((og_a < amax) ? 1.0f : 0.0f, (og_b < amax) ? 1.0f : 0.0f);
+                const f32x2 dpow2 = mul2(mul2(pack2(og_a, og_b), da2), m2);
                 const f32x2 dxp2 = mul2(dx2[p], dpow2);
                 if (p == 0) { sp2 = dpow2; spx2 = dxp2; spxx2 = mul2(dx2[p], dxp2); }
                 else { sp2 = add2(sp2, dpow2); spx2 = add2(spx2, dxp2); spxx2 = fma2(dx2[p], dxp2, spxx2); }
@@ -471,12 +473,12 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
                 float r2 = ((lane & 16) ? sz : sp) + __shfl_xor_sync(0xffffffffu, (lane & 16) ? sp : sz, 16);
 #pragma unroll
                 for (int o = 8; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
-                if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
+                if (red_lane) atomicAdd(red_base + red_stride * g, tot);
                 if (lane == 0) atomicAdd(g_opac + g, r2 * rcp_approx(c.w));
                 if (lane == 16) atomicAdd(g_depth + g, r2);
             } else {
                 const float sp_tot = warp_sum(sp);     // dL/do = (sum dpow) / o, divided by the one lane that adds it
-                if (red_lane) atomicAdd(red_base + (size_t)red_stride * g, tot);
+                if (red_lane) atomicAdd(red_base + red_stride * g, tot);
                 if (lane == 0) atomicAdd(g_opac + g, sp_tot * rcp_approx(c.w));
             }
         }
@@ -542,6 +544,7 @@ int32_t launch_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, cons
                    void* stream, int loss_kind = -1, const float* image = nullptr, const float* target = nullptr) {
     if (int32_t s = check_cam_cfg(cam, cfg)) return s;
     if (N < 0) return XPR_ERR_INVALID_ARG;
+    if (N >= (1ll << 30)) return XPR_ERR_UNSUPPORTED;      // xpr_bin_sort's limit; the kernel indexes the gradients with 32 bits
     if (!aligned(tile_ranges, 8) || !aligned(final_T, 4) || !aligned(n_contrib, 4)) return XPR_ERR_INVALID_ARG;
     if (loss_kind < 0 ? !aligned(dL_dimage, 4) : (loss_kind > 1 || !aligned(image, 4) || !aligned(target, 4)))
         return XPR_ERR_INVALID_ARG;
