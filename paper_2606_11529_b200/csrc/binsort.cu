@@ -603,7 +603,54 @@ rank_scan_kernel(const uint32_t* __restrict__ vidx, const int4* __restrict__ rec
 // intersection with the strip's edges) and then settles each end with the exact per-tile predicate tile_keep --
 // the decision that defines the result (bit-identical to the oracle's) -- stepping while the predicate disagrees.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, float C, float lnv, uint32_t tx, uint32_t ty);
+// tile_cull of XPR-3DGS ("Cull", Listing 1, A.1.1 L435) for the tiles of ONE tile row: operator()(tx) is
+// true when the pair (Gaussian, tile (tx, ty)) survives, i.e. unless min over the hull of the tile's pixel centres of
+// 1/2 d^T K d exceeds lnv = ln(o / alpha_thresh) by more than the conservative margin.  Evaluation order and margin are
+// reading C8 of DESIGN.md; every operation is individually rounded (explicit _rn intrinsics: this file is compiled with
+// FMA contraction).  The terms that depend on the row only (the y edges, the facing y edge's minimiser -B dy / A and its
+// c term) are formed once in init(): the same operations on the same operands as a per-tile evaluation, hoisted.
+struct RowKeep {
+    float mx, my, B, C, lnv, hA, hC, y_lo, y_hi, dyE, dxE, cE;
+    bool in_y;
+    __device__ __forceinline__ void init(float mx_, float my_, float A, float B_, float C_, float lnv_, uint32_t ty) {
+        const float ts = (float)TILE;
+        mx = mx_; my = my_; B = B_; C = C_; lnv = lnv_;
+        hA = __fmul_rn(0.5f, A); hC = __fmul_rn(0.5f, C);
+        const float y0 = __fadd_rn(__fmul_rn(ts, (float)ty), 0.5f), y1 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)ty), ts), 0.5f);
+        in_y = (my >= y0) && (my <= y1);
+        y_lo = __fsub_rn(y0, my); y_hi = __fsub_rn(y1, my);
+        dyE = __fsub_rn((my < y0) ? y0 : y1, my);               // the facing y edge (used when !in_y)
+        dxE = __fdiv_rn(-__fmul_rn(B, dyE), A);
+        cE = __fmul_rn(__fmul_rn(hC, dyE), dyE);
+    }
+    __device__ __forceinline__ bool drop(float a, float b, float c) const {
+        const float margin = 1.0f / 262144.0f;   // 2^-18
+        const float q = __fadd_rn(__fadd_rn(a, b), c);
+        const float mag = __fadd_rn(__fadd_rn(__fadd_rn(fabsf(a), fabsf(b)), fabsf(c)), lnv);
+        return q > __fadd_rn(lnv, __fmul_rn(mag, margin));
+    }
+    __device__ __forceinline__ bool operator()(uint32_t tx) const {
+        const float ts = (float)TILE;
+        const float x0 = __fadd_rn(__fmul_rn(ts, (float)tx), 0.5f), x1 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)tx), ts), 0.5f);
+        const bool in_x = (mx >= x0) && (mx <= x1);
+        if (in_x && in_y) return true;
+        bool dropped = true;                      // dropped by every facing edge
+        if (!in_x) {
+            const float dx = __fsub_rn((mx < x0) ? x0 : x1, mx);
+            const float bx = __fmul_rn(B, dx);
+            float dy = __fdiv_rn(-bx, C);
+            dy = (dy < y_lo) ? y_lo : dy; dy = (y_hi < dy) ? y_hi : dy;
+            dropped = drop(__fmul_rn(__fmul_rn(hA, dx), dx), __fmul_rn(bx, dy), __fmul_rn(__fmul_rn(hC, dy), dy));
+        }
+        if (!in_y) {
+            const float lo = __fsub_rn(x0, mx), hi = __fsub_rn(x1, mx);
+            float dx = dxE;
+            dx = (dx < lo) ? lo : dx; dx = (hi < dx) ? hi : dx;
+            dropped = dropped && drop(__fmul_rn(__fmul_rn(hA, dx), dx), __fmul_rn(__fmul_rn(B, dx), dyE), cE);
+        }
+        return !dropped;
+    }
+};
 
 __device__ __forceinline__ float approx_sqrt(float x) {   // the interval estimate needs no exact rounding
     float y;
@@ -725,7 +772,8 @@ rows_kernel(int TW, int TH, int TH_view, const uint32_t* __restrict__ vidx, cons
         }
         if (CULL == 1) {
             const int tyv = ty % TH_view;              // batch of views: the tile rows of view v are offset by v * TH_view
-            const auto keep = [&](int tx) { return tile_keep(mx, my, A, B, C, L, (uint32_t)tx, (uint32_t)tyv); };
+            RowKeep keep;
+            keep.init(mx, my, A, B, C, L, (uint32_t)tyv);
             // estimate: x extent of {q <= L} over dy in [lo, hi] (pixel-centre hull of the row)
             const float lo = (float)(TILE * tyv) + 0.5f - my, hi = (float)(TILE * tyv + TILE) - 0.5f - my;
             float left = 1e30f, right = -1e30f;
@@ -743,39 +791,57 @@ rows_kernel(int TW, int TH, int TH_view, const uint32_t* __restrict__ vidx, cons
                 }
             }
             if (lo <= 0.0f && hi >= 0.0f) { left = fminf(left, 0.0f); right = fmaxf(right, 0.0f); }   // the mean's row
-            bool found = false;
+            // q_min over the row's tiles is convex in x, so if any tile is kept the one nearest the row's minimiser x* is:
+            // x* = mx when the mean lies in the row's strip, else mx - B c / A with c the strip edge nearest the mean
+            const float cm = (lo <= 0.0f && hi >= 0.0f) ? 0.0f : ((lo > 0.0f) ? lo : hi);
+            const int tc = max(r.x, min(r.z - 1, (int)floorf((mx - B * cm * rA) * (1.0f / (float)TILE))));
+            // The two ends are settled with the exact predicate by ONE loop around ONE evaluation: every lane carries a
+            // small state (which end, which direction, the candidate tile), so that the lanes of a warp evaluate their
+            // candidates together whatever paths their rows take (separate loops per case serialise the warp and repeat
+            // the predicate's code a dozen times).  Typical row: 4 evaluations (keep(a), !keep(a - 1), keep(b - 1), !keep(b)).
+            //   L0 first probe of the left end · LOUT stepping outwards while kept · LIN stepping inwards until kept
+            //   R0 / ROUT / RIN the same for the right end · C0 C1 C2 the estimate saw nothing: probe the tile nearest x*
+            //   and its two neighbours (rounding of x*), then grow from there
+            enum { L0, LOUT, LIN, R0, ROUT, RIN, C0, C1, C2, DONE };
+            int st, cand, a = r.x, b = r.x, xe = r.z;
             if (left <= right) {
-                xa = max(r.x, min(r.z - 1, (int)floorf((mx + left - ((float)TILE - 0.5f)) * (1.0f / (float)TILE)) + 1));
-                xb = max(xa, min(r.z - 1, (int)floorf((mx + right - 0.5f) * (1.0f / (float)TILE)))) + 1;   // exclusive
-                // settle the left end with the exact predicate
-                int t = xa;
-                if (keep(t)) { while (t > r.x && keep(t - 1)) --t; found = true; }
-                else { while (t < xb && !keep(t)) ++t; found = t < xb; }
-                xa = t;
-                if (found) {
-                    t = max(xb - 1, xa);
-                    if (keep(t)) { while (t + 1 < r.z && keep(t + 1)) ++t; }
-                    else { while (t > xa && !keep(t)) --t; }
-                    xb = t + 1;
+                const int a0 = max(r.x, min(r.z - 1, (int)floorf((mx + left - ((float)TILE - 0.5f)) * (1.0f / (float)TILE)) + 1));
+                xe = max(a0, min(r.z - 1, (int)floorf((mx + right - 0.5f) * (1.0f / (float)TILE)))) + 1;   // exclusive
+                st = L0; cand = a0;
+            } else { st = C0; cand = tc; }
+            while (st != DONE) {
+                const bool k = keep((uint32_t)cand);
+                const bool was_centre = st >= C0;
+                bool to_right = false, to_centre = false, empty = false;
+                if (st == L0 || st == LOUT || was_centre) {
+                    if (k) {
+                        a = cand;
+                        if (was_centre) xe = cand + 1;
+                        if (cand > r.x) { st = LOUT; cand = cand - 1; } else to_right = true;
+                    } else if (st == LOUT) to_right = true;
+                    else if (st == L0) { if (cand + 1 < xe) { st = LIN; cand = cand + 1; } else to_centre = true; }
+                    else if (st == C0 && tc > r.x) { st = C1; cand = tc - 1; }
+                    else if (st != C2 && tc + 1 < r.z) { st = C2; cand = tc + 1; }
+                    else empty = true;
+                } else if (st == LIN) {
+                    if (k) { a = cand; to_right = true; }
+                    else if (cand + 1 < xe) cand = cand + 1;
+                    else to_centre = true;
+                } else if (st == R0 || st == ROUT) {
+                    if (k) { b = cand + 1; if (b < r.z) { st = ROUT; cand = b; } else st = DONE; }
+                    else if (st == ROUT) st = DONE;
+                    else if (cand - 1 > a) { st = RIN; cand = cand - 1; }
+                    else { b = a + 1; st = DONE; }
+                } else {   // RIN
+                    if (k) { b = cand + 1; st = DONE; }
+                    else if (cand - 1 > a) cand = cand - 1;
+                    else { b = a + 1; st = DONE; }
                 }
+                if (to_right) { st = R0; cand = max(xe - 1, a); }
+                if (to_centre) { st = C0; cand = tc; }
+                if (empty) { a = b = r.x; st = DONE; }
             }
-            if (!found) {
-                // the estimate saw nothing.  q_min over the row's tiles is convex in x, so if any tile is kept the
-                // one nearest the row's minimiser x* is: x* = mx when the mean lies in the row's strip, else
-                // mx - B c / A with c the strip edge nearest the mean.  Test it and its neighbours (rounding of
-                // x*), then grow the interval with the predicate.
-                const float c = (lo <= 0.0f && hi >= 0.0f) ? 0.0f : ((lo > 0.0f) ? lo : hi);
-                const int tc = max(r.x, min(r.z - 1, (int)floorf((mx - B * c * rA) * (1.0f / (float)TILE))));
-                int t = -1;
-                if (keep(tc)) t = tc;
-                else if (tc > r.x && keep(tc - 1)) t = tc - 1;
-                else if (tc + 1 < r.z && keep(tc + 1)) t = tc + 1;
-                if (t < 0) { xa = xb = r.x; }
-                else {
-                    xa = t; while (xa > r.x && keep(xa - 1)) --xa;
-                    xb = t + 1; while (xb < r.z && keep(xb)) ++xb;
-                }
-            }
+            xa = a; xb = b;
         }
         // the row as (first column, length); its tiles ty TW + xa ... are consecutive ids: +1 where the run starts,
         // -1 behind its end -- the running sum of the array is the number of pairs of every tile
@@ -793,42 +859,6 @@ rows_kernel(int TW, int TH, int TH_view, const uint32_t* __restrict__ vidx, cons
         const int v = s_rowstart[y];
         if (v) atomicAdd(tile_diff + y * TW, v);
     }
-}
-
-// tile_cull of XPR-3DGS ("Cull", Listing 1, A.1.1 L435): true when the pair survives,
-// i.e. unless min over the hull of the tile's pixel centres of 1/2 d^T K d exceeds lnv = ln(o / alpha_thresh)
-// by more than the conservative margin.  Evaluation order and margin are reading C8 of DESIGN.md; every
-// operation is individually rounded (explicit _rn intrinsics: this file is compiled with FMA contraction).
-__device__ __forceinline__ bool tile_keep(float mx, float my, float A, float B, float C, float lnv, uint32_t tx, uint32_t ty) {
-    const float ts = (float)TILE;
-    const float x0 = __fadd_rn(__fmul_rn(ts, (float)tx), 0.5f), x1 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)tx), ts), 0.5f);
-    const float y0 = __fadd_rn(__fmul_rn(ts, (float)ty), 0.5f), y1 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)ty), ts), 0.5f);
-    const bool in_x = (mx >= x0) && (mx <= x1), in_y = (my >= y0) && (my <= y1);
-    if (in_x && in_y) return true;
-    const float margin = 1.0f / 262144.0f;   // 2^-18
-    auto drop = [&](float dx, float dy) {
-        const float a = __fmul_rn(__fmul_rn(__fmul_rn(0.5f, A), dx), dx), b = __fmul_rn(__fmul_rn(B, dx), dy),
-                    c = __fmul_rn(__fmul_rn(__fmul_rn(0.5f, C), dy), dy);
-        const float q = __fadd_rn(__fadd_rn(a, b), c);
-        const float mag = __fadd_rn(__fadd_rn(__fadd_rn(fabsf(a), fabsf(b)), fabsf(c)), lnv);
-        return q > __fadd_rn(lnv, __fmul_rn(mag, margin));
-    };
-    bool dropped = true;                      // dropped by every facing edge
-    if (!in_x) {
-        const float dx = __fsub_rn((mx < x0) ? x0 : x1, mx);
-        float dy = __fdiv_rn(-__fmul_rn(B, dx), C);
-        const float lo = __fsub_rn(y0, my), hi = __fsub_rn(y1, my);
-        dy = (dy < lo) ? lo : dy; dy = (hi < dy) ? hi : dy;
-        dropped = dropped && drop(dx, dy);
-    }
-    if (!in_y) {
-        const float dy = __fsub_rn((my < y0) ? y0 : y1, my);
-        float dx = __fdiv_rn(-__fmul_rn(B, dy), A);
-        const float lo = __fsub_rn(x0, mx), hi = __fsub_rn(x1, mx);
-        dx = (dx < lo) ? lo : dx; dx = (hi < dx) ? hi : dx;
-        dropped = dropped && drop(dx, dy);
-    }
-    return !dropped;
 }
 
 // ---------------------------------------------------------------------------------------------
