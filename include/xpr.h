@@ -90,8 +90,11 @@ int32_t xpr_version(void);           /* 10000*major + 100*minor + patch */
  *        tile_count[N] = rectangle area if visible else 0, flags[N];
  *        shade_rec[N,12] (may be NULL) = the shader data p_sd of the primitive packed as the
  *        compositing calls read it, 3 x float4, 16-byte aligned:
- *          (mx, my, -A/2, -B | -C/2, -lnv, log2 o_eff, depth | r, g, b, o_eff)
- *        -- the pre-scaled conic of reading C25 (exact in fp32); log2 by lg2.approx (it only feeds exp()).
+ *          (mx, my, -A/2, -B | -C/2, lnv, log2 o_eff, depth | r, g, b, o_eff)
+ *        -- the pre-scaled conic of reading C25 (exact in fp32); log2 by lg2.approx (it only feeds exp()).  lnv > 0 in
+ *        every record xpr_project writes (a Gaussian with lnv <= 0 has an empty extent and is culled); the compositing
+ *        kernels rely on it: they test both gates of a list entry (power <= 0, power >= -lnv) as ONE unsigned compare
+ *        bits(-power) <= bits(lnv), so a record built by the caller (xpr_shade_record) must come from such a Gaussian.
  *   For a culled Gaussian only tile_count (=0) and flags (=0) are written; its other outputs are
  *   left untouched (they are never read downstream).
  *   Arithmetic follows rule R1: fp32, every operation individually rounded, no FMA contraction,

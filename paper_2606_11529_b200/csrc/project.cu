@@ -388,7 +388,7 @@ project_kernel(int64_t N, const __grid_constant__ ProjBatch PB, const float* __r
             const float2 m = reinterpret_cast<const float2*>(mean2d)[o];        // written in phase B by this CTA
             const float4 co = reinterpret_cast<const float4*>(conic_opac)[o];
             shade_rec[3 * o] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-            shade_rec[3 * o + 1] = make_float4(-0.5f * co.z, -lnv[o], __log2f(co.w), depth[o]);
+            shade_rec[3 * o + 1] = make_float4(-0.5f * co.z, lnv[o], __log2f(co.w), depth[o]);
             shade_rec[3 * o + 2] = make_float4(col[0], col[1], col[2], co.w);
         }
     }

@@ -4,7 +4,7 @@
 //
 // One CTA per 16x16 tile.  The tile's list vals_sorted[start..end) is a list of Gaussian indices; the shader
 // data p_sd of a Gaussian is one 48-byte record shade_rec[g] = 3 x float4
-//     (mx, my, qa, qb | qc, thr, log2 o, z | r, g, b, o),   qa = -A/2, qb = -B, qc = -C/2, thr = -lnv   (C25),
+//     (mx, my, qa, qb | qc, lnv, log2 o, z | r, g, b, o),   qa = -A/2, qb = -B, qc = -C/2   (C25),
 // written by xpr_project.  Batches of records are gathered into shared memory with cp.async (16-byte LDGSTS, no
 // register staging) through a three-stage ring: while batch b is walked, the copies of batches b+1 and b+2 are
 // in flight and the list indices of batch b+3 are being loaded, so a CTA waits for memory only at its start and
@@ -138,7 +138,7 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
                 const float dxa = pxc0 - ge.x;
                 pw_a[u] = __fmaf_rn(__fmaf_rn(-ge.z, dxa, t1), dxa, t2);
             }
-            lim[u] = __float_as_uint(-ga.y); l2o[u] = ga.z;
+            lim[u] = __float_as_uint(ga.y); l2o[u] = ga.z;
             if (FEAT) zz[u] = ga.w;
             if (BF) col[u] = rq[2];
         };
@@ -407,7 +407,7 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
             const float4 ga = rq[1];       // qc thr log2o z
             const float dy = pyc - ge.y;
             const float t1 = __fmul_rn(-ge.w, dy), t2 = __fmul_rn(__fmul_rn(-ga.x, dy), dy);   // row terms of -power
-            const uint32_t lim = __float_as_uint(-ga.y);                                         // bits of lnv
+            const uint32_t lim = __float_as_uint(ga.y);                                          // bits of lnv
             f32x2 dx2[NP], pw2[NP];                                                              // pw2 = -power (forward kernel)
             bool contrib[PPT], any_c = false;
 #pragma unroll
@@ -498,7 +498,7 @@ shade_record_kernel(int64_t N, const float2* __restrict__ mean2d, const float4* 
     const float2 m = mean2d[i];
     const float4 co = conic_opac[i];
     rec[3 * i] = make_float4(m.x, m.y, -0.5f * co.x, -co.y);
-    rec[3 * i + 1] = make_float4(-0.5f * co.z, -lnv[i], __log2f(co.w), depth ? depth[i] : 0.0f);
+    rec[3 * i + 1] = make_float4(-0.5f * co.z, lnv[i], __log2f(co.w), depth ? depth[i] : 0.0f);
     rec[3 * i + 2] = make_float4(rgb[3 * i], rgb[3 * i + 1], rgb[3 * i + 2], co.w);
 }
 
