@@ -28,6 +28,7 @@ struct RasterParams {
     float amax, tmin;
     float bg[3];
     const uint32_t* order;   // xpr_config.tile_order: CTA b works on tile order[b] (longest lists first), or NULL
+    int vec;                 // backward: W % 4 == 0 and the per-pixel arrays are 16-byte aligned (128-bit prologue loads)
 };
 
 // Both gates of a list entry on m = -power: valid (power <= 0, L289) and alpha >= alpha_thresh (power >= -lnv, L679)
@@ -323,38 +324,81 @@ rasterize_bwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
     uint32_t n[PPT];
     f32x2 px2[NP], T2[NP], R2[NP], g0_2[NP], g1_2[NP], g2_2[NP], gD_2[NP];
     uint32_t wmax = 0;
+    {
+        // per-pixel inputs: n_contrib, T_final and dL/dpixel (or image and target).  A thread's PPT pixels are consecutive,
+        // so when the row is whole and the arrays are 16-byte aligned (P.vec: W % 4 == 0) they are read as 128-bit words
+        float tt[PPT], a0[PPT], a1[PPT], a2[PPT], aD[PPT], gA[PPT];
+        auto sgn = [](float d) { return d > 0.0f ? 1.0f : (d < 0.0f ? -1.0f : d); };
 #pragma unroll
-    for (int p = 0; p < NP; ++p) {
-        float t[2], q[2], a0[2], a1[2], a2[2], aD[2];
+        for (int k = 0; k < PPT; ++k) { n[k] = 0; tt[k] = a0[k] = a1[k] = a2[k] = aD[k] = gA[k] = 0.0f; }
+        if ((PPT % 4 == 0) && P.vec && (px0 + PPT <= P.W) && (py < P.H)) {
+            const int64_t pid0 = vbase + (int64_t)py * P.W + px0;
+            constexpr int Q = (PPT % 4 == 0) ? PPT / 4 : 1;
+            float c[12 * Q];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int k = 2 * p + h, px = px0 + k;
-            n[k] = 0; t[h] = 0.0f; a0[h] = a1[h] = a2[h] = aD[h] = 0.0f;
-            float gA = 0.0f;
-            if (px < P.W && py < P.H) {
-                const int64_t pid = vbase + (int64_t)py * P.W + px;
-                n[k] = n_contrib[pid];
-                t[h] = final_T[pid];
-                if (loss_kind < 0) {
-                    a0[h] = dL[3 * pid]; a1[h] = dL[3 * pid + 1]; a2[h] = dL[3 * pid + 2];
-                } else {
-                    const float d0 = image[3 * pid] - target[3 * pid], d1 = image[3 * pid + 1] - target[3 * pid + 1],
-                                d2 = image[3 * pid + 2] - target[3 * pid + 2];
-                    auto sgn = [](float d) { return d > 0.0f ? 1.0f : (d < 0.0f ? -1.0f : d); };
-                    a0[h] = loss_kind == 0 ? sgn(d0) : 2.0f * d0;
-                    a1[h] = loss_kind == 0 ? sgn(d1) : 2.0f * d1;
-                    a2[h] = loss_kind == 0 ? sgn(d2) : 2.0f * d2;
+            for (int v = 0; v < Q; ++v) {
+                const uint4 nv = __ldg(reinterpret_cast<const uint4*>(n_contrib + pid0) + v);
+                const float4 tv = __ldg(reinterpret_cast<const float4*>(final_T + pid0) + v);
+                n[4 * v] = nv.x; n[4 * v + 1] = nv.y; n[4 * v + 2] = nv.z; n[4 * v + 3] = nv.w;
+                tt[4 * v] = tv.x; tt[4 * v + 1] = tv.y; tt[4 * v + 2] = tv.z; tt[4 * v + 3] = tv.w;
+                if (FEAT) {
+                    const float4 dv = __ldg(reinterpret_cast<const float4*>(dL_dD + pid0) + v);
+                    const float4 av = __ldg(reinterpret_cast<const float4*>(dL_dA + pid0) + v);
+                    aD[4 * v] = dv.x; aD[4 * v + 1] = dv.y; aD[4 * v + 2] = dv.z; aD[4 * v + 3] = dv.w;
+                    gA[4 * v] = av.x; gA[4 * v + 1] = av.y; gA[4 * v + 2] = av.z; gA[4 * v + 3] = av.w;
                 }
-                if (FEAT) { aD[h] = dL_dD[pid]; gA = dL_dA[pid]; }
             }
-            // Q = g . S behind the last entry = T_final (g . bg) (C13) (FEAT: - gA T_final)
-            q[h] = t[h] * (fmaf(a2[h], P.bg[2], fmaf(a1[h], P.bg[1], a0[h] * P.bg[0])) - gA);
-            wmax = max(wmax, n[k]);
+#pragma unroll
+            for (int v = 0; v < 3 * Q; ++v) {
+                float4 x;
+                if (loss_kind < 0) x = __ldg(reinterpret_cast<const float4*>(dL + 3 * pid0) + v);
+                else {
+                    const float4 im = __ldg(reinterpret_cast<const float4*>(image + 3 * pid0) + v);
+                    const float4 tg = __ldg(reinterpret_cast<const float4*>(target + 3 * pid0) + v);
+                    const float d0 = im.x - tg.x, d1 = im.y - tg.y, d2 = im.z - tg.z, d3 = im.w - tg.w;
+                    x = loss_kind == 0 ? make_float4(sgn(d0), sgn(d1), sgn(d2), sgn(d3)) : make_float4(2.0f * d0, 2.0f * d1, 2.0f * d2, 2.0f * d3);
+                }
+                c[4 * v] = x.x; c[4 * v + 1] = x.y; c[4 * v + 2] = x.z; c[4 * v + 3] = x.w;
+            }
+#pragma unroll
+            for (int k = 0; k < 4 * Q; ++k) { a0[k] = c[3 * k]; a1[k] = c[3 * k + 1]; a2[k] = c[3 * k + 2]; }
+        } else {
+#pragma unroll
+            for (int k = 0; k < PPT; ++k) {
+                const int px = px0 + k;
+                if (px < P.W && py < P.H) {
+                    const int64_t pid = vbase + (int64_t)py * P.W + px;
+                    n[k] = n_contrib[pid];
+                    tt[k] = final_T[pid];
+                    if (loss_kind < 0) {
+                        a0[k] = dL[3 * pid]; a1[k] = dL[3 * pid + 1]; a2[k] = dL[3 * pid + 2];
+                    } else {
+                        const float d0 = image[3 * pid] - target[3 * pid], d1 = image[3 * pid + 1] - target[3 * pid + 1],
+                                    d2 = image[3 * pid + 2] - target[3 * pid + 2];
+                        a0[k] = loss_kind == 0 ? sgn(d0) : 2.0f * d0;
+                        a1[k] = loss_kind == 0 ? sgn(d1) : 2.0f * d1;
+                        a2[k] = loss_kind == 0 ? sgn(d2) : 2.0f * d2;
+                    }
+                    if (FEAT) { aD[k] = dL_dD[pid]; gA[k] = dL_dA[pid]; }
+                }
+            }
         }
-        px2[p] = pack2((float)(px0 + 2 * p) + 0.5f, (float)(px0 + 2 * p + 1) + 0.5f);
-        T2[p] = pack2(t[0], t[1]); R2[p] = pack2(-q[0], -q[1]);
-        g0_2[p] = pack2(a0[0], a0[1]); g1_2[p] = pack2(a1[0], a1[1]); g2_2[p] = pack2(a2[0], a2[1]);
-        gD_2[p] = pack2(aD[0], aD[1]);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            float q[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int k = 2 * p + h;
+                // Q = g . S behind the last entry = T_final (g . bg) (C13) (FEAT: - gA T_final)
+                q[h] = tt[k] * (fmaf(a2[k], P.bg[2], fmaf(a1[k], P.bg[1], a0[k] * P.bg[0])) - gA[k]);
+                wmax = max(wmax, n[k]);
+            }
+            px2[p] = pack2((float)(px0 + 2 * p) + 0.5f, (float)(px0 + 2 * p + 1) + 0.5f);
+            T2[p] = pack2(tt[2 * p], tt[2 * p + 1]); R2[p] = pack2(-q[0], -q[1]);
+            g0_2[p] = pack2(a0[2 * p], a0[2 * p + 1]); g1_2[p] = pack2(a1[2 * p], a1[2 * p + 1]);
+            g2_2[p] = pack2(a2[2 * p], a2[2 * p + 1]);
+            gD_2[p] = pack2(aD[2 * p], aD[2 * p + 1]);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
@@ -507,6 +551,7 @@ void make_raster_params(const xpr_camera* cam, const xpr_config* cfg, RasterPara
     P.amax = cfg->alpha_max; P.tmin = cfg->t_min;
     for (int i = 0; i < 3; ++i) P.bg[i] = cfg->bg[i];
     P.order = cfg->tile_order;
+    P.vec = 0;
 }
 
 template <bool FEAT>
@@ -569,8 +614,11 @@ int32_t launch_bwd(const xpr_camera* cam, const xpr_config* cfg, int64_t N, cons
     }
     RasterParams P;
     make_raster_params(cam, cfg, P);
+    P.vec = (cam->width % 4 == 0) && aligned(final_T, 16) && aligned(n_contrib, 16) &&
+            (loss_kind < 0 ? aligned(dL_dimage, 16) : (aligned(image, 16) && aligned(target, 16))) &&
+            (!FEAT || (aligned(dL_ddepth, 16) && aligned(dL_dalpha, 16)));
     const int T = tiles_x(cam) * tiles_y(cam) * num_views(cfg);
-    // 4 pixels per thread (64 threads) is the throughput shape; images with few tiles are bounded by their
+    // 8 pixels per thread (one warp per tile) is the throughput shape; images with few tiles are bounded by their
     // heaviest tile, where more warps per tile (2 pixels per thread) shorten the critical path
 #define XPR_BWD(PPT_)                                                                                               \
     rasterize_bwd_kernel<PPT_, FEAT><<<T, BLOCK / PPT_, 0, st>>>(                                                     \
