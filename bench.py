@@ -54,9 +54,10 @@ def parse():
     ap.add_argument("--fuse-loss", type=int, default=1, choices=(0, 1),
                     help="1: the loss gradient is formed inside the compositing backward (xpr_rasterize_bwd_loss) instead of a "
                          "separate xpr_loss_grad pass (colour pass of the 2D evaluation only; same results)")
-    ap.add_argument("--overlap-fill", type=int, default=-1, choices=(-1, 0, 1, 2),
+    ap.add_argument("--overlap-fill", type=int, default=-1, choices=(-1, 0, 1, 2, 4),
                     help="pipeline option overlap_fill: the zero-fill of the parameter gradients on a second stream, forked at the "
-                         "compositing backward (1) or at the binning stage (2); 0 off; -1 the pipeline's default")
+                         "forward compositing kernel (4), the compositing backward (1) or the binning stage (2); 0: inside "
+                         "xpr_project_bwd; -1 the pipeline's default (4)")
     ap.add_argument("--features", type=int, default=0, choices=(0, 1),
                     help="1: also render the depth image and the accumulated opacity and take their gradients "
                          "(SURVEY 8(f) f3, DESIGN.md 6.8; with --ray-eval 1 through the ray kernels; not part of the headline workload)")
@@ -451,12 +452,19 @@ def run_ours(args):
         timed.append(evs)
     barrier()
     assert pipe.check_capacity() == n_pairs          # the asynchronous steps produced the same, fitting, pair count
-    for _ in range(args.steps):             # a second pass of K steps with an event between the stages: the breakdown
+    # a second pass of K steps with an event between the stages: the breakdown.  Every stage is timed ALONE here: the
+    # zero-fill of the parameter gradients, which the timed steps above run on a second stream under the forward
+    # compositing kernel (pipeline option overlap_fill), is back inside project_bwd, so no stage shares the GPU
+    timed_overlap = int(pipe.overlap_fill)
+    torch.cuda.synchronize()
+    pipe.overlap_fill = 0                   # (every timed step consumed the fill it forked: none is pending)
+    for _ in range(args.steps):
         flush.fill_(1)
         evs = []
         step(evs)
         all_events.append(evs)
     barrier()
+    pipe.overlap_fill = timed_overlap
     step_ms = [e[0].elapsed_time(e[-1]) for e in timed]
     total_ms = max_over_ranks(float(sum(step_ms)), world, dev)
     ms = total_ms / args.steps
@@ -466,8 +474,10 @@ def run_ours(args):
     step_stats = {"mean": float(np.mean(step_ms)), "median": float(np.median(step_ms)), "min": float(np.min(step_ms)),
                   "max": float(np.max(step_ms)), "note": "this rank's K timed steps, one CUDA event before and one after each; ms_per_step is the mean, max over ranks",
                   "instrumented_ms_per_step": instrumented_ms,
-                  "stage_ms_note": "stage_ms comes from a second pass of K steps with an event between the stages; those events cost "
-                                   "stream time, so the stages sum to instrumented_ms_per_step, not to ms_per_step"}
+                  "stage_ms_note": "stage_ms comes from a second pass of K steps with an event between the stages and every stage alone "
+                                   "on the GPU (overlap_fill 0: the 236 B/Gaussian zero-fill inside project_bwd); the events cost stream "
+                                   "time and the timed steps run that fill under the forward kernel, so the stages sum to "
+                                   "instrumented_ms_per_step, not to ms_per_step"}
     mp = V * cam.width * cam.height / 1e6
     value = aggregate_value(world, mp, ms)
 
@@ -760,7 +770,7 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "view": args.view, "gaussians": sc.N,
-                           "image": [cam.width, cam.height], "views": V, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "fuse_loss": int(fused), "pairs": n_pairs,
+                           "image": [cam.width, cam.height], "views": V, "tile_cull": args.tile_cull, "ray_eval": args.ray_eval, "features": args.features, "tile_order": int(pipe.tile_order is not None), "fuse_loss": int(fused), "overlap_fill": int(pipe.overlap_fill), "pairs": n_pairs,
                            "candidate_pairs": n_cand, "rows": n_rows, "supertile_words": n_words, "visible_gaussians": n_vis,
                            "sort_passes": {"depth_digits_on_gaussians": 4, "supertile_digits_on_words": tile_passes,
                                            "on_pairs": 0},

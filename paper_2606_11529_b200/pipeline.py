@@ -36,10 +36,12 @@ class SplatPipeline:
         if self.V > 1 and self.ray_eval:
             raise ValueError("xpr: a batch of views is built for the 2D evaluation (colour, depth and accumulated opacity)")
         self._dL = None
-        # overlap_fill = 1: the zero-fill of the parameter gradients (xpr_project_bwd_fill: HBM traffic without inputs) runs on
-        # a second stream under the compositing backward.  Off by default: measured on config 3 / 5 the compositing kernel
-        # slows down by what the fill saves (0.326 -> 0.351 ms, project_bwd 0.083 -> 0.045 ms: step -1 %), DESIGN.md 6.5
-        self.overlap_fill = int(cfg.get("overlap_fill", 0)) if isinstance(cfg, dict) else 0
+        # overlap_fill: the zero-fill of the parameter gradients (xpr_project_bwd_fill: 236 B per Gaussian of HBM stores without
+        # inputs) runs on a second stream, forked at the forward compositing kernel (4, the default), at the compositing
+        # backward (1) or at the binning stage (2); 0: inside xpr_project_bwd.  Measured: under the forward
+        # kernel -- ALU-bound, no atomics -- the step gets 16 us shorter on configs 3 and 5; under the backward or the
+        # binning kernels the host kernel slows down by what the fill saves.
+        self.overlap_fill = int(cfg.get("overlap_fill", 4)) if isinstance(cfg, dict) else 4
         self._filled = False
         # fuse_loss: step_async() forms dL/dimage of the two configured losses inside the compositing backward
         # (xpr_rasterize_bwd_loss) instead of a separate xpr_loss_grad pass; colour pass of the 2D evaluation only
@@ -174,6 +176,7 @@ class SplatPipeline:
         return n
 
     def rasterize_fwd(self):
+        self._fork_fill(4)      # (the parameter-gradient arrays of the previous step are cleared from here on)
         if self.ray_eval and self.features:
             xb.xpr_rasterize_ray_feat_fwd(self.cam, self.cfg, self.ray_rec, self.conic_opac, self.rgb, self.lnv, self.depth,
                                           self.pixel_rays, self.vals_sorted, self.tile_ranges, self.image, self.final_T,

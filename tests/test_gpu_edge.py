@@ -298,8 +298,10 @@ def test_tile_cull_needle_gaussians_bit_exact(seed):
 
 
 @pytest.mark.gpu
-def test_overlapped_zero_fill_gives_the_same_gradients():
-    """xpr_project_bwd_fill on a second stream + xpr_project_bwd_filled (pipeline option overlap_fill) against the plain
+@pytest.mark.parametrize("mode", [4, 1, 2])
+def test_overlapped_zero_fill_gives_the_same_gradients(mode):
+    """xpr_project_bwd_fill on a second stream + xpr_project_bwd_filled (pipeline option overlap_fill: forked at the
+    forward compositing kernel (4, the default), at the backward (1) or at the binning stage (2)) against the plain
     xpr_project_bwd: same parameter gradients bit for bit (no atomics at one view), also when captured in a CUDA graph."""
     import numpy as np
     import torch
@@ -309,8 +311,11 @@ def test_overlapped_zero_fill_gives_the_same_gradients():
     params = pipeline.scene_to_device(sc)
     target = torch.from_numpy(sc.target(0)).cuda()
     names = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
-    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], dict(cfg, overlap_fill=1))
+    pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], dict(cfg, overlap_fill=mode))
+    assert pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg).overlap_fill == 4
     pipe.forward(*params)
+    pipe.step_async(*params, target, sc.loss)               # consumes the fill a first forward may have forked
+    torch.cuda.synchronize()
     for k in names:
         getattr(pipe, k).fill_(float("nan"))                # the fill must really happen
     pipe.step_async(*params, target, sc.loss)               # fill on the side stream, xpr_project_bwd_filled
@@ -318,8 +323,10 @@ def test_overlapped_zero_fill_gives_the_same_gradients():
     a = {k: getattr(pipe, k).cpu().numpy().copy() for k in names}
     for k in names:
         getattr(pipe, k).fill_(float("nan"))
+    pipe.overlap_fill = 0
     pipe.project_bwd()                                      # no fork before it: the plain xpr_project_bwd on the same 2D gradients
     torch.cuda.synchronize()
+    pipe.overlap_fill = mode
     for k in names:
         b = getattr(pipe, k).cpu().numpy()
         assert np.isfinite(b).all() and np.array_equal(a[k], b), k
