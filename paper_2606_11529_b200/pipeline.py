@@ -194,8 +194,12 @@ class SplatPipeline:
         xb.xpr_rasterize_fwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.image,
                              self.final_T, self.n_contrib)
 
+    OVERLAP_MIN_BYTES = 32 << 20
+
     def _fork_fill(self, where: int):
         if self.overlap_fill != where or self._filled:
+            return
+        if self.N * (11 + 3 * self.K) * 4 < self.OVERLAP_MIN_BYTES:      # small scenes: the fork / join costs more than the fill
             return
         if not hasattr(self, "_side"):
             self._side = torch.cuda.Stream(device=self.device)

@@ -312,6 +312,7 @@ def test_overlapped_zero_fill_gives_the_same_gradients(mode):
     target = torch.from_numpy(sc.target(0)).cuda()
     names = ("g_means", "g_scales", "g_quats", "g_opacities", "g_sh")
     pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], dict(cfg, overlap_fill=mode))
+    pipe.OVERLAP_MIN_BYTES = 0                              # (the pipeline skips the fork for scenes this small)
     assert pipeline.SplatPipeline(sc.N, sc.cameras[0], cfg).overlap_fill == 4
     pipe.forward(*params)
     pipe.step_async(*params, target, sc.loss)               # consumes the fill a first forward may have forked
