@@ -192,6 +192,18 @@ def test_tile_cull_ragged_and_edge():
     full_parity(scenes.make_scene(1, n_override=600, image_override=(33, 17)), 0, CULL)
 
 
+@pytest.mark.parametrize("wh", [(1924, 1083), (1925, 1081)])
+@pytest.mark.parametrize("cull", [0, 1])
+def test_throughput_shapes_on_ragged_widths(wh, cull):
+    """>= 4096 tiles select the throughput shapes of the compositing kernels (forward: pixel pairs (x, x + 8); backward: 8
+    consecutive pixels per thread, one warp per tile, per-pixel inputs as 128-bit words when W % 4 == 0).  Widths that are not
+    a multiple of 8 (a thread's pixels straddle the image edge) or of 4 (no vector loads) and a ragged last tile row, with
+    and without tile_cull (the branch-free and the branching forward blend)."""
+    sc = scenes.make_scene(3, n_override=40000, image_override=wh)
+    assert ((wh[0] + 15) // 16) * ((wh[1] + 15) // 16) >= 4096
+    full_parity(sc, 0, dict(tile_cull=cull))
+
+
 def test_tile_cull_config3_full_size_bench_configuration():
     g, o = full_parity(scenes.make_scene(3), 0, CULL)
     assert o["binned"]["num_pairs"] < 0.75 * o["binned"]["num_candidates"]
