@@ -82,6 +82,7 @@ class SplatPipeline:
         # the compositing gradients share one allocation, in the order the library checks for, so that
         # xpr_rasterize_bwd zero-fills them with a single memset
         g2 = e(10 * N)                                     # ... | g_depth (f3) last
+        self._g2, self._zeroed2d = g2, False
         self.g_mean2d, self.g_conic = g2[:2 * N].view(N, 2), g2[2 * N:5 * N].view(N, 3)
         self.g_opac, self.g_rgb, self.g_depth = g2[5 * N:6 * N], g2[6 * N:9 * N].view(N, 3), g2[9 * N:]
         if self.features:
@@ -203,9 +204,15 @@ class SplatPipeline:
             return
         if not hasattr(self, "_side"):
             self._side = torch.cuda.Stream(device=self.device)
-            self._ev_fork, self._ev_join = torch.cuda.Event(), torch.cuda.Event()
+            self._ev_fork, self._ev_join, self._ev_join2d = torch.cuda.Event(), torch.cuda.Event(), torch.cuda.Event()
         self._ev_fork.record(torch.cuda.current_stream())      # after every earlier reader / writer of the gradient arrays
         self._side.wait_event(self._ev_fork)
+        if where == 4 and not self.ray_eval:
+            # the 2D gradients of the compositing backward (40 B per Gaussian) first: the backward waits for THIS event only
+            with torch.cuda.stream(self._side):
+                self._g2.zero_()
+            self._ev_join2d.record(self._side)
+            self._zeroed2d = True
         xb.xpr_project_bwd_fill(self.cfg, self.g_means, self.g_scales, self.g_quats, self.g_opacities, self.g_sh,
                                 stream=self._side)
         self._ev_join.record(self._side)
@@ -226,7 +233,7 @@ class SplatPipeline:
             xb.xpr_rasterize_feat_bwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges,
                                       self.final_T, self.n_contrib, dL_dimage,
                                       z(dL_ddepth), z(dL_dalpha), self.g_mean2d, self.g_conic, self.g_opac,
-                                      self.g_rgb, self.g_depth, zero_init=True)
+                                      self.g_rgb, self.g_depth, zero_init=self._zero_init_2d())
             self._feat_bwd = True
             return
         if self.ray_eval:
@@ -236,7 +243,16 @@ class SplatPipeline:
             return
         xb.xpr_rasterize_bwd(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.final_T,
                              self.n_contrib, dL_dimage, self.g_mean2d, self.g_conic, self.g_opac, self.g_rgb,
-                             zero_init=True)
+                             zero_init=self._zero_init_2d())
+
+    def _zero_init_2d(self) -> bool:
+        """False when the 2D gradient arrays were already cleared on the side stream (overlap_fill 4): the backward then
+        waits for that memset instead of issuing its own."""
+        if not self._zeroed2d:
+            return True
+        self._zeroed2d = False
+        torch.cuda.current_stream().wait_event(self._ev_join2d)
+        return False
 
     def can_fuse_loss(self) -> bool:
         return self.fuse_loss and not self.ray_eval and not self.features
@@ -247,7 +263,7 @@ class SplatPipeline:
         self._fork_fill(1)
         xb.xpr_rasterize_bwd_loss(self.cam, self.cfg, self.shade_rec, self.vals_sorted, self.tile_ranges, self.image,
                                   self.final_T, self.n_contrib, loss, target, self.g_mean2d, self.g_conic, self.g_opac,
-                                  self.g_rgb, zero_init=True)
+                                  self.g_rgb, zero_init=self._zero_init_2d())
 
     # ---- N-channel features (f3): replay of the finished colour pass ---------------------------
     def rasterize_featn_fwd(self, feat, feat_img=None):

@@ -319,8 +319,16 @@ def test_overlapped_zero_fill_gives_the_same_gradients(mode):
     torch.cuda.synchronize()
     for k in names:
         getattr(pipe, k).fill_(float("nan"))                # the fill must really happen
+    pipe._g2.fill_(float("nan"))                            # ... and so must that of the 2D gradients (mode 4: side stream too)
     pipe.step_async(*params, target, sc.loss)               # fill on the side stream, xpr_project_bwd_filled
     torch.cuda.synchronize()
+    ref = pipeline.SplatPipeline(sc.N, sc.cameras[0], dict(cfg, overlap_fill=0))
+    ref.forward(*params)
+    ref.step_async(*params, target, sc.loss)
+    torch.cuda.synchronize()
+    for k in ("g_mean2d", "g_conic", "g_opac", "g_rgb"):    # same terms, another order of the fp32 atomics
+        x, y = getattr(pipe, k).cpu().numpy(), getattr(ref, k).cpu().numpy()
+        assert np.isfinite(x).all() and np.allclose(x, y, rtol=1e-2, atol=1e-3 * np.abs(y).max()), k
     a = {k: getattr(pipe, k).cpu().numpy().copy() for k in names}
     for k in names:
         getattr(pipe, k).fill_(float("nan"))
