@@ -66,7 +66,7 @@ constexpr int FWD_PPT2_MIN_TILES = XPR_FWD_PPT2_MIN_TILES;
 #define XPR_FWD_MINB 1
 #endif
 template <bool STATS, int PPT, bool BF, bool FEAT>
-__global__ void __launch_bounds__(BLOCK / PPT, (PPT == 2 && BF) ? XPR_FWD_MINB : 1)
+__global__ void __launch_bounds__(BLOCK / PPT, (PPT == 2 && BF) ? XPR_FWD_MINB : 0)
 rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint32_t* __restrict__ vals,
                      const uint2* __restrict__ ranges, float* __restrict__ image, float* __restrict__ final_T,
                      uint32_t* __restrict__ n_contrib, unsigned long long* __restrict__ stats,
