@@ -633,22 +633,24 @@ struct RowKeep {
         const float ts = (float)TILE;
         const float x0 = __fadd_rn(__fmul_rn(ts, (float)tx), 0.5f), x1 = __fsub_rn(__fadd_rn(__fmul_rn(ts, (float)tx), ts), 0.5f);
         const bool in_x = (mx >= x0) && (mx <= x1);
-        if (in_x && in_y) return true;
-        bool dropped = true;                      // dropped by every facing edge
-        if (!in_x) {
+        // both facing edges are evaluated unconditionally and selected afterwards (the same operations on the same operands
+        // as the branching form; an edge that does not face the mean is ignored): the lanes of a warp stay together
+        bool drop_x, drop_y;
+        {
             const float dx = __fsub_rn((mx < x0) ? x0 : x1, mx);
             const float bx = __fmul_rn(B, dx);
             float dy = __fdiv_rn(-bx, C);
             dy = (dy < y_lo) ? y_lo : dy; dy = (y_hi < dy) ? y_hi : dy;
-            dropped = drop(__fmul_rn(__fmul_rn(hA, dx), dx), __fmul_rn(bx, dy), __fmul_rn(__fmul_rn(hC, dy), dy));
+            drop_x = drop(__fmul_rn(__fmul_rn(hA, dx), dx), __fmul_rn(bx, dy), __fmul_rn(__fmul_rn(hC, dy), dy));
         }
-        if (!in_y) {
+        {
             const float lo = __fsub_rn(x0, mx), hi = __fsub_rn(x1, mx);
             float dx = dxE;
             dx = (dx < lo) ? lo : dx; dx = (hi < dx) ? hi : dx;
-            dropped = dropped && drop(__fmul_rn(__fmul_rn(hA, dx), dx), __fmul_rn(__fmul_rn(B, dx), dyE), cE);
+            drop_y = drop(__fmul_rn(__fmul_rn(hA, dx), dx), __fmul_rn(__fmul_rn(B, dx), dyE), cE);
         }
-        return !dropped;
+        // kept inside both ranges; else dropped iff dropped by every facing edge
+        return (in_x && in_y) || !((in_x || drop_x) && (in_y || drop_y));
     }
 };
 
