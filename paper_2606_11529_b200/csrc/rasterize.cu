@@ -10,7 +10,7 @@
 // in flight and the list indices of batch b+3 are being loaded, so a CTA waits for memory only at its start and
 // there is one barrier per batch.  Every thread walks the batch with warp-broadcast LDS.128 reads.
 // Decisions (the power > 0 guard and the alpha gate) are taken on `power`, computed in the fixed fp32 order of
-// rule R3, never on exp().  A thread owns 2 (forward) or 4 (backward) pixels of one tile row and works on them
+// rule R3 (carried negated: `gate`), never on exp().  A thread owns 2 (forward) or 8 (backward) pixels of one tile row and works on them
 // as PAIRS with the packed fp32 instructions of sm_100 (fma.rn.f32x2 -> FFMA2 ...: two individually rounded
 // results per issue slot -- the kernels are issue-bound), packed.cuh.
 #include "common.cuh"
@@ -269,8 +269,8 @@ rasterize_fwd_kernel(RasterParams P, const float4* __restrict__ rec, const uint3
 }
 
 // Backward compositing (a9).  One CTA per 16x16 tile; a thread owns PPT consecutive pixels of one row
-// (4 -> 64 threads, the throughput shape; 2 -> 128 threads for images with few tiles), handled as PPT/2 packed
-// pairs, so that a Gaussian's record is read from shared memory once per PPT pixel-pairs, the row terms of
+// (8 -> 32 threads, ONE WARP PER TILE, the throughput shape; 2 -> 128 threads for images with few tiles), handled as PPT/2
+// packed pairs, so that a Gaussian's record is read from shared memory once per PPT pixel-pairs, the row terms of
 // `power` are shared, and the per-Gaussian reduction runs once per 32 * PPT pixel-pairs: each lane first sums
 // its own pixels in registers, then one transposed butterfly (14 shuffles for the 9 gradients) leaves the totals
 // spread over lanes, which issue two RED instructions (8 lanes + 1 lane).
