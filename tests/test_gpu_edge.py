@@ -420,3 +420,26 @@ def test_fused_loss_backward_matches_separate_loss_grad(config, n, wh):
         assert np.isfinite(got).all() and np.abs(ref[k]).max() > 0
         tol = 1e-3 * np.abs(ref[k]) + 2e-6 + 4e-6 * mass[ko].reshape(got.shape)
         assert (np.abs(got - ref[k]) <= tol).all(), (k, int((np.abs(got - ref[k]) > tol).sum()))
+
+
+@pytest.mark.gpu
+def test_shade_record_equals_the_projection_record():
+    """xpr_shade_record (for a caller with its own projection) builds, from the separate projection outputs, the 48-byte record
+    xpr_project writes itself: bit for bit on every visible Gaussian (layout of xpr.h: the pre-scaled conic, +lnv, log2 o)."""
+    import numpy as np
+    import torch
+    from paper_2606_11529_b200 import binding as xb, pipeline, scenes
+    for config in (3, 4):
+        sc = scenes.make_scene(config, n_override=30000, image_override=(320, 180))
+        pipe = pipeline.SplatPipeline(sc.N, sc.cameras[0], scenes.default_render_config(sc))
+        pipe.project(*pipeline.scene_to_device(sc))
+        rec = torch.full_like(pipe.shade_rec, float("nan"))
+        xb.xpr_shade_record(pipe.mean2d, pipe.conic_opac, pipe.rgb, pipe.lnv, pipe.depth, pipe.tile_count, rec)
+        torch.cuda.synchronize()
+        vis = (pipe.tile_count > 0).cpu().numpy()
+        a = pipe.shade_rec.cpu().numpy().reshape(sc.N, 12).view(np.uint32)
+        b = rec.cpu().numpy().reshape(sc.N, 12).view(np.uint32)
+        assert vis.sum() > 1000 and np.array_equal(a[vis], b[vis])
+        assert np.isnan(rec.cpu().numpy().reshape(sc.N, 12)[~vis]).all()          # culled Gaussians are skipped
+        lnv = pipe.lnv.cpu().numpy()[vis]
+        assert (lnv > 0).all() and np.array_equal(a[vis][:, 5], lnv.view(np.uint32))   # the gate's limit: +lnv, positive
