@@ -443,3 +443,81 @@ def test_shade_record_equals_the_projection_record():
         assert np.isnan(rec.cpu().numpy().reshape(sc.N, 12)[~vis]).all()          # culled Gaussians are skipped
         lnv = pipe.lnv.cpu().numpy()[vis]
         assert (lnv > 0).all() and np.array_equal(a[vis][:, 5], lnv.view(np.uint32))   # the gate's limit: +lnv, positive
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("wh,cull", [((48, 40), 0), ((1024, 1024), 1), ((1024, 1024), 0)])
+def test_hand_built_records_on_pixel_centres(wh, cull):
+    """The compositing calls on hand-built projection outputs (no xpr_project): means EXACTLY on pixel centres (power is a
+    signed zero at that pixel, for either sign of B, and must pass both gates: R3's one-compare form on -power), opacities a
+    hair above alpha_thresh (lnv ~ 1e-6: only the centre pixel contributes), a saturating stack (exit), the latency shapes
+    (3 x 3 tiles) and the throughput shapes (4096 tiles, most of them empty), forward and backward against the oracle."""
+    import types
+    import numpy as np
+    import torch
+    import parity_util as pu
+    import xpr_oracle as xo
+    from paper_2606_11529_b200 import binding as xb
+    W, H = wh
+    TW, TH = (W + 15) // 16, (H + 15) // 16
+    rng = np.random.default_rng(11)
+    at = 1.0 / 255.0
+    cen = [(8.5, 8.5), (24.5, 8.5), (40.5 if W > 40 else 8.5, 24.5), (W - 7.5, H - 3.5), (16.5, 15.5)]
+    m, con, op, col = [], [], [], []
+    for cx, cy in cen:
+        for sB in (+1.0, -1.0, 0.0):
+            A_, C_ = rng.uniform(0.01, 0.05, 2)
+            m.append((cx, cy)); con.append((A_, sB * 0.6 * np.sqrt(A_ * C_), C_)); op.append(rng.uniform(0.2, 0.7)); col.append(rng.uniform(0, 1, 3))
+        m.append((cx, cy)); con.append((0.02, 0.004, 0.03)); op.append(at * (1.0 + 1e-6)); col.append((1.0, 1.0, 1.0))   # lnv ~ 1e-6
+    for _ in range(40):                                                        # a saturating stack on one tile + random ones
+        m.append((rng.uniform(0, min(W, 48)), rng.uniform(0, min(H, 40)))); con.append((0.004, 0.001, 0.005)); op.append(0.9); col.append(rng.uniform(0, 1, 3))
+    N = len(m)
+    mean2d = np.asarray(m, np.float32); conic = np.asarray(con, np.float32); opac = np.asarray(op, np.float32)
+    rgb = np.asarray(col, np.float32)
+    lnv = np.log(opac.astype(np.float64) / at).astype(np.float32)
+    assert (lnv > 0).all()
+    # lists: every Gaussian on every tile its 3.5 sigma box touches, in index order
+    sx, sy = 3.5 / np.sqrt(conic[:, 0] * (1 - 0.36)), 3.5 / np.sqrt(conic[:, 2] * (1 - 0.36))
+    vals, ranges = [], np.zeros((TW * TH, 2), np.uint32)
+    for t in range(TW * TH):
+        tx, ty = t % TW, t // TW
+        hit = (mean2d[:, 0] + sx > 16 * tx) & (mean2d[:, 0] - sx < 16 * tx + 16) & (mean2d[:, 1] + sy > 16 * ty) & (mean2d[:, 1] - sy < 16 * ty + 16)
+        idx = np.flatnonzero(hit)
+        ranges[t] = (len(vals), len(vals) + len(idx)); vals.extend(idx.tolist())
+    vals = np.asarray(vals, np.uint32)
+    camo = types.SimpleNamespace(model=0, width=W, height=H, fx=100.0, fy=100.0, cx=W / 2, cy=H / 2, k=(0, 0, 0, 0),
+                                 w2c=np.eye(4)[:3])
+    cfgd = dict(projection=0, sh_degree=0, tile=16, antialias=0, alpha_thresh=at, alpha_max=0.99, t_min=1e-4, z_near=0.2,
+                lowpass=0.3, ut_alpha=1.0, ut_beta=2.0, ut_kappa=0.0, bg=(0.1, 0.2, 0.3), tile_cull=cull)
+    proj = dict(mean2d=mean2d, conic=conic, opac_eff=opac, rgb=rgb, lnv=lnv, tile_count=np.ones(N, np.uint32))
+    binned = dict(vals=vals, ranges=ranges)
+    ocam, ocfg = xo.make_camera(camo), xo.make_config(cfgd)
+    of = xo.rasterize_fwd(proj, binned, ocam, ocfg, np.float32)
+    d = "cuda:0"
+    t = lambda a, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(a)).to(d, dt)
+    co4 = t(np.concatenate([conic, opac[:, None]], 1))
+    rec = torch.empty(N, 12, device=d)
+    xb.xpr_shade_record(t(mean2d), co4, t(rgb), t(lnv), t(np.ones(N, np.float32)), t(np.ones(N), torch.int32), rec)
+    cam, cfg = xb.make_camera(camo), xb.make_config(cfgd)
+    image, fT, nc = torch.empty(H, W, 3, device=d), torch.empty(H, W, device=d), torch.empty(H, W, dtype=torch.int32, device=d)
+    v_d, r_d = t(vals.astype(np.int32), torch.int32), t(ranges.astype(np.int32), torch.int32)
+    xb.xpr_rasterize_fwd(cam, cfg, rec, v_d, r_d, image, fT, nc)
+    ok = (of["fragile"] & pu.FRAG_EXIT) == 0
+    np.testing.assert_array_equal(nc.cpu().numpy().view(np.uint32)[ok], of["n_contrib"][ok])
+    assert np.abs(image.cpu().numpy() - of["image"])[ok].max() <= 1e-4
+    for cx, cy in cen:                                  # the centre pixels: every Gaussian centred there was blended
+        px, py = int(cx), int(cy)
+        mine = [i for i in range(N) if m[i] == (cx, cy)]
+        lst = vals[ranges[(py // 16) * TW + px // 16][0]:ranges[(py // 16) * TW + px // 16][1]]
+        assert of["n_contrib"][py, px] >= 1 + max(int(np.flatnonzero(lst == i)[0]) for i in mine[:3])
+    assert (of["fragile"] & pu.FRAG_EXIT).sum() < 10 and (of["final_T"] < 0.01).any()
+    dL = np.where(ok[..., None], rng.normal(0, 1, (H, W, 3)), 0.0).astype(np.float32)
+    og = xo.rasterize_bwd(proj, binned, of, dL, ocam, ocfg, np.float32)
+    mass = xo.rasterize_bwd(proj, binned, of, dL, ocam, ocfg, np.float32, mass=True)
+    g = [torch.empty(N, k, device=d) for k in (2, 3, 1, 3)]
+    nc_o = t(of["n_contrib"].astype(np.int32), torch.int32)        # both sides replay the oracle's n_contrib and T
+    xb.xpr_rasterize_bwd(cam, cfg, rec, v_d, r_d, t(of["final_T"]), nc_o, t(dL), g[0], g[1], g[2].view(-1), g[3])
+    for got, key in zip(g, ("g_mean2d", "g_conic", "g_opac_eff", "g_rgb")):
+        bad, err = pu.grad_violations(got.cpu().numpy(), og[key], mass[key])
+        assert bad.sum() == 0, (key, int(bad.sum()), float(err.max()))
+    assert np.abs(og["g_opac_eff"]).max() > 0
