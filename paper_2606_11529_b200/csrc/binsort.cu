@@ -1048,6 +1048,19 @@ tile_scan_kernel(uint32_t T, uint32_t ST, unsigned long long pair_capacity, cons
 #ifndef XPR_FINAL_LB
 #define XPR_FINAL_LB 4
 #endif
+// Transpose of a 32 x 32 bit matrix held one row per lane: on return lane j holds column j (bit i = row i's bit j).
+// Five exchange steps; in step s the lanes without bit s keep their columns without bit s and take those of their partner
+// into the upper positions, the lanes with bit s do the opposite.
+__device__ __forceinline__ uint32_t warp_transpose32(uint32_t x, int lane) {
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        const uint32_t m = (s == 16) ? 0x0000ffffu : (s == 8) ? 0x00ff00ffu : (s == 4) ? 0x0f0f0f0fu : (s == 2) ? 0x33333333u : 0x55555555u;
+        const uint32_t t = __shfl_xor_sync(0xffffffffu, x, s);
+        x = (lane & s) ? ((x & ~m) | ((t & ~m) >> s)) : ((x & m) | ((t & m) << s));
+    }
+    return x;
+}
+
 __global__ void __launch_bounds__(CHUNK)
 final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ words,
              const uint32_t* __restrict__ seg_start, const uint32_t* __restrict__ chunk_start,
@@ -1067,7 +1080,6 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
     while (true) {
         __syncthreads();                                // previous chunk done with the shared arrays
         if (tid == 0) s_chunk = atomicAdd(&hdr->final_ticket, 1u);
-        for (int i = tid; i < CHUNK_WARPS * ST_BINS; i += CHUNK) (&s_cnt[0][0])[i] = 0u;
         __syncthreads();
         const uint32_t chunk = s_chunk;
         if (chunk >= n_chunks) break;
@@ -1114,17 +1126,14 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
                 if (k < 4) m_lo |= bits << (8 * k); else m_hi |= bits << (8 * (k - 4));
             }
         }
-        // 2. per warp: the column and the count of every bit present
+        // 2. per warp: the column (which lanes cover the bit's tile) and the count of every bit.  The 32 masks of a warp are
+        //    a 32 x 64 bit matrix; its transpose -- lane b ends with columns b and 32 + b -- takes 5 exchange steps per
+        //    32 x 32 half (a ballot per bit present was 64 iterations of ~8 instructions)
         const uint32_t u_lo = __reduce_or_sync(0xffffffffu, m_lo), u_hi = __reduce_or_sync(0xffffffffu, m_hi);
-        for (uint32_t u = u_lo; u; u &= u - 1u) {
-            const int b = __ffs(u) - 1;
-            const uint32_t bal = __ballot_sync(0xffffffffu, (m_lo >> b) & 1u);
-            if (lane == 0) { s_col[warp][b] = bal; s_cnt[warp][b] = (uint32_t)__popc(bal); }
-        }
-        for (uint32_t u = u_hi; u; u &= u - 1u) {
-            const int b = __ffs(u) - 1;
-            const uint32_t bal = __ballot_sync(0xffffffffu, (m_hi >> b) & 1u);
-            if (lane == 0) { s_col[warp][32 + b] = bal; s_cnt[warp][32 + b] = (uint32_t)__popc(bal); }
+        {
+            const uint32_t c_lo = warp_transpose32(m_lo, lane), c_hi = warp_transpose32(m_hi, lane);
+            s_col[warp][lane] = c_lo; s_cnt[warp][lane] = (uint32_t)__popc(c_lo);
+            s_col[warp][32 + lane] = c_hi; s_cnt[warp][32 + lane] = (uint32_t)__popc(c_hi);
         }
         __syncthreads();
         // 3. per bit: prefix over the warps, look-back over the earlier chunks of this segment
