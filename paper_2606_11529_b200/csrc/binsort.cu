@@ -1070,9 +1070,7 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
              uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out) {
     pdl_entry();
     __shared__ uint32_t s_cnt[CHUNK_WARPS][ST_BINS];    // per warp: covering lanes, then exclusive prefix over warps
-    __shared__ uint32_t s_col[CHUNK_WARPS][ST_BINS];    // per warp: the lanes whose Gaussian covers the bit's tile
     __shared__ uint32_t s_base[ST_BINS];                // global position of the chunk's first pair of every bit
-    __shared__ uint32_t s_tile[ST_BINS];                // tile id of every bit
     __shared__ uint32_t s_chunk, s_seg, s_seg_c0;       // ticket; supertile of the chunk; first chunk of that supertile
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t n_chunks = hdr->n_chunks;
@@ -1130,11 +1128,9 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
         //    a 32 x 64 bit matrix; its transpose -- lane b ends with columns b and 32 + b -- takes 5 exchange steps per
         //    32 x 32 half (a ballot per bit present was 64 iterations of ~8 instructions)
         const uint32_t u_lo = __reduce_or_sync(0xffffffffu, m_lo), u_hi = __reduce_or_sync(0xffffffffu, m_hi);
-        {
-            const uint32_t c_lo = warp_transpose32(m_lo, lane), c_hi = warp_transpose32(m_hi, lane);
-            s_col[warp][lane] = c_lo; s_cnt[warp][lane] = (uint32_t)__popc(c_lo);
-            s_col[warp][32 + lane] = c_hi; s_cnt[warp][32 + lane] = (uint32_t)__popc(c_hi);
-        }
+        const uint32_t c_lo = warp_transpose32(m_lo, lane), c_hi = warp_transpose32(m_hi, lane);
+        s_cnt[warp][lane] = (uint32_t)__popc(c_lo);
+        s_cnt[warp][32 + lane] = (uint32_t)__popc(c_hi);
         __syncthreads();
         // 3. per bit: prefix over the warps, look-back over the earlier chunks of this segment
         if (tid < ST_BINS) {
@@ -1172,32 +1168,39 @@ final_kernel(int TW, int TH, int STW, uint32_t ST, const uint64_t* __restrict__ 
             }
             const int tx = tx0 + (tid & (ST_EDGE - 1)), ty = ty0 + (tid >> ST_SHIFT);
             const bool inside = tx < TW && ty < TH;
-            s_tile[tid] = (uint32_t)(ty * TW + tx);
             s_base[tid] = (inside ? ranges[ty * TW + tx].x : 0u) + excl_prev;
         }
         __syncthreads();
-        // 4. scatter: the warp walks the bits present in it once more (warp-uniform loop); for a fixed bit the covering
-        //    lanes (the column saved in step 2) write consecutive positions: tile start + pairs of earlier chunks + pairs
-        //    of earlier warps + covering lanes before me
+        // 4. scatter: the warp walks the 64 bits once more (unrolled; a bit absent from the whole warp is skipped); for a
+        //    fixed bit the covering lanes (the column of step 2, still in lane b's register) write consecutive positions:
+        //    tile start + pairs of earlier chunks + pairs of earlier warps + covering lanes before me.  Column, first
+        //    position and tile id of bit b are broadcast from lane b by shuffles (the loop over __ffs with three
+        //    shared-memory reads per bit took 30 instructions per bit: 76 % of the kernel's instructions)
         {
-            s_cnt[warp][lane] += s_base[lane];          // per warp: first position of the warp's pairs of every bit
-            s_cnt[warp][lane + 32] += s_base[lane + 32];
-            __syncwarp();
+            const uint32_t p_lo = s_cnt[warp][lane] + s_base[lane], p_hi = s_cnt[warp][lane + 32] + s_base[lane + 32];
+            const uint32_t t_lo = (uint32_t)((ty0 + (lane >> ST_SHIFT)) * TW + tx0 + (lane & (ST_EDGE - 1)));
+            const uint32_t t_hi = t_lo + (uint32_t)(4 * TW);
             const uint32_t lt = (1u << lane) - 1u;
             const uint64_t dkey = (uint64_t)dbits;
-            for (uint32_t u = u_lo; u; u &= u - 1u) {
-                const int b = __ffs(u) - 1;
+#pragma unroll
+            for (int b = 0; b < 32; ++b) {
+                if (!((u_lo >> b) & 1u)) continue;                       // warp-uniform
+                const uint32_t col = __shfl_sync(0xffffffffu, c_lo, b), p0 = __shfl_sync(0xffffffffu, p_lo, b);
+                const uint32_t tl = __shfl_sync(0xffffffffu, t_lo, b);
                 if ((m_lo >> b) & 1u) {
-                    const uint32_t pos = s_cnt[warp][b] + (uint32_t)__popc(s_col[warp][b] & lt);
-                    keys_out[pos] = ((uint64_t)s_tile[b] << 32) | dkey;
+                    const uint32_t pos = p0 + (uint32_t)__popc(col & lt);
+                    keys_out[pos] = ((uint64_t)tl << 32) | dkey;
                     vals_out[pos] = g;
                 }
             }
-            for (uint32_t u = u_hi; u; u &= u - 1u) {
-                const int b = __ffs(u) - 1;
+#pragma unroll
+            for (int b = 0; b < 32; ++b) {
+                if (!((u_hi >> b) & 1u)) continue;
+                const uint32_t col = __shfl_sync(0xffffffffu, c_hi, b), p0 = __shfl_sync(0xffffffffu, p_hi, b);
+                const uint32_t tl = __shfl_sync(0xffffffffu, t_hi, b);
                 if ((m_hi >> b) & 1u) {
-                    const uint32_t pos = s_cnt[warp][32 + b] + (uint32_t)__popc(s_col[warp][32 + b] & lt);
-                    keys_out[pos] = ((uint64_t)s_tile[32 + b] << 32) | dkey;
+                    const uint32_t pos = p0 + (uint32_t)__popc(col & lt);
+                    keys_out[pos] = ((uint64_t)tl << 32) | dkey;
                     vals_out[pos] = g;
                 }
             }
